@@ -1,0 +1,264 @@
+/*
+ * lacosmic_oracle.c -- CPU ORACLE for the L.A.Cosmic iteration.  TEST INFRASTRUCTURE ONLY.
+ *
+ * This file is the plain, slow, obviously-correct definition that the CUDA path is
+ * checked against.  It is NOT part of the product: only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may build, load or call it.
+ * It shares no code, header, table or helper with paper_2602_17938_b200/csrc/.
+ *
+ * What it follows
+ *   step list : PAPER.md:53-62 (section Methods/Algorithm, items 1-7)
+ *   formulas  : BASELINE.json north_star (1)-(7)
+ *   readings  : SURVEY.md section 8(c), O0-O7 and R1-R20 (restated in DESIGN.md section 3)
+ *
+ * Precision: north_star fixes fp32 ("4000x6500 fp32 L.A.Cosmic", "fp32 L+, N, S and S'"),
+ * so every arithmetic step is ONE fp32 round-to-nearest operation, in the order written
+ * (compile with -ffp-contract=off, never -ffast-math).  Every median is a full sort of the
+ * gathered window (insertion sort) followed by picking the middle element.  No blocking,
+ * fusion, or reordering: each step materialises its whole plane before the next starts.
+ *
+ * Pins (tests/test_oracle_pins.py, -m "not gpu"): closed forms for constant and
+ * single-spike frames, scipy.ndimage median_filter / binary_dilation equivalence, brute
+ * force on tiny tiles, hand-computed replacement cases (tests/golden/), 180-degree rotation
+ * and flip invariance, fixed-point behaviour of the iteration.  No function here is
+ * "parity unpinned".
+ *
+ * Notation: X<y,x> = X[clamp(y,0,h-1)][clamp(x,0,w-1)]  (edge-replicate read of a stored
+ * plane, R3).  OpenMP only splits independent output rows between threads.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_OK 0
+#define ORC_ERR_ARG (-1)
+#define ORC_ERR_MEM (-2)
+
+/* R1: Laplacian kernel [0 -1 0; -1 4 -1; 0 -1 0], no 1/4 normalisation. */
+
+typedef struct {
+    int iter;          /* which iteration (0-based) to dump */
+    float *Lp, *N, *S, *Sp, *m3, *F;       /* fp32 [h][w], nullable */
+    uint8_t *G1, *G2, *M1, *M2, *M3, *C;   /* 0/1 [h][w], nullable; C = cumulative mask AFTER the iteration */
+    float *work_in;                        /* the iteration's input image, nullable */
+} orc_debug;
+
+static inline int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+static inline float rd(const float *X, int h, int w, int y, int x) {
+    return X[(size_t)clampi(y, 0, h - 1) * (size_t)w + (size_t)clampi(x, 0, w - 1)];
+}
+
+static void sort_ascending(float *v, int n) { /* insertion sort */
+    for (int i = 1; i < n; ++i) {
+        float t = v[i];
+        int j = i - 1;
+        while (j >= 0 && v[j] > t) { v[j + 1] = v[j]; --j; }
+        v[j + 1] = t;
+    }
+}
+
+void orc_set_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+int orc_get_max_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* O1 -- north_star (1).  2x block-replicate, 3x3 Laplacian, clip, 2x2 block-average.
+ * Sub-pixel (2y+i, 2x+j) of the replicated grid has value c; two of its four 4-neighbours lie in
+ * its own block (value c), one is the vertical neighbour V in {U,D} and one the horizontal
+ * neighbour H in {Lf,R}:  4c - c - c - V - H = 2c - (V + H).  Clamping on the 2h x 2w grid and on
+ * the h x w grid select the same neighbours. */
+void orc_lplus(const float *work, float *Lp, int h, int w) {
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < h; ++y)
+        for (int x = 0; x < w; ++x) {
+            float c = work[(size_t)y * w + x];
+            float U = rd(work, h, w, y - 1, x), D = rd(work, h, w, y + 1, x);
+            float Lf = rd(work, h, w, y, x - 1), R = rd(work, h, w, y, x + 1);
+            float two = 2.0f * c;
+            float a = two - (U + Lf);
+            float b = two - (U + R);
+            float g = two - (D + Lf);
+            float d = two - (D + R);
+            a = a > 0.0f ? a : 0.0f;
+            b = b > 0.0f ? b : 0.0f;
+            g = g > 0.0f ? g : 0.0f;
+            d = d > 0.0f ? d : 0.0f;
+            Lp[(size_t)y * w + x] = ((a + b) + (g + d)) * 0.25f;
+        }
+}
+
+/* True (non-separable) k x k median; edge-replicate (R3).  k in {3,5,7}. */
+int orc_medfilt(const float *X, float *out, int h, int w, int k) {
+    if (!(k == 3 || k == 5 || k == 7) || h < 1 || w < 1) return ORC_ERR_ARG;
+    int r = (k - 1) / 2, n = k * k;
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < h; ++y) {
+        float v[49];
+        for (int x = 0; x < w; ++x) {
+            int m = 0;
+            for (int dy = -r; dy <= r; ++dy)
+                for (int dx = -r; dx <= r; ++dx) v[m++] = rd(X, h, w, y + dy, x + dx);
+            sort_ascending(v, n);
+            out[(size_t)y * w + x] = v[(n - 1) / 2];
+        }
+    }
+    return ORC_OK;
+}
+
+/* 3x3 binary dilation, 8-connected, out-of-frame = 0 (O6, R10). */
+void orc_dilate3(const uint8_t *in, uint8_t *out, int h, int w) {
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < h; ++y)
+        for (int x = 0; x < w; ++x) {
+            uint8_t o = 0;
+            for (int dy = -1; dy <= 1; ++dy)
+                for (int dx = -1; dx <= 1; ++dx) {
+                    int yy = y + dy, xx = x + dx;
+                    if (yy >= 0 && yy < h && xx >= 0 && xx < w && in[(size_t)yy * w + xx]) o = 1;
+                }
+            out[(size_t)y * w + x] = o;
+        }
+}
+
+/* O7 -- north_star (7), R13-R16.  out = img where mask == 0; where mask != 0 the
+ * median of the 5x5 edge-replicated taps of img whose (clamped) pixel is unmasked; duplicated
+ * taps count with multiplicity; even count -> mean of the two middle values; no donor -> plain
+ * median of all 25 taps. */
+void orc_masked_median(const float *img, const uint8_t *mask, float *out, int h, int w) {
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < h; ++y) {
+        float v[25];
+        for (int x = 0; x < w; ++x) {
+            size_t p = (size_t)y * w + x;
+            if (!mask[p]) { out[p] = img[p]; continue; }
+            int k = 0;
+            for (int dy = -2; dy <= 2; ++dy)
+                for (int dx = -2; dx <= 2; ++dx) {
+                    size_t q = (size_t)clampi(y + dy, 0, h - 1) * w + (size_t)clampi(x + dx, 0, w - 1);
+                    if (!mask[q]) v[k++] = img[q];
+                }
+            if (k == 0)
+                for (int dy = -2; dy <= 2; ++dy)
+                    for (int dx = -2; dx <= 2; ++dx) v[k++] = rd(img, h, w, y + dy, x + dx);
+            sort_ascending(v, k);
+            out[p] = (k & 1) ? v[k / 2] : (v[k / 2 - 1] + v[k / 2]) * 0.5f;
+        }
+    }
+}
+
+#define COPY_IF(dst, src, bytes) do { if (dst) memcpy((dst), (src), (bytes)); } while (0)
+
+/* The whole path: O0-O7 of SURVEY.md 8(c).  Returns 0, or <0 on bad arguments / out of memory.
+ * iter_counts (nullable) receives new_t for t = 0..niter-1; dbg (nullable) receives the planes
+ * of iteration dbg->iter.  All niter iterations are always executed (R17: stopping at new_t = 0
+ * would give the identical result; the oracle does not take the shortcut). */
+int orc_run(const float *img, int h, int w, float gain, float readnoise, float sigclip,
+            float sigfrac, float objlim, int niter, float satlevel, uint8_t *mask_out,
+            float *clean_out, int32_t *iter_counts, orc_debug *dbg) {
+    if (!img || !mask_out || !clean_out || h < 1 || w < 1 || niter < 0) return ORC_ERR_ARG;
+    if (!(gain > 0.0f) || !(readnoise >= 0.0f) || !(sigclip > 0.0f) || !(sigfrac > 0.0f) ||
+        !(objlim >= 0.0f))
+        return ORC_ERR_ARG;
+    size_t P = (size_t)h * (size_t)w;
+    float *work = clean_out;
+    float *Lp = malloc(P * 4), *m5 = malloc(P * 4), *N = malloc(P * 4), *S = malloc(P * 4);
+    float *mS = malloc(P * 4), *Sp = malloc(P * 4), *m3 = malloc(P * 4), *m7 = malloc(P * 4);
+    float *F = malloc(P * 4);
+    uint8_t *G1 = malloc(P), *G2 = malloc(P), *M1 = malloc(P), *D = malloc(P), *M2 = malloc(P);
+    uint8_t *M3 = malloc(P), *C = mask_out;
+    int rc = ORC_OK;
+    if (!Lp || !m5 || !N || !S || !mS || !Sp || !m3 || !m7 || !F || !G1 || !G2 || !M1 || !D ||
+        !M2 || !M3) {
+        rc = ORC_ERR_MEM;
+        goto done;
+    }
+    /* O0 */
+    memset(C, 0, P);
+    memcpy(work, img, P * 4);
+    const float siglow = sigfrac * sigclip;   /* R9: one fp32 multiply */
+    const float rn2 = readnoise * readnoise;
+
+    for (int t = 0; t < niter; ++t) {
+        if (dbg && dbg->iter == t) COPY_IF(dbg->work_in, work, P * 4);
+        /* O1 */
+        orc_lplus(work, Lp, h, w);
+        /* O2 -- north_star (2): N = sqrt(gain*med5(img) + rn^2)/gain, med5 floored at 1e-4 (R5) */
+        orc_medfilt(work, m5, h, w, 5);
+#pragma omp parallel for schedule(static)
+        for (size_t p = 0; p < P; ++p) {
+            float m = m5[p] > 1e-4f ? m5[p] : 1e-4f;
+            float gm = gain * m;
+            float var = gm + rn2;
+            N[p] = sqrtf(var) / gain;
+        }
+        /* O3 -- north_star (3): S = L+/(2N); S' = S - med5(S) */
+#pragma omp parallel for schedule(static)
+        for (size_t p = 0; p < P; ++p) {
+            float twoN = 2.0f * N[p];
+            S[p] = Lp[p] / twoN;
+        }
+        orc_medfilt(S, mS, h, w, 5);
+#pragma omp parallel for schedule(static)
+        for (size_t p = 0; p < P; ++p) Sp[p] = S[p] - mS[p];
+        /* O4 -- north_star (4): F = med3(img) - med7(med3(img)), floored at 0.01; med7 replicates
+         * the stored m3 plane's edges (R4) */
+        orc_medfilt(work, m3, h, w, 3);
+        orc_medfilt(m3, m7, h, w, 7);
+#pragma omp parallel for schedule(static)
+        for (size_t p = 0; p < P; ++p) {
+            float f = m3[p] - m7[p];
+            F[p] = f > 0.01f ? f : 0.01f;
+        }
+        /* O5 -- north_star (5), R8 (strict >, IEEE division then compare), R12 (satlevel) */
+#pragma omp parallel for schedule(static)
+        for (size_t p = 0; p < P; ++p) {
+            int ok = work[p] < satlevel;
+            G1[p] = (uint8_t)(ok && (Sp[p] > sigclip));
+            G2[p] = (uint8_t)(ok && (Sp[p] > siglow));
+            float ratio = Lp[p] / F[p];
+            M1[p] = (uint8_t)(G1[p] && (ratio > objlim));
+        }
+        /* O6 -- north_star (6), R10, R11 */
+        orc_dilate3(M1, D, h, w);
+#pragma omp parallel for schedule(static)
+        for (size_t p = 0; p < P; ++p) M2[p] = (uint8_t)(D[p] && G1[p]);
+        orc_dilate3(M2, D, h, w);
+        int64_t newc = 0;
+#pragma omp parallel for schedule(static) reduction(+ : newc)
+        for (size_t p = 0; p < P; ++p) {
+            M3[p] = (uint8_t)(D[p] && G2[p]);
+            if (M3[p] && !C[p]) ++newc;
+            C[p] = (uint8_t)(C[p] || M3[p]);
+        }
+        if (iter_counts) iter_counts[t] = (int32_t)newc;
+        /* O7 -- donors from img_in, cumulative mask (R13) */
+        orc_masked_median(img, C, work, h, w);
+
+        if (dbg && dbg->iter == t) {
+            COPY_IF(dbg->Lp, Lp, P * 4); COPY_IF(dbg->N, N, P * 4); COPY_IF(dbg->S, S, P * 4);
+            COPY_IF(dbg->Sp, Sp, P * 4); COPY_IF(dbg->m3, m3, P * 4); COPY_IF(dbg->F, F, P * 4);
+            COPY_IF(dbg->G1, G1, P); COPY_IF(dbg->G2, G2, P); COPY_IF(dbg->M1, M1, P);
+            COPY_IF(dbg->M2, M2, P); COPY_IF(dbg->M3, M3, P); COPY_IF(dbg->C, C, P);
+        }
+    }
+done:
+    free(Lp); free(m5); free(N); free(S); free(mS); free(Sp); free(m3); free(m7); free(F);
+    free(G1); free(G2); free(M1); free(D); free(M2); free(M3);
+    return rc;
+}
