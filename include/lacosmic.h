@@ -1,0 +1,154 @@
+/*
+ * lacosmic.h -- C ABI of the B200-native L.A.Cosmic hot path (liblacosmic_b200.so).
+ *
+ * The operation is the cosmic-ray detection-and-cleaning iteration that PAPER.md:53-62
+ * (section Methods/Algorithm, items 1-7) lists and BASELINE.json north_star (1)-(7) defines:
+ *   (1) L+  : 2x block-replicate, 3x3 Laplacian, clip negatives, 2x2 block-average
+ *   (2) N   = sqrt(gain*med5(img) + readnoise^2)/gain
+ *   (3) S   = L+/(2N),  S' = S - med5(S)
+ *   (4) F   = max(med3(img) - med7(med3(img)), 0.01)
+ *   (5) candidates: S' > sigclip and L+/F > objlim
+ *   (6) two 3x3 binary dilations gated by S' > sigclip, then S' > sigfrac*sigclip
+ *   (7) every flagged pixel <- median of its unflagged 5x5 neighbours
+ * repeated niter times on the cleaned image (parameters: PAPER.md:66-74).  The exact arithmetic
+ * (operation order, boundary rule, tie rules) is DESIGN.md section 3, readings R1-R20.
+ * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ *
+ * Conventions for EVERY entry point unless stated otherwise
+ *   - Pointers named *_dev / img / mask_out / clean_out / workspace are DEVICE pointers on the
+ *     current CUDA device, owned and allocated by the caller; the library keeps no reference to
+ *     them once the work enqueued on `stream` has completed and never frees caller memory.
+ *   - Images are row-major contiguous [h][w] (h rows, w columns, pitch = w elements).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls only
+ *     ENQUEUE work and return; they never synchronise the host.  Outputs are valid once the
+ *     caller has synchronised `stream`.
+ *   - Return value: LACOSMIC_OK (0) or a negative LACOSMIC_ERR_* code.  Nothing is printed, no
+ *     exception crosses the boundary, the process is never aborted.  On an argument error no
+ *     work is enqueued and no output is touched.
+ *   - Input pixels must be finite.  NaN/Inf input is a caller error with unspecified output (a
+ *     validation pass would cost a full extra read of the frame).
+ */
+#ifndef LACOSMIC_H_
+#define LACOSMIC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LACOSMIC_OK 0
+#define LACOSMIC_ERR_NULL (-1)      /* a required pointer is NULL */
+#define LACOSMIC_ERR_SHAPE (-2)     /* h < 1, w < 1, or h*w >= 2^31 (or n < 0 for a batch) */
+#define LACOSMIC_ERR_PARAM (-3)     /* non-finite parameter; gain <= 0; readnoise < 0; sigclip <= 0;
+                                       sigfrac <= 0 or > 1; objlim < 0; niter < 0 or > LACOSMIC_MAX_NITER;
+                                       satlevel NaN; k not in {3,5,7} */
+#define LACOSMIC_ERR_ALIGN (-4)     /* fp32 image pointer not 16-byte aligned, workspace not 256-byte aligned */
+#define LACOSMIC_ERR_ALIAS (-5)     /* img, mask_out, clean_out (or workspace) overlap */
+#define LACOSMIC_ERR_WORKSPACE (-6) /* workspace_bytes smaller than lacosmic_workspace_bytes(h, w) */
+#define LACOSMIC_ERR_CUDA (-7)      /* a CUDA call failed; see lacosmic_last_cuda_error() */
+
+#define LACOSMIC_MAX_NITER 64
+
+/* Parameters of one frame (PAPER.md:66-74 plus niter/satlevel of the north_star signature).
+ * gain [e-/ADU] > 0 (gain estimation, is not part of this path); readnoise [e-] >= 0;
+ * sigclip > 0: detection limit in sigma; sigfrac in (0,1]: fractional limit for neighbours;
+ * objlim >= 0: contrast limit L+/F; satlevel: pixels >= satlevel are never flagged (+INF disables);
+ * niter in [0, LACOSMIC_MAX_NITER]: number of iterations (0: clean_out = img, mask_out = 0). */
+typedef struct lacosmic_params {
+    float gain, readnoise, sigclip, sigfrac, objlim, satlevel;
+    int32_t niter;
+} lacosmic_params;
+
+/* Optional per-step dump of ONE iteration (used by the parity tests).  Every pointer is a
+ * nullable device pointer to a [h][w] plane: fp32 for Lp (step 1), N (2), S, Sp (3), m3, F (4);
+ * uint8 0/1 for G1 = (S' > sigclip), G2 = (S' > sigfrac*sigclip) (both AND img < satlevel),
+ * M1 (step 5), M2, M3 (step 6) and C (cumulative mask after the iteration). */
+typedef struct lacosmic_debug {
+    int32_t iter;
+    float *Lp, *N, *S, *Sp, *m3, *F;
+    uint8_t *G1, *G2, *M1, *M2, *M3, *C;
+} lacosmic_debug;
+
+/* ---- the whole path ------------------------------------------------------------------------- */
+
+/* North-star signature (BASELINE.json north_star).  Cleans one frame: mask_out[h][w] uint8 is 1
+ * where a pixel was flagged (and replaced) in any iteration, else 0; clean_out[h][w] fp32 is the
+ * cleaned frame (equal to img wherever mask_out is 0).  img (const), mask_out and clean_out must
+ * not overlap; img and clean_out 16-byte aligned.  Scratch comes from the stream-ordered pool
+ * (cudaMallocAsync/cudaFreeAsync on `stream`). */
+int lacosmic_run(const float *img, int h, int w, float gain, float readnoise, float sigclip,
+                 float sigfrac, float objlim, int niter, float satlevel, uint8_t *mask_out,
+                 float *clean_out, void *stream);
+
+/* Scratch size in bytes that lacosmic_run_ws / lacosmic_run_batch / lacosmic_masked_median need for
+ * an h x w frame (0 if the shape is invalid). */
+size_t lacosmic_workspace_bytes(int h, int w);
+
+/* Same as lacosmic_run with caller-supplied scratch (256-byte aligned device memory of at least
+ * lacosmic_workspace_bytes(h,w) bytes, contents undefined before and after).  This is the timed
+ * entry point.  iter_counts: nullable DEVICE array of p->niter int32; element t receives the number
+ * of pixels newly flagged in iteration t (0 for iterations skipped after a fixed point, which
+ * leaves the result unchanged -- DESIGN.md R17).  dbg: nullable HOST struct (read during the call)
+ * of device planes to fill for iteration dbg->iter. */
+int lacosmic_run_ws(const float *img, int h, int w, const lacosmic_params *p, uint8_t *mask_out,
+                    float *clean_out, void *workspace, size_t workspace_bytes, int32_t *iter_counts,
+                    const lacosmic_debug *dbg, void *stream);
+
+/* n independent frames back to back ("batch processing"; BASELINE.json configs[3]).
+ * imgs/masks_out/cleans_out are [n][h][w]; params is a HOST array of n structs (per-frame
+ * parameters, read during the call); workspace as for lacosmic_run_ws (one frame's worth, reused);
+ * iter_counts: nullable device array [n][LACOSMIC_MAX_NITER]. */
+int lacosmic_run_batch(const float *imgs, int n, int h, int w, const lacosmic_params *params,
+                       uint8_t *masks_out, float *cleans_out, void *workspace,
+                       size_t workspace_bytes, int32_t *iter_counts, void *stream);
+
+/* End-to-end variant with HOST buffers: img_host, mask_out_host, clean_out_host are host pointers
+ * (pinned memory makes the copies asynchronous); the call enqueues H2D copy, the whole path and
+ * the D2H copies on `stream`.  dev_workspace: device scratch of at least
+ * lacosmic_host_workspace_bytes(h,w) bytes (frame staging + lacosmic_workspace_bytes), 256-byte
+ * aligned.  Results are valid after the caller synchronises `stream`. */
+size_t lacosmic_host_workspace_bytes(int h, int w);
+int lacosmic_run_host(const float *img_host, int h, int w, const lacosmic_params *p,
+                      uint8_t *mask_out_host, float *clean_out_host, void *dev_workspace,
+                      size_t dev_workspace_bytes, void *stream);
+
+/* ---- single steps (each is the kernel the whole path uses; exported for parity tests) -------- */
+
+/* Step (1): out = L+(in).  in/out fp32 [h][w], distinct. */
+int lacosmic_lplus(const float *in, float *out, int h, int w, void *stream);
+
+/* True (non-separable) k x k median with edge-replicate borders, k in {3,5,7}.
+ * in/out fp32 [h][w], distinct. */
+int lacosmic_medfilt(const float *in, float *out, int h, int w, int k, void *stream);
+
+/* Bit-plane layout used by the mask steps: row pitch lacosmic_bitplane_pitch_words(w) =
+ * ceil(w/32) uint32 words, pixel x of a row in word x/32, bit x%32 (LSB = lowest x); pad bits 0. */
+int lacosmic_bitplane_pitch_words(int w);
+int lacosmic_pack_bits(const uint8_t *mask_u8, uint32_t *bits, int h, int w, void *stream);
+int lacosmic_unpack_bits(const uint32_t *bits, uint8_t *mask_u8, int h, int w, void *stream);
+
+/* Step (6) primitive: 3x3 binary dilation (8-connected, outside the frame = 0) on bit-planes.
+ * bits_in/bits_out distinct, [h][pitch] uint32. */
+int lacosmic_dilate3(const uint32_t *bits_in, uint32_t *bits_out, int h, int w, void *stream);
+
+/* Step (7): out = img where mask_u8 == 0, else the median of the unmasked 5x5 edge-replicated
+ * neighbours (even count: mean of the two middle values; none: plain 5x5 median).  workspace as
+ * for lacosmic_run_ws. */
+int lacosmic_masked_median(const float *img, const uint8_t *mask_u8, float *out, int h, int w,
+                           void *workspace, size_t workspace_bytes, void *stream);
+
+/* ---- diagnostics ---------------------------------------------------------------------------- */
+const char *lacosmic_strerror(int code);
+/* cudaError_t (as int) of the last failing CUDA call made by this library on the calling thread. */
+int lacosmic_last_cuda_error(void);
+/* Number of kernel launches the last lacosmic_run* call on this thread enqueued (bench.py reports
+ * it as gpu_launches). */
+int lacosmic_last_launch_count(void);
+const char *lacosmic_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LACOSMIC_H_ */

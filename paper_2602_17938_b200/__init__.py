@@ -1,0 +1,31 @@
+"""B200-native L.A.Cosmic hot path (arxiv/paper_2602_17938, dfcosmic): thin Python binding.
+
+The product is liblacosmic_b200.so (hand-written sm_100a CUDA kernels behind the C ABI declared in
+include/lacosmic.h).  This package only marshals arguments; torch is used for device memory and
+streams.  There is no CPU fallback: every call raises if the CUDA library cannot be loaded.
+"""
+from .binding import (  # noqa: F401
+    LacosmicError,
+    Params,
+    lacosmic_bitplane_pitch_words,
+    lacosmic_dilate3,
+    lacosmic_host_workspace_bytes,
+    lacosmic_last_launch_count,
+    lacosmic_lplus,
+    lacosmic_masked_median,
+    lacosmic_medfilt,
+    lacosmic_pack_bits,
+    lacosmic_run,
+    lacosmic_run_batch,
+    lacosmic_run_host,
+    lacosmic_run_ws,
+    lacosmic_strerror,
+    lacosmic_unpack_bits,
+    lacosmic_version,
+    lacosmic_workspace_bytes,
+    library_path,
+    load_library,
+)
+
+__all__ = [n for n in dir() if n.startswith("lacosmic_")] + ["LacosmicError", "Params",
+                                                              "library_path", "load_library"]

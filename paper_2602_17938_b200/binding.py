@@ -1,0 +1,348 @@
+"""ctypes binding of include/lacosmic.h -- same names, argument marshalling only.
+
+Device buffers are torch CUDA tensors (torch = device memory + streams, nothing else); every step
+of the path runs inside liblacosmic_b200.so.  The library must exist: a missing or unloadable
+library raises LacosmicError (there is deliberately no fallback of any kind).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+MAX_NITER = 64
+_PKG = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_PKG, "liblacosmic_b200.so")
+_lib = None
+
+EXPORTS = (
+    "lacosmic_run", "lacosmic_workspace_bytes", "lacosmic_run_ws", "lacosmic_run_batch",
+    "lacosmic_host_workspace_bytes", "lacosmic_run_host", "lacosmic_lplus", "lacosmic_medfilt",
+    "lacosmic_bitplane_pitch_words", "lacosmic_pack_bits", "lacosmic_unpack_bits",
+    "lacosmic_dilate3", "lacosmic_masked_median", "lacosmic_strerror",
+    "lacosmic_last_cuda_error", "lacosmic_last_launch_count", "lacosmic_version",
+)
+
+
+class LacosmicError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        msg = load_library().lacosmic_strerror(code).decode()
+        if code == -7:
+            msg += " [cudaError %d]" % load_library().lacosmic_last_cuda_error()
+        super().__init__("%s: %s (code %d)" % (where, msg, code))
+
+
+class _CParams(C.Structure):
+    _fields_ = [(n, C.c_float) for n in ("gain", "readnoise", "sigclip", "sigfrac", "objlim",
+                                         "satlevel")] + [("niter", C.c_int32)]
+
+
+class _CDebug(C.Structure):
+    _fields_ = [("iter", C.c_int32)] + [(n, C.c_void_p) for n in (
+        "Lp", "N", "S", "Sp", "m3", "F", "G1", "G2", "M1", "M2", "M3", "C")]
+
+
+DEBUG_F32 = ("Lp", "N", "S", "Sp", "m3", "F")
+DEBUG_U8 = ("G1", "G2", "M1", "M2", "M3", "C")
+
+
+@dataclass
+class Params:
+    """Per-frame parameters (niter/satlevel from the north_star signature)."""
+    gain: float = 1.0
+    readnoise: float = 10.0
+    sigclip: float = 4.5
+    sigfrac: float = 0.3
+    objlim: float = 5.0
+    satlevel: float = 65535.0
+    niter: int = 4
+
+    def _c(self):
+        return _CParams(self.gain, self.readnoise, self.sigclip, self.sigfrac, self.objlim,
+                        self.satlevel, int(self.niter))
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen liblacosmic_b200.so (built in-tree by paper_2602_17938_b200/build.py)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise RuntimeError(
+            "liblacosmic_b200.so is missing at %s -- build it with "
+            "`python -m paper_2602_17938_b200.build` (needs nvcc); there is no CPU fallback"
+            % _LIB_PATH)
+    L = C.CDLL(_LIB_PATH)
+    vp, i, f, sz = C.c_void_p, C.c_int, C.c_float, C.c_size_t
+    sig = {
+        "lacosmic_run": (i, [vp, i, i, f, f, f, f, f, i, f, vp, vp, vp]),
+        "lacosmic_workspace_bytes": (sz, [i, i]),
+        "lacosmic_run_ws": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp,
+                                C.POINTER(_CDebug), vp]),
+        "lacosmic_run_batch": (i, [vp, i, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp, vp]),
+        "lacosmic_host_workspace_bytes": (sz, [i, i]),
+        "lacosmic_run_host": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp]),
+        "lacosmic_lplus": (i, [vp, vp, i, i, vp]),
+        "lacosmic_medfilt": (i, [vp, vp, i, i, i, vp]),
+        "lacosmic_bitplane_pitch_words": (i, [i]),
+        "lacosmic_pack_bits": (i, [vp, vp, i, i, vp]),
+        "lacosmic_unpack_bits": (i, [vp, vp, i, i, vp]),
+        "lacosmic_dilate3": (i, [vp, vp, i, i, vp]),
+        "lacosmic_masked_median": (i, [vp, vp, vp, i, i, vp, sz, vp]),
+        "lacosmic_strerror": (C.c_char_p, [i]),
+        "lacosmic_last_cuda_error": (i, []),
+        "lacosmic_last_launch_count": (i, []),
+        "lacosmic_version": (C.c_char_p, []),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)      # AttributeError if the header and the library disagree
+        fn.restype, fn.argtypes = res, args
+    _lib = L
+    return L
+
+
+# ----------------------------------------------------------------------------- marshalling helpers
+def _torch():
+    import torch
+    return torch
+
+
+def _dev(t, dtype, name, shape=None):
+    torch = _torch()
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError("%s must be a CUDA torch tensor" % name)
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError("%s must be contiguous %s" % (name, dtype))
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError("%s has shape %s, expected %s" % (name, tuple(t.shape), tuple(shape)))
+    return t.data_ptr()
+
+
+def _stream(stream):
+    if stream is None:
+        return _torch().cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+def _check(rc, where):
+    if rc != 0:
+        raise LacosmicError(rc, where)
+
+
+def _params(p=None, **kw):
+    if p is None:
+        p = Params(**kw)
+    elif kw:
+        raise TypeError("give either a Params object or keyword parameters")
+    return p
+
+
+def _workspace(h, w, like, host=False):
+    torch = _torch()
+    n = lacosmic_host_workspace_bytes(h, w) if host else lacosmic_workspace_bytes(h, w)
+    return torch.empty(n, dtype=torch.uint8, device=like)
+
+
+# ----------------------------------------------------------------------------- the whole path
+def lacosmic_workspace_bytes(h, w):
+    return int(load_library().lacosmic_workspace_bytes(int(h), int(w)))
+
+
+def lacosmic_host_workspace_bytes(h, w):
+    return int(load_library().lacosmic_host_workspace_bytes(int(h), int(w)))
+
+
+def lacosmic_run(img, gain=1.0, readnoise=10.0, sigclip=4.5, sigfrac=0.3, objlim=5.0, niter=4,
+                 satlevel=65535.0, mask_out=None, clean_out=None, stream=None):
+    """North-star call: returns (mask_out uint8 [h][w], clean_out fp32 [h][w])."""
+    torch = _torch()
+    L = load_library()
+    if img.dim() != 2:
+        raise ValueError("img must be [h][w]")
+    h, w = img.shape
+    ip = _dev(img, torch.float32, "img")
+    if mask_out is None:
+        mask_out = torch.empty((h, w), dtype=torch.uint8, device=img.device)
+    if clean_out is None:
+        clean_out = torch.empty_like(img)
+    rc = L.lacosmic_run(ip, h, w, gain, readnoise, sigclip, sigfrac, objlim, int(niter), satlevel,
+                        _dev(mask_out, torch.uint8, "mask_out", (h, w)),
+                        _dev(clean_out, torch.float32, "clean_out", (h, w)), _stream(stream))
+    _check(rc, "lacosmic_run")
+    return mask_out, clean_out
+
+
+def lacosmic_run_ws(img, params=None, mask_out=None, clean_out=None, workspace=None,
+                    iter_counts=None, debug_iter=None, debug_planes=None, stream=None, **kw):
+    """Timed entry point.  Returns dict(mask, clean, counts[, debug planes of iteration debug_iter])."""
+    torch = _torch()
+    L = load_library()
+    p = _params(params, **kw)
+    if img.dim() != 2:
+        raise ValueError("img must be [h][w]")
+    h, w = img.shape
+    ip = _dev(img, torch.float32, "img")
+    if mask_out is None:
+        mask_out = torch.empty((h, w), dtype=torch.uint8, device=img.device)
+    if clean_out is None:
+        clean_out = torch.empty_like(img)
+    if workspace is None:
+        workspace = _workspace(h, w, img.device)
+    if iter_counts is None:
+        iter_counts = torch.zeros(max(int(p.niter), 1), dtype=torch.int32, device=img.device)
+    out = dict(mask=mask_out, clean=clean_out, counts=iter_counts)
+    dbg_ref = None
+    if debug_iter is not None:
+        dbg = _CDebug()
+        dbg.iter = int(debug_iter)
+        names = debug_planes if debug_planes is not None else DEBUG_F32 + DEBUG_U8
+        for n in names:
+            dt = torch.float32 if n in DEBUG_F32 else torch.uint8
+            out[n] = torch.zeros((h, w), dtype=dt, device=img.device)
+            setattr(dbg, n, out[n].data_ptr())
+        dbg_ref = C.byref(dbg)
+    cp = p._c()
+    rc = L.lacosmic_run_ws(ip, h, w, C.byref(cp), _dev(mask_out, torch.uint8, "mask_out", (h, w)),
+                           _dev(clean_out, torch.float32, "clean_out", (h, w)),
+                           _dev(workspace, torch.uint8, "workspace"), workspace.numel(),
+                           _dev(iter_counts, torch.int32, "iter_counts"), dbg_ref, _stream(stream))
+    _check(rc, "lacosmic_run_ws")
+    return out
+
+
+def lacosmic_run_batch(imgs, params, masks_out=None, cleans_out=None, workspace=None,
+                       iter_counts=None, stream=None):
+    """imgs [n][h][w]; params: list of n Params.  Returns dict(mask, clean, counts [n][MAX_NITER])."""
+    torch = _torch()
+    L = load_library()
+    if imgs.dim() != 3:
+        raise ValueError("imgs must be [n][h][w]")
+    n, h, w = imgs.shape
+    if len(params) != n:
+        raise ValueError("need one Params per frame")
+    arr = (_CParams * max(n, 1))(*[p._c() for p in params])
+    if masks_out is None:
+        masks_out = torch.empty((n, h, w), dtype=torch.uint8, device=imgs.device)
+    if cleans_out is None:
+        cleans_out = torch.empty_like(imgs)
+    if workspace is None:
+        workspace = _workspace(h, w, imgs.device)
+    if iter_counts is None:
+        iter_counts = torch.zeros((max(n, 1), MAX_NITER), dtype=torch.int32, device=imgs.device)
+    rc = L.lacosmic_run_batch(_dev(imgs, torch.float32, "imgs"), n, h, w, arr,
+                              _dev(masks_out, torch.uint8, "masks_out", (n, h, w)),
+                              _dev(cleans_out, torch.float32, "cleans_out", (n, h, w)),
+                              _dev(workspace, torch.uint8, "workspace"), workspace.numel(),
+                              _dev(iter_counts, torch.int32, "iter_counts"), _stream(stream))
+    _check(rc, "lacosmic_run_batch")
+    return dict(mask=masks_out, clean=cleans_out, counts=iter_counts)
+
+
+def lacosmic_run_host(img_host, params=None, mask_out_host=None, clean_out_host=None,
+                      dev_workspace=None, device="cuda:0", stream=None, **kw):
+    """End-to-end call with HOST (ideally pinned) torch CPU tensors; copies are part of the call."""
+    torch = _torch()
+    L = load_library()
+    p = _params(params, **kw)
+    for t, dt, nm in ((img_host, torch.float32, "img_host"),):
+        if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != dt or not t.is_contiguous():
+            raise TypeError("%s must be a contiguous CPU %s tensor" % (nm, dt))
+    h, w = img_host.shape
+    if mask_out_host is None:
+        mask_out_host = torch.empty((h, w), dtype=torch.uint8).pin_memory()
+    if clean_out_host is None:
+        clean_out_host = torch.empty((h, w), dtype=torch.float32).pin_memory()
+    if dev_workspace is None:
+        dev_workspace = _workspace(h, w, device, host=True)
+    cp = p._c()
+    rc = L.lacosmic_run_host(img_host.data_ptr(), h, w, C.byref(cp), mask_out_host.data_ptr(),
+                             clean_out_host.data_ptr(), _dev(dev_workspace, torch.uint8, "dev_workspace"),
+                             dev_workspace.numel(), _stream(stream))
+    _check(rc, "lacosmic_run_host")
+    return dict(mask=mask_out_host, clean=clean_out_host)
+
+
+# ----------------------------------------------------------------------------- single steps
+def lacosmic_lplus(img, out=None, stream=None):
+    torch = _torch()
+    h, w = img.shape
+    if out is None:
+        out = torch.empty_like(img)
+    _check(load_library().lacosmic_lplus(_dev(img, torch.float32, "img"),
+                                         _dev(out, torch.float32, "out", (h, w)), h, w,
+                                         _stream(stream)), "lacosmic_lplus")
+    return out
+
+
+def lacosmic_medfilt(img, k, out=None, stream=None):
+    torch = _torch()
+    h, w = img.shape
+    if out is None:
+        out = torch.empty_like(img)
+    _check(load_library().lacosmic_medfilt(_dev(img, torch.float32, "img"),
+                                           _dev(out, torch.float32, "out", (h, w)), h, w, int(k),
+                                           _stream(stream)), "lacosmic_medfilt")
+    return out
+
+
+def lacosmic_bitplane_pitch_words(w):
+    return int(load_library().lacosmic_bitplane_pitch_words(int(w)))
+
+
+def lacosmic_pack_bits(mask_u8, stream=None):
+    torch = _torch()
+    h, w = mask_u8.shape
+    bits = torch.empty((h, lacosmic_bitplane_pitch_words(w)), dtype=torch.int32, device=mask_u8.device)
+    _check(load_library().lacosmic_pack_bits(_dev(mask_u8, torch.uint8, "mask_u8"), bits.data_ptr(),
+                                             h, w, _stream(stream)), "lacosmic_pack_bits")
+    return bits
+
+
+def lacosmic_unpack_bits(bits, h, w, stream=None):
+    torch = _torch()
+    out = torch.empty((h, w), dtype=torch.uint8, device=bits.device)
+    _check(load_library().lacosmic_unpack_bits(
+        _dev(bits, torch.int32, "bits", (h, lacosmic_bitplane_pitch_words(w))), out.data_ptr(), h, w,
+        _stream(stream)), "lacosmic_unpack_bits")
+    return out
+
+
+def lacosmic_dilate3(bits, h, w, stream=None):
+    """bits: int32 [h][pitch] bit-plane (LSB = lowest x).  Returns the dilated bit-plane."""
+    torch = _torch()
+    out = torch.empty_like(bits)
+    _check(load_library().lacosmic_dilate3(
+        _dev(bits, torch.int32, "bits", (h, lacosmic_bitplane_pitch_words(w))), out.data_ptr(), h, w,
+        _stream(stream)), "lacosmic_dilate3")
+    return out
+
+
+def lacosmic_masked_median(img, mask_u8, out=None, workspace=None, stream=None):
+    torch = _torch()
+    h, w = img.shape
+    if out is None:
+        out = torch.empty_like(img)
+    if workspace is None:
+        workspace = _workspace(h, w, img.device)
+    _check(load_library().lacosmic_masked_median(
+        _dev(img, torch.float32, "img"), _dev(mask_u8, torch.uint8, "mask_u8", (h, w)),
+        _dev(out, torch.float32, "out", (h, w)), h, w, _dev(workspace, torch.uint8, "workspace"),
+        workspace.numel(), _stream(stream)), "lacosmic_masked_median")
+    return out
+
+
+def lacosmic_strerror(code):
+    return load_library().lacosmic_strerror(int(code)).decode()
+
+
+def lacosmic_last_launch_count():
+    return int(load_library().lacosmic_last_launch_count())
+
+
+def lacosmic_version():
+    return load_library().lacosmic_version().decode()

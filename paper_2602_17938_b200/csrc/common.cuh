@@ -1,0 +1,62 @@
+// Common device helpers for the L.A.Cosmic sm_100a kernels.
+// No code here is shared with oracle/ (the CPU oracle is an independent C file).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace lac {
+
+__device__ __forceinline__ int clampi(int v, int lo, int hi) { return min(max(v, lo), hi); }
+
+// compare-exchange: a <- min, b <- max (two FMNMX on the ALU pipe)
+__device__ __forceinline__ void ce(float& a, float& b) {
+    float t = fminf(a, b);
+    b = fmaxf(a, b);
+    a = t;
+}
+
+// 3-input min / max: one FMNMX3 each on sm_100a
+__device__ __forceinline__ float min3(float a, float b, float c) {
+    float r;
+    asm("min.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
+    return r;
+}
+__device__ __forceinline__ float max3(float a, float b, float c) {
+    float r;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
+    return r;
+}
+
+// exact median of three
+__device__ __forceinline__ float med3(float a, float b, float c) {
+    return fmaxf(fminf(a, b), fminf(fmaxf(a, b), c));
+}
+
+// Edge-replicate tile load (R3): sm[r][c] = src<y0-R+r, x0-R+c>, r < TH+2R, c < TW+2R.
+template <int TW, int TH, int R, int PITCH, int NT>
+__device__ __forceinline__ void load_tile_clamped(float* sm, const float* __restrict__ src, int h,
+                                                  int w, int y0, int x0, int tid) {
+    constexpr int SW = TW + 2 * R, SH = TH + 2 * R;
+    for (int i = tid; i < SW * SH; i += NT) {
+        int r = i / SW, c = i - r * SW;
+        int yy = clampi(y0 - R + r, 0, h - 1), xx = clampi(x0 - R + c, 0, w - 1);
+        sm[r * PITCH + c] = __ldg(src + (size_t)yy * w + xx);
+    }
+}
+
+// Step (1), O1: L+ from the centre and its four edge-replicated neighbours.
+// Operation order is normative (bit-exact against the oracle); no FMA contraction.
+__device__ __forceinline__ float lplus_px(float c, float U, float D, float Lf, float R) {
+    float two = __fmul_rn(2.0f, c);
+    float a = __fsub_rn(two, __fadd_rn(U, Lf));
+    float b = __fsub_rn(two, __fadd_rn(U, R));
+    float g = __fsub_rn(two, __fadd_rn(D, Lf));
+    float d = __fsub_rn(two, __fadd_rn(D, R));
+    a = a > 0.0f ? a : 0.0f;
+    b = b > 0.0f ? b : 0.0f;
+    g = g > 0.0f ? g : 0.0f;
+    d = d > 0.0f ? d : 0.0f;
+    return __fmul_rn(__fadd_rn(__fadd_rn(a, b), __fadd_rn(g, d)), 0.25f);
+}
+
+}  // namespace lac

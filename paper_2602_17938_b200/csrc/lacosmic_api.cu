@@ -1,0 +1,358 @@
+// C-ABI boundary of liblacosmic_b200.so: argument checks, workspace carve-up, kernel sequence.
+// See include/lacosmic.h for the contract of every entry point.
+#include "../../include/lacosmic.h"
+
+#include <cmath>
+#include <cstring>
+
+#include "kernels.cuh"
+
+namespace {
+
+thread_local int g_last_cuda_error = 0;
+thread_local int g_launches = 0;
+
+inline bool cuda_ok(cudaError_t e) {
+    if (e != cudaSuccess) {
+        g_last_cuda_error = (int)e;
+        return false;
+    }
+    return true;
+}
+#define CK(expr) do { if (!cuda_ok(expr)) return LACOSMIC_ERR_CUDA; } while (0)
+#define LAUNCHED() do { ++g_launches; if (!cuda_ok(cudaGetLastError())) return LACOSMIC_ERR_CUDA; } while (0)
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+inline int words_per_row(int w) { return (w + 31) / 32; }
+
+inline int check_shape(int h, int w) {
+    if (h < 1 || w < 1) return LACOSMIC_ERR_SHAPE;
+    if ((long long)h * (long long)w >= (1LL << 31)) return LACOSMIC_ERR_SHAPE;
+    return LACOSMIC_OK;
+}
+
+inline int check_params(const lacosmic_params& p) {
+    if (!std::isfinite(p.gain) || !std::isfinite(p.readnoise) || !std::isfinite(p.sigclip) ||
+        !std::isfinite(p.sigfrac) || !std::isfinite(p.objlim) || std::isnan(p.satlevel))
+        return LACOSMIC_ERR_PARAM;
+    if (!(p.gain > 0.0f) || p.readnoise < 0.0f || !(p.sigclip > 0.0f) || !(p.sigfrac > 0.0f) ||
+        p.sigfrac > 1.0f || p.objlim < 0.0f || p.niter < 0 || p.niter > LACOSMIC_MAX_NITER)
+        return LACOSMIC_ERR_PARAM;
+    return LACOSMIC_OK;
+}
+
+inline bool overlap(const void* a, size_t na, const void* b, size_t nb) {
+    uintptr_t pa = (uintptr_t)a, pb = (uintptr_t)b;
+    return pa < pb + nb && pb < pa + na;
+}
+
+// Workspace layout (all offsets 256-byte aligned)
+struct Workspace {
+    float* S;
+    uint32_t *G1, *G2, *M1, *M2, *M3, *C;
+    int32_t* counts;   // LACOSMIC_MAX_NITER ints
+    size_t bytes;
+};
+
+Workspace carve(void* base, int h, int w) {
+    Workspace ws;
+    size_t P = (size_t)h * w, plane = align_up(P * 4, 256);
+    size_t bp = align_up((size_t)h * words_per_row(w) * 4, 256);
+    char* p = (char*)base;
+    size_t off = 0;
+    ws.S = (float*)(p + off); off += plane;
+    ws.G1 = (uint32_t*)(p + off); off += bp;
+    ws.G2 = (uint32_t*)(p + off); off += bp;
+    ws.M1 = (uint32_t*)(p + off); off += bp;
+    ws.M2 = (uint32_t*)(p + off); off += bp;
+    ws.M3 = (uint32_t*)(p + off); off += bp;
+    ws.C = (uint32_t*)(p + off); off += bp;
+    ws.counts = (int32_t*)(p + off); off += align_up(LACOSMIC_MAX_NITER * 4, 256);
+    ws.bytes = off;
+    return ws;
+}
+
+int unpack(const uint32_t* bits, uint8_t* u8, int h, int w, cudaStream_t st) {
+    dim3 g((w + 255) / 256, h);
+    lac::k_unpack_bits<<<g, 256, 0, st>>>(bits, u8, h, w, words_per_row(w));
+    LAUNCHED();
+    return LACOSMIC_OK;
+}
+
+int replace_pass(const float* img, const uint32_t* C, float* work, int h, int w, const int* prev,
+                 cudaStream_t st) {
+    long long nwords = (long long)h * words_per_row(w);
+    unsigned blocks = (unsigned)((nwords + 255) / 256);
+    lac::k_replace<<<blocks, 256, 0, st>>>(img, C, work, h, w, words_per_row(w), prev);
+    LAUNCHED();
+    return LACOSMIC_OK;
+}
+
+// The iteration loop (O0-O7) for one frame.
+int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t* mask_out,
+              float* clean_out, const Workspace& ws, int32_t* iter_counts, const lacosmic_debug* dbg,
+              cudaStream_t st) {
+    const size_t P = (size_t)h * w;
+    const int wpr = words_per_row(w);
+    const size_t bp_bytes = (size_t)h * wpr * 4;
+    float* work = clean_out;
+    // O0
+    CK(cudaMemcpyAsync(work, img, P * 4, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemsetAsync(ws.C, 0, bp_bytes, st));
+    CK(cudaMemsetAsync(ws.counts, 0, LACOSMIC_MAX_NITER * 4, st));
+    const float siglow = p.sigfrac * p.sigclip;   // R9: one fp32 multiply on the host
+    const float rn2 = p.readnoise * p.readnoise;
+    lac::GateParams gp{p.sigclip, siglow, p.objlim, p.satlevel};
+    dim3 tb(32, 8), tg((w + lac::TW - 1) / lac::TW, (h + lac::TH - 1) / lac::TH);
+    dim3 dg((wpr + 31) / 32, (h + 7) / 8);
+    for (int t = 0; t < p.niter; ++t) {
+        const int* prev = t > 0 ? ws.counts + (t - 1) : nullptr;
+        const bool d = dbg && dbg->iter == t;
+        lac::k_noise_S<<<tg, tb, 0, st>>>(work, ws.S, d ? dbg->Lp : nullptr, d ? dbg->N : nullptr, h,
+                                         w, p.gain, rn2, prev);
+        LAUNCHED();
+        lac::k_fine_gates<<<tg, tb, 0, st>>>(work, ws.S, ws.G1, ws.G2, ws.M1, d ? dbg->Sp : nullptr,
+                                            d ? dbg->m3 : nullptr, d ? dbg->F : nullptr, h, w, wpr, gp,
+                                            prev);
+        LAUNCHED();
+        lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M1, ws.G1, ws.M2, nullptr, nullptr, h, w, wpr, prev);
+        LAUNCHED();
+        lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M2, ws.G2, ws.M3, ws.C, ws.counts + t, h, w, wpr,
+                                              prev);
+        LAUNCHED();
+        int rc = replace_pass(img, ws.C, work, h, w, prev, st);
+        if (rc) return rc;
+        if (d) {
+            if (dbg->S) CK(cudaMemcpyAsync(dbg->S, ws.S, P * 4, cudaMemcpyDeviceToDevice, st));
+            struct { const uint32_t* b; uint8_t* o; } planes[] = {
+                {ws.G1, dbg->G1}, {ws.G2, dbg->G2}, {ws.M1, dbg->M1},
+                {ws.M2, dbg->M2}, {ws.M3, dbg->M3}, {ws.C, dbg->C}};
+            for (auto& pl : planes)
+                if (pl.o && (rc = unpack(pl.b, pl.o, h, w, st))) return rc;
+        }
+    }
+    int rc = unpack(ws.C, mask_out, h, w, st);
+    if (rc) return rc;
+    if (iter_counts && p.niter > 0)
+        CK(cudaMemcpyAsync(iter_counts, ws.counts, (size_t)p.niter * 4, cudaMemcpyDeviceToDevice, st));
+    return LACOSMIC_OK;
+}
+
+int check_frame_args(const float* img, int h, int w, const lacosmic_params* p, const uint8_t* mask_out,
+                     const float* clean_out, const void* workspace, size_t workspace_bytes) {
+    if (!img || !p || !mask_out || !clean_out || !workspace) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    if ((rc = check_params(*p))) return rc;
+    if (((uintptr_t)img & 15) || ((uintptr_t)clean_out & 15) || ((uintptr_t)workspace & 255))
+        return LACOSMIC_ERR_ALIGN;
+    size_t P = (size_t)h * w, need = lacosmic_workspace_bytes(h, w);
+    if (workspace_bytes < need) return LACOSMIC_ERR_WORKSPACE;
+    if (overlap(img, P * 4, clean_out, P * 4) || overlap(img, P * 4, mask_out, P) ||
+        overlap(clean_out, P * 4, mask_out, P) || overlap(workspace, need, img, P * 4) ||
+        overlap(workspace, need, clean_out, P * 4) || overlap(workspace, need, mask_out, P))
+        return LACOSMIC_ERR_ALIAS;
+    return LACOSMIC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t lacosmic_workspace_bytes(int h, int w) {
+    if (check_shape(h, w)) return 0;
+    return carve(nullptr, h, w).bytes;
+}
+
+int lacosmic_run_ws(const float* img, int h, int w, const lacosmic_params* p, uint8_t* mask_out,
+                    float* clean_out, void* workspace, size_t workspace_bytes, int32_t* iter_counts,
+                    const lacosmic_debug* dbg, void* stream) {
+    g_launches = 0;
+    int rc = check_frame_args(img, h, w, p, mask_out, clean_out, workspace, workspace_bytes);
+    if (rc) return rc;
+    if (dbg && (dbg->iter < 0 || dbg->iter >= LACOSMIC_MAX_NITER)) return LACOSMIC_ERR_PARAM;
+    return run_frame(img, h, w, *p, mask_out, clean_out, carve(workspace, h, w), iter_counts, dbg,
+                     (cudaStream_t)stream);
+}
+
+int lacosmic_run(const float* img, int h, int w, float gain, float readnoise, float sigclip,
+                 float sigfrac, float objlim, int niter, float satlevel, uint8_t* mask_out,
+                 float* clean_out, void* stream) {
+    g_launches = 0;
+    lacosmic_params p{gain, readnoise, sigclip, sigfrac, objlim, satlevel, niter};
+    if (!img || !mask_out || !clean_out) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    if ((rc = check_params(p))) return rc;
+    size_t need = lacosmic_workspace_bytes(h, w);
+    void* ws = nullptr;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaMallocAsync(&ws, need, st));
+    rc = check_frame_args(img, h, w, &p, mask_out, clean_out, ws, need);
+    if (!rc) rc = run_frame(img, h, w, p, mask_out, clean_out, carve(ws, h, w), nullptr, nullptr, st);
+    if (!cuda_ok(cudaFreeAsync(ws, st)) && !rc) rc = LACOSMIC_ERR_CUDA;
+    return rc;
+}
+
+int lacosmic_run_batch(const float* imgs, int n, int h, int w, const lacosmic_params* params,
+                       uint8_t* masks_out, float* cleans_out, void* workspace, size_t workspace_bytes,
+                       int32_t* iter_counts, void* stream) {
+    g_launches = 0;
+    if (n < 0) return LACOSMIC_ERR_SHAPE;
+    if (n == 0) return LACOSMIC_OK;
+    if (!imgs || !params || !masks_out || !cleans_out || !workspace) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    size_t P = (size_t)h * w;
+    if ((P * 4) & 15) {
+        // frames inside the batch must each stay 16-byte aligned
+        if (n > 1) return LACOSMIC_ERR_ALIGN;
+    }
+    for (int f = 0; f < n; ++f) {
+        rc = check_frame_args(imgs + f * P, h, w, params + f, masks_out + f * P, cleans_out + f * P,
+                              workspace, workspace_bytes);
+        if (rc) return rc;
+    }
+    if (overlap(imgs, n * P * 4, cleans_out, n * P * 4) || overlap(imgs, n * P * 4, masks_out, n * P) ||
+        overlap(cleans_out, n * P * 4, masks_out, n * P))
+        return LACOSMIC_ERR_ALIAS;
+    Workspace ws = carve(workspace, h, w);
+    for (int f = 0; f < n; ++f) {
+        rc = run_frame(imgs + f * P, h, w, params[f], masks_out + f * P, cleans_out + f * P, ws, nullptr,
+                       nullptr, (cudaStream_t)stream);
+        if (rc) return rc;
+        if (iter_counts)
+            CK(cudaMemcpyAsync(iter_counts + (size_t)f * LACOSMIC_MAX_NITER, ws.counts,
+                               LACOSMIC_MAX_NITER * 4, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    }
+    return LACOSMIC_OK;
+}
+
+size_t lacosmic_host_workspace_bytes(int h, int w) {
+    if (check_shape(h, w)) return 0;
+    size_t P = (size_t)h * w;
+    return align_up(P * 4, 256) * 2 + align_up(P, 256) + lacosmic_workspace_bytes(h, w);
+}
+
+int lacosmic_run_host(const float* img_host, int h, int w, const lacosmic_params* p,
+                      uint8_t* mask_out_host, float* clean_out_host, void* dev_workspace,
+                      size_t dev_workspace_bytes, void* stream) {
+    g_launches = 0;
+    if (!img_host || !p || !mask_out_host || !clean_out_host || !dev_workspace) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    if ((rc = check_params(*p))) return rc;
+    if ((uintptr_t)dev_workspace & 255) return LACOSMIC_ERR_ALIGN;
+    if (dev_workspace_bytes < lacosmic_host_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
+    size_t P = (size_t)h * w, plane = align_up(P * 4, 256);
+    char* base = (char*)dev_workspace;
+    float* d_img = (float*)base;
+    float* d_clean = (float*)(base + plane);
+    uint8_t* d_mask = (uint8_t*)(base + 2 * plane);
+    void* ws = base + 2 * plane + align_up(P, 256);
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaMemcpyAsync(d_img, img_host, P * 4, cudaMemcpyHostToDevice, st));
+    rc = run_frame(d_img, h, w, *p, d_mask, d_clean, carve(ws, h, w), nullptr, nullptr, st);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(clean_out_host, d_clean, P * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(mask_out_host, d_mask, P, cudaMemcpyDeviceToHost, st));
+    return LACOSMIC_OK;
+}
+
+// ---- single steps -----------------------------------------------------------------------------
+
+int lacosmic_lplus(const float* in, float* out, int h, int w, void* stream) {
+    if (!in || !out) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    if (overlap(in, (size_t)h * w * 4, out, (size_t)h * w * 4)) return LACOSMIC_ERR_ALIAS;
+    dim3 g((w + 31) / 32, (h + 7) / 8), b(32, 8);
+    lac::k_lplus<<<g, b, 0, (cudaStream_t)stream>>>(in, out, h, w);
+    LAUNCHED();
+    return LACOSMIC_OK;
+}
+
+int lacosmic_medfilt(const float* in, float* out, int h, int w, int k, void* stream) {
+    if (!in || !out) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    if (k != 3 && k != 5 && k != 7) return LACOSMIC_ERR_PARAM;
+    if (overlap(in, (size_t)h * w * 4, out, (size_t)h * w * 4)) return LACOSMIC_ERR_ALIAS;
+    dim3 tb(32, 8), tg((w + lac::TW - 1) / lac::TW, (h + lac::TH - 1) / lac::TH);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (k == 3) lac::k_medfilt<3><<<tg, tb, 0, st>>>(in, out, h, w);
+    else if (k == 5) lac::k_medfilt<5><<<tg, tb, 0, st>>>(in, out, h, w);
+    else lac::k_medfilt<7><<<tg, tb, 0, st>>>(in, out, h, w);
+    LAUNCHED();
+    return LACOSMIC_OK;
+}
+
+int lacosmic_bitplane_pitch_words(int w) { return w < 1 ? 0 : words_per_row(w); }
+
+int lacosmic_pack_bits(const uint8_t* mask_u8, uint32_t* bits, int h, int w, void* stream) {
+    if (!mask_u8 || !bits) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    dim3 g((w + 255) / 256, h);
+    lac::k_pack_bits<<<g, 256, 0, (cudaStream_t)stream>>>(mask_u8, bits, h, w, words_per_row(w));
+    LAUNCHED();
+    return LACOSMIC_OK;
+}
+
+int lacosmic_unpack_bits(const uint32_t* bits, uint8_t* mask_u8, int h, int w, void* stream) {
+    if (!mask_u8 || !bits) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    return unpack(bits, mask_u8, h, w, (cudaStream_t)stream);
+}
+
+int lacosmic_dilate3(const uint32_t* bits_in, uint32_t* bits_out, int h, int w, void* stream) {
+    if (!bits_in || !bits_out) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    int wpr = words_per_row(w);
+    if (overlap(bits_in, (size_t)h * wpr * 4, bits_out, (size_t)h * wpr * 4)) return LACOSMIC_ERR_ALIAS;
+    dim3 dg((wpr + 31) / 32, (h + 7) / 8);
+    lac::k_dilate_gate<<<dg, 256, 0, (cudaStream_t)stream>>>(bits_in, nullptr, bits_out, nullptr, nullptr,
+                                                           h, w, wpr, nullptr);
+    LAUNCHED();
+    return LACOSMIC_OK;
+}
+
+int lacosmic_masked_median(const float* img, const uint8_t* mask_u8, float* out, int h, int w,
+                           void* workspace, size_t workspace_bytes, void* stream) {
+    if (!img || !mask_u8 || !out || !workspace) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    if ((uintptr_t)workspace & 255) return LACOSMIC_ERR_ALIGN;
+    if (workspace_bytes < lacosmic_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
+    size_t P = (size_t)h * w;
+    if (overlap(img, P * 4, out, P * 4)) return LACOSMIC_ERR_ALIAS;
+    Workspace ws = carve(workspace, h, w);
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = lacosmic_pack_bits(mask_u8, ws.C, h, w, stream))) return rc;
+    CK(cudaMemcpyAsync(out, img, P * 4, cudaMemcpyDeviceToDevice, st));
+    return replace_pass(img, ws.C, out, h, w, nullptr, st);
+}
+
+// ---- diagnostics ------------------------------------------------------------------------------
+
+const char* lacosmic_strerror(int code) {
+    switch (code) {
+        case LACOSMIC_OK: return "ok";
+        case LACOSMIC_ERR_NULL: return "required pointer is NULL";
+        case LACOSMIC_ERR_SHAPE: return "invalid shape (h, w >= 1 and h*w < 2^31 required)";
+        case LACOSMIC_ERR_PARAM: return "invalid parameter";
+        case LACOSMIC_ERR_ALIGN: return "pointer not sufficiently aligned";
+        case LACOSMIC_ERR_ALIAS: return "buffers overlap";
+        case LACOSMIC_ERR_WORKSPACE: return "workspace too small";
+        case LACOSMIC_ERR_CUDA: return "CUDA call failed (see lacosmic_last_cuda_error)";
+        default: return "unknown error code";
+    }
+}
+
+int lacosmic_last_cuda_error(void) { return g_last_cuda_error; }
+int lacosmic_last_launch_count(void) { return g_launches; }
+const char* lacosmic_version(void) { return "lacosmic-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"
