@@ -1,0 +1,356 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the L.A.Cosmic hot path on B200 (contract: see DESIGN.md section 7).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config2|config1|config0|stream]
+    python bench.py --impl reference ...        # the CPU oracle on the host cores, same metric
+
+One "step" = one whole pass of the hot path (all section-8(a) rows: niter = 4 iterations of steps
+(1)-(7) plus frame prologue/epilogue) over one synthetic 4000x6500 fp32 frame (BASELINE.json
+configs[2]).  `value` = frames/s with the frame resident in HBM (CUDA events around each step, L2
+flushed between steps, max over ranks); `e2e` = the same through lacosmic_run_host with pinned HOST
+buffers, H2D + D2H inside the timed region.  Frames are independent, so N GPUs run N replicas with
+no collective ("scaling": "weak").  Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_2602_17938_b200 import synth  # noqa: E402
+
+METRIC = "frames/s, 4000x6500 fp32 L.A.Cosmic (niter=4)"
+# ALU-pipe roofline: FMNMX/FMNMX3 issue at 64 lanes/clk/SM (measured,
+# profiles/r01_alu_minmax_microbench.txt) -> 148 SM x 64 x clocks.max.sm.
+ALU_LANES_PER_CLK_SM = 64
+N_SM = 148
+# min/max (ALU-pipe FMNMX) instructions the dominant kernel executes per output pixel, from its SASS
+# (DESIGN.md section 5 table; cross-checked against ncu smsp__inst_executed_pipe_alu in profiles/).
+FINE_GATES_MINMAX_PER_PX = None   # filled from the library's own accounting below
+# reference compare-exchanges per pixel per iteration with per-pixel networks:
+REF_COMPARISONS_PER_PX_ITER = 19 + 99 + 99 + 480
+# dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture
+# (profiles/; None until captured)
+NCU_TRAFFIC_BYTES = None
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)),
+                    source="measured (MEASURED_PEAKS.json)")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback (B200_PROFILING.md)")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (profiling recipe's clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu, self.proc, self.lines = gpu_index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if not self.proc:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); smax.append(float(f[2])); power.append(float(f[3]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        return dict(sm_mhz=statistics.median(sm) if sm else None,
+                    sm_max_mhz=max(smax) if smax else None,
+                    power_w_max=max(power) if power else None,
+                    samples=len(sm), reasons=sorted(reasons))
+
+
+def _workload(name):
+    if name == "config2":
+        return dict(cfg=2, label="configs[2]: 4000x6500 fp32, 8000 stars, 30000 CRs, 0.5% salt-and-pepper")
+    if name == "config1":
+        return dict(cfg=1, label="configs[1]: 2048x2048 fp32")
+    if name == "config0":
+        return dict(cfg=0, label="configs[0]: 512x512 fp32")
+    raise SystemExit("unknown workload " + name)
+
+
+# ------------------------------------------------------------------------------------------- oracle legs
+def _oracle_sample(img, params, rows):
+    """Time the oracle, as it stands, on the top `rows` rows of the frame (a bounded sample)."""
+    from oracle import lacosmic_oracle as orc   # allowed here: cpu_baseline / --impl reference legs
+    orc.build()
+    crop = np.ascontiguousarray(img[:rows])
+    t0 = time.perf_counter()
+    orc.run(crop, **params)
+    dt = time.perf_counter() - t0
+    return dt, crop.size, orc.max_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    wl = _workload(args.workload)
+    frame = synth.make_config(wl["cfg"])
+    params = dict(synth.DEFAULT_PARAMS)
+    h, w = frame.img.shape
+    rows = min(h, max(64, h // 8))          # 1/8 of the frame per step: a few seconds per step
+    times = []
+    for i in range(args.warmup + args.steps):
+        dt, px, cores = _oracle_sample(frame.img, params, rows)
+        if i >= args.warmup:
+            times.append(dt)
+    per_frame = statistics.mean(times) * (h * w) / px
+    value = 1.0 / per_frame
+    sample = "top %d of %d rows of the frame per step, time scaled by pixel count" % (rows, h)
+    line = dict(impl="reference", metric=METRIC, value=value, unit="frames/s", n_gpus=args.gpus,
+                steps=args.steps, warmup=args.warmup, ms_per_step=per_frame * 1e3,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+                config=dict(workload=wl["label"], h=h, w=w, niter=params["niter"]),
+                mpix_per_s=value * h * w / 1e6,
+                cpu_baseline=dict(value=value, unit="frames/s", cores=cores, kind="oracle", sample=sample),
+                e2e=dict(value=value, unit="frames/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------- CUDA arm
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2602_17938_b200 as lc
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    lc.load_library()
+    peaks = _peaks()
+
+    wl = _workload(args.workload)
+    # replicas: every rank cleans its own frame (same generator, seed offset by rank)
+    kw = dict(synth.CONFIGS[wl["cfg"]])
+    kw["seed"] = kw["seed"] + 100 * rank
+    frame = synth.make_frame(**kw)
+    params = dict(synth.DEFAULT_PARAMS)
+    P = lc.Params(**params)
+    h, w = frame.img.shape
+    npx = h * w
+
+    img = torch.from_numpy(frame.img).to(dev)
+    mask = torch.empty((h, w), dtype=torch.uint8, device=dev)
+    clean = torch.empty_like(img)
+    ws = torch.empty(lc.lacosmic_workspace_bytes(h, w), dtype=torch.uint8, device=dev)
+    counts = torch.zeros(params["niter"], dtype=torch.int32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step():
+        lc.lacosmic_run_ws(img, P, mask_out=mask, clean_out=clean, workspace=ws, iter_counts=counts)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps, warmup):
+        for _ in range(warmup):
+            fn()
+        barrier()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+               for _ in range(steps)]
+        for a, b in evs:
+            flush.zero_()                    # L2 flush, outside the event pair
+            a.record(stream)
+            fn()
+            b.record(stream)
+        barrier()
+        total_ms = sum(a.elapsed_time(b) for a, b in evs)
+        if world > 1:
+            t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            total_ms = float(t.item())
+        return total_ms / steps
+
+    # ---- device-resident timing (value), with per-kernel event spans from the library
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    lc.lacosmic_kernel_timing_enable(True)
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    lc.lacosmic_kernel_timing_read()         # drop warm-up spans
+    ms_step = timed(step, args.steps, 0)
+    ktimes = lc.lacosmic_kernel_timing_read()
+    lc.lacosmic_kernel_timing_enable(False)
+    launches_per_step = lc.lacosmic_last_launch_count()
+    clocks = sampler.stop() if rank == 0 else None
+    counts_host = counts.cpu().numpy().tolist()
+    mask_frac = float(mask.float().mean().item())
+
+    # the same region without the event spans (reported for transparency)
+    ms_step_nospans = timed(step, max(2, args.steps // 2), 1)
+
+    # ---- end to end through the host-buffer C-ABI call
+    img_h = torch.from_numpy(frame.img).pin_memory()
+    mask_h = torch.empty((h, w), dtype=torch.uint8).pin_memory()
+    clean_h = torch.empty((h, w), dtype=torch.float32).pin_memory()
+    hws = torch.empty(lc.lacosmic_host_workspace_bytes(h, w), dtype=torch.uint8, device=dev)
+
+    def step_host():
+        lc.lacosmic_run_host(img_h, P, mask_out_host=mask_h, clean_out_host=clean_h, dev_workspace=hws)
+
+    ms_e2e = timed(step_host, args.steps, max(1, args.warmup // 2))
+    same = bool((mask_h.numpy() == mask.cpu().numpy()).all() and
+                (clean_h.numpy() == clean.cpu().numpy()).all())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    frames_per_s = world * 1e3 / ms_step
+    e2e_fps = world * 1e3 / ms_e2e
+    niter = params["niter"]
+
+    # ---- roofline of the dominant kernel
+    dom = max((k for k in ktimes if k != "whole_frame"), key=lambda k: ktimes[k][0])
+    dom_ms, dom_spans = ktimes[dom]
+    dom_avg_ms = dom_ms / max(dom_spans, 1)
+    share = {k: round(v[0] / max(ktimes["whole_frame"][0], 1e-9), 4) for k, v in ktimes.items()
+             if k != "whole_frame"}
+    sm_max = (clocks or {}).get("sm_max_mhz") or peaks["sm_max_mhz"]
+    alu_peak = N_SM * ALU_LANES_PER_CLK_SM * sm_max * 1e6 / 1e12          # T min/max instr / s
+    ops_px = KERNEL_MINMAX_PER_PX.get(dom)
+    roof = None
+    if ops_px is not None:
+        achieved = npx * ops_px / (dom_avg_ms * 1e-3) / 1e12
+        roof = dict(bound="alu", kernel=dom, achieved=achieved, peak=alu_peak,
+                    unit="T min/max instr/s", frac=achieved / alu_peak, traffic=NCU_TRAFFIC_BYTES,
+                    peak_source="148 SM x 64 ALU lanes/clk x %.0f MHz (DESIGN.md section 5; lanes/clk "
+                                "measured in profiles/r01_alu_minmax_microbench.txt)" % sm_max,
+                    minmax_instr_per_px=ops_px, avg_launch_ms=dom_avg_ms, launches_timed=dom_spans)
+    hbm_bytes_step = npx * (HBM_BYTES_PER_PX_ITER * niter + HBM_BYTES_PER_PX_FRAME)
+    hbm = dict(algorithmic_bytes_per_step=hbm_bytes_step,
+               achieved_gbs=hbm_bytes_step / (ms_step * 1e-3) / 1e9 * 1.0,
+               peak_gbs=peaks["hbm_gbs"], peak_source=peaks["source"],
+               frac=hbm_bytes_step / (ms_step * 1e-3) / 1e9 / peaks["hbm_gbs"])
+    ref_cmp_rate = npx * REF_COMPARISONS_PER_PX_ITER * niter / (ms_step * 1e-3) / 1e12
+
+    # ---- the oracle on the host cores: a bounded sample of the same frame
+    cpu = None
+    if not args.no_cpu_baseline:
+        rows = min(h, 1000)
+        dt, px, cores = _oracle_sample(frame.img, params, rows)
+        cpu = dict(value=(px / npx) / dt, unit="frames/s", cores=cores, kind="oracle",
+                   sample="top %d of %d rows of the same frame, one run, %.1f s; frames/s scaled by "
+                          "pixel count" % (rows, h, dt))
+
+    line = dict(
+        metric=METRIC, value=frames_per_s, unit="frames/s", n_gpus=world, steps=args.steps,
+        warmup=args.warmup, ms_per_step=ms_step, higher_is_better=True, scaling="weak",
+        vs_baseline=None, dtype="f32", data="synthetic",
+        config=dict(workload=wl["label"], h=h, w=w, niter=niter, sigclip=params["sigclip"],
+                    sigfrac=params["sigfrac"], objlim=params["objlim"],
+                    l2="flushed between steps (256 MiB write outside the event pair)",
+                    parallelism="replicas (one frame per GPU, no collective)"),
+        mpix_per_s=frames_per_s * npx / 1e6,
+        e2e=dict(value=e2e_fps, unit="frames/s", h2d_bytes_per_step=npx * 4,
+                 d2h_bytes_per_step=npx * 5, ms_per_step=ms_e2e, matches_device_path=same,
+                 call="lacosmic_run_host (pinned host buffers)"),
+        gpu_launches=launches_per_step * args.steps,
+        launches_per_step=launches_per_step,
+        roofline=roof, hbm=hbm,
+        kernels_ms_per_step={k: round(v[0] / args.steps, 4) for k, v in ktimes.items()},
+        kernel_share_of_step=share,
+        ms_per_step_without_event_spans=ms_step_nospans,
+        ref_comparisons_T_per_s=ref_cmp_rate,
+        new_cr_per_iteration=counts_host, mask_fraction=mask_frac,
+        clocks=clocks, cpu_baseline=cpu,
+        context="paper (PAPER.md:31,47): 55 s/frame dfcosmic C++ at 2 threads on AWS; GPU variant on an "
+                "RTX 5060 Ti >10x faster than CPU variants (no absolute number in the text)",
+    )
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+# ALU-pipe min/max instructions per output pixel of each kernel class (static SASS
+# count of FMNMX/FMNMX3 per pixel, halo recomputation included) -- the per-unit figure behind
+# roofline.achieved.  v1 kernels: forgetful selection, per-pixel.
+KERNEL_MINMAX_PER_PX = {
+    "fine_gates": 2 * (99 + 480) + 1.28 * 2 * 19 + 5,    # med5(S) + med7(m3) + med3 on the haloed tile
+    "noise_S": 2 * 99 + 6,
+}
+# HBM bytes per pixel the path must move with the current fusion:
+# noise_S: read work 4 + write S 4; fine_gates: read work 4 + S 4 + 0.375 bit-planes; dilate/replace ~1
+HBM_BYTES_PER_PX_ITER = 4 + 4 + 4 + 4 + 0.375 + 1.0
+HBM_BYTES_PER_PX_FRAME = 8 + 1.125
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="config2", choices=["config2", "config1", "config0"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "cuda":
+        args.warmup = 3                          # timing rule: at least 3 warm-up steps
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

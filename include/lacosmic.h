@@ -148,6 +148,18 @@ int lacosmic_last_cuda_error(void);
 int lacosmic_last_launch_count(void);
 const char *lacosmic_version(void);
 
+/* Optional CUDA-event timing per kernel class, per calling thread.  After
+ * lacosmic_kernel_timing_enable(1) every launch of the whole-path entry points is bracketed by an
+ * event pair on the caller's stream (up to 8192 spans between reads).  Once the caller has
+ * synchronised the stream, lacosmic_kernel_timing_read() writes, for each class c <
+ * LACOSMIC_NUM_KERNEL_CLASSES, the summed device time ms_sum[c] and the number of spans[c] (HOST
+ * arrays), and clears the record.  Class names: lacosmic_kernel_class_name(c); the last class is the
+ * whole frame (copies included). */
+#define LACOSMIC_NUM_KERNEL_CLASSES 6
+int lacosmic_kernel_timing_enable(int enable);
+int lacosmic_kernel_timing_read(float *ms_sum, int32_t *spans);
+const char *lacosmic_kernel_class_name(int cls);
+
 #ifdef __cplusplus
 }
 #endif

@@ -10,6 +10,8 @@ from .binding import (  # noqa: F401
     lacosmic_bitplane_pitch_words,
     lacosmic_dilate3,
     lacosmic_host_workspace_bytes,
+    lacosmic_kernel_timing_enable,
+    lacosmic_kernel_timing_read,
     lacosmic_last_launch_count,
     lacosmic_lplus,
     lacosmic_masked_median,

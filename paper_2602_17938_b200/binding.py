@@ -21,7 +21,9 @@ EXPORTS = (
     "lacosmic_bitplane_pitch_words", "lacosmic_pack_bits", "lacosmic_unpack_bits",
     "lacosmic_dilate3", "lacosmic_masked_median", "lacosmic_strerror",
     "lacosmic_last_cuda_error", "lacosmic_last_launch_count", "lacosmic_version",
+    "lacosmic_kernel_timing_enable", "lacosmic_kernel_timing_read", "lacosmic_kernel_class_name",
 )
+NUM_KERNEL_CLASSES = 6
 
 
 class LacosmicError(RuntimeError):
@@ -98,6 +100,9 @@ def load_library():
         "lacosmic_last_cuda_error": (i, []),
         "lacosmic_last_launch_count": (i, []),
         "lacosmic_version": (C.c_char_p, []),
+        "lacosmic_kernel_timing_enable": (i, [i]),
+        "lacosmic_kernel_timing_read": (i, [vp, vp]),
+        "lacosmic_kernel_class_name": (C.c_char_p, [i]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)      # AttributeError if the header and the library disagree
@@ -346,3 +351,18 @@ def lacosmic_last_launch_count():
 
 def lacosmic_version():
     return load_library().lacosmic_version().decode()
+
+
+def lacosmic_kernel_timing_enable(enable=True):
+    _check(load_library().lacosmic_kernel_timing_enable(1 if enable else 0),
+           "lacosmic_kernel_timing_enable")
+
+
+def lacosmic_kernel_timing_read():
+    """{class name: (summed ms, spans)} since the last read; synchronise the stream first."""
+    L = load_library()
+    ms = (C.c_float * NUM_KERNEL_CLASSES)()
+    n = (C.c_int32 * NUM_KERNEL_CLASSES)()
+    _check(L.lacosmic_kernel_timing_read(ms, n), "lacosmic_kernel_timing_read")
+    return {L.lacosmic_kernel_class_name(c).decode(): (float(ms[c]), int(n[c]))
+            for c in range(NUM_KERNEL_CLASSES)}

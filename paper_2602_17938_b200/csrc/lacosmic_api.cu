@@ -22,6 +22,34 @@ inline bool cuda_ok(cudaError_t e) {
 #define CK(expr) do { if (!cuda_ok(expr)) return LACOSMIC_ERR_CUDA; } while (0)
 #define LAUNCHED() do { ++g_launches; if (!cuda_ok(cudaGetLastError())) return LACOSMIC_ERR_CUDA; } while (0)
 
+// Optional per-kernel-class CUDA-event timing (lacosmic_kernel_timing_*): bench.py switches it on to
+// measure the dominant kernel's average launch duration on the launching stream.
+enum KClass { KC_NOISE_S = 0, KC_FINE_GATES, KC_DILATE, KC_REPLACE, KC_BITS, KC_STEP, KC_COUNT };
+static_assert(KC_COUNT == LACOSMIC_NUM_KERNEL_CLASSES, "header and library disagree");
+struct KTiming {
+    static constexpr int MAXSPANS = 8192;
+    bool enabled = false;
+    int n = 0;
+    cudaEvent_t* ev = nullptr;   // 2 * MAXSPANS events, created on first enable
+    int cls[MAXSPANS];
+};
+thread_local KTiming g_kt;
+
+struct Span {   // records an event pair around one launch when timing is enabled
+    int i = -1;
+    cudaStream_t st;
+    Span(int cls, cudaStream_t s) : st(s) {
+        if (g_kt.enabled && g_kt.n < KTiming::MAXSPANS) {
+            i = g_kt.n++;
+            g_kt.cls[i] = cls;
+            cudaEventRecord(g_kt.ev[2 * i], st);
+        }
+    }
+    ~Span() {
+        if (i >= 0) cudaEventRecord(g_kt.ev[2 * i + 1], st);
+    }
+};
+
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 inline int words_per_row(int w) { return (w + 31) / 32; }
 
@@ -74,6 +102,7 @@ Workspace carve(void* base, int h, int w) {
 
 int unpack(const uint32_t* bits, uint8_t* u8, int h, int w, cudaStream_t st) {
     dim3 g((w + 255) / 256, h);
+    Span sp(KC_BITS, st);
     lac::k_unpack_bits<<<g, 256, 0, st>>>(bits, u8, h, w, words_per_row(w));
     LAUNCHED();
     return LACOSMIC_OK;
@@ -83,6 +112,7 @@ int replace_pass(const float* img, const uint32_t* C, float* work, int h, int w,
                  cudaStream_t st) {
     long long nwords = (long long)h * words_per_row(w);
     unsigned blocks = (unsigned)((nwords + 255) / 256);
+    Span sp(KC_REPLACE, st);
     lac::k_replace<<<blocks, 256, 0, st>>>(img, C, work, h, w, words_per_row(w), prev);
     LAUNCHED();
     return LACOSMIC_OK;
@@ -96,6 +126,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     const int wpr = words_per_row(w);
     const size_t bp_bytes = (size_t)h * wpr * 4;
     float* work = clean_out;
+    Span whole(KC_STEP, st);   // the whole frame, copies included
     // O0
     CK(cudaMemcpyAsync(work, img, P * 4, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemsetAsync(ws.C, 0, bp_bytes, st));
@@ -108,18 +139,28 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     for (int t = 0; t < p.niter; ++t) {
         const int* prev = t > 0 ? ws.counts + (t - 1) : nullptr;
         const bool d = dbg && dbg->iter == t;
-        lac::k_noise_S<<<tg, tb, 0, st>>>(work, ws.S, d ? dbg->Lp : nullptr, d ? dbg->N : nullptr, h,
-                                         w, p.gain, rn2, prev);
-        LAUNCHED();
-        lac::k_fine_gates<<<tg, tb, 0, st>>>(work, ws.S, ws.G1, ws.G2, ws.M1, d ? dbg->Sp : nullptr,
-                                            d ? dbg->m3 : nullptr, d ? dbg->F : nullptr, h, w, wpr, gp,
-                                            prev);
-        LAUNCHED();
-        lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M1, ws.G1, ws.M2, nullptr, nullptr, h, w, wpr, prev);
-        LAUNCHED();
-        lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M2, ws.G2, ws.M3, ws.C, ws.counts + t, h, w, wpr,
-                                              prev);
-        LAUNCHED();
+        {
+            Span sp(KC_NOISE_S, st);
+            lac::k_noise_S<<<tg, tb, 0, st>>>(work, ws.S, d ? dbg->Lp : nullptr, d ? dbg->N : nullptr,
+                                             h, w, p.gain, rn2, prev);
+            LAUNCHED();
+        }
+        {
+            Span sp(KC_FINE_GATES, st);
+            lac::k_fine_gates<<<tg, tb, 0, st>>>(work, ws.S, ws.G1, ws.G2, ws.M1,
+                                                d ? dbg->Sp : nullptr, d ? dbg->m3 : nullptr,
+                                                d ? dbg->F : nullptr, h, w, wpr, gp, prev);
+            LAUNCHED();
+        }
+        {
+            Span sp(KC_DILATE, st);
+            lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M1, ws.G1, ws.M2, nullptr, nullptr, h, w, wpr,
+                                                  prev);
+            LAUNCHED();
+            lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M2, ws.G2, ws.M3, ws.C, ws.counts + t, h, w, wpr,
+                                                  prev);
+            LAUNCHED();
+        }
         int rc = replace_pass(img, ws.C, work, h, w, prev, st);
         if (rc) return rc;
         if (d) {
@@ -349,6 +390,35 @@ const char* lacosmic_strerror(int code) {
         case LACOSMIC_ERR_CUDA: return "CUDA call failed (see lacosmic_last_cuda_error)";
         default: return "unknown error code";
     }
+}
+
+int lacosmic_kernel_timing_enable(int enable) {
+    if (enable && !g_kt.ev) {
+        g_kt.ev = new cudaEvent_t[2 * KTiming::MAXSPANS];
+        for (int i = 0; i < 2 * KTiming::MAXSPANS; ++i) CK(cudaEventCreate(&g_kt.ev[i]));
+    }
+    g_kt.enabled = enable != 0;
+    g_kt.n = 0;
+    return LACOSMIC_OK;
+}
+
+int lacosmic_kernel_timing_read(float* ms_sum, int32_t* spans) {
+    if (!ms_sum || !spans) return LACOSMIC_ERR_NULL;
+    for (int c = 0; c < KC_COUNT; ++c) ms_sum[c] = 0.0f, spans[c] = 0;
+    for (int i = 0; i < g_kt.n; ++i) {
+        float ms = 0.0f;
+        CK(cudaEventElapsedTime(&ms, g_kt.ev[2 * i], g_kt.ev[2 * i + 1]));
+        ms_sum[g_kt.cls[i]] += ms;
+        spans[g_kt.cls[i]] += 1;
+    }
+    g_kt.n = 0;
+    return LACOSMIC_OK;
+}
+
+const char* lacosmic_kernel_class_name(int cls) {
+    static const char* names[KC_COUNT] = {"noise_S", "fine_gates", "dilate_x2", "replace", "bits",
+                                          "whole_frame"};
+    return (cls >= 0 && cls < KC_COUNT) ? names[cls] : "?";
 }
 
 int lacosmic_last_cuda_error(void) { return g_last_cuda_error; }
