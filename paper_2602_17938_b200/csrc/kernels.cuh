@@ -1,58 +1,97 @@
 // sm_100a kernels of the L.A.Cosmic iteration (DESIGN.md section 5 lists each with its roofline).
 #pragma once
+#include <cuda.h>
+
 #include "common.cuh"
-#include "median_select.cuh"
+#include "median_networks.cuh"
 
 namespace lac {
 
-constexpr int TW = 64;    // output tile width  (two ballot words)
-constexpr int TH = 32;    // output tile height
-constexpr int NT = 256;   // threads per CTA, laid out 32 x 8
-constexpr int PX = TW / 32;
-constexpr int PY = TH / 8;
+constexpr int TW = 128;   // output tile width: 32 lanes x 4 adjacent outputs per thread
+constexpr int TH = 16;    // output tile height: 8 warps x 2 rows
+constexpr int NT = 256;   // threads per CTA (8 warps)
+constexpr int NWARP = NT / 32;
 
 struct GateParams {
     float sigclip, siglow, objlim, satlevel;
 };
 
-// median of the K x K window centred at tile-local (r, c) of a shared-memory tile (r, c already
-// include the halo offset)
+// Edge-replicate tile load with margins (R3): sm[r][c] = src<y0-MY+r, x0-MX+c>.
+template <int MX, int MY, int PITCH>
+__device__ __forceinline__ void load_tile(float* sm, const float* __restrict__ src, int h, int w, int y0,
+                                          int x0, int tid) {
+    constexpr int SW = TW + 2 * MX, SH = TH + 2 * MY;
+    static_assert(PITCH >= SW && PITCH % 4 == 0, "pitch must hold the tile and keep float4 alignment");
+    for (int i = tid; i < SW * SH; i += NT) {
+        int r = i / SW, c = i - r * SW;
+        int yy = clampi(y0 - MY + r, 0, h - 1), xx = clampi(x0 - MX + c, 0, w - 1);
+        sm[r * PITCH + c] = __ldg(src + (size_t)yy * w + xx);
+    }
+}
+
+// K x (K+3) register window for 4 adjacent outputs: in[c][r], c = 0..K+2 left to right, r = 0..K-1 top
+// to bottom.  `p` points at (top row, the 16-byte aligned column 4 to the left of the first output).
 template <int K, int PITCH>
-__device__ __forceinline__ float median_window(const float* sm, int r, int c) {
+__device__ __forceinline__ void load_window(const float* p, float (&in)[K + 3][K]) {
     constexpr int R = K / 2;
-    float v[K * K];
 #pragma unroll
-    for (int dy = 0; dy < K; ++dy)
+    for (int r = 0; r < K; ++r) {
+        const float4 a = *reinterpret_cast<const float4*>(p + r * PITCH);
+        const float4 b = *reinterpret_cast<const float4*>(p + r * PITCH + 4);
+        const float4 c = *reinterpret_cast<const float4*>(p + r * PITCH + 8);
+        const float v[12] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, c.x, c.y, c.z, c.w};
 #pragma unroll
-        for (int dx = 0; dx < K; ++dx) v[dy * K + dx] = sm[(r - R + dy) * PITCH + (c - R + dx)];
-    return median_forgetful<K * K>(v);
+        for (int cc = 0; cc < K + 3; ++cc) in[cc][r] = v[4 - R + cc];
+    }
+}
+
+template <int K>
+__device__ __forceinline__ void median_x4(const float (&in)[K + 3][K], float (&out)[4]);
+template <>
+__device__ __forceinline__ void median_x4<3>(const float (&in)[6][3], float (&out)[4]) { median3x3_x4(in, out); }
+template <>
+__device__ __forceinline__ void median_x4<5>(const float (&in)[8][5], float (&out)[4]) { median5x5_x4(in, out); }
+template <>
+__device__ __forceinline__ void median_x4<7>(const float (&in)[10][7], float (&out)[4]) { median7x7_x4(in, out); }
+
+__device__ __forceinline__ void store4(float* __restrict__ dst, size_t row_off, int x, int w,
+                                       const float (&v)[4]) {
+    if (x + 3 < w && ((row_off + x) & 3) == 0) {
+        *reinterpret_cast<float4*>(dst + row_off + x) = make_float4(v[0], v[1], v[2], v[3]);
+    } else {
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (x + j < w) dst[row_off + x + j] = v[j];
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
-// Standalone k x k median (lacosmic_medfilt; also the dense reference for the fused kernels).
+// Standalone k x k median (lacosmic_medfilt): same selection networks and tile shape as the fused
+// kernels.  Each thread produces 4 adjacent outputs from a (k+3) x k register window.
 template <int K>
 __global__ void __launch_bounds__(NT) k_medfilt(const float* __restrict__ in, float* __restrict__ out,
                                                int h, int w) {
-    constexpr int R = K / 2, PITCH = TW + 2 * R + 1;
-    __shared__ float sm[(TH + 2 * R) * PITCH];
-    const int tid = threadIdx.y * 32 + threadIdx.x;
+    constexpr int R = K / 2, MX = 4, PITCH = TW + 2 * MX;
+    __shared__ __align__(16) float sm[(TH + 2 * R) * PITCH];
+    const int tid = threadIdx.x, lane = tid & 31, wi = tid >> 5;
     const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
-    load_tile_clamped<TW, TH, R, PITCH, NT>(sm, in, h, w, y0, x0, tid);
+    load_tile<MX, R, PITCH>(sm, in, h, w, y0, x0, tid);
     __syncthreads();
 #pragma unroll 1
-    for (int j = 0; j < PY; ++j)
-#pragma unroll 1
-        for (int i = 0; i < PX; ++i) {
-            int ly = threadIdx.y + 8 * j, lx = threadIdx.x + 32 * i;
-            int y = y0 + ly, x = x0 + lx;
-            if (y < h && x < w) out[(size_t)y * w + x] = median_window<K, PITCH>(sm, ly + R, lx + R);
-        }
+    for (int ly = wi; ly < TH; ly += NWARP) {
+        int y = y0 + ly, x = x0 + 4 * lane;
+        if (y >= h || x >= w) continue;
+        float win[K + 3][K], o[4];
+        load_window<K, PITCH>(sm + ly * PITCH + 4 * lane, win);
+        median_x4<K>(win, o);
+        store4(out, (size_t)y * w, x, w, o);
+    }
 }
 
 // Standalone L+ (lacosmic_lplus).
 __global__ void __launch_bounds__(NT) k_lplus(const float* __restrict__ in, float* __restrict__ out,
                                              int h, int w) {
-    int x = blockIdx.x * 32 + threadIdx.x, y = blockIdx.y * 8 + threadIdx.y;
+    int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
     if (x >= w || y >= h) return;
     const float* row = in + (size_t)y * w;
     float c = row[x];
@@ -64,104 +103,313 @@ __global__ void __launch_bounds__(NT) k_lplus(const float* __restrict__ in, floa
 // ------------------------------------------------------------------------------------------------
 // K_A: steps (1)-(3a).  work -> L+ (recomputed later, not stored), N = sqrt(gain*med5+rn^2)/gain,
 // S = L+/(2N).  Writes S; Lp/N only when a debug plane is requested.
-__global__ void __launch_bounds__(NT)
-k_noise_S(const float* __restrict__ work, float* __restrict__ S, float* __restrict__ dbgLp,
-          float* __restrict__ dbgN, int h, int w, float gain, float rn2, const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;   // fixed point reached (R17)
-    constexpr int R = 2, PITCH = TW + 2 * R + 1;
-    __shared__ float sm[(TH + 2 * R) * PITCH];
-    const int tid = threadIdx.y * 32 + threadIdx.x;
-    const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
-    load_tile_clamped<TW, TH, R, PITCH, NT>(sm, work, h, w, y0, x0, tid);
-    __syncthreads();
+constexpr int NS_MX = 4, NS_MY = 2, NS_PITCH = TW + 2 * NS_MX, NS_ROWS = TH + 2 * NS_MY;
+
+struct NoiseArgs {
+    float* S;
+    float* dbgLp;
+    float* dbgN;
+    int h, w;
+    float gain, rn2;
+};
+
+// sm: work tile with margins (NS_MX, NS_MY), edge-replicated
+__device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a, int x0, int y0, int lane,
+                                             int wi) {
 #pragma unroll 1
-    for (int j = 0; j < PY; ++j)
-#pragma unroll 1
-        for (int i = 0; i < PX; ++i) {
-            int ly = threadIdx.y + 8 * j, lx = threadIdx.x + 32 * i;
-            int y = y0 + ly, x = x0 + lx;
-            if (y >= h || x >= w) continue;
-            int r = ly + R, c = lx + R;
-            float m5 = median_window<5, PITCH>(sm, r, c);
-            float lp = lplus_px(sm[r * PITCH + c], sm[(r - 1) * PITCH + c], sm[(r + 1) * PITCH + c],
-                                sm[r * PITCH + c - 1], sm[r * PITCH + c + 1]);
-            float m5c = m5 > 1e-4f ? m5 : 1e-4f;                                  // R5
-            float n = __fdiv_rn(__fsqrt_rn(__fadd_rn(__fmul_rn(gain, m5c), rn2)), gain);
-            float s = __fdiv_rn(lp, __fmul_rn(2.0f, n));
-            size_t p = (size_t)y * w + x;
-            S[p] = s;
-            if (dbgLp) dbgLp[p] = lp;
-            if (dbgN) dbgN[p] = n;
+    for (int ly = wi; ly < TH; ly += NWARP) {
+        int y = y0 + ly, x = x0 + 4 * lane;
+        if (y >= a.h || x >= a.w) continue;
+        float win[8][5], m5[4], s[4], lp[4], n[4];
+        load_window<5, NS_PITCH>(sm + ly * NS_PITCH + 4 * lane, win);
+        median5x5_x4(win, m5);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            lp[j] = lplus_px(win[2 + j][2], win[2 + j][1], win[2 + j][3], win[1 + j][2], win[3 + j][2]);
+            float m5c = m5[j] > 1e-4f ? m5[j] : 1e-4f;                                 // R5
+            n[j] = __fdiv_rn(__fsqrt_rn(__fadd_rn(__fmul_rn(a.gain, m5c), a.rn2)), a.gain);
+            s[j] = __fdiv_rn(lp[j], __fmul_rn(2.0f, n[j]));
         }
+        size_t ro = (size_t)y * a.w;
+        store4(a.S, ro, x, a.w, s);
+        if (a.dbgLp) store4(a.dbgLp, ro, x, a.w, lp);
+        if (a.dbgN) store4(a.dbgN, ro, x, a.w, n);
+    }
+}
+
+// generic path (any w): one tile per CTA, tile loaded with clamped scalar loads
+__global__ void __launch_bounds__(NT)
+k_noise_S(const float* __restrict__ work, NoiseArgs a, const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;   // fixed point reached (R17)
+    __shared__ __align__(16) float sm[NS_ROWS * NS_PITCH];
+    const int tid = threadIdx.x;
+    const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
+    load_tile<NS_MX, NS_MY, NS_PITCH>(sm, work, a.h, a.w, y0, x0, tid);
+    __syncthreads();
+    noise_S_tile(sm, a, x0, y0, tid & 31, tid >> 5);
+}
+
+// gather the 4-bit nibbles of the 8 lanes that share a 32-pixel word
+__device__ __forceinline__ uint32_t nibbles_to_word(uint32_t nib, int lane) {
+    uint32_t v = nib << ((lane & 7) * 4);
+    v |= __shfl_xor_sync(0xffffffffu, v, 1);
+    v |= __shfl_xor_sync(0xffffffffu, v, 2);
+    v |= __shfl_xor_sync(0xffffffffu, v, 4);
+    return v;
 }
 
 // K_B: steps (3b)-(5).  S' = S - med5(S); m3 = med3(work) (tile in shared memory, replicated at the
 // frame border as a STORED plane would be, R4); F = max(m3 - med7(m3), 0.01); gates -> bit-planes.
-__global__ void __launch_bounds__(NT)
-k_fine_gates(const float* __restrict__ work, const float* __restrict__ S, uint32_t* __restrict__ G1,
-             uint32_t* __restrict__ G2, uint32_t* __restrict__ M1, float* __restrict__ dbgSp,
-             float* __restrict__ dbgM3, float* __restrict__ dbgF, int h, int w, int wpr,
-             GateParams gp, const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;
-    constexpr int RA = 4, PA = TW + 2 * RA + 1;   // work tile, halo 4
-    constexpr int RB = 3, PB = TW + 2 * RB + 1;   // m3 tile, halo 3
-    constexpr int RS = 2, PS = TW + 2 * RS + 1;   // S tile, halo 2
-    __shared__ float smA[(TH + 2 * RA) * PA];
-    __shared__ float smB[(TH + 2 * RB) * PB];
-    __shared__ float smS[(TH + 2 * RS) * PS];
-    const int tid = threadIdx.y * 32 + threadIdx.x;
-    const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
-    load_tile_clamped<TW, TH, RA, PA, NT>(smA, work, h, w, y0, x0, tid);
-    load_tile_clamped<TW, TH, RS, PS, NT>(smS, S, h, w, y0, x0, tid);
-    __syncthreads();
-    {
-        constexpr int BW = TW + 2 * RB, BH = TH + 2 * RB;
-        for (int i = tid; i < BW * BH; i += NT) {
-            int r = i / BW, c = i - r * BW;
-            int cy = clampi(y0 - RB + r, 0, h - 1), cx = clampi(x0 - RB + c, 0, w - 1);
-            int ar = cy - (y0 - RA), ac = cx - (x0 - RA);
-            smB[r * PB + c] = median_window<3, PA>(smA, ar, ac);
-        }
+constexpr int FG_AX = 8, FG_AY = 4, FG_PA = TW + 2 * FG_AX, FG_AROWS = TH + 2 * FG_AY;   // work tile
+constexpr int FG_BX = 4, FG_BY = 3, FG_PB = TW + 2 * FG_BX, FG_BROWS = TH + 2 * FG_BY;   // m3 tile
+constexpr int FG_SX = 4, FG_SY = 2, FG_PS = TW + 2 * FG_SX, FG_SROWS = TH + 2 * FG_SY;   // S tile
+
+struct FineArgs {
+    uint32_t *G1, *G2, *M1;
+    float *dbgSp, *dbgM3, *dbgF;
+    int h, w, wpr;
+    GateParams gp;
+};
+
+// smA / smS: edge-replicated work / S tiles; smB: scratch for the m3 tile.  Contains block barriers.
+__device__ __forceinline__ void fine_gates_tile(const float* smA, float* smB, const float* smS,
+                                                const FineArgs& a, int x0, int y0, int tid) {
+    constexpr int PA = FG_PA, PB = FG_PB, PS = FG_PS, BX = FG_BX, BY = FG_BY, AY = FG_AY;
+    constexpr int BH = FG_BROWS, BG = PB / 4;
+    const int lane = tid & 31, wi = tid >> 5;
+    const int h = a.h, w = a.w;
+    // m3 tile: B[r][4g..4g+3] = med3 at frame rows y0-3+r, columns x0-4+4g .. +3
+    for (int i = tid; i < BH * BG; i += NT) {
+        int r = i / BG, g = i - r * BG;
+        float win[6][3], o[4];
+        load_window<3, PA>(smA + r * PA + 4 * g, win);
+        median3x3_x4(win, o);
+        *reinterpret_cast<float4*>(smB + r * PB + 4 * g) = make_float4(o[0], o[1], o[2], o[3]);
     }
     __syncthreads();
-#pragma unroll 1
-    for (int j = 0; j < PY; ++j)
-#pragma unroll 1
-        for (int i = 0; i < PX; ++i) {
-            int ly = threadIdx.y + 8 * j, lx = threadIdx.x + 32 * i;
-            int y = y0 + ly, x = x0 + lx;
-            bool inside = (y < h) && (x < w);
-            bool g1 = false, g2 = false, m1 = false;
-            if (inside) {
-                float s = smS[(ly + RS) * PS + lx + RS];
-                float sp = __fsub_rn(s, median_window<5, PS>(smS, ly + RS, lx + RS));
-                float m3 = smB[(ly + RB) * PB + lx + RB];
-                float f = __fsub_rn(m3, median_window<7, PB>(smB, ly + RB, lx + RB));
-                f = f > 0.01f ? f : 0.01f;
-                int r = ly + RA, c = lx + RA;
-                float ctr = smA[r * PA + c];
-                float lp = lplus_px(ctr, smA[(r - 1) * PA + c], smA[(r + 1) * PA + c],
-                                    smA[r * PA + c - 1], smA[r * PA + c + 1]);
-                bool ok = ctr < gp.satlevel;                                  // R12
-                g1 = ok && (sp > gp.sigclip);
-                g2 = ok && (sp > gp.siglow);
-                m1 = g1 && (__fdiv_rn(lp, f) > gp.objlim);                    // R8
-                size_t p = (size_t)y * w + x;
-                if (dbgSp) dbgSp[p] = sp;
-                if (dbgM3) dbgM3[p] = m3;
-                if (dbgF) dbgF[p] = f;
-            }
-            uint32_t b1 = __ballot_sync(0xffffffffu, g1);
-            uint32_t b2 = __ballot_sync(0xffffffffu, g2);
-            uint32_t b3 = __ballot_sync(0xffffffffu, m1);
-            int wx = (x0 >> 5) + i;
-            if (threadIdx.x == 0 && y < h && wx < wpr) {
-                size_t q = (size_t)y * wpr + wx;
-                G1[q] = b1;
-                G2[q] = b2;
-                M1[q] = b3;
+    // R4: positions outside the frame take the value of the stored plane's edge, not a median evaluated
+    // at virtual coordinates.  Only tiles that touch the frame border have such positions.
+    if (y0 - BY < 0 || y0 + TH + BY > h || x0 - BX < 0 || x0 + TW + BX > w) {
+        constexpr int NFIX = (BH * PB + NT - 1) / NT;
+        float fix[NFIX];
+#pragma unroll
+        for (int q = 0; q < NFIX; ++q) {
+            int i = tid + q * NT;
+            if (i < BH * PB) {
+                int r = i / PB, c = i - r * PB;
+                int cr = clampi(y0 - BY + r, 0, h - 1) - (y0 - BY);
+                int cc = clampi(x0 - BX + c, 0, w - 1) - (x0 - BX);
+                fix[q] = smB[cr * PB + cc];
             }
         }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < NFIX; ++q) {
+            int i = tid + q * NT;
+            if (i < BH * PB) smB[i] = fix[q];
+        }
+        __syncthreads();
+    }
+#pragma unroll 1
+    for (int ly = wi; ly < TH; ly += NWARP) {
+        const int y = y0 + ly, x = x0 + 4 * lane;
+        uint32_t n1 = 0, n2 = 0, n3 = 0;
+        if (y < h && x < w) {
+            float sp[4], f[4], m3[4];
+            {
+                float win[8][5], mS[4];
+                load_window<5, PS>(smS + ly * PS + 4 * lane, win);
+                median5x5_x4(win, mS);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) sp[j] = __fsub_rn(win[2 + j][2], mS[j]);
+            }
+            {
+                float win[10][7], m7[4];
+                load_window<7, PB>(smB + ly * PB + 4 * lane, win);
+                median7x7_x4(win, m7);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    m3[j] = win[3 + j][3];
+                    float d = __fsub_rn(m3[j], m7[j]);
+                    f[j] = d > 0.01f ? d : 0.01f;
+                }
+            }
+            const float* ac = smA + (ly + AY) * PA + 4 * lane + 4;      // columns x-4 .. x+7 of row y
+            const float4 c0 = *reinterpret_cast<const float4*>(ac);
+            const float4 c1 = *reinterpret_cast<const float4*>(ac + 4);
+            const float4 c2 = *reinterpret_cast<const float4*>(ac + 8);
+            const float4 up = *reinterpret_cast<const float4*>(ac - PA + 4);
+            const float4 dn = *reinterpret_cast<const float4*>(ac + PA + 4);
+            const float ctr[6] = {c0.w, c1.x, c1.y, c1.z, c1.w, c2.x};
+            const float u[4] = {up.x, up.y, up.z, up.w}, d4[4] = {dn.x, dn.y, dn.z, dn.w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                float lp = lplus_px(ctr[1 + j], u[j], d4[j], ctr[j], ctr[2 + j]);
+                bool ok = (x + j < w) && (ctr[1 + j] < a.gp.satlevel);            // R12
+                bool g1 = ok && (sp[j] > a.gp.sigclip);
+                bool g2 = ok && (sp[j] > a.gp.siglow);
+                bool m1 = g1 && (__fdiv_rn(lp, f[j]) > a.gp.objlim);               // R8
+                n1 |= (uint32_t)g1 << j;
+                n2 |= (uint32_t)g2 << j;
+                n3 |= (uint32_t)m1 << j;
+            }
+            size_t ro = (size_t)y * w;
+            if (a.dbgSp) store4(a.dbgSp, ro, x, w, sp);
+            if (a.dbgM3) store4(a.dbgM3, ro, x, w, m3);
+            if (a.dbgF) store4(a.dbgF, ro, x, w, f);
+        }
+        uint32_t b1 = nibbles_to_word(n1, lane), b2 = nibbles_to_word(n2, lane), b3 = nibbles_to_word(n3, lane);
+        int wx = (x0 >> 5) + (lane >> 3);
+        if ((lane & 7) == 0 && y < h && wx < a.wpr) {
+            size_t q = (size_t)y * a.wpr + wx;
+            a.G1[q] = b1;
+            a.G2[q] = b2;
+            a.M1[q] = b3;
+        }
+    }
+}
+
+// generic path (any w): one tile per CTA, tiles loaded with clamped scalar loads
+__global__ void __launch_bounds__(NT)
+k_fine_gates(const float* __restrict__ work, const float* __restrict__ S, FineArgs a,
+             const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;
+    __shared__ __align__(16) float smA[FG_AROWS * FG_PA];
+    __shared__ __align__(16) float smB[FG_BROWS * FG_PB];
+    __shared__ __align__(16) float smS[FG_SROWS * FG_PS];
+    const int tid = threadIdx.x;
+    const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
+    load_tile<FG_AX, FG_AY, FG_PA>(smA, work, a.h, a.w, y0, x0, tid);
+    load_tile<FG_SX, FG_SY, FG_PS>(smS, S, a.h, a.w, y0, x0, tid);
+    __syncthreads();
+    fine_gates_tile(smA, smB, smS, a, x0, y0, tid);
+}
+
+// ------------------------------------------------------------------------------------------------
+// TMA path (w % 4 == 0): persistent CTAs, each walking tiles t = blockIdx.x, +gridDim.x, ... with a
+// two-stage pipeline: one elected thread issues cp.async.bulk.tensor loads of the NEXT tile's boxes
+// while all warps run the selection networks on the current one.  TMA fills out-of-frame elements
+// with zeros; tiles touching the frame border repair them in shared memory to edge-replicate (R3).
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int cx, int cy, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(cx), "r"(cy), "r"(smem_u32(bar)) : "memory");
+}
+
+// repair a TMA-loaded tile (zeros outside the frame) to edge-replicate; tile origin (ox, oy) in frame coords
+template <int ROWS, int PITCH>
+__device__ __forceinline__ void replicate_fix(float* sm, int oy, int ox, int h, int w, int tid) {
+    for (int i = tid; i < ROWS * PITCH; i += NT) {
+        int r = i / PITCH, c = i - r * PITCH;
+        int yy = oy + r, xx = ox + c;
+        if (yy < 0 || yy >= h || xx < 0 || xx >= w)
+            sm[i] = sm[(clampi(yy, 0, h - 1) - oy) * PITCH + (clampi(xx, 0, w - 1) - ox)];
+    }
+}
+
+__global__ void __launch_bounds__(NT)
+k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx, int ntiles,
+              const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int TILE_BYTES = NS_ROWS * NS_PITCH * 4;
+    auto buf = [&](int st) { return reinterpret_cast<float*>(smem_raw + st * TILE_BYTES); };
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + 2 * TILE_BYTES);
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        fence_mbar_init();
+    }
+    __syncthreads();
+    auto issue = [&](int t, int st) {
+        int ty = t / ntx, tx = t - ty * ntx;
+        mbar_expect_tx(&full[st], TILE_BYTES);
+        tma_load_2d(buf(st), &mapWork, tx * TW - NS_MX, ty * TH - NS_MY, &full[st]);
+    };
+    int t = blockIdx.x;
+    if (tid == 0 && t < ntiles) issue(t, 0);
+    for (int it = 0; t < ntiles; t += gridDim.x, ++it) {
+        const int st = it & 1;
+        if (tid == 0 && t + (int)gridDim.x < ntiles) issue(t + gridDim.x, st ^ 1);
+        mbar_wait(&full[st], (it >> 1) & 1);
+        const int ty = t / ntx, tx = t - ty * ntx;
+        const int x0 = tx * TW, y0 = ty * TH;
+        if (y0 - NS_MY < 0 || y0 + TH + NS_MY > a.h || x0 - NS_MX < 0 || x0 + TW + NS_MX > a.w) {
+            replicate_fix<NS_ROWS, NS_PITCH>(buf(st), y0 - NS_MY, x0 - NS_MX, a.h, a.w, tid);
+            fence_proxy_async();
+            __syncthreads();
+        }
+        noise_S_tile(buf(st), a, x0, y0, tid & 31, tid >> 5);
+        __syncthreads();   // stage st is free for the load issued at the top of the next iteration
+    }
+}
+
+constexpr int FG_A_BYTES = FG_AROWS * FG_PA * 4, FG_S_BYTES = FG_SROWS * FG_PS * 4,
+              FG_B_BYTES = FG_BROWS * FG_PB * 4;
+constexpr int FG_SMEM_BYTES = 2 * FG_A_BYTES + 2 * FG_S_BYTES + FG_B_BYTES + 16;
+constexpr int NS_SMEM_BYTES = 2 * NS_ROWS * NS_PITCH * 4 + 16;
+static_assert(FG_A_BYTES % 128 == 0 && FG_S_BYTES % 128 == 0, "TMA destinations must stay 128-byte aligned");
+static_assert((NS_ROWS * NS_PITCH * 4) % 128 == 0, "TMA destinations must stay 128-byte aligned");
+
+__global__ void __launch_bounds__(NT)
+k_fine_gates_tma(const __grid_constant__ CUtensorMap mapWork, const __grid_constant__ CUtensorMap mapS,
+                 FineArgs a, int ntx, int ntiles, const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    auto bufA = [&](int st) { return reinterpret_cast<float*>(smem_raw + st * FG_A_BYTES); };
+    auto bufS = [&](int st) { return reinterpret_cast<float*>(smem_raw + 2 * FG_A_BYTES + st * FG_S_BYTES); };
+    float* smB = reinterpret_cast<float*>(smem_raw + 2 * FG_A_BYTES + 2 * FG_S_BYTES);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + 2 * FG_A_BYTES + 2 * FG_S_BYTES + FG_B_BYTES);
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        fence_mbar_init();
+    }
+    __syncthreads();
+    auto issue = [&](int t, int st) {
+        int ty = t / ntx, tx = t - ty * ntx;
+        mbar_expect_tx(&full[st], FG_A_BYTES + FG_S_BYTES);
+        tma_load_2d(bufA(st), &mapWork, tx * TW - FG_AX, ty * TH - FG_AY, &full[st]);
+        tma_load_2d(bufS(st), &mapS, tx * TW - FG_SX, ty * TH - FG_SY, &full[st]);
+    };
+    int t = blockIdx.x;
+    if (tid == 0 && t < ntiles) issue(t, 0);
+    for (int it = 0; t < ntiles; t += gridDim.x, ++it) {
+        const int st = it & 1;
+        if (tid == 0 && t + (int)gridDim.x < ntiles) issue(t + gridDim.x, st ^ 1);
+        mbar_wait(&full[st], (it >> 1) & 1);
+        const int ty = t / ntx, tx = t - ty * ntx;
+        const int x0 = tx * TW, y0 = ty * TH;
+        if (y0 - FG_AY < 0 || y0 + TH + FG_AY > a.h || x0 - FG_AX < 0 || x0 + TW + FG_AX > a.w) {
+            replicate_fix<FG_AROWS, FG_PA>(bufA(st), y0 - FG_AY, x0 - FG_AX, a.h, a.w, tid);
+            replicate_fix<FG_SROWS, FG_PS>(bufS(st), y0 - FG_SY, x0 - FG_SX, a.h, a.w, tid);
+            fence_proxy_async();
+            __syncthreads();
+        }
+        fine_gates_tile(bufA(st), smB, bufS(st), a, x0, y0, tid);
+        __syncthreads();   // stage st and smB are free again
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -170,8 +418,8 @@ k_fine_gates(const float* __restrict__ work, const float* __restrict__ S, uint32
 // them).  If Cio is given: count += popc(out & ~C); C |= out  (R11).
 __global__ void __launch_bounds__(256)
 k_dilate_gate(const uint32_t* __restrict__ in, const uint32_t* __restrict__ gate,
-              uint32_t* __restrict__ out, uint32_t* __restrict__ Cio, int* __restrict__ count, int h,
-              int w, int wpr, const int* prev_count) {
+              uint32_t* __restrict__ out, uint32_t* __restrict__ Cio, uint32_t* __restrict__ newp,
+              int* __restrict__ count, int h, int w, int wpr, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     const int lane = threadIdx.x & 31;
     int wx = blockIdx.x * 32 + lane;
@@ -215,8 +463,10 @@ k_dilate_gate(const uint32_t* __restrict__ in, const uint32_t* __restrict__ gate
         int n = 0;
         if (valid) {
             uint32_t c = Cio[(size_t)y * wpr + wx];
-            n = __popc(res & ~c);
-            if (res & ~c) Cio[(size_t)y * wpr + wx] = c | res;
+            uint32_t fresh = res & ~c;
+            n = __popc(fresh);
+            if (fresh) Cio[(size_t)y * wpr + wx] = c | res;
+            newp[(size_t)y * wpr + wx] = fresh;      // pixels first flagged in this iteration
         }
         n = __reduce_add_sync(0xffffffffu, n);
         if (lane == 0 && n) atomicAdd(count, n);
@@ -224,58 +474,104 @@ k_dilate_gate(const uint32_t* __restrict__ in, const uint32_t* __restrict__ gate
 }
 
 // ------------------------------------------------------------------------------------------------
-// Step (7): sparse masked-median replacement.  A warp owns 32 consecutive words of the cumulative
-// mask C; the non-empty words are found by ballot and their set bits walked one pixel at a time.
-// For a pixel the 25 taps sit on lanes 0..24; each lane ranks its tap among the donors by 25
-// shuffles (ties broken by lane so ranks are a permutation), and the lanes holding the middle
-// rank(s) supply the median (R13-R16).  Reads only img_in and C, writes only work.
+// Step (7): sparse masked-median replacement over a warp-compacted CR list.
+//
+// work[p] for p in C is a pure function of img_in and of C inside p's 5x5 window (R13), so after an
+// iteration only the pixels of C that have a NEWLY flagged pixel in their window need (re)computing;
+// all others already hold the right value.  k_build_list compacts exactly those pixels:
+//   need = dil5x5(newp) & C,   one thread per 32-pixel word, warp-aggregated append (one atomic per warp)
+// and k_replace_list gives each listed pixel to one thread: 25 clamped taps -> +inf where the tap's
+// pixel is in C -> 25-input sorting network -> middle element(s) of the k donors (R14-R16).
 __global__ void __launch_bounds__(256)
-k_replace(const float* __restrict__ img, const uint32_t* __restrict__ Cb, float* __restrict__ work,
-          int h, int w, int wpr, const int* prev_count) {
+k_build_list(const uint32_t* __restrict__ newp, const uint32_t* __restrict__ Cb, int* __restrict__ list,
+             int* __restrict__ nlist, int h, int w, int wpr, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     const int lane = threadIdx.x & 31;
-    const long long nwords = (long long)h * wpr;
-    long long base = ((long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32;
-    if (base >= nwords) return;
-    long long mine = base + lane;
-    uint32_t cw = mine < nwords ? Cb[mine] : 0u;
-    uint32_t nz = __ballot_sync(0xffffffffu, cw != 0u);
-    const int dy = lane / 5 - 2, dx = lane % 5 - 2;   // lanes >= 25 idle in the vote
-    while (nz) {
-        int src = __ffs(nz) - 1;
-        nz &= nz - 1;
-        uint32_t word = __shfl_sync(0xffffffffu, cw, src);
-        long long idx = base + src;
-        int y = (int)(idx / wpr), wx = (int)(idx - (long long)y * wpr);
-        while (word) {
-            int b = __ffs(word) - 1;
-            word &= word - 1;
-            int x = wx * 32 + b;
-            float val = 0.0f;
-            bool donor = false;
-            if (lane < 25) {
-                int yy = clampi(y + dy, 0, h - 1), xx = clampi(x + dx, 0, w - 1);
-                val = __ldg(img + (size_t)yy * w + xx);
-                donor = !((Cb[(size_t)yy * wpr + (xx >> 5)] >> (xx & 31)) & 1u);
+    const int wx = blockIdx.x * 32 + lane;
+    const int y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    uint32_t need = 0;
+    if (wx < wpr && y < h) {
+        const uint32_t c = Cb[(size_t)y * wpr + wx];
+        if (c) {
+            uint32_t vl = 0, vc = 0, vr = 0;
+            for (int yy = max(y - 2, 0); yy <= min(y + 2, h - 1); ++yy) {
+                const uint32_t* row = newp + (size_t)yy * wpr;
+                vc |= row[wx];
+                if (wx > 0) vl |= row[wx - 1];
+                if (wx + 1 < wpr) vr |= row[wx + 1];
             }
-            uint32_t dm = __ballot_sync(0xffffffffu, donor);
-            if (dm == 0u) dm = 0x01ffffffu;            // R15: no donor -> all 25 taps
-            const int k = __popc(dm);
-            int rank = 0;
-#pragma unroll
-            for (int t = 0; t < 25; ++t) {
-                float vt = __shfl_sync(0xffffffffu, val, t);
-                bool before = (vt < val) || (vt == val && t < lane);
-                rank += (((dm >> t) & 1u) && before) ? 1 : 0;
-            }
-            bool mineIn = (dm >> lane) & 1u;
-            uint32_t hiM = __ballot_sync(0xffffffffu, mineIn && rank == (k >> 1));
-            uint32_t loM = __ballot_sync(0xffffffffu, mineIn && rank == (k >> 1) - 1);
-            float hi = __shfl_sync(0xffffffffu, val, __ffs(hiM) - 1);
-            float lo = __shfl_sync(0xffffffffu, val, (k & 1) ? 0 : __ffs(loM) - 1);
-            float r = (k & 1) ? hi : __fmul_rn(__fadd_rn(lo, hi), 0.5f);   // R14
-            if (lane == 0) work[(size_t)y * w + x] = r;
+            uint32_t spread = vc | (vc << 1) | (vc << 2) | (vc >> 1) | (vc >> 2) | (vl >> 31) | (vl >> 30) |
+                              (vr << 31) | (vr << 30);
+            need = spread & c;
         }
+    }
+    int n = __popc(need), incl = n;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        int o = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += o;
+    }
+    int total = __shfl_sync(0xffffffffu, incl, 31);
+    if (total == 0) return;
+    int base = 0;
+    if (lane == 31) base = atomicAdd(nlist, total);
+    base = __shfl_sync(0xffffffffu, base, 31) + incl - n;
+    const int p0 = y * w + wx * 32;
+    while (need) {
+        int b = __ffs(need) - 1;
+        need &= need - 1;
+        list[base++] = p0 + b;
+    }
+}
+
+__global__ void __launch_bounds__(128)
+k_replace_list(const float* __restrict__ img, const uint32_t* __restrict__ Cb, float* __restrict__ work,
+               const int* __restrict__ list, const int* __restrict__ nlist, int h, int w, int wpr,
+               const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;
+    const int n = *nlist;
+    const float INF = __int_as_float(0x7f800000);
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const int p = list[i];
+        const int y = p / w, x = p - y * w;
+        int xx[5], yy[5];
+#pragma unroll
+        for (int d = 0; d < 5; ++d) {
+            xx[d] = clampi(x + d - 2, 0, w - 1);
+            yy[d] = clampi(y + d - 2, 0, h - 1);
+        }
+        // donor mask: bit (5*dy + dx) set when the (clamped) tap is NOT in C
+        uint32_t donors = 0;
+#pragma unroll
+        for (int dy = 0; dy < 5; ++dy) {
+            const uint32_t* row = Cb + (size_t)yy[dy] * wpr;
+            const int wl = xx[0] >> 5, wr = xx[4] >> 5;
+            const uint32_t cl = row[wl], cr = row[wr];
+#pragma unroll
+            for (int dx = 0; dx < 5; ++dx) {
+                uint32_t word = (xx[dx] >> 5) == wl ? cl : cr;
+                donors |= (((word >> (xx[dx] & 31)) & 1u) ^ 1u) << (5 * dy + dx);
+            }
+        }
+        if (donors == 0u) donors = 0x01ffffffu;            // R15: no donor -> all 25 taps
+        const int k = __popc(donors);
+        float v[25], s[25];
+#pragma unroll
+        for (int dy = 0; dy < 5; ++dy)
+#pragma unroll
+            for (int dx = 0; dx < 5; ++dx) {
+                float t = __ldg(img + (size_t)yy[dy] * w + xx[dx]);
+                v[5 * dy + dx] = ((donors >> (5 * dy + dx)) & 1u) ? t : INF;
+            }
+        sort25(v, s);
+        const int ihi = k >> 1, ilo = (k - 1) >> 1;
+        float lo = s[0], hi = s[0];
+#pragma unroll
+        for (int q = 1; q < 25; ++q) {
+            lo = (q == ilo) ? s[q] : lo;
+            hi = (q == ihi) ? s[q] : hi;
+        }
+        work[p] = (k & 1) ? hi : __fmul_rn(__fadd_rn(lo, hi), 0.5f);   // R14
     }
 }
 

@@ -2,6 +2,7 @@
 // See include/lacosmic.h for the contract of every entry point.
 #include "../../include/lacosmic.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstring>
 
@@ -50,6 +51,64 @@ struct Span {   // records an event pair around one launch when timing is enable
     }
 };
 
+// ---- TMA descriptors and persistent-grid sizing -------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = []() -> EncodeTiledFn {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            return nullptr;
+        return (EncodeTiledFn)p;
+    }();
+    return fn;
+}
+
+// 2-D map over a row-major fp32 [h][w] plane (w % 4 == 0), box = boxW x boxH elements, zero fill
+// outside; elements are moved as raw 32-bit words.
+bool make_map(CUtensorMap* m, const float* base, int h, int w, int boxW, int boxH) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return false;
+    cuuint64_t dims[2] = {(cuuint64_t)w, (cuuint64_t)h};
+    cuuint64_t strides[1] = {(cuuint64_t)w * 4};
+    cuuint32_t box[2] = {(cuuint32_t)boxW, (cuuint32_t)boxH};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, (void*)base, dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+struct DeviceInfo {
+    int sms = 0, occ_noise = 0, occ_fine = 0;
+    bool ok = false;
+};
+
+const DeviceInfo& device_info() {
+    static DeviceInfo info = []() {
+        DeviceInfo d;
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return d;
+        if (cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return d;
+        if (cudaFuncSetAttribute(lac::k_fine_gates_tma, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 lac::FG_SMEM_BYTES) != cudaSuccess) return d;
+        if (cudaFuncSetAttribute(lac::k_noise_S_tma, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 lac::NS_SMEM_BYTES) != cudaSuccess) return d;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_fine, lac::k_fine_gates_tma, lac::NT,
+                                                          lac::FG_SMEM_BYTES) != cudaSuccess) return d;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_noise, lac::k_noise_S_tma, lac::NT,
+                                                          lac::NS_SMEM_BYTES) != cudaSuccess) return d;
+        d.ok = d.sms > 0 && d.occ_fine > 0 && d.occ_noise > 0;
+        return d;
+    }();
+    return info;
+}
+
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 inline int words_per_row(int w) { return (w + 31) / 32; }
 
@@ -77,8 +136,10 @@ inline bool overlap(const void* a, size_t na, const void* b, size_t nb) {
 // Workspace layout (all offsets 256-byte aligned)
 struct Workspace {
     float* S;
-    uint32_t *G1, *G2, *M1, *M2, *M3, *C;
-    int32_t* counts;   // LACOSMIC_MAX_NITER ints
+    uint32_t *G1, *G2, *M1, *M2, *M3, *C, *NEWP;
+    int32_t* counts;   // LACOSMIC_MAX_NITER new-pixel counts, then LACOSMIC_MAX_NITER list lengths
+    int32_t* nlist;
+    int32_t* list;     // compacted pixel list; aliases the S plane (dead once the gates are written)
     size_t bytes;
 };
 
@@ -95,7 +156,10 @@ Workspace carve(void* base, int h, int w) {
     ws.M2 = (uint32_t*)(p + off); off += bp;
     ws.M3 = (uint32_t*)(p + off); off += bp;
     ws.C = (uint32_t*)(p + off); off += bp;
-    ws.counts = (int32_t*)(p + off); off += align_up(LACOSMIC_MAX_NITER * 4, 256);
+    ws.NEWP = (uint32_t*)(p + off); off += bp;
+    ws.counts = (int32_t*)(p + off); off += align_up(2 * LACOSMIC_MAX_NITER * 4, 256);
+    ws.nlist = ws.counts + LACOSMIC_MAX_NITER;
+    ws.list = (int32_t*)ws.S;
     ws.bytes = off;
     return ws;
 }
@@ -108,12 +172,19 @@ int unpack(const uint32_t* bits, uint8_t* u8, int h, int w, cudaStream_t st) {
     return LACOSMIC_OK;
 }
 
-int replace_pass(const float* img, const uint32_t* C, float* work, int h, int w, const int* prev,
-                 cudaStream_t st) {
-    long long nwords = (long long)h * words_per_row(w);
-    unsigned blocks = (unsigned)((nwords + 255) / 256);
+// (re)compute work at every pixel of C whose 5x5 window holds a pixel of `newp`
+int replace_pass(const float* img, const Workspace& ws, const uint32_t* newp, int* nlist, float* work,
+                 int h, int w, const int* prev, cudaStream_t st) {
+    const int wpr = words_per_row(w);
+    dim3 dg((wpr + 31) / 32, (h + 7) / 8);
     Span sp(KC_REPLACE, st);
-    lac::k_replace<<<blocks, 256, 0, st>>>(img, C, work, h, w, words_per_row(w), prev);
+    lac::k_build_list<<<dg, 256, 0, st>>>(newp, ws.C, ws.list, nlist, h, w, wpr, prev);
+    LAUNCHED();
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    long long want = ((long long)h * w / 64 + 127) / 128;      // enough threads for a 1.6 % mask
+    int blocks = (int)std::max(1LL, std::min((long long)sms * 16, want));
+    lac::k_replace_list<<<blocks, 128, 0, st>>>(img, ws.C, work, ws.list, nlist, h, w, wpr, prev);
     LAUNCHED();
     return LACOSMIC_OK;
 }
@@ -130,41 +201,61 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     // O0
     CK(cudaMemcpyAsync(work, img, P * 4, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemsetAsync(ws.C, 0, bp_bytes, st));
-    CK(cudaMemsetAsync(ws.counts, 0, LACOSMIC_MAX_NITER * 4, st));
+    CK(cudaMemsetAsync(ws.counts, 0, 2 * LACOSMIC_MAX_NITER * 4, st));
     const float siglow = p.sigfrac * p.sigclip;   // R9: one fp32 multiply on the host
     const float rn2 = p.readnoise * p.readnoise;
     lac::GateParams gp{p.sigclip, siglow, p.objlim, p.satlevel};
-    dim3 tb(32, 8), tg((w + lac::TW - 1) / lac::TW, (h + lac::TH - 1) / lac::TH);
+    dim3 tb(lac::NT), tg((w + lac::TW - 1) / lac::TW, (h + lac::TH - 1) / lac::TH);
     dim3 dg((wpr + 31) / 32, (h + 7) / 8);
+    // TMA path needs 16-byte row pitch; other widths take the generic tile loader
+    const bool tma = (w % 4 == 0);
+    const int ntx = (int)tg.x, ntiles = (int)(tg.x * tg.y);
+    CUtensorMap mapWorkNS, mapWorkFG, mapS;
+    int gridNS = 0, gridFG = 0;
+    if (tma && p.niter > 0) {
+        const DeviceInfo& di = device_info();
+        if (!di.ok) { g_last_cuda_error = (int)cudaGetLastError(); return LACOSMIC_ERR_CUDA; }
+        if (!make_map(&mapWorkNS, work, h, w, lac::NS_PITCH, lac::NS_ROWS) ||
+            !make_map(&mapWorkFG, work, h, w, lac::FG_PA, lac::FG_AROWS) ||
+            !make_map(&mapS, ws.S, h, w, lac::FG_PS, lac::FG_SROWS)) {
+            g_last_cuda_error = (int)cudaErrorInvalidValue;
+            return LACOSMIC_ERR_CUDA;
+        }
+        gridNS = std::min(ntiles, di.sms * di.occ_noise);
+        gridFG = std::min(ntiles, di.sms * di.occ_fine);
+    }
     for (int t = 0; t < p.niter; ++t) {
         const int* prev = t > 0 ? ws.counts + (t - 1) : nullptr;
         const bool d = dbg && dbg->iter == t;
+        lac::NoiseArgs na{ws.S, d ? dbg->Lp : nullptr, d ? dbg->N : nullptr, h, w, p.gain, rn2};
+        lac::FineArgs fa{ws.G1, ws.G2, ws.M1, d ? dbg->Sp : nullptr, d ? dbg->m3 : nullptr,
+                         d ? dbg->F : nullptr, h, w, wpr, gp};
         {
             Span sp(KC_NOISE_S, st);
-            lac::k_noise_S<<<tg, tb, 0, st>>>(work, ws.S, d ? dbg->Lp : nullptr, d ? dbg->N : nullptr,
-                                             h, w, p.gain, rn2, prev);
+            if (tma) lac::k_noise_S_tma<<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(mapWorkNS, na, ntx, ntiles, prev);
+            else lac::k_noise_S<<<tg, tb, 0, st>>>(work, na, prev);
             LAUNCHED();
         }
         {
             Span sp(KC_FINE_GATES, st);
-            lac::k_fine_gates<<<tg, tb, 0, st>>>(work, ws.S, ws.G1, ws.G2, ws.M1,
-                                                d ? dbg->Sp : nullptr, d ? dbg->m3 : nullptr,
-                                                d ? dbg->F : nullptr, h, w, wpr, gp, prev);
+            if (tma) lac::k_fine_gates_tma<<<gridFG, tb, lac::FG_SMEM_BYTES, st>>>(mapWorkFG, mapS, fa, ntx, ntiles, prev);
+            else lac::k_fine_gates<<<tg, tb, 0, st>>>(work, ws.S, fa, prev);
             LAUNCHED();
         }
         {
             Span sp(KC_DILATE, st);
-            lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M1, ws.G1, ws.M2, nullptr, nullptr, h, w, wpr,
-                                                  prev);
+            lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M1, ws.G1, ws.M2, nullptr, nullptr, nullptr, h, w,
+                                                  wpr, prev);
             LAUNCHED();
-            lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M2, ws.G2, ws.M3, ws.C, ws.counts + t, h, w, wpr,
-                                                  prev);
+            lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M2, ws.G2, ws.M3, ws.C, ws.NEWP, ws.counts + t, h, w,
+                                                  wpr, prev);
             LAUNCHED();
         }
-        int rc = replace_pass(img, ws.C, work, h, w, prev, st);
+        // the S plane is dead from here on; its storage becomes the compacted pixel list
+        if (d && dbg->S) CK(cudaMemcpyAsync(dbg->S, ws.S, P * 4, cudaMemcpyDeviceToDevice, st));
+        int rc = replace_pass(img, ws, ws.NEWP, ws.nlist + t, work, h, w, prev, st);
         if (rc) return rc;
         if (d) {
-            if (dbg->S) CK(cudaMemcpyAsync(dbg->S, ws.S, P * 4, cudaMemcpyDeviceToDevice, st));
             struct { const uint32_t* b; uint8_t* o; } planes[] = {
                 {ws.G1, dbg->G1}, {ws.G2, dbg->G2}, {ws.M1, dbg->M1},
                 {ws.M2, dbg->M2}, {ws.M3, dbg->M3}, {ws.C, dbg->C}};
@@ -307,7 +398,7 @@ int lacosmic_lplus(const float* in, float* out, int h, int w, void* stream) {
     int rc = check_shape(h, w);
     if (rc) return rc;
     if (overlap(in, (size_t)h * w * 4, out, (size_t)h * w * 4)) return LACOSMIC_ERR_ALIAS;
-    dim3 g((w + 31) / 32, (h + 7) / 8), b(32, 8);
+    dim3 g((w + 31) / 32, (h + 7) / 8), b(256);
     lac::k_lplus<<<g, b, 0, (cudaStream_t)stream>>>(in, out, h, w);
     LAUNCHED();
     return LACOSMIC_OK;
@@ -319,7 +410,7 @@ int lacosmic_medfilt(const float* in, float* out, int h, int w, int k, void* str
     if (rc) return rc;
     if (k != 3 && k != 5 && k != 7) return LACOSMIC_ERR_PARAM;
     if (overlap(in, (size_t)h * w * 4, out, (size_t)h * w * 4)) return LACOSMIC_ERR_ALIAS;
-    dim3 tb(32, 8), tg((w + lac::TW - 1) / lac::TW, (h + lac::TH - 1) / lac::TH);
+    dim3 tb(lac::NT), tg((w + lac::TW - 1) / lac::TW, (h + lac::TH - 1) / lac::TH);
     cudaStream_t st = (cudaStream_t)stream;
     if (k == 3) lac::k_medfilt<3><<<tg, tb, 0, st>>>(in, out, h, w);
     else if (k == 5) lac::k_medfilt<5><<<tg, tb, 0, st>>>(in, out, h, w);
@@ -355,7 +446,7 @@ int lacosmic_dilate3(const uint32_t* bits_in, uint32_t* bits_out, int h, int w, 
     if (overlap(bits_in, (size_t)h * wpr * 4, bits_out, (size_t)h * wpr * 4)) return LACOSMIC_ERR_ALIAS;
     dim3 dg((wpr + 31) / 32, (h + 7) / 8);
     lac::k_dilate_gate<<<dg, 256, 0, (cudaStream_t)stream>>>(bits_in, nullptr, bits_out, nullptr, nullptr,
-                                                           h, w, wpr, nullptr);
+                                                           nullptr, h, w, wpr, nullptr);
     LAUNCHED();
     return LACOSMIC_OK;
 }
@@ -373,7 +464,8 @@ int lacosmic_masked_median(const float* img, const uint8_t* mask_u8, float* out,
     cudaStream_t st = (cudaStream_t)stream;
     if ((rc = lacosmic_pack_bits(mask_u8, ws.C, h, w, stream))) return rc;
     CK(cudaMemcpyAsync(out, img, P * 4, cudaMemcpyDeviceToDevice, st));
-    return replace_pass(img, ws.C, out, h, w, nullptr, st);
+    CK(cudaMemsetAsync(ws.nlist, 0, 4, st));
+    return replace_pass(img, ws, ws.C, ws.nlist, out, h, w, nullptr, st);   // every masked pixel is "new"
 }
 
 // ---- diagnostics ------------------------------------------------------------------------------
