@@ -325,10 +325,11 @@ def run_cuda(args):
 
 # ALU-pipe min/max instructions per output pixel of each kernel class (static SASS
 # count of FMNMX/FMNMX3 per pixel, halo recomputation included) -- the per-unit figure behind
-# roofline.achieved.  v1 kernels: forgetful selection, per-pixel.
+# roofline.achieved.  
 KERNEL_MINMAX_PER_PX = {
-    "fine_gates": 2 * (99 + 480) + 1.28 * 2 * 19 + 5,    # med5(S) + med7(m3) + med3 on the haloed tile
-    "noise_S": 2 * 99 + 6,
+    # generated networks (median_networks.cuh): med7 764/4, med5 326/4, med3 76/4 x 1.46 (haloed m3 tile)
+    "fine_gates": 764 / 4 + 326 / 4 + 1.46 * 76 / 4,
+    "noise_S": 326 / 4 + 13 / 4,                     # med5 + the clamp/floor selects of L+ and N
 }
 # HBM bytes per pixel the path must move with the current fusion:
 # noise_S: read work 4 + write S 4; fine_gates: read work 4 + S 4 + 0.375 bit-planes; dilate/replace ~1
