@@ -41,7 +41,7 @@ FINE_GATES_MINMAX_PER_PX = None   # filled from the library's own accounting bel
 REF_COMPARISONS_PER_PX_ITER = 19 + 99 + 99 + 480
 # dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture
 # (profiles/; None until captured)
-NCU_TRAFFIC_BYTES = None
+NCU_TRAFFIC_BYTES = {"fine_gates": 238157312, "noise_S": 167198464}   # profiles/r01_v2_ncu_full.md
 
 
 def _peaks():
@@ -273,7 +273,7 @@ def run_cuda(args):
     if ops_px is not None:
         achieved = npx * ops_px / (dom_avg_ms * 1e-3) / 1e12
         roof = dict(bound="alu", kernel=dom, achieved=achieved, peak=alu_peak,
-                    unit="T min/max instr/s", frac=achieved / alu_peak, traffic=NCU_TRAFFIC_BYTES,
+                    unit="T min/max instr/s", frac=achieved / alu_peak, traffic=(NCU_TRAFFIC_BYTES or {}).get(dom),
                     peak_source="148 SM x 64 ALU lanes/clk x %.0f MHz (DESIGN.md section 5; lanes/clk "
                                 "measured in profiles/r01_alu_minmax_microbench.txt)" % sm_max,
                     minmax_instr_per_px=ops_px, avg_launch_ms=dom_avg_ms, launches_timed=dom_spans)
