@@ -43,7 +43,7 @@ extern "C" {
 #define LACOSMIC_ERR_SHAPE (-2)     /* h < 1, w < 1, or h*w >= 2^31 (or n < 0 for a batch) */
 #define LACOSMIC_ERR_PARAM (-3)     /* non-finite parameter; gain <= 0; readnoise < 0; sigclip <= 0;
                                        sigfrac <= 0 or > 1; objlim < 0; niter < 0 or > LACOSMIC_MAX_NITER;
-                                       satlevel NaN; k not in {3,5,7} */
+                                       satlevel NaN; unknown mode; k not in {3,5,7} */
 #define LACOSMIC_ERR_ALIGN (-4)     /* fp32 image pointer not 16-byte aligned, workspace not 256-byte aligned */
 #define LACOSMIC_ERR_ALIAS (-5)     /* img, mask_out, clean_out (or workspace) overlap */
 #define LACOSMIC_ERR_WORKSPACE (-6) /* workspace_bytes smaller than lacosmic_workspace_bytes(h, w) */
@@ -59,12 +59,27 @@ extern "C" {
 typedef struct lacosmic_params {
     float gain, readnoise, sigclip, sigfrac, objlim, satlevel;
     int32_t niter;
+    int32_t mode; /* LACOSMIC_MODE_LAZY (0, default) or LACOSMIC_MODE_DENSE */
 } lacosmic_params;
+
+/* Evaluation mode.  Both modes execute the same fp32 operations on the pixels that decide the result
+ * and return bit-identical masks, cleaned frames and counts.
+ *   LACOSMIC_MODE_DENSE: med5(S), med3 and med7(med3) are selected at every pixel by the fused
+ *     k_fine_gates kernel (the reference path; every debug plane is available).
+ *   LACOSMIC_MODE_LAZY: after the dense noise/significance pass, the threshold tests S' > sigclip,
+ *     S' > sigfrac*sigclip and L+/F > objlim are evaluated only on the pixels with S above the
+ *     threshold (S' <= S because med5(S) >= 0), by counting the window elements that satisfy the same
+ *     monotone fp32 test (no selection is needed to compare a median with a threshold); from the
+ *     second iteration on the dense pass skips row segments farther than 2 px from a rewritten pixel. */
+#define LACOSMIC_MODE_LAZY 0
+#define LACOSMIC_MODE_DENSE 1
 
 /* Optional per-step dump of ONE iteration (used by the parity tests).  Every pointer is a
  * nullable device pointer to a [h][w] plane: fp32 for Lp (step 1), N (2), S, Sp (3), m3, F (4);
  * uint8 0/1 for G1 = (S' > sigclip), G2 = (S' > sigfrac*sigclip) (both AND img < satlevel),
- * M1 (step 5), M2, M3 (step 6) and C (cumulative mask after the iteration). */
+ * M1 (step 5), M2, M3 (step 6) and C (cumulative mask after the iteration).  LACOSMIC_MODE_LAZY never
+ * forms Sp, m3, F and evaluates G2 only where step (6) reads it: those four planes are left untouched
+ * there; every other plane is filled and identical in both modes. */
 typedef struct lacosmic_debug {
     int32_t iter;
     float *Lp, *N, *S, *Sp, *m3, *F;
@@ -155,7 +170,7 @@ const char *lacosmic_version(void);
  * LACOSMIC_NUM_KERNEL_CLASSES, the summed device time ms_sum[c] and the number of spans[c] (HOST
  * arrays), and clears the record.  Class names: lacosmic_kernel_class_name(c); the last class is the
  * whole frame (copies included). */
-#define LACOSMIC_NUM_KERNEL_CLASSES 6
+#define LACOSMIC_NUM_KERNEL_CLASSES 7
 int lacosmic_kernel_timing_enable(int enable);
 int lacosmic_kernel_timing_read(float *ms_sum, int32_t *spans);
 const char *lacosmic_kernel_class_name(int cls);

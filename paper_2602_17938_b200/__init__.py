@@ -5,6 +5,8 @@ include/lacosmic.h).  This package only marshals arguments; torch is used for de
 streams.  There is no CPU fallback: every call raises if the CUDA library cannot be loaded.
 """
 from .binding import (  # noqa: F401
+    MODE_DENSE,
+    MODE_LAZY,
     LacosmicError,
     Params,
     lacosmic_bitplane_pitch_words,
@@ -30,4 +32,5 @@ from .binding import (  # noqa: F401
 )
 
 __all__ = [n for n in dir() if n.startswith("lacosmic_")] + ["LacosmicError", "Params",
-                                                              "library_path", "load_library"]
+                                                              "library_path", "load_library",
+                                                              "MODE_LAZY", "MODE_DENSE"]

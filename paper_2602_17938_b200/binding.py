@@ -23,7 +23,8 @@ EXPORTS = (
     "lacosmic_last_cuda_error", "lacosmic_last_launch_count", "lacosmic_version",
     "lacosmic_kernel_timing_enable", "lacosmic_kernel_timing_read", "lacosmic_kernel_class_name",
 )
-NUM_KERNEL_CLASSES = 6
+NUM_KERNEL_CLASSES = 7
+MODE_LAZY, MODE_DENSE = 0, 1
 
 
 class LacosmicError(RuntimeError):
@@ -37,7 +38,7 @@ class LacosmicError(RuntimeError):
 
 class _CParams(C.Structure):
     _fields_ = [(n, C.c_float) for n in ("gain", "readnoise", "sigclip", "sigfrac", "objlim",
-                                         "satlevel")] + [("niter", C.c_int32)]
+                                         "satlevel")] + [("niter", C.c_int32), ("mode", C.c_int32)]
 
 
 class _CDebug(C.Structure):
@@ -59,10 +60,11 @@ class Params:
     objlim: float = 5.0
     satlevel: float = 65535.0
     niter: int = 4
+    mode: int = MODE_LAZY      # MODE_DENSE: the dense reference path (same results)
 
     def _c(self):
         return _CParams(self.gain, self.readnoise, self.sigclip, self.sigfrac, self.objlim,
-                        self.satlevel, int(self.niter))
+                        self.satlevel, int(self.niter), int(self.mode))
 
 
 def library_path() -> str:

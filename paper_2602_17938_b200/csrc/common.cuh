@@ -59,4 +59,40 @@ __device__ __forceinline__ float lplus_px(float c, float U, float D, float Lf, f
     return __fmul_rn(__fadd_rn(__fadd_rn(a, b), __fadd_rn(g, d)), 0.25f);
 }
 
+// ---- block-wide compaction of one 32-pixel word per thread into a pixel list ------------------------
+// All 256 threads of the CTA must call this.  Appends flat indices p0 + bit for every set bit of
+// `bits` (one atomicAdd per CTA).
+__device__ __forceinline__ void block_append(uint32_t bits, int p0, int* __restrict__ list,
+                                             int* __restrict__ nlist) {
+    __shared__ int s_warp[8];
+    __shared__ int s_base;
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    const int n = __popc(bits);
+    int incl = n;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        int o = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += o;
+    }
+    if (lane == 31) s_warp[wi] = incl;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int tot = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            int c = s_warp[i];
+            s_warp[i] = tot;
+            tot += c;
+        }
+        s_base = tot ? atomicAdd(nlist, tot) : 0;
+    }
+    __syncthreads();
+    int base = s_base + s_warp[wi] + incl - n;
+    while (bits) {
+        int b = __ffs(bits) - 1;
+        bits &= bits - 1;
+        list[base++] = p0 + b;
+    }
+}
+
 }  // namespace lac

@@ -109,31 +109,75 @@ struct NoiseArgs {
     float* S;
     float* dbgLp;
     float* dbgN;
-    int h, w;
-    float gain, rn2;
+    uint32_t *A1, *A2;       // nullable (lazy path): bit-planes ok & (S > sigclip), ok & (S > siglow)
+    const uint32_t* dirty;   // nullable: pixels whose `work` changed since S/A1/A2 were last written
+    int h, w, wpr;
+    float gain, rn2, sigclip, siglow, satlevel;
 };
+
+// gather the 4-bit nibbles of the 8 lanes that share a 32-pixel word
+__device__ __forceinline__ uint32_t nibbles_to_word(uint32_t nib, int lane) {
+    uint32_t v = nib << ((lane & 7) * 4);
+    v |= __shfl_xor_sync(0xffffffffu, v, 1);
+    v |= __shfl_xor_sync(0xffffffffu, v, 2);
+    v |= __shfl_xor_sync(0xffffffffu, v, 4);
+    return v;
+}
+
+// Does any pixel of `dirty` lie within 2 px (Chebyshev) of the 128 px of row y starting at x0?  S, A1 and
+// A2 at a pixel depend on `work` within that distance only (med5 window; L+ needs 1), so a warp whose
+// row segment is clean keeps the planes written by an earlier iteration.  Warp-uniform result.
+__device__ __forceinline__ bool row_segment_dirty(const uint32_t* __restrict__ dirty, int y, int x0, int h,
+                                                  int wpr, int lane) {
+    uint32_t v = 0;
+    if (lane < 30) {
+        const int r = y - 2 + lane / 6, k = lane % 6, wq = (x0 >> 5) - 1 + k;
+        if (r >= 0 && r < h && wq >= 0 && wq < wpr) {
+            v = dirty[(size_t)r * wpr + wq];
+            if (k == 0) v &= 0xC0000000u;
+            if (k == 5) v &= 0x00000003u;
+        }
+    }
+    return __any_sync(0xffffffffu, v != 0);
+}
 
 // sm: work tile with margins (NS_MX, NS_MY), edge-replicated
 __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a, int x0, int y0, int lane,
                                              int wi) {
 #pragma unroll 1
     for (int ly = wi; ly < TH; ly += NWARP) {
-        int y = y0 + ly, x = x0 + 4 * lane;
-        if (y >= a.h || x >= a.w) continue;
-        float win[8][5], m5[4], s[4], lp[4], n[4];
-        load_window<5, NS_PITCH>(sm + ly * NS_PITCH + 4 * lane, win);
-        median5x5_x4(win, m5);
+        const int y = y0 + ly, x = x0 + 4 * lane;
+        if (y >= a.h) continue;                                                       // warp-uniform
+        if (a.dirty && !row_segment_dirty(a.dirty, y, x0, a.h, a.wpr, lane)) continue;   // warp-uniform
+        uint32_t n1 = 0, n2 = 0;
+        if (x < a.w) {
+            float win[8][5], m5[4], s[4], lp[4], n[4];
+            load_window<5, NS_PITCH>(sm + ly * NS_PITCH + 4 * lane, win);
+            median5x5_x4(win, m5);
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            lp[j] = lplus_px(win[2 + j][2], win[2 + j][1], win[2 + j][3], win[1 + j][2], win[3 + j][2]);
-            float m5c = m5[j] > 1e-4f ? m5[j] : 1e-4f;                                 // R5
-            n[j] = __fdiv_rn(__fsqrt_rn(__fadd_rn(__fmul_rn(a.gain, m5c), a.rn2)), a.gain);
-            s[j] = __fdiv_rn(lp[j], __fmul_rn(2.0f, n[j]));
+            for (int j = 0; j < 4; ++j) {
+                lp[j] = lplus_px(win[2 + j][2], win[2 + j][1], win[2 + j][3], win[1 + j][2], win[3 + j][2]);
+                float m5c = m5[j] > 1e-4f ? m5[j] : 1e-4f;                                 // R5
+                n[j] = __fdiv_rn(__fsqrt_rn(__fadd_rn(__fmul_rn(a.gain, m5c), a.rn2)), a.gain);
+                s[j] = __fdiv_rn(lp[j], __fmul_rn(2.0f, n[j]));
+                const bool ok = (x + j < a.w) && (win[2 + j][2] < a.satlevel);            // R12
+                n1 |= (uint32_t)(ok && s[j] > a.sigclip) << j;
+                n2 |= (uint32_t)(ok && s[j] > a.siglow) << j;
+            }
+            size_t ro = (size_t)y * a.w;
+            store4(a.S, ro, x, a.w, s);
+            if (a.dbgLp) store4(a.dbgLp, ro, x, a.w, lp);
+            if (a.dbgN) store4(a.dbgN, ro, x, a.w, n);
         }
-        size_t ro = (size_t)y * a.w;
-        store4(a.S, ro, x, a.w, s);
-        if (a.dbgLp) store4(a.dbgLp, ro, x, a.w, lp);
-        if (a.dbgN) store4(a.dbgN, ro, x, a.w, n);
+        if (a.A1) {
+            const uint32_t b1 = nibbles_to_word(n1, lane), b2 = nibbles_to_word(n2, lane);
+            const int wx = (x0 >> 5) + (lane >> 3);
+            if ((lane & 7) == 0 && wx < a.wpr) {
+                size_t q = (size_t)y * a.wpr + wx;
+                a.A1[q] = b1;
+                a.A2[q] = b2;
+            }
+        }
     }
 }
 
@@ -147,15 +191,6 @@ k_noise_S(const float* __restrict__ work, NoiseArgs a, const int* prev_count) {
     load_tile<NS_MX, NS_MY, NS_PITCH>(sm, work, a.h, a.w, y0, x0, tid);
     __syncthreads();
     noise_S_tile(sm, a, x0, y0, tid & 31, tid >> 5);
-}
-
-// gather the 4-bit nibbles of the 8 lanes that share a 32-pixel word
-__device__ __forceinline__ uint32_t nibbles_to_word(uint32_t nib, int lane) {
-    uint32_t v = nib << ((lane & 7) * 4);
-    v |= __shfl_xor_sync(0xffffffffu, v, 1);
-    v |= __shfl_xor_sync(0xffffffffu, v, 2);
-    v |= __shfl_xor_sync(0xffffffffu, v, 4);
-    return v;
 }
 
 // K_B: steps (3b)-(5).  S' = S - med5(S); m3 = med3(work) (tile in shared memory, replicated at the
@@ -483,8 +518,8 @@ k_dilate_gate(const uint32_t* __restrict__ in, const uint32_t* __restrict__ gate
 // and k_replace_list gives each listed pixel to one thread: 25 clamped taps -> +inf where the tap's
 // pixel is in C -> 25-input sorting network -> middle element(s) of the k donors (R14-R16).
 __global__ void __launch_bounds__(256)
-k_build_list(const uint32_t* __restrict__ newp, const uint32_t* __restrict__ Cb, int* __restrict__ list,
-             int* __restrict__ nlist, int h, int w, int wpr, const int* prev_count) {
+k_build_list(const uint32_t* __restrict__ newp, const uint32_t* __restrict__ Cb, uint32_t* __restrict__ needp,
+             int* __restrict__ list, int* __restrict__ nlist, int h, int w, int wpr, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     const int lane = threadIdx.x & 31;
     const int wx = blockIdx.x * 32 + lane;
@@ -504,24 +539,9 @@ k_build_list(const uint32_t* __restrict__ newp, const uint32_t* __restrict__ Cb,
                               (vr << 31) | (vr << 30);
             need = spread & c;
         }
+        if (needp) needp[(size_t)y * wpr + wx] = need;   // the pixels k_replace_list rewrites
     }
-    int n = __popc(need), incl = n;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        int o = __shfl_up_sync(0xffffffffu, incl, d);
-        if (lane >= d) incl += o;
-    }
-    int total = __shfl_sync(0xffffffffu, incl, 31);
-    if (total == 0) return;
-    int base = 0;
-    if (lane == 31) base = atomicAdd(nlist, total);
-    base = __shfl_sync(0xffffffffu, base, 31) + incl - n;
-    const int p0 = y * w + wx * 32;
-    while (need) {
-        int b = __ffs(need) - 1;
-        need &= need - 1;
-        list[base++] = p0 + b;
-    }
+    block_append(need, y * w + wx * 32, list, nlist);
 }
 
 __global__ void __launch_bounds__(128)
@@ -579,9 +599,16 @@ k_replace_list(const float* __restrict__ img, const uint32_t* __restrict__ Cb, f
 // bit-plane <-> uint8 plane
 __global__ void __launch_bounds__(256)
 k_unpack_bits(const uint32_t* __restrict__ bits, uint8_t* __restrict__ u8, int h, int w, int wpr) {
-    int x = blockIdx.x * 256 + threadIdx.x, y = blockIdx.y;
+    const int x = (blockIdx.x * 256 + threadIdx.x) * 4, y = blockIdx.y;
     if (x >= w) return;
-    u8[(size_t)y * w + x] = (uint8_t)((bits[(size_t)y * wpr + (x >> 5)] >> (x & 31)) & 1u);
+    const uint32_t nib = (bits[(size_t)y * wpr + (x >> 5)] >> (x & 31)) & 0xfu;   // x % 4 == 0: one word
+    uint8_t* dst = u8 + (size_t)y * w + x;
+    if (x + 3 < w && (reinterpret_cast<uintptr_t>(dst) & 3) == 0) {
+        // spread the 4 bits into 4 bytes (0x01 each)
+        *reinterpret_cast<uint32_t*>(dst) = (nib & 1u) | ((nib & 2u) << 7) | ((nib & 4u) << 14) | ((nib & 8u) << 21);
+    } else {
+        for (int j = 0; j < 4 && x + j < w; ++j) dst[j] = (uint8_t)((nib >> j) & 1u);
+    }
 }
 
 __global__ void __launch_bounds__(256)

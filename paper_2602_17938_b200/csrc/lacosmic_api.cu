@@ -7,6 +7,7 @@
 #include <cstring>
 
 #include "kernels.cuh"
+#include "lazy.cuh"
 
 namespace {
 
@@ -25,7 +26,7 @@ inline bool cuda_ok(cudaError_t e) {
 
 // Optional per-kernel-class CUDA-event timing (lacosmic_kernel_timing_*): bench.py switches it on to
 // measure the dominant kernel's average launch duration on the launching stream.
-enum KClass { KC_NOISE_S = 0, KC_FINE_GATES, KC_DILATE, KC_REPLACE, KC_BITS, KC_STEP, KC_COUNT };
+enum KClass { KC_NOISE_S = 0, KC_FINE_GATES, KC_DILATE, KC_REPLACE, KC_BITS, KC_LAZY, KC_STEP, KC_COUNT };
 static_assert(KC_COUNT == LACOSMIC_NUM_KERNEL_CLASSES, "header and library disagree");
 struct KTiming {
     static constexpr int MAXSPANS = 8192;
@@ -125,6 +126,7 @@ inline int check_params(const lacosmic_params& p) {
     if (!(p.gain > 0.0f) || p.readnoise < 0.0f || !(p.sigclip > 0.0f) || !(p.sigfrac > 0.0f) ||
         p.sigfrac > 1.0f || p.objlim < 0.0f || p.niter < 0 || p.niter > LACOSMIC_MAX_NITER)
         return LACOSMIC_ERR_PARAM;
+    if (p.mode != LACOSMIC_MODE_LAZY && p.mode != LACOSMIC_MODE_DENSE) return LACOSMIC_ERR_PARAM;
     return LACOSMIC_OK;
 }
 
@@ -135,13 +137,16 @@ inline bool overlap(const void* a, size_t na, const void* b, size_t nb) {
 
 // Workspace layout (all offsets 256-byte aligned)
 struct Workspace {
-    float* S;
-    uint32_t *G1, *G2, *M1, *M2, *M3, *C, *NEWP;
-    int32_t* counts;   // LACOSMIC_MAX_NITER new-pixel counts, then LACOSMIC_MAX_NITER list lengths
-    int32_t* nlist;
-    int32_t* list;     // compacted pixel list; aliases the S plane (dead once the gates are written)
+    float* S;          // significance plane; persistent across the iterations of a frame
+    int32_t* list;     // compacted pixel list (capacity h*w), reused by every list pass of an iteration
+    uint32_t *G1, *G2, *M1, *M2, *M3, *C, *NEWP, *A1, *A2, *NEED;
+    int32_t* counts;   // per iteration: newly flagged pixels
+    int32_t* nneed;    // per iteration: pixels (re)replaced
+    int32_t* ncand;    // per iteration (lazy path): pixels of A1
+    int32_t* nnb;      // per iteration (lazy path): neighbour pixels whose G2 was evaluated
     size_t bytes;
 };
+constexpr int NCOUNTERS = 4 * LACOSMIC_MAX_NITER;
 
 Workspace carve(void* base, int h, int w) {
     Workspace ws;
@@ -150,41 +155,42 @@ Workspace carve(void* base, int h, int w) {
     char* p = (char*)base;
     size_t off = 0;
     ws.S = (float*)(p + off); off += plane;
-    ws.G1 = (uint32_t*)(p + off); off += bp;
-    ws.G2 = (uint32_t*)(p + off); off += bp;
-    ws.M1 = (uint32_t*)(p + off); off += bp;
-    ws.M2 = (uint32_t*)(p + off); off += bp;
-    ws.M3 = (uint32_t*)(p + off); off += bp;
-    ws.C = (uint32_t*)(p + off); off += bp;
-    ws.NEWP = (uint32_t*)(p + off); off += bp;
-    ws.counts = (int32_t*)(p + off); off += align_up(2 * LACOSMIC_MAX_NITER * 4, 256);
-    ws.nlist = ws.counts + LACOSMIC_MAX_NITER;
-    ws.list = (int32_t*)ws.S;
+    ws.list = (int32_t*)(p + off); off += plane;
+    uint32_t** planes[] = {&ws.G1, &ws.G2, &ws.M1, &ws.M2, &ws.M3, &ws.C, &ws.NEWP, &ws.A1, &ws.A2, &ws.NEED};
+    for (uint32_t** pl : planes) { *pl = (uint32_t*)(p + off); off += bp; }
+    ws.counts = (int32_t*)(p + off); off += align_up(NCOUNTERS * 4, 256);
+    ws.nneed = ws.counts + LACOSMIC_MAX_NITER;
+    ws.ncand = ws.counts + 2 * LACOSMIC_MAX_NITER;
+    ws.nnb = ws.counts + 3 * LACOSMIC_MAX_NITER;
     ws.bytes = off;
     return ws;
 }
 
+int list_grid(int h, int w, int threads) {
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    long long want = ((long long)h * w / 64 + threads - 1) / threads;      // enough threads for a 1.6 % list
+    return (int)std::max(1LL, std::min((long long)sms * 16, want));
+}
+
 int unpack(const uint32_t* bits, uint8_t* u8, int h, int w, cudaStream_t st) {
-    dim3 g((w + 255) / 256, h);
+    dim3 g((w + 1023) / 1024, h);
     Span sp(KC_BITS, st);
     lac::k_unpack_bits<<<g, 256, 0, st>>>(bits, u8, h, w, words_per_row(w));
     LAUNCHED();
     return LACOSMIC_OK;
 }
 
-// (re)compute work at every pixel of C whose 5x5 window holds a pixel of `newp`
-int replace_pass(const float* img, const Workspace& ws, const uint32_t* newp, int* nlist, float* work,
-                 int h, int w, const int* prev, cudaStream_t st) {
+// (re)compute work at every pixel of C whose 5x5 window holds a pixel of `newp`; `need_plane`
+// (nullable) receives the bit-plane of the pixels rewritten
+int replace_pass(const float* img, const Workspace& ws, const uint32_t* newp, uint32_t* need_plane,
+                 int* nlist, float* work, int h, int w, const int* prev, cudaStream_t st) {
     const int wpr = words_per_row(w);
     dim3 dg((wpr + 31) / 32, (h + 7) / 8);
     Span sp(KC_REPLACE, st);
-    lac::k_build_list<<<dg, 256, 0, st>>>(newp, ws.C, ws.list, nlist, h, w, wpr, prev);
+    lac::k_build_list<<<dg, 256, 0, st>>>(newp, ws.C, need_plane, ws.list, nlist, h, w, wpr, prev);
     LAUNCHED();
-    int dev = 0, sms = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    long long want = ((long long)h * w / 64 + 127) / 128;      // enough threads for a 1.6 % mask
-    int blocks = (int)std::max(1LL, std::min((long long)sms * 16, want));
-    lac::k_replace_list<<<blocks, 128, 0, st>>>(img, ws.C, work, ws.list, nlist, h, w, wpr, prev);
+    lac::k_replace_list<<<list_grid(h, w, 128), 128, 0, st>>>(img, ws.C, work, ws.list, nlist, h, w, wpr, prev);
     LAUNCHED();
     return LACOSMIC_OK;
 }
@@ -201,9 +207,10 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     // O0
     CK(cudaMemcpyAsync(work, img, P * 4, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemsetAsync(ws.C, 0, bp_bytes, st));
-    CK(cudaMemsetAsync(ws.counts, 0, 2 * LACOSMIC_MAX_NITER * 4, st));
+    CK(cudaMemsetAsync(ws.counts, 0, NCOUNTERS * 4, st));
     const float siglow = p.sigfrac * p.sigclip;   // R9: one fp32 multiply on the host
     const float rn2 = p.readnoise * p.readnoise;
+    const bool lazy = p.mode == LACOSMIC_MODE_LAZY;
     lac::GateParams gp{p.sigclip, siglow, p.objlim, p.satlevel};
     dim3 tb(lac::NT), tg((w + lac::TW - 1) / lac::TW, (h + lac::TH - 1) / lac::TH);
     dim3 dg((wpr + 31) / 32, (h + 7) / 8);
@@ -227,37 +234,78 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     for (int t = 0; t < p.niter; ++t) {
         const int* prev = t > 0 ? ws.counts + (t - 1) : nullptr;
         const bool d = dbg && dbg->iter == t;
-        lac::NoiseArgs na{ws.S, d ? dbg->Lp : nullptr, d ? dbg->N : nullptr, h, w, p.gain, rn2};
-        lac::FineArgs fa{ws.G1, ws.G2, ws.M1, d ? dbg->Sp : nullptr, d ? dbg->m3 : nullptr,
-                         d ? dbg->F : nullptr, h, w, wpr, gp};
+        int rc;
+        lac::NoiseArgs na{ws.S, d ? dbg->Lp : nullptr, d ? dbg->N : nullptr,
+                          lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
+                          // from the second iteration on S, A1, A2 only change near the pixels the previous
+                          // replacement pass rewrote (a debug dump recomputes everything)
+                          (lazy && t > 0 && !d) ? ws.NEED : nullptr,
+                          h, w, wpr, p.gain, rn2, p.sigclip, siglow, p.satlevel};
         {
             Span sp(KC_NOISE_S, st);
             if (tma) lac::k_noise_S_tma<<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(mapWorkNS, na, ntx, ntiles, prev);
             else lac::k_noise_S<<<tg, tb, 0, st>>>(work, na, prev);
             LAUNCHED();
         }
-        {
-            Span sp(KC_FINE_GATES, st);
-            if (tma) lac::k_fine_gates_tma<<<gridFG, tb, lac::FG_SMEM_BYTES, st>>>(mapWorkFG, mapS, fa, ntx, ntiles, prev);
-            else lac::k_fine_gates<<<tg, tb, 0, st>>>(work, ws.S, fa, prev);
-            LAUNCHED();
+        if (lazy) {
+            // steps (3b)-(5) on the pixels of A1 only (lazy.cuh), then the two gated growths; G2 is
+            // evaluated on the further pixels the second growth can reach
+            lac::CandArgs ca{ws.S, work, ws.G1, ws.G2, ws.M1, h, w, wpr, p.sigclip, siglow, p.objlim};
+            {
+                Span sp(KC_LAZY, st);
+                lac::k_list_candidates<<<dg, 256, 0, st>>>(ws.A1, ws.G1, ws.G2, ws.M1, ws.list, ws.ncand + t,
+                                                          h, w, wpr, prev);
+                LAUNCHED();
+                lac::k_eval_candidates<<<list_grid(h, w, 128), 128, 0, st>>>(ca, ws.list, ws.ncand + t, prev);
+                LAUNCHED();
+            }
+            {
+                Span sp(KC_DILATE, st);
+                lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M1, ws.G1, ws.M2, nullptr, nullptr, nullptr, h, w,
+                                                      wpr, prev);
+                LAUNCHED();
+            }
+            {
+                Span sp(KC_LAZY, st);
+                lac::k_list_neighbours<<<dg, 256, 0, st>>>(ws.M2, ws.A1, ws.A2, ws.list, ws.nnb + t, h, w, wpr,
+                                                          prev);
+                LAUNCHED();
+                lac::k_eval_neighbours<<<list_grid(h, w, 128), 128, 0, st>>>(ws.S, ws.G2, h, w, wpr, siglow,
+                                                                            ws.list, ws.nnb + t, prev);
+                LAUNCHED();
+            }
+            {
+                Span sp(KC_DILATE, st);
+                lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M2, ws.G2, ws.M3, ws.C, ws.NEWP, ws.counts + t, h, w,
+                                                      wpr, prev);
+                LAUNCHED();
+            }
+        } else {
+            lac::FineArgs fa{ws.G1, ws.G2, ws.M1, d ? dbg->Sp : nullptr, d ? dbg->m3 : nullptr,
+                             d ? dbg->F : nullptr, h, w, wpr, gp};
+            {
+                Span sp(KC_FINE_GATES, st);
+                if (tma) lac::k_fine_gates_tma<<<gridFG, tb, lac::FG_SMEM_BYTES, st>>>(mapWorkFG, mapS, fa, ntx, ntiles, prev);
+                else lac::k_fine_gates<<<tg, tb, 0, st>>>(work, ws.S, fa, prev);
+                LAUNCHED();
+            }
+            {
+                Span sp(KC_DILATE, st);
+                lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M1, ws.G1, ws.M2, nullptr, nullptr, nullptr, h, w,
+                                                      wpr, prev);
+                LAUNCHED();
+                lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M2, ws.G2, ws.M3, ws.C, ws.NEWP, ws.counts + t, h, w,
+                                                      wpr, prev);
+                LAUNCHED();
+            }
         }
-        {
-            Span sp(KC_DILATE, st);
-            lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M1, ws.G1, ws.M2, nullptr, nullptr, nullptr, h, w,
-                                                  wpr, prev);
-            LAUNCHED();
-            lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M2, ws.G2, ws.M3, ws.C, ws.NEWP, ws.counts + t, h, w,
-                                                  wpr, prev);
-            LAUNCHED();
-        }
-        // the S plane is dead from here on; its storage becomes the compacted pixel list
         if (d && dbg->S) CK(cudaMemcpyAsync(dbg->S, ws.S, P * 4, cudaMemcpyDeviceToDevice, st));
-        int rc = replace_pass(img, ws, ws.NEWP, ws.nlist + t, work, h, w, prev, st);
+        rc = replace_pass(img, ws, ws.NEWP, ws.NEED, ws.nneed + t, work, h, w, prev, st);
         if (rc) return rc;
         if (d) {
+            // lazy path: G2 is only evaluated where step (6) needs it, so it is not dumped
             struct { const uint32_t* b; uint8_t* o; } planes[] = {
-                {ws.G1, dbg->G1}, {ws.G2, dbg->G2}, {ws.M1, dbg->M1},
+                {ws.G1, dbg->G1}, {ws.G2, lazy ? nullptr : dbg->G2}, {ws.M1, dbg->M1},
                 {ws.M2, dbg->M2}, {ws.M3, dbg->M3}, {ws.C, dbg->C}};
             for (auto& pl : planes)
                 if (pl.o && (rc = unpack(pl.b, pl.o, h, w, st))) return rc;
@@ -311,7 +359,7 @@ int lacosmic_run(const float* img, int h, int w, float gain, float readnoise, fl
                  float sigfrac, float objlim, int niter, float satlevel, uint8_t* mask_out,
                  float* clean_out, void* stream) {
     g_launches = 0;
-    lacosmic_params p{gain, readnoise, sigclip, sigfrac, objlim, satlevel, niter};
+    lacosmic_params p{gain, readnoise, sigclip, sigfrac, objlim, satlevel, niter, LACOSMIC_MODE_LAZY};
     if (!img || !mask_out || !clean_out) return LACOSMIC_ERR_NULL;
     int rc = check_shape(h, w);
     if (rc) return rc;
@@ -464,8 +512,8 @@ int lacosmic_masked_median(const float* img, const uint8_t* mask_u8, float* out,
     cudaStream_t st = (cudaStream_t)stream;
     if ((rc = lacosmic_pack_bits(mask_u8, ws.C, h, w, stream))) return rc;
     CK(cudaMemcpyAsync(out, img, P * 4, cudaMemcpyDeviceToDevice, st));
-    CK(cudaMemsetAsync(ws.nlist, 0, 4, st));
-    return replace_pass(img, ws, ws.C, ws.nlist, out, h, w, nullptr, st);   // every masked pixel is "new"
+    CK(cudaMemsetAsync(ws.nneed, 0, 4, st));
+    return replace_pass(img, ws, ws.C, nullptr, ws.nneed, out, h, w, nullptr, st);   // every masked pixel is "new"
 }
 
 // ---- diagnostics ------------------------------------------------------------------------------
@@ -509,12 +557,12 @@ int lacosmic_kernel_timing_read(float* ms_sum, int32_t* spans) {
 
 const char* lacosmic_kernel_class_name(int cls) {
     static const char* names[KC_COUNT] = {"noise_S", "fine_gates", "dilate_x2", "replace", "bits",
-                                          "whole_frame"};
+                                          "lazy_eval", "whole_frame"};
     return (cls >= 0 && cls < KC_COUNT) ? names[cls] : "?";
 }
 
 int lacosmic_last_cuda_error(void) { return g_last_cuda_error; }
 int lacosmic_last_launch_count(void) { return g_launches; }
-const char* lacosmic_version(void) { return "lacosmic-b200 0.1 (sm_100a)"; }
+const char* lacosmic_version(void) { return "lacosmic-b200 0.2 (sm_100a)"; }
 
 }  // extern "C"

@@ -36,7 +36,7 @@ def test_binding_lists_every_declared_symbol():
 
 def test_params_struct_layout():
     from paper_2602_17938_b200 import binding
-    assert C.sizeof(binding._CParams) == 28          # 6 floats + 1 int32, no padding
+    assert C.sizeof(binding._CParams) == 32          # 6 floats + 2 int32, no padding
     assert C.sizeof(binding._CDebug) == 8 + 12 * 8
 
 
@@ -45,7 +45,7 @@ def test_workspace_sizes(L):
     assert L.lacosmic_workspace_bytes(5, -1) == 0
     assert L.lacosmic_workspace_bytes(65536, 65536) == 0          # h*w >= 2^31
     n = L.lacosmic_workspace_bytes(4000, 6500)
-    assert 4000 * 6500 * 4 < n < 3 * 4000 * 6500 * 4
+    assert 2 * 4000 * 6500 * 4 < n < 3 * 4000 * 6500 * 4
     assert L.lacosmic_host_workspace_bytes(4000, 6500) > n + 2 * 4000 * 6500 * 4
     assert L.lacosmic_bitplane_pitch_words(6500) == 204
     assert L.lacosmic_bitplane_pitch_words(32) == 1 and L.lacosmic_bitplane_pitch_words(33) == 2
@@ -54,7 +54,7 @@ def test_workspace_sizes(L):
 def test_argument_errors_without_gpu(L):
     """Validation happens before any CUDA call, so these run on a machine with no GPU."""
     from paper_2602_17938_b200.binding import _CParams
-    ok = _CParams(1.0, 10.0, 4.5, 0.3, 5.0, 65535.0, 4)
+    ok = _CParams(1.0, 10.0, 4.5, 0.3, 5.0, 65535.0, 4, 0)
     fake = lambda a: C.c_void_p(a)                     # never dereferenced: checks fail first
     img, mask, clean, ws = 0x10000000, 0x20000000, 0x30000000, 0x40000000
     need = L.lacosmic_workspace_bytes(64, 64)
@@ -67,13 +67,13 @@ def test_argument_errors_without_gpu(L):
     assert run(nb=need - 1) == -6
     bads = [dict(gain=0.0), dict(gain=float("nan")), dict(readnoise=-1.0), dict(sigclip=0.0),
             dict(sigfrac=0.0), dict(sigfrac=1.5), dict(objlim=-0.1), dict(niter=-1), dict(niter=65),
-            dict(satlevel=float("nan")), dict(sigclip=float("inf"))]
+            dict(satlevel=float("nan")), dict(sigclip=float("inf")), dict(mode=2), dict(mode=-1)]
     for b in bads:
         kw = dict(gain=1.0, readnoise=10.0, sigclip=4.5, sigfrac=0.3, objlim=5.0, satlevel=65535.0,
-                  niter=4)
+                  niter=4, mode=0)
         kw.update(b)
         assert run(p=_CParams(*[kw[k] for k in ("gain", "readnoise", "sigclip", "sigfrac", "objlim",
-                                                 "satlevel", "niter")])) == -3, b
+                                                 "satlevel", "niter", "mode")])) == -3, b
     assert L.lacosmic_medfilt(fake(img), fake(clean), 8, 8, 4, None) == -3
     assert L.lacosmic_medfilt(fake(img), fake(img), 8, 8, 3, None) == -5
     assert L.lacosmic_lplus(None, fake(clean), 8, 8, None) == -1

@@ -120,13 +120,23 @@ def _near_threshold_report(o, p):
                 objlim=int(((np.abs(ratio - p["objlim"]) <= 1e-4 * p["objlim"]) & (o["G1"] > 0)).sum()))
 
 
-def _compare_run(lc, orc, img, p, debug_iter=None, label=""):
+MODES = ["lazy", "dense"]
+# planes LACOSMIC_MODE_LAZY never forms (include/lacosmic.h, lacosmic_debug)
+LAZY_SKIPS = ("Sp", "m3", "F", "G2")
+
+
+def _compare_run(lc, orc, img, p, debug_iter=None, label="", mode="lazy"):
     o = orc.run(img, debug_iter=debug_iter, **p)
-    g = lc.lacosmic_run_ws(_t(img), lc.Params(**p), debug_iter=debug_iter)
+    lazy = mode == "lazy"
+    label = "%s [%s]" % (label, mode)
+    g = lc.lacosmic_run_ws(_t(img), lc.Params(mode=lc.MODE_LAZY if lazy else lc.MODE_DENSE, **p),
+                           debug_iter=debug_iter)
     import torch
     torch.cuda.synchronize()
     if debug_iter is not None and debug_iter < p["niter"]:
         for name in ("Lp", "N", "S", "Sp", "m3", "F"):
+            if lazy and name in LAZY_SKIPS:
+                continue
             a, b = _n(g[name]), o[name]
             assert not np.isnan(a).any(), name
             rel = np.abs(a - b) / np.maximum(np.abs(b), 1e-30)
@@ -136,6 +146,8 @@ def _compare_run(lc, orc, img, p, debug_iter=None, label=""):
             assert rel.max() <= 1e-6, name          # the north_star tolerance
             assert nbad == 0, name                   # the stricter design bar: ==
         for name in ("G1", "G2", "M1", "M2", "M3", "C"):
+            if lazy and name in LAZY_SKIPS:
+                continue
             assert np.array_equal(_n(g[name]), o[name]), name
         print(label, "near-threshold pixels (within 1e-4 rel):", _near_threshold_report(o, p))
     ndiff = int((_n(g["mask"]) != o["mask"]).sum())
@@ -145,45 +157,63 @@ def _compare_run(lc, orc, img, p, debug_iter=None, label=""):
     return o, g
 
 
-@pytest.mark.parametrize("debug_iter", [0, 1, 3])
-def test_config0_every_plane(lc, orc, debug_iter):
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("debug_iter", [0, 1, 3, None])
+def test_config0_every_plane(lc, orc, debug_iter, mode):
     f = synth.make_config(0)
-    o, _ = _compare_run(lc, orc, f.img, PARAMS, debug_iter, "configs[0]")
+    o, _ = _compare_run(lc, orc, f.img, PARAMS, debug_iter, "configs[0]", mode)
     assert o["mask"].sum() > 500
 
 
-def test_config1_whole_frame(lc, orc):
+@pytest.mark.parametrize("mode", MODES)
+def test_config1_whole_frame(lc, orc, mode):
     f = synth.make_config(1)
-    o, _ = _compare_run(lc, orc, f.img, PARAMS, 0, "configs[1]")
+    o, _ = _compare_run(lc, orc, f.img, PARAMS, 0 if mode == "dense" else None, "configs[1]", mode)
     assert o["mask"].sum() > 10000
 
 
-@pytest.mark.parametrize("shape", [(1, 1), (1, 40), (40, 1), (2, 2), (5, 33), (31, 65), (100, 203)])
-def test_ragged_and_tiny_frames(lc, orc, shape):
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("shape", [(1, 1), (1, 40), (40, 1), (2, 2), (5, 33), (31, 65), (100, 203), (9, 300),
+                                   (300, 9), (64, 128), (131, 260)])
+def test_ragged_and_tiny_frames(lc, orc, shape, mode):
     f = synth.make_frame(shape[0], shape[1], seed=77, n_star=2, n_cr=max(1, shape[0] * shape[1] // 150),
                          n_hot=3, sp_frac=0.01)
-    _compare_run(lc, orc, f.img, PARAMS, 0, str(shape))
+    _compare_run(lc, orc, f.img, PARAMS, 0, str(shape), mode)
+    _compare_run(lc, orc, f.img, PARAMS, None, str(shape), mode)
 
 
 @pytest.mark.parametrize("p", [dict(niter=0), dict(niter=1), dict(niter=12), dict(satlevel=float("inf")),
                                dict(gain=1.7, readnoise=6.5), dict(sigclip=4.0, sigfrac=1.0, objlim=0.0),
                                dict(readnoise=0.0, gain=2.0), dict(satlevel=500.0)])
-def test_parameter_variants(lc, orc, p):
+@pytest.mark.parametrize("mode", MODES)
+def test_parameter_variants(lc, orc, p, mode):
     f = synth.make_frame(160, 190, seed=78, n_star=10, n_cr=120, n_hot=30, sp_frac=0.005, n_sat=2)
-    _compare_run(lc, orc, f.img, dict(PARAMS, **p), 0, str(p))
+    _compare_run(lc, orc, f.img, dict(PARAMS, **p), 0, str(p), mode)
+    _compare_run(lc, orc, f.img, dict(PARAMS, **p), None, str(p), mode)
 
 
-def test_fixed_point_early_exit_is_exact(lc, orc):
+@pytest.mark.parametrize("mode", MODES)
+def test_fixed_point_early_exit_is_exact(lc, orc, mode):
     """R17: iterations after new_t = 0 are skipped on the device; the output must not change."""
     f = synth.make_frame(128, 128, seed=32, n_star=8, n_cr=80, n_hot=20)
-    o, g = _compare_run(lc, orc, f.img, dict(PARAMS, niter=12), None, "niter=12")
+    o, g = _compare_run(lc, orc, f.img, dict(PARAMS, niter=12), None, "niter=12", mode)
     assert (o["counts"] == 0).any()
 
 
-def test_negative_image_and_constant(lc, orc):
+@pytest.mark.parametrize("mode", MODES)
+def test_negative_image_and_constant(lc, orc, mode):
     img = (-50.0 - 10.0 * _rng(61).random((50, 70))).astype(np.float32)
-    _compare_run(lc, orc, img, dict(PARAMS, readnoise=0.0, gain=2.0), 0, "negative")
-    _compare_run(lc, orc, np.full((40, 45), 100.0, np.float32), PARAMS, 0, "constant")
+    _compare_run(lc, orc, img, dict(PARAMS, readnoise=0.0, gain=2.0), 0, "negative", mode)
+    _compare_run(lc, orc, np.full((40, 45), 100.0, np.float32), PARAMS, 0, "constant", mode)
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_dense_candidates_low_thresholds(lc, orc, mode):
+    """Degenerate thresholds: almost every pixel has S above sigclip, so the lazy lists hold a large
+    part of the frame, borders included; ties from quantised pixel values."""
+    f = synth.make_frame(150, 230, seed=79, n_star=10, n_cr=200, n_hot=30, sp_frac=0.02, n_sat=2)
+    _compare_run(lc, orc, f.img, dict(PARAMS, sigclip=0.05, sigfrac=0.5, objlim=0.3), 0, "low thr", mode)
+    _compare_run(lc, orc, np.round(f.img / 8) * 8, dict(PARAMS, sigclip=1.0, objlim=1.0), 1, "quantised", mode)
 
 
 def test_rot180_invariance_on_gpu(lc):
@@ -244,13 +274,13 @@ def _windows(h, w, size=192):
     return [(y, x, size) for y in ys for x in xs]
 
 
-def _check_full_frame(lc, orc, img, p, label):
+def _check_full_frame(lc, orc, img, p, label, mode="lazy"):
     """Sampled windows the oracle can compute one by one: the result inside a window depends only on
     input within HALO pixels (4 iterations x radius 8 + 6), so the oracle run on the haloed crop is
     exact on the window interior (crop edges that coincide with frame edges replicate identically)."""
     import torch
     h, w = img.shape
-    g = lc.lacosmic_run_ws(_t(img), lc.Params(**p))
+    g = lc.lacosmic_run_ws(_t(img), lc.Params(mode=lc.MODE_LAZY if mode == "lazy" else lc.MODE_DENSE, **p))
     torch.cuda.synchronize()
     gm, gc, counts = _n(g["mask"]), _n(g["clean"]), _n(g["counts"])
     nmask = 0
@@ -272,9 +302,12 @@ def _check_full_frame(lc, orc, img, p, label):
 
 
 def test_config2_full_size_windows(lc, orc):
+    """Both modes in the launch configuration bench.py times; they must also agree on the whole frame."""
     f = synth.make_config(2)
-    gm = _check_full_frame(lc, orc, f.img, PARAMS, "configs[2]")
+    gm = _check_full_frame(lc, orc, f.img, PARAMS, "configs[2]", "lazy")
     assert gm[f.cr_truth].mean() > 0.95
+    gd = _check_full_frame(lc, orc, f.img, PARAMS, "configs[2]", "dense")
+    assert np.array_equal(gm, gd)
 
 
 def test_config4_saturation_stress_full_size(lc, orc):
