@@ -66,10 +66,13 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
-                 "--format=csv,noheader,nounits", "-lms", "100"],
+                 "--format=csv,noheader,nounits", "-lms", "50"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
+            t0 = time.time()
+            while not self.lines and time.time() - t0 < 5.0:     # first sample before the timed region
+                time.sleep(0.01)
         except OSError:
             self.proc = None
 
@@ -179,7 +182,8 @@ def run_cuda(args):
     kw["seed"] = kw["seed"] + 100 * rank
     frame = synth.make_frame(**kw)
     params = dict(synth.DEFAULT_PARAMS)
-    P = lc.Params(**params)
+    modes = {"lazy": lc.MODE_LAZY, "dense": lc.MODE_DENSE}
+    P = {m: lc.Params(mode=v, **params) for m, v in modes.items()}
     h, w = frame.img.shape
     npx = h * w
 
@@ -191,8 +195,10 @@ def run_cuda(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
     stream = torch.cuda.current_stream()
 
-    def step():
-        lc.lacosmic_run_ws(img, P, mask_out=mask, clean_out=clean, workspace=ws, iter_counts=counts)
+    def make_step(mode):
+        def step():
+            lc.lacosmic_run_ws(img, P[mode], mask_out=mask, clean_out=clean, workspace=ws, iter_counts=counts)
+        return step
 
     def barrier():
         if world > 1:
@@ -218,25 +224,33 @@ def run_cuda(args):
             total_ms = float(t.item())
         return total_ms / steps
 
-    # ---- device-resident timing (value), with per-kernel event spans from the library
+    def measure(mode):
+        """value leg: K timed steps with the library's per-kernel event spans, then the same without."""
+        step = make_step(mode)
+        lc.lacosmic_kernel_timing_enable(True)
+        for _ in range(args.warmup):
+            step()
+        torch.cuda.synchronize()
+        lc.lacosmic_kernel_timing_read()         # drop warm-up spans
+        ms = timed(step, args.steps, 0)
+        kt = lc.lacosmic_kernel_timing_read()
+        lc.lacosmic_kernel_timing_enable(False)
+        launches = lc.lacosmic_last_launch_count()
+        ms_nospans = timed(step, args.steps, 1)
+        return dict(ms=ms, ms_nospans=ms_nospans, kt=kt, launches=launches,
+                    counts=counts.cpu().numpy().tolist(), mask=mask.clone(), clean=clean.clone())
+
+    # ---- device-resident timing (value): the production path, then the dense reference path
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
-    lc.lacosmic_kernel_timing_enable(True)
-    for _ in range(args.warmup):
-        step()
-    torch.cuda.synchronize()
-    lc.lacosmic_kernel_timing_read()         # drop warm-up spans
-    ms_step = timed(step, args.steps, 0)
-    ktimes = lc.lacosmic_kernel_timing_read()
-    lc.lacosmic_kernel_timing_enable(False)
-    launches_per_step = lc.lacosmic_last_launch_count()
-    clocks = sampler.stop() if rank == 0 else None
-    counts_host = counts.cpu().numpy().tolist()
-    mask_frac = float(mask.float().mean().item())
-
-    # the same region without the event spans (reported for transparency)
-    ms_step_nospans = timed(step, max(2, args.steps // 2), 1)
+    main_mode = args.mode
+    other_mode = "dense" if main_mode == "lazy" else "lazy"
+    res = measure(main_mode)
+    res_other = measure(other_mode)
+    modes_agree = bool(torch.equal(res["mask"], res_other["mask"]) and torch.equal(res["clean"], res_other["clean"])
+                       and res["counts"] == res_other["counts"])
+    mask_frac = float(res["mask"].float().mean().item())
 
     # ---- end to end through the host-buffer C-ABI call
     img_h = torch.from_numpy(frame.img).pin_memory()
@@ -245,44 +259,56 @@ def run_cuda(args):
     hws = torch.empty(lc.lacosmic_host_workspace_bytes(h, w), dtype=torch.uint8, device=dev)
 
     def step_host():
-        lc.lacosmic_run_host(img_h, P, mask_out_host=mask_h, clean_out_host=clean_h, dev_workspace=hws)
+        lc.lacosmic_run_host(img_h, P[main_mode], mask_out_host=mask_h, clean_out_host=clean_h, dev_workspace=hws)
 
     ms_e2e = timed(step_host, args.steps, max(1, args.warmup // 2))
-    same = bool((mask_h.numpy() == mask.cpu().numpy()).all() and
-                (clean_h.numpy() == clean.cpu().numpy()).all())
+    same = bool((mask_h.numpy() == res["mask"].cpu().numpy()).all() and
+                (clean_h.numpy() == res["clean"].cpu().numpy()).all())
+    clocks = sampler.stop() if rank == 0 else None
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
 
-    frames_per_s = world * 1e3 / ms_step
-    e2e_fps = world * 1e3 / ms_e2e
     niter = params["niter"]
-
-    # ---- roofline of the dominant kernel
-    dom = max((k for k in ktimes if k != "whole_frame"), key=lambda k: ktimes[k][0])
-    dom_ms, dom_spans = ktimes[dom]
-    dom_avg_ms = dom_ms / max(dom_spans, 1)
-    share = {k: round(v[0] / max(ktimes["whole_frame"][0], 1e-9), 4) for k, v in ktimes.items()
-             if k != "whole_frame"}
     sm_max = (clocks or {}).get("sm_max_mhz") or peaks["sm_max_mhz"]
     alu_peak = N_SM * ALU_LANES_PER_CLK_SM * sm_max * 1e6 / 1e12          # T min/max instr / s
-    ops_px = KERNEL_MINMAX_PER_PX.get(dom)
-    roof = None
-    if ops_px is not None:
+
+    def summarise(r):
+        kt = r["kt"]
+        whole = max(kt["whole_frame"][0], 1e-9)
+        return dict(frames_per_s=world * 1e3 / r["ms"], ms_per_step=r["ms"],
+                    ms_per_step_without_event_spans=r["ms_nospans"], launches_per_step=r["launches"],
+                    kernels_ms_per_step={k: round(v[0] / args.steps, 4) for k, v in kt.items() if v[1]},
+                    kernel_share_of_step={k: round(v[0] / whole, 4) for k, v in kt.items()
+                                          if k != "whole_frame" and v[1]})
+
+    def roofline(r):
+        """ALU roofline of the class with the largest summed time."""
+        kt = r["kt"]
+        dom = max((k for k in kt if k != "whole_frame"), key=lambda k: kt[k][0])
+        dom_ms, dom_spans = kt[dom]
+        dom_avg_ms = dom_ms / max(dom_spans, 1)
+        ops_px = KERNEL_MINMAX_PER_PX.get(dom)
+        if ops_px is None:
+            return None
         achieved = npx * ops_px / (dom_avg_ms * 1e-3) / 1e12
-        roof = dict(bound="alu", kernel=dom, achieved=achieved, peak=alu_peak,
-                    unit="T min/max instr/s", frac=achieved / alu_peak, traffic=(NCU_TRAFFIC_BYTES or {}).get(dom),
+        return dict(bound="alu", kernel=dom, achieved=achieved, peak=alu_peak, unit="T min/max instr/s",
+                    frac=achieved / alu_peak, traffic=(NCU_TRAFFIC_BYTES or {}).get(dom),
                     peak_source="148 SM x 64 ALU lanes/clk x %.0f MHz (DESIGN.md section 5; lanes/clk "
                                 "measured in profiles/r01_alu_minmax_microbench.txt)" % sm_max,
                     minmax_instr_per_px=ops_px, avg_launch_ms=dom_avg_ms, launches_timed=dom_spans)
-    hbm_bytes_step = npx * (HBM_BYTES_PER_PX_ITER * niter + HBM_BYTES_PER_PX_FRAME)
+
+    frames_per_s = world * 1e3 / res["ms"]
+    e2e_fps = world * 1e3 / ms_e2e
+    bytes_iter = HBM_BYTES_PER_PX_ITER[main_mode]
+    hbm_bytes_step = npx * (bytes_iter * niter + HBM_BYTES_PER_PX_FRAME)
     hbm = dict(algorithmic_bytes_per_step=hbm_bytes_step,
-               achieved_gbs=hbm_bytes_step / (ms_step * 1e-3) / 1e9 * 1.0,
+               achieved_gbs=hbm_bytes_step / (res["ms"] * 1e-3) / 1e9,
                peak_gbs=peaks["hbm_gbs"], peak_source=peaks["source"],
-               frac=hbm_bytes_step / (ms_step * 1e-3) / 1e9 / peaks["hbm_gbs"])
-    ref_cmp_rate = npx * REF_COMPARISONS_PER_PX_ITER * niter / (ms_step * 1e-3) / 1e12
+               frac=hbm_bytes_step / (res["ms"] * 1e-3) / 1e9 / peaks["hbm_gbs"])
+    ref_cmp_rate = npx * REF_COMPARISONS_PER_PX_ITER * niter / (res["ms"] * 1e-3) / 1e12
 
     # ---- the oracle on the host cores: a bounded sample of the same frame
     cpu = None
@@ -293,26 +319,29 @@ def run_cuda(args):
                    sample="top %d of %d rows of the same frame, one run, %.1f s; frames/s scaled by "
                           "pixel count" % (rows, h, dt))
 
+    main_sum = summarise(res)
     line = dict(
         metric=METRIC, value=frames_per_s, unit="frames/s", n_gpus=world, steps=args.steps,
-        warmup=args.warmup, ms_per_step=ms_step, higher_is_better=True, scaling="weak",
+        warmup=args.warmup, ms_per_step=res["ms"], higher_is_better=True, scaling="weak",
         vs_baseline=None, dtype="f32", data="synthetic",
         config=dict(workload=wl["label"], h=h, w=w, niter=niter, sigclip=params["sigclip"],
-                    sigfrac=params["sigfrac"], objlim=params["objlim"],
+                    sigfrac=params["sigfrac"], objlim=params["objlim"], mode=main_mode,
                     l2="flushed between steps (256 MiB write outside the event pair)",
                     parallelism="replicas (one frame per GPU, no collective)"),
         mpix_per_s=frames_per_s * npx / 1e6,
         e2e=dict(value=e2e_fps, unit="frames/s", h2d_bytes_per_step=npx * 4,
                  d2h_bytes_per_step=npx * 5, ms_per_step=ms_e2e, matches_device_path=same,
                  call="lacosmic_run_host (pinned host buffers)"),
-        gpu_launches=launches_per_step * args.steps,
-        launches_per_step=launches_per_step,
-        roofline=roof, hbm=hbm,
-        kernels_ms_per_step={k: round(v[0] / args.steps, 4) for k, v in ktimes.items()},
-        kernel_share_of_step=share,
-        ms_per_step_without_event_spans=ms_step_nospans,
+        gpu_launches=res["launches"] * args.steps,
+        launches_per_step=res["launches"],
+        roofline=roofline(res), hbm=hbm,
+        kernels_ms_per_step=main_sum["kernels_ms_per_step"],
+        kernel_share_of_step=main_sum["kernel_share_of_step"],
+        ms_per_step_without_event_spans=res["ms_nospans"],
         ref_comparisons_T_per_s=ref_cmp_rate,
-        new_cr_per_iteration=counts_host, mask_fraction=mask_frac,
+        other_mode=dict(mode=other_mode, same_mask_clean_counts=modes_agree, roofline=roofline(res_other),
+                        **summarise(res_other)),
+        new_cr_per_iteration=res["counts"], mask_fraction=mask_frac,
         clocks=clocks, cpu_baseline=cpu,
         context="paper (PAPER.md:31,47): 55 s/frame dfcosmic C++ at 2 threads on AWS; GPU variant on an "
                 "RTX 5060 Ti >10x faster than CPU variants (no absolute number in the text)",
@@ -325,15 +354,16 @@ def run_cuda(args):
 
 # ALU-pipe min/max instructions per output pixel of each kernel class (static SASS
 # count of FMNMX/FMNMX3 per pixel, halo recomputation included) -- the per-unit figure behind
-# roofline.achieved.  
+# roofline.achieved.
 KERNEL_MINMAX_PER_PX = {
     # generated networks (median_networks.cuh): med7 764/4, med5 326/4, med3 76/4 x 1.46 (haloed m3 tile)
     "fine_gates": 764 / 4 + 326 / 4 + 1.46 * 76 / 4,
     "noise_S": 326 / 4 + 13 / 4,                     # med5 + the clamp/floor selects of L+ and N
 }
-# HBM bytes per pixel the path must move with the current fusion:
-# noise_S: read work 4 + write S 4; fine_gates: read work 4 + S 4 + 0.375 bit-planes; dilate/replace ~1
-HBM_BYTES_PER_PX_ITER = 4 + 4 + 4 + 4 + 0.375 + 1.0
+# HBM bytes per pixel per iteration the path must move with the current fusion:
+# noise_S: read work 4 + write S 4; dense fine_gates: read work 4 + S 4 + 0.375 bit-planes; lazy: A1/A2
+# bit-planes 0.25 + list passes ~1; dilate/replace ~1
+HBM_BYTES_PER_PX_ITER = {"dense": 4 + 4 + 4 + 4 + 0.375 + 1.0, "lazy": 4 + 4 + 0.25 + 1.0 + 1.0}
 HBM_BYTES_PER_PX_FRAME = 8 + 1.125
 
 
@@ -344,6 +374,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="config2", choices=["config2", "config1", "config0"])
+    ap.add_argument("--mode", default="lazy", choices=["lazy", "dense"],
+                    help="which evaluation mode is the headline (the other is measured and reported too)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":

@@ -170,7 +170,7 @@ const char *lacosmic_version(void);
  * LACOSMIC_NUM_KERNEL_CLASSES, the summed device time ms_sum[c] and the number of spans[c] (HOST
  * arrays), and clears the record.  Class names: lacosmic_kernel_class_name(c); the last class is the
  * whole frame (copies included). */
-#define LACOSMIC_NUM_KERNEL_CLASSES 7
+#define LACOSMIC_NUM_KERNEL_CLASSES 8
 int lacosmic_kernel_timing_enable(int enable);
 int lacosmic_kernel_timing_read(float *ms_sum, int32_t *spans);
 const char *lacosmic_kernel_class_name(int cls);

@@ -23,7 +23,7 @@ EXPORTS = (
     "lacosmic_last_cuda_error", "lacosmic_last_launch_count", "lacosmic_version",
     "lacosmic_kernel_timing_enable", "lacosmic_kernel_timing_read", "lacosmic_kernel_class_name",
 )
-NUM_KERNEL_CLASSES = 7
+NUM_KERNEL_CLASSES = 8
 MODE_LAZY, MODE_DENSE = 0, 1
 
 

@@ -59,15 +59,22 @@ __device__ __forceinline__ float lplus_px(float c, float U, float D, float Lf, f
     return __fmul_rn(__fadd_rn(__fadd_rn(a, b), __fadd_rn(g, d)), 0.25f);
 }
 
-// ---- block-wide compaction of one 32-pixel word per thread into a pixel list ------------------------
-// All 256 threads of the CTA must call this.  Appends flat indices p0 + bit for every set bit of
-// `bits` (one atomicAdd per CTA).
-__device__ __forceinline__ void block_append(uint32_t bits, int p0, int* __restrict__ list,
-                                             int* __restrict__ nlist) {
+// ---- block-wide compaction of bit-plane words into a pixel list ------------------------------------
+// Bit-plane kernels use 256-thread CTAs (32 lanes x 8 warps); thread (lane, wi) of CTA (bx, by) owns the
+// BW_ROWS words (wx = 32 bx + lane, y = 64 by + 8 wi + i), i < BW_ROWS.  All 256 threads must call
+// block_append: it appends the flat pixel index of every set bit (one atomicAdd per CTA; same-address
+// atomics are what bounds a compaction pass, hence 2048 words per CTA).
+constexpr int BW_ROWS = 8;
+constexpr int BW_CTA_ROWS = 64;
+
+__device__ __forceinline__ void block_append(const uint32_t (&bits)[BW_ROWS], int p0, int w,
+                                             int* __restrict__ list, int* __restrict__ nlist) {
     __shared__ int s_warp[8];
     __shared__ int s_base;
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
-    const int n = __popc(bits);
+    int n = 0;
+#pragma unroll
+    for (int i = 0; i < BW_ROWS; ++i) n += __popc(bits[i]);
     int incl = n;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -88,10 +95,49 @@ __device__ __forceinline__ void block_append(uint32_t bits, int p0, int* __restr
     }
     __syncthreads();
     int base = s_base + s_warp[wi] + incl - n;
-    while (bits) {
-        int b = __ffs(bits) - 1;
-        bits &= bits - 1;
-        list[base++] = p0 + b;
+#pragma unroll
+    for (int i = 0; i < BW_ROWS; ++i) {
+        uint32_t b = bits[i];
+        const int pi = p0 + i * w;
+        while (b) {
+            int k = __ffs(b) - 1;
+            b &= b - 1;
+            list[base++] = pi + k;
+        }
+    }
+}
+
+// horizontal dilation by R pixels of the word vc given its left / right neighbour words
+template <int R>
+__device__ __forceinline__ uint32_t hdil(uint32_t vl, uint32_t vc, uint32_t vr) {
+    uint32_t o = vc;
+#pragma unroll
+    for (int k = 1; k <= R; ++k) o |= (vc << k) | (vc >> k) | (vl >> (32 - k)) | (vr << (32 - k));
+    return o;
+}
+
+// (2R+1) x (2R+1) dilation of a bit-plane at the BW_ROWS words a thread owns (rows y0 .. y0+BW_ROWS-1,
+// word column wx; outside the frame = 0): horizontally dilated rows are shared between the outputs
+template <int R>
+__device__ __forceinline__ void dilate_rows(const uint32_t* __restrict__ in, int y0, int wx, int h, int wpr,
+                                            uint32_t (&out)[BW_ROWS]) {
+    uint32_t hd[BW_ROWS + 2 * R];
+#pragma unroll
+    for (int r = 0; r < BW_ROWS + 2 * R; ++r) {
+        const int yy = y0 - R + r;
+        uint32_t v = 0;
+        if (yy >= 0 && yy < h) {
+            const uint32_t* row = in + (size_t)yy * wpr;
+            v = hdil<R>(wx > 0 ? row[wx - 1] : 0u, row[wx], wx + 1 < wpr ? row[wx + 1] : 0u);
+        }
+        hd[r] = v;
+    }
+#pragma unroll
+    for (int i = 0; i < BW_ROWS; ++i) {
+        uint32_t o = 0;
+#pragma unroll
+        for (int r = 0; r <= 2 * R; ++r) o |= hd[i + r];
+        out[i] = o;
     }
 }
 

@@ -110,7 +110,13 @@ struct NoiseArgs {
     float* dbgLp;
     float* dbgN;
     uint32_t *A1, *A2;       // nullable (lazy path): bit-planes ok & (S > sigclip), ok & (S > siglow)
-    const uint32_t* dirty;   // nullable: pixels whose `work` changed since S/A1/A2 were last written
+    // incremental pass (nullable): `dirty` = pixels whose `work` changed since S/A1/A2 were last written,
+    // tile_list/ntile = the tiles within 2 px of such a pixel, nneed = how many such pixels there are
+    const uint32_t* dirty;
+    const int* tile_list;
+    const int* ntile;
+    const int* nneed;
+    int dense_threshold;     // nneed >= this: nearly every unit is dirty, skip the per-unit test
     int h, w, wpr;
     float gain, rn2, sigclip, siglow, satlevel;
 };
@@ -124,35 +130,39 @@ __device__ __forceinline__ uint32_t nibbles_to_word(uint32_t nib, int lane) {
     return v;
 }
 
-// Does any pixel of `dirty` lie within 2 px (Chebyshev) of the 128 px of row y starting at x0?  S, A1 and
-// A2 at a pixel depend on `work` within that distance only (med5 window; L+ needs 1), so a warp whose
-// row segment is clean keeps the planes written by an earlier iteration.  Warp-uniform result.
-__device__ __forceinline__ bool row_segment_dirty(const uint32_t* __restrict__ dirty, int y, int x0, int h,
-                                                  int wpr, int lane) {
+// A warp computes one UNIT of 32 x 4 pixels at a time (lane = 8 quads x 4 rows).  Does any pixel of
+// `dirty` lie within 2 px (Chebyshev) of the unit at (yu, xu)?  S, A1 and A2 at a pixel depend on `work`
+// within that distance only (med5 window; L+ needs 1), so a clean unit keeps the values an earlier
+// iteration wrote.  Warp-uniform result.
+constexpr int UW = 32, UH = 4;
+__device__ __forceinline__ bool unit_dirty(const uint32_t* __restrict__ dirty, int yu, int xu, int h, int wpr,
+                                           int lane) {
     uint32_t v = 0;
-    if (lane < 30) {
-        const int r = y - 2 + lane / 6, k = lane % 6, wq = (x0 >> 5) - 1 + k;
+    if (lane < 3 * (UH + 4)) {
+        const int r = yu - 2 + lane / 3, k = lane % 3, wq = (xu >> 5) - 1 + k;
         if (r >= 0 && r < h && wq >= 0 && wq < wpr) {
             v = dirty[(size_t)r * wpr + wq];
             if (k == 0) v &= 0xC0000000u;
-            if (k == 5) v &= 0x00000003u;
+            if (k == 2) v &= 0x00000003u;
         }
     }
     return __any_sync(0xffffffffu, v != 0);
 }
 
 // sm: work tile with margins (NS_MX, NS_MY), edge-replicated
-__device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a, int x0, int y0, int lane,
-                                             int wi) {
+__device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a, bool check_dirty, int x0,
+                                             int y0, int lane, int wi) {
+    const int lx = lane & 7, lr = lane >> 3;
 #pragma unroll 1
-    for (int ly = wi; ly < TH; ly += NWARP) {
-        const int y = y0 + ly, x = x0 + 4 * lane;
-        if (y >= a.h) continue;                                                       // warp-uniform
-        if (a.dirty && !row_segment_dirty(a.dirty, y, x0, a.h, a.wpr, lane)) continue;   // warp-uniform
+    for (int u = wi; u < (TW / UW) * (TH / UH); u += NWARP) {
+        const int xu = x0 + (u & 3) * UW, lyu = (u >> 2) * UH, yu = y0 + lyu;
+        if (yu >= a.h || xu >= a.w) continue;                                            // warp-uniform
+        if (check_dirty && !unit_dirty(a.dirty, yu, xu, a.h, a.wpr, lane)) continue;     // warp-uniform
+        const int ly = lyu + lr, y = y0 + ly, x = xu + 4 * lx;
         uint32_t n1 = 0, n2 = 0;
-        if (x < a.w) {
+        if (y < a.h && x < a.w) {
             float win[8][5], m5[4], s[4], lp[4], n[4];
-            load_window<5, NS_PITCH>(sm + ly * NS_PITCH + 4 * lane, win);
+            load_window<5, NS_PITCH>(sm + ly * NS_PITCH + (x - x0), win);
             median5x5_x4(win, m5);
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
@@ -171,9 +181,8 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
         }
         if (a.A1) {
             const uint32_t b1 = nibbles_to_word(n1, lane), b2 = nibbles_to_word(n2, lane);
-            const int wx = (x0 >> 5) + (lane >> 3);
-            if ((lane & 7) == 0 && wx < a.wpr) {
-                size_t q = (size_t)y * a.wpr + wx;
+            if (lx == 0 && y < a.h) {
+                size_t q = (size_t)y * a.wpr + (xu >> 5);
                 a.A1[q] = b1;
                 a.A2[q] = b2;
             }
@@ -181,16 +190,27 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
     }
 }
 
+// incremental pass: is the per-unit test worth doing, and which tiles does this launch walk
+__device__ __forceinline__ bool noise_check_dirty(const NoiseArgs& a) {
+    return a.dirty && (!a.nneed || *a.nneed < a.dense_threshold);
+}
+
 // generic path (any w): one tile per CTA, tile loaded with clamped scalar loads
 __global__ void __launch_bounds__(NT)
-k_noise_S(const float* __restrict__ work, NoiseArgs a, const int* prev_count) {
+k_noise_S(const float* __restrict__ work, NoiseArgs a, int ntx, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;   // fixed point reached (R17)
     __shared__ __align__(16) float sm[NS_ROWS * NS_PITCH];
     const int tid = threadIdx.x;
-    const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
+    int t = blockIdx.x;
+    if (a.tile_list) {
+        if (t >= *a.ntile) return;
+        t = a.tile_list[t];
+    }
+    const int ty = t / ntx, tx = t - ty * ntx;
+    const int x0 = tx * TW, y0 = ty * TH;
     load_tile<NS_MX, NS_MY, NS_PITCH>(sm, work, a.h, a.w, y0, x0, tid);
     __syncthreads();
-    noise_S_tile(sm, a, x0, y0, tid & 31, tid >> 5);
+    noise_S_tile(sm, a, noise_check_dirty(a), x0, y0, tid & 31, tid >> 5);
 }
 
 // K_B: steps (3b)-(5).  S' = S - med5(S); m3 = med3(work) (tile in shared memory, replicated at the
@@ -361,7 +381,7 @@ __device__ __forceinline__ void replicate_fix(float* sm, int oy, int ox, int h, 
     }
 }
 
-__global__ void __launch_bounds__(NT)
+__global__ void __launch_bounds__(NT, 4)
 k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx, int ntiles,
               const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
@@ -376,17 +396,21 @@ k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx,
         fence_mbar_init();
     }
     __syncthreads();
+    const int nt = a.tile_list ? *a.ntile : ntiles;     // incremental pass: only the listed tiles
+    const bool check_dirty = noise_check_dirty(a);
+    auto tile_of = [&](int i) { return a.tile_list ? a.tile_list[i] : i; };
     auto issue = [&](int t, int st) {
         int ty = t / ntx, tx = t - ty * ntx;
         mbar_expect_tx(&full[st], TILE_BYTES);
         tma_load_2d(buf(st), &mapWork, tx * TW - NS_MX, ty * TH - NS_MY, &full[st]);
     };
-    int t = blockIdx.x;
-    if (tid == 0 && t < ntiles) issue(t, 0);
-    for (int it = 0; t < ntiles; t += gridDim.x, ++it) {
+    int i = blockIdx.x;
+    if (tid == 0 && i < nt) issue(tile_of(i), 0);
+    for (int it = 0; i < nt; i += gridDim.x, ++it) {
         const int st = it & 1;
-        if (tid == 0 && t + (int)gridDim.x < ntiles) issue(t + gridDim.x, st ^ 1);
+        if (tid == 0 && i + (int)gridDim.x < nt) issue(tile_of(i + gridDim.x), st ^ 1);
         mbar_wait(&full[st], (it >> 1) & 1);
+        const int t = tile_of(i);
         const int ty = t / ntx, tx = t - ty * ntx;
         const int x0 = tx * TW, y0 = ty * TH;
         if (y0 - NS_MY < 0 || y0 + TH + NS_MY > a.h || x0 - NS_MX < 0 || x0 + TW + NS_MX > a.w) {
@@ -394,7 +418,7 @@ k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx,
             fence_proxy_async();
             __syncthreads();
         }
-        noise_S_tile(buf(st), a, x0, y0, tid & 31, tid >> 5);
+        noise_S_tile(buf(st), a, check_dirty, x0, y0, tid & 31, tid >> 5);
         __syncthreads();   // stage st is free for the load issued at the top of the next iteration
     }
 }
@@ -448,63 +472,48 @@ k_fine_gates_tma(const __grid_constant__ CUtensorMap mapWork, const __grid_const
 }
 
 // ------------------------------------------------------------------------------------------------
-// Step (6) primitive on bit-planes: out = dil3(in) & gate.  One thread per 32-pixel word; the left
-// and right neighbour words come from the adjacent lanes by shuffle (lanes at a warp edge load
-// them).  If Cio is given: count += popc(out & ~C); C |= out  (R11).
+// Step (6) primitive on bit-planes: out = dil3(in) & gate.  Thread layout of common.cuh (8 words of one
+// column of words per thread; the horizontally dilated rows are shared between them).  If Cio is given:
+// count += popc(out & ~C); newp = out & ~C; C |= out  (R11), one atomicAdd per CTA.
 __global__ void __launch_bounds__(256)
 k_dilate_gate(const uint32_t* __restrict__ in, const uint32_t* __restrict__ gate,
               uint32_t* __restrict__ out, uint32_t* __restrict__ Cio, uint32_t* __restrict__ newp,
               int* __restrict__ count, int h, int w, int wpr, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
-    const int lane = threadIdx.x & 31;
-    int wx = blockIdx.x * 32 + lane;
-    int y = blockIdx.y * 8 + (threadIdx.x >> 5);
-    uint32_t v = 0, res = 0;
-    bool valid = (wx < wpr) && (y < h);
-    if (valid) {
-        v = in[(size_t)y * wpr + wx];
-        if (y > 0) v |= in[(size_t)(y - 1) * wpr + wx];
-        if (y + 1 < h) v |= in[(size_t)(y + 1) * wpr + wx];
-    }
-    uint32_t vl = __shfl_up_sync(0xffffffffu, v, 1), vr = __shfl_down_sync(0xffffffffu, v, 1);
-    if (valid) {
-        if (lane == 0) {
-            vl = 0;
-            if (wx > 0) {
-                vl = in[(size_t)y * wpr + wx - 1];
-                if (y > 0) vl |= in[(size_t)(y - 1) * wpr + wx - 1];
-                if (y + 1 < h) vl |= in[(size_t)(y + 1) * wpr + wx - 1];
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    const int wx = blockIdx.x * 32 + lane, y0 = blockIdx.y * BW_CTA_ROWS + wi * BW_ROWS;
+    int n = 0;
+    if (wx < wpr && y0 < h) {
+        uint32_t res[BW_ROWS];
+        dilate_rows<1>(in, y0, wx, h, wpr, res);
+        const int rem = w - wx * 32;
+        const uint32_t pad = rem >= 32 ? 0xffffffffu : ((1u << rem) - 1u);   // no gate: clear the pad bits
+#pragma unroll
+        for (int i = 0; i < BW_ROWS; ++i) {
+            const int y = y0 + i;
+            if (y >= h) break;
+            const size_t q = (size_t)y * wpr + wx;
+            const uint32_t r = res[i] & (gate ? gate[q] : pad);
+            out[q] = r;
+            if (Cio) {
+                const uint32_t c = Cio[q], fresh = r & ~c;
+                n += __popc(fresh);
+                if (fresh) Cio[q] = c | r;
+                newp[q] = fresh;      // pixels first flagged in this iteration
             }
         }
-        if (lane == 31 || wx + 1 >= wpr) {
-            vr = 0;
-            if (wx + 1 < wpr) {
-                vr = in[(size_t)y * wpr + wx + 1];
-                if (y > 0) vr |= in[(size_t)(y - 1) * wpr + wx + 1];
-                if (y + 1 < h) vr |= in[(size_t)(y + 1) * wpr + wx + 1];
-            }
-        }
-        res = v | (v << 1) | (v >> 1) | (vl >> 31) | (vr << 31);
-        uint32_t g;
-        if (gate) g = gate[(size_t)y * wpr + wx];
-        else {   // no gate: only clear the pad bits beyond column w-1
-            int rem = w - wx * 32;
-            g = rem >= 32 ? 0xffffffffu : ((1u << rem) - 1u);
-        }
-        res &= g;
-        out[(size_t)y * wpr + wx] = res;
     }
     if (Cio) {
-        int n = 0;
-        if (valid) {
-            uint32_t c = Cio[(size_t)y * wpr + wx];
-            uint32_t fresh = res & ~c;
-            n = __popc(fresh);
-            if (fresh) Cio[(size_t)y * wpr + wx] = c | res;
-            newp[(size_t)y * wpr + wx] = fresh;      // pixels first flagged in this iteration
-        }
+        __shared__ int s_n[8];
         n = __reduce_add_sync(0xffffffffu, n);
-        if (lane == 0 && n) atomicAdd(count, n);
+        if (lane == 0) s_n[wi] = n;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int tot = 0;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) tot += s_n[k];
+            if (tot) atomicAdd(count, tot);
+        }
     }
 }
 
@@ -519,29 +528,55 @@ k_dilate_gate(const uint32_t* __restrict__ in, const uint32_t* __restrict__ gate
 // pixel is in C -> 25-input sorting network -> middle element(s) of the k donors (R14-R16).
 __global__ void __launch_bounds__(256)
 k_build_list(const uint32_t* __restrict__ newp, const uint32_t* __restrict__ Cb, uint32_t* __restrict__ needp,
-             int* __restrict__ list, int* __restrict__ nlist, int h, int w, int wpr, const int* prev_count) {
+             uint8_t* __restrict__ tileflag, int ntx, int* __restrict__ list, int* __restrict__ nlist, int h,
+             int w, int wpr, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
-    const int lane = threadIdx.x & 31;
-    const int wx = blockIdx.x * 32 + lane;
-    const int y = blockIdx.y * 8 + (threadIdx.x >> 5);
-    uint32_t need = 0;
-    if (wx < wpr && y < h) {
-        const uint32_t c = Cb[(size_t)y * wpr + wx];
-        if (c) {
-            uint32_t vl = 0, vc = 0, vr = 0;
-            for (int yy = max(y - 2, 0); yy <= min(y + 2, h - 1); ++yy) {
-                const uint32_t* row = newp + (size_t)yy * wpr;
-                vc |= row[wx];
-                if (wx > 0) vl |= row[wx - 1];
-                if (wx + 1 < wpr) vr |= row[wx + 1];
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    const int wx = blockIdx.x * 32 + lane, y0 = blockIdx.y * BW_CTA_ROWS + wi * BW_ROWS;
+    uint32_t need[BW_ROWS];
+#pragma unroll
+    for (int i = 0; i < BW_ROWS; ++i) need[i] = 0;
+    if (wx < wpr && y0 < h) {
+        uint32_t spread[BW_ROWS];
+        dilate_rows<2>(newp, y0, wx, h, wpr, spread);
+#pragma unroll
+        for (int i = 0; i < BW_ROWS; ++i) {
+            const int y = y0 + i;
+            if (y >= h) break;
+            const size_t q = (size_t)y * wpr + wx;
+            need[i] = spread[i] & Cb[q];
+            if (needp) needp[q] = need[i];   // the pixels k_replace_list rewrites
+            if (need[i] && tileflag) {
+                // detect tiles (TW x TH) holding a pixel within 2 px of these: their S must be redone
+                const int tx0 = max(wx * 32 - 2, 0) / TW, tx1 = min(wx * 32 + 33, w - 1) / TW;
+                const int ty0 = max(y - 2, 0) / TH, ty1 = min(y + 2, h - 1) / TH;
+                tileflag[ty0 * ntx + tx0] = 1;
+                tileflag[ty0 * ntx + tx1] = 1;
+                tileflag[ty1 * ntx + tx0] = 1;
+                tileflag[ty1 * ntx + tx1] = 1;
             }
-            uint32_t spread = vc | (vc << 1) | (vc << 2) | (vc >> 1) | (vc >> 2) | (vl >> 31) | (vl >> 30) |
-                              (vr << 31) | (vr << 30);
-            need = spread & c;
         }
-        if (needp) needp[(size_t)y * wpr + wx] = need;   // the pixels k_replace_list rewrites
     }
-    block_append(need, y * w + wx * 32, list, nlist);
+    block_append(need, y0 * w + wx * 32, w, list, nlist);
+}
+
+// tile_list <- the tiles k_build_list flagged; flags are cleared for the next iteration
+__global__ void __launch_bounds__(256)
+k_tile_list(uint8_t* __restrict__ tileflag, int ntiles, int* __restrict__ tile_list, int* __restrict__ ntile,
+            const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;
+    const int t = blockIdx.x * 256 + threadIdx.x, lane = threadIdx.x & 31;
+    bool f = false;
+    if (t < ntiles) {
+        f = tileflag[t] != 0;
+        if (f) tileflag[t] = 0;
+    }
+    const uint32_t m = __ballot_sync(0xffffffffu, f);
+    if (!m) return;
+    int base = 0;
+    if (lane == 0) base = atomicAdd(ntile, __popc(m));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (f) tile_list[base + __popc(m & ((1u << lane) - 1u))] = t;
 }
 
 __global__ void __launch_bounds__(128)

@@ -26,7 +26,7 @@ inline bool cuda_ok(cudaError_t e) {
 
 // Optional per-kernel-class CUDA-event timing (lacosmic_kernel_timing_*): bench.py switches it on to
 // measure the dominant kernel's average launch duration on the launching stream.
-enum KClass { KC_NOISE_S = 0, KC_FINE_GATES, KC_DILATE, KC_REPLACE, KC_BITS, KC_LAZY, KC_STEP, KC_COUNT };
+enum KClass { KC_NOISE_S = 0, KC_FINE_GATES, KC_DILATE, KC_REPLACE, KC_BITS, KC_LAZY, KC_NOISE_S_INCR, KC_STEP, KC_COUNT };
 static_assert(KC_COUNT == LACOSMIC_NUM_KERNEL_CLASSES, "header and library disagree");
 struct KTiming {
     static constexpr int MAXSPANS = 8192;
@@ -144,9 +144,15 @@ struct Workspace {
     int32_t* nneed;    // per iteration: pixels (re)replaced
     int32_t* ncand;    // per iteration (lazy path): pixels of A1
     int32_t* nnb;      // per iteration (lazy path): neighbour pixels whose G2 was evaluated
-    size_t bytes;
+    int32_t* ntile;    // per iteration (lazy path): tiles the incremental noise/S pass walks
+    int32_t* tile_list;
+    uint8_t* tileflag; // one byte per TW x TH tile; zero between uses
+    size_t bytes;      // total
+    size_t zero_off, zero_bytes;   // region cleared at the start of a frame: counters and tile flags
 };
-constexpr int NCOUNTERS = 4 * LACOSMIC_MAX_NITER;
+constexpr int NCOUNTERS = 5 * LACOSMIC_MAX_NITER;
+inline int tiles_x(int w) { return (w + lac::TW - 1) / lac::TW; }
+inline int tiles_y(int h) { return (h + lac::TH - 1) / lac::TH; }
 
 Workspace carve(void* base, int h, int w) {
     Workspace ws;
@@ -158,10 +164,16 @@ Workspace carve(void* base, int h, int w) {
     ws.list = (int32_t*)(p + off); off += plane;
     uint32_t** planes[] = {&ws.G1, &ws.G2, &ws.M1, &ws.M2, &ws.M3, &ws.C, &ws.NEWP, &ws.A1, &ws.A2, &ws.NEED};
     for (uint32_t** pl : planes) { *pl = (uint32_t*)(p + off); off += bp; }
+    const size_t ntiles = (size_t)tiles_x(w) * tiles_y(h);
+    ws.tile_list = (int32_t*)(p + off); off += align_up(ntiles * 4, 256);
+    ws.zero_off = off;
     ws.counts = (int32_t*)(p + off); off += align_up(NCOUNTERS * 4, 256);
     ws.nneed = ws.counts + LACOSMIC_MAX_NITER;
     ws.ncand = ws.counts + 2 * LACOSMIC_MAX_NITER;
     ws.nnb = ws.counts + 3 * LACOSMIC_MAX_NITER;
+    ws.ntile = ws.counts + 4 * LACOSMIC_MAX_NITER;
+    ws.tileflag = (uint8_t*)(p + off); off += align_up(ntiles, 256);
+    ws.zero_bytes = off - ws.zero_off;
     ws.bytes = off;
     return ws;
 }
@@ -181,14 +193,17 @@ int unpack(const uint32_t* bits, uint8_t* u8, int h, int w, cudaStream_t st) {
     return LACOSMIC_OK;
 }
 
-// (re)compute work at every pixel of C whose 5x5 window holds a pixel of `newp`; `need_plane`
-// (nullable) receives the bit-plane of the pixels rewritten
+// grid of the bit-plane kernels: 32 words x 64 rows per CTA (common.cuh)
+inline dim3 bit_grid(int h, int w) { return dim3((words_per_row(w) + 31) / 32, (h + lac::BW_CTA_ROWS - 1) / lac::BW_CTA_ROWS); }
+
+// (re)compute work at every pixel of C whose 5x5 window holds a pixel of `newp`; `need_plane` (nullable)
+// receives the bit-plane of the pixels rewritten, `tileflag` (nullable) the tiles within 2 px of them
 int replace_pass(const float* img, const Workspace& ws, const uint32_t* newp, uint32_t* need_plane,
-                 int* nlist, float* work, int h, int w, const int* prev, cudaStream_t st) {
+                 uint8_t* tileflag, int* nlist, float* work, int h, int w, const int* prev, cudaStream_t st) {
     const int wpr = words_per_row(w);
-    dim3 dg((wpr + 31) / 32, (h + 7) / 8);
     Span sp(KC_REPLACE, st);
-    lac::k_build_list<<<dg, 256, 0, st>>>(newp, ws.C, need_plane, ws.list, nlist, h, w, wpr, prev);
+    lac::k_build_list<<<bit_grid(h, w), 256, 0, st>>>(newp, ws.C, need_plane, tileflag, tiles_x(w), ws.list, nlist,
+                                                     h, w, wpr, prev);
     LAUNCHED();
     lac::k_replace_list<<<list_grid(h, w, 128), 128, 0, st>>>(img, ws.C, work, ws.list, nlist, h, w, wpr, prev);
     LAUNCHED();
@@ -207,13 +222,13 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     // O0
     CK(cudaMemcpyAsync(work, img, P * 4, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemsetAsync(ws.C, 0, bp_bytes, st));
-    CK(cudaMemsetAsync(ws.counts, 0, NCOUNTERS * 4, st));
+    CK(cudaMemsetAsync((char*)ws.S + ws.zero_off, 0, ws.zero_bytes, st));   // counters, tile flags
     const float siglow = p.sigfrac * p.sigclip;   // R9: one fp32 multiply on the host
     const float rn2 = p.readnoise * p.readnoise;
     const bool lazy = p.mode == LACOSMIC_MODE_LAZY;
     lac::GateParams gp{p.sigclip, siglow, p.objlim, p.satlevel};
     dim3 tb(lac::NT), tg((w + lac::TW - 1) / lac::TW, (h + lac::TH - 1) / lac::TH);
-    dim3 dg((wpr + 31) / 32, (h + 7) / 8);
+    const dim3 dg = bit_grid(h, w);
     // TMA path needs 16-byte row pitch; other widths take the generic tile loader
     const bool tma = (w % 4 == 0);
     const int ntx = (int)tg.x, ntiles = (int)(tg.x * tg.y);
@@ -235,16 +250,24 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         const int* prev = t > 0 ? ws.counts + (t - 1) : nullptr;
         const bool d = dbg && dbg->iter == t;
         int rc;
+        // from the second iteration on S, A1, A2 only change near the pixels the previous replacement pass
+        // rewrote (ws.NEED); a debug dump recomputes everything
+        const bool incr = lazy && t > 0 && !d;
         lac::NoiseArgs na{ws.S, d ? dbg->Lp : nullptr, d ? dbg->N : nullptr,
                           lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
-                          // from the second iteration on S, A1, A2 only change near the pixels the previous
-                          // replacement pass rewrote (a debug dump recomputes everything)
-                          (lazy && t > 0 && !d) ? ws.NEED : nullptr,
+                          incr ? ws.NEED : nullptr, incr ? ws.tile_list : nullptr, incr ? ws.ntile + t : nullptr,
+                          incr ? ws.nneed + (t - 1) : nullptr, (int)std::max<size_t>(P / 64, 1),
                           h, w, wpr, p.gain, rn2, p.sigclip, siglow, p.satlevel};
+        if (lazy && t > 0) {
+            // always drain the tile flags the previous replacement pass set, even when `incr` is off
+            Span sp(KC_NOISE_S_INCR, st);
+            lac::k_tile_list<<<(ntiles + 255) / 256, 256, 0, st>>>(ws.tileflag, ntiles, ws.tile_list, ws.ntile + t, prev);
+            LAUNCHED();
+        }
         {
-            Span sp(KC_NOISE_S, st);
+            Span sp(na.dirty ? KC_NOISE_S_INCR : KC_NOISE_S, st);
             if (tma) lac::k_noise_S_tma<<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(mapWorkNS, na, ntx, ntiles, prev);
-            else lac::k_noise_S<<<tg, tb, 0, st>>>(work, na, prev);
+            else lac::k_noise_S<<<ntiles, tb, 0, st>>>(work, na, ntx, prev);
             LAUNCHED();
         }
         if (lazy) {
@@ -253,8 +276,8 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
             lac::CandArgs ca{ws.S, work, ws.G1, ws.G2, ws.M1, h, w, wpr, p.sigclip, siglow, p.objlim};
             {
                 Span sp(KC_LAZY, st);
-                lac::k_list_candidates<<<dg, 256, 0, st>>>(ws.A1, ws.G1, ws.G2, ws.M1, ws.list, ws.ncand + t,
-                                                          h, w, wpr, prev);
+                lac::k_list_candidates<<<dg, 256, 0, st>>>(ws.A1, t > 0 ? ws.NEED : nullptr, ws.G1, ws.G2, ws.M1,
+                                                          ws.list, ws.ncand + t, h, w, wpr, prev);
                 LAUNCHED();
                 lac::k_eval_candidates<<<list_grid(h, w, 128), 128, 0, st>>>(ca, ws.list, ws.ncand + t, prev);
                 LAUNCHED();
@@ -267,8 +290,8 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
             }
             {
                 Span sp(KC_LAZY, st);
-                lac::k_list_neighbours<<<dg, 256, 0, st>>>(ws.M2, ws.A1, ws.A2, ws.list, ws.nnb + t, h, w, wpr,
-                                                          prev);
+                lac::k_list_neighbours<<<dg, 256, 0, st>>>(ws.M2, ws.A1, ws.A2, ws.G2, ws.list, ws.nnb + t, h, w,
+                                                          wpr, prev);
                 LAUNCHED();
                 lac::k_eval_neighbours<<<list_grid(h, w, 128), 128, 0, st>>>(ws.S, ws.G2, h, w, wpr, siglow,
                                                                             ws.list, ws.nnb + t, prev);
@@ -300,7 +323,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
             }
         }
         if (d && dbg->S) CK(cudaMemcpyAsync(dbg->S, ws.S, P * 4, cudaMemcpyDeviceToDevice, st));
-        rc = replace_pass(img, ws, ws.NEWP, ws.NEED, ws.nneed + t, work, h, w, prev, st);
+        rc = replace_pass(img, ws, ws.NEWP, ws.NEED, lazy ? ws.tileflag : nullptr, ws.nneed + t, work, h, w, prev, st);
         if (rc) return rc;
         if (d) {
             // lazy path: G2 is only evaluated where step (6) needs it, so it is not dumped
@@ -492,8 +515,7 @@ int lacosmic_dilate3(const uint32_t* bits_in, uint32_t* bits_out, int h, int w, 
     if (rc) return rc;
     int wpr = words_per_row(w);
     if (overlap(bits_in, (size_t)h * wpr * 4, bits_out, (size_t)h * wpr * 4)) return LACOSMIC_ERR_ALIAS;
-    dim3 dg((wpr + 31) / 32, (h + 7) / 8);
-    lac::k_dilate_gate<<<dg, 256, 0, (cudaStream_t)stream>>>(bits_in, nullptr, bits_out, nullptr, nullptr,
+    lac::k_dilate_gate<<<bit_grid(h, w), 256, 0, (cudaStream_t)stream>>>(bits_in, nullptr, bits_out, nullptr, nullptr,
                                                            nullptr, h, w, wpr, nullptr);
     LAUNCHED();
     return LACOSMIC_OK;
@@ -513,7 +535,7 @@ int lacosmic_masked_median(const float* img, const uint8_t* mask_u8, float* out,
     if ((rc = lacosmic_pack_bits(mask_u8, ws.C, h, w, stream))) return rc;
     CK(cudaMemcpyAsync(out, img, P * 4, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemsetAsync(ws.nneed, 0, 4, st));
-    return replace_pass(img, ws, ws.C, nullptr, ws.nneed, out, h, w, nullptr, st);   // every masked pixel is "new"
+    return replace_pass(img, ws, ws.C, nullptr, nullptr, ws.nneed, out, h, w, nullptr, st);   // every masked pixel is "new"
 }
 
 // ---- diagnostics ------------------------------------------------------------------------------
@@ -557,7 +579,7 @@ int lacosmic_kernel_timing_read(float* ms_sum, int32_t* spans) {
 
 const char* lacosmic_kernel_class_name(int cls) {
     static const char* names[KC_COUNT] = {"noise_S", "fine_gates", "dilate_x2", "replace", "bits",
-                                          "lazy_eval", "whole_frame"};
+                                          "lazy_eval", "noise_S_incremental", "whole_frame"};
     return (cls >= 0 && cls < KC_COUNT) ? names[cls] : "?";
 }
 

@@ -22,52 +22,71 @@
 
 namespace lac {
 
-// 3x3 dilation of one word of a bit-plane (outside the frame = 0), neighbours loaded directly
-__device__ __forceinline__ uint32_t dil3_word(const uint32_t* __restrict__ in, int y, int wx, int h, int wpr) {
-    uint32_t vl = 0, vc = 0, vr = 0;
-    for (int yy = max(y - 1, 0); yy <= min(y + 1, h - 1); ++yy) {
-        const uint32_t* row = in + (size_t)yy * wpr;
-        vc |= row[wx];
-        if (wx > 0) vl |= row[wx - 1];
-        if (wx + 1 < wpr) vr |= row[wx + 1];
-    }
-    return vc | (vc << 1) | (vc >> 1) | (vl >> 31) | (vr << 31);
-}
+// Incremental evaluation: G1, G2, M1 persist across the iterations of a frame.  A test at pixel p reads
+// `work` within 4 px of p (S' : S within 2, each S from work within 2; fine structure: 9x9), so after the
+// replacement pass of iteration t-1 rewrote the pixels NEED, only the tests inside R = dil9x9(NEED) can
+// change: iteration t clears G1, G2, M1 inside R and re-evaluates the candidates there.
 
-// list <- pixels of A1; zero the words of G1, G2, M1 (they are filled by atomicOr afterwards)
+// list <- pixels of A1 & R; clear G1, G2, M1 inside R (R = everything when `dirty` is NULL)
 __global__ void __launch_bounds__(256)
-k_list_candidates(const uint32_t* __restrict__ A1, uint32_t* __restrict__ G1, uint32_t* __restrict__ G2,
-                  uint32_t* __restrict__ M1, int* __restrict__ list, int* __restrict__ nlist, int h, int w,
-                  int wpr, const int* prev_count) {
+k_list_candidates(const uint32_t* __restrict__ A1, const uint32_t* __restrict__ dirty, uint32_t* __restrict__ G1,
+                  uint32_t* __restrict__ G2, uint32_t* __restrict__ M1, int* __restrict__ list,
+                  int* __restrict__ nlist, int h, int w, int wpr, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
-    const int wx = blockIdx.x * 32 + (threadIdx.x & 31);
-    const int y = blockIdx.y * 8 + (threadIdx.x >> 5);
-    uint32_t bits = 0;
-    if (wx < wpr && y < h) {
-        size_t q = (size_t)y * wpr + wx;
-        bits = A1[q];
-        G1[q] = 0;
-        G2[q] = 0;
-        M1[q] = 0;
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    const int wx = blockIdx.x * 32 + lane, y0 = blockIdx.y * BW_CTA_ROWS + wi * BW_ROWS;
+    uint32_t bits[BW_ROWS];
+#pragma unroll
+    for (int i = 0; i < BW_ROWS; ++i) bits[i] = 0;
+    if (wx < wpr && y0 < h) {
+        uint32_t reg[BW_ROWS];
+        if (dirty) {
+            dilate_rows<4>(dirty, y0, wx, h, wpr, reg);
+        } else {
+#pragma unroll
+            for (int i = 0; i < BW_ROWS; ++i) reg[i] = 0xffffffffu;
+        }
+#pragma unroll
+        for (int i = 0; i < BW_ROWS; ++i) {
+            const int y = y0 + i;
+            if (y >= h) break;
+            const size_t q = (size_t)y * wpr + wx;
+            const uint32_t r = reg[i];
+            if (r == 0) continue;
+            bits[i] = A1[q] & r;
+            if (r == 0xffffffffu) {
+                G1[q] = 0; G2[q] = 0; M1[q] = 0;
+            } else {
+                G1[q] &= ~r; G2[q] &= ~r; M1[q] &= ~r;
+            }
+        }
     }
-    block_append(bits, y * w + wx * 32, list, nlist);
+    block_append(bits, y0 * w + wx * 32, w, list, nlist);
 }
 
-// list <- pixels of dil3(M2) & A2 & ~A1: the only pixels where G2 is still unknown and needed by O6
+// list <- pixels of dil3(M2) & A2 & ~A1 & ~G2: the only pixels where G2 is needed by O6 and not known
 __global__ void __launch_bounds__(256)
 k_list_neighbours(const uint32_t* __restrict__ M2, const uint32_t* __restrict__ A1,
-                  const uint32_t* __restrict__ A2, int* __restrict__ list, int* __restrict__ nlist, int h,
-                  int w, int wpr, const int* prev_count) {
+                  const uint32_t* __restrict__ A2, const uint32_t* __restrict__ G2, int* __restrict__ list,
+                  int* __restrict__ nlist, int h, int w, int wpr, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
-    const int wx = blockIdx.x * 32 + (threadIdx.x & 31);
-    const int y = blockIdx.y * 8 + (threadIdx.x >> 5);
-    uint32_t bits = 0;
-    if (wx < wpr && y < h) {
-        size_t q = (size_t)y * wpr + wx;
-        const uint32_t cand = A2[q] & ~A1[q];
-        if (cand) bits = dil3_word(M2, y, wx, h, wpr) & cand;
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    const int wx = blockIdx.x * 32 + lane, y0 = blockIdx.y * BW_CTA_ROWS + wi * BW_ROWS;
+    uint32_t bits[BW_ROWS];
+#pragma unroll
+    for (int i = 0; i < BW_ROWS; ++i) bits[i] = 0;
+    if (wx < wpr && y0 < h) {
+        uint32_t d[BW_ROWS];
+        dilate_rows<1>(M2, y0, wx, h, wpr, d);
+#pragma unroll
+        for (int i = 0; i < BW_ROWS; ++i) {
+            const int y = y0 + i;
+            if (y >= h) break;
+            const size_t q = (size_t)y * wpr + wx;
+            if (d[i]) bits[i] = d[i] & A2[q] & ~A1[q] & ~G2[q];
+        }
     }
-    block_append(bits, y * w + wx * 32, list, nlist);
+    block_append(bits, y0 * w + wx * 32, w, list, nlist);
 }
 
 // exact median of 9 (19 compare-exchanges)
@@ -85,9 +104,36 @@ __device__ __forceinline__ float med9(float a0, float a1, float a2, float a3, fl
     return fminf(a4, a2);
 }
 
-// #{25 clamped taps v of S around (y, x) : fsub(Sc, v) > thr} for thr = sigclip (c1) and siglow (c2)
-__device__ __forceinline__ void count_sp(const float* __restrict__ S, int y, int x, int h, int w,
-                                         float sigclip, float siglow, int& c1, int& c2) {
+__device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+
+// #{25 taps v of S around pixel p : fsub(Sc, v) > thr} for thr = sigclip (c1) and siglow (c2).
+// Interior pixels (window inside the frame): each window row is read as two 16-byte aligned vectors that
+// cover it, the test is evaluated on all 8 values and the 5 of the window are selected by a shift.
+__device__ __forceinline__ void count_sp_interior(const float* __restrict__ S, int p, int w, float sigclip,
+                                                  float siglow, int& c1, int& c2) {
+    const float sc = __ldg(S + p);
+    c1 = 0;
+    c2 = 0;
+#pragma unroll
+    for (int r = 0; r < 5; ++r) {
+        const int base = p + (r - 2) * w - 2, b = base & ~3, sh = base - b;
+        const float4 a0 = ldg4(S + b), a1 = ldg4(S + b + 4);
+        const float e[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+        uint32_t m1 = 0, m2 = 0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const float sp = __fsub_rn(sc, e[k]);
+            m1 |= (uint32_t)(sp > sigclip) << k;
+            m2 |= (uint32_t)(sp > siglow) << k;
+        }
+        c1 += __popc((m1 >> sh) & 31u);
+        c2 += __popc((m2 >> sh) & 31u);
+    }
+}
+
+// any pixel: clamped scalar taps (R3)
+__device__ __forceinline__ void count_sp_clamped(const float* __restrict__ S, int y, int x, int h, int w,
+                                                 float sigclip, float siglow, int& c1, int& c2) {
     const float sc = __ldg(S + (size_t)y * w + x);
     int xx[5];
 #pragma unroll
@@ -106,6 +152,14 @@ __device__ __forceinline__ void count_sp(const float* __restrict__ S, int y, int
     }
 }
 
+__device__ __forceinline__ void count_sp(const float* __restrict__ S, int y, int x, int h, int w, float sigclip,
+                                         float siglow, int& c1, int& c2) {
+    if (y >= 2 && x >= 2 && x + 2 < w && y + 2 < h && (size_t)(y + 2) * w + x + 6 <= (size_t)h * w)
+        count_sp_interior(S, y * w + x, w, sigclip, siglow, c1, c2);
+    else
+        count_sp_clamped(S, y, x, h, w, sigclip, siglow, c1, c2);
+}
+
 struct CandArgs {
     const float* S;
     const float* work;
@@ -114,13 +168,93 @@ struct CandArgs {
     float sigclip, siglow, objlim;
 };
 
-// One thread per pixel of A1: G1, G2 by counting; where G1 holds, the fine-structure test by counting.
+// P(v) of the header comment, with exactly the operations of O4/O5
+__device__ __forceinline__ bool fine_test(float lp, float m3c, float v, float objlim) {
+    const float d = __fsub_rn(m3c, v);
+    const float f = d > 0.01f ? d : 0.01f;
+    return __fdiv_rn(lp, f) > objlim;
+}
+
+// bit k = P(e[k]).  P is non-decreasing in v and (tlo, thi) brackets its switch point: P(v) is false for
+// v <= tlo and true for v >= thi (both verified by the caller with fine_test itself); only values strictly
+// inside the bracket need the division.  tlo = -inf, thi = +inf evaluates every value exactly.
+template <int N>
+__device__ __forceinline__ uint32_t fine_bits(const float (&e)[N], float lp, float m3c, float objlim, float tlo,
+                                              float thi) {
+    uint32_t m = 0, amb = 0;
+#pragma unroll
+    for (int k = 0; k < N; ++k) {
+        m |= (uint32_t)(e[k] >= thi) << k;
+        amb |= (uint32_t)((e[k] > tlo) & (e[k] < thi)) << k;
+    }
+    if (amb) {
+#pragma unroll
+        for (int k = 0; k < N; ++k)
+            if ((amb >> k) & 1u) m |= (uint32_t)fine_test(lp, m3c, e[k], objlim) << k;
+    }
+    return m;
+}
+
+// rows[r] bit c = P(V[r][c]) for the 9x9 window -> #{7x7 taps of the m3 plane with P} (see k_eval_candidates)
+__device__ __forceinline__ int fine_count(const uint32_t (&rows)[9], int y, int x, int h, int w) {
+    // ge5[ry] bit rx = (#P in the 3x3 block rows ry..ry+2, columns rx..rx+2) >= 5, bit-sliced adders
+    uint32_t ge5[7];
+#pragma unroll
+    for (int ry = 0; ry < 7; ++ry) {
+        const uint32_t b0 = rows[ry], b1 = rows[ry + 1], b2 = rows[ry + 2];
+        const uint32_t s0 = b0 ^ b1 ^ b2, s1 = (b0 & b1) | (b2 & (b0 | b1));      // column sums 0..3
+        const uint32_t l = s0 ^ (s0 >> 1) ^ (s0 >> 2);
+        const uint32_t cl = (s0 & (s0 >> 1)) | ((s0 >> 2) & (s0 | (s0 >> 1)));
+        const uint32_t hx = s1 ^ (s1 >> 1) ^ (s1 >> 2);
+        const uint32_t ch = (s1 & (s1 >> 1)) | ((s1 >> 2) & (s1 | (s1 >> 1)));
+        const uint32_t x1 = cl ^ hx, c1b = cl & hx;                                // total = l + 2 x1 + 4 (c1b + ch)
+        const uint32_t y0 = c1b ^ ch, y1 = c1b & ch;
+        ge5[ry] = (y1 | (y0 & (x1 | l))) & 0x7fu;
+    }
+    int cnt = 0;
+    if (y >= 3 && y + 3 < h && x >= 3 && x + 3 < w) {
+#pragma unroll
+        for (int ry = 0; ry < 7; ++ry) cnt += __popc(ge5[ry]);
+    } else {   // frame border: taps of the m3 plane repeat (clamped coordinates)
+        for (int dy = -3; dy <= 3; ++dy) {
+            const int ry = clampi(y + dy, 0, h - 1) - y + 3;
+            uint32_t g = 0;
+#pragma unroll
+            for (int r = 0; r < 7; ++r) g = (r == ry) ? ge5[r] : g;
+            for (int dx = -3; dx <= 3; ++dx) cnt += (g >> (clampi(x + dx, 0, w - 1) - x + 3)) & 1u;
+        }
+    }
+    return cnt;
+}
+
+// bracket of the switch point of P (see fine_bits); returns false when P is false everywhere
+__device__ __forceinline__ bool fine_bracket(float lp, float m3c, float objlim, float& tlo, float& thi) {
+    const float INF = __int_as_float(0x7f800000);
+    tlo = -INF;
+    thi = INF;
+    if (!(__fdiv_rn(lp, 0.01f) > objlim)) return false;        // F at its floor is the most favourable case
+    const float fs = lp / objlim;                               // F at the switch point, approximately
+    const float tau = m3c - fs;
+    const float mg = fmaxf(fabsf(m3c), fabsf(fs)) * 9.5367431640625e-07f;   // 2^-20: >= 8 ulp of either term
+    const float hi = tau + mg, lo = tau - mg;
+    if (fabsf(hi) < INF && fabsf(lo) < INF && fine_test(lp, m3c, hi, objlim) && !fine_test(lp, m3c, lo, objlim)) {
+        thi = hi;
+        tlo = lo;
+    }
+    return true;
+}
+
+// One thread per listed pixel of A1: G1, G2 by counting; where G1 holds, the fine-structure test by counting.
+// Virtual 9x9 window V[r][c] = work<y-4+r, x-4+c>; the m3-plane tap (dy, dx) of the 7x7 window is med3x3
+// centred on the virtual position (cy(dy), cx(dx)), cy(dy) = clamp(y+dy) - y (R4: the STORED m3 plane is
+// replicated), whose own taps are V[cy+4+-1][cx+4+-1] (R3).
 __global__ void __launch_bounds__(128)
 k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restrict__ nlist,
                   const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     const int n = *nlist;
     const int h = a.h, w = a.w;
+    const size_t npx = (size_t)h * w;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const int p = list[i];
         const int y = p / w, x = p - y * w;
@@ -131,67 +265,75 @@ k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restric
         if (c2 >= 13) atomicOr(a.G2 + q, bit);
         if (c1 < 13) continue;
         atomicOr(a.G1 + q, bit);
-        // fine-structure test.  Virtual 9x9 window V[r][c] = work<y-4+r, x-4+c>; the m3-plane tap (dy, dx)
-        // of the 7x7 window is med3x3 centred on the virtual position (cy(dy), cx(dx)) with
-        // cy(dy) = clamp(y+dy) - y (R4: the STORED m3 plane is replicated), whose own taps are
-        // V[cy+4+-1][cx+4+-1] (R3).
-        int xx[9];
-#pragma unroll
-        for (int c = 0; c < 9; ++c) xx[c] = clampi(x + c - 4, 0, w - 1);
-        float ctr[3][3];
-#pragma unroll
-        for (int r = 0; r < 3; ++r)
-#pragma unroll
-            for (int c = 0; c < 3; ++c)
-                ctr[r][c] = __ldg(a.work + (size_t)clampi(y + r - 1, 0, h - 1) * w + xx[3 + c]);
-        const float lp = lplus_px(ctr[1][1], ctr[0][1], ctr[2][1], ctr[1][0], ctr[1][2]);
-        const float m3c = med9(ctr[0][0], ctr[0][1], ctr[0][2], ctr[1][0], ctr[1][1], ctr[1][2], ctr[2][0],
-                               ctr[2][1], ctr[2][2]);
         uint32_t rows[9];   // bit c of rows[r] = P(V[r][c])
+        float tlo, thi;
+        if (y >= 4 && x >= 4 && x + 4 < w && y + 4 < h && (size_t)(y + 4) * w + x + 8 <= npx) {
+            // interior: every window row is covered by three 16-byte aligned vectors; P is evaluated on all
+            // 12 values and the 9 of the window are selected by a shift
+            float e[3][12];
+            int sh[3];
 #pragma unroll
-        for (int r = 0; r < 9; ++r) {
-            const float* row = a.work + (size_t)clampi(y + r - 4, 0, h - 1) * w;
-            uint32_t b = 0;
-#pragma unroll
-            for (int c = 0; c < 9; ++c) {
-                const float d = __fsub_rn(m3c, __ldg(row + xx[c]));
-                const float f = d > 0.01f ? d : 0.01f;
-                b |= (uint32_t)(__fdiv_rn(lp, f) > a.objlim) << c;
+            for (int r = 0; r < 3; ++r) {
+                const int base = p + (r - 1) * w - 4, b = base & ~3;
+                sh[r] = base - b;
+                const float4 a0 = ldg4(a.work + b), a1 = ldg4(a.work + b + 4), a2 = ldg4(a.work + b + 8);
+                e[r][0] = a0.x; e[r][1] = a0.y; e[r][2] = a0.z; e[r][3] = a0.w;
+                e[r][4] = a1.x; e[r][5] = a1.y; e[r][6] = a1.z; e[r][7] = a1.w;
+                e[r][8] = a2.x; e[r][9] = a2.y; e[r][10] = a2.z; e[r][11] = a2.w;
             }
-            rows[r] = b;
-        }
-        // ge5[ry] bit rx = (#P in the 3x3 block rows ry..ry+2, columns rx..rx+2) >= 5, bit-sliced adders
-        uint32_t ge5[7];
+            float ctr[3][3];   // work at rows y-1..y+1, columns x-1..x+1 = elements sh+3 .. sh+5
 #pragma unroll
-        for (int ry = 0; ry < 7; ++ry) {
-            const uint32_t b0 = rows[ry], b1 = rows[ry + 1], b2 = rows[ry + 2];
-            const uint32_t s0 = b0 ^ b1 ^ b2, s1 = (b0 & b1) | (b2 & (b0 | b1));      // column sums 0..3
-            const uint32_t l = s0 ^ (s0 >> 1) ^ (s0 >> 2);
-            const uint32_t cl = (s0 & (s0 >> 1)) | ((s0 >> 2) & (s0 | (s0 >> 1)));
-            const uint32_t hx = s1 ^ (s1 >> 1) ^ (s1 >> 2);
-            const uint32_t ch = (s1 & (s1 >> 1)) | ((s1 >> 2) & (s1 | (s1 >> 1)));
-            const uint32_t x1 = cl ^ hx, c1b = cl & hx;                                // total = l + 2 x1 + 4 (c1b + ch)
-            const uint32_t y0 = c1b ^ ch, y1 = c1b & ch;
-            ge5[ry] = (y1 | (y0 & (x1 | l))) & 0x7fu;
-        }
-        int cnt = 0;
-        if (y >= 3 && y + 3 < h && x >= 3 && x + 3 < w) {
+            for (int r = 0; r < 3; ++r)
 #pragma unroll
-            for (int ry = 0; ry < 7; ++ry) cnt += __popc(ge5[ry]);
-        } else {   // frame border: taps of the m3 plane repeat (clamped coordinates)
-            for (int dy = -3; dy <= 3; ++dy) {
-                const int ry = clampi(y + dy, 0, h - 1) - y + 3;
-                uint32_t g = 0;
+                for (int c = 0; c < 3; ++c) {
+                    const int s = sh[r];
+                    ctr[r][c] = s == 0 ? e[r][3 + c] : s == 1 ? e[r][4 + c] : s == 2 ? e[r][5 + c] : e[r][6 + c];
+                }
+            const float lp = lplus_px(ctr[1][1], ctr[0][1], ctr[2][1], ctr[1][0], ctr[1][2]);
+            const float m3c = med9(ctr[0][0], ctr[0][1], ctr[0][2], ctr[1][0], ctr[1][1], ctr[1][2], ctr[2][0],
+                                   ctr[2][1], ctr[2][2]);
+            if (!fine_bracket(lp, m3c, a.objlim, tlo, thi)) continue;
 #pragma unroll
-                for (int r = 0; r < 7; ++r) g = (r == ry) ? ge5[r] : g;
-                for (int dx = -3; dx <= 3; ++dx) cnt += (g >> (clampi(x + dx, 0, w - 1) - x + 3)) & 1u;
+            for (int r = 0; r < 9; ++r) {
+                if (r >= 3 && r <= 5) {
+                    rows[r] = (fine_bits<12>(e[r - 3], lp, m3c, a.objlim, tlo, thi) >> sh[r - 3]) & 0x1ffu;
+                } else {
+                    const int base = p + (r - 4) * w - 4, b = base & ~3;
+                    const float4 a0 = ldg4(a.work + b), a1 = ldg4(a.work + b + 4), a2 = ldg4(a.work + b + 8);
+                    const float f[12] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w, a2.x, a2.y, a2.z, a2.w};
+                    rows[r] = (fine_bits<12>(f, lp, m3c, a.objlim, tlo, thi) >> (base - b)) & 0x1ffu;
+                }
+            }
+        } else {
+            int xx[9];
+#pragma unroll
+            for (int c = 0; c < 9; ++c) xx[c] = clampi(x + c - 4, 0, w - 1);
+            float ctr[3][3];
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+                    ctr[r][c] = __ldg(a.work + (size_t)clampi(y + r - 1, 0, h - 1) * w + xx[3 + c]);
+            const float lp = lplus_px(ctr[1][1], ctr[0][1], ctr[2][1], ctr[1][0], ctr[1][2]);
+            const float m3c = med9(ctr[0][0], ctr[0][1], ctr[0][2], ctr[1][0], ctr[1][1], ctr[1][2], ctr[2][0],
+                                   ctr[2][1], ctr[2][2]);
+            if (!fine_bracket(lp, m3c, a.objlim, tlo, thi)) continue;
+#pragma unroll 1
+            for (int r = 0; r < 9; ++r) {
+                const float* row = a.work + (size_t)clampi(y + r - 4, 0, h - 1) * w;
+                float f[9];
+#pragma unroll
+                for (int c = 0; c < 9; ++c) f[c] = __ldg(row + xx[c]);
+                const uint32_t m = fine_bits<9>(f, lp, m3c, a.objlim, tlo, thi);
+#pragma unroll
+                for (int k = 0; k < 9; ++k) rows[k] = (k == r) ? m : rows[k];
             }
         }
-        if (cnt >= 25) atomicOr(a.M1 + q, bit);
+        if (fine_count(rows, y, x, h, w) >= 25) atomicOr(a.M1 + q, bit);
     }
 }
 
-// One thread per pixel of dil3(M2) & A2 & ~A1: G2 by counting.
+// One thread per pixel of dil3(M2) & A2 & ~A1 & ~G2: G2 by counting.
 __global__ void __launch_bounds__(128)
 k_eval_neighbours(const float* __restrict__ S, uint32_t* __restrict__ G2, int h, int w, int wpr, float siglow,
                   const int* __restrict__ list, const int* __restrict__ nlist, const int* prev_count) {
