@@ -287,12 +287,13 @@ def run_cuda(args):
     def roofline(r):
         """ALU roofline of the class with the largest summed time."""
         kt = r["kt"]
-        dom = max((k for k in kt if k != "whole_frame"), key=lambda k: kt[k][0])
+        # dominant kernel = the launch that takes longest (classes whose launches all process the full
+        # frame: their algorithmic work per launch is pixels x the per-pixel figure)
+        dom = max((k for k in kt if k in KERNEL_MINMAX_PER_PX and kt[k][1]),
+                  key=lambda k: kt[k][0] / kt[k][1])
         dom_ms, dom_spans = kt[dom]
         dom_avg_ms = dom_ms / max(dom_spans, 1)
-        ops_px = KERNEL_MINMAX_PER_PX.get(dom)
-        if ops_px is None:
-            return None
+        ops_px = KERNEL_MINMAX_PER_PX[dom]
         achieved = npx * ops_px / (dom_avg_ms * 1e-3) / 1e12
         return dict(bound="alu", kernel=dom, achieved=achieved, peak=alu_peak, unit="T min/max instr/s",
                     frac=achieved / alu_peak, traffic=(NCU_TRAFFIC_BYTES or {}).get(dom),
