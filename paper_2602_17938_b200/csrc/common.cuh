@@ -60,21 +60,23 @@ __device__ __forceinline__ float lplus_px(float c, float U, float D, float Lf, f
 }
 
 // ---- block-wide compaction of bit-plane words into a pixel list ------------------------------------
-// Bit-plane kernels use 256-thread CTAs (32 lanes x 8 warps); thread (lane, wi) of CTA (bx, by) owns the
-// BW_ROWS words (wx = 32 bx + lane, y = 64 by + 8 wi + i), i < BW_ROWS.  All 256 threads must call
-// block_append: it appends the flat pixel index of every set bit (one atomicAdd per CTA; same-address
-// atomics are what bounds a compaction pass, hence 2048 words per CTA).
+// Bit-plane kernels use 256-thread CTAs (32 lanes x 8 warps); thread (lane, wi) owns NR words of one word
+// column (word wx, rows y .. y+NR-1).  All 256 threads must call block_append: it appends the flat pixel
+// index p0 + i*w + k of every set bit k of bits[i] (one atomicAdd per CTA: same-address atomics serialise
+// in L2, so they are aggregated per CTA).  Contains block barriers; a second call in the same kernel must
+// be separated from the first by __syncthreads().
 constexpr int BW_ROWS = 8;
 constexpr int BW_CTA_ROWS = 64;
 
-__device__ __forceinline__ void block_append(const uint32_t (&bits)[BW_ROWS], int p0, int w,
+template <int NR>
+__device__ __forceinline__ void block_append(const uint32_t (&bits)[NR], int p0, int w,
                                              int* __restrict__ list, int* __restrict__ nlist) {
     __shared__ int s_warp[8];
     __shared__ int s_base;
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     int n = 0;
 #pragma unroll
-    for (int i = 0; i < BW_ROWS; ++i) n += __popc(bits[i]);
+    for (int i = 0; i < NR; ++i) n += __popc(bits[i]);
     int incl = n;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -96,7 +98,7 @@ __device__ __forceinline__ void block_append(const uint32_t (&bits)[BW_ROWS], in
     __syncthreads();
     int base = s_base + s_warp[wi] + incl - n;
 #pragma unroll
-    for (int i = 0; i < BW_ROWS; ++i) {
+    for (int i = 0; i < NR; ++i) {
         uint32_t b = bits[i];
         const int pi = p0 + i * w;
         while (b) {
@@ -122,15 +124,15 @@ template <int R>
 __device__ __forceinline__ void dilate_rows(const uint32_t* __restrict__ in, int y0, int wx, int h, int wpr,
                                             uint32_t (&out)[BW_ROWS]) {
     uint32_t hd[BW_ROWS + 2 * R];
+    const int wl = max(wx - 1, 0), wr = min(wx + 1, wpr - 1);
 #pragma unroll
     for (int r = 0; r < BW_ROWS + 2 * R; ++r) {
+        // branch-free: clamped addresses, masked values (all loads of a thread are in flight together)
         const int yy = y0 - R + r;
-        uint32_t v = 0;
-        if (yy >= 0 && yy < h) {
-            const uint32_t* row = in + (size_t)yy * wpr;
-            v = hdil<R>(wx > 0 ? row[wx - 1] : 0u, row[wx], wx + 1 < wpr ? row[wx + 1] : 0u);
-        }
-        hd[r] = v;
+        const bool ok = (yy >= 0) & (yy < h);
+        const uint32_t* row = in + (size_t)clampi(yy, 0, h - 1) * wpr;
+        const uint32_t vl = row[wl], vc = row[wx], vr = row[wr];
+        hd[r] = hdil<R>((ok & (wx > 0)) ? vl : 0u, ok ? vc : 0u, (ok & (wx + 1 < wpr)) ? vr : 0u);
     }
 #pragma unroll
     for (int i = 0; i < BW_ROWS; ++i) {

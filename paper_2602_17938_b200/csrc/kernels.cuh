@@ -110,13 +110,8 @@ struct NoiseArgs {
     float* dbgLp;
     float* dbgN;
     uint32_t *A1, *A2;       // nullable (lazy path): bit-planes ok & (S > sigclip), ok & (S > siglow)
-    // incremental pass (nullable): `dirty` = pixels whose `work` changed since S/A1/A2 were last written,
-    // tile_list/ntile = the tiles within 2 px of such a pixel, nneed = how many such pixels there are
-    const uint32_t* dirty;
-    const int* tile_list;
-    const int* ntile;
-    const int* nneed;
-    int dense_threshold;     // nneed >= this: nearly every unit is dirty, skip the per-unit test
+    float* copy_out;         // nullable: also write the input tile here (frame prologue work = img_in fused
+                             // into the first pass, which then reads img_in itself)
     int h, w, wpr;
     float gain, rn2, sigclip, siglow, satlevel;
 };
@@ -130,42 +125,27 @@ __device__ __forceinline__ uint32_t nibbles_to_word(uint32_t nib, int lane) {
     return v;
 }
 
-// A warp computes one UNIT of 32 x 4 pixels at a time (lane = 8 quads x 4 rows).  Does any pixel of
-// `dirty` lie within 2 px (Chebyshev) of the unit at (yu, xu)?  S, A1 and A2 at a pixel depend on `work`
-// within that distance only (med5 window; L+ needs 1), so a clean unit keeps the values an earlier
-// iteration wrote.  Warp-uniform result.
+// A warp computes one UNIT of 32 x 4 pixels at a time (lane = 8 quads x 4 rows), so that the 8 lanes of a
+// row assemble whole 32-pixel words of A1 / A2.
 constexpr int UW = 32, UH = 4;
-__device__ __forceinline__ bool unit_dirty(const uint32_t* __restrict__ dirty, int yu, int xu, int h, int wpr,
-                                           int lane) {
-    uint32_t v = 0;
-    if (lane < 3 * (UH + 4)) {
-        const int r = yu - 2 + lane / 3, k = lane % 3, wq = (xu >> 5) - 1 + k;
-        if (r >= 0 && r < h && wq >= 0 && wq < wpr) {
-            v = dirty[(size_t)r * wpr + wq];
-            if (k == 0) v &= 0xC0000000u;
-            if (k == 2) v &= 0x00000003u;
-        }
-    }
-    return __any_sync(0xffffffffu, v != 0);
-}
 
 // sm: work tile with margins (NS_MX, NS_MY), edge-replicated
-__device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a, bool check_dirty, int x0,
-                                             int y0, int lane, int wi) {
+__device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a, int x0, int y0, int lane,
+                                             int wi) {
     const int lx = lane & 7, lr = lane >> 3;
 #pragma unroll 1
     for (int u = wi; u < (TW / UW) * (TH / UH); u += NWARP) {
         const int xu = x0 + (u & 3) * UW, lyu = (u >> 2) * UH, yu = y0 + lyu;
         if (yu >= a.h || xu >= a.w) continue;                                            // warp-uniform
-        if (check_dirty && !unit_dirty(a.dirty, yu, xu, a.h, a.wpr, lane)) continue;     // warp-uniform
         const int ly = lyu + lr, y = y0 + ly, x = xu + 4 * lx;
         uint32_t n1 = 0, n2 = 0;
         if (y < a.h && x < a.w) {
-            float win[8][5], m5[4], s[4], lp[4], n[4];
+            float win[8][5], m5[4], s[4], lp[4], n[4], ctr[4];
             load_window<5, NS_PITCH>(sm + ly * NS_PITCH + (x - x0), win);
             median5x5_x4(win, m5);
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
+                ctr[j] = win[2 + j][2];
                 lp[j] = lplus_px(win[2 + j][2], win[2 + j][1], win[2 + j][3], win[1 + j][2], win[3 + j][2]);
                 float m5c = m5[j] > 1e-4f ? m5[j] : 1e-4f;                                 // R5
                 n[j] = __fdiv_rn(__fsqrt_rn(__fadd_rn(__fmul_rn(a.gain, m5c), a.rn2)), a.gain);
@@ -178,6 +158,7 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
             store4(a.S, ro, x, a.w, s);
             if (a.dbgLp) store4(a.dbgLp, ro, x, a.w, lp);
             if (a.dbgN) store4(a.dbgN, ro, x, a.w, n);
+            if (a.copy_out) store4(a.copy_out, ro, x, a.w, ctr);
         }
         if (a.A1) {
             const uint32_t b1 = nibbles_to_word(n1, lane), b2 = nibbles_to_word(n2, lane);
@@ -190,27 +171,18 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
     }
 }
 
-// incremental pass: is the per-unit test worth doing, and which tiles does this launch walk
-__device__ __forceinline__ bool noise_check_dirty(const NoiseArgs& a) {
-    return a.dirty && (!a.nneed || *a.nneed < a.dense_threshold);
-}
-
 // generic path (any w): one tile per CTA, tile loaded with clamped scalar loads
 __global__ void __launch_bounds__(NT)
 k_noise_S(const float* __restrict__ work, NoiseArgs a, int ntx, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;   // fixed point reached (R17)
     __shared__ __align__(16) float sm[NS_ROWS * NS_PITCH];
     const int tid = threadIdx.x;
-    int t = blockIdx.x;
-    if (a.tile_list) {
-        if (t >= *a.ntile) return;
-        t = a.tile_list[t];
-    }
+    const int t = blockIdx.x;
     const int ty = t / ntx, tx = t - ty * ntx;
     const int x0 = tx * TW, y0 = ty * TH;
     load_tile<NS_MX, NS_MY, NS_PITCH>(sm, work, a.h, a.w, y0, x0, tid);
     __syncthreads();
-    noise_S_tile(sm, a, noise_check_dirty(a), x0, y0, tid & 31, tid >> 5);
+    noise_S_tile(sm, a, x0, y0, tid & 31, tid >> 5);
 }
 
 // K_B: steps (3b)-(5).  S' = S - med5(S); m3 = med3(work) (tile in shared memory, replicated at the
@@ -396,9 +368,8 @@ k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx,
         fence_mbar_init();
     }
     __syncthreads();
-    const int nt = a.tile_list ? *a.ntile : ntiles;     // incremental pass: only the listed tiles
-    const bool check_dirty = noise_check_dirty(a);
-    auto tile_of = [&](int i) { return a.tile_list ? a.tile_list[i] : i; };
+    const int nt = ntiles;
+    auto tile_of = [&](int i) { return i; };
     auto issue = [&](int t, int st) {
         int ty = t / ntx, tx = t - ty * ntx;
         mbar_expect_tx(&full[st], TILE_BYTES);
@@ -418,7 +389,7 @@ k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx,
             fence_proxy_async();
             __syncthreads();
         }
-        noise_S_tile(buf(st), a, check_dirty, x0, y0, tid & 31, tid >> 5);
+        noise_S_tile(buf(st), a, x0, y0, tid & 31, tid >> 5);
         __syncthreads();   // stage st is free for the load issued at the top of the next iteration
     }
 }
@@ -472,162 +443,21 @@ k_fine_gates_tma(const __grid_constant__ CUtensorMap mapWork, const __grid_const
 }
 
 // ------------------------------------------------------------------------------------------------
-// Step (6) primitive on bit-planes: out = dil3(in) & gate.  Thread layout of common.cuh (8 words of one
-// column of words per thread; the horizontally dilated rows are shared between them).  If Cio is given:
-// count += popc(out & ~C); newp = out & ~C; C |= out  (R11), one atomicAdd per CTA.
+// Step (6) primitive on bit-planes (lacosmic_dilate3): out = dil3(in), pad bits cleared.  Thread layout of
+// common.cuh (8 words of one column of words per thread; the horizontally dilated rows are shared between
+// them).  The whole path runs the same word arithmetic inside k_grow_replace (grow.cuh).
 __global__ void __launch_bounds__(256)
-k_dilate_gate(const uint32_t* __restrict__ in, const uint32_t* __restrict__ gate,
-              uint32_t* __restrict__ out, uint32_t* __restrict__ Cio, uint32_t* __restrict__ newp,
-              int* __restrict__ count, int h, int w, int wpr, const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;
+k_dilate3(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, int h, int w, int wpr) {
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const int wx = blockIdx.x * 32 + lane, y0 = blockIdx.y * BW_CTA_ROWS + wi * BW_ROWS;
-    int n = 0;
-    if (wx < wpr && y0 < h) {
-        uint32_t res[BW_ROWS];
-        dilate_rows<1>(in, y0, wx, h, wpr, res);
-        const int rem = w - wx * 32;
-        const uint32_t pad = rem >= 32 ? 0xffffffffu : ((1u << rem) - 1u);   // no gate: clear the pad bits
+    if (wx >= wpr || y0 >= h) return;
+    uint32_t res[BW_ROWS];
+    dilate_rows<1>(in, y0, wx, h, wpr, res);
+    const int rem = w - wx * 32;
+    const uint32_t pad = rem >= 32 ? 0xffffffffu : ((1u << rem) - 1u);
 #pragma unroll
-        for (int i = 0; i < BW_ROWS; ++i) {
-            const int y = y0 + i;
-            if (y >= h) break;
-            const size_t q = (size_t)y * wpr + wx;
-            const uint32_t r = res[i] & (gate ? gate[q] : pad);
-            out[q] = r;
-            if (Cio) {
-                const uint32_t c = Cio[q], fresh = r & ~c;
-                n += __popc(fresh);
-                if (fresh) Cio[q] = c | r;
-                newp[q] = fresh;      // pixels first flagged in this iteration
-            }
-        }
-    }
-    if (Cio) {
-        __shared__ int s_n[8];
-        n = __reduce_add_sync(0xffffffffu, n);
-        if (lane == 0) s_n[wi] = n;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            int tot = 0;
-#pragma unroll
-            for (int k = 0; k < 8; ++k) tot += s_n[k];
-            if (tot) atomicAdd(count, tot);
-        }
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
-// Step (7): sparse masked-median replacement over a warp-compacted CR list.
-//
-// work[p] for p in C is a pure function of img_in and of C inside p's 5x5 window (R13), so after an
-// iteration only the pixels of C that have a NEWLY flagged pixel in their window need (re)computing;
-// all others already hold the right value.  k_build_list compacts exactly those pixels:
-//   need = dil5x5(newp) & C,   one thread per 32-pixel word, warp-aggregated append (one atomic per warp)
-// and k_replace_list gives each listed pixel to one thread: 25 clamped taps -> +inf where the tap's
-// pixel is in C -> 25-input sorting network -> middle element(s) of the k donors (R14-R16).
-__global__ void __launch_bounds__(256)
-k_build_list(const uint32_t* __restrict__ newp, const uint32_t* __restrict__ Cb, uint32_t* __restrict__ needp,
-             uint8_t* __restrict__ tileflag, int ntx, int* __restrict__ list, int* __restrict__ nlist, int h,
-             int w, int wpr, const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;
-    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
-    const int wx = blockIdx.x * 32 + lane, y0 = blockIdx.y * BW_CTA_ROWS + wi * BW_ROWS;
-    uint32_t need[BW_ROWS];
-#pragma unroll
-    for (int i = 0; i < BW_ROWS; ++i) need[i] = 0;
-    if (wx < wpr && y0 < h) {
-        uint32_t spread[BW_ROWS];
-        dilate_rows<2>(newp, y0, wx, h, wpr, spread);
-#pragma unroll
-        for (int i = 0; i < BW_ROWS; ++i) {
-            const int y = y0 + i;
-            if (y >= h) break;
-            const size_t q = (size_t)y * wpr + wx;
-            need[i] = spread[i] & Cb[q];
-            if (needp) needp[q] = need[i];   // the pixels k_replace_list rewrites
-            if (need[i] && tileflag) {
-                // detect tiles (TW x TH) holding a pixel within 2 px of these: their S must be redone
-                const int tx0 = max(wx * 32 - 2, 0) / TW, tx1 = min(wx * 32 + 33, w - 1) / TW;
-                const int ty0 = max(y - 2, 0) / TH, ty1 = min(y + 2, h - 1) / TH;
-                tileflag[ty0 * ntx + tx0] = 1;
-                tileflag[ty0 * ntx + tx1] = 1;
-                tileflag[ty1 * ntx + tx0] = 1;
-                tileflag[ty1 * ntx + tx1] = 1;
-            }
-        }
-    }
-    block_append(need, y0 * w + wx * 32, w, list, nlist);
-}
-
-// tile_list <- the tiles k_build_list flagged; flags are cleared for the next iteration
-__global__ void __launch_bounds__(256)
-k_tile_list(uint8_t* __restrict__ tileflag, int ntiles, int* __restrict__ tile_list, int* __restrict__ ntile,
-            const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;
-    const int t = blockIdx.x * 256 + threadIdx.x, lane = threadIdx.x & 31;
-    bool f = false;
-    if (t < ntiles) {
-        f = tileflag[t] != 0;
-        if (f) tileflag[t] = 0;
-    }
-    const uint32_t m = __ballot_sync(0xffffffffu, f);
-    if (!m) return;
-    int base = 0;
-    if (lane == 0) base = atomicAdd(ntile, __popc(m));
-    base = __shfl_sync(0xffffffffu, base, 0);
-    if (f) tile_list[base + __popc(m & ((1u << lane) - 1u))] = t;
-}
-
-__global__ void __launch_bounds__(128)
-k_replace_list(const float* __restrict__ img, const uint32_t* __restrict__ Cb, float* __restrict__ work,
-               const int* __restrict__ list, const int* __restrict__ nlist, int h, int w, int wpr,
-               const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;
-    const int n = *nlist;
-    const float INF = __int_as_float(0x7f800000);
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        const int p = list[i];
-        const int y = p / w, x = p - y * w;
-        int xx[5], yy[5];
-#pragma unroll
-        for (int d = 0; d < 5; ++d) {
-            xx[d] = clampi(x + d - 2, 0, w - 1);
-            yy[d] = clampi(y + d - 2, 0, h - 1);
-        }
-        // donor mask: bit (5*dy + dx) set when the (clamped) tap is NOT in C
-        uint32_t donors = 0;
-#pragma unroll
-        for (int dy = 0; dy < 5; ++dy) {
-            const uint32_t* row = Cb + (size_t)yy[dy] * wpr;
-            const int wl = xx[0] >> 5, wr = xx[4] >> 5;
-            const uint32_t cl = row[wl], cr = row[wr];
-#pragma unroll
-            for (int dx = 0; dx < 5; ++dx) {
-                uint32_t word = (xx[dx] >> 5) == wl ? cl : cr;
-                donors |= (((word >> (xx[dx] & 31)) & 1u) ^ 1u) << (5 * dy + dx);
-            }
-        }
-        if (donors == 0u) donors = 0x01ffffffu;            // R15: no donor -> all 25 taps
-        const int k = __popc(donors);
-        float v[25], s[25];
-#pragma unroll
-        for (int dy = 0; dy < 5; ++dy)
-#pragma unroll
-            for (int dx = 0; dx < 5; ++dx) {
-                float t = __ldg(img + (size_t)yy[dy] * w + xx[dx]);
-                v[5 * dy + dx] = ((donors >> (5 * dy + dx)) & 1u) ? t : INF;
-            }
-        sort25(v, s);
-        const int ihi = k >> 1, ilo = (k - 1) >> 1;
-        float lo = s[0], hi = s[0];
-#pragma unroll
-        for (int q = 1; q < 25; ++q) {
-            lo = (q == ilo) ? s[q] : lo;
-            hi = (q == ihi) ? s[q] : hi;
-        }
-        work[p] = (k & 1) ? hi : __fmul_rn(__fadd_rn(lo, hi), 0.5f);   // R14
-    }
+    for (int i = 0; i < BW_ROWS; ++i)
+        if (y0 + i < h) out[(size_t)(y0 + i) * wpr + wx] = res[i] & pad;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -8,6 +8,7 @@
 
 #include "kernels.cuh"
 #include "lazy.cuh"
+#include "grow.cuh"
 
 namespace {
 
@@ -26,7 +27,7 @@ inline bool cuda_ok(cudaError_t e) {
 
 // Optional per-kernel-class CUDA-event timing (lacosmic_kernel_timing_*): bench.py switches it on to
 // measure the dominant kernel's average launch duration on the launching stream.
-enum KClass { KC_NOISE_S = 0, KC_FINE_GATES, KC_DILATE, KC_REPLACE, KC_BITS, KC_LAZY, KC_NOISE_S_INCR, KC_STEP, KC_COUNT };
+enum KClass { KC_NOISE_S = 0, KC_FINE_GATES, KC_GROW, KC_LISTS, KC_BITS, KC_EVAL, KC_NOISE_S_QUADS, KC_STEP, KC_COUNT };
 static_assert(KC_COUNT == LACOSMIC_NUM_KERNEL_CLASSES, "header and library disagree");
 struct KTiming {
     static constexpr int MAXSPANS = 8192;
@@ -86,7 +87,7 @@ bool make_map(CUtensorMap* m, const float* base, int h, int w, int boxW, int box
 }
 
 struct DeviceInfo {
-    int sms = 0, occ_noise = 0, occ_fine = 0;
+    int sms = 0, occ_noise = 0, occ_fine = 0, occ_quads = 0, occ_eval = 0;
     bool ok = false;
 };
 
@@ -104,7 +105,9 @@ const DeviceInfo& device_info() {
                                                           lac::FG_SMEM_BYTES) != cudaSuccess) return d;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_noise, lac::k_noise_S_tma, lac::NT,
                                                           lac::NS_SMEM_BYTES) != cudaSuccess) return d;
-        d.ok = d.sms > 0 && d.occ_fine > 0 && d.occ_noise > 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_quads, lac::k_noise_S_quads, 256, 0) != cudaSuccess) return d;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_eval, lac::k_eval_candidates, 128, 0) != cudaSuccess) return d;
+        d.ok = d.sms > 0 && d.occ_fine > 0 && d.occ_noise > 0 && d.occ_quads > 0 && d.occ_eval > 0;
         return d;
     }();
     return info;
@@ -138,21 +141,16 @@ inline bool overlap(const void* a, size_t na, const void* b, size_t nb) {
 // Workspace layout (all offsets 256-byte aligned)
 struct Workspace {
     float* S;          // significance plane; persistent across the iterations of a frame
-    int32_t* list;     // compacted pixel list (capacity h*w), reused by every list pass of an iteration
-    uint32_t *G1, *G2, *M1, *M2, *M3, *C, *NEWP, *A1, *A2, *NEED;
+    int32_t* clist;    // compacted candidate pixel list (capacity h*w)
+    int32_t* qlist;    // compacted quad list of the incremental noise/S pass (capacity h*ceil(w/4))
+    uint32_t *G1, *G2, *M1, *M2, *M3, *C[2], *A1, *A2, *NEED;
     int32_t* counts;   // per iteration: newly flagged pixels
-    int32_t* nneed;    // per iteration: pixels (re)replaced
-    int32_t* ncand;    // per iteration (lazy path): pixels of A1
-    int32_t* nnb;      // per iteration (lazy path): neighbour pixels whose G2 was evaluated
-    int32_t* ntile;    // per iteration (lazy path): tiles the incremental noise/S pass walks
-    int32_t* tile_list;
-    uint8_t* tileflag; // one byte per TW x TH tile; zero between uses
+    int32_t* ncand;    // per iteration (lazy path): candidate pixels evaluated
+    int32_t* nquad;    // per iteration (lazy path): quads the incremental noise/S pass recomputed
     size_t bytes;      // total
-    size_t zero_off, zero_bytes;   // region cleared at the start of a frame: counters and tile flags
+    size_t zero_off, zero_bytes;   // region cleared at the start of a frame: the counters
 };
-constexpr int NCOUNTERS = 5 * LACOSMIC_MAX_NITER;
-inline int tiles_x(int w) { return (w + lac::TW - 1) / lac::TW; }
-inline int tiles_y(int h) { return (h + lac::TH - 1) / lac::TH; }
+constexpr int NCOUNTERS = 3 * LACOSMIC_MAX_NITER;
 
 Workspace carve(void* base, int h, int w) {
     Workspace ws;
@@ -161,28 +159,17 @@ Workspace carve(void* base, int h, int w) {
     char* p = (char*)base;
     size_t off = 0;
     ws.S = (float*)(p + off); off += plane;
-    ws.list = (int32_t*)(p + off); off += plane;
-    uint32_t** planes[] = {&ws.G1, &ws.G2, &ws.M1, &ws.M2, &ws.M3, &ws.C, &ws.NEWP, &ws.A1, &ws.A2, &ws.NEED};
+    ws.clist = (int32_t*)(p + off); off += plane;
+    ws.qlist = (int32_t*)(p + off); off += align_up((size_t)h * ((w + 3) / 4) * 4, 256);
+    uint32_t** planes[] = {&ws.G1, &ws.G2, &ws.M1, &ws.M2, &ws.M3, &ws.C[0], &ws.C[1], &ws.A1, &ws.A2, &ws.NEED};
     for (uint32_t** pl : planes) { *pl = (uint32_t*)(p + off); off += bp; }
-    const size_t ntiles = (size_t)tiles_x(w) * tiles_y(h);
-    ws.tile_list = (int32_t*)(p + off); off += align_up(ntiles * 4, 256);
     ws.zero_off = off;
     ws.counts = (int32_t*)(p + off); off += align_up(NCOUNTERS * 4, 256);
-    ws.nneed = ws.counts + LACOSMIC_MAX_NITER;
-    ws.ncand = ws.counts + 2 * LACOSMIC_MAX_NITER;
-    ws.nnb = ws.counts + 3 * LACOSMIC_MAX_NITER;
-    ws.ntile = ws.counts + 4 * LACOSMIC_MAX_NITER;
-    ws.tileflag = (uint8_t*)(p + off); off += align_up(ntiles, 256);
+    ws.ncand = ws.counts + LACOSMIC_MAX_NITER;
+    ws.nquad = ws.counts + 2 * LACOSMIC_MAX_NITER;
     ws.zero_bytes = off - ws.zero_off;
     ws.bytes = off;
     return ws;
-}
-
-int list_grid(int h, int w, int threads) {
-    int dev = 0, sms = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    long long want = ((long long)h * w / 64 + threads - 1) / threads;      // enough threads for a 1.6 % list
-    return (int)std::max(1LL, std::min((long long)sms * 16, want));
 }
 
 int unpack(const uint32_t* bits, uint8_t* u8, int h, int w, cudaStream_t st) {
@@ -193,19 +180,15 @@ int unpack(const uint32_t* bits, uint8_t* u8, int h, int w, cudaStream_t st) {
     return LACOSMIC_OK;
 }
 
-// grid of the bit-plane kernels: 32 words x 64 rows per CTA (common.cuh)
+// grid of the bit-plane list kernels: 32 words x 64 rows per CTA (common.cuh)
 inline dim3 bit_grid(int h, int w) { return dim3((words_per_row(w) + 31) / 32, (h + lac::BW_CTA_ROWS - 1) / lac::BW_CTA_ROWS); }
+// grid of k_grow_replace / k_dirty_lists: 32 words x 32 rows per CTA (grow.cuh)
+inline dim3 grow_grid(int h, int w) { return dim3((words_per_row(w) + lac::GT_W - 1) / lac::GT_W, (h + lac::GT_H - 1) / lac::GT_H); }
 
-// (re)compute work at every pixel of C whose 5x5 window holds a pixel of `newp`; `need_plane` (nullable)
-// receives the bit-plane of the pixels rewritten, `tileflag` (nullable) the tiles within 2 px of them
-int replace_pass(const float* img, const Workspace& ws, const uint32_t* newp, uint32_t* need_plane,
-                 uint8_t* tileflag, int* nlist, float* work, int h, int w, const int* prev, cudaStream_t st) {
-    const int wpr = words_per_row(w);
-    Span sp(KC_REPLACE, st);
-    lac::k_build_list<<<bit_grid(h, w), 256, 0, st>>>(newp, ws.C, need_plane, tileflag, tiles_x(w), ws.list, nlist,
-                                                     h, w, wpr, prev);
-    LAUNCHED();
-    lac::k_replace_list<<<list_grid(h, w, 128), 128, 0, st>>>(img, ws.C, work, ws.list, nlist, h, w, wpr, prev);
+// steps (6)-(7) of one iteration, fused (grow.cuh)
+int grow_replace(const lac::GrowArgs& ga, const int* prev, cudaStream_t st) {
+    Span sp(KC_GROW, st);
+    lac::k_grow_replace<<<grow_grid(ga.h, ga.w), 256, 0, st>>>(ga, prev);
     LAUNCHED();
     return LACOSMIC_OK;
 }
@@ -219,122 +202,106 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     const size_t bp_bytes = (size_t)h * wpr * 4;
     float* work = clean_out;
     Span whole(KC_STEP, st);   // the whole frame, copies included
-    // O0
-    CK(cudaMemcpyAsync(work, img, P * 4, cudaMemcpyDeviceToDevice, st));
-    CK(cudaMemsetAsync(ws.C, 0, bp_bytes, st));
-    CK(cudaMemsetAsync((char*)ws.S + ws.zero_off, 0, ws.zero_bytes, st));   // counters, tile flags
+    const bool lazy = p.mode == LACOSMIC_MODE_LAZY;
+    // O0.  The lazy path fuses work = img_in into its first pass (which then reads img_in itself).
+    const bool fused_copy = lazy && p.niter > 0;
+    if (!fused_copy) CK(cudaMemcpyAsync(work, img, P * 4, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemsetAsync(ws.C[0], 0, bp_bytes, st));
+    CK(cudaMemsetAsync((char*)ws.S + ws.zero_off, 0, ws.zero_bytes, st));   // counters
     const float siglow = p.sigfrac * p.sigclip;   // R9: one fp32 multiply on the host
     const float rn2 = p.readnoise * p.readnoise;
-    const bool lazy = p.mode == LACOSMIC_MODE_LAZY;
     lac::GateParams gp{p.sigclip, siglow, p.objlim, p.satlevel};
     dim3 tb(lac::NT), tg((w + lac::TW - 1) / lac::TW, (h + lac::TH - 1) / lac::TH);
-    const dim3 dg = bit_grid(h, w);
     // TMA path needs 16-byte row pitch; other widths take the generic tile loader
     const bool tma = (w % 4 == 0);
     const int ntx = (int)tg.x, ntiles = (int)(tg.x * tg.y);
-    CUtensorMap mapWorkNS, mapWorkFG, mapS;
-    int gridNS = 0, gridFG = 0;
-    if (tma && p.niter > 0) {
+    CUtensorMap mapWorkNS, mapImgNS, mapWorkFG, mapS;
+    int gridNS = 0, gridFG = 0, gridQ = 1184, gridE = 2368;
+    if (p.niter > 0) {
         const DeviceInfo& di = device_info();
         if (!di.ok) { g_last_cuda_error = (int)cudaGetLastError(); return LACOSMIC_ERR_CUDA; }
-        if (!make_map(&mapWorkNS, work, h, w, lac::NS_PITCH, lac::NS_ROWS) ||
-            !make_map(&mapWorkFG, work, h, w, lac::FG_PA, lac::FG_AROWS) ||
-            !make_map(&mapS, ws.S, h, w, lac::FG_PS, lac::FG_SROWS)) {
-            g_last_cuda_error = (int)cudaErrorInvalidValue;
-            return LACOSMIC_ERR_CUDA;
+        gridQ = di.sms * di.occ_quads;
+        gridE = di.sms * di.occ_eval;
+        if (tma) {
+            if (!make_map(&mapWorkNS, work, h, w, lac::NS_PITCH, lac::NS_ROWS) ||
+                !make_map(&mapImgNS, img, h, w, lac::NS_PITCH, lac::NS_ROWS) ||
+                !make_map(&mapWorkFG, work, h, w, lac::FG_PA, lac::FG_AROWS) ||
+                !make_map(&mapS, ws.S, h, w, lac::FG_PS, lac::FG_SROWS)) {
+                g_last_cuda_error = (int)cudaErrorInvalidValue;
+                return LACOSMIC_ERR_CUDA;
+            }
+            gridNS = std::min(ntiles, di.sms * di.occ_noise);
+            gridFG = std::min(ntiles, di.sms * di.occ_fine);
         }
-        gridNS = std::min(ntiles, di.sms * di.occ_noise);
-        gridFG = std::min(ntiles, di.sms * di.occ_fine);
     }
     for (int t = 0; t < p.niter; ++t) {
         const int* prev = t > 0 ? ws.counts + (t - 1) : nullptr;
         const bool d = dbg && dbg->iter == t;
         int rc;
-        // from the second iteration on S, A1, A2 only change near the pixels the previous replacement pass
-        // rewrote (ws.NEED); a debug dump recomputes everything
+        // lazy path, t >= 1: S, A1, A2 and the tests only change near the pixels the previous replacement
+        // rewrote (ws.NEED); a debug dump recomputes the planes everywhere
         const bool incr = lazy && t > 0 && !d;
         lac::NoiseArgs na{ws.S, d ? dbg->Lp : nullptr, d ? dbg->N : nullptr,
                           lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
-                          incr ? ws.NEED : nullptr, incr ? ws.tile_list : nullptr, incr ? ws.ntile + t : nullptr,
-                          incr ? ws.nneed + (t - 1) : nullptr, (int)std::max<size_t>(P / 64, 1),
+                          (fused_copy && t == 0) ? work : nullptr,
                           h, w, wpr, p.gain, rn2, p.sigclip, siglow, p.satlevel};
-        if (lazy && t > 0) {
-            // always drain the tile flags the previous replacement pass set, even when `incr` is off
-            Span sp(KC_NOISE_S_INCR, st);
-            lac::k_tile_list<<<(ntiles + 255) / 256, 256, 0, st>>>(ws.tileflag, ntiles, ws.tile_list, ws.ntile + t, prev);
-            LAUNCHED();
-        }
-        {
-            Span sp(na.dirty ? KC_NOISE_S_INCR : KC_NOISE_S, st);
-            if (tma) lac::k_noise_S_tma<<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(mapWorkNS, na, ntx, ntiles, prev);
-            else lac::k_noise_S<<<ntiles, tb, 0, st>>>(work, na, ntx, prev);
-            LAUNCHED();
-        }
-        if (lazy) {
-            // steps (3b)-(5) on the pixels of A1 only (lazy.cuh), then the two gated growths; G2 is
-            // evaluated on the further pixels the second growth can reach
-            lac::CandArgs ca{ws.S, work, ws.G1, ws.G2, ws.M1, h, w, wpr, p.sigclip, siglow, p.objlim};
+        if (incr) {
             {
-                Span sp(KC_LAZY, st);
-                lac::k_list_candidates<<<dg, 256, 0, st>>>(ws.A1, t > 0 ? ws.NEED : nullptr, ws.G1, ws.G2, ws.M1,
-                                                          ws.list, ws.ncand + t, h, w, wpr, prev);
-                LAUNCHED();
-                lac::k_eval_candidates<<<list_grid(h, w, 128), 128, 0, st>>>(ca, ws.list, ws.ncand + t, prev);
+                Span sp(KC_LISTS, st);
+                lac::k_dirty_lists<<<grow_grid(h, w), 256, 0, st>>>(ws.NEED, ws.A1, ws.G1, ws.G2, ws.M1, ws.qlist,
+                                                                   ws.nquad + t, ws.clist, ws.ncand + t, h, w, wpr, prev);
                 LAUNCHED();
             }
             {
-                Span sp(KC_DILATE, st);
-                lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M1, ws.G1, ws.M2, nullptr, nullptr, nullptr, h, w,
-                                                      wpr, prev);
-                LAUNCHED();
-            }
-            {
-                Span sp(KC_LAZY, st);
-                lac::k_list_neighbours<<<dg, 256, 0, st>>>(ws.M2, ws.A1, ws.A2, ws.G2, ws.list, ws.nnb + t, h, w,
-                                                          wpr, prev);
-                LAUNCHED();
-                lac::k_eval_neighbours<<<list_grid(h, w, 128), 128, 0, st>>>(ws.S, ws.G2, h, w, wpr, siglow,
-                                                                            ws.list, ws.nnb + t, prev);
-                LAUNCHED();
-            }
-            {
-                Span sp(KC_DILATE, st);
-                lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M2, ws.G2, ws.M3, ws.C, ws.NEWP, ws.counts + t, h, w,
-                                                      wpr, prev);
+                Span sp(KC_NOISE_S_QUADS, st);
+                lac::k_noise_S_quads<<<gridQ, 256, 0, st>>>(work, na, ws.qlist, ws.nquad + t, ws.clist, ws.ncand + t, prev);
                 LAUNCHED();
             }
         } else {
-            lac::FineArgs fa{ws.G1, ws.G2, ws.M1, d ? dbg->Sp : nullptr, d ? dbg->m3 : nullptr,
-                             d ? dbg->F : nullptr, h, w, wpr, gp};
+            const float* src = (fused_copy && t == 0) ? img : work;
             {
-                Span sp(KC_FINE_GATES, st);
-                if (tma) lac::k_fine_gates_tma<<<gridFG, tb, lac::FG_SMEM_BYTES, st>>>(mapWorkFG, mapS, fa, ntx, ntiles, prev);
-                else lac::k_fine_gates<<<tg, tb, 0, st>>>(work, ws.S, fa, prev);
+                Span sp(KC_NOISE_S, st);
+                if (tma) lac::k_noise_S_tma<<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(src == img ? mapImgNS : mapWorkNS, na, ntx, ntiles, prev);
+                else lac::k_noise_S<<<ntiles, tb, 0, st>>>(src, na, ntx, prev);
                 LAUNCHED();
             }
-            {
-                Span sp(KC_DILATE, st);
-                lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M1, ws.G1, ws.M2, nullptr, nullptr, nullptr, h, w,
-                                                      wpr, prev);
-                LAUNCHED();
-                lac::k_dilate_gate<<<dg, 256, 0, st>>>(ws.M2, ws.G2, ws.M3, ws.C, ws.NEWP, ws.counts + t, h, w,
-                                                      wpr, prev);
+            if (lazy) {
+                Span sp(KC_LISTS, st);
+                lac::k_list_candidates<<<bit_grid(h, w), 256, 0, st>>>(ws.A1, t > 0 ? ws.NEED : nullptr, ws.G1, ws.G2, ws.M1,
+                                                                      ws.clist, ws.ncand + t, h, w, wpr, prev);
                 LAUNCHED();
             }
         }
+        if (lazy) {
+            // steps (3b)-(5) on the listed candidates only (lazy.cuh)
+            lac::CandArgs ca{ws.S, work, ws.G1, ws.G2, ws.M1, h, w, wpr, p.sigclip, siglow, p.objlim};
+            Span sp(KC_EVAL, st);
+            lac::k_eval_candidates<<<gridE, 128, 0, st>>>(ca, ws.clist, ws.ncand + t, prev);
+            LAUNCHED();
+        } else {
+            lac::FineArgs fa{ws.G1, ws.G2, ws.M1, d ? dbg->Sp : nullptr, d ? dbg->m3 : nullptr,
+                             d ? dbg->F : nullptr, h, w, wpr, gp};
+            Span sp(KC_FINE_GATES, st);
+            if (tma) lac::k_fine_gates_tma<<<gridFG, tb, lac::FG_SMEM_BYTES, st>>>(mapWorkFG, mapS, fa, ntx, ntiles, prev);
+            else lac::k_fine_gates<<<tg, tb, 0, st>>>(work, ws.S, fa, prev);
+            LAUNCHED();
+        }
         if (d && dbg->S) CK(cudaMemcpyAsync(dbg->S, ws.S, P * 4, cudaMemcpyDeviceToDevice, st));
-        rc = replace_pass(img, ws, ws.NEWP, ws.NEED, lazy ? ws.tileflag : nullptr, ws.nneed + t, work, h, w, prev, st);
-        if (rc) return rc;
+        // steps (6)-(7), fused; in the lazy path G2 is completed on the pixels the second growth reaches
+        lac::GrowArgs ga{ws.M1, ws.G1, ws.G2, lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
+                         ws.C[t & 1], ws.C[(t + 1) & 1], ws.NEED, d ? ws.M2 : nullptr, d ? ws.M3 : nullptr,
+                         ws.S, img, work, ws.counts + t, h, w, wpr, siglow};
+        if ((rc = grow_replace(ga, prev, st))) return rc;
         if (d) {
             // lazy path: G2 is only evaluated where step (6) needs it, so it is not dumped
             struct { const uint32_t* b; uint8_t* o; } planes[] = {
                 {ws.G1, dbg->G1}, {ws.G2, lazy ? nullptr : dbg->G2}, {ws.M1, dbg->M1},
-                {ws.M2, dbg->M2}, {ws.M3, dbg->M3}, {ws.C, dbg->C}};
+                {ws.M2, dbg->M2}, {ws.M3, dbg->M3}, {ws.C[(t + 1) & 1], dbg->C}};
             for (auto& pl : planes)
                 if (pl.o && (rc = unpack(pl.b, pl.o, h, w, st))) return rc;
         }
     }
-    int rc = unpack(ws.C, mask_out, h, w, st);
+    int rc = unpack(ws.C[p.niter & 1], mask_out, h, w, st);
     if (rc) return rc;
     if (iter_counts && p.niter > 0)
         CK(cudaMemcpyAsync(iter_counts, ws.counts, (size_t)p.niter * 4, cudaMemcpyDeviceToDevice, st));
@@ -515,8 +482,7 @@ int lacosmic_dilate3(const uint32_t* bits_in, uint32_t* bits_out, int h, int w, 
     if (rc) return rc;
     int wpr = words_per_row(w);
     if (overlap(bits_in, (size_t)h * wpr * 4, bits_out, (size_t)h * wpr * 4)) return LACOSMIC_ERR_ALIAS;
-    lac::k_dilate_gate<<<bit_grid(h, w), 256, 0, (cudaStream_t)stream>>>(bits_in, nullptr, bits_out, nullptr, nullptr,
-                                                           nullptr, h, w, wpr, nullptr);
+    lac::k_dilate3<<<bit_grid(h, w), 256, 0, (cudaStream_t)stream>>>(bits_in, bits_out, h, w, wpr);
     LAUNCHED();
     return LACOSMIC_OK;
 }
@@ -532,10 +498,16 @@ int lacosmic_masked_median(const float* img, const uint8_t* mask_u8, float* out,
     if (overlap(img, P * 4, out, P * 4)) return LACOSMIC_ERR_ALIAS;
     Workspace ws = carve(workspace, h, w);
     cudaStream_t st = (cudaStream_t)stream;
-    if ((rc = lacosmic_pack_bits(mask_u8, ws.C, h, w, stream))) return rc;
+    const int wpr = words_per_row(w);
+    // the fused growth/replacement kernel with M1 = G1 = G2 = mask and C = 0 flags exactly the mask
+    // (M2 = dil3(mask) & mask, M3 likewise) and replaces every pixel of it
+    if ((rc = lacosmic_pack_bits(mask_u8, ws.M1, h, w, stream))) return rc;
     CK(cudaMemcpyAsync(out, img, P * 4, cudaMemcpyDeviceToDevice, st));
-    CK(cudaMemsetAsync(ws.nneed, 0, 4, st));
-    return replace_pass(img, ws, ws.C, nullptr, nullptr, ws.nneed, out, h, w, nullptr, st);   // every masked pixel is "new"
+    CK(cudaMemsetAsync(ws.C[0], 0, (size_t)h * wpr * 4, st));
+    CK(cudaMemsetAsync(ws.counts, 0, 4, st));
+    lac::GrowArgs ga{ws.M1, ws.M1, ws.M1, nullptr, nullptr, ws.C[0], ws.C[1], ws.NEED, nullptr, nullptr,
+                     nullptr, img, out, ws.counts, h, w, wpr, 0.0f};
+    return grow_replace(ga, nullptr, st);
 }
 
 // ---- diagnostics ------------------------------------------------------------------------------
@@ -578,13 +550,13 @@ int lacosmic_kernel_timing_read(float* ms_sum, int32_t* spans) {
 }
 
 const char* lacosmic_kernel_class_name(int cls) {
-    static const char* names[KC_COUNT] = {"noise_S", "fine_gates", "dilate_x2", "replace", "bits",
-                                          "lazy_eval", "noise_S_incremental", "whole_frame"};
+    static const char* names[KC_COUNT] = {"noise_S", "fine_gates", "grow_replace", "lists", "bits",
+                                          "eval_candidates", "noise_S_quads", "whole_frame"};
     return (cls >= 0 && cls < KC_COUNT) ? names[cls] : "?";
 }
 
 int lacosmic_last_cuda_error(void) { return g_last_cuda_error; }
 int lacosmic_last_launch_count(void) { return g_launches; }
-const char* lacosmic_version(void) { return "lacosmic-b200 0.2 (sm_100a)"; }
+const char* lacosmic_version(void) { return "lacosmic-b200 0.3 (sm_100a)"; }
 
 }  // extern "C"

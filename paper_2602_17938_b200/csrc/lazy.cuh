@@ -19,6 +19,9 @@
 // A2 = ok & (S > siglow).  Masks, counts and cleaned frames are identical to the dense path.
 #pragma once
 #include "common.cuh"
+#include "kernels.cuh"
+#include "lazy_count.cuh"
+#include "median_networks.cuh"
 
 namespace lac {
 
@@ -64,31 +67,6 @@ k_list_candidates(const uint32_t* __restrict__ A1, const uint32_t* __restrict__ 
     block_append(bits, y0 * w + wx * 32, w, list, nlist);
 }
 
-// list <- pixels of dil3(M2) & A2 & ~A1 & ~G2: the only pixels where G2 is needed by O6 and not known
-__global__ void __launch_bounds__(256)
-k_list_neighbours(const uint32_t* __restrict__ M2, const uint32_t* __restrict__ A1,
-                  const uint32_t* __restrict__ A2, const uint32_t* __restrict__ G2, int* __restrict__ list,
-                  int* __restrict__ nlist, int h, int w, int wpr, const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;
-    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
-    const int wx = blockIdx.x * 32 + lane, y0 = blockIdx.y * BW_CTA_ROWS + wi * BW_ROWS;
-    uint32_t bits[BW_ROWS];
-#pragma unroll
-    for (int i = 0; i < BW_ROWS; ++i) bits[i] = 0;
-    if (wx < wpr && y0 < h) {
-        uint32_t d[BW_ROWS];
-        dilate_rows<1>(M2, y0, wx, h, wpr, d);
-#pragma unroll
-        for (int i = 0; i < BW_ROWS; ++i) {
-            const int y = y0 + i;
-            if (y >= h) break;
-            const size_t q = (size_t)y * wpr + wx;
-            if (d[i]) bits[i] = d[i] & A2[q] & ~A1[q] & ~G2[q];
-        }
-    }
-    block_append(bits, y0 * w + wx * 32, w, list, nlist);
-}
-
 // exact median of 9 (19 compare-exchanges)
 __device__ __forceinline__ float med9(float a0, float a1, float a2, float a3, float a4, float a5, float a6,
                                       float a7, float a8) {
@@ -102,62 +80,6 @@ __device__ __forceinline__ float med9(float a0, float a1, float a2, float a3, fl
     ce(a4, a2);
     a4 = fmaxf(a6, a4);
     return fminf(a4, a2);
-}
-
-__device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
-
-// #{25 taps v of S around pixel p : fsub(Sc, v) > thr} for thr = sigclip (c1) and siglow (c2).
-// Interior pixels (window inside the frame): each window row is read as two 16-byte aligned vectors that
-// cover it, the test is evaluated on all 8 values and the 5 of the window are selected by a shift.
-__device__ __forceinline__ void count_sp_interior(const float* __restrict__ S, int p, int w, float sigclip,
-                                                  float siglow, int& c1, int& c2) {
-    const float sc = __ldg(S + p);
-    c1 = 0;
-    c2 = 0;
-#pragma unroll
-    for (int r = 0; r < 5; ++r) {
-        const int base = p + (r - 2) * w - 2, b = base & ~3, sh = base - b;
-        const float4 a0 = ldg4(S + b), a1 = ldg4(S + b + 4);
-        const float e[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
-        uint32_t m1 = 0, m2 = 0;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            const float sp = __fsub_rn(sc, e[k]);
-            m1 |= (uint32_t)(sp > sigclip) << k;
-            m2 |= (uint32_t)(sp > siglow) << k;
-        }
-        c1 += __popc((m1 >> sh) & 31u);
-        c2 += __popc((m2 >> sh) & 31u);
-    }
-}
-
-// any pixel: clamped scalar taps (R3)
-__device__ __forceinline__ void count_sp_clamped(const float* __restrict__ S, int y, int x, int h, int w,
-                                                 float sigclip, float siglow, int& c1, int& c2) {
-    const float sc = __ldg(S + (size_t)y * w + x);
-    int xx[5];
-#pragma unroll
-    for (int d = 0; d < 5; ++d) xx[d] = clampi(x + d - 2, 0, w - 1);
-    c1 = 0;
-    c2 = 0;
-#pragma unroll
-    for (int dy = 0; dy < 5; ++dy) {
-        const float* row = S + (size_t)clampi(y + dy - 2, 0, h - 1) * w;
-#pragma unroll
-        for (int dx = 0; dx < 5; ++dx) {
-            const float sp = __fsub_rn(sc, __ldg(row + xx[dx]));
-            c1 += sp > sigclip;
-            c2 += sp > siglow;
-        }
-    }
-}
-
-__device__ __forceinline__ void count_sp(const float* __restrict__ S, int y, int x, int h, int w, float sigclip,
-                                         float siglow, int& c1, int& c2) {
-    if (y >= 2 && x >= 2 && x + 2 < w && y + 2 < h && (size_t)(y + 2) * w + x + 6 <= (size_t)h * w)
-        count_sp_interior(S, y * w + x, w, sigclip, siglow, c1, c2);
-    else
-        count_sp_clamped(S, y, x, h, w, sigclip, siglow, c1, c2);
 }
 
 struct CandArgs {
@@ -333,18 +255,96 @@ k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restric
     }
 }
 
-// One thread per pixel of dil3(M2) & A2 & ~A1 & ~G2: G2 by counting.
-__global__ void __launch_bounds__(128)
-k_eval_neighbours(const float* __restrict__ S, uint32_t* __restrict__ G2, int h, int w, int wpr, float siglow,
-                  const int* __restrict__ list, const int* __restrict__ nlist, const int* prev_count) {
+// ------------------------------------------------------------------------------------------------
+// Incremental steps (1)-(3a) (iterations t >= 1): S, A1, A2 are recomputed only on the listed quads (aligned
+// groups of 4 pixels holding a pixel within 2 px of a rewritten one; k_dirty_lists), one quad per thread, with
+// the same window network and the same operations as the dense pass (kernels.cuh, noise_S_tile).  The
+// pixels of the quad with S > sigclip are appended to the candidate list (one atomic per CTA and round).
+__global__ void __launch_bounds__(256)
+k_noise_S_quads(const float* __restrict__ work, NoiseArgs a, const int* __restrict__ qlist,
+                const int* __restrict__ nq, int* __restrict__ clist, int* __restrict__ nc, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
-    const int n = *nlist;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        const int p = list[i];
-        const int y = p / w, x = p - y * w;
-        int c1, c2;
-        count_sp(S, y, x, h, w, siglow, siglow, c1, c2);
-        if (c2 >= 13) atomicOr(G2 + (size_t)y * wpr + (x >> 5), 1u << (x & 31));
+    __shared__ int s_warp[8];
+    __shared__ int s_base;
+    const int n = *nq, h = a.h, w = a.w;
+    const int tid = threadIdx.x, lane = tid & 31, wi = tid >> 5;
+    const bool vec = (w & 3) == 0;
+    for (int base = blockIdx.x * 256; base < n; base += gridDim.x * 256) {   // uniform trip count per CTA
+        const int i = base + tid;
+        uint32_t n1 = 0;
+        int p = 0;
+        if (i < n) {
+            p = qlist[i];
+            const int y = p / w, x = p - y * w;
+            float win[8][5];   // win[c][r] = work<y-2+r, x-2+c>
+            if (vec && x >= 4 && x + 8 <= w && y >= 2 && y + 2 < h) {
+#pragma unroll
+                for (int r = 0; r < 5; ++r) {
+                    const float* row = work + (size_t)(y - 2 + r) * w + (x - 4);
+                    const float4 q0 = *reinterpret_cast<const float4*>(row);
+                    const float4 q1 = *reinterpret_cast<const float4*>(row + 4);
+                    const float4 q2 = *reinterpret_cast<const float4*>(row + 8);
+                    const float v[12] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w, q2.x, q2.y, q2.z, q2.w};
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) win[c][r] = v[2 + c];
+                }
+            } else {
+                int xx[8];
+#pragma unroll
+                for (int c = 0; c < 8; ++c) xx[c] = clampi(x - 2 + c, 0, w - 1);
+#pragma unroll
+                for (int r = 0; r < 5; ++r) {
+                    const float* row = work + (size_t)clampi(y - 2 + r, 0, h - 1) * w;
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) win[c][r] = row[xx[c]];
+                }
+            }
+            float m5[4], s[4];
+            median5x5_x4(win, m5);
+            uint32_t n2 = 0;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const float lp = lplus_px(win[2 + j][2], win[2 + j][1], win[2 + j][3], win[1 + j][2], win[3 + j][2]);
+                const float m5c = m5[j] > 1e-4f ? m5[j] : 1e-4f;                                 // R5
+                const float nn = __fdiv_rn(__fsqrt_rn(__fadd_rn(__fmul_rn(a.gain, m5c), a.rn2)), a.gain);
+                s[j] = __fdiv_rn(lp, __fmul_rn(2.0f, nn));
+                const bool ok = (x + j < w) && (win[2 + j][2] < a.satlevel);                    // R12
+                n1 |= (uint32_t)(ok && s[j] > a.sigclip) << j;
+                n2 |= (uint32_t)(ok && s[j] > a.siglow) << j;
+            }
+            store4(a.S, (size_t)y * w, x, w, s);
+            // this thread alone owns its nibble of the A1 / A2 words; the other nibbles change concurrently
+            const size_t q = (size_t)y * a.wpr + (x >> 5);
+            const int sh = x & 31;
+            const uint32_t o1 = (a.A1[q] >> sh) & 0xFu, o2 = (a.A2[q] >> sh) & 0xFu;
+            if (o1 != n1) atomicXor(a.A1 + q, (o1 ^ n1) << sh);
+            if (o2 != n2) atomicXor(a.A2 + q, (o2 ^ n2) << sh);
+        }
+        const int cnt = __popc(n1);
+        int incl = cnt;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int o = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += o;
+        }
+        if (lane == 31) s_warp[wi] = incl;
+        __syncthreads();
+        if (tid == 0) {
+            int tot = 0;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const int c = s_warp[k];
+                s_warp[k] = tot;
+                tot += c;
+            }
+            s_base = tot ? atomicAdd(nc, tot) : 0;
+        }
+        __syncthreads();
+        int o = s_base + s_warp[wi] + incl - cnt;
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if ((n1 >> j) & 1u) clist[o++] = p + j;
+        __syncthreads();   // s_warp / s_base are rewritten in the next round
     }
 }
 
