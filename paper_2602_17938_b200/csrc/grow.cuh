@@ -1,16 +1,19 @@
 // Steps (6)-(7) fused, and the bit-plane pass that opens an incremental iteration.
 //
-// k_grow_replace: one CTA per 1024 x 32 pixel tile of the bit-planes, staged in shared memory with a halo
-// of 4 rows / 1 word, does
-//     M2 = dil3(M1) & G1                                   on tile + 3 px
-//     G2 where the second growth reads it and it is not known yet (lazy path only)   on tile + 2 px
-//     M3 = dil3(M2) & G2,  fresh = M3 & ~C,  C' = C | M3   on tile + 2 px
-//     need = dil5x5(fresh) & C'                            on the tile
+// Both kernels are WARP-AUTONOMOUS: a warp owns a strip of 30 words x 8 rows (960 x 8 pixels) of the
+// bit-planes, lane l holds word column wx0 - 1 + l (lanes 0 and 31 are the horizontal halo) of every row it
+// needs in registers, horizontal neighbours come from warp shuffles, and everything in the halo is
+// recomputed from the same inputs by the neighbouring warp (bit arithmetic, plus a handful of redundant G2
+// evaluations).  There is no exchange between warps, no block barrier and no staging of whole planes.
+//
+// k_grow_replace, per warp:
+//     M2 = dil3(M1) & G1                                   on strip + 3 px      (G1 read only under dil3(M1))
+//     G2 where the second growth reads it and it is not known yet (lazy path)   on strip + 2 px
+//     M3 = dil3(M2) & G2,  fresh = M3 & ~C,  C' = C | M3   on strip + 2 px
+//     need = dil5x5(fresh) & C'                            on the strip
 //     work[p] = masked 5x5 median of img_in around p       for p in need
-// Every quantity in the halo is recomputed from the same inputs by the neighbouring CTA (bit arithmetic,
-// and a handful of redundant G2 evaluations), so there is no exchange between CTAs and the six launches
-// of the unfused sequence (dilate, list, evaluate, dilate, list, replace) become one.  C is double
-// buffered (read `Cold`, write `Cnew`) because a neighbour still reads the old plane in its halo.
+// so the six launches of the unfused sequence (dilate, list, evaluate, dilate, list, replace) become one.
+// C is double buffered (read `Cold`, write `Cnew`) because a neighbour still reads the old plane in its halo.
 #pragma once
 #include "common.cuh"
 #include "lazy_count.cuh"
@@ -18,61 +21,71 @@
 
 namespace lac {
 
-constexpr int GT_W = 32;                      // tile width in 32-px words
-constexpr int GT_H = 32;                      // tile height in rows
-constexpr int GT_HALO = 4;                    // halo rows (and pixels: one halo word on each side)
-constexpr int GS_W = GT_W + 2, GS_H = GT_H + 2 * GT_HALO, GS_N = GS_W * GS_H;
-constexpr int G_CAP = 2048;                   // shared pixel list capacity per compaction round
+constexpr int WG_OWN = 30;                    // own word columns of a warp (lanes 1..30)
+constexpr int WG_R = 8;                       // own rows of a warp
+constexpr int WG_WARPS = 8;                   // warps per CTA, stacked vertically
+constexpr int WG_J = WG_R + 8;                // register rows: y = ya - 4 + j, j < WG_J
+constexpr int WG_LCAP = 128;                  // per-warp pixel list capacity of one round
+constexpr unsigned FULL = 0xffffffffu;
 
-// haloed tile of a bit-plane into shared memory; outside the frame (and for a null plane) = 0
-__device__ __forceinline__ void load_bits_tile(uint32_t* sm, const uint32_t* __restrict__ g, int y0, int wx0,
-                                               int h, int wpr, int tid) {
-    for (int i = tid; i < GS_N; i += 256) {
-        const int r = i / GS_W, c = i - r * GS_W;
-        const int y = y0 - GT_HALO + r, wx = wx0 - 1 + c;
-        const bool ok = (y >= 0) & (y < h) & (wx >= 0) & (wx < wpr);
-        uint32_t v = 0;
-        if (g) v = g[(size_t)clampi(y, 0, h - 1) * wpr + clampi(wx, 0, wpr - 1)];   // branch-free address
-        sm[i] = ok ? v : 0u;
-    }
+__device__ __forceinline__ uint32_t lane_left(uint32_t v, int lane) {
+    const uint32_t t = __shfl_up_sync(FULL, v, 1);
+    return lane > 0 ? t : 0u;
 }
-
-// horizontally dilated word (r, c) of a shared tile; words beyond the tile's halo read as 0 (only the
-// outer bits of the halo words depend on them, and no result of the own tile depends on those)
+__device__ __forceinline__ uint32_t lane_right(uint32_t v, int lane) {
+    const uint32_t t = __shfl_down_sync(FULL, v, 1);
+    return lane < 31 ? t : 0u;
+}
+// horizontal dilation of a row held one word per lane; lanes 0 / 31 miss their outer neighbour, which only
+// affects their outer bits, and no result of the own columns depends on those
 template <int R>
-__device__ __forceinline__ uint32_t hdil_sm(const uint32_t* sm, int r, int c) {
-    const uint32_t* row = sm + r * GS_W;
-    return hdil<R>(c > 0 ? row[c - 1] : 0u, row[c], c + 1 < GS_W ? row[c + 1] : 0u);
+__device__ __forceinline__ uint32_t hdil_w(uint32_t v, int lane) {
+    return hdil<R>(lane_left(v, lane), v, lane_right(v, lane));
 }
 
-// One compaction round: every thread offers the set bits of its words (code = tile-local word index * 32 +
-// bit); up to G_CAP of them are written to s_list, the bits that did not fit stay in `bits` for the next
-// round.  Returns the number of entries.  Contains block barriers.
-template <int NW>
-__device__ __forceinline__ int smem_compact(uint32_t (&bits)[NW], const int (&widx)[NW], int* s_cnt, int* s_list,
-                                            int tid) {
-    if (tid == 0) *s_cnt = 0;
-    __syncthreads();
+// Warp-cooperative loop over every set bit of bits[J0..J1) of every lane: the bits are compacted into the
+// warp's shared list (rounds of at most WG_LCAP) and handed out one per lane: f(j, source lane, bit).
+template <int J0, int J1, class F>
+__device__ __forceinline__ void warp_for_each_bit(uint32_t (&bits)[WG_J], int* s_list, int lane, F f) {
+    for (;;) {
+        int n = 0;
 #pragma unroll
-    for (int k = 0; k < NW; ++k) {
-        uint32_t b = bits[k];
-        if (b) {
-            int slot = atomicAdd(s_cnt, __popc(b));
-            while (b && slot < G_CAP) {
+        for (int j = J0; j < J1; ++j) n += __popc(bits[j]);
+        int incl = n;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int o = __shfl_up_sync(FULL, incl, d);
+            if (lane >= d) incl += o;
+        }
+        const int total = __shfl_sync(FULL, incl, 31);
+        if (total == 0) break;
+        int off = incl - n;
+#pragma unroll
+        for (int j = J0; j < J1; ++j) {
+            uint32_t b = bits[j];
+            while (b && off < WG_LCAP) {
                 const int bit = __ffs(b) - 1;
                 b &= b - 1;
-                s_list[slot++] = widx[k] * 32 + bit;
+                s_list[off++] = (j << 10) | (lane << 5) | bit;
             }
-            bits[k] = b;
+            bits[j] = b;
         }
+        __syncwarp();
+        const int m = min(total, WG_LCAP);
+        for (int i = lane; i < m; i += 32) {
+            const int code = s_list[i];
+            f(code >> 10, (code >> 5) & 31, code & 31);
+        }
+        __syncwarp();
     }
-    __syncthreads();
-    return min(*s_cnt, G_CAP);
 }
 
 struct GrowArgs {
     const uint32_t *M1, *G1;
-    uint32_t* G2;                 // lazy path: completed where step (6) reads it (own words rewritten)
+    uint32_t* G2;                 // lazy path: completed where step (6) reads it
+    uint32_t* G2F;                // lazy path: pixels (outside A1) whose G2 was evaluated and is false.  A bit
+                                  // of G2 or of G2F is conclusive on its own, so a neighbouring warp may read
+                                  // either plane before or after the owner's update
     const uint32_t *A1, *A2;      // lazy path: S > sigclip / S > siglow planes; null: G2 is complete
     const uint32_t* Cold;
     uint32_t* Cnew;
@@ -82,249 +95,333 @@ struct GrowArgs {
     const float* img;             // img_in: donor values (R13)
     float* work;
     int* count;                   // += |M3 & ~C|
+    const uint8_t* stripflag;     // nullable: per strip, set by k_dirty_lists when R is not empty in it
     int h, w, wpr;
     float siglow;
 };
 
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(32 * WG_WARPS, 3)
 k_grow_replace(GrowArgs a, const int* prev_count) {
-    const int tid = threadIdx.x, lane = tid & 31, wi = tid >> 5;
-    const int wx0 = blockIdx.x * GT_W, y0 = blockIdx.y * GT_H;
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const int h = a.h, w = a.w, wpr = a.wpr;
+    const int wxh = blockIdx.x * WG_OWN - 1;                 // word column of lane 0
+    const int wx = wxh + lane;
+    const int ya = (blockIdx.y * WG_WARPS + wi) * WG_R;       // first own row
+    if (ya >= h) return;                                      // warp-uniform; the kernel has no block barrier
+    const bool colok = wx >= 0 && wx < wpr;
+    const bool own = lane >= 1 && lane <= WG_OWN && colok;
+    const int wxc = clampi(wx, 0, wpr - 1);
+    __shared__ uint32_t s_plane_all[WG_WARPS][(WG_R + 4) * 32];   // G2, then C', rows ya-2 .. ya+WG_R+1
+    __shared__ int s_list_all[WG_WARPS][WG_LCAP];
+    uint32_t* s_plane = s_plane_all[wi];
+    int* s_list = s_list_all[wi];
+    // word (row j, this lane's column) of a plane; 0 outside the frame.  Branch-free: clamped address.
+    auto ld = [&](const uint32_t* __restrict__ pl, int j) -> uint32_t {
+        const int y = ya - 4 + j;
+        const uint32_t v = pl[(size_t)clampi(y, 0, h - 1) * wpr + wxc];
+        return (colok && y >= 0 && y < h) ? v : 0u;
+    };
+    auto qof = [&](int j) -> size_t { return (size_t)(ya - 4 + j) * wpr + wx; };
     if (prev_count && *prev_count == 0) {
         // fixed point (R17): nothing changes; carry C over to the plane the next reader expects
-        for (int i = tid; i < GT_W * GT_H; i += 256) {
-            const int y = y0 + i / GT_W, wx = wx0 + i % GT_W;
-            if (y < h && wx < wpr) a.Cnew[(size_t)y * wpr + wx] = a.Cold[(size_t)y * wpr + wx];
-        }
+#pragma unroll
+        for (int j = 4; j < 4 + WG_R; ++j)
+            if (own && ya - 4 + j < h) a.Cnew[qof(j)] = a.Cold[qof(j)];
         return;
     }
-    __shared__ uint32_t sA[GS_N];    // M1, then D = dil3(M2)
-    __shared__ uint32_t sB[GS_N];    // G1, then M2
-    __shared__ uint32_t sC[GS_N];    // C, then C'
-    __shared__ uint32_t sG2[GS_N];
-    __shared__ uint32_t sN[GS_N];    // A1, then fresh
-    __shared__ uint32_t sA2[GS_N];
-    __shared__ int s_list[G_CAP];
-    __shared__ int s_cnt;
-    __shared__ int s_red[8];
     const bool lazy = a.A2 != nullptr;
-    load_bits_tile(sA, a.M1, y0, wx0, h, wpr, tid);
-    load_bits_tile(sB, a.G1, y0, wx0, h, wpr, tid);
-    load_bits_tile(sC, a.Cold, y0, wx0, h, wpr, tid);
-    load_bits_tile(sG2, a.G2, y0, wx0, h, wpr, tid);
-    if (lazy) {
-        load_bits_tile(sN, a.A1, y0, wx0, h, wpr, tid);
-        load_bits_tile(sA2, a.A2, y0, wx0, h, wpr, tid);
-    }
-    __syncthreads();
-    // M2 = dil3(M1) & G1 on rows 1 .. GS_H-2 (in place of G1: each element is read by its writer only)
-    for (int i = tid + GS_W; i < GS_N - GS_W; i += 256) {
-        const int r = i / GS_W, c = i - r * GS_W;
-        sB[i] = (hdil_sm<1>(sA, r - 1, c) | hdil_sm<1>(sA, r, c) | hdil_sm<1>(sA, r + 1, c)) & sB[i];
-    }
-    __syncthreads();
-    // D = dil3(M2) on rows 2 .. GS_H-3 (over M1, which is dead); pixels whose G2 is still unknown
-    constexpr int NWD = ((GS_H - 4) * GS_W + 255) / 256;
-    uint32_t nb[NWD];
-    int nbw[NWD];
+    if (a.stripflag) {
+        // incremental iteration: M1, G1, G2 only changed inside the strips k_dirty_lists flagged.  A pixel is
+        // fresh only if one of them changed within 2 px of it, and `need` reads fresh within 2 px of the own
+        // strip, so with no flagged strip among this one and its 8 neighbours nothing is fresh here.
+        bool f = false;
+        if (lane < 9) {
+            const int sy = blockIdx.y * WG_WARPS + wi - 1 + lane / 3, sx = (int)blockIdx.x - 1 + lane % 3;
+            if (sy >= 0 && sy < (h + WG_R - 1) / WG_R && sx >= 0 && sx < (int)gridDim.x)
+                f = a.stripflag[sy * gridDim.x + sx] != 0;
+        }
+        if (!__any_sync(FULL, f)) {
 #pragma unroll
-    for (int k = 0; k < NWD; ++k) {
-        const int i = 2 * GS_W + tid + k * 256;
-        nb[k] = 0;
-        nbw[k] = i;
-        if (i < GS_N - 2 * GS_W) {
-            const int r = i / GS_W, c = i - r * GS_W;
-            const uint32_t d = hdil_sm<1>(sB, r - 1, c) | hdil_sm<1>(sB, r, c) | hdil_sm<1>(sB, r + 1, c);
-            sA[i] = d;
-            if (lazy) {
-                // only within 2 px of the own tile: the neighbouring CTAs evaluate the rest
-                const uint32_t keep = c == 0 ? 0xC0000000u : c == GS_W - 1 ? 0x00000003u : 0xffffffffu;
-                nb[k] = d & sA2[i] & ~sN[i] & ~sG2[i] & keep;
-            }
+            for (int j = 4; j < 4 + WG_R; ++j)
+                if (own && ya - 4 + j < h) {
+                    a.Cnew[qof(j)] = a.Cold[qof(j)];
+                    a.NEED[qof(j)] = 0u;
+                }
+            return;
         }
     }
+    // every word the strip can need, requested up front (independent loads, one round trip)
+    uint32_t m2[WG_J], g2[WG_J], nbm[WG_J], cold[WG_J];
+    {
+        uint32_t m1[WG_J], g1[WG_J];
+#pragma unroll
+        for (int j = 0; j < WG_J; ++j) m1[j] = ld(a.M1, j);
+#pragma unroll
+        for (int j = 1; j < WG_J - 1; ++j) g1[j] = ld(a.G1, j);
+#pragma unroll
+        for (int j = 2; j < WG_J - 2; ++j) {
+            g2[j] = ld(a.G2, j);
+            cold[j] = ld(a.Cold, j);
+            nbm[j] = lazy ? (ld(a.A2, j) & ~ld(a.A1, j) & ~ld(a.G2F, j)) : 0u;
+        }
+        // ---- M2 = dil3(M1) & G1, rows 1 .. WG_J-2
+#pragma unroll
+        for (int j = 0; j < WG_J; ++j) m1[j] = hdil_w<1>(m1[j], lane);
+        m2[0] = m2[WG_J - 1] = 0;
+#pragma unroll
+        for (int j = 1; j < WG_J - 1; ++j) m2[j] = (m1[j - 1] | m1[j] | m1[j + 1]) & g1[j];
+    }
+    // ---- D = dil3(M2), rows 2 .. WG_J-3
+    uint32_t d[WG_J];
+    {
+        uint32_t hm[WG_J];
+#pragma unroll
+        for (int j = 1; j < WG_J - 1; ++j) hm[j] = hdil_w<1>(m2[j], lane);
+#pragma unroll
+        for (int j = 2; j < WG_J - 2; ++j) d[j] = hm[j - 1] | hm[j] | hm[j + 1];
+    }
     if (lazy) {
-        // G2 = (S' > siglow) at those pixels, by counting (lazy_count.cuh); rounds of at most G_CAP pixels
-        for (;;) {
-            const int n = smem_compact(nb, nbw, &s_cnt, s_list, tid);
-            for (int i = tid; i < n; i += 256) {
-                const int code = s_list[i], wd = code >> 5, bit = code & 31;
-                const int r = wd / GS_W, c = wd - r * GS_W;
-                const int y = y0 - GT_HALO + r, x = (wx0 - 1 + c) * 32 + bit;
+        // pixels under D whose G2 = (S' > siglow) is not known yet: evaluate by counting (lazy_count.cuh).
+        // Only within 2 px of the own columns: the neighbouring warps evaluate the rest.
+        const uint32_t keep = lane == 0 ? 0xC0000000u : lane == 31 ? 0x00000003u : 0xffffffffu;
+        uint32_t nb[WG_J];
+        bool any = false;
+#pragma unroll
+        for (int j = 2; j < WG_J - 2; ++j) {
+            nb[j] = d[j] & nbm[j] & ~g2[j] & keep;
+            any |= nb[j] != 0;
+        }
+        if (__any_sync(FULL, any)) {
+#pragma unroll
+            for (int j = 2; j < WG_J - 2; ++j) s_plane[(j - 2) * 32 + lane] = g2[j];
+            __syncwarp();
+            uint32_t todo[WG_J];
+#pragma unroll
+            for (int j = 0; j < WG_J; ++j) todo[j] = (j >= 2 && j < WG_J - 2) ? nb[j] : 0u;
+            warp_for_each_bit<2, WG_J - 2>(todo, s_list, lane, [&](int j, int sl, int bit) {
+                const int y = ya - 4 + j, x = (wxh + sl) * 32 + bit;
                 int c1, c2;
                 count_sp(a.S, y, x, h, w, a.siglow, a.siglow, c1, c2);
-                if (c2 >= 13) atomicOr(&sG2[wd], 1u << bit);
-            }
-            bool more = false;
+                if (c2 >= 13) atomicOr(&s_plane[(j - 2) * 32 + sl], 1u << bit);
+            });
 #pragma unroll
-            for (int k = 0; k < NWD; ++k) more |= nb[k] != 0;
-            if (!__syncthreads_or(more)) break;
+            for (int j = 2; j < WG_J - 2; ++j) g2[j] = s_plane[(j - 2) * 32 + lane];
+            __syncwarp();
+            // remember the evaluations of the own words
+#pragma unroll
+            for (int j = 4; j < 4 + WG_R; ++j)
+                if (nb[j] && own && ya - 4 + j < h) {
+                    a.G2[qof(j)] = g2[j];
+                    a.G2F[qof(j)] |= nb[j] & ~g2[j];
+                }
         }
-    } else {
-        __syncthreads();
     }
-    // M3 = D & G2; fresh = M3 & ~C; C' = C | M3 on rows 2 .. GS_H-3
+    // ---- M3 = D & G2; fresh = M3 & ~C; C' = C | M3, rows 2 .. WG_J-3
+    uint32_t cn[WG_J], fresh[WG_J];
     int nfresh = 0;
-    for (int i = 2 * GS_W + tid; i < GS_N - 2 * GS_W; i += 256) {
-        const int r = i / GS_W, c = i - r * GS_W;
-        const uint32_t m3 = sA[i] & sG2[i], cold = sC[i], fresh = m3 & ~cold;
-        sC[i] = cold | m3;
-        sN[i] = fresh;
-        const int y = y0 - GT_HALO + r, wx = wx0 - 1 + c;
-        if (r >= GT_HALO && r < GT_HALO + GT_H && c >= 1 && c <= GT_W && y < h && wx < wpr) {
-            const size_t q = (size_t)y * wpr + wx;
-            a.Cnew[q] = cold | m3;
-            if (lazy) a.G2[q] = sG2[i];
-            if (a.M2out) a.M2out[q] = sB[i];
-            if (a.M3out) a.M3out[q] = m3;
-            nfresh += __popc(fresh);
+    bool anyfresh = false;
+#pragma unroll
+    for (int j = 2; j < WG_J - 2; ++j) {
+        const uint32_t m3 = d[j] & g2[j];
+        fresh[j] = m3 & ~cold[j];
+        cn[j] = cold[j] | m3;
+        anyfresh |= fresh[j] != 0;
+        if (j >= 4 && j < 4 + WG_R && own && ya - 4 + j < h) {
+            a.Cnew[qof(j)] = cn[j];
+            if (a.M2out) a.M2out[qof(j)] = m2[j];
+            if (a.M3out) a.M3out[qof(j)] = m3;
+            nfresh += __popc(fresh[j]);
         }
     }
-    nfresh = __reduce_add_sync(0xffffffffu, nfresh);
-    if (lane == 0) s_red[wi] = nfresh;
-    __syncthreads();
-    if (tid == 0) {
-        int tot = 0;
+    nfresh = __reduce_add_sync(FULL, nfresh);
+    if (lane == 0 && nfresh) atomicAdd(a.count, nfresh);
+    // ---- need = dil5x5(fresh) & C' on the own words
+    uint32_t need[WG_J];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) tot += s_red[k];
-        if (tot) atomicAdd(a.count, tot);
+    for (int j = 0; j < WG_J; ++j) need[j] = 0;
+    if (__any_sync(FULL, anyfresh)) {
+        uint32_t hf[WG_J];
+#pragma unroll
+        for (int j = 2; j < WG_J - 2; ++j) hf[j] = hdil_w<2>(fresh[j], lane);
+#pragma unroll
+        for (int j = 4; j < 4 + WG_R; ++j)
+            if (own && ya - 4 + j < h) need[j] = (hf[j - 2] | hf[j - 1] | hf[j] | hf[j + 1] | hf[j + 2]) & cn[j];
     }
-    // need = dil5x5(fresh) & C' on the own tile: thread (lane, wi) owns rows 4 wi .. 4 wi + 3 of column lane
-    constexpr int NWN = GT_H / 8;
-    uint32_t need[NWN];
-    int needw[NWN];
-    {
-        const int c = 1 + lane, r0 = GT_HALO + wi * NWN;
-        uint32_t hd[NWN + 4];
 #pragma unroll
-        for (int k = 0; k < NWN + 4; ++k) hd[k] = hdil_sm<2>(sN, r0 - 2 + k, c);
+    for (int j = 4; j < 4 + WG_R; ++j)
+        if (own && ya - 4 + j < h) a.NEED[qof(j)] = need[j];
+    bool anyneed = false;
 #pragma unroll
-        for (int k = 0; k < NWN; ++k) {
-            const int i = (r0 + k) * GS_W + c, y = y0 + wi * NWN + k, wx = wx0 + lane;
-            need[k] = (hd[k] | hd[k + 1] | hd[k + 2] | hd[k + 3] | hd[k + 4]) & sC[i];
-            needw[k] = i;
-            if (y < h && wx < wpr) a.NEED[(size_t)y * wpr + wx] = need[k];
-            else need[k] = 0;
-        }
-    }
-    // step (7) at those pixels: 25 clamped taps of img_in, +inf where the tap's pixel is in C', 25-input
+    for (int j = 4; j < 4 + WG_R; ++j) anyneed |= need[j] != 0;
+    if (!__any_sync(FULL, anyneed)) return;
+    // ---- step (7) at those pixels: 25 clamped taps of img_in, +inf where the tap's pixel is in C', 25-input
     // sorting network, middle element(s) of the k donors (R13-R16)
+#pragma unroll
+    for (int j = 2; j < WG_J - 2; ++j) s_plane[(j - 2) * 32 + lane] = cn[j];
+    __syncwarp();
     const float INF = __int_as_float(0x7f800000);
-    for (;;) {
-        const int n = smem_compact(need, needw, &s_cnt, s_list, tid);
-        for (int i = tid; i < n; i += 256) {
-            const int code = s_list[i], wd = code >> 5, bit = code & 31;
-            const int r = wd / GS_W, c = wd - r * GS_W;
-            const int y = y0 - GT_HALO + r, x = (wx0 - 1 + c) * 32 + bit;
-            int xx[5], yy[5];
+    warp_for_each_bit<4, 4 + WG_R>(need, s_list, lane, [&](int j, int sl, int bit) {
+        const int y = ya - 4 + j, x = (wxh + sl) * 32 + bit;
+        int xx[5], yy[5];
 #pragma unroll
-            for (int d = 0; d < 5; ++d) {
-                xx[d] = clampi(x + d - 2, 0, w - 1);
-                yy[d] = clampi(y + d - 2, 0, h - 1);
-            }
-            uint32_t donors = 0;   // bit (5 dy + dx): the (clamped) tap is NOT in C'
-#pragma unroll
-            for (int dy = 0; dy < 5; ++dy) {
-                const uint32_t* row = sC + (yy[dy] - (y0 - GT_HALO)) * GS_W - (wx0 - 1);
-                const int wl = xx[0] >> 5, wr = xx[4] >> 5;
-                const uint32_t cl = row[wl], cr = row[wr];
-#pragma unroll
-                for (int dx = 0; dx < 5; ++dx) {
-                    const uint32_t word = (xx[dx] >> 5) == wl ? cl : cr;
-                    donors |= (((word >> (xx[dx] & 31)) & 1u) ^ 1u) << (5 * dy + dx);
-                }
-            }
-            if (donors == 0u) donors = 0x01ffffffu;            // R15: no donor -> all 25 taps
-            const int k = __popc(donors);
-            float v[25], s[25];
-#pragma unroll
-            for (int dy = 0; dy < 5; ++dy)
-#pragma unroll
-                for (int dx = 0; dx < 5; ++dx) {
-                    const float t = __ldg(a.img + (size_t)yy[dy] * w + xx[dx]);
-                    v[5 * dy + dx] = ((donors >> (5 * dy + dx)) & 1u) ? t : INF;
-                }
-            sort25(v, s);
-            const int ihi = k >> 1, ilo = (k - 1) >> 1;
-            float lo = s[0], hi = s[0];
-#pragma unroll
-            for (int q = 1; q < 25; ++q) {
-                lo = (q == ilo) ? s[q] : lo;
-                hi = (q == ihi) ? s[q] : hi;
-            }
-            a.work[(size_t)y * w + x] = (k & 1) ? hi : __fmul_rn(__fadd_rn(lo, hi), 0.5f);   // R14
+        for (int t = 0; t < 5; ++t) {
+            xx[t] = clampi(x + t - 2, 0, w - 1);
+            yy[t] = clampi(y + t - 2, 0, h - 1);
         }
-        bool more = false;
+        uint32_t donors = 0;   // bit (5 dy + dx): the (clamped) tap is NOT in C'
 #pragma unroll
-        for (int k = 0; k < NWN; ++k) more |= need[k] != 0;
-        if (!__syncthreads_or(more)) break;
-    }
+        for (int dy = 0; dy < 5; ++dy) {
+            const uint32_t* row = s_plane + (yy[dy] - (ya - 2)) * 32 - wxh;
+            const int wl = xx[0] >> 5, wr = xx[4] >> 5;
+            const uint32_t cl = row[wl], cr = row[wr];
+#pragma unroll
+            for (int dx = 0; dx < 5; ++dx) {
+                const uint32_t word = (xx[dx] >> 5) == wl ? cl : cr;
+                donors |= (((word >> (xx[dx] & 31)) & 1u) ^ 1u) << (5 * dy + dx);
+            }
+        }
+        if (donors == 0u) donors = 0x01ffffffu;            // R15: no donor -> all 25 taps
+        const int k = __popc(donors);
+        float v[25], s[25];
+#pragma unroll
+        for (int dy = 0; dy < 5; ++dy)
+#pragma unroll
+            for (int dx = 0; dx < 5; ++dx) {
+                const float t = __ldg(a.img + (size_t)yy[dy] * w + xx[dx]);
+                v[5 * dy + dx] = ((donors >> (5 * dy + dx)) & 1u) ? t : INF;
+            }
+        sort25(v, s);
+        const int ihi = k >> 1, ilo = (k - 1) >> 1;
+        float lo = s[0], hi = s[0];
+#pragma unroll
+        for (int q = 1; q < 25; ++q) {
+            lo = (q == ilo) ? s[q] : lo;
+            hi = (q == ihi) ? s[q] : hi;
+        }
+        a.work[(size_t)y * w + x] = (k & 1) ? hi : __fmul_rn(__fadd_rn(lo, hi), 0.5f);   // R14
+    });
 }
 
 // ------------------------------------------------------------------------------------------------
+// warp-aggregated append of the set bits of bits[J0..J1) (pixel index p0 + (j - J0) * w + bit) to a global
+// list: one atomicAdd per warp that has something to append
+template <int J0, int J1>
+__device__ __forceinline__ void warp_append(const uint32_t (&bits)[WG_J], int p0, int w, int* __restrict__ list,
+                                            int* __restrict__ nlist, int lane) {
+    int n = 0;
+#pragma unroll
+    for (int j = J0; j < J1; ++j) n += __popc(bits[j]);
+    int incl = n;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int o = __shfl_up_sync(FULL, incl, d);
+        if (lane >= d) incl += o;
+    }
+    const int total = __shfl_sync(FULL, incl, 31);
+    if (total == 0) return;
+    int base = 0;
+    if (lane == 31) base = atomicAdd(nlist, total);
+    int off = __shfl_sync(FULL, base, 31) + incl - n;
+#pragma unroll
+    for (int j = J0; j < J1; ++j) {
+        uint32_t b = bits[j];
+        const int pj = p0 + (j - J0) * w;
+        while (b) {
+            const int bit = __ffs(b) - 1;
+            b &= b - 1;
+            list[off++] = pj + bit;
+        }
+    }
+}
+
 // Opening pass of an incremental iteration (lazy path, t >= 1).  NEED = the pixels the previous
 // k_grow_replace rewrote in `work`.
 //   D5 = dil5x5(NEED): the pixels whose S changes (med5 window; L+ needs 1 px).  Their aligned 4-pixel
 //        groups ("quads") go to qlist for k_noise_S_quads, which also re-lists the candidates among them.
 //   R  = dil9x9(NEED) | quads: the pixels whose tests (3b)-(5) can change (S' reads S within 2 px, the fine
-//        structure test reads work within 4 px).  G1, G2, M1 are cleared inside R and the pixels of A1 in R
-//        outside the quads (their A1 is unchanged) go to the candidate list.
-__global__ void __launch_bounds__(256)
+//        structure test reads work within 4 px).  G1, G2, G2F, M1 are cleared inside R and the pixels of A1 in
+//        R outside the quads (their A1 is unchanged) go to the candidate list.
+// Same warp-autonomous layout as k_grow_replace.
+__global__ void __launch_bounds__(32 * WG_WARPS, 3)
 k_dirty_lists(const uint32_t* __restrict__ NEED, const uint32_t* __restrict__ A1, uint32_t* __restrict__ G1,
-              uint32_t* __restrict__ G2, uint32_t* __restrict__ M1, int* __restrict__ qlist, int* __restrict__ nq,
-              int* __restrict__ clist, int* __restrict__ nc, int h, int w, int wpr, const int* prev_count) {
+              uint32_t* __restrict__ G2, uint32_t* __restrict__ G2F, uint32_t* __restrict__ M1,
+              int* __restrict__ qlist, int* __restrict__ nq, int* __restrict__ clist, int* __restrict__ nc,
+              uint8_t* __restrict__ stripflag, int h, int w, int wpr, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
-    __shared__ uint32_t sN[GS_N];
-    const int tid = threadIdx.x, lane = tid & 31, wi = tid >> 5;
-    const int wx0 = blockIdx.x * GT_W, y0 = blockIdx.y * GT_H;
-    load_bits_tile(sN, NEED, y0, wx0, h, wpr, tid);
-    __syncthreads();
-    constexpr int NR = GT_H / 8;
-    const int c = 1 + lane, r0 = GT_HALO + wi * NR, wx = wx0 + lane, yb = y0 + wi * NR;
-    uint32_t h2[NR + 8], h4[NR + 8];
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    const int wx = blockIdx.x * WG_OWN - 1 + lane;
+    const int ya = (blockIdx.y * WG_WARPS + wi) * WG_R;
+    if (ya >= h) return;                                      // warp-uniform; no block barrier in this kernel
+    const bool colok = wx >= 0 && wx < wpr;
+    const bool own = lane >= 1 && lane <= WG_OWN && colok;
+    const int wxc = clampi(wx, 0, wpr - 1);
+    uint32_t h2[WG_J], h4[WG_J];
+    bool any = false;
 #pragma unroll
-    for (int k = 0; k < NR + 8; ++k) {
-        const uint32_t* row = sN + (r0 - 4 + k) * GS_W;
-        const uint32_t vl = row[c - 1], vc = row[c], vr = row[c + 1];
-        h2[k] = hdil<2>(vl, vc, vr);
-        h4[k] = hdil<4>(vl, vc, vr);
+    for (int j = 0; j < WG_J; ++j) {
+        const int y = ya - 4 + j;
+        const uint32_t v = NEED[(size_t)clampi(y, 0, h - 1) * wpr + wxc];
+        h2[j] = (colok && y >= 0 && y < h) ? v : 0u;
+        any |= h2[j] != 0;
     }
-    uint32_t quads[NR], cand[NR];
+    uint8_t* flag = stripflag + (size_t)(blockIdx.y * WG_WARPS + wi) * gridDim.x + blockIdx.x;
+    if (!__any_sync(FULL, any)) {                             // nothing was rewritten near this strip
+        if (lane == 0) *flag = 0;
+        return;
+    }
+    // the words of the own rows, requested up front (R is not known yet, but a dependent load per row would
+    // serialise eight round trips)
+    uint32_t a1[WG_R], g1[WG_R], g2[WG_R], g2f[WG_R], m1[WG_R];
+#pragma unroll
+    for (int k = 0; k < WG_R; ++k) {
+        const size_t q = (size_t)min(ya + k, h - 1) * wpr + wxc;
+        a1[k] = A1[q]; g1[k] = G1[q]; g2[k] = G2[q]; g2f[k] = G2F[q]; m1[k] = M1[q];
+    }
+#pragma unroll
+    for (int j = 0; j < WG_J; ++j) {
+        const uint32_t vl = lane_left(h2[j], lane), vc = h2[j], vr = lane_right(h2[j], lane);
+        h2[j] = hdil<2>(vl, vc, vr);
+        h4[j] = hdil<4>(vl, vc, vr);
+    }
+    uint32_t quads[WG_J], cand[WG_J];
+    bool anyR = false;
     const int rem = w - wx * 32;
     const uint32_t valid = rem >= 32 ? 0xffffffffu : rem > 0 ? ((1u << rem) - 1u) : 0u;
 #pragma unroll
-    for (int k = 0; k < NR; ++k) {
-        quads[k] = 0;
-        cand[k] = 0;
-        const int y = yb + k;
-        if (y < h && wx < wpr) {
+    for (int j = 0; j < WG_J; ++j) quads[j] = cand[j] = 0;
+#pragma unroll
+    for (int j = 4; j < 4 + WG_R; ++j) {
+        const int y = ya - 4 + j;
+        if (own && y < h) {
             uint32_t d5 = 0, r9 = 0;
 #pragma unroll
-            for (int d = 2; d <= 6; ++d) d5 |= h2[k + d];
+            for (int d = -2; d <= 2; ++d) d5 |= h2[j + d];
 #pragma unroll
-            for (int d = 0; d <= 8; ++d) r9 |= h4[k + d];
+            for (int d = -4; d <= 4; ++d) r9 |= h4[j + d];
             d5 &= valid;
             uint32_t t = d5 | (d5 >> 1);
             t |= t >> 2;
-            t &= 0x11111111u;                       // bit 4j: quad j of this word holds a pixel of D5
+            t &= 0x11111111u;                       // bit 4k: quad k of this word holds a pixel of D5
             const uint32_t dq = t * 0xFu;           // all four pixels of those quads
             const uint32_t R = (r9 | dq) & valid;
-            quads[k] = t;
+            quads[j] = t;
             if (R) {
                 const size_t q = (size_t)y * wpr + wx;
-                cand[k] = A1[q] & R & ~dq;
-                if (R == 0xffffffffu) {
-                    G1[q] = 0; G2[q] = 0; M1[q] = 0;
-                } else {
-                    G1[q] &= ~R; G2[q] &= ~R; M1[q] &= ~R;
-                }
+                const int k = j - 4;
+                anyR = true;
+                cand[j] = a1[k] & R & ~dq;
+                if (g1[k] & R) G1[q] = g1[k] & ~R;
+                if (g2[k] & R) G2[q] = g2[k] & ~R;
+                if (g2f[k] & R) G2F[q] = g2f[k] & ~R;
+                if (m1[k] & R) M1[q] = m1[k] & ~R;
             }
         }
     }
-    block_append<NR>(quads, yb * w + wx * 32, w, qlist, nq);
-    __syncthreads();
-    block_append<NR>(cand, yb * w + wx * 32, w, clist, nc);
+    anyR = __any_sync(FULL, anyR);
+    if (lane == 0) *flag = anyR ? 1 : 0;
+    const int p0 = ya * w + wx * 32;
+    warp_append<4, 4 + WG_R>(quads, p0, w, qlist, nq, lane);
+    warp_append<4, 4 + WG_R>(cand, p0, w, clist, nc, lane);
 }
 
 }  // namespace lac

@@ -464,15 +464,38 @@ k_dilate3(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, int h, in
 // bit-plane <-> uint8 plane
 __global__ void __launch_bounds__(256)
 k_unpack_bits(const uint32_t* __restrict__ bits, uint8_t* __restrict__ u8, int h, int w, int wpr) {
-    const int x = (blockIdx.x * 256 + threadIdx.x) * 4, y = blockIdx.y;
-    if (x >= w) return;
-    const uint32_t nib = (bits[(size_t)y * wpr + (x >> 5)] >> (x & 31)) & 0xfu;   // x % 4 == 0: one word
-    uint8_t* dst = u8 + (size_t)y * w + x;
-    if (x + 3 < w && (reinterpret_cast<uintptr_t>(dst) & 3) == 0) {
-        // spread the 4 bits into 4 bytes (0x01 each)
-        *reinterpret_cast<uint32_t*>(dst) = (nib & 1u) | ((nib & 2u) << 7) | ((nib & 4u) << 14) | ((nib & 8u) << 21);
+    // 16 consecutive bytes of the flat uint8 plane per thread, aligned to 16 bytes of the destination (the
+    // first thread starts at the first aligned address); a group may straddle two rows when w % 16 != 0
+    const size_t P = (size_t)h * w;
+    const int lead = (int)((16 - (reinterpret_cast<uintptr_t>(u8) & 15)) & 15);
+    const size_t g = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (g == 0) {                                    // unaligned head of the plane
+        for (int p = 0; p < lead && (size_t)p < P; ++p) {
+            const int y = p / w, x = p - y * w;
+            u8[p] = (uint8_t)((bits[(size_t)y * wpr + (x >> 5)] >> (x & 31)) & 1u);
+        }
+    }
+    const size_t p0 = (size_t)lead + g * 16;
+    if (p0 >= P) return;
+    const int y = (int)(p0 / w), x = (int)(p0 - (size_t)y * w);
+    if (x + 16 <= w && p0 + 16 <= P) {
+        const uint32_t* row = bits + (size_t)y * wpr;
+        const int wq = x >> 5, sh = x & 31;
+        const uint32_t lo = row[wq], hi = (sh > 16 && wq + 1 < wpr) ? row[wq + 1] : 0u;
+        const uint32_t half = __funnelshift_r(lo, hi, sh) & 0xffffu;
+        uint32_t o[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const uint32_t nib = (half >> (4 * q)) & 0xfu;   // spread 4 bits into 4 bytes (0x01 each)
+            o[q] = (nib & 1u) | ((nib & 2u) << 7) | ((nib & 4u) << 14) | ((nib & 8u) << 21);
+        }
+        *reinterpret_cast<uint4*>(u8 + p0) = make_uint4(o[0], o[1], o[2], o[3]);
     } else {
-        for (int j = 0; j < 4 && x + j < w; ++j) dst[j] = (uint8_t)((nib >> j) & 1u);
+        for (int j = 0; j < 16 && p0 + j < P; ++j) {
+            const size_t p = p0 + j;
+            const int yy = (int)(p / w), xx = (int)(p - (size_t)yy * w);
+            u8[p] = (uint8_t)((bits[(size_t)yy * wpr + (xx >> 5)] >> (xx & 31)) & 1u);
+        }
     }
 }
 

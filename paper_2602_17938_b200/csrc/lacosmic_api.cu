@@ -143,10 +143,11 @@ struct Workspace {
     float* S;          // significance plane; persistent across the iterations of a frame
     int32_t* clist;    // compacted candidate pixel list (capacity h*w)
     int32_t* qlist;    // compacted quad list of the incremental noise/S pass (capacity h*ceil(w/4))
-    uint32_t *G1, *G2, *M1, *M2, *M3, *C[2], *A1, *A2, *NEED;
+    uint32_t *G1, *G2, *G2F, *M1, *M2, *M3, *C[2], *A1, *A2, *NEED;
     int32_t* counts;   // per iteration: newly flagged pixels
     int32_t* ncand;    // per iteration (lazy path): candidate pixels evaluated
     int32_t* nquad;    // per iteration (lazy path): quads the incremental noise/S pass recomputed
+    uint8_t* stripflag; // per 30-word x 8-row strip of the bit-planes (grow.cuh): R not empty in it
     size_t bytes;      // total
     size_t zero_off, zero_bytes;   // region cleared at the start of a frame: the counters
 };
@@ -161,8 +162,10 @@ Workspace carve(void* base, int h, int w) {
     ws.S = (float*)(p + off); off += plane;
     ws.clist = (int32_t*)(p + off); off += plane;
     ws.qlist = (int32_t*)(p + off); off += align_up((size_t)h * ((w + 3) / 4) * 4, 256);
-    uint32_t** planes[] = {&ws.G1, &ws.G2, &ws.M1, &ws.M2, &ws.M3, &ws.C[0], &ws.C[1], &ws.A1, &ws.A2, &ws.NEED};
+    uint32_t** planes[] = {&ws.G1, &ws.G2, &ws.G2F, &ws.M1, &ws.M2, &ws.M3, &ws.C[0], &ws.C[1], &ws.A1, &ws.A2, &ws.NEED};
     for (uint32_t** pl : planes) { *pl = (uint32_t*)(p + off); off += bp; }
+    ws.stripflag = (uint8_t*)(p + off);
+    off += align_up((size_t)((words_per_row(w) + lac::WG_OWN - 1) / lac::WG_OWN) * ((h + lac::WG_R - 1) / lac::WG_R + lac::WG_WARPS), 256);
     ws.zero_off = off;
     ws.counts = (int32_t*)(p + off); off += align_up(NCOUNTERS * 4, 256);
     ws.ncand = ws.counts + LACOSMIC_MAX_NITER;
@@ -173,7 +176,7 @@ Workspace carve(void* base, int h, int w) {
 }
 
 int unpack(const uint32_t* bits, uint8_t* u8, int h, int w, cudaStream_t st) {
-    dim3 g((w + 1023) / 1024, h);
+    const unsigned g = (unsigned)(((size_t)h * w / 16 + 1 + 255) / 256);   // one thread per aligned 16 bytes (+ head)
     Span sp(KC_BITS, st);
     lac::k_unpack_bits<<<g, 256, 0, st>>>(bits, u8, h, w, words_per_row(w));
     LAUNCHED();
@@ -182,13 +185,16 @@ int unpack(const uint32_t* bits, uint8_t* u8, int h, int w, cudaStream_t st) {
 
 // grid of the bit-plane list kernels: 32 words x 64 rows per CTA (common.cuh)
 inline dim3 bit_grid(int h, int w) { return dim3((words_per_row(w) + 31) / 32, (h + lac::BW_CTA_ROWS - 1) / lac::BW_CTA_ROWS); }
-// grid of k_grow_replace / k_dirty_lists: 32 words x 32 rows per CTA (grow.cuh)
-inline dim3 grow_grid(int h, int w) { return dim3((words_per_row(w) + lac::GT_W - 1) / lac::GT_W, (h + lac::GT_H - 1) / lac::GT_H); }
+// grid of k_grow_replace / k_dirty_lists: 30 words x 64 rows per CTA, one 30 x 8 strip per warp (grow.cuh)
+inline dim3 grow_grid(int h, int w) {
+    const int rows = lac::WG_R * lac::WG_WARPS;
+    return dim3((words_per_row(w) + lac::WG_OWN - 1) / lac::WG_OWN, (h + rows - 1) / rows);
+}
 
 // steps (6)-(7) of one iteration, fused (grow.cuh)
 int grow_replace(const lac::GrowArgs& ga, const int* prev, cudaStream_t st) {
     Span sp(KC_GROW, st);
-    lac::k_grow_replace<<<grow_grid(ga.h, ga.w), 256, 0, st>>>(ga, prev);
+    lac::k_grow_replace<<<grow_grid(ga.h, ga.w), 32 * lac::WG_WARPS, 0, st>>>(ga, prev);
     LAUNCHED();
     return LACOSMIC_OK;
 }
@@ -248,8 +254,8 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         if (incr) {
             {
                 Span sp(KC_LISTS, st);
-                lac::k_dirty_lists<<<grow_grid(h, w), 256, 0, st>>>(ws.NEED, ws.A1, ws.G1, ws.G2, ws.M1, ws.qlist,
-                                                                   ws.nquad + t, ws.clist, ws.ncand + t, h, w, wpr, prev);
+                lac::k_dirty_lists<<<grow_grid(h, w), 32 * lac::WG_WARPS, 0, st>>>(ws.NEED, ws.A1, ws.G1, ws.G2, ws.G2F, ws.M1, ws.qlist,
+                                                                   ws.nquad + t, ws.clist, ws.ncand + t, ws.stripflag, h, w, wpr, prev);
                 LAUNCHED();
             }
             {
@@ -267,7 +273,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
             }
             if (lazy) {
                 Span sp(KC_LISTS, st);
-                lac::k_list_candidates<<<bit_grid(h, w), 256, 0, st>>>(ws.A1, t > 0 ? ws.NEED : nullptr, ws.G1, ws.G2, ws.M1,
+                lac::k_list_candidates<<<bit_grid(h, w), 256, 0, st>>>(ws.A1, t > 0 ? ws.NEED : nullptr, ws.G1, ws.G2, ws.G2F, ws.M1,
                                                                       ws.clist, ws.ncand + t, h, w, wpr, prev);
                 LAUNCHED();
             }
@@ -288,9 +294,9 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         }
         if (d && dbg->S) CK(cudaMemcpyAsync(dbg->S, ws.S, P * 4, cudaMemcpyDeviceToDevice, st));
         // steps (6)-(7), fused; in the lazy path G2 is completed on the pixels the second growth reaches
-        lac::GrowArgs ga{ws.M1, ws.G1, ws.G2, lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
+        lac::GrowArgs ga{ws.M1, ws.G1, ws.G2, ws.G2F, lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
                          ws.C[t & 1], ws.C[(t + 1) & 1], ws.NEED, d ? ws.M2 : nullptr, d ? ws.M3 : nullptr,
-                         ws.S, img, work, ws.counts + t, h, w, wpr, siglow};
+                         ws.S, img, work, ws.counts + t, incr ? ws.stripflag : nullptr, h, w, wpr, siglow};
         if ((rc = grow_replace(ga, prev, st))) return rc;
         if (d) {
             // lazy path: G2 is only evaluated where step (6) needs it, so it is not dumped
@@ -505,8 +511,8 @@ int lacosmic_masked_median(const float* img, const uint8_t* mask_u8, float* out,
     CK(cudaMemcpyAsync(out, img, P * 4, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemsetAsync(ws.C[0], 0, (size_t)h * wpr * 4, st));
     CK(cudaMemsetAsync(ws.counts, 0, 4, st));
-    lac::GrowArgs ga{ws.M1, ws.M1, ws.M1, nullptr, nullptr, ws.C[0], ws.C[1], ws.NEED, nullptr, nullptr,
-                     nullptr, img, out, ws.counts, h, w, wpr, 0.0f};
+    lac::GrowArgs ga{ws.M1, ws.M1, ws.M1, nullptr, nullptr, nullptr, ws.C[0], ws.C[1], ws.NEED, nullptr, nullptr,
+                     nullptr, img, out, ws.counts, nullptr, h, w, wpr, 0.0f};
     return grow_replace(ga, nullptr, st);
 }
 

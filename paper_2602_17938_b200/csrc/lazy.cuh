@@ -30,10 +30,10 @@ namespace lac {
 // replacement pass of iteration t-1 rewrote the pixels NEED, only the tests inside R = dil9x9(NEED) can
 // change: iteration t clears G1, G2, M1 inside R and re-evaluates the candidates there.
 
-// list <- pixels of A1 & R; clear G1, G2, M1 inside R (R = everything when `dirty` is NULL)
+// list <- pixels of A1 & R; clear G1, G2, G2F (grow.cuh), M1 inside R (R = everything when `dirty` is NULL)
 __global__ void __launch_bounds__(256)
 k_list_candidates(const uint32_t* __restrict__ A1, const uint32_t* __restrict__ dirty, uint32_t* __restrict__ G1,
-                  uint32_t* __restrict__ G2, uint32_t* __restrict__ M1, int* __restrict__ list,
+                  uint32_t* __restrict__ G2, uint32_t* __restrict__ G2F, uint32_t* __restrict__ M1, int* __restrict__ list,
                   int* __restrict__ nlist, int h, int w, int wpr, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
@@ -58,9 +58,9 @@ k_list_candidates(const uint32_t* __restrict__ A1, const uint32_t* __restrict__ 
             if (r == 0) continue;
             bits[i] = A1[q] & r;
             if (r == 0xffffffffu) {
-                G1[q] = 0; G2[q] = 0; M1[q] = 0;
+                G1[q] = 0; G2[q] = 0; G2F[q] = 0; M1[q] = 0;
             } else {
-                G1[q] &= ~r; G2[q] &= ~r; M1[q] &= ~r;
+                G1[q] &= ~r; G2[q] &= ~r; G2F[q] &= ~r; M1[q] &= ~r;
             }
         }
     }
@@ -260,7 +260,7 @@ k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restric
 // groups of 4 pixels holding a pixel within 2 px of a rewritten one; k_dirty_lists), one quad per thread, with
 // the same window network and the same operations as the dense pass (kernels.cuh, noise_S_tile).  The
 // pixels of the quad with S > sigclip are appended to the candidate list (one atomic per CTA and round).
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 k_noise_S_quads(const float* __restrict__ work, NoiseArgs a, const int* __restrict__ qlist,
                 const int* __restrict__ nq, int* __restrict__ clist, int* __restrict__ nc, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
