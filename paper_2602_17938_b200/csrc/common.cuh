@@ -59,6 +59,23 @@ __device__ __forceinline__ float lplus_px(float c, float U, float D, float Lf, f
     return __fmul_rn(__fadd_rn(__fadd_rn(a, b), __fadd_rn(g, d)), 0.25f);
 }
 
+// fdiv(num, den) for num >= +0: the value of __fdiv_rn(num, den), but a zero numerator (about 30 % of the L+
+// values) does not take the division's slow path, which the range check of the fast path (FCHK) sends it to:
+// +0 / den = +0 for every den > 0, infinity included.
+__device__ __forceinline__ float fdiv_nn(float num, float den) {
+    const bool z = (num == 0.0f) & (den > 0.0f);
+    const float q = __fdiv_rn(z ? 1.0f : num, den);
+    return z ? 0.0f : q;
+}
+
+// O2: N = sqrt(gain * max(med5, 1e-4) + rn^2) / gain.  gain == 1 (uniform) skips the multiply and the
+// division, which are exact identities then.
+__device__ __forceinline__ float noise_px(float m5, float gain, float rn2) {
+    const float m5c = m5 > 1e-4f ? m5 : 1e-4f;                                            // R5
+    if (gain == 1.0f) return __fsqrt_rn(__fadd_rn(m5c, rn2));
+    return __fdiv_rn(__fsqrt_rn(__fadd_rn(__fmul_rn(gain, m5c), rn2)), gain);
+}
+
 // ---- block-wide compaction of bit-plane words into a pixel list ------------------------------------
 // Bit-plane kernels use 256-thread CTAs (32 lanes x 8 warps); thread (lane, wi) owns NR words of one word
 // column (word wx, rows y .. y+NR-1).  All 256 threads must call block_append: it appends the flat pixel

@@ -147,9 +147,8 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
             for (int j = 0; j < 4; ++j) {
                 ctr[j] = win[2 + j][2];
                 lp[j] = lplus_px(win[2 + j][2], win[2 + j][1], win[2 + j][3], win[1 + j][2], win[3 + j][2]);
-                float m5c = m5[j] > 1e-4f ? m5[j] : 1e-4f;                                 // R5
-                n[j] = __fdiv_rn(__fsqrt_rn(__fadd_rn(__fmul_rn(a.gain, m5c), a.rn2)), a.gain);
-                s[j] = __fdiv_rn(lp[j], __fmul_rn(2.0f, n[j]));
+                n[j] = noise_px(m5[j], a.gain, a.rn2);
+                s[j] = fdiv_nn(lp[j], __fmul_rn(2.0f, n[j]));
                 const bool ok = (x + j < a.w) && (win[2 + j][2] < a.satlevel);            // R12
                 n1 |= (uint32_t)(ok && s[j] > a.sigclip) << j;
                 n2 |= (uint32_t)(ok && s[j] > a.siglow) << j;
@@ -275,7 +274,7 @@ __device__ __forceinline__ void fine_gates_tile(const float* smA, float* smB, co
                 bool ok = (x + j < w) && (ctr[1 + j] < a.gp.satlevel);            // R12
                 bool g1 = ok && (sp[j] > a.gp.sigclip);
                 bool g2 = ok && (sp[j] > a.gp.siglow);
-                bool m1 = g1 && (__fdiv_rn(lp, f[j]) > a.gp.objlim);               // R8
+                bool m1 = g1 && (fdiv_nn(lp, f[j]) > a.gp.objlim);               // R8
                 n1 |= (uint32_t)g1 << j;
                 n2 |= (uint32_t)g2 << j;
                 n3 |= (uint32_t)m1 << j;
@@ -466,18 +465,19 @@ __global__ void __launch_bounds__(256)
 k_unpack_bits(const uint32_t* __restrict__ bits, uint8_t* __restrict__ u8, int h, int w, int wpr) {
     // 16 consecutive bytes of the flat uint8 plane per thread, aligned to 16 bytes of the destination (the
     // first thread starts at the first aligned address); a group may straddle two rows when w % 16 != 0
-    const size_t P = (size_t)h * w;
+    const unsigned P = (unsigned)h * (unsigned)w;   // h * w < 2^31 (checked at the boundary): 32-bit index math
     const int lead = (int)((16 - (reinterpret_cast<uintptr_t>(u8) & 15)) & 15);
-    const size_t g = (size_t)blockIdx.x * 256 + threadIdx.x;
+    const unsigned g = blockIdx.x * 256u + threadIdx.x;
     if (g == 0) {                                    // unaligned head of the plane
-        for (int p = 0; p < lead && (size_t)p < P; ++p) {
+        for (int p = 0; p < lead && (unsigned)p < P; ++p) {
             const int y = p / w, x = p - y * w;
             u8[p] = (uint8_t)((bits[(size_t)y * wpr + (x >> 5)] >> (x & 31)) & 1u);
         }
     }
-    const size_t p0 = (size_t)lead + g * 16;
+    if (g >= (P + 15u) / 16u + 1u) return;
+    const unsigned p0 = (unsigned)lead + g * 16u;
     if (p0 >= P) return;
-    const int y = (int)(p0 / w), x = (int)(p0 - (size_t)y * w);
+    const int y = (int)(p0 / (unsigned)w), x = (int)(p0 - (unsigned)y * (unsigned)w);
     if (x + 16 <= w && p0 + 16 <= P) {
         const uint32_t* row = bits + (size_t)y * wpr;
         const int wq = x >> 5, sh = x & 31;
@@ -492,8 +492,8 @@ k_unpack_bits(const uint32_t* __restrict__ bits, uint8_t* __restrict__ u8, int h
         *reinterpret_cast<uint4*>(u8 + p0) = make_uint4(o[0], o[1], o[2], o[3]);
     } else {
         for (int j = 0; j < 16 && p0 + j < P; ++j) {
-            const size_t p = p0 + j;
-            const int yy = (int)(p / w), xx = (int)(p - (size_t)yy * w);
+            const unsigned p = p0 + j;
+            const int yy = (int)(p / (unsigned)w), xx = (int)(p - (unsigned)yy * (unsigned)w);
             u8[p] = (uint8_t)((bits[(size_t)yy * wpr + (xx >> 5)] >> (xx & 31)) & 1u);
         }
     }
