@@ -100,7 +100,10 @@ struct GrowArgs {
     float siglow;
 };
 
-__global__ void __launch_bounds__(32 * WG_WARPS, 3)
+#ifndef LAC_GROW_MINB
+#define LAC_GROW_MINB 3
+#endif
+__global__ void __launch_bounds__(32 * WG_WARPS, LAC_GROW_MINB)
 k_grow_replace(GrowArgs a, const int* prev_count) {
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const int h = a.h, w = a.w, wpr = a.wpr;

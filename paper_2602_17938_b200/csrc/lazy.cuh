@@ -170,7 +170,10 @@ __device__ __forceinline__ bool fine_bracket(float lp, float m3c, float objlim, 
 // Virtual 9x9 window V[r][c] = work<y-4+r, x-4+c>; the m3-plane tap (dy, dx) of the 7x7 window is med3x3
 // centred on the virtual position (cy(dy), cx(dx)), cy(dy) = clamp(y+dy) - y (R4: the STORED m3 plane is
 // replicated), whose own taps are V[cy+4+-1][cx+4+-1] (R3).
-__global__ void __launch_bounds__(128)
+#ifndef LAC_EVAL_MINB
+#define LAC_EVAL_MINB 6
+#endif
+__global__ void __launch_bounds__(128, LAC_EVAL_MINB)
 k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restrict__ nlist,
                   const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
