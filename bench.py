@@ -252,6 +252,42 @@ def run_cuda(args):
                        and res["counts"] == res_other["counts"])
     mask_frac = float(res["mask"].float().mean().item())
 
+    # ---- configs[3] in small: a stream of independent frames with per-frame parameters, resident in HBM,
+    # through lacosmic_run_batch, back to back (concurrency 1) and with several frames in flight
+    stream_res = None
+    if args.stream_frames > 0 and main_mode == "lazy":
+        nf = args.stream_frames
+        cfg = synth.stream_config(nf)
+        imgs = torch.empty((nf, h, w), dtype=torch.float32, device=dev)
+        for j, (kwj, _) in enumerate(cfg):
+            kwj = dict(kwj)
+            kwj["seed"] += 100 * rank
+            imgs[j].copy_(torch.from_numpy(synth.make_frame(**kwj).img))
+        plist = [lc.Params(mode=lc.MODE_LAZY, **pj) for _, pj in cfg]
+        masks = torch.empty((nf, h, w), dtype=torch.uint8, device=dev)
+        cleans = torch.empty_like(imgs)
+        bcounts = torch.zeros((nf, lc.MAX_NITER), dtype=torch.int32, device=dev)
+        stream_res = dict(frames=nf, workload="configs[3] generator (seeds 1000.., sigclip cycling 4.0/4.5/5.0), "
+                                             "%d frames resident in HBM" % nf)
+        ref_out = None
+        for kc in (1, args.stream_concurrency):
+            bws = torch.empty(lc.lacosmic_batch_workspace_bytes(h, w, kc), dtype=torch.uint8, device=dev)
+
+            def step_batch():
+                lc.lacosmic_run_batch(imgs, plist, masks_out=masks, cleans_out=cleans, workspace=bws,
+                                      iter_counts=bcounts)
+            ms_b = timed(step_batch, 3, 1)
+            out = (masks.clone(), cleans.clone())
+            if ref_out is None:
+                ref_out = out
+            else:
+                stream_res["same_as_back_to_back"] = bool(torch.equal(out[0], ref_out[0]) and
+                                                          torch.equal(out[1], ref_out[1]))
+            stream_res["concurrency_%d" % kc] = dict(frames_per_s=world * nf * 1e3 / ms_b, ms_per_frame=ms_b / nf)
+            del bws
+        del imgs, masks, cleans, ref_out, out
+        torch.cuda.empty_cache()
+
     # ---- end to end through the host-buffer C-ABI call
     img_h = torch.from_numpy(frame.img).pin_memory()
     mask_h = torch.empty((h, w), dtype=torch.uint8).pin_memory()
@@ -342,6 +378,7 @@ def run_cuda(args):
         ref_comparisons_T_per_s=ref_cmp_rate,
         other_mode=dict(mode=other_mode, same_mask_clean_counts=modes_agree, roofline=roofline(res_other),
                         **summarise(res_other)),
+        stream=stream_res,
         new_cr_per_iteration=res["counts"], mask_fraction=mask_frac,
         clocks=clocks, cpu_baseline=cpu,
         context="paper (PAPER.md:31,47): 55 s/frame dfcosmic C++ at 2 threads on AWS; GPU variant on an "
@@ -378,6 +415,10 @@ def main():
     ap.add_argument("--mode", default="lazy", choices=["lazy", "dense"],
                     help="which evaluation mode is the headline (the other is measured and reported too)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--stream-frames", type=int, default=12,
+                    help="frames of the configs[3] stream leg (0 = skip; 64 = the full configuration)")
+    ap.add_argument("--stream-concurrency", type=int, default=4,
+                    help="frames in flight in the stream leg (lacosmic_run_batch internal streams)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3                          # timing rule: at least 3 warm-up steps

@@ -111,10 +111,17 @@ int lacosmic_run_ws(const float *img, int h, int w, const lacosmic_params *p, ui
                     float *clean_out, void *workspace, size_t workspace_bytes, int32_t *iter_counts,
                     const lacosmic_debug *dbg, void *stream);
 
-/* n independent frames back to back ("batch processing"; BASELINE.json configs[3]).
+/* n independent frames ("batch processing"; BASELINE.json configs[3]).
  * imgs/masks_out/cleans_out are [n][h][w]; params is a HOST array of n structs (per-frame
- * parameters, read during the call); workspace as for lacosmic_run_ws (one frame's worth, reused);
- * iter_counts: nullable device array [n][LACOSMIC_MAX_NITER]. */
+ * parameters, read during the call); iter_counts: nullable device array [n][LACOSMIC_MAX_NITER].
+ * workspace: k = min(n, LACOSMIC_MAX_BATCH_STREAMS, workspace_bytes / lacosmic_workspace_bytes(h,w))
+ * frames are in flight at a time, each with its own slice of the workspace, on k internal streams
+ * that fork from and join back into `stream` with events (no host synchronisation; outputs are valid
+ * once `stream` reaches the end of the call's work).  One frame's worth of workspace (k = 1) runs the
+ * frames back to back on `stream` itself.  Most launches of a frame are latency bound, so frames in
+ * flight together overlap well: lacosmic_batch_workspace_bytes(h, w, k) gives the size for k. */
+size_t lacosmic_batch_workspace_bytes(int h, int w, int concurrency);
+#define LACOSMIC_MAX_BATCH_STREAMS 8
 int lacosmic_run_batch(const float *imgs, int n, int h, int w, const lacosmic_params *params,
                        uint8_t *masks_out, float *cleans_out, void *workspace,
                        size_t workspace_bytes, int32_t *iter_counts, void *stream);

@@ -5,6 +5,7 @@ include/lacosmic.h).  This package only marshals arguments; torch is used for de
 streams.  There is no CPU fallback: every call raises if the CUDA library cannot be loaded.
 """
 from .binding import (  # noqa: F401
+    MAX_NITER,
     MODE_DENSE,
     MODE_LAZY,
     LacosmicError,
@@ -27,10 +28,11 @@ from .binding import (  # noqa: F401
     lacosmic_unpack_bits,
     lacosmic_version,
     lacosmic_workspace_bytes,
+    lacosmic_batch_workspace_bytes,
     library_path,
     load_library,
 )
 
 __all__ = [n for n in dir() if n.startswith("lacosmic_")] + ["LacosmicError", "Params",
                                                               "library_path", "load_library",
-                                                              "MODE_LAZY", "MODE_DENSE"]
+                                                              "MODE_LAZY", "MODE_DENSE", "MAX_NITER"]

@@ -17,6 +17,7 @@ _lib = None
 
 EXPORTS = (
     "lacosmic_run", "lacosmic_workspace_bytes", "lacosmic_run_ws", "lacosmic_run_batch",
+    "lacosmic_batch_workspace_bytes",
     "lacosmic_host_workspace_bytes", "lacosmic_run_host", "lacosmic_lplus", "lacosmic_medfilt",
     "lacosmic_bitplane_pitch_words", "lacosmic_pack_bits", "lacosmic_unpack_bits",
     "lacosmic_dilate3", "lacosmic_masked_median", "lacosmic_strerror",
@@ -86,6 +87,7 @@ def load_library():
     sig = {
         "lacosmic_run": (i, [vp, i, i, f, f, f, f, f, i, f, vp, vp, vp]),
         "lacosmic_workspace_bytes": (sz, [i, i]),
+        "lacosmic_batch_workspace_bytes": (sz, [i, i, i]),
         "lacosmic_run_ws": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp,
                                 C.POINTER(_CDebug), vp]),
         "lacosmic_run_batch": (i, [vp, i, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp, vp]),
@@ -160,6 +162,10 @@ def lacosmic_workspace_bytes(h, w):
     return int(load_library().lacosmic_workspace_bytes(int(h), int(w)))
 
 
+def lacosmic_batch_workspace_bytes(h, w, concurrency):
+    return int(load_library().lacosmic_batch_workspace_bytes(int(h), int(w), int(concurrency)))
+
+
 def lacosmic_host_workspace_bytes(h, w):
     return int(load_library().lacosmic_host_workspace_bytes(int(h), int(w)))
 
@@ -223,8 +229,9 @@ def lacosmic_run_ws(img, params=None, mask_out=None, clean_out=None, workspace=N
 
 
 def lacosmic_run_batch(imgs, params, masks_out=None, cleans_out=None, workspace=None,
-                       iter_counts=None, stream=None):
-    """imgs [n][h][w]; params: list of n Params.  Returns dict(mask, clean, counts [n][MAX_NITER])."""
+                       iter_counts=None, stream=None, concurrency=1):
+    """imgs [n][h][w]; params: list of n Params.  Returns dict(mask, clean, counts [n][MAX_NITER]).
+    `concurrency` sizes the workspace this call allocates when none is given (frames in flight)."""
     torch = _torch()
     L = load_library()
     if imgs.dim() != 3:
@@ -238,7 +245,8 @@ def lacosmic_run_batch(imgs, params, masks_out=None, cleans_out=None, workspace=
     if cleans_out is None:
         cleans_out = torch.empty_like(imgs)
     if workspace is None:
-        workspace = _workspace(h, w, imgs.device)
+        workspace = torch.empty(max(lacosmic_batch_workspace_bytes(h, w, max(1, concurrency)), 256),
+                                dtype=torch.uint8, device=imgs.device)
     if iter_counts is None:
         iter_counts = torch.zeros((max(n, 1), MAX_NITER), dtype=torch.int32, device=imgs.device)
     rc = L.lacosmic_run_batch(_dev(imgs, torch.float32, "imgs"), n, h, w, arr,

@@ -17,10 +17,10 @@ struct GateParams {
 };
 
 // Edge-replicate tile load with margins (R3): sm[r][c] = src<y0-MY+r, x0-MX+c>.
-template <int MX, int MY, int PITCH>
+template <int MX, int MY, int PITCH, int TILE_H = TH>
 __device__ __forceinline__ void load_tile(float* sm, const float* __restrict__ src, int h, int w, int y0,
                                           int x0, int tid) {
-    constexpr int SW = TW + 2 * MX, SH = TH + 2 * MY;
+    constexpr int SW = TW + 2 * MX, SH = TILE_H + 2 * MY;
     static_assert(PITCH >= SW && PITCH % 4 == 0, "pitch must hold the tile and keep float4 alignment");
     for (int i = tid; i < SW * SH; i += NT) {
         int r = i / SW, c = i - r * SW;
@@ -103,7 +103,11 @@ __global__ void __launch_bounds__(NT) k_lplus(const float* __restrict__ in, floa
 // ------------------------------------------------------------------------------------------------
 // K_A: steps (1)-(3a).  work -> L+ (recomputed later, not stored), N = sqrt(gain*med5+rn^2)/gain,
 // S = L+/(2N).  Writes S; Lp/N only when a debug plane is requested.
-constexpr int NS_MX = 4, NS_MY = 2, NS_PITCH = TW + 2 * NS_MX, NS_ROWS = TH + 2 * NS_MY;
+#ifndef LAC_NS_TH
+#define LAC_NS_TH 16
+#endif
+constexpr int NS_TH = LAC_NS_TH;   // tile height of the noise/S pass (own constant: its tile is much lighter than K_B's)
+constexpr int NS_MX = 4, NS_MY = 2, NS_PITCH = TW + 2 * NS_MX, NS_ROWS = NS_TH + 2 * NS_MY;
 
 struct NoiseArgs {
     float* S;
@@ -134,7 +138,7 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
                                              int wi) {
     const int lx = lane & 7, lr = lane >> 3;
 #pragma unroll 1
-    for (int u = wi; u < (TW / UW) * (TH / UH); u += NWARP) {
+    for (int u = wi; u < (TW / UW) * (NS_TH / UH); u += NWARP) {
         const int xu = x0 + (u & 3) * UW, lyu = (u >> 2) * UH, yu = y0 + lyu;
         if (yu >= a.h || xu >= a.w) continue;                                            // warp-uniform
         const int ly = lyu + lr, y = y0 + ly, x = xu + 4 * lx;
@@ -178,8 +182,8 @@ k_noise_S(const float* __restrict__ work, NoiseArgs a, int ntx, const int* prev_
     const int tid = threadIdx.x;
     const int t = blockIdx.x;
     const int ty = t / ntx, tx = t - ty * ntx;
-    const int x0 = tx * TW, y0 = ty * TH;
-    load_tile<NS_MX, NS_MY, NS_PITCH>(sm, work, a.h, a.w, y0, x0, tid);
+    const int x0 = tx * TW, y0 = ty * NS_TH;
+    load_tile<NS_MX, NS_MY, NS_PITCH, NS_TH>(sm, work, a.h, a.w, y0, x0, tid);
     __syncthreads();
     noise_S_tile(sm, a, x0, y0, tid & 31, tid >> 5);
 }
@@ -372,7 +376,7 @@ k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx,
     auto issue = [&](int t, int st) {
         int ty = t / ntx, tx = t - ty * ntx;
         mbar_expect_tx(&full[st], TILE_BYTES);
-        tma_load_2d(buf(st), &mapWork, tx * TW - NS_MX, ty * TH - NS_MY, &full[st]);
+        tma_load_2d(buf(st), &mapWork, tx * TW - NS_MX, ty * NS_TH - NS_MY, &full[st]);
     };
     int i = blockIdx.x;
     if (tid == 0 && i < nt) issue(tile_of(i), 0);
@@ -382,8 +386,8 @@ k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx,
         mbar_wait(&full[st], (it >> 1) & 1);
         const int t = tile_of(i);
         const int ty = t / ntx, tx = t - ty * ntx;
-        const int x0 = tx * TW, y0 = ty * TH;
-        if (y0 - NS_MY < 0 || y0 + TH + NS_MY > a.h || x0 - NS_MX < 0 || x0 + TW + NS_MX > a.w) {
+        const int x0 = tx * TW, y0 = ty * NS_TH;
+        if (y0 - NS_MY < 0 || y0 + NS_TH + NS_MY > a.h || x0 - NS_MX < 0 || x0 + TW + NS_MX > a.w) {
             replicate_fix<NS_ROWS, NS_PITCH>(buf(st), y0 - NS_MY, x0 - NS_MX, a.h, a.w, tid);
             fence_proxy_async();
             __syncthreads();

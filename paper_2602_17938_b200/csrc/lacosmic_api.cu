@@ -221,6 +221,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     // TMA path needs 16-byte row pitch; other widths take the generic tile loader
     const bool tma = (w % 4 == 0);
     const int ntx = (int)tg.x, ntiles = (int)(tg.x * tg.y);
+    const int ntilesNS = ntx * ((h + lac::NS_TH - 1) / lac::NS_TH);   // tiles of the noise/S pass
     CUtensorMap mapWorkNS, mapImgNS, mapWorkFG, mapS;
     int gridNS = 0, gridFG = 0, gridQ = 1184, gridE = 2368;
     if (p.niter > 0) {
@@ -236,7 +237,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                 g_last_cuda_error = (int)cudaErrorInvalidValue;
                 return LACOSMIC_ERR_CUDA;
             }
-            gridNS = std::min(ntiles, di.sms * di.occ_noise);
+            gridNS = std::min(ntilesNS, di.sms * di.occ_noise);
             gridFG = std::min(ntiles, di.sms * di.occ_fine);
         }
     }
@@ -267,8 +268,8 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
             const float* src = (fused_copy && t == 0) ? img : work;
             {
                 Span sp(KC_NOISE_S, st);
-                if (tma) lac::k_noise_S_tma<<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(src == img ? mapImgNS : mapWorkNS, na, ntx, ntiles, prev);
-                else lac::k_noise_S<<<ntiles, tb, 0, st>>>(src, na, ntx, prev);
+                if (tma) lac::k_noise_S_tma<<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(src == img ? mapImgNS : mapWorkNS, na, ntx, ntilesNS, prev);
+                else lac::k_noise_S<<<ntilesNS, tb, 0, st>>>(src, na, ntx, prev);
                 LAUNCHED();
             }
             if (lazy) {
@@ -312,6 +313,32 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     if (iter_counts && p.niter > 0)
         CK(cudaMemcpyAsync(iter_counts, ws.counts, (size_t)p.niter * 4, cudaMemcpyDeviceToDevice, st));
     return LACOSMIC_OK;
+}
+
+// Internal streams of lacosmic_run_batch (per calling thread and device, created on first use, kept for the
+// life of the thread): non-blocking, forked from / joined into the caller's stream with events.
+struct BatchStreams {
+    int dev = -1;
+    cudaStream_t st[LACOSMIC_MAX_BATCH_STREAMS];
+    cudaEvent_t fork, join[LACOSMIC_MAX_BATCH_STREAMS];
+};
+BatchStreams* batch_streams() {
+    thread_local BatchStreams pool[16];
+    thread_local int npool = 0;
+    int dev = 0;
+    if (!cuda_ok(cudaGetDevice(&dev))) return nullptr;
+    for (int i = 0; i < npool; ++i)
+        if (pool[i].dev == dev) return &pool[i];
+    if (npool == 16) return nullptr;
+    BatchStreams& b = pool[npool];
+    if (!cuda_ok(cudaEventCreateWithFlags(&b.fork, cudaEventDisableTiming))) return nullptr;
+    for (int s = 0; s < LACOSMIC_MAX_BATCH_STREAMS; ++s) {
+        if (!cuda_ok(cudaStreamCreateWithFlags(&b.st[s], cudaStreamNonBlocking))) return nullptr;
+        if (!cuda_ok(cudaEventCreateWithFlags(&b.join[s], cudaEventDisableTiming))) return nullptr;
+    }
+    b.dev = dev;
+    ++npool;
+    return &b;
 }
 
 int check_frame_args(const float* img, int h, int w, const lacosmic_params* p, const uint8_t* mask_out,
@@ -370,6 +397,11 @@ int lacosmic_run(const float* img, int h, int w, float gain, float readnoise, fl
     return rc;
 }
 
+size_t lacosmic_batch_workspace_bytes(int h, int w, int concurrency) {
+    if (check_shape(h, w) || concurrency < 1) return 0;
+    return (size_t)std::min(concurrency, LACOSMIC_MAX_BATCH_STREAMS) * align_up(lacosmic_workspace_bytes(h, w), 256);
+}
+
 int lacosmic_run_batch(const float* imgs, int n, int h, int w, const lacosmic_params* params,
                        uint8_t* masks_out, float* cleans_out, void* workspace, size_t workspace_bytes,
                        int32_t* iter_counts, void* stream) {
@@ -392,16 +424,40 @@ int lacosmic_run_batch(const float* imgs, int n, int h, int w, const lacosmic_pa
     if (overlap(imgs, n * P * 4, cleans_out, n * P * 4) || overlap(imgs, n * P * 4, masks_out, n * P) ||
         overlap(cleans_out, n * P * 4, masks_out, n * P))
         return LACOSMIC_ERR_ALIAS;
-    Workspace ws = carve(workspace, h, w);
-    for (int f = 0; f < n; ++f) {
-        rc = run_frame(imgs + f * P, h, w, params[f], masks_out + f * P, cleans_out + f * P, ws, nullptr,
-                       nullptr, (cudaStream_t)stream);
-        if (rc) return rc;
-        if (iter_counts)
-            CK(cudaMemcpyAsync(iter_counts + (size_t)f * LACOSMIC_MAX_NITER, ws.counts,
-                               LACOSMIC_MAX_NITER * 4, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    const size_t slice = align_up(lacosmic_workspace_bytes(h, w), 256);
+    const int k = (int)std::min<size_t>(std::min(n, LACOSMIC_MAX_BATCH_STREAMS), workspace_bytes / slice);
+    if (overlap(workspace, (size_t)k * slice, imgs, n * P * 4) || overlap(workspace, (size_t)k * slice, cleans_out, n * P * 4) ||
+        overlap(workspace, (size_t)k * slice, masks_out, n * P))
+        return LACOSMIC_ERR_ALIAS;
+    cudaStream_t caller = (cudaStream_t)stream;
+    BatchStreams* bs = nullptr;
+    if (k > 1) {
+        bs = batch_streams();
+        if (!bs) return LACOSMIC_ERR_CUDA;
+        CK(cudaEventRecord(bs->fork, caller));
+        for (int s = 0; s < k; ++s) CK(cudaStreamWaitEvent(bs->st[s], bs->fork, 0));
     }
-    return LACOSMIC_OK;
+    for (int f = 0; f < n; ++f) {
+        const int s = f % k;
+        cudaStream_t st = k > 1 ? bs->st[s] : caller;
+        Workspace ws = carve((char*)workspace + (size_t)s * slice, h, w);
+        rc = run_frame(imgs + f * P, h, w, params[f], masks_out + f * P, cleans_out + f * P, ws, nullptr,
+                       nullptr, st);
+        if (rc) break;
+        if (iter_counts && !cuda_ok(cudaMemcpyAsync(iter_counts + (size_t)f * LACOSMIC_MAX_NITER, ws.counts,
+                                                    LACOSMIC_MAX_NITER * 4, cudaMemcpyDeviceToDevice, st))) {
+            rc = LACOSMIC_ERR_CUDA;
+            break;
+        }
+    }
+    if (k > 1) {   // join, also after an error: the caller's stream must not run ahead of work already enqueued
+        for (int s = 0; s < k; ++s) {
+            if (!cuda_ok(cudaEventRecord(bs->join[s], bs->st[s])) ||
+                !cuda_ok(cudaStreamWaitEvent(caller, bs->join[s], 0)))
+                rc = rc ? rc : LACOSMIC_ERR_CUDA;
+        }
+    }
+    return rc;
 }
 
 size_t lacosmic_host_workspace_bytes(int h, int w) {

@@ -237,16 +237,21 @@ def test_north_star_signature_and_host_variant(lc, orc):
     assert np.array_equal(r["mask"].numpy(), o["mask"]) and np.array_equal(r["clean"].numpy(), o["clean"])
 
 
-def test_batch_with_per_frame_parameters(lc, orc):
+@pytest.mark.parametrize("concurrency", [1, 3, 8])
+def test_batch_with_per_frame_parameters(lc, orc, concurrency):
+    """configs[3] in small: independent frames with per-frame parameters; `concurrency` frames in flight on
+    the library's internal streams (1 = back to back on the caller's stream), each with its own scratch."""
     import torch
+    nf = 7
     frames = [synth.make_frame(200, 264, seed=1000 + j, n_star=12, n_cr=150, sp_frac=0.005)
-              for j in range(4)]
-    ps = [dict(PARAMS, sigclip=(4.0, 4.5, 5.0)[(1000 + j) % 3]) for j in range(4)]
+              for j in range(nf)]
+    ps = [dict(PARAMS, sigclip=(4.0, 4.5, 5.0)[(1000 + j) % 3]) for j in range(nf)]
     ps[3]["niter"] = 2
+    ps[5]["niter"] = 0
     imgs = _t(np.stack([f.img for f in frames]))
-    g = lc.lacosmic_run_batch(imgs, [lc.Params(**p) for p in ps])
+    g = lc.lacosmic_run_batch(imgs, [lc.Params(**p) for p in ps], concurrency=concurrency)
     torch.cuda.synchronize()
-    for j in range(4):
+    for j in range(nf):
         o = orc.run(frames[j].img, **ps[j])
         assert np.array_equal(_n(g["mask"][j]), o["mask"]), j
         assert np.array_equal(_n(g["clean"][j]), o["clean"]), j
