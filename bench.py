@@ -300,6 +300,31 @@ def run_cuda(args):
     ms_e2e = timed(step_host, args.steps, max(1, args.warmup // 2))
     same = bool((mask_h.numpy() == res["mask"].cpu().numpy()).all() and
                 (clean_h.numpy() == res["clean"].cpu().numpy()).all())
+    # ---- end to end on a stream of frames: lacosmic_run_host_batch overlaps the H2D copy of one frame, the
+    # kernels of another and the D2H copy of a third
+    e2e_stream = None
+    if args.stream_frames > 0:
+        nh = min(args.stream_frames, 8)
+        imgs_h = torch.empty((nh, h, w), dtype=torch.float32).pin_memory()
+        for j in range(nh):
+            imgs_h[j].copy_(img_h)                     # the bench frame, nh times: timing only
+        masks_h = torch.empty((nh, h, w), dtype=torch.uint8).pin_memory()
+        cleans_h = torch.empty((nh, h, w), dtype=torch.float32).pin_memory()
+        kslots = 3
+        hbws = torch.empty(lc.lacosmic_host_batch_workspace_bytes(h, w, kslots), dtype=torch.uint8, device=dev)
+        plist_h = [P[main_mode]] * nh
+
+        def step_host_batch():
+            lc.lacosmic_run_host_batch(imgs_h, plist_h, masks_host=masks_h, cleans_host=cleans_h,
+                                       dev_workspace=hbws)
+        ms_hb = timed(step_host_batch, 3, 1)
+        ok_hb = bool((masks_h[nh - 1].numpy() == mask_h.numpy()).all() and
+                     (cleans_h[nh - 1].numpy() == clean_h.numpy()).all())
+        e2e_stream = dict(value=world * nh * 1e3 / ms_hb, unit="frames/s", frames=nh, slots=kslots,
+                          ms_per_frame=ms_hb / nh, h2d_bytes_per_frame=npx * 4, d2h_bytes_per_frame=npx * 5,
+                          matches_single_frame_call=ok_hb,
+                          call="lacosmic_run_host_batch (pinned host buffers, %d staging slots)" % kslots)
+        del imgs_h, masks_h, cleans_h, hbws
     clocks = sampler.stop() if rank == 0 else None
 
     if rank != 0:
@@ -378,7 +403,7 @@ def run_cuda(args):
         ref_comparisons_T_per_s=ref_cmp_rate,
         other_mode=dict(mode=other_mode, same_mask_clean_counts=modes_agree, roofline=roofline(res_other),
                         **summarise(res_other)),
-        stream=stream_res,
+        stream=stream_res, e2e_stream=e2e_stream,
         new_cr_per_iteration=res["counts"], mask_fraction=mask_frac,
         clocks=clocks, cpu_baseline=cpu,
         context="paper (PAPER.md:31,47): 55 s/frame dfcosmic C++ at 2 threads on AWS; GPU variant on an "

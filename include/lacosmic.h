@@ -136,6 +136,19 @@ int lacosmic_run_host(const float *img_host, int h, int w, const lacosmic_params
                       uint8_t *mask_out_host, float *clean_out_host, void *dev_workspace,
                       size_t dev_workspace_bytes, void *stream);
 
+/* Stream of n independent frames in HOST buffers (a nightly pipeline
+ * of >1000 frames per 15 minutes).  imgs_host/masks_host/cleans_host are [n][h][w] host arrays (pinned
+ * memory makes the copies asynchronous and lets them overlap), params a host array of n structs.  Frame f
+ * uses staging slot f % k on an internal stream (H2D copy, the whole path, D2H copies, in that order),
+ * k = min(n, LACOSMIC_MAX_BATCH_STREAMS, dev_workspace_bytes / lacosmic_host_workspace_bytes(h,w)), so with
+ * k >= 3 the H2D copy of one frame, the kernels of another and the D2H copy of a third run at the same
+ * time; the streams fork from and join back into `stream` with events (no host synchronisation).
+ * lacosmic_host_batch_workspace_bytes(h, w, k) gives the device scratch size for k slots. */
+size_t lacosmic_host_batch_workspace_bytes(int h, int w, int concurrency);
+int lacosmic_run_host_batch(const float *imgs_host, int n, int h, int w, const lacosmic_params *params,
+                            uint8_t *masks_host, float *cleans_host, void *dev_workspace,
+                            size_t dev_workspace_bytes, void *stream);
+
 /* ---- single steps (each is the kernel the whole path uses; exported for parity tests) -------- */
 
 /* Step (1): out = L+(in).  in/out fp32 [h][w], distinct. */

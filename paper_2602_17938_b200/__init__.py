@@ -29,6 +29,8 @@ from .binding import (  # noqa: F401
     lacosmic_version,
     lacosmic_workspace_bytes,
     lacosmic_batch_workspace_bytes,
+    lacosmic_host_batch_workspace_bytes,
+    lacosmic_run_host_batch,
     library_path,
     load_library,
 )

@@ -17,7 +17,7 @@ _lib = None
 
 EXPORTS = (
     "lacosmic_run", "lacosmic_workspace_bytes", "lacosmic_run_ws", "lacosmic_run_batch",
-    "lacosmic_batch_workspace_bytes",
+    "lacosmic_batch_workspace_bytes", "lacosmic_host_batch_workspace_bytes", "lacosmic_run_host_batch",
     "lacosmic_host_workspace_bytes", "lacosmic_run_host", "lacosmic_lplus", "lacosmic_medfilt",
     "lacosmic_bitplane_pitch_words", "lacosmic_pack_bits", "lacosmic_unpack_bits",
     "lacosmic_dilate3", "lacosmic_masked_median", "lacosmic_strerror",
@@ -88,6 +88,8 @@ def load_library():
         "lacosmic_run": (i, [vp, i, i, f, f, f, f, f, i, f, vp, vp, vp]),
         "lacosmic_workspace_bytes": (sz, [i, i]),
         "lacosmic_batch_workspace_bytes": (sz, [i, i, i]),
+        "lacosmic_host_batch_workspace_bytes": (sz, [i, i, i]),
+        "lacosmic_run_host_batch": (i, [vp, i, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp]),
         "lacosmic_run_ws": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp,
                                 C.POINTER(_CDebug), vp]),
         "lacosmic_run_batch": (i, [vp, i, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp, vp]),
@@ -280,6 +282,37 @@ def lacosmic_run_host(img_host, params=None, mask_out_host=None, clean_out_host=
                              dev_workspace.numel(), _stream(stream))
     _check(rc, "lacosmic_run_host")
     return dict(mask=mask_out_host, clean=clean_out_host)
+
+
+def lacosmic_host_batch_workspace_bytes(h, w, concurrency):
+    return int(load_library().lacosmic_host_batch_workspace_bytes(int(h), int(w), int(concurrency)))
+
+
+def lacosmic_run_host_batch(imgs_host, params, masks_host=None, cleans_host=None, dev_workspace=None,
+                            device="cuda:0", stream=None, concurrency=3):
+    """Stream of frames in HOST (ideally pinned) tensors [n][h][w]; params: list of n Params.  `concurrency`
+    staging slots are in flight (sizes the device scratch this call allocates when none is given)."""
+    torch = _torch()
+    L = load_library()
+    if (not isinstance(imgs_host, torch.Tensor) or imgs_host.is_cuda or imgs_host.dtype != torch.float32
+            or not imgs_host.is_contiguous() or imgs_host.dim() != 3):
+        raise TypeError("imgs_host must be a contiguous CPU float32 tensor [n][h][w]")
+    n, h, w = imgs_host.shape
+    if len(params) != n:
+        raise ValueError("need one Params per frame")
+    arr = (_CParams * max(n, 1))(*[p._c() for p in params])
+    if masks_host is None:
+        masks_host = torch.empty((n, h, w), dtype=torch.uint8).pin_memory()
+    if cleans_host is None:
+        cleans_host = torch.empty((n, h, w), dtype=torch.float32).pin_memory()
+    if dev_workspace is None:
+        dev_workspace = torch.empty(max(lacosmic_host_batch_workspace_bytes(h, w, max(1, concurrency)), 256),
+                                    dtype=torch.uint8, device=device)
+    rc = L.lacosmic_run_host_batch(imgs_host.data_ptr(), n, h, w, arr, masks_host.data_ptr(),
+                                   cleans_host.data_ptr(), _dev(dev_workspace, torch.uint8, "dev_workspace"),
+                                   dev_workspace.numel(), _stream(stream))
+    _check(rc, "lacosmic_run_host_batch")
+    return dict(mask=masks_host, clean=cleans_host)
 
 
 # ----------------------------------------------------------------------------- single steps

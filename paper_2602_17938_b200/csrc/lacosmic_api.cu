@@ -466,6 +466,25 @@ size_t lacosmic_host_workspace_bytes(int h, int w) {
     return align_up(P * 4, 256) * 2 + align_up(P, 256) + lacosmic_workspace_bytes(h, w);
 }
 
+namespace {
+// one frame through a staging slot: H2D, the path, D2H (slot layout: img | clean | mask | workspace)
+int run_host_frame(const float* img_host, int h, int w, const lacosmic_params& p, uint8_t* mask_out_host,
+                   float* clean_out_host, void* slot, cudaStream_t st) {
+    size_t P = (size_t)h * w, plane = align_up(P * 4, 256);
+    char* base = (char*)slot;
+    float* d_img = (float*)base;
+    float* d_clean = (float*)(base + plane);
+    uint8_t* d_mask = (uint8_t*)(base + 2 * plane);
+    void* ws = base + 2 * plane + align_up(P, 256);
+    CK(cudaMemcpyAsync(d_img, img_host, P * 4, cudaMemcpyHostToDevice, st));
+    int rc = run_frame(d_img, h, w, p, d_mask, d_clean, carve(ws, h, w), nullptr, nullptr, st);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(clean_out_host, d_clean, P * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(mask_out_host, d_mask, P, cudaMemcpyDeviceToHost, st));
+    return LACOSMIC_OK;
+}
+}  // namespace
+
 int lacosmic_run_host(const float* img_host, int h, int w, const lacosmic_params* p,
                       uint8_t* mask_out_host, float* clean_out_host, void* dev_workspace,
                       size_t dev_workspace_bytes, void* stream) {
@@ -476,19 +495,52 @@ int lacosmic_run_host(const float* img_host, int h, int w, const lacosmic_params
     if ((rc = check_params(*p))) return rc;
     if ((uintptr_t)dev_workspace & 255) return LACOSMIC_ERR_ALIGN;
     if (dev_workspace_bytes < lacosmic_host_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
-    size_t P = (size_t)h * w, plane = align_up(P * 4, 256);
-    char* base = (char*)dev_workspace;
-    float* d_img = (float*)base;
-    float* d_clean = (float*)(base + plane);
-    uint8_t* d_mask = (uint8_t*)(base + 2 * plane);
-    void* ws = base + 2 * plane + align_up(P, 256);
-    cudaStream_t st = (cudaStream_t)stream;
-    CK(cudaMemcpyAsync(d_img, img_host, P * 4, cudaMemcpyHostToDevice, st));
-    rc = run_frame(d_img, h, w, *p, d_mask, d_clean, carve(ws, h, w), nullptr, nullptr, st);
+    return run_host_frame(img_host, h, w, *p, mask_out_host, clean_out_host, dev_workspace, (cudaStream_t)stream);
+}
+
+size_t lacosmic_host_batch_workspace_bytes(int h, int w, int concurrency) {
+    if (check_shape(h, w) || concurrency < 1) return 0;
+    return (size_t)std::min(concurrency, LACOSMIC_MAX_BATCH_STREAMS) * align_up(lacosmic_host_workspace_bytes(h, w), 256);
+}
+
+int lacosmic_run_host_batch(const float* imgs_host, int n, int h, int w, const lacosmic_params* params,
+                            uint8_t* masks_host, float* cleans_host, void* dev_workspace,
+                            size_t dev_workspace_bytes, void* stream) {
+    g_launches = 0;
+    if (n < 0) return LACOSMIC_ERR_SHAPE;
+    if (n == 0) return LACOSMIC_OK;
+    if (!imgs_host || !params || !masks_host || !cleans_host || !dev_workspace) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
     if (rc) return rc;
-    CK(cudaMemcpyAsync(clean_out_host, d_clean, P * 4, cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(mask_out_host, d_mask, P, cudaMemcpyDeviceToHost, st));
-    return LACOSMIC_OK;
+    for (int f = 0; f < n; ++f)
+        if ((rc = check_params(params[f]))) return rc;
+    if ((uintptr_t)dev_workspace & 255) return LACOSMIC_ERR_ALIGN;
+    const size_t slot = align_up(lacosmic_host_workspace_bytes(h, w), 256);
+    const int k = (int)std::min<size_t>(std::min(n, LACOSMIC_MAX_BATCH_STREAMS), dev_workspace_bytes / slot);
+    if (k < 1) return LACOSMIC_ERR_WORKSPACE;
+    const size_t P = (size_t)h * w;
+    cudaStream_t caller = (cudaStream_t)stream;
+    BatchStreams* bs = nullptr;
+    if (k > 1) {
+        bs = batch_streams();
+        if (!bs) return LACOSMIC_ERR_CUDA;
+        CK(cudaEventRecord(bs->fork, caller));
+        for (int s = 0; s < k; ++s) CK(cudaStreamWaitEvent(bs->st[s], bs->fork, 0));
+    }
+    for (int f = 0; f < n; ++f) {
+        const int s = f % k;
+        rc = run_host_frame(imgs_host + f * P, h, w, params[f], masks_host + f * P, cleans_host + f * P,
+                            (char*)dev_workspace + (size_t)s * slot, k > 1 ? bs->st[s] : caller);
+        if (rc) break;
+    }
+    if (k > 1) {   // join, also after an error
+        for (int s = 0; s < k; ++s) {
+            if (!cuda_ok(cudaEventRecord(bs->join[s], bs->st[s])) ||
+                !cuda_ok(cudaStreamWaitEvent(caller, bs->join[s], 0)))
+                rc = rc ? rc : LACOSMIC_ERR_CUDA;
+        }
+    }
+    return rc;
 }
 
 // ---- single steps -----------------------------------------------------------------------------

@@ -258,6 +258,23 @@ def test_batch_with_per_frame_parameters(lc, orc, concurrency):
         assert np.array_equal(_n(g["counts"][j])[:ps[j]["niter"]], o["counts"]), j
 
 
+@pytest.mark.parametrize("concurrency", [1, 3])
+def test_host_batch_pipeline(lc, orc, concurrency):
+    """lacosmic_run_host_batch: frames in pinned host memory, H2D / kernels / D2H of different frames
+    overlapped on the library's internal streams; every frame must equal the oracle."""
+    import torch
+    nf = 5
+    frames = [synth.make_frame(120, 200, seed=2000 + j, n_star=8, n_cr=80, sp_frac=0.004) for j in range(nf)]
+    ps = [dict(PARAMS, sigclip=(4.0, 4.5, 5.0)[j % 3]) for j in range(nf)]
+    imgs = torch.from_numpy(np.stack([f.img for f in frames])).pin_memory()
+    r = lc.lacosmic_run_host_batch(imgs, [lc.Params(**p) for p in ps], concurrency=concurrency)
+    torch.cuda.synchronize()
+    for j in range(nf):
+        o = orc.run(frames[j].img, **ps[j])
+        assert np.array_equal(r["mask"][j].numpy(), o["mask"]), j
+        assert np.array_equal(r["clean"][j].numpy(), o["clean"]), j
+
+
 def test_gpu_argument_errors(lc):
     import torch
     img = torch.zeros((16, 16), device="cuda")
