@@ -27,7 +27,7 @@ sys.path.insert(0, ROOT)
 
 import numpy as np  # noqa: E402
 
-from paper_2602_17938_b200 import synth  # noqa: E402
+from paper_2602_17938_b200 import replicas, synth  # noqa: E402
 
 METRIC = "frames/s, 4000x6500 fp32 L.A.Cosmic (niter=4)"
 # ALU-pipe roofline: FMNMX/FMNMX3 issue at 64 lanes/clk/SM (measured,
@@ -130,8 +130,8 @@ def _oracle_sample(img, params, rows):
 
 
 def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    rank, _, _ = replicas.env_rank_world()
+    if rank != 0:                            # under torchrun rank 0 alone runs the oracle; the others exit 0
         return 0
     wl = _workload(args.workload)
     frame = synth.make_config(wl["cfg"])
@@ -164,9 +164,7 @@ def run_cuda(args):
 
     import paper_2602_17938_b200 as lc
 
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank, local_rank, world = replicas.env_rank_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
     torch.cuda.set_device(local_rank)
@@ -179,7 +177,7 @@ def run_cuda(args):
     wl = _workload(args.workload)
     # replicas: every rank cleans its own frame (same generator, seed offset by rank)
     kw = dict(synth.CONFIGS[wl["cfg"]])
-    kw["seed"] = kw["seed"] + 100 * rank
+    kw["seed"] = replicas.rank_seed(kw["seed"], rank)
     frame = synth.make_frame(**kw)
     params = dict(synth.DEFAULT_PARAMS)
     modes = {"lazy": lc.MODE_LAZY, "dense": lc.MODE_DENSE}
@@ -201,9 +199,7 @@ def run_cuda(args):
         return step
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        replicas.barrier(world, torch.cuda.synchronize)
 
     def timed(fn, steps, warmup):
         for _ in range(warmup):
@@ -217,11 +213,7 @@ def run_cuda(args):
             fn()
             b.record(stream)
         barrier()
-        total_ms = sum(a.elapsed_time(b) for a, b in evs)
-        if world > 1:
-            t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            total_ms = float(t.item())
+        total_ms = replicas.max_over_ranks(sum(a.elapsed_time(b) for a, b in evs), world, dev)
         return total_ms / steps
 
     def measure(mode):
@@ -261,7 +253,7 @@ def run_cuda(args):
         imgs = torch.empty((nf, h, w), dtype=torch.float32, device=dev)
         for j, (kwj, _) in enumerate(cfg):
             kwj = dict(kwj)
-            kwj["seed"] += 100 * rank
+            kwj["seed"] = replicas.rank_seed(kwj["seed"], rank)
             imgs[j].copy_(torch.from_numpy(synth.make_frame(**kwj).img))
         plist = [lc.Params(mode=lc.MODE_LAZY, **pj) for _, pj in cfg]
         masks = torch.empty((nf, h, w), dtype=torch.uint8, device=dev)
