@@ -9,7 +9,8 @@
  * What it follows
  *   step list : PAPER.md:53-62 (section Methods/Algorithm, items 1-7)
  *   formulas  : BASELINE.json north_star (1)-(7)
- *   readings  : SURVEY.md section 8(c), O0-O7 and R1-R20 (restated in DESIGN.md section 3)
+ *   readings  : SURVEY.md section 8(c), O0-O7 and R1-R20 (restated in DESIGN.md section 3);
+ *               R21 (gain estimation, PAPER.md:74,43 -- SURVEY.md 8(f)-2) in DESIGN.md section 3
  *
  * Precision: north_star fixes fp32 ("4000x6500 fp32 L.A.Cosmic", "fp32 L+, N, S and S'"),
  * so every arithmetic step is ONE fp32 round-to-nearest operation, in the order written
@@ -162,17 +163,85 @@ void orc_masked_median(const float *img, const uint8_t *mask, float *out, int h,
     }
 }
 
+/* ---- R21: gain estimation ("If a gain is not supplied, then it will be estimated at each
+ * iteration"; PAPER.md:43 sigma_clip).  The paper gives no formula; R21 is the reading:
+ * for Poisson-dominated noise var(work) = signal/gain, so r = (work - med5(work)) / sqrt(med5(work)) has
+ * standard deviation 1/sqrt(gain).  sigma is estimated robustly and ORDER-INDEPENDENTLY (selection
+ * only, no sums): three rounds of { c = median of r over the kept set, d = median of |r - c| over the
+ * kept set, s = 1.4826 d, keep c - 5 s <= r <= c + 5 s (intersected with the previous interval) },
+ * "median" = the element of 0-based rank (n-1)/2 of the ascending sort.  gain = 1/s^2 (1 if s is 0 or
+ * not finite).  Read noise is not subtracted (stated bias, R21). */
+static int cmp_float(const void *a, const void *b) {
+    float x = *(const float *)a, y = *(const float *)b;
+    return (x > y) - (x < y);
+}
+
+/* rank-(n-1)/2 element of v[0..n-1] by a full sort (v is reordered) */
+static float lower_median(float *v, size_t n) {
+    qsort(v, n, sizeof(float), cmp_float);
+    return v[(n - 1) / 2];
+}
+
+/* sigma clipping of r[0..n-1] as defined above.  stats (nullable) receives, for the LAST round,
+ * {c, s, lo, hi, kept count} where lo/hi is the interval the round started from.  Returns s. */
+float orc_sigma_clip(const float *r, size_t n, int rounds, float *stats) {
+    float lo = -INFINITY, hi = INFINITY, c = 0.0f, s = 0.0f;
+    float *v = malloc((n ? n : 1) * sizeof(float));
+    if (!v) return NAN;
+    for (int j = 0; j < rounds; ++j) {
+        size_t m = 0;
+        for (size_t p = 0; p < n; ++p)
+            if (r[p] >= lo && r[p] <= hi) v[m++] = r[p];
+        if (m == 0) break;
+        float lo0 = lo, hi0 = hi;
+        c = lower_median(v, m);
+        m = 0;
+        for (size_t p = 0; p < n; ++p)
+            if (r[p] >= lo0 && r[p] <= hi0) v[m++] = fabsf(r[p] - c);
+        float d = lower_median(v, m);
+        s = 1.4826f * d;
+        float five_s = 5.0f * s;
+        float nlo = c - five_s, nhi = c + five_s;
+        if (stats) { stats[0] = c; stats[1] = s; stats[2] = lo0; stats[3] = hi0; stats[4] = (float)m; }
+        lo = nlo > lo0 ? nlo : lo0;
+        hi = nhi < hi0 ? nhi : hi0;
+    }
+    free(v);
+    return s;
+}
+
+/* gain estimate of one image (the `work` plane of an iteration).  stats: nullable float[5], see above. */
+int orc_estimate_gain(const float *work, int h, int w, float *gain_out, float *stats) {
+    if (!work || !gain_out || h < 1 || w < 1) return ORC_ERR_ARG;
+    size_t P = (size_t)h * (size_t)w;
+    float *m5 = malloc(P * 4), *r = malloc(P * 4);
+    if (!m5 || !r) { free(m5); free(r); return ORC_ERR_MEM; }
+    orc_medfilt(work, m5, h, w, 5);
+#pragma omp parallel for schedule(static)
+    for (size_t p = 0; p < P; ++p) {
+        float m = m5[p] > 1e-4f ? m5[p] : 1e-4f;
+        float dev = work[p] - m5[p];
+        r[p] = dev / sqrtf(m);
+    }
+    float s = orc_sigma_clip(r, P, 3, stats);
+    float s2 = s * s;
+    *gain_out = (s > 0.0f && isfinite(s) && isfinite(1.0f / s2)) ? 1.0f / s2 : 1.0f;
+    free(m5); free(r);
+    return ORC_OK;
+}
+
 #define COPY_IF(dst, src, bytes) do { if (dst) memcpy((dst), (src), (bytes)); } while (0)
 
 /* The whole path: O0-O7 of SURVEY.md 8(c).  Returns 0, or <0 on bad arguments / out of memory.
  * iter_counts (nullable) receives new_t for t = 0..niter-1; dbg (nullable) receives the planes
- * of iteration dbg->iter.  All niter iterations are always executed (R17: stopping at new_t = 0
+ * of iteration dbg->iter; iter_gains (nullable) the gain used in each iteration (gain == 0: R21).  All niter iterations are always executed (R17: stopping at new_t = 0
  * would give the identical result; the oracle does not take the shortcut). */
 int orc_run(const float *img, int h, int w, float gain, float readnoise, float sigclip,
             float sigfrac, float objlim, int niter, float satlevel, uint8_t *mask_out,
-            float *clean_out, int32_t *iter_counts, orc_debug *dbg) {
+            float *clean_out, int32_t *iter_counts, orc_debug *dbg, float *iter_gains) {
     if (!img || !mask_out || !clean_out || h < 1 || w < 1 || niter < 0) return ORC_ERR_ARG;
-    if (!(gain > 0.0f) || !(readnoise >= 0.0f) || !(sigclip > 0.0f) || !(sigfrac > 0.0f) ||
+    const int estimate = (gain == 0.0f);   /* R21: gain 0 = "not supplied" */
+    if (!(gain >= 0.0f) || !(readnoise >= 0.0f) || !(sigclip > 0.0f) || !(sigfrac > 0.0f) ||
         !(objlim >= 0.0f))
         return ORC_ERR_ARG;
     size_t P = (size_t)h * (size_t)w;
@@ -196,6 +265,11 @@ int orc_run(const float *img, int h, int w, float gain, float readnoise, float s
 
     for (int t = 0; t < niter; ++t) {
         if (dbg && dbg->iter == t) COPY_IF(dbg->work_in, work, P * 4);
+        if (estimate) {   /* R21: estimated at each iteration, from the iteration's input image */
+            rc = orc_estimate_gain(work, h, w, &gain, NULL);
+            if (rc) goto done;
+        }
+        if (iter_gains) iter_gains[t] = gain;
         /* O1 */
         orc_lplus(work, Lp, h, w);
         /* O2 -- north_star (2): N = sqrt(gain*med5(img) + rn^2)/gain, med5 floored at 1e-4 (R5) */

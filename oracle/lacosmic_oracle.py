@@ -55,7 +55,11 @@ def lib():
         L.orc_masked_median.argtypes = [fp, u8p, fp, C.c_int, C.c_int]
         L.orc_masked_median.restype = None
         L.orc_run.argtypes = [fp, C.c_int, C.c_int] + [C.c_float] * 5 + [C.c_int, C.c_float,
-                                                                        u8p, fp, i32p, C.c_void_p]
+                                                                        u8p, fp, i32p, C.c_void_p, fp]
+        L.orc_estimate_gain.argtypes = [fp, C.c_int, C.c_int, fp, fp]
+        L.orc_estimate_gain.restype = C.c_int
+        L.orc_sigma_clip.argtypes = [fp, C.c_size_t, C.c_int, fp]
+        L.orc_sigma_clip.restype = C.c_float
         L.orc_run.restype = C.c_int
         L.orc_set_threads.argtypes = [C.c_int]
         L.orc_get_max_threads.restype = C.c_int
@@ -118,9 +122,29 @@ def masked_median(img, mask):
     return out
 
 
+def sigma_clip(r, rounds=3):
+    """R21 sigma clipping of a 1-D fp32 vector.  Returns (s, stats = [c, s, lo, hi, kept] of the last round)."""
+    r = np.ascontiguousarray(r, dtype=np.float32).ravel()
+    stats = np.zeros(5, np.float32)
+    s = lib().orc_sigma_clip(_p(r), r.size, int(rounds), _p(stats))
+    return float(np.float32(s)), stats
+
+
+def estimate_gain(img):
+    """R21 gain estimate of one image.  Returns (gain fp32, stats)."""
+    img = _f32(img)
+    g = np.zeros(1, np.float32)
+    stats = np.zeros(5, np.float32)
+    rc = lib().orc_estimate_gain(_p(img), img.shape[0], img.shape[1], _p(g), _p(stats))
+    if rc != 0:
+        raise ValueError("orc_estimate_gain failed with code %d" % rc)
+    return np.float32(g[0]), stats
+
+
 def run(img, gain=1.0, readnoise=10.0, sigclip=4.5, sigfrac=0.3, objlim=5.0, niter=4,
         satlevel=65535.0, debug_iter=None):
-    """Whole path (O0-O7).  Returns dict(mask=u8, clean=f32, counts=int32[niter], [debug planes])."""
+    """Whole path (O0-O7).  gain = 0: estimated at each iteration (R21).  Returns dict(mask=u8, clean=f32,
+    counts=int32[niter], gains=f32[niter] (the gain each iteration used), [debug planes])."""
     img = _f32(img)
     h, w = img.shape
     mask = np.empty((h, w), np.uint8)
@@ -138,9 +162,10 @@ def run(img, gain=1.0, readnoise=10.0, sigclip=4.5, sigfrac=0.3, objlim=5.0, nit
             out[n] = np.zeros((h, w), np.uint8)
             setattr(dbg, n, out[n].ctypes.data)
         dbg_ref = C.byref(dbg)
+    gains = np.zeros(max(niter, 1), np.float32)
     rc = lib().orc_run(_p(img), h, w, gain, readnoise, sigclip, sigfrac, objlim, int(niter),
-                       satlevel, _p(mask), _p(clean), _p(counts), dbg_ref)
+                       satlevel, _p(mask), _p(clean), _p(counts), dbg_ref, _p(gains))
     if rc != 0:
         raise ValueError("orc_run failed with code %d" % rc)
-    out.update(mask=mask, clean=clean, counts=counts[:niter].copy())
+    out.update(mask=mask, clean=clean, counts=counts[:niter].copy(), gains=gains[:niter].copy())
     return out

@@ -365,7 +365,100 @@ def test_p12_generator_recall_and_determinism(orc):
 
 def test_bad_arguments_rejected(orc):
     img = np.zeros((8, 8), np.float32)
-    for bad in (dict(gain=0.0), dict(gain=-1.0), dict(readnoise=-1.0), dict(sigclip=0.0),
+    for bad in (dict(gain=-1.0), dict(gain=float("nan")), dict(readnoise=-1.0), dict(sigclip=0.0),
                 dict(sigfrac=0.0), dict(objlim=-1.0), dict(niter=-1)):
         with pytest.raises(ValueError):
             orc.run(img, **dict(PARAMS, **bad))
+
+
+# ------------------------------------------------------------------------------------------------
+# R21: gain estimation when no gain is supplied (gain = 0).
+def _sigma_clip_cases():
+    cases, cur = [], None
+    for ln in open(os.path.join(GOLDEN, "sigma_clip_cases.txt")):
+        ln = ln.strip()
+        if not ln or ln.startswith("#"):
+            continue
+        key, _, rest = ln.partition(" ")
+        if key == "case":
+            cur = dict(name=rest)
+            cases.append(cur)
+        elif key == "r":
+            cur["r"] = [float(v) for v in rest.split()]
+        elif key == "rounds":
+            cur["rounds"] = int(rest)
+        elif key == "expect":
+            cur["expect"] = [float(v) for v in rest.split()]
+    return cases
+
+
+@pytest.mark.parametrize("case", _sigma_clip_cases(), ids=lambda c: c["name"])
+def test_p13_hand_computed_sigma_clip(orc, case):
+    s, stats = orc.sigma_clip(np.array(case["r"], np.float32), case["rounds"])
+    c_e, s_e, lo_e, hi_e, kept_e = case["expect"]
+    assert stats[0] == np.float32(c_e) and stats[4] == kept_e
+    assert abs(s - s_e) <= 1e-6 * max(1.0, abs(s_e)) and abs(stats[1] - s_e) <= 1e-6 * max(1.0, abs(s_e))
+    for got, exp in ((stats[2], lo_e), (stats[3], hi_e)):
+        assert (got == exp) if math.isinf(exp) else abs(got - exp) <= 1e-5 * max(1.0, abs(exp))
+
+
+def test_p13_sigma_clip_is_order_independent_and_rank_based(orc):
+    """Selection only: any permutation of the input gives the same bits; the centre and the MAD are elements
+    of fixed rank (library cross-check with np.partition on the first round)."""
+    rng = np.random.default_rng(11)
+    r = np.concatenate([rng.standard_normal(4001), 50 + 10 * rng.standard_normal(37)]).astype(np.float32)
+    s0, st0 = orc.sigma_clip(r, 3)
+    for _ in range(3):
+        s1, st1 = orc.sigma_clip(rng.permutation(r), 3)
+        assert s1 == s0 and np.array_equal(st1, st0)
+    _, st = orc.sigma_clip(r, 1)
+    k = (r.size - 1) // 2
+    c = np.partition(r, k)[k]
+    d = np.partition(np.abs(r - c), k)[k]
+    assert st[0] == c and st[1] == np.float32(1.4826) * d
+    assert 0.9 < s0 < 1.1 and st0[4] <= 4001 + 1          # the 50-sigma cluster is clipped away, sigma ~ 1
+
+
+@pytest.mark.parametrize("gain", [0.5, 2.0, 7.0])
+def test_p13_gain_of_pure_poisson_like_noise_is_recovered(orc, gain):
+    """Closed form behind R21: var(work) = signal/gain => (work - med5)/sqrt(med5) has sigma 1/sqrt(gain).  The
+    pixel is part of its own median window, which lowers the residual variance by a few per cent."""
+    rng = np.random.default_rng(5)
+    B = 900.0
+    img = (B + np.sqrt(B / gain) * rng.standard_normal((500, 620))).astype(np.float32)
+    g, stats = orc.estimate_gain(img)
+    assert abs(g / gain - 1.0) < 0.12
+    assert abs(stats[0]) < 0.05 / math.sqrt(gain)
+    # robust: 1 % of the pixels hit by cosmic rays barely moves the estimate
+    hit = rng.random(img.shape) < 0.01
+    g2, _ = orc.estimate_gain(np.where(hit, img + 5000.0, img).astype(np.float32))
+    assert abs(g2 / g - 1.0) < 0.05
+
+
+def test_p13_gain_scaling_is_exact(orc):
+    """img -> 4 img scales every residual by exactly 2 (all operations scale by powers of two), hence
+    gain -> gain / 4 bit for bit: pins the structure (difference over sqrt(median)) of the estimator."""
+    f = synth.make_frame(96, 130, seed=4, n_star=5, n_cr=30, sp_frac=0.003)
+    g1, st1 = orc.estimate_gain(f.img)
+    g4, st4 = orc.estimate_gain(4.0 * f.img)
+    assert g4 * np.float32(4.0) == g1
+    assert st4[0] == 2 * st1[0] and st4[1] == 2 * st1[1] and st4[4] == st1[4]
+
+
+def test_p13_degenerate_and_whole_path(orc):
+    g, stats = orc.estimate_gain(np.full((20, 30), 50.0, np.float32))
+    assert g == 1.0 and stats[1] == 0.0                                     # sigma = 0 -> gain 1 (R21)
+    f = synth.make_config(0)
+    est = orc.run(f.img, **dict(PARAMS, gain=0.0))
+    assert est["gains"].shape == (PARAMS["niter"],) and np.all(est["gains"] > 0)
+    # iteration 0 estimates from the input frame; feeding the estimates back as supplied gains, one
+    # iteration at a time, reproduces the run: the estimate only enters through the noise model
+    g0, _ = orc.estimate_gain(f.img)
+    assert est["gains"][0] == g0
+    one = orc.run(f.img, **dict(PARAMS, gain=float(g0), niter=1))
+    est1 = orc.run(f.img, **dict(PARAMS, gain=0.0, niter=1))
+    assert np.array_equal(one["mask"], est1["mask"]) and np.array_equal(one["clean"], est1["clean"])
+    g1, _ = orc.estimate_gain(est1["clean"])
+    assert est["gains"][1] == g1                                            # iteration 1 sees the cleaned frame
+    fixed = orc.run(f.img, **PARAMS)
+    assert np.all(fixed["gains"] == np.float32(PARAMS["gain"]))
