@@ -41,7 +41,7 @@ extern "C" {
 #define LACOSMIC_OK 0
 #define LACOSMIC_ERR_NULL (-1)      /* a required pointer is NULL */
 #define LACOSMIC_ERR_SHAPE (-2)     /* h < 1, w < 1, or h*w >= 2^31 (or n < 0 for a batch) */
-#define LACOSMIC_ERR_PARAM (-3)     /* non-finite parameter; gain <= 0; readnoise < 0; sigclip <= 0;
+#define LACOSMIC_ERR_PARAM (-3)     /* non-finite parameter; gain < 0; readnoise < 0; sigclip <= 0;
                                        sigfrac <= 0 or > 1; objlim < 0; niter < 0 or > LACOSMIC_MAX_NITER;
                                        satlevel NaN; unknown mode; k not in {3,5,7} */
 #define LACOSMIC_ERR_ALIGN (-4)     /* fp32 image pointer not 16-byte aligned, workspace not 256-byte aligned */
@@ -52,7 +52,9 @@ extern "C" {
 #define LACOSMIC_MAX_NITER 64
 
 /* Parameters of one frame (PAPER.md:66-74 plus niter/satlevel of the north_star signature).
- * gain [e-/ADU] > 0 (gain estimation, is not part of this path); readnoise [e-] >= 0;
+ * gain [e-/ADU] > 0, or 0 = "not supplied": it is then estimated at each iteration from that iteration's
+ * input image (reading R21: residual over sqrt(med5), three rounds of rank-based
+ * sigma clipping, gain = 1/s^2; every iteration then recomputes all planes); readnoise [e-] >= 0;
  * sigclip > 0: detection limit in sigma; sigfrac in (0,1]: fractional limit for neighbours;
  * objlim >= 0: contrast limit L+/F; satlevel: pixels >= satlevel are never flagged (+INF disables);
  * niter in [0, LACOSMIC_MAX_NITER]: number of iterations (0: clean_out = img, mask_out = 0). */
@@ -81,9 +83,11 @@ typedef struct lacosmic_params {
  * forms Sp, m3, F and evaluates G2 only where step (6) reads it: those four planes are left untouched
  * there; every other plane is filled and identical in both modes. */
 typedef struct lacosmic_debug {
-    int32_t iter;
+    int32_t iter;   /* iteration whose planes are dumped; -1: none (only `gains` is filled) */
     float *Lp, *N, *S, *Sp, *m3, *F;
     uint8_t *G1, *G2, *M1, *M2, *M3, *C;
+    float *gains;   /* nullable device array of p->niter floats: the gain each iteration's noise model used
+                       (the supplied gain, or the estimates of R21 when p->gain == 0) */
 } lacosmic_debug;
 
 /* ---- the whole path ------------------------------------------------------------------------- */
@@ -151,6 +155,13 @@ int lacosmic_run_host_batch(const float *imgs_host, int n, int h, int w, const l
 
 /* ---- single steps (each is the kernel the whole path uses; exported for parity tests) -------- */
 
+/* R21 alone: the gain estimate of one image (what the whole path computes at the start of an iteration when
+ * p->gain == 0).  gain_out: DEVICE pointer to one float; stats_out: nullable DEVICE pointer to 5 floats
+ * {c, s, lo, hi, kept} of the last clipping round (centre, 1.4826 MAD, the interval the round started from,
+ * number of pixels inside it).  workspace as for lacosmic_run_ws. */
+int lacosmic_estimate_gain(const float *img, int h, int w, float *gain_out, float *stats_out,
+                           void *workspace, size_t workspace_bytes, void *stream);
+
 /* Step (1): out = L+(in).  in/out fp32 [h][w], distinct. */
 int lacosmic_lplus(const float *in, float *out, int h, int w, void *stream);
 
@@ -190,7 +201,7 @@ const char *lacosmic_version(void);
  * LACOSMIC_NUM_KERNEL_CLASSES, the summed device time ms_sum[c] and the number of spans[c] (HOST
  * arrays), and clears the record.  Class names: lacosmic_kernel_class_name(c); the last class is the
  * whole frame (copies included). */
-#define LACOSMIC_NUM_KERNEL_CLASSES 8
+#define LACOSMIC_NUM_KERNEL_CLASSES 9
 int lacosmic_kernel_timing_enable(int enable);
 int lacosmic_kernel_timing_read(float *ms_sum, int32_t *spans);
 const char *lacosmic_kernel_class_name(int cls);

@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     Params,
     lacosmic_bitplane_pitch_words,
     lacosmic_dilate3,
+    lacosmic_estimate_gain,
     lacosmic_host_workspace_bytes,
     lacosmic_kernel_timing_enable,
     lacosmic_kernel_timing_read,

@@ -18,13 +18,14 @@ _lib = None
 EXPORTS = (
     "lacosmic_run", "lacosmic_workspace_bytes", "lacosmic_run_ws", "lacosmic_run_batch",
     "lacosmic_batch_workspace_bytes", "lacosmic_host_batch_workspace_bytes", "lacosmic_run_host_batch",
-    "lacosmic_host_workspace_bytes", "lacosmic_run_host", "lacosmic_lplus", "lacosmic_medfilt",
+    "lacosmic_host_workspace_bytes", "lacosmic_run_host", "lacosmic_estimate_gain", "lacosmic_lplus",
+    "lacosmic_medfilt",
     "lacosmic_bitplane_pitch_words", "lacosmic_pack_bits", "lacosmic_unpack_bits",
     "lacosmic_dilate3", "lacosmic_masked_median", "lacosmic_strerror",
     "lacosmic_last_cuda_error", "lacosmic_last_launch_count", "lacosmic_version",
     "lacosmic_kernel_timing_enable", "lacosmic_kernel_timing_read", "lacosmic_kernel_class_name",
 )
-NUM_KERNEL_CLASSES = 8
+NUM_KERNEL_CLASSES = 9
 MODE_LAZY, MODE_DENSE = 0, 1
 
 
@@ -44,7 +45,7 @@ class _CParams(C.Structure):
 
 class _CDebug(C.Structure):
     _fields_ = [("iter", C.c_int32)] + [(n, C.c_void_p) for n in (
-        "Lp", "N", "S", "Sp", "m3", "F", "G1", "G2", "M1", "M2", "M3", "C")]
+        "Lp", "N", "S", "Sp", "m3", "F", "G1", "G2", "M1", "M2", "M3", "C", "gains")]
 
 
 DEBUG_F32 = ("Lp", "N", "S", "Sp", "m3", "F")
@@ -54,7 +55,7 @@ DEBUG_U8 = ("G1", "G2", "M1", "M2", "M3", "C")
 @dataclass
 class Params:
     """Per-frame parameters (niter/satlevel from the north_star signature)."""
-    gain: float = 1.0
+    gain: float = 1.0          # 0 = not supplied: estimated at each iteration (DESIGN.md R21)
     readnoise: float = 10.0
     sigclip: float = 4.5
     sigfrac: float = 0.3
@@ -95,6 +96,7 @@ def load_library():
         "lacosmic_run_batch": (i, [vp, i, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp, vp]),
         "lacosmic_host_workspace_bytes": (sz, [i, i]),
         "lacosmic_run_host": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp]),
+        "lacosmic_estimate_gain": (i, [vp, i, i, vp, vp, vp, sz, vp]),
         "lacosmic_lplus": (i, [vp, vp, i, i, vp]),
         "lacosmic_medfilt": (i, [vp, vp, i, i, i, vp]),
         "lacosmic_bitplane_pitch_words": (i, [i]),
@@ -193,8 +195,9 @@ def lacosmic_run(img, gain=1.0, readnoise=10.0, sigclip=4.5, sigfrac=0.3, objlim
 
 
 def lacosmic_run_ws(img, params=None, mask_out=None, clean_out=None, workspace=None,
-                    iter_counts=None, debug_iter=None, debug_planes=None, stream=None, **kw):
-    """Timed entry point.  Returns dict(mask, clean, counts[, debug planes of iteration debug_iter])."""
+                    iter_counts=None, debug_iter=None, debug_planes=None, want_gains=False, stream=None, **kw):
+    """Timed entry point.  Returns dict(mask, clean, counts[, debug planes of iteration debug_iter][, gains =
+    the gain each iteration used, when want_gains])."""
     torch = _torch()
     L = load_library()
     p = _params(params, **kw)
@@ -212,14 +215,18 @@ def lacosmic_run_ws(img, params=None, mask_out=None, clean_out=None, workspace=N
         iter_counts = torch.zeros(max(int(p.niter), 1), dtype=torch.int32, device=img.device)
     out = dict(mask=mask_out, clean=clean_out, counts=iter_counts)
     dbg_ref = None
-    if debug_iter is not None:
+    if debug_iter is not None or want_gains:
         dbg = _CDebug()
-        dbg.iter = int(debug_iter)
-        names = debug_planes if debug_planes is not None else DEBUG_F32 + DEBUG_U8
-        for n in names:
-            dt = torch.float32 if n in DEBUG_F32 else torch.uint8
-            out[n] = torch.zeros((h, w), dtype=dt, device=img.device)
-            setattr(dbg, n, out[n].data_ptr())
+        dbg.iter = int(debug_iter) if debug_iter is not None else -1
+        if debug_iter is not None:
+            names = debug_planes if debug_planes is not None else DEBUG_F32 + DEBUG_U8
+            for n in names:
+                dt = torch.float32 if n in DEBUG_F32 else torch.uint8
+                out[n] = torch.zeros((h, w), dtype=dt, device=img.device)
+                setattr(dbg, n, out[n].data_ptr())
+        if want_gains:
+            out["gains"] = torch.zeros(max(int(p.niter), 1), dtype=torch.float32, device=img.device)
+            dbg.gains = out["gains"].data_ptr()
         dbg_ref = C.byref(dbg)
     cp = p._c()
     rc = L.lacosmic_run_ws(ip, h, w, C.byref(cp), _dev(mask_out, torch.uint8, "mask_out", (h, w)),
@@ -316,6 +323,20 @@ def lacosmic_run_host_batch(imgs_host, params, masks_host=None, cleans_host=None
 
 
 # ----------------------------------------------------------------------------- single steps
+def lacosmic_estimate_gain(img, workspace=None, stream=None):
+    """R21 alone.  Returns (gain: device float tensor [1], stats: device float tensor [5] = c, s, lo, hi, kept)."""
+    torch = _torch()
+    h, w = img.shape
+    if workspace is None:
+        workspace = _workspace(h, w, img.device)
+    gain = torch.zeros(1, dtype=torch.float32, device=img.device)
+    stats = torch.zeros(5, dtype=torch.float32, device=img.device)
+    _check(load_library().lacosmic_estimate_gain(
+        _dev(img, torch.float32, "img"), h, w, gain.data_ptr(), stats.data_ptr(),
+        _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)), "lacosmic_estimate_gain")
+    return gain, stats
+
+
 def lacosmic_lplus(img, out=None, stream=None):
     torch = _torch()
     h, w = img.shape

@@ -118,6 +118,8 @@ struct NoiseArgs {
                              // into the first pass, which then reads img_in itself)
     int h, w, wpr;
     float gain, rn2, sigclip, siglow, satlevel;
+    float* R;                // nullable (R21): also write r = (work - med5) / sqrt(max(med5, 1e-4)) here
+    const float* gain_dev;   // nullable (R21): the gain of this iteration, estimated on the device
 };
 
 // gather the 4-bit nibbles of the 8 lanes that share a 32-pixel word
@@ -137,6 +139,7 @@ constexpr int UW = 32, UH = 4;
 __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a, int x0, int y0, int lane,
                                              int wi) {
     const int lx = lane & 7, lr = lane >> 3;
+    const float gain = a.gain_dev ? __ldg(a.gain_dev) : a.gain;
 #pragma unroll 1
     for (int u = wi; u < (TW / UW) * (NS_TH / UH); u += NWARP) {
         const int xu = x0 + (u & 3) * UW, lyu = (u >> 2) * UH, yu = y0 + lyu;
@@ -151,7 +154,7 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
             for (int j = 0; j < 4; ++j) {
                 ctr[j] = win[2 + j][2];
                 lp[j] = lplus_px(win[2 + j][2], win[2 + j][1], win[2 + j][3], win[1 + j][2], win[3 + j][2]);
-                n[j] = noise_px(m5[j], a.gain, a.rn2);
+                n[j] = noise_px(m5[j], gain, a.rn2);
                 s[j] = fdiv_nn(lp[j], __fmul_rn(2.0f, n[j]));
                 const bool ok = (x + j < a.w) && (win[2 + j][2] < a.satlevel);            // R12
                 n1 |= (uint32_t)(ok && s[j] > a.sigclip) << j;
@@ -162,6 +165,15 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
             if (a.dbgLp) store4(a.dbgLp, ro, x, a.w, lp);
             if (a.dbgN) store4(a.dbgN, ro, x, a.w, n);
             if (a.copy_out) store4(a.copy_out, ro, x, a.w, ctr);
+            if (a.R) {   // R21: residual in units of sqrt(signal)
+                float r[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const float m5c = m5[j] > 1e-4f ? m5[j] : 1e-4f;
+                    r[j] = __fdiv_rn(__fsub_rn(ctr[j], m5[j]), __fsqrt_rn(m5c));
+                }
+                store4(a.R, ro, x, a.w, r);
+            }
         }
         if (a.A1) {
             const uint32_t b1 = nibbles_to_word(n1, lane), b2 = nibbles_to_word(n2, lane);

@@ -9,6 +9,7 @@
 #include "kernels.cuh"
 #include "lazy.cuh"
 #include "grow.cuh"
+#include "select.cuh"
 
 namespace {
 
@@ -27,7 +28,7 @@ inline bool cuda_ok(cudaError_t e) {
 
 // Optional per-kernel-class CUDA-event timing (lacosmic_kernel_timing_*): bench.py switches it on to
 // measure the dominant kernel's average launch duration on the launching stream.
-enum KClass { KC_NOISE_S = 0, KC_FINE_GATES, KC_GROW, KC_LISTS, KC_BITS, KC_EVAL, KC_NOISE_S_QUADS, KC_STEP, KC_COUNT };
+enum KClass { KC_NOISE_S = 0, KC_FINE_GATES, KC_GROW, KC_LISTS, KC_BITS, KC_EVAL, KC_NOISE_S_QUADS, KC_SELECT, KC_STEP, KC_COUNT };
 static_assert(KC_COUNT == LACOSMIC_NUM_KERNEL_CLASSES, "header and library disagree");
 struct KTiming {
     static constexpr int MAXSPANS = 8192;
@@ -126,7 +127,7 @@ inline int check_params(const lacosmic_params& p) {
     if (!std::isfinite(p.gain) || !std::isfinite(p.readnoise) || !std::isfinite(p.sigclip) ||
         !std::isfinite(p.sigfrac) || !std::isfinite(p.objlim) || std::isnan(p.satlevel))
         return LACOSMIC_ERR_PARAM;
-    if (!(p.gain > 0.0f) || p.readnoise < 0.0f || !(p.sigclip > 0.0f) || !(p.sigfrac > 0.0f) ||
+    if (!(p.gain >= 0.0f) || p.readnoise < 0.0f || !(p.sigclip > 0.0f) || !(p.sigfrac > 0.0f) ||
         p.sigfrac > 1.0f || p.objlim < 0.0f || p.niter < 0 || p.niter > LACOSMIC_MAX_NITER)
         return LACOSMIC_ERR_PARAM;
     if (p.mode != LACOSMIC_MODE_LAZY && p.mode != LACOSMIC_MODE_DENSE) return LACOSMIC_ERR_PARAM;
@@ -147,6 +148,9 @@ struct Workspace {
     int32_t* counts;   // per iteration: newly flagged pixels
     int32_t* ncand;    // per iteration (lazy path): candidate pixels evaluated
     int32_t* nquad;    // per iteration (lazy path): quads the incremental noise/S pass recomputed
+    float* gains;      // per iteration: the gain the noise model used (R21: estimated when p.gain == 0)
+    lac::SelState* sel; // radix selection state and histogram of the gain estimation (select.cuh)
+    uint32_t* hist;
     uint8_t* stripflag; // per 30-word x 8-row strip of the bit-planes (grow.cuh): R not empty in it
     size_t bytes;      // total
     size_t zero_off, zero_bytes;   // region cleared at the start of a frame: the counters
@@ -170,6 +174,9 @@ Workspace carve(void* base, int h, int w) {
     ws.counts = (int32_t*)(p + off); off += align_up(NCOUNTERS * 4, 256);
     ws.ncand = ws.counts + LACOSMIC_MAX_NITER;
     ws.nquad = ws.counts + 2 * LACOSMIC_MAX_NITER;
+    ws.gains = (float*)(p + off); off += align_up(LACOSMIC_MAX_NITER * 4, 256);
+    ws.sel = (lac::SelState*)(p + off); off += 256;
+    ws.hist = (uint32_t*)(p + off); off += align_up(lac::SEL_BINS * 4, 256);
     ws.zero_bytes = off - ws.zero_off;
     ws.bytes = off;
     return ws;
@@ -199,6 +206,41 @@ int grow_replace(const lac::GrowArgs& ga, const int* prev, cudaStream_t st) {
     return LACOSMIC_OK;
 }
 
+// R21: sigma clipping of the residual plane R (select.cuh) -> *gain_out (device), stats (nullable, device)
+template <int MODE, int PASS>
+int sel_step(const float* R, size_t npx, const Workspace& ws, int grid, int last, float* gain_out, float* stats,
+             const int* prev, cudaStream_t st) {
+    lac::k_sel_hist<MODE, PASS><<<grid, 256, 0, st>>>(R, npx, ws.sel, ws.hist, prev);
+    LAUNCHED();
+    lac::k_sel_pick<MODE, PASS><<<1, 256, 0, st>>>(ws.sel, ws.hist, last, gain_out, stats, prev);
+    LAUNCHED();
+    return LACOSMIC_OK;
+}
+int sigma_clip_gain(const float* R, size_t npx, const Workspace& ws, float* gain_out, float* stats, const int* prev,
+                    cudaStream_t st) {
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int grid = (int)std::min<size_t>((size_t)sms * 8, (npx / 4 + 255) / 256 + 1);
+    Span sp(KC_SELECT, st);
+    lac::k_sel_init<<<1, 256, 0, st>>>(ws.sel, ws.hist, prev);
+    LAUNCHED();
+    for (int j = 0; j < lac::SEL_ROUNDS; ++j) {
+        const int last = j == lac::SEL_ROUNDS - 1;
+        int rc;
+        if ((rc = sel_step<0, 0>(R, npx, ws, grid, 0, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<0, 1>(R, npx, ws, grid, 0, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<0, 2>(R, npx, ws, grid, 0, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<1, 0>(R, npx, ws, grid, 0, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<1, 1>(R, npx, ws, grid, 0, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<1, 2>(R, npx, ws, grid, last, gain_out, stats, prev, st))) return rc;
+    }
+    return LACOSMIC_OK;
+}
+
+__global__ void k_fill_floats(float* dst, int n, float v) {
+    for (int i = threadIdx.x; i < n; i += blockDim.x) dst[i] = v;
+}
+
 // The iteration loop (O0-O7) for one frame.
 int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t* mask_out,
               float* clean_out, const Workspace& ws, int32_t* iter_counts, const lacosmic_debug* dbg,
@@ -209,6 +251,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     float* work = clean_out;
     Span whole(KC_STEP, st);   // the whole frame, copies included
     const bool lazy = p.mode == LACOSMIC_MODE_LAZY;
+    const bool estimate = p.gain == 0.0f;   // R21: no gain supplied
     // O0.  The lazy path fuses work = img_in into its first pass (which then reads img_in itself).
     const bool fused_copy = lazy && p.niter > 0;
     if (!fused_copy) CK(cudaMemcpyAsync(work, img, P * 4, cudaMemcpyDeviceToDevice, st));
@@ -244,14 +287,34 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     for (int t = 0; t < p.niter; ++t) {
         const int* prev = t > 0 ? ws.counts + (t - 1) : nullptr;
         const bool d = dbg && dbg->iter == t;
-        int rc;
+        int rc = LACOSMIC_OK;
+        const float* src = (fused_copy && t == 0) ? img : work;
+        auto noise_pass = [&](const lac::NoiseArgs& na, const float* from) -> int {
+            Span sp(KC_NOISE_S, st);
+            if (tma) lac::k_noise_S_tma<<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(from == img ? mapImgNS : mapWorkNS, na, ntx, ntilesNS, prev);
+            else lac::k_noise_S<<<ntilesNS, tb, 0, st>>>(from, na, ntx, prev);
+            LAUNCHED();
+            return LACOSMIC_OK;
+        };
+        if (estimate) {
+            // R21: the gain of this iteration from its input image.  One dense pass writes the residual plane
+            // (into the candidate list's storage, which is not in use yet) and, at t = 0, the work = img_in
+            // copy; its S output (gain 1) is scratch.  The selection leaves the gain in ws.gains[t].
+            lac::NoiseArgs ne{ws.S, nullptr, nullptr, nullptr, nullptr, (fused_copy && t == 0) ? work : nullptr,
+                              h, w, wpr, 1.0f, rn2, p.sigclip, siglow, p.satlevel, (float*)ws.clist, nullptr};
+            if ((rc = noise_pass(ne, src))) return rc;
+            if ((rc = sigma_clip_gain((const float*)ws.clist, P, ws, ws.gains + t, nullptr, prev, st))) return rc;
+            src = work;
+        }
         // lazy path, t >= 1: S, A1, A2 and the tests only change near the pixels the previous replacement
-        // rewrote (ws.NEED); a debug dump recomputes the planes everywhere
-        const bool incr = lazy && t > 0 && !d;
+        // rewrote (ws.NEED); a debug dump recomputes the planes everywhere, and so does an estimated gain
+        // (it changes with every iteration, and S with it)
+        const bool incr = lazy && t > 0 && !d && !estimate;
         lac::NoiseArgs na{ws.S, d ? dbg->Lp : nullptr, d ? dbg->N : nullptr,
                           lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
-                          (fused_copy && t == 0) ? work : nullptr,
-                          h, w, wpr, p.gain, rn2, p.sigclip, siglow, p.satlevel};
+                          (fused_copy && t == 0 && !estimate) ? work : nullptr,
+                          h, w, wpr, p.gain, rn2, p.sigclip, siglow, p.satlevel, nullptr,
+                          estimate ? ws.gains + t : nullptr};
         if (incr) {
             {
                 Span sp(KC_LISTS, st);
@@ -265,16 +328,10 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                 LAUNCHED();
             }
         } else {
-            const float* src = (fused_copy && t == 0) ? img : work;
-            {
-                Span sp(KC_NOISE_S, st);
-                if (tma) lac::k_noise_S_tma<<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(src == img ? mapImgNS : mapWorkNS, na, ntx, ntilesNS, prev);
-                else lac::k_noise_S<<<ntilesNS, tb, 0, st>>>(src, na, ntx, prev);
-                LAUNCHED();
-            }
+            if ((rc = noise_pass(na, src))) return rc;
             if (lazy) {
                 Span sp(KC_LISTS, st);
-                lac::k_list_candidates<<<bit_grid(h, w), 256, 0, st>>>(ws.A1, t > 0 ? ws.NEED : nullptr, ws.G1, ws.G2, ws.G2F, ws.M1,
+                lac::k_list_candidates<<<bit_grid(h, w), 256, 0, st>>>(ws.A1, (t > 0 && !estimate) ? ws.NEED : nullptr, ws.G1, ws.G2, ws.G2F, ws.M1,
                                                                       ws.clist, ws.ncand + t, h, w, wpr, prev);
                 LAUNCHED();
             }
@@ -312,6 +369,13 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     if (rc) return rc;
     if (iter_counts && p.niter > 0)
         CK(cudaMemcpyAsync(iter_counts, ws.counts, (size_t)p.niter * 4, cudaMemcpyDeviceToDevice, st));
+    if (dbg && dbg->gains && p.niter > 0) {
+        if (!estimate) {
+            k_fill_floats<<<1, 64, 0, st>>>(ws.gains, p.niter, p.gain);
+            LAUNCHED();
+        }
+        CK(cudaMemcpyAsync(dbg->gains, ws.gains, (size_t)p.niter * 4, cudaMemcpyDeviceToDevice, st));
+    }
     return LACOSMIC_OK;
 }
 
@@ -373,7 +437,7 @@ int lacosmic_run_ws(const float* img, int h, int w, const lacosmic_params* p, ui
     g_launches = 0;
     int rc = check_frame_args(img, h, w, p, mask_out, clean_out, workspace, workspace_bytes);
     if (rc) return rc;
-    if (dbg && (dbg->iter < 0 || dbg->iter >= LACOSMIC_MAX_NITER)) return LACOSMIC_ERR_PARAM;
+    if (dbg && (dbg->iter < -1 || dbg->iter >= LACOSMIC_MAX_NITER)) return LACOSMIC_ERR_PARAM;
     return run_frame(img, h, w, *p, mask_out, clean_out, carve(workspace, h, w), iter_counts, dbg,
                      (cudaStream_t)stream);
 }
@@ -545,6 +609,26 @@ int lacosmic_run_host_batch(const float* imgs_host, int n, int h, int w, const l
 
 // ---- single steps -----------------------------------------------------------------------------
 
+int lacosmic_estimate_gain(const float* img, int h, int w, float* gain_out, float* stats_out, void* workspace,
+                           size_t workspace_bytes, void* stream) {
+    g_launches = 0;
+    if (!img || !gain_out || !workspace) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    if (((uintptr_t)img & 15) || ((uintptr_t)workspace & 255)) return LACOSMIC_ERR_ALIGN;
+    if (workspace_bytes < lacosmic_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
+    Workspace ws = carve(workspace, h, w);
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t P = (size_t)h * w;
+    // the dense noise/S kernel (generic loader) with the residual plane switched on; S (gain 1) is scratch
+    lac::NoiseArgs ne{ws.S, nullptr, nullptr, nullptr, nullptr, nullptr, h, w, words_per_row(w), 1.0f, 0.0f,
+                      1.0f, 1.0f, 0.0f, (float*)ws.clist, nullptr};
+    const int ntx = (w + lac::TW - 1) / lac::TW, nt = ntx * ((h + lac::NS_TH - 1) / lac::NS_TH);
+    lac::k_noise_S<<<nt, lac::NT, 0, st>>>(img, ne, ntx, nullptr);
+    LAUNCHED();
+    return sigma_clip_gain((const float*)ws.clist, P, ws, gain_out, stats_out, nullptr, st);
+}
+
 int lacosmic_lplus(const float* in, float* out, int h, int w, void* stream) {
     if (!in || !out) return LACOSMIC_ERR_NULL;
     int rc = check_shape(h, w);
@@ -665,7 +749,7 @@ int lacosmic_kernel_timing_read(float* ms_sum, int32_t* spans) {
 
 const char* lacosmic_kernel_class_name(int cls) {
     static const char* names[KC_COUNT] = {"noise_S", "fine_gates", "grow_replace", "lists", "bits",
-                                          "eval_candidates", "noise_S_quads", "whole_frame"};
+                                          "eval_candidates", "noise_S_quads", "gain_select", "whole_frame"};
     return (cls >= 0 && cls < KC_COUNT) ? names[cls] : "?";
 }
 

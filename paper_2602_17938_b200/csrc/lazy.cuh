@@ -308,7 +308,7 @@ k_noise_S_quads(const float* __restrict__ work, NoiseArgs a, const int* __restri
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const float lp = lplus_px(win[2 + j][2], win[2 + j][1], win[2 + j][3], win[1 + j][2], win[3 + j][2]);
-                s[j] = fdiv_nn(lp, __fmul_rn(2.0f, noise_px(m5[j], a.gain, a.rn2)));
+                s[j] = fdiv_nn(lp, __fmul_rn(2.0f, noise_px(m5[j], a.gain_dev ? __ldg(a.gain_dev) : a.gain, a.rn2)));
                 const bool ok = (x + j < w) && (win[2 + j][2] < a.satlevel);                    // R12
                 n1 |= (uint32_t)(ok && s[j] > a.sigclip) << j;
                 n2 |= (uint32_t)(ok && s[j] > a.siglow) << j;

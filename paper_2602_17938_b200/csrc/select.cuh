@@ -1,0 +1,156 @@
+// Gain estimation when no gain is supplied (reading R21; "sigma_clip"):
+// sigma clipping of the residual plane r = (work - med5) / sqrt(med5) made of SELECTION only, so the
+// result does not depend on the order in which pixels are visited and equals the CPU oracle bit for bit.
+//
+// An element of given rank is found by a three-pass radix selection over an order-preserving 32-bit key of
+// the value (11 + 11 + 10 bits): every pass histograms one digit of the keys that match the digits already
+// fixed (shared-memory histogram per CTA, flushed with atomics), a one-CTA kernel then walks the histogram
+// to the bucket holding the wanted rank.  One round of the clipping is two selections over the kept set
+// K = { lo <= r <= hi }: the centre c (rank (n-1)/2 of r) and the MAD d (same rank of |r - c|).
+#pragma once
+#include "common.cuh"
+
+namespace lac {
+
+constexpr int SEL_BINS = 2048;
+constexpr int SEL_ROUNDS = 3;
+
+struct SelState {
+    float lo, hi;          // interval the current round started from
+    float c, s;            // centre and 1.4826 * MAD of the current round
+    uint32_t prefix;       // key digits fixed so far
+    uint32_t kth;          // wanted rank among the keys that match `prefix`
+    uint32_t n;            // |K| of the current round
+    uint32_t pad;
+};
+
+// order-preserving key: ascending keys <=> ascending floats; -0 is keyed as +0
+__device__ __forceinline__ uint32_t sel_key(float v) {
+    const uint32_t u = __float_as_uint(v == 0.0f ? 0.0f : v);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float sel_unkey(uint32_t k) {
+    return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
+}
+
+__global__ void k_sel_init(SelState* st, uint32_t* hist, const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;
+    for (int i = threadIdx.x; i < SEL_BINS; i += blockDim.x) hist[i] = 0;
+    if (threadIdx.x == 0) {
+        st->lo = -__int_as_float(0x7f800000);
+        st->hi = __int_as_float(0x7f800000);
+        st->c = 0.0f;
+        st->s = 0.0f;
+        st->prefix = 0;
+        st->kth = 0;
+        st->n = 0;
+    }
+}
+
+// MODE 0: value = r; MODE 1: value = |r - c|.  PASS 0/1/2: key bits 31..21 / 20..10 / 9..0.
+template <int MODE, int PASS>
+__global__ void __launch_bounds__(256)
+k_sel_hist(const float* __restrict__ R, size_t npx, const SelState* __restrict__ st, uint32_t* __restrict__ hist,
+           const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;   // fixed point (R17): the image did not change
+    __shared__ uint32_t sh[SEL_BINS];
+    for (int i = threadIdx.x; i < SEL_BINS; i += 256) sh[i] = 0;
+    __syncthreads();
+    const float lo = st->lo, hi = st->hi, c = st->c;
+    const uint32_t prefix = st->prefix;
+    auto visit = [&](float r) {
+        if (!(r >= lo && r <= hi)) return;
+        const float v = MODE == 0 ? r : fabsf(__fsub_rn(r, c));
+        const uint32_t k = sel_key(v);
+        if (PASS == 0) atomicAdd(&sh[k >> 21], 1u);
+        if (PASS == 1 && (k >> 21) == prefix) atomicAdd(&sh[(k >> 10) & 0x7ffu], 1u);
+        if (PASS == 2 && (k >> 10) == prefix) atomicAdd(&sh[k & 0x3ffu], 1u);
+    };
+    const size_t nvec = npx / 4;
+    const size_t stride = (size_t)gridDim.x * 256;
+    for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < nvec; i += stride) {
+        const float4 q = __ldg(reinterpret_cast<const float4*>(R) + i);
+        visit(q.x); visit(q.y); visit(q.z); visit(q.w);
+    }
+    if (blockIdx.x == 0 && threadIdx.x < (int)(npx - nvec * 4)) visit(R[nvec * 4 + threadIdx.x]);
+    __syncthreads();
+    for (int i = threadIdx.x; i < SEL_BINS; i += 256)
+        if (sh[i]) atomicAdd(&hist[i], sh[i]);
+}
+
+// One CTA of 256 threads: find the bucket holding rank kth, fix its digit, clear the histogram.  After the
+// last pass of MODE 0 the selected value is the centre c; after the last pass of MODE 1 it is the MAD d:
+// s = 1.4826 d and the next round's interval follow with exactly the oracle's operations; the `last` round
+// writes the gain instead (and the statistics {c, s, lo, hi, kept} of the round when stats is given).
+template <int MODE, int PASS>
+__global__ void __launch_bounds__(256)
+k_sel_pick(SelState* st, uint32_t* hist, int last, float* gain_out, float* stats, const int* prev_count) {
+    if (prev_count && *prev_count == 0) {          // fixed point (R17): same image, same estimate
+        if (MODE == 1 && PASS == 2 && last && threadIdx.x == 0) *gain_out = gain_out[-1];
+        return;
+    }
+    __shared__ uint32_t part[256];
+    __shared__ uint32_t s_bucket, s_before;
+    const int tid = threadIdx.x;
+    constexpr int PER = SEL_BINS / 256;
+    uint32_t loc[PER], sum = 0;
+#pragma unroll
+    for (int i = 0; i < PER; ++i) {
+        loc[i] = hist[tid * PER + i];
+        sum += loc[i];
+    }
+    part[tid] = sum;
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t kth = st->kth;
+        if (PASS == 0) {
+            uint32_t n = 0;
+            for (int i = 0; i < 256; ++i) n += part[i];
+            st->n = n;
+            kth = (n - 1u) / 2u;
+        }
+        uint32_t acc = 0;
+        int b = 0;
+        while (b < 255 && acc + part[b] <= kth) acc += part[b++];
+        s_bucket = (uint32_t)b;
+        s_before = acc;
+        st->kth = kth;   // rank within the chosen group is fixed below by the owner of the group
+    }
+    __syncthreads();
+    if (tid == (int)s_bucket) {
+        uint32_t kth = st->kth, acc = s_before;
+        int i = 0;
+        while (i < PER - 1 && acc + loc[i] <= kth) acc += loc[i++];
+        const uint32_t digit = (uint32_t)(tid * PER + i);
+        const uint32_t prefix = PASS == 0 ? digit : PASS == 1 ? ((st->prefix << 11) | digit) : ((st->prefix << 10) | digit);
+        st->kth = kth - acc;
+        st->prefix = prefix;
+        if (PASS == 2) {
+            const float v = sel_unkey(prefix);
+            if (MODE == 0) {
+                st->c = v;
+            } else {
+                const float s = __fmul_rn(1.4826f, v);
+                const float five_s = __fmul_rn(5.0f, s);
+                const float nlo = __fsub_rn(st->c, five_s), nhi = __fadd_rn(st->c, five_s);
+                st->s = s;
+                if (!last) {   // the next round starts from the intersection
+                    st->lo = nlo > st->lo ? nlo : st->lo;
+                    st->hi = nhi < st->hi ? nhi : st->hi;
+                } else {
+                    const float g = __fdiv_rn(1.0f, __fmul_rn(s, s));
+                    const float INF = __int_as_float(0x7f800000);
+                    *gain_out = (s > 0.0f && s < INF && g < INF) ? g : 1.0f;
+                    if (stats) {
+                        stats[0] = st->c; stats[1] = s; stats[2] = st->lo; stats[3] = st->hi; stats[4] = (float)st->n;
+                    }
+                }
+            }
+            st->prefix = 0;
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < PER; ++i) hist[tid * PER + i] = 0;
+}
+
+}  // namespace lac

@@ -37,7 +37,7 @@ def test_binding_lists_every_declared_symbol():
 def test_params_struct_layout():
     from paper_2602_17938_b200 import binding
     assert C.sizeof(binding._CParams) == 32          # 6 floats + 2 int32, no padding
-    assert C.sizeof(binding._CDebug) == 8 + 12 * 8
+    assert C.sizeof(binding._CDebug) == 8 + 13 * 8
 
 
 def test_workspace_sizes(L):
@@ -65,7 +65,7 @@ def test_argument_errors_without_gpu(L):
     assert run(i=img + 4) == -4 and run(w_=ws + 16) == -4
     assert run(c=img) == -5 and run(m=img + 100) == -5 and run(w_=img) == -5
     assert run(nb=need - 1) == -6
-    bads = [dict(gain=0.0), dict(gain=float("nan")), dict(readnoise=-1.0), dict(sigclip=0.0),
+    bads = [dict(gain=-1.0), dict(gain=float("nan")), dict(readnoise=-1.0), dict(sigclip=0.0),
             dict(sigfrac=0.0), dict(sigfrac=1.5), dict(objlim=-0.1), dict(niter=-1), dict(niter=65),
             dict(satlevel=float("nan")), dict(sigclip=float("inf")), dict(mode=2), dict(mode=-1)]
     for b in bads:

@@ -275,11 +275,72 @@ def test_host_batch_pipeline(lc, orc, concurrency):
         assert np.array_equal(r["clean"][j].numpy(), o["clean"]), j
 
 
+# ---------------------------------------------------------------- R21: gain estimation (gain = 0)
+@pytest.mark.parametrize("shape", [(1, 1), (3, 7), (33, 47), (70, 131), (64, 128), (257, 300)])
+def test_estimate_gain_bit_exact(lc, orc, shape):
+    """The estimator alone (selection only): gain and the clipping statistics equal the oracle's bits."""
+    import torch
+    rng = _rng(31)
+    x = (300.0 + np.sqrt(300.0 / 1.9) * rng.standard_normal(shape)).astype(np.float32)
+    if x.size > 50:
+        x.flat[rng.integers(0, x.size, x.size // 40)] += 4000.0          # cosmic-ray-like outliers
+    g, st = lc.lacosmic_estimate_gain(_t(x))
+    torch.cuda.synchronize()
+    go, sto = orc.estimate_gain(x)
+    assert _n(g)[0] == go, (float(_n(g)[0]), float(go))
+    assert np.array_equal(_n(st), sto), (_n(st), sto)
+
+
+def test_estimate_gain_ties_and_degenerate(lc, orc):
+    import torch
+    for x in (np.full((40, 50), 77.0, np.float32),                          # sigma = 0 -> gain 1
+              np.tile(np.array([10.0, 11.0], np.float32), (30, 20)),          # two values: massive ties
+              -np.abs(_rng(3).standard_normal((50, 60))).astype(np.float32)):  # negative image: med5 floored
+        g, st = lc.lacosmic_estimate_gain(_t(x))
+        torch.cuda.synchronize()
+        go, sto = orc.estimate_gain(x)
+        assert _n(g)[0] == go and np.array_equal(_n(st), sto)
+
+
+@pytest.mark.parametrize("mode", [0, 1], ids=["lazy", "dense"])
+@pytest.mark.parametrize("cfg", [dict(h=200, w=264, seed=71, n_star=12, n_cr=150, n_hot=30, sp_frac=0.004),
+                                 dict(h=131, w=97, seed=72, n_star=4, n_cr=60, sp_frac=0.0)])
+def test_whole_path_with_estimated_gain(lc, orc, cfg, mode):
+    """gain = 0: the gain of every iteration is estimated from that iteration's input (R21); masks, cleaned
+    frames, counts and the per-iteration gains equal the oracle's, in both evaluation modes."""
+    import torch
+    f = synth.make_frame(**cfg)
+    p = dict(PARAMS, gain=0.0)
+    o = orc.run(f.img, debug_iter=1, **p)
+    g = lc.lacosmic_run_ws(_t(f.img), lc.Params(mode=mode, **p), debug_iter=1, want_gains=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(_n(g["gains"]), o["gains"]), (_n(g["gains"]), o["gains"])
+    assert np.array_equal(_n(g["counts"])[:p["niter"]], o["counts"])
+    assert np.array_equal(_n(g["mask"]), o["mask"]) and np.array_equal(_n(g["clean"]), o["clean"])
+    for k in ("Lp", "N", "S", "G1", "M1", "M2", "M3", "C"):
+        assert np.array_equal(_n(g[k]), o[k]), k
+    # a supplied gain is reported back unchanged
+    g1 = lc.lacosmic_run_ws(_t(f.img), lc.Params(mode=mode, **PARAMS), want_gains=True)
+    torch.cuda.synchronize()
+    assert np.all(_n(g1["gains"]) == np.float32(PARAMS["gain"]))
+
+
+def test_estimated_gain_on_config0(lc, orc):
+    import torch
+    f = synth.make_config(0)
+    p = dict(PARAMS, gain=0.0)
+    o = orc.run(f.img, **p)
+    g = lc.lacosmic_run_ws(_t(f.img), lc.Params(**p), want_gains=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(_n(g["gains"]), o["gains"]) and np.array_equal(_n(g["mask"]), o["mask"])
+    assert np.array_equal(_n(g["clean"]), o["clean"]) and np.array_equal(_n(g["counts"])[:4], o["counts"])
+
+
 def test_gpu_argument_errors(lc):
     import torch
     img = torch.zeros((16, 16), device="cuda")
     with pytest.raises(lc.LacosmicError) as e:
-        lc.lacosmic_run_ws(img, lc.Params(gain=0.0))
+        lc.lacosmic_run_ws(img, lc.Params(gain=-1.0))
     assert e.value.code == -3
     with pytest.raises(lc.LacosmicError) as e:
         lc.lacosmic_run_ws(img, lc.Params(), clean_out=img)
