@@ -244,6 +244,36 @@ def run_cuda(args):
                        and res["counts"] == res_other["counts"])
     mask_frac = float(res["mask"].float().mean().item())
 
+    # ---- the same frame with no gain supplied (estimated at each iteration, R21)
+    gain_est = None
+    if not args.no_gain_estimation:
+        pe = lc.Params(mode=modes[main_mode], **dict(params, gain=0.0))
+        gains_t = torch.zeros(params["niter"], dtype=torch.float32, device=dev)
+
+        def step_est():
+            return lc.lacosmic_run_ws(img, pe, mask_out=mask, clean_out=clean, workspace=ws, iter_counts=counts)
+        lc.lacosmic_kernel_timing_enable(True)
+        step_est()
+        torch.cuda.synchronize()
+        lc.lacosmic_kernel_timing_read()
+        ms_est = timed(step_est, max(3, args.steps // 2), 1)
+        kt_est = lc.lacosmic_kernel_timing_read()
+        lc.lacosmic_kernel_timing_enable(False)
+        ge = lc.lacosmic_run_ws(img, pe, mask_out=mask, clean_out=clean, workspace=ws, iter_counts=counts,
+                                want_gains=True)
+        torch.cuda.synchronize()
+        nsel = max(kt_est["gain_select"][1], 1)
+        # one clipping = 18 histogram passes over the residual plane (4 B/px each)
+        sel_ms = kt_est["gain_select"][0] / nsel
+        gain_est = dict(frames_per_s=world * 1e3 / ms_est, ms_per_step=ms_est,
+                        gains=[float(v) for v in ge["gains"].cpu().numpy()],
+                        new_cr_per_iteration=counts.cpu().numpy().tolist(),
+                        select_ms_per_estimate=sel_ms,
+                        select_hbm_gbs=18 * npx * 4 / (sel_ms * 1e-3) / 1e9,
+                        select_hbm_frac=18 * npx * 4 / (sel_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                        note="gain = 0: residual plane + 3 rounds x 2 selections x 3 radix passes per iteration, "
+                             "then every plane recomputed with the estimated gain (no incremental iterations)")
+
     # ---- configs[3] in small: a stream of independent frames with per-frame parameters, resident in HBM,
     # through lacosmic_run_batch, back to back (concurrency 1) and with several frames in flight
     stream_res = None
@@ -395,7 +425,7 @@ def run_cuda(args):
         ref_comparisons_T_per_s=ref_cmp_rate,
         other_mode=dict(mode=other_mode, same_mask_clean_counts=modes_agree, roofline=roofline(res_other),
                         **summarise(res_other)),
-        stream=stream_res, e2e_stream=e2e_stream,
+        stream=stream_res, e2e_stream=e2e_stream, gain_estimation=gain_est,
         new_cr_per_iteration=res["counts"], mask_fraction=mask_frac,
         clocks=clocks, cpu_baseline=cpu,
         context="paper (PAPER.md:31,47): 55 s/frame dfcosmic C++ at 2 threads on AWS; GPU variant on an "
@@ -432,6 +462,7 @@ def main():
     ap.add_argument("--mode", default="lazy", choices=["lazy", "dense"],
                     help="which evaluation mode is the headline (the other is measured and reported too)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-gain-estimation", action="store_true", help="skip the gain = 0 leg (DESIGN.md R21)")
     ap.add_argument("--stream-frames", type=int, default=12,
                     help="frames of the configs[3] stream leg (0 = skip; 64 = the full configuration)")
     ap.add_argument("--stream-concurrency", type=int, default=4,
