@@ -404,3 +404,51 @@ def test_transposed_orientation_windows(lc, orc):
     """R19: PAPER.md:31 says 4000x6500 without naming the axis order; exercise 6500 rows x 4000 cols."""
     f = synth.make_frame(6500, 4000, seed=3, n_star=8000, n_cr=30000, sp_frac=0.005)
     _check_full_frame(lc, orc, f.img, PARAMS, "6500x4000")
+
+
+def test_maximum_frame_size(lc, orc):
+    """Largest frame the ABI accepts on a square grid (h*w < 2^31, w % 4 == 0): 46336 x 46336 = 2 147 024 896 px.
+    Flat pixel indices run up to the int32 limit in every kernel.  The frame is made on the device (sky +
+    Gaussian noise + 0.1 % single-pixel hits), nine windows (corners, edges, centre) are compared with the
+    oracle run on the haloed crop, the two modes must agree on the whole frame, and the size-independent
+    properties (P7, R11) are checked on the device."""
+    import torch
+    h = w = 46336
+    assert h * w < 2 ** 31 and (h + 1) * (w + 4) >= 2 ** 31 - 2 ** 18
+    free, _ = torch.cuda.mem_get_info()
+    if free < 70 * 2 ** 30:
+        pytest.skip("needs 70 GB of free device memory")
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(77)
+    img = torch.empty((h, w), dtype=torch.float32, device="cuda")
+    img.normal_(100.0, 14.142, generator=gen)
+    nhit = h * w // 1000
+    idx = torch.unique(torch.randint(0, h * w, (nhit,), device="cuda", generator=gen))
+    amp = torch.empty(idx.numel(), dtype=torch.float32, device="cuda").uniform_(500.0, 10000.0, generator=gen)
+    img.view(-1)[idx] += amp
+    # make sure the extreme corners hold a hit each (last flat index included)
+    for (y, x) in ((0, 0), (0, w - 1), (h - 1, 0), (h - 1, w - 1), (h - 2, w - 3)):
+        img[y, x] = 5000.0
+    del idx, amp
+    ws = torch.empty(lc.lacosmic_workspace_bytes(h, w), dtype=torch.uint8, device="cuda")
+    out = {}
+    for mode in (lc.MODE_LAZY, lc.MODE_DENSE):
+        g = lc.lacosmic_run_ws(img, lc.Params(mode=mode, **PARAMS), workspace=ws)
+        torch.cuda.synchronize()
+        out[mode] = g
+        if mode == lc.MODE_LAZY:
+            gm, gc, counts = g["mask"], g["clean"], _n(g["counts"])
+            for (y0, x0, s) in _windows(h, w):
+                ya, yb, xa, xb = max(y0 - HALO, 0), min(y0 + s + HALO, h), max(x0 - HALO, 0), min(x0 + s + HALO, w)
+                o = orc.run(_n(img[ya:yb, xa:xb].contiguous()), **PARAMS)
+                sl = (slice(y0 - ya, y0 - ya + s), slice(x0 - xa, x0 - xa + s))
+                assert np.array_equal(_n(gm[y0:y0 + s, x0:x0 + s]), o["mask"][sl]), (y0, x0)
+                assert np.array_equal(_n(gc[y0:y0 + s, x0:x0 + s]), o["clean"][sl]), (y0, x0)
+                assert o["mask"][sl].sum() > 0
+            nmask = int(gm.sum(dtype=torch.int64).item())
+            assert int(counts[:PARAMS["niter"]].astype(np.int64).sum()) == nmask and nmask > nhit // 2
+            assert bool(torch.equal(torch.where(gm == 0, gc, img), img))          # unmasked pixels untouched
+            assert int(gm[0, 0]) == 1 and int(gm[h - 1, w - 1]) == 1 and int(gm[h - 2, w - 3]) == 1
+    a, b = out[lc.MODE_LAZY], out[lc.MODE_DENSE]
+    assert bool(torch.equal(a["mask"], b["mask"])) and bool(torch.equal(a["clean"], b["clean"]))
+    assert np.array_equal(_n(a["counts"]), _n(b["counts"]))
