@@ -179,7 +179,6 @@ k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restric
     if (prev_count && *prev_count == 0) return;
     const int n = *nlist;
     const int h = a.h, w = a.w;
-    const size_t npx = (size_t)h * w;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const int p = list[i];
         const int y = p / w, x = p - y * w;
@@ -192,44 +191,7 @@ k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restric
         atomicOr(a.G1 + q, bit);
         uint32_t rows[9];   // bit c of rows[r] = P(V[r][c])
         float tlo, thi;
-        if (y >= 4 && x >= 4 && x + 4 < w && y + 4 < h && (size_t)(y + 4) * w + x + 8 <= npx) {
-            // interior: every window row is covered by three 16-byte aligned vectors; P is evaluated on all
-            // 12 values and the 9 of the window are selected by a shift
-            float e[3][12];
-            int sh[3];
-#pragma unroll
-            for (int r = 0; r < 3; ++r) {
-                const int base = p + (r - 1) * w - 4, b = base & ~3;
-                sh[r] = base - b;
-                const float4 a0 = ldg4(a.work + b), a1 = ldg4(a.work + b + 4), a2 = ldg4(a.work + b + 8);
-                e[r][0] = a0.x; e[r][1] = a0.y; e[r][2] = a0.z; e[r][3] = a0.w;
-                e[r][4] = a1.x; e[r][5] = a1.y; e[r][6] = a1.z; e[r][7] = a1.w;
-                e[r][8] = a2.x; e[r][9] = a2.y; e[r][10] = a2.z; e[r][11] = a2.w;
-            }
-            float ctr[3][3];   // work at rows y-1..y+1, columns x-1..x+1 = elements sh+3 .. sh+5
-#pragma unroll
-            for (int r = 0; r < 3; ++r)
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    const int s = sh[r];
-                    ctr[r][c] = s == 0 ? e[r][3 + c] : s == 1 ? e[r][4 + c] : s == 2 ? e[r][5 + c] : e[r][6 + c];
-                }
-            const float lp = lplus_px(ctr[1][1], ctr[0][1], ctr[2][1], ctr[1][0], ctr[1][2]);
-            const float m3c = med9(ctr[0][0], ctr[0][1], ctr[0][2], ctr[1][0], ctr[1][1], ctr[1][2], ctr[2][0],
-                                   ctr[2][1], ctr[2][2]);
-            if (!fine_bracket(lp, m3c, a.objlim, tlo, thi)) continue;
-#pragma unroll
-            for (int r = 0; r < 9; ++r) {
-                if (r >= 3 && r <= 5) {
-                    rows[r] = (fine_bits<12>(e[r - 3], lp, m3c, a.objlim, tlo, thi) >> sh[r - 3]) & 0x1ffu;
-                } else {
-                    const int base = p + (r - 4) * w - 4, b = base & ~3;
-                    const float4 a0 = ldg4(a.work + b), a1 = ldg4(a.work + b + 4), a2 = ldg4(a.work + b + 8);
-                    const float f[12] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w, a2.x, a2.y, a2.z, a2.w};
-                    rows[r] = (fine_bits<12>(f, lp, m3c, a.objlim, tlo, thi) >> (base - b)) & 0x1ffu;
-                }
-            }
-        } else {
+        {
             int xx[9];
 #pragma unroll
             for (int c = 0; c < 9; ++c) xx[c] = clampi(x + c - 4, 0, w - 1);
@@ -243,7 +205,7 @@ k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restric
             const float m3c = med9(ctr[0][0], ctr[0][1], ctr[0][2], ctr[1][0], ctr[1][1], ctr[1][2], ctr[2][0],
                                    ctr[2][1], ctr[2][2]);
             if (!fine_bracket(lp, m3c, a.objlim, tlo, thi)) continue;
-#pragma unroll 1
+#pragma unroll 3
             for (int r = 0; r < 9; ++r) {
                 const float* row = a.work + (size_t)clampi(y + r - 4, 0, h - 1) * w;
                 float f[9];
