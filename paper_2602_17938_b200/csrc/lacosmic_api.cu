@@ -210,9 +210,7 @@ int grow_replace(const lac::GrowArgs& ga, const int* prev, cudaStream_t st) {
 template <int MODE, int PASS>
 int sel_step(const float* R, size_t npx, const Workspace& ws, int grid, int last, float* gain_out, float* stats,
              const int* prev, cudaStream_t st) {
-    lac::k_sel_hist<MODE, PASS><<<grid, 256, 0, st>>>(R, npx, ws.sel, ws.hist, prev);
-    LAUNCHED();
-    lac::k_sel_pick<MODE, PASS><<<1, 256, 0, st>>>(ws.sel, ws.hist, last, gain_out, stats, prev);
+    lac::k_sel_hist<MODE, PASS><<<grid, 256, 0, st>>>(R, npx, ws.sel, ws.hist, last, gain_out, stats, prev);
     LAUNCHED();
     return LACOSMIC_OK;
 }
@@ -220,7 +218,11 @@ int sigma_clip_gain(const float* R, size_t npx, const Workspace& ws, float* gain
                     cudaStream_t st) {
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const int grid = (int)std::min<size_t>((size_t)sms * 8, (npx / 4 + 255) / 256 + 1);
+#ifndef LAC_SEL_CTAS_PER_SM
+#define LAC_SEL_CTAS_PER_SM 8
+#endif
+    // full occupancy measured best on B200 (8 > 4 > 2 > 1 CTAs per SM): the pass is a streaming read
+    const int grid = (int)std::min<size_t>((size_t)sms * LAC_SEL_CTAS_PER_SM, (npx / 4 + 255) / 256 + 1);
     Span sp(KC_SELECT, st);
     lac::k_sel_init<<<1, 256, 0, st>>>(ws.sel, ws.hist, prev);
     LAUNCHED();

@@ -4,8 +4,8 @@
 //
 // An element of given rank is found by a three-pass radix selection over an order-preserving 32-bit key of
 // the value (11 + 11 + 10 bits): every pass histograms one digit of the keys that match the digits already
-// fixed (shared-memory histogram per CTA, flushed with atomics), a one-CTA kernel then walks the histogram
-// to the bucket holding the wanted rank.  One round of the clipping is two selections over the kept set
+// fixed (shared-memory histogram per CTA, flushed with atomics); the CTA that finishes last (atomic ticket)
+// then walks the 2048 counts to the bucket holding the wanted rank, so a pass is one launch.  One round of the clipping is two selections over the kept set
 // K = { lo <= r <= hi }: the centre c (rank (n-1)/2 of r) and the MAD d (same rank of |r - c|).
 #pragma once
 #include "common.cuh"
@@ -21,13 +21,15 @@ struct SelState {
     uint32_t prefix;       // key digits fixed so far
     uint32_t kth;          // wanted rank among the keys that match `prefix`
     uint32_t n;            // |K| of the current round
-    uint32_t pad;
+    uint32_t ticket;       // CTAs of the running pass that have flushed their histogram
 };
 
-// order-preserving key: ascending keys <=> ascending floats; -0 is keyed as +0
+// order-preserving key: ascending keys <=> ascending floats (a total order that refines the float order:
+// -0 sorts directly below +0, so an element of given rank has the right VALUE; NaNs fall outside
+// [key(-inf), key(+inf)])
 __device__ __forceinline__ uint32_t sel_key(float v) {
-    const uint32_t u = __float_as_uint(v == 0.0f ? 0.0f : v);
-    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+    const uint32_t u = __float_as_uint(v);
+    return u ^ ((uint32_t)((int32_t)u >> 31) | 0x80000000u);
 }
 __device__ __forceinline__ float sel_unkey(uint32_t k) {
     return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
@@ -44,85 +46,44 @@ __global__ void k_sel_init(SelState* st, uint32_t* hist, const int* prev_count) 
         st->prefix = 0;
         st->kth = 0;
         st->n = 0;
+        st->ticket = 0;
     }
 }
 
-// MODE 0: value = r; MODE 1: value = |r - c|.  PASS 0/1/2: key bits 31..21 / 20..10 / 9..0.
+// Executed by the last CTA of a pass (256 threads; `scan` is 256 words of shared memory): find the bucket
+// holding rank kth, fix its digit, clear the histogram.  After the last pass of MODE 0 the selected value is
+// the centre c; after the last pass of MODE 1 it is the MAD d: s = 1.4826 d and the next round's interval
+// follow with exactly the oracle's operations; the `last` round writes the gain instead (and the statistics
+// {c, s, lo, hi, kept} of the round when stats is given).
 template <int MODE, int PASS>
-__global__ void __launch_bounds__(256)
-k_sel_hist(const float* __restrict__ R, size_t npx, const SelState* __restrict__ st, uint32_t* __restrict__ hist,
-           const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;   // fixed point (R17): the image did not change
-    __shared__ uint32_t sh[SEL_BINS];
-    for (int i = threadIdx.x; i < SEL_BINS; i += 256) sh[i] = 0;
-    __syncthreads();
-    const float lo = st->lo, hi = st->hi, c = st->c;
-    const uint32_t prefix = st->prefix;
-    auto visit = [&](float r) {
-        if (!(r >= lo && r <= hi)) return;
-        const float v = MODE == 0 ? r : fabsf(__fsub_rn(r, c));
-        const uint32_t k = sel_key(v);
-        if (PASS == 0) atomicAdd(&sh[k >> 21], 1u);
-        if (PASS == 1 && (k >> 21) == prefix) atomicAdd(&sh[(k >> 10) & 0x7ffu], 1u);
-        if (PASS == 2 && (k >> 10) == prefix) atomicAdd(&sh[k & 0x3ffu], 1u);
-    };
-    const size_t nvec = npx / 4;
-    const size_t stride = (size_t)gridDim.x * 256;
-    for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < nvec; i += stride) {
-        const float4 q = __ldg(reinterpret_cast<const float4*>(R) + i);
-        visit(q.x); visit(q.y); visit(q.z); visit(q.w);
-    }
-    if (blockIdx.x == 0 && threadIdx.x < (int)(npx - nvec * 4)) visit(R[nvec * 4 + threadIdx.x]);
-    __syncthreads();
-    for (int i = threadIdx.x; i < SEL_BINS; i += 256)
-        if (sh[i]) atomicAdd(&hist[i], sh[i]);
-}
-
-// One CTA of 256 threads: find the bucket holding rank kth, fix its digit, clear the histogram.  After the
-// last pass of MODE 0 the selected value is the centre c; after the last pass of MODE 1 it is the MAD d:
-// s = 1.4826 d and the next round's interval follow with exactly the oracle's operations; the `last` round
-// writes the gain instead (and the statistics {c, s, lo, hi, kept} of the round when stats is given).
-template <int MODE, int PASS>
-__global__ void __launch_bounds__(256)
-k_sel_pick(SelState* st, uint32_t* hist, int last, float* gain_out, float* stats, const int* prev_count) {
-    if (prev_count && *prev_count == 0) {          // fixed point (R17): same image, same estimate
-        if (MODE == 1 && PASS == 2 && last && threadIdx.x == 0) *gain_out = gain_out[-1];
-        return;
-    }
-    __shared__ uint32_t part[256];
-    __shared__ uint32_t s_bucket, s_before;
+__device__ __forceinline__ void sel_pick(SelState* st, uint32_t* hist, uint32_t* scan, int last, float* gain_out,
+                                         float* stats) {
     const int tid = threadIdx.x;
     constexpr int PER = SEL_BINS / 256;
     uint32_t loc[PER], sum = 0;
 #pragma unroll
     for (int i = 0; i < PER; ++i) {
-        loc[i] = hist[tid * PER + i];
+        loc[i] = __ldcg(hist + tid * PER + i);
         sum += loc[i];
+        hist[tid * PER + i] = 0;
     }
-    part[tid] = sum;
+    scan[tid] = sum;
     __syncthreads();
-    if (tid == 0) {
-        uint32_t kth = st->kth;
-        if (PASS == 0) {
-            uint32_t n = 0;
-            for (int i = 0; i < 256; ++i) n += part[i];
-            st->n = n;
-            kth = (n - 1u) / 2u;
-        }
-        uint32_t acc = 0;
-        int b = 0;
-        while (b < 255 && acc + part[b] <= kth) acc += part[b++];
-        s_bucket = (uint32_t)b;
-        s_before = acc;
-        st->kth = kth;   // rank within the chosen group is fixed below by the owner of the group
+    for (int d = 1; d < 256; d <<= 1) {   // inclusive prefix sums of the 256 group totals
+        const uint32_t v = tid >= d ? scan[tid - d] : 0u;
+        __syncthreads();
+        scan[tid] += v;
+        __syncthreads();
     }
-    __syncthreads();
-    if (tid == (int)s_bucket) {
-        uint32_t kth = st->kth, acc = s_before;
+    const uint32_t incl = scan[tid], excl = incl - sum, n = scan[255];
+    const uint32_t kth = PASS == 0 ? (n - 1u) / 2u : st->kth;
+    if (kth >= excl && kth < incl) {      // exactly one thread: the group that holds the rank
+        uint32_t acc = excl;
         int i = 0;
         while (i < PER - 1 && acc + loc[i] <= kth) acc += loc[i++];
         const uint32_t digit = (uint32_t)(tid * PER + i);
         const uint32_t prefix = PASS == 0 ? digit : PASS == 1 ? ((st->prefix << 11) | digit) : ((st->prefix << 10) | digit);
+        if (PASS == 0) st->n = n;
         st->kth = kth - acc;
         st->prefix = prefix;
         if (PASS == 2) {
@@ -149,8 +110,72 @@ k_sel_pick(SelState* st, uint32_t* hist, int last, float* gain_out, float* stats
             st->prefix = 0;
         }
     }
+}
+
+// MODE 0: value = r; MODE 1: value = |r - c|.  PASS 0/1/2: key bits 31..21 / 20..10 / 9..0.
+template <int MODE, int PASS>
+__global__ void __launch_bounds__(256)
+k_sel_hist(const float* __restrict__ R, size_t npx, SelState* st, uint32_t* hist, int last, float* gain_out,
+           float* stats, const int* prev_count) {
+    if (prev_count && *prev_count == 0) {          // fixed point (R17): same image, same estimate
+        if (MODE == 1 && PASS == 2 && last && blockIdx.x == 0 && threadIdx.x == 0) *gain_out = gain_out[-1];
+        return;
+    }
+    __shared__ uint32_t sh[SEL_BINS];
+    for (int i = threadIdx.x; i < SEL_BINS; i += 256) sh[i] = 0;
+    __syncthreads();
+    const float lo = st->lo, hi = st->hi, c = st->c;
+    // keys under the digits already fixed form one range; MODE 0 intersects it with the kept interval, which
+    // is a key range too (the key is monotone), so a value costs one key and one unsigned range check
+    constexpr int SHIFT = PASS == 0 ? 21 : PASS == 1 ? 10 : 0;
+    constexpr uint32_t MASK = PASS == 2 ? 0x3ffu : 0x7ffu;
+    uint32_t klo = 0u, khi = 0xffffffffu;
+    if (PASS == 1) { klo = st->prefix << 21; khi = klo | 0x1fffffu; }
+    if (PASS == 2) { klo = st->prefix << 10; khi = klo | 0x3ffu; }
+    if (MODE == 0) {
+        klo = max(klo, sel_key(lo));
+        khi = min(khi, sel_key(hi));
+    }
+    const bool none = klo > khi;                    // empty intersection (cannot hold the wanted rank)
+    const uint32_t span = khi - klo;
+    auto visit = [&](float r) {
+        uint32_t k;
+        if (MODE == 0) {
+            k = sel_key(r);
+        } else {
+            if (!(r >= lo && r <= hi)) return;
+            k = __float_as_uint(fabsf(__fsub_rn(r, c))) | 0x80000000u;   // non-negative value
+        }
+        if (!none && k - klo <= span) atomicAdd(&sh[(k >> SHIFT) & MASK], 1u);
+    };
+    const size_t nvec = npx / 4;
+    const size_t stride = (size_t)gridDim.x * 256, end = nvec;
+    size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
+    for (; i + 3 * stride < end; i += 4 * stride) {   // four independent 16-byte loads in flight per thread
+        float4 q[4];
 #pragma unroll
-    for (int i = 0; i < PER; ++i) hist[tid * PER + i] = 0;
+        for (int u = 0; u < 4; ++u) q[u] = __ldg(reinterpret_cast<const float4*>(R) + i + u * stride);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { visit(q[u].x); visit(q[u].y); visit(q[u].z); visit(q[u].w); }
+    }
+    for (; i < end; i += stride) {
+        const float4 q = __ldg(reinterpret_cast<const float4*>(R) + i);
+        visit(q.x); visit(q.y); visit(q.z); visit(q.w);
+    }
+    if (blockIdx.x == 0 && threadIdx.x < (int)(npx - nvec * 4)) visit(R[nvec * 4 + threadIdx.x]);
+    __syncthreads();
+    for (int i = threadIdx.x; i < SEL_BINS; i += 256)
+        if (sh[i]) atomicAdd(&hist[i], sh[i]);
+    // the CTA that flushes last picks the bucket (threadFenceReduction pattern)
+    __shared__ bool s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(&st->ticket, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    sel_pick<MODE, PASS>(st, hist, sh, last, gain_out, stats);
+    if (threadIdx.x == 0) st->ticket = 0;
 }
 
 }  // namespace lac
