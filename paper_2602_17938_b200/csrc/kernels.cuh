@@ -118,7 +118,8 @@ struct NoiseArgs {
                              // into the first pass, which then reads img_in itself)
     int h, w, wpr;
     float gain, rn2, sigclip, siglow, satlevel;
-    float* R;                // nullable (R21): also write r = (work - med5) / sqrt(max(med5, 1e-4)) here
+    float* R;                // nullable (R21): also write r = (work - med5) / sqrt(max(med5, 1e-4)) here, and
+                             // store med5 itself in the S plane (k_S_from_m5 turns it into S once the gain is known)
     const float* gain_dev;   // nullable (R21): the gain of this iteration, estimated on the device
 };
 
@@ -161,7 +162,8 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
                 n2 |= (uint32_t)(ok && s[j] > a.siglow) << j;
             }
             size_t ro = (size_t)y * a.w;
-            store4(a.S, ro, x, a.w, s);
+            if (a.R) store4(a.S, ro, x, a.w, m5);
+            else store4(a.S, ro, x, a.w, s);
             if (a.dbgLp) store4(a.dbgLp, ro, x, a.w, lp);
             if (a.dbgN) store4(a.dbgN, ro, x, a.w, n);
             if (a.copy_out) store4(a.copy_out, ro, x, a.w, ctr);
@@ -454,6 +456,109 @@ k_fine_gates_tma(const __grid_constant__ CUtensorMap mapWork, const __grid_const
         }
         fine_gates_tile(bufA(st), smB, bufS(st), a, x0, y0, tid);
         __syncthreads();   // stage st and smB are free again
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// R21, second half of an iteration with an estimated gain: the S plane holds med5(work) (written by the
+// residual pass); turn it into S in place, with L+, N and the A1 / A2 planes, using the gain the selection left
+// on the device.  Same operations as noise_S_tile; no median here, so the pass is HBM bound (work and med5
+// read, S written).  one_S_px: one pixel.
+__device__ __forceinline__ float one_S_px(float c, float U, float D, float Lf, float R, float m5, float gain,
+                                          const NoiseArgs& a, bool inframe, int j, uint32_t& n1, uint32_t& n2,
+                                          float& lp, float& nn) {
+    lp = lplus_px(c, U, D, Lf, R);
+    nn = noise_px(m5, gain, a.rn2);
+    const float s = fdiv_nn(lp, __fmul_rn(2.0f, nn));
+    const bool ok = inframe && (c < a.satlevel);                                         // R12
+    n1 |= (uint32_t)(ok && s > a.sigclip) << j;
+    n2 |= (uint32_t)(ok && s > a.siglow) << j;
+    return s;
+}
+
+// w % 4 == 0: a warp owns 128 columns x SM5_ROWS rows; lane l keeps the four pixels x0 + 4 l .. + 3 of three
+// consecutive rows in registers (sliding down), horizontal neighbours come from the adjacent lanes.
+constexpr int SM5_ROWS = 16;
+__global__ void __launch_bounds__(256)
+k_S_from_m5(const float* __restrict__ work, NoiseArgs a, const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    const int h = a.h, w = a.w;
+    const int x = blockIdx.x * 128 + 4 * lane;
+    const int ya = (blockIdx.y * 8 + wi) * SM5_ROWS;
+    if (ya >= h) return;                          // warp-uniform
+    const bool inx = x < w;                       // w % 4 == 0: a quad is inside or outside as a whole
+    const int xc = inx ? x : w - 4;               // out-of-frame lanes read a valid quad; results unused
+    const float gain = a.gain_dev ? __ldg(a.gain_dev) : a.gain;
+    auto ldrow = [&](int y) -> float4 {
+        return __ldg(reinterpret_cast<const float4*>(work + (size_t)clampi(y, 0, h - 1) * w + xc));
+    };
+    float4 up = ldrow(ya - 1), cur = ldrow(ya), dn;
+    const int yend = min(ya + SM5_ROWS, h);
+    for (int y = ya; y < yend; ++y) {
+        dn = ldrow(y + 1);
+        const size_t o = (size_t)y * w + xc;
+        const float4 m5 = *reinterpret_cast<const float4*>(a.S + o);
+        float lf = __shfl_up_sync(0xffffffffu, cur.w, 1);          // R3: clamped at the frame edge
+        float rt = __shfl_down_sync(0xffffffffu, cur.x, 1);
+        if (lane == 0) lf = x > 0 ? __ldg(work + (size_t)y * w + x - 1) : cur.x;
+        if (x + 4 >= w) rt = cur.w;
+        else if (lane == 31) rt = __ldg(work + (size_t)y * w + x + 4);
+        uint32_t n1 = 0, n2 = 0;
+        float lp[4], nn[4], s[4];
+        s[0] = one_S_px(cur.x, up.x, dn.x, lf, cur.y, m5.x, gain, a, inx, 0, n1, n2, lp[0], nn[0]);
+        s[1] = one_S_px(cur.y, up.y, dn.y, cur.x, cur.z, m5.y, gain, a, inx, 1, n1, n2, lp[1], nn[1]);
+        s[2] = one_S_px(cur.z, up.z, dn.z, cur.y, cur.w, m5.z, gain, a, inx, 2, n1, n2, lp[2], nn[2]);
+        s[3] = one_S_px(cur.w, up.w, dn.w, cur.z, rt, m5.w, gain, a, inx, 3, n1, n2, lp[3], nn[3]);
+        const uint32_t b1 = nibbles_to_word(n1, lane), b2 = nibbles_to_word(n2, lane);
+        if (inx) {
+            *reinterpret_cast<float4*>(a.S + o) = make_float4(s[0], s[1], s[2], s[3]);
+            if (a.dbgLp) store4(a.dbgLp, (size_t)y * w, x, w, lp);
+            if (a.dbgN) store4(a.dbgN, (size_t)y * w, x, w, nn);
+            if (a.A1 && (lane & 7) == 0) {
+                const size_t q = (size_t)y * a.wpr + (x >> 5);
+                a.A1[q] = b1;
+                a.A2[q] = b2;
+            }
+        }
+        up = cur;
+        cur = dn;
+    }
+}
+
+// any w: one thread per aligned group of 4 pixels, clamped scalar loads
+__global__ void __launch_bounds__(256)
+k_S_from_m5_generic(const float* __restrict__ work, NoiseArgs a, const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    const int h = a.h, w = a.w;
+    const int x = blockIdx.x * 128 + 4 * lane, y = blockIdx.y * 8 + wi;
+    if (y >= h) return;                           // warp-uniform
+    const float gain = a.gain_dev ? __ldg(a.gain_dev) : a.gain;
+    const float* rc = work + (size_t)y * w;
+    const float* ru = work + (size_t)max(y - 1, 0) * w;
+    const float* rd = work + (size_t)min(y + 1, h - 1) * w;
+    float c[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) c[k] = __ldg(rc + clampi(x - 1 + k, 0, w - 1));
+    uint32_t n1 = 0, n2 = 0;
+    float lp[4], nn[4], s[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int xj = min(x + j, w - 1);
+        s[j] = one_S_px(c[1 + j], __ldg(ru + xj), __ldg(rd + xj), c[j], c[2 + j], a.S[(size_t)y * w + xj], gain, a,
+                        x + j < w, j, n1, n2, lp[j], nn[j]);
+    }
+    const uint32_t b1 = nibbles_to_word(n1, lane), b2 = nibbles_to_word(n2, lane);
+    if (x < w) {
+        store4(a.S, (size_t)y * w, x, w, s);
+        if (a.dbgLp) store4(a.dbgLp, (size_t)y * w, x, w, lp);
+        if (a.dbgN) store4(a.dbgN, (size_t)y * w, x, w, nn);
+        if (a.A1 && (lane & 7) == 0) {
+            const size_t q = (size_t)y * a.wpr + (x >> 5);
+            a.A1[q] = b1;
+            a.A2[q] = b2;
+        }
     }
 }
 

@@ -300,8 +300,8 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         };
         if (estimate) {
             // R21: the gain of this iteration from its input image.  One dense pass writes the residual plane
-            // (into the candidate list's storage, which is not in use yet) and, at t = 0, the work = img_in
-            // copy; its S output (gain 1) is scratch.  The selection leaves the gain in ws.gains[t].
+            // (into the candidate list's storage, which is not in use yet), med5(work) into the S plane and, at
+            // t = 0, the work = img_in copy.  The selection leaves the gain in ws.gains[t].
             lac::NoiseArgs ne{ws.S, nullptr, nullptr, nullptr, nullptr, (fused_copy && t == 0) ? work : nullptr,
                               h, w, wpr, 1.0f, rn2, p.sigclip, siglow, p.satlevel, (float*)ws.clist, nullptr};
             if ((rc = noise_pass(ne, src))) return rc;
@@ -330,7 +330,15 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                 LAUNCHED();
             }
         } else {
-            if ((rc = noise_pass(na, src))) return rc;
+            if (estimate) {
+                // the residual pass left med5(work) in the S plane: S, A1, A2 follow elementwise (HBM bound)
+                Span sp(KC_NOISE_S, st);
+                if (tma) lac::k_S_from_m5<<<dim3((w + 127) / 128, (h + 8 * lac::SM5_ROWS - 1) / (8 * lac::SM5_ROWS)), 256, 0, st>>>(work, na, prev);
+                else lac::k_S_from_m5_generic<<<dim3((w + 127) / 128, (h + 7) / 8), 256, 0, st>>>(work, na, prev);
+                LAUNCHED();
+            } else if ((rc = noise_pass(na, src))) {
+                return rc;
+            }
             if (lazy) {
                 Span sp(KC_LISTS, st);
                 lac::k_list_candidates<<<bit_grid(h, w), 256, 0, st>>>(ws.A1, (t > 0 && !estimate) ? ws.NEED : nullptr, ws.G1, ws.G2, ws.G2F, ws.M1,
