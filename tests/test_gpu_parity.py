@@ -452,3 +452,36 @@ def test_maximum_frame_size(lc, orc):
     a, b = out[lc.MODE_LAZY], out[lc.MODE_DENSE]
     assert bool(torch.equal(a["mask"], b["mask"])) and bool(torch.equal(a["clean"], b["clean"]))
     assert np.array_equal(_n(a["counts"]), _n(b["counts"]))
+
+
+def test_cuda_graph_capture_and_replay(lc, orc):
+    """The whole-path call enqueues work only (no host synchronisation, no allocation with a caller-supplied
+    workspace), so it can be captured into a CUDA graph and replayed: small frames are launch-latency bound
+    (DESIGN.md section 7).  The replayed graph must reproduce the oracle's result from cleared outputs."""
+    import torch
+    f = synth.make_frame(256, 320, seed=21, n_star=20, n_cr=150, n_hot=40, sp_frac=0.003)
+    o = orc.run(f.img, **PARAMS)
+    img = _t(f.img)
+    h, w = img.shape
+    mask = torch.empty((h, w), dtype=torch.uint8, device="cuda")
+    clean = torch.empty_like(img)
+    ws = torch.empty(lc.lacosmic_workspace_bytes(h, w), dtype=torch.uint8, device="cuda")
+    counts = torch.zeros(PARAMS["niter"], dtype=torch.int32, device="cuda")
+    P = lc.Params(**PARAMS)
+
+    def step():
+        lc.lacosmic_run_ws(img, P, mask_out=mask, clean_out=clean, workspace=ws, iter_counts=counts)
+    g = torch.cuda.CUDAGraph()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        step()                                  # first call outside the capture (one-time occupancy queries)
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g, stream=s):
+            step()
+    torch.cuda.synchronize()
+    for _ in range(3):
+        mask.zero_(); clean.zero_(); counts.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(_n(mask), o["mask"]) and np.array_equal(_n(clean), o["clean"])
+        assert np.array_equal(_n(counts), o["counts"])
