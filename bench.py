@@ -150,7 +150,9 @@ def run_reference(args):
     line = dict(impl="reference", metric=METRIC, value=value, unit="frames/s", n_gpus=args.gpus,
                 steps=args.steps, warmup=args.warmup, ms_per_step=per_frame * 1e3,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
-                config=dict(workload=wl["label"], h=h, w=w, niter=params["niter"]),
+                config=dict(workload=wl["label"], h=h, w=w, niter=params["niter"], sigclip=params["sigclip"],
+                            sigfrac=params["sigfrac"], objlim=params["objlim"],
+                            parallelism="rank 0 only (the oracle on the host cores)"),
                 mpix_per_s=value * h * w / 1e6,
                 cpu_baseline=dict(value=value, unit="frames/s", cores=cores, kind="oracle", sample=sample),
                 e2e=dict(value=value, unit="frames/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0))
