@@ -72,7 +72,8 @@ typedef struct lacosmic_params {
  *     S' > sigfrac*sigclip and L+/F > objlim are evaluated only on the pixels with S above the
  *     threshold (S' <= S because med5(S) >= 0), by counting the window elements that satisfy the same
  *     monotone fp32 test (no selection is needed to compare a median with a threshold); from the
- *     second iteration on the dense pass skips row segments farther than 2 px from a rewritten pixel. */
+ *     second iteration on, S and the tests are only recomputed near the pixels the previous replacement
+ *     rewrote (within 2 px for S, within 4 px for the tests). */
 #define LACOSMIC_MODE_LAZY 0
 #define LACOSMIC_MODE_DENSE 1
 
