@@ -325,6 +325,18 @@ def run_cuda(args):
     ms_e2e = timed(step_host, args.steps, max(1, args.warmup // 2))
     same = bool((mask_h.numpy() == res["mask"].cpu().numpy()).all() and
                 (clean_h.numpy() == res["clean"].cpu().numpy()).all())
+    # ---- raw uint16 ingest: the same frame rounded to detector counts, 2 bytes per pixel H2D
+    raw_h = torch.from_numpy(np.clip(np.rint(frame.img), 0, 65535).astype(np.uint16)).pin_memory()
+
+    def step_host_u16():
+        lc.lacosmic_run_host(raw_h, P[main_mode], mask_out_host=mask_h, clean_out_host=clean_h, dev_workspace=hws)
+    ms_u16 = timed(step_host_u16, max(3, args.steps // 2), 1)
+    e2e_u16 = dict(value=world * 1e3 / ms_u16, unit="frames/s", ms_per_step=ms_u16, h2d_bytes_per_step=npx * 2,
+                   d2h_bytes_per_step=npx * 5, call="lacosmic_run_host_u16 (pinned host buffers, uint16 input)",
+                   note="input = the bench frame rounded to uint16 counts: a different input, reported beside e2e")
+    step_host()                                  # leave the fp32 results in mask_h / clean_h for the checks below
+    torch.cuda.synchronize()
+
     # ---- end to end on a stream of frames: lacosmic_run_host_batch overlaps the H2D copy of one frame, the
     # kernels of another and the D2H copy of a third
     e2e_stream = None
@@ -428,7 +440,7 @@ def run_cuda(args):
         ref_comparisons_T_per_s=ref_cmp_rate,
         other_mode=dict(mode=other_mode, same_mask_clean_counts=modes_agree, roofline=roofline(res_other),
                         **summarise(res_other)),
-        stream=stream_res, e2e_stream=e2e_stream, gain_estimation=gain_est,
+        stream=stream_res, e2e_stream=e2e_stream, e2e_u16=e2e_u16, gain_estimation=gain_est,
         new_cr_per_iteration=res["counts"], mask_fraction=mask_frac,
         clocks=clocks, cpu_baseline=cpu,
         context="paper (PAPER.md:31,47): 55 s/frame dfcosmic C++ at 2 threads on AWS; GPU variant on an "

@@ -141,6 +141,14 @@ int lacosmic_run_host(const float *img_host, int h, int w, const lacosmic_params
                       uint8_t *mask_out_host, float *clean_out_host, void *dev_workspace,
                       size_t dev_workspace_bytes, void *stream);
 
+/* Raw-frame ingest: as lacosmic_run_host, but the input is the detector's uint16 frame
+ * (ADU counts, row-major [h][w], 2-byte aligned); it is copied as 2 bytes per pixel and widened to fp32 on
+ * the device (exact: every uint16 is an fp32 value), which halves the host-to-device traffic.  The result
+ * equals lacosmic_run_host on the widened frame.  dev_workspace as for lacosmic_run_host. */
+int lacosmic_run_host_u16(const uint16_t *img_host, int h, int w, const lacosmic_params *p,
+                          uint8_t *mask_out_host, float *clean_out_host, void *dev_workspace,
+                          size_t dev_workspace_bytes, void *stream);
+
 /* Stream of n independent frames in HOST buffers (a nightly pipeline
  * of >1000 frames per 15 minutes).  imgs_host/masks_host/cleans_host are [n][h][w] host arrays (pinned
  * memory makes the copies asynchronous and lets them overlap), params a host array of n structs.  Frame f

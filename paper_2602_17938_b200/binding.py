@@ -18,7 +18,7 @@ _lib = None
 EXPORTS = (
     "lacosmic_run", "lacosmic_workspace_bytes", "lacosmic_run_ws", "lacosmic_run_batch",
     "lacosmic_batch_workspace_bytes", "lacosmic_host_batch_workspace_bytes", "lacosmic_run_host_batch",
-    "lacosmic_host_workspace_bytes", "lacosmic_run_host", "lacosmic_estimate_gain", "lacosmic_lplus",
+    "lacosmic_host_workspace_bytes", "lacosmic_run_host", "lacosmic_run_host_u16", "lacosmic_estimate_gain", "lacosmic_lplus",
     "lacosmic_medfilt",
     "lacosmic_bitplane_pitch_words", "lacosmic_pack_bits", "lacosmic_unpack_bits",
     "lacosmic_dilate3", "lacosmic_masked_median", "lacosmic_strerror",
@@ -96,6 +96,7 @@ def load_library():
         "lacosmic_run_batch": (i, [vp, i, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp, vp]),
         "lacosmic_host_workspace_bytes": (sz, [i, i]),
         "lacosmic_run_host": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp]),
+        "lacosmic_run_host_u16": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp]),
         "lacosmic_estimate_gain": (i, [vp, i, i, vp, vp, vp, sz, vp]),
         "lacosmic_lplus": (i, [vp, vp, i, i, vp]),
         "lacosmic_medfilt": (i, [vp, vp, i, i, i, vp]),
@@ -269,13 +270,14 @@ def lacosmic_run_batch(imgs, params, masks_out=None, cleans_out=None, workspace=
 
 def lacosmic_run_host(img_host, params=None, mask_out_host=None, clean_out_host=None,
                       dev_workspace=None, device="cuda:0", stream=None, **kw):
-    """End-to-end call with HOST (ideally pinned) torch CPU tensors; copies are part of the call."""
+    """End-to-end call with HOST (ideally pinned) torch CPU tensors; copies are part of the call.  img_host is
+    float32, or uint16 (the detector's raw counts: copied as 2 bytes per pixel, widened on the device)."""
     torch = _torch()
     L = load_library()
     p = _params(params, **kw)
-    for t, dt, nm in ((img_host, torch.float32, "img_host"),):
-        if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != dt or not t.is_contiguous():
-            raise TypeError("%s must be a contiguous CPU %s tensor" % (nm, dt))
+    if (not isinstance(img_host, torch.Tensor) or img_host.is_cuda or not img_host.is_contiguous()
+            or img_host.dtype not in (torch.float32, torch.uint16)):
+        raise TypeError("img_host must be a contiguous CPU float32 or uint16 tensor")
     h, w = img_host.shape
     if mask_out_host is None:
         mask_out_host = torch.empty((h, w), dtype=torch.uint8).pin_memory()
@@ -284,9 +286,10 @@ def lacosmic_run_host(img_host, params=None, mask_out_host=None, clean_out_host=
     if dev_workspace is None:
         dev_workspace = _workspace(h, w, device, host=True)
     cp = p._c()
-    rc = L.lacosmic_run_host(img_host.data_ptr(), h, w, C.byref(cp), mask_out_host.data_ptr(),
-                             clean_out_host.data_ptr(), _dev(dev_workspace, torch.uint8, "dev_workspace"),
-                             dev_workspace.numel(), _stream(stream))
+    fn = L.lacosmic_run_host_u16 if img_host.dtype == torch.uint16 else L.lacosmic_run_host
+    rc = fn(img_host.data_ptr(), h, w, C.byref(cp), mask_out_host.data_ptr(),
+            clean_out_host.data_ptr(), _dev(dev_workspace, torch.uint8, "dev_workspace"),
+            dev_workspace.numel(), _stream(stream))
     _check(rc, "lacosmic_run_host")
     return dict(mask=mask_out_host, clean=clean_out_host)
 

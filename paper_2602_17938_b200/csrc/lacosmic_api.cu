@@ -541,8 +541,27 @@ size_t lacosmic_host_workspace_bytes(int h, int w) {
 }
 
 namespace {
+// uint16 -> fp32 (exact), 8 pixels per thread; src and dst must not overlap
+__global__ void __launch_bounds__(256) k_u16_to_f32(const uint16_t* __restrict__ src, float* __restrict__ dst, size_t n) {
+    const size_t i = ((size_t)blockIdx.x * 256 + threadIdx.x) * 8;
+    if (i + 8 <= n) {
+        const uint4 q = __ldg(reinterpret_cast<const uint4*>(src + i));
+        const uint32_t v[4] = {q.x, q.y, q.z, q.w};
+        float o[8];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            o[2 * k] = (float)(v[k] & 0xffffu);
+            o[2 * k + 1] = (float)(v[k] >> 16);
+        }
+        *reinterpret_cast<float4*>(dst + i) = make_float4(o[0], o[1], o[2], o[3]);
+        *reinterpret_cast<float4*>(dst + i + 4) = make_float4(o[4], o[5], o[6], o[7]);
+    } else {
+        for (size_t k = i; k < n; ++k) dst[k] = (float)src[k];
+    }
+}
+
 // one frame through a staging slot: H2D, the path, D2H (slot layout: img | clean | mask | workspace)
-int run_host_frame(const float* img_host, int h, int w, const lacosmic_params& p, uint8_t* mask_out_host,
+int run_host_frame(const void* img_host, bool u16, int h, int w, const lacosmic_params& p, uint8_t* mask_out_host,
                    float* clean_out_host, void* slot, cudaStream_t st) {
     size_t P = (size_t)h * w, plane = align_up(P * 4, 256);
     char* base = (char*)slot;
@@ -550,7 +569,15 @@ int run_host_frame(const float* img_host, int h, int w, const lacosmic_params& p
     float* d_clean = (float*)(base + plane);
     uint8_t* d_mask = (uint8_t*)(base + 2 * plane);
     void* ws = base + 2 * plane + align_up(P, 256);
-    CK(cudaMemcpyAsync(d_img, img_host, P * 4, cudaMemcpyHostToDevice, st));
+    if (u16) {
+        // the raw frame is staged in the mask slot's neighbour: the clean plane is dead until the path starts
+        uint16_t* d_raw = (uint16_t*)d_clean;
+        CK(cudaMemcpyAsync(d_raw, img_host, P * 2, cudaMemcpyHostToDevice, st));
+        k_u16_to_f32<<<(unsigned)((P + 2047) / 2048), 256, 0, st>>>(d_raw, d_img, P);
+        LAUNCHED();
+    } else {
+        CK(cudaMemcpyAsync(d_img, img_host, P * 4, cudaMemcpyHostToDevice, st));
+    }
     int rc = run_frame(d_img, h, w, p, d_mask, d_clean, carve(ws, h, w), nullptr, nullptr, st);
     if (rc) return rc;
     CK(cudaMemcpyAsync(clean_out_host, d_clean, P * 4, cudaMemcpyDeviceToHost, st));
@@ -569,7 +596,20 @@ int lacosmic_run_host(const float* img_host, int h, int w, const lacosmic_params
     if ((rc = check_params(*p))) return rc;
     if ((uintptr_t)dev_workspace & 255) return LACOSMIC_ERR_ALIGN;
     if (dev_workspace_bytes < lacosmic_host_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
-    return run_host_frame(img_host, h, w, *p, mask_out_host, clean_out_host, dev_workspace, (cudaStream_t)stream);
+    return run_host_frame(img_host, false, h, w, *p, mask_out_host, clean_out_host, dev_workspace, (cudaStream_t)stream);
+}
+
+int lacosmic_run_host_u16(const uint16_t* img_host, int h, int w, const lacosmic_params* p,
+                          uint8_t* mask_out_host, float* clean_out_host, void* dev_workspace,
+                          size_t dev_workspace_bytes, void* stream) {
+    g_launches = 0;
+    if (!img_host || !p || !mask_out_host || !clean_out_host || !dev_workspace) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    if ((rc = check_params(*p))) return rc;
+    if (((uintptr_t)dev_workspace & 255) || ((uintptr_t)img_host & 1)) return LACOSMIC_ERR_ALIGN;
+    if (dev_workspace_bytes < lacosmic_host_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
+    return run_host_frame(img_host, true, h, w, *p, mask_out_host, clean_out_host, dev_workspace, (cudaStream_t)stream);
 }
 
 size_t lacosmic_host_batch_workspace_bytes(int h, int w, int concurrency) {
@@ -603,7 +643,7 @@ int lacosmic_run_host_batch(const float* imgs_host, int n, int h, int w, const l
     }
     for (int f = 0; f < n; ++f) {
         const int s = f % k;
-        rc = run_host_frame(imgs_host + f * P, h, w, params[f], masks_host + f * P, cleans_host + f * P,
+        rc = run_host_frame(imgs_host + f * P, false, h, w, params[f], masks_host + f * P, cleans_host + f * P,
                             (char*)dev_workspace + (size_t)s * slot, k > 1 ? bs->st[s] : caller);
         if (rc) break;
     }

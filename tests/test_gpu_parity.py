@@ -258,6 +258,20 @@ def test_batch_with_per_frame_parameters(lc, orc, concurrency):
         assert np.array_equal(_n(g["counts"][j])[:ps[j]["niter"]], o["counts"]), j
 
 
+@pytest.mark.parametrize("shape", [(120, 200), (77, 131), (1, 1), (3, 5)])
+def test_host_u16_ingest(lc, orc, shape):
+    """lacosmic_run_host_u16: the raw uint16 frame is copied as 2 bytes per pixel and widened on the device
+    (exact); the result equals the oracle on the widened frame."""
+    import torch
+    h, w = shape
+    f = synth.make_frame(h, w, seed=55, n_star=max(1, h * w // 3000), n_cr=max(1, h * w // 300), sp_frac=0.004)
+    raw = np.clip(np.rint(f.img), 0, 65535).astype(np.uint16)
+    o = orc.run(raw.astype(np.float32), **PARAMS)
+    r = lc.lacosmic_run_host(torch.from_numpy(raw).pin_memory(), lc.Params(**PARAMS))
+    torch.cuda.synchronize()
+    assert np.array_equal(r["mask"].numpy(), o["mask"]) and np.array_equal(r["clean"].numpy(), o["clean"])
+
+
 @pytest.mark.parametrize("concurrency", [1, 3])
 def test_host_batch_pipeline(lc, orc, concurrency):
     """lacosmic_run_host_batch: frames in pinned host memory, H2D / kernels / D2H of different frames
