@@ -334,6 +334,22 @@ def run_cuda(args):
     e2e_u16 = dict(value=world * 1e3 / ms_u16, unit="frames/s", ms_per_step=ms_u16, h2d_bytes_per_step=npx * 2,
                    d2h_bytes_per_step=npx * 5, call="lacosmic_run_host_u16 (pinned host buffers, uint16 input)",
                    note="input = the bench frame rounded to uint16 counts: a different input, reported beside e2e")
+    # ---- sparse results: bit-plane mask + list of replaced pixels instead of the two full planes over PCIe
+    sp_out = lc.lacosmic_run_host_sparse(img_h, P[main_mode], capacity=npx // 32, dev_workspace=hws)
+    torch.cuda.synchronize()
+
+    def step_host_sparse():
+        lc.lacosmic_run_host_sparse(img_h, P[main_mode], out=sp_out, dev_workspace=hws)
+    ms_sp = timed(step_host_sparse, max(3, args.steps // 2), 1)
+    nsp = int(sp_out["count"][0])
+    sp_idx = sp_out["idx"].numpy()[:nsp]
+    sp_ok = bool(nsp == int(res["mask"].sum().item()) and nsp <= sp_out["capacity"] and
+                 (sp_out["val"].numpy()[:nsp] == res["clean"].cpu().numpy().ravel()[sp_idx]).all())
+    e2e_sparse = dict(value=world * 1e3 / ms_sp, unit="frames/s", ms_per_step=ms_sp, h2d_bytes_per_step=npx * 4,
+                      d2h_bytes_per_step=int(sp_out["maskbits"].numel() * 4 + 8 * sp_out["capacity"] + 4),
+                      flagged=nsp, capacity=int(sp_out["capacity"]), matches_device_path=sp_ok,
+                      call="lacosmic_run_host_sparse (pinned host buffers; outputs: bit-plane mask + ascending "
+                           "list of flagged pixels with their replacement values)")
     step_host()                                  # leave the fp32 results in mask_h / clean_h for the checks below
     torch.cuda.synchronize()
 
@@ -440,7 +456,7 @@ def run_cuda(args):
         ref_comparisons_T_per_s=ref_cmp_rate,
         other_mode=dict(mode=other_mode, same_mask_clean_counts=modes_agree, roofline=roofline(res_other),
                         **summarise(res_other)),
-        stream=stream_res, e2e_stream=e2e_stream, e2e_u16=e2e_u16, gain_estimation=gain_est,
+        stream=stream_res, e2e_stream=e2e_stream, e2e_u16=e2e_u16, e2e_sparse=e2e_sparse, gain_estimation=gain_est,
         new_cr_per_iteration=res["counts"], mask_fraction=mask_frac,
         clocks=clocks, cpu_baseline=cpu,
         context="paper (PAPER.md:31,47): 55 s/frame dfcosmic C++ at 2 threads on AWS; GPU variant on an "

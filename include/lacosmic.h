@@ -149,6 +149,20 @@ int lacosmic_run_host_u16(const uint16_t *img_host, int h, int w, const lacosmic
                           uint8_t *mask_out_host, float *clean_out_host, void *dev_workspace,
                           size_t dev_workspace_bytes, void *stream);
 
+/* Sparse results for a pipeline that keeps the input frame on the host: the cleaned
+ * frame equals the input outside the mask, so instead of the two full planes (5 bytes per pixel over PCIe)
+ * the call returns the final mask as a bit-plane (maskbits_host: [h][lacosmic_bitplane_pitch_words(w)] words,
+ * bit k of word j of a row = pixel 32 j + k) and the flagged pixels as a list in ascending flat-index order:
+ * idx_host[i] = y*w + x, val_host[i] = the replacement value, for i < min(*count_host, capacity);
+ * *count_host is the number of flagged pixels (a value above `capacity` means the list was truncated).
+ * `capacity` entries of idx/val are copied whatever the count (no host synchronisation inside the call), so
+ * size it to the expected mask fraction.  All four outputs are HOST pointers; dev_workspace as for
+ * lacosmic_run_host.  clean[idx[i]] = val[i] applied to a copy of the input reproduces lacosmic_run_host. */
+int lacosmic_run_host_sparse(const float *img_host, int h, int w, const lacosmic_params *p,
+                             uint32_t *maskbits_host, int32_t *idx_host, float *val_host,
+                             int32_t *count_host, int capacity, void *dev_workspace,
+                             size_t dev_workspace_bytes, void *stream);
+
 /* Stream of n independent frames in HOST buffers (a nightly pipeline
  * of >1000 frames per 15 minutes).  imgs_host/masks_host/cleans_host are [n][h][w] host arrays (pinned
  * memory makes the copies asynchronous and lets them overlap), params a host array of n structs.  Frame f

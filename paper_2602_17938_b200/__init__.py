@@ -32,6 +32,7 @@ from .binding import (  # noqa: F401
     lacosmic_batch_workspace_bytes,
     lacosmic_host_batch_workspace_bytes,
     lacosmic_run_host_batch,
+    lacosmic_run_host_sparse,
     library_path,
     load_library,
 )

@@ -18,7 +18,7 @@ _lib = None
 EXPORTS = (
     "lacosmic_run", "lacosmic_workspace_bytes", "lacosmic_run_ws", "lacosmic_run_batch",
     "lacosmic_batch_workspace_bytes", "lacosmic_host_batch_workspace_bytes", "lacosmic_run_host_batch",
-    "lacosmic_host_workspace_bytes", "lacosmic_run_host", "lacosmic_run_host_u16", "lacosmic_estimate_gain", "lacosmic_lplus",
+    "lacosmic_host_workspace_bytes", "lacosmic_run_host", "lacosmic_run_host_u16", "lacosmic_run_host_sparse", "lacosmic_estimate_gain", "lacosmic_lplus",
     "lacosmic_medfilt",
     "lacosmic_bitplane_pitch_words", "lacosmic_pack_bits", "lacosmic_unpack_bits",
     "lacosmic_dilate3", "lacosmic_masked_median", "lacosmic_strerror",
@@ -97,6 +97,7 @@ def load_library():
         "lacosmic_host_workspace_bytes": (sz, [i, i]),
         "lacosmic_run_host": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp]),
         "lacosmic_run_host_u16": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp]),
+        "lacosmic_run_host_sparse": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, vp, i, vp, sz, vp]),
         "lacosmic_estimate_gain": (i, [vp, i, i, vp, vp, vp, sz, vp]),
         "lacosmic_lplus": (i, [vp, vp, i, i, vp]),
         "lacosmic_medfilt": (i, [vp, vp, i, i, i, vp]),
@@ -292,6 +293,36 @@ def lacosmic_run_host(img_host, params=None, mask_out_host=None, clean_out_host=
             dev_workspace.numel(), _stream(stream))
     _check(rc, "lacosmic_run_host")
     return dict(mask=mask_out_host, clean=clean_out_host)
+
+
+def lacosmic_run_host_sparse(img_host, params=None, capacity=None, out=None, dev_workspace=None,
+                             device="cuda:0", stream=None, **kw):
+    """Sparse results (host tensors): dict(maskbits int32 [h][pitch], idx int32 [capacity], val float32
+    [capacity], count int32 [1]).  capacity defaults to 1/16 of the frame.  Pass `out` (a previous result) to
+    reuse its pinned buffers."""
+    torch = _torch()
+    L = load_library()
+    p = _params(params, **kw)
+    if (not isinstance(img_host, torch.Tensor) or img_host.is_cuda or not img_host.is_contiguous()
+            or img_host.dtype != torch.float32):
+        raise TypeError("img_host must be a contiguous CPU float32 tensor")
+    h, w = img_host.shape
+    pitch = lacosmic_bitplane_pitch_words(w)
+    if out is None:
+        cap = int(capacity) if capacity is not None else max(1, (h * w) // 16)
+        out = dict(maskbits=torch.empty((h, pitch), dtype=torch.int32).pin_memory(),
+                   idx=torch.empty(max(cap, 1), dtype=torch.int32).pin_memory(),
+                   val=torch.empty(max(cap, 1), dtype=torch.float32).pin_memory(),
+                   count=torch.zeros(1, dtype=torch.int32).pin_memory(), capacity=cap)
+    if dev_workspace is None:
+        dev_workspace = _workspace(h, w, device, host=True)
+    cp = p._c()
+    rc = L.lacosmic_run_host_sparse(img_host.data_ptr(), h, w, C.byref(cp), out["maskbits"].data_ptr(),
+                                    out["idx"].data_ptr(), out["val"].data_ptr(), out["count"].data_ptr(),
+                                    int(out["capacity"]), _dev(dev_workspace, torch.uint8, "dev_workspace"),
+                                    dev_workspace.numel(), _stream(stream))
+    _check(rc, "lacosmic_run_host_sparse")
+    return out
 
 
 def lacosmic_host_batch_workspace_bytes(h, w, concurrency):

@@ -10,6 +10,7 @@
 #include "lazy.cuh"
 #include "grow.cuh"
 #include "select.cuh"
+#include "compact.cuh"
 
 namespace {
 
@@ -375,7 +376,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                 if (pl.o && (rc = unpack(pl.b, pl.o, h, w, st))) return rc;
         }
     }
-    int rc = unpack(ws.C[p.niter & 1], mask_out, h, w, st);
+    int rc = mask_out ? unpack(ws.C[p.niter & 1], mask_out, h, w, st) : LACOSMIC_OK;   // null: the caller reads the bit-plane
     if (rc) return rc;
     if (iter_counts && p.niter > 0)
         CK(cudaMemcpyAsync(iter_counts, ws.counts, (size_t)p.niter * 4, cudaMemcpyDeviceToDevice, st));
@@ -610,6 +611,48 @@ int lacosmic_run_host_u16(const uint16_t* img_host, int h, int w, const lacosmic
     if (((uintptr_t)dev_workspace & 255) || ((uintptr_t)img_host & 1)) return LACOSMIC_ERR_ALIGN;
     if (dev_workspace_bytes < lacosmic_host_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
     return run_host_frame(img_host, true, h, w, *p, mask_out_host, clean_out_host, dev_workspace, (cudaStream_t)stream);
+}
+
+int lacosmic_run_host_sparse(const float* img_host, int h, int w, const lacosmic_params* p,
+                             uint32_t* maskbits_host, int32_t* idx_host, float* val_host, int32_t* count_host,
+                             int capacity, void* dev_workspace, size_t dev_workspace_bytes, void* stream) {
+    g_launches = 0;
+    if (!img_host || !p || !maskbits_host || !idx_host || !val_host || !count_host || !dev_workspace)
+        return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    if ((rc = check_params(*p))) return rc;
+    if (capacity < 0) return LACOSMIC_ERR_PARAM;
+    if ((uintptr_t)dev_workspace & 255) return LACOSMIC_ERR_ALIGN;
+    if (dev_workspace_bytes < lacosmic_host_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
+    const size_t P = (size_t)h * w, plane = align_up(P * 4, 256);
+    const int cap = (int)std::min<size_t>((size_t)capacity, P);
+    char* base = (char*)dev_workspace;
+    float* d_img = (float*)base;
+    float* d_clean = (float*)(base + plane);
+    Workspace ws = carve(base + 2 * plane + align_up(P, 256), h, w);
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaMemcpyAsync(d_img, img_host, P * 4, cudaMemcpyHostToDevice, st));
+    if ((rc = run_frame(d_img, h, w, *p, nullptr, d_clean, ws, nullptr, nullptr, st))) return rc;
+    // the S plane, the candidate list and the quad list are dead now: values, indices, block sums
+    const uint32_t* C = ws.C[p->niter & 1];
+    const int wpr = words_per_row(w), nwords = h * wpr;
+    const int nblocks = (nwords + lac::CP_WORDS_PER_CTA - 1) / lac::CP_WORDS_PER_CTA;
+    int* blocksum = ws.qlist;
+    if ((size_t)(nblocks + 1) > (size_t)h * ((w + 3) / 4)) blocksum = (int*)ws.G1;   // tiny frames: any dead plane
+    lac::k_popc_blocks<<<nblocks, 256, 0, st>>>(C, nwords, blocksum);
+    LAUNCHED();
+    lac::k_scan_blocks<<<1, 256, 0, st>>>(blocksum, nblocks);
+    LAUNCHED();
+    lac::k_emit_flagged<<<nblocks, 256, 0, st>>>(C, nwords, blocksum, d_clean, ws.clist, ws.S, cap, w, wpr);
+    LAUNCHED();
+    CK(cudaMemcpyAsync(maskbits_host, C, (size_t)nwords * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(count_host, blocksum + nblocks, 4, cudaMemcpyDeviceToHost, st));
+    if (cap > 0) {
+        CK(cudaMemcpyAsync(idx_host, ws.clist, (size_t)cap * 4, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(val_host, ws.S, (size_t)cap * 4, cudaMemcpyDeviceToHost, st));
+    }
+    return LACOSMIC_OK;
 }
 
 size_t lacosmic_host_batch_workspace_bytes(int h, int w, int concurrency) {

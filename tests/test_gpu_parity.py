@@ -272,6 +272,35 @@ def test_host_u16_ingest(lc, orc, shape):
     assert np.array_equal(r["mask"].numpy(), o["mask"]) and np.array_equal(r["clean"].numpy(), o["clean"])
 
 
+@pytest.mark.parametrize("shape", [(120, 200), (77, 131), (1, 1), (40, 33), (300, 1100)])
+def test_host_sparse_results(lc, orc, shape):
+    """lacosmic_run_host_sparse: bit-plane mask + ascending list of (flat index, replacement value).  Patched
+    into a copy of the input it must reproduce the oracle's cleaned frame; a short list is truncated."""
+    import torch
+    h, w = shape
+    f = synth.make_frame(h, w, seed=56, n_star=max(1, h * w // 3000), n_cr=max(1, h * w // 300), sp_frac=0.004)
+    o = orc.run(f.img, **PARAMS)
+    r = lc.lacosmic_run_host_sparse(torch.from_numpy(f.img).pin_memory(), lc.Params(**PARAMS), capacity=h * w)
+    torch.cuda.synchronize()
+    n = int(r["count"][0])
+    assert n == int(o["mask"].sum())
+    bits = np.unpackbits(r["maskbits"].numpy().view(np.uint8), axis=1, bitorder="little")[:, :w]
+    assert np.array_equal(bits, o["mask"])
+    idx, val = r["idx"].numpy()[:n], r["val"].numpy()[:n]
+    assert np.array_equal(idx, np.flatnonzero(o["mask"]))                  # ascending flat indices
+    clean = f.img.copy()
+    clean.flat[idx] = val
+    assert np.array_equal(clean, o["clean"])
+    if n > 3:
+        r2 = lc.lacosmic_run_host_sparse(torch.from_numpy(f.img).pin_memory(), lc.Params(**PARAMS), capacity=n - 2)
+        torch.cuda.synchronize()
+        assert int(r2["count"][0]) == n                                    # count says the list is short
+        assert np.array_equal(r2["idx"].numpy()[:n - 2], idx[:n - 2])
+    r0 = lc.lacosmic_run_host_sparse(torch.from_numpy(f.img).pin_memory(), lc.Params(**dict(PARAMS, niter=0)))
+    torch.cuda.synchronize()
+    assert int(r0["count"][0]) == 0 and not r0["maskbits"].numpy().any()
+
+
 @pytest.mark.parametrize("concurrency", [1, 3])
 def test_host_batch_pipeline(lc, orc, concurrency):
     """lacosmic_run_host_batch: frames in pinned host memory, H2D / kernels / D2H of different frames
