@@ -5,14 +5,12 @@
 
 namespace lac {
 
-__device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
-
 // #{25 clamped taps v of S around (y, x) : fsub(Sc, v) > thr} for thr = sigclip (c1) and siglow (c2).
 // Plain scalar taps: on B200 they beat covering each window row with aligned 16-byte vectors and selecting
 // the taps by a shift (fewer bytes per lane and no select chains; measured in k_eval_candidates and
 // k_grow_replace).
-__device__ __forceinline__ void count_sp_clamped(const float* __restrict__ S, int y, int x, int h, int w,
-                                                 float sigclip, float siglow, int& c1, int& c2) {
+__device__ __forceinline__ void count_sp(const float* __restrict__ S, int y, int x, int h, int w, float sigclip,
+                                         float siglow, int& c1, int& c2) {
     const float sc = __ldg(S + (size_t)y * w + x);
     int xx[5];
 #pragma unroll
@@ -29,11 +27,6 @@ __device__ __forceinline__ void count_sp_clamped(const float* __restrict__ S, in
             c2 += sp > siglow;
         }
     }
-}
-
-__device__ __forceinline__ void count_sp(const float* __restrict__ S, int y, int x, int h, int w, float sigclip,
-                                         float siglow, int& c1, int& c2) {
-    count_sp_clamped(S, y, x, h, w, sigclip, siglow, c1, c2);
 }
 
 }  // namespace lac
