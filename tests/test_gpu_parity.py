@@ -528,3 +528,40 @@ def test_cuda_graph_capture_and_replay(lc, orc):
         torch.cuda.synchronize()
         assert np.array_equal(_n(mask), o["mask"]) and np.array_equal(_n(clean), o["clean"])
         assert np.array_equal(_n(counts), o["counts"])
+
+
+def test_config3_stream_full_size(lc, orc):
+    """configs[3] at full frame size, shortened to 8 frames (seeds 1000..1007, sigclip cycling 4.0/4.5/5.0 by
+    seed: per-frame parameters): lacosmic_run_batch with 4 frames in flight, in the configuration bench.py's
+    stream leg times.  Frames 0, 3 and 7 are compared with the oracle on nine windows each; every frame must
+    equal the single-frame call and satisfy the size-independent properties."""
+    import torch
+    nf = 8
+    cfg = synth.stream_config(nf)
+    assert len({p["sigclip"] for _, p in cfg}) == 3
+    h, w = cfg[0][0]["h"], cfg[0][0]["w"]
+    imgs = torch.empty((nf, h, w), dtype=torch.float32, device="cuda")
+    host = {}
+    for j, (kw, _) in enumerate(cfg):
+        f = synth.make_frame(**kw)
+        imgs[j].copy_(torch.from_numpy(f.img))
+        if j in (0, 3, 7):
+            host[j] = f.img
+    plist = [lc.Params(**p) for _, p in cfg]
+    g = lc.lacosmic_run_batch(imgs, plist, concurrency=4)
+    torch.cuda.synchronize()
+    for j in range(nf):
+        one = lc.lacosmic_run_ws(imgs[j], plist[j])
+        torch.cuda.synchronize()
+        assert bool(torch.equal(one["mask"], g["mask"][j])) and bool(torch.equal(one["clean"], g["clean"][j])), j
+        assert np.array_equal(_n(one["counts"])[:4], _n(g["counts"][j])[:4]), j
+        assert int(g["counts"][j][:4].sum()) == int(g["mask"][j].sum(dtype=torch.int64)), j
+    for j, img in host.items():
+        p = cfg[j][1]
+        gm, gc = _n(g["mask"][j]), _n(g["clean"][j])
+        for (y0, x0, s) in _windows(h, w):
+            ya, yb, xa, xb = max(y0 - HALO, 0), min(y0 + s + HALO, h), max(x0 - HALO, 0), min(x0 + s + HALO, w)
+            o = orc.run(np.ascontiguousarray(img[ya:yb, xa:xb]), **p)
+            sl = (slice(y0 - ya, y0 - ya + s), slice(x0 - xa, x0 - xa + s))
+            assert np.array_equal(gm[y0:y0 + s, x0:x0 + s], o["mask"][sl]), (j, y0, x0)
+            assert np.array_equal(gc[y0:y0 + s, x0:x0 + s], o["clean"][sl]), (j, y0, x0)
