@@ -121,7 +121,14 @@ struct NoiseArgs {
     float* R;                // nullable (R21): also write r = (work - med5) / sqrt(max(med5, 1e-4)) here, and
                              // store med5 itself in the S plane (k_S_from_m5 turns it into S once the gain is known)
     const float* gain_dev;   // nullable (R21): the gain of this iteration, estimated on the device
+    int* zero_ptr;           // nullable: the frame's counter block, cleared by the first launch of a frame
+    int zero_n;              // (nothing reads or adds to it before the next launch)
 };
+
+__device__ __forceinline__ void zero_counters(const NoiseArgs& a) {
+    if (a.zero_ptr)
+        for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < a.zero_n; i += gridDim.x * blockDim.x) a.zero_ptr[i] = 0;
+}
 
 // gather the 4-bit nibbles of the 8 lanes that share a 32-pixel word
 __device__ __forceinline__ uint32_t nibbles_to_word(uint32_t nib, int lane) {
@@ -192,6 +199,7 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
 __global__ void __launch_bounds__(NT)
 k_noise_S(const float* __restrict__ work, NoiseArgs a, int ntx, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;   // fixed point reached (R17)
+    zero_counters(a);
     __shared__ __align__(16) float sm[NS_ROWS * NS_PITCH];
     const int tid = threadIdx.x;
     const int t = blockIdx.x;
@@ -374,6 +382,7 @@ __global__ void __launch_bounds__(NT, 4)
 k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx, int ntiles,
               const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
+    zero_counters(a);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int TILE_BYTES = NS_ROWS * NS_PITCH * 4;
     auto buf = [&](int st) { return reinterpret_cast<float*>(smem_raw + st * TILE_BYTES); };
@@ -583,7 +592,10 @@ k_dilate3(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, int h, in
 // ------------------------------------------------------------------------------------------------
 // bit-plane <-> uint8 plane
 __global__ void __launch_bounds__(256)
-k_unpack_bits(const uint32_t* __restrict__ bits, uint8_t* __restrict__ u8, int h, int w, int wpr) {
+k_unpack_bits(const uint32_t* __restrict__ bits, uint8_t* __restrict__ u8, int h, int w, int wpr,
+              const int* __restrict__ counts_src, int* __restrict__ counts_dst, int ncounts) {
+    // epilogue of a frame: the per-iteration counts go to the caller's array in the same launch
+    if (counts_dst && blockIdx.x == 0 && (int)threadIdx.x < ncounts) counts_dst[threadIdx.x] = counts_src[threadIdx.x];
     // 16 consecutive bytes of the flat uint8 plane per thread, aligned to 16 bytes of the destination (the
     // first thread starts at the first aligned address); a group may straddle two rows when w % 16 != 0
     const unsigned P = (unsigned)h * (unsigned)w;   // h * w < 2^31 (checked at the boundary): 32-bit index math

@@ -183,10 +183,11 @@ Workspace carve(void* base, int h, int w) {
     return ws;
 }
 
-int unpack(const uint32_t* bits, uint8_t* u8, int h, int w, cudaStream_t st) {
+int unpack(const uint32_t* bits, uint8_t* u8, int h, int w, cudaStream_t st, const int* counts_src = nullptr,
+           int* counts_dst = nullptr, int ncounts = 0) {
     const unsigned g = (unsigned)(((size_t)h * w / 16 + 1 + 255) / 256);   // one thread per aligned 16 bytes (+ head)
     Span sp(KC_BITS, st);
-    lac::k_unpack_bits<<<g, 256, 0, st>>>(bits, u8, h, w, words_per_row(w));
+    lac::k_unpack_bits<<<g, 256, 0, st>>>(bits, u8, h, w, words_per_row(w), counts_src, counts_dst, ncounts);
     LAUNCHED();
     return LACOSMIC_OK;
 }
@@ -258,8 +259,13 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     // O0.  The lazy path fuses work = img_in into its first pass (which then reads img_in itself).
     const bool fused_copy = lazy && p.niter > 0;
     if (!fused_copy) CK(cudaMemcpyAsync(work, img, P * 4, cudaMemcpyDeviceToDevice, st));
-    CK(cudaMemsetAsync(ws.C[0], 0, bp_bytes, st));
-    CK(cudaMemsetAsync((char*)ws.S + ws.zero_off, 0, ws.zero_bytes, st));   // counters
+    // C = 0 and the counter block: cleared by the first kernels of the frame (k_list_candidates clears C in the
+    // lazy path, the first noise pass clears the counters); plain memsets where those kernels do not run
+    const bool fused_zero = p.niter > 0;
+    if (!(lazy && p.niter > 0)) CK(cudaMemsetAsync(ws.C[0], 0, bp_bytes, st));
+    if (!fused_zero) CK(cudaMemsetAsync((char*)ws.S + ws.zero_off, 0, ws.zero_bytes, st));
+    int* const zero_ptr = (int*)((char*)ws.S + ws.zero_off);
+    const int zero_n = (int)(ws.zero_bytes / 4);
     const float siglow = p.sigfrac * p.sigclip;   // R9: one fp32 multiply on the host
     const float rn2 = p.readnoise * p.readnoise;
     lac::GateParams gp{p.sigclip, siglow, p.objlim, p.satlevel};
@@ -304,7 +310,8 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
             // (into the candidate list's storage, which is not in use yet), med5(work) into the S plane and, at
             // t = 0, the work = img_in copy.  The selection leaves the gain in ws.gains[t].
             lac::NoiseArgs ne{ws.S, nullptr, nullptr, nullptr, nullptr, (fused_copy && t == 0) ? work : nullptr,
-                              h, w, wpr, 1.0f, rn2, p.sigclip, siglow, p.satlevel, (float*)ws.clist, nullptr};
+                              h, w, wpr, 1.0f, rn2, p.sigclip, siglow, p.satlevel, (float*)ws.clist, nullptr,
+                              t == 0 ? zero_ptr : nullptr, zero_n};
             if ((rc = noise_pass(ne, src))) return rc;
             if ((rc = sigma_clip_gain((const float*)ws.clist, P, ws, ws.gains + t, nullptr, prev, st))) return rc;
             src = work;
@@ -317,7 +324,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                           lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
                           (fused_copy && t == 0 && !estimate) ? work : nullptr,
                           h, w, wpr, p.gain, rn2, p.sigclip, siglow, p.satlevel, nullptr,
-                          estimate ? ws.gains + t : nullptr};
+                          estimate ? ws.gains + t : nullptr, (t == 0 && !estimate) ? zero_ptr : nullptr, zero_n};
         if (incr) {
             {
                 Span sp(KC_LISTS, st);
@@ -343,7 +350,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
             if (lazy) {
                 Span sp(KC_LISTS, st);
                 lac::k_list_candidates<<<bit_grid(h, w), 256, 0, st>>>(ws.A1, (t > 0 && !estimate) ? ws.NEED : nullptr, ws.G1, ws.G2, ws.G2F, ws.M1,
-                                                                      ws.clist, ws.ncand + t, h, w, wpr, prev);
+                                                                      ws.clist, ws.ncand + t, t == 0 ? ws.C[0] : nullptr, h, w, wpr, prev);
                 LAUNCHED();
             }
         }
@@ -376,9 +383,12 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                 if (pl.o && (rc = unpack(pl.b, pl.o, h, w, st))) return rc;
         }
     }
-    int rc = mask_out ? unpack(ws.C[p.niter & 1], mask_out, h, w, st) : LACOSMIC_OK;   // null: the caller reads the bit-plane
+    const bool want_counts = iter_counts && p.niter > 0;
+    // mask_out null: the caller reads the bit-plane.  The iteration counts ride along with the unpack launch.
+    int rc = mask_out ? unpack(ws.C[p.niter & 1], mask_out, h, w, st, ws.counts, want_counts ? iter_counts : nullptr, p.niter)
+                      : LACOSMIC_OK;
     if (rc) return rc;
-    if (iter_counts && p.niter > 0)
+    if (want_counts && !mask_out)
         CK(cudaMemcpyAsync(iter_counts, ws.counts, (size_t)p.niter * 4, cudaMemcpyDeviceToDevice, st));
     if (dbg && dbg->gains && p.niter > 0) {
         if (!estimate) {

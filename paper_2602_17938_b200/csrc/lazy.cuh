@@ -34,7 +34,7 @@ namespace lac {
 __global__ void __launch_bounds__(256)
 k_list_candidates(const uint32_t* __restrict__ A1, const uint32_t* __restrict__ dirty, uint32_t* __restrict__ G1,
                   uint32_t* __restrict__ G2, uint32_t* __restrict__ G2F, uint32_t* __restrict__ M1, int* __restrict__ list,
-                  int* __restrict__ nlist, int h, int w, int wpr, const int* prev_count) {
+                  int* __restrict__ nlist, uint32_t* __restrict__ Czero, int h, int w, int wpr, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const int wx = blockIdx.x * 32 + lane, y0 = blockIdx.y * BW_CTA_ROWS + wi * BW_ROWS;
@@ -59,6 +59,7 @@ k_list_candidates(const uint32_t* __restrict__ A1, const uint32_t* __restrict__ 
             bits[i] = A1[q] & r;
             if (r == 0xffffffffu) {
                 G1[q] = 0; G2[q] = 0; G2F[q] = 0; M1[q] = 0;
+                if (Czero) Czero[q] = 0;   // frame prologue C = 0, fused (t = 0: every word takes this branch)
             } else {
                 G1[q] &= ~r; G2[q] &= ~r; G2F[q] &= ~r; M1[q] &= ~r;
             }

@@ -6,7 +6,8 @@
 // the value (11 + 11 + 10 bits): every pass histograms one digit of the keys that match the digits already
 // fixed (shared-memory histogram per CTA, flushed with atomics); the CTA that finishes last (atomic ticket)
 // then walks the 2048 counts to the bucket holding the wanted rank, so a pass is one launch.  One round of
-// the clipping is two selections over the kept set K = { lo <= r <= hi }: the centre c (rank (n-1)/2 of r) and the MAD d (same rank of |r - c|).
+// the clipping is two selections over the kept set K = { lo <= r <= hi }: the centre c (rank (n-1)/2 of r)
+// and the MAD d (same rank of |r - c|).
 #pragma once
 #include "common.cuh"
 
