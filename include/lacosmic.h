@@ -78,7 +78,7 @@ typedef struct lacosmic_params {
 #define LACOSMIC_MODE_DENSE 1
 
 /* Optional per-step dump of ONE iteration (used by the parity tests).  Every pointer is a
- * nullable device pointer to a [h][w] plane: fp32 for Lp (step 1), N (2), S, Sp (3), m3, F (4);
+ * nullable device pointer to a [h][w] plane (fp32 planes 16-byte aligned): fp32 for Lp (step 1), N (2), S, Sp (3), m3, F (4);
  * uint8 0/1 for G1 = (S' > sigclip), G2 = (S' > sigfrac*sigclip) (both AND img < satlevel),
  * M1 (step 5), M2, M3 (step 6) and C (cumulative mask after the iteration).  LACOSMIC_MODE_LAZY never
  * forms Sp, m3, F and evaluates G2 only where step (6) reads it: those four planes are left untouched

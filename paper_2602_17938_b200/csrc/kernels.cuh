@@ -65,6 +65,12 @@ __device__ __forceinline__ void store4(float* __restrict__ dst, size_t row_off, 
     }
 }
 
+template <bool ALIGNED>
+__device__ __forceinline__ void store4q(float* __restrict__ dst, size_t row_off, int x, int w, const float (&v)[4]) {
+    if (ALIGNED) *reinterpret_cast<float4*>(dst + row_off + x) = make_float4(v[0], v[1], v[2], v[3]);
+    else store4(dst, row_off, x, w, v);
+}
+
 // ------------------------------------------------------------------------------------------------
 // Standalone k x k median (lacosmic_medfilt): same selection networks and tile shape as the fused
 // kernels.  Each thread produces 4 adjacent outputs from a (k+3) x k register window.
@@ -144,6 +150,8 @@ __device__ __forceinline__ uint32_t nibbles_to_word(uint32_t nib, int lane) {
 constexpr int UW = 32, UH = 4;
 
 // sm: work tile with margins (NS_MX, NS_MY), edge-replicated
+// W4: w % 4 == 0 and 16-byte aligned planes (the TMA path): quads are whole and every store is one vector
+template <bool W4>
 __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a, int x0, int y0, int lane,
                                              int wi) {
     const int lx = lane & 7, lr = lane >> 3;
@@ -164,16 +172,16 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
                 lp[j] = lplus_px(win[2 + j][2], win[2 + j][1], win[2 + j][3], win[1 + j][2], win[3 + j][2]);
                 n[j] = noise_px(m5[j], gain, a.rn2);
                 s[j] = fdiv_nn(lp[j], __fmul_rn(2.0f, n[j]));
-                const bool ok = (x + j < a.w) && (win[2 + j][2] < a.satlevel);            // R12
+                const bool ok = (W4 || x + j < a.w) && (win[2 + j][2] < a.satlevel);            // R12
                 n1 |= (uint32_t)(ok && s[j] > a.sigclip) << j;
                 n2 |= (uint32_t)(ok && s[j] > a.siglow) << j;
             }
             size_t ro = (size_t)y * a.w;
-            if (a.R) store4(a.S, ro, x, a.w, m5);
-            else store4(a.S, ro, x, a.w, s);
-            if (a.dbgLp) store4(a.dbgLp, ro, x, a.w, lp);
-            if (a.dbgN) store4(a.dbgN, ro, x, a.w, n);
-            if (a.copy_out) store4(a.copy_out, ro, x, a.w, ctr);
+            if (a.R) store4q<W4>(a.S, ro, x, a.w, m5);
+            else store4q<W4>(a.S, ro, x, a.w, s);
+            if (a.dbgLp) store4q<W4>(a.dbgLp, ro, x, a.w, lp);
+            if (a.dbgN) store4q<W4>(a.dbgN, ro, x, a.w, n);
+            if (a.copy_out) store4q<W4>(a.copy_out, ro, x, a.w, ctr);
             if (a.R) {   // R21: residual in units of sqrt(signal)
                 float r[4];
 #pragma unroll
@@ -181,7 +189,7 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
                     const float m5c = m5[j] > 1e-4f ? m5[j] : 1e-4f;
                     r[j] = __fdiv_rn(__fsub_rn(ctr[j], m5[j]), __fsqrt_rn(m5c));
                 }
-                store4(a.R, ro, x, a.w, r);
+                store4q<W4>(a.R, ro, x, a.w, r);
             }
         }
         if (a.A1) {
@@ -207,7 +215,7 @@ k_noise_S(const float* __restrict__ work, NoiseArgs a, int ntx, const int* prev_
     const int x0 = tx * TW, y0 = ty * NS_TH;
     load_tile<NS_MX, NS_MY, NS_PITCH, NS_TH>(sm, work, a.h, a.w, y0, x0, tid);
     __syncthreads();
-    noise_S_tile(sm, a, x0, y0, tid & 31, tid >> 5);
+    noise_S_tile<false>(sm, a, x0, y0, tid & 31, tid >> 5);
 }
 
 // K_B: steps (3b)-(5).  S' = S - med5(S); m3 = med3(work) (tile in shared memory, replicated at the
@@ -415,7 +423,7 @@ k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx,
             fence_proxy_async();
             __syncthreads();
         }
-        noise_S_tile(buf(st), a, x0, y0, tid & 31, tid >> 5);
+        noise_S_tile<true>(buf(st), a, x0, y0, tid & 31, tid >> 5);
         __syncthreads();   // stage st is free for the load issued at the top of the next iteration
     }
 }

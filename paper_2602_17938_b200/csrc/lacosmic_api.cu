@@ -459,6 +459,9 @@ int lacosmic_run_ws(const float* img, int h, int w, const lacosmic_params* p, ui
     int rc = check_frame_args(img, h, w, p, mask_out, clean_out, workspace, workspace_bytes);
     if (rc) return rc;
     if (dbg && (dbg->iter < -1 || dbg->iter >= LACOSMIC_MAX_NITER)) return LACOSMIC_ERR_PARAM;
+    if (dbg)   // fp32 debug planes are written with 16-byte vectors
+        for (const float* pl : {dbg->Lp, dbg->N, dbg->S, dbg->Sp, dbg->m3, dbg->F})
+            if ((uintptr_t)pl & 15) return LACOSMIC_ERR_ALIGN;
     return run_frame(img, h, w, *p, mask_out, clean_out, carve(workspace, h, w), iter_counts, dbg,
                      (cudaStream_t)stream);
 }
