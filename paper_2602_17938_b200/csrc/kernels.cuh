@@ -386,7 +386,10 @@ __device__ __forceinline__ void replicate_fix(float* sm, int oy, int ox, int h, 
     }
 }
 
-__global__ void __launch_bounds__(NT, 4)
+#ifndef LAC_NS_MINB
+#define LAC_NS_MINB 4
+#endif
+__global__ void __launch_bounds__(NT, LAC_NS_MINB)
 k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx, int ntiles,
               const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
