@@ -59,11 +59,12 @@ __device__ __forceinline__ float lplus_px(float c, float U, float D, float Lf, f
     return __fmul_rn(__fadd_rn(__fadd_rn(a, b), __fadd_rn(g, d)), 0.25f);
 }
 
-// fdiv(num, den) for num >= +0: the value of __fdiv_rn(num, den), but a zero numerator (about 30 % of the L+
-// values) does not take the division's slow path, which the range check of the fast path (FCHK) sends it to:
-// +0 / den = +0 for every den > 0, infinity included.
+// fdiv(num, den) for num >= +0 and den > 0: the value of __fdiv_rn(num, den), but a zero numerator (about 30 %
+// of the L+ values) does not take the division's slow path, which the range check of the fast path (FCHK)
+// sends it to: +0 / den = +0 for every den > 0, infinity included.  Both callers have den > 0: den = 2N with
+// N >= 1e-2 / sqrt(gain) > 0 for every finite positive gain (med5 is floored at 1e-4, R5), and den = F >= 0.01.
 __device__ __forceinline__ float fdiv_nn(float num, float den) {
-    const bool z = (num == 0.0f) & (den > 0.0f);
+    const bool z = num == 0.0f;
     const float q = __fdiv_rn(z ? 1.0f : num, den);
     return z ? 0.0f : q;
 }
