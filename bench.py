@@ -379,7 +379,28 @@ def run_cuda(args):
                           ms_per_frame=ms_hb / nh, h2d_bytes_per_frame=npx * 4, d2h_bytes_per_frame=npx * 5,
                           matches_single_frame_call=ok_hb,
                           call="lacosmic_run_host_batch (pinned host buffers, %d staging slots)" % kslots)
-        del imgs_h, masks_h, cleans_h, hbws
+        # the production configuration: raw uint16 frames in, sparse results out (2 B/px in, ~0.4 B/px out)
+        del masks_h, cleans_h
+        prod = {}
+        for name, src in (("f32", imgs_h), ("u16", None)):
+            if src is None:
+                src = torch.empty((nh, h, w), dtype=torch.uint16).pin_memory()
+                for j in range(nh):
+                    src[j].copy_(raw_h)
+            sp_stream = lc.lacosmic_run_host_stream_sparse(src, plist_h, capacity=npx // 32, dev_workspace=hbws)
+            torch.cuda.synchronize()
+
+            def step_stream_sparse():
+                lc.lacosmic_run_host_stream_sparse(src, plist_h, out=sp_stream, dev_workspace=hbws)
+            ms_ss = timed(step_stream_sparse, 3, 1)
+            prod[name] = dict(value=world * nh * 1e3 / ms_ss, unit="frames/s", ms_per_frame=ms_ss / nh,
+                              h2d_bytes_per_frame=npx * (4 if name == "f32" else 2),
+                              d2h_bytes_per_frame=int(sp_stream["maskbits"][0].numel() * 4 + 8 * sp_stream["capacity"] + 4),
+                              flagged_per_frame=int(sp_stream["count"][nh - 1]))
+            del sp_stream
+        e2e_stream["sparse_results"] = dict(call="lacosmic_run_host_stream_sparse (%d frames, %d staging slots)" % (nh, kslots),
+                                            **prod)
+        del imgs_h, hbws, src
     clocks = sampler.stop() if rank == 0 else None
 
     if rank != 0:

@@ -163,6 +163,18 @@ int lacosmic_run_host_sparse(const float *img_host, int h, int w, const lacosmic
                              int32_t *count_host, int capacity, void *dev_workspace,
                              size_t dev_workspace_bytes, void *stream);
 
+/* The production configuration of a nightly pipeline: a stream of n raw
+ * frames in, sparse results out.  imgs_host: [n][h][w] fp32 (input_is_u16 = 0) or uint16 (= 1) host frames;
+ * per frame f the call returns maskbits_host[f] ([h][pitch] words), idx_host[f*capacity ...], val_host[f*capacity
+ * ...] and counts_host[f] exactly as lacosmic_run_host_sparse does for one frame.  Frames go through staging
+ * slots on internal streams like lacosmic_run_host_batch (same dev_workspace sizing), so the H2D copy of one
+ * frame overlaps the kernels of another; per frame only 2 or 4 bytes per pixel cross PCIe on the way in and
+ * about 0.4 bytes per pixel on the way out. */
+int lacosmic_run_host_stream_sparse(const void *imgs_host, int input_is_u16, int n, int h, int w,
+                                    const lacosmic_params *params, uint32_t *maskbits_host,
+                                    int32_t *idx_host, float *val_host, int32_t *counts_host, int capacity,
+                                    void *dev_workspace, size_t dev_workspace_bytes, void *stream);
+
 /* Stream of n independent frames in HOST buffers (a nightly pipeline
  * of >1000 frames per 15 minutes).  imgs_host/masks_host/cleans_host are [n][h][w] host arrays (pinned
  * memory makes the copies asynchronous and lets them overlap), params a host array of n structs.  Frame f

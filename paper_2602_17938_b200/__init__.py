@@ -33,6 +33,7 @@ from .binding import (  # noqa: F401
     lacosmic_host_batch_workspace_bytes,
     lacosmic_run_host_batch,
     lacosmic_run_host_sparse,
+    lacosmic_run_host_stream_sparse,
     library_path,
     load_library,
 )

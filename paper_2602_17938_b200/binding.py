@@ -18,7 +18,7 @@ _lib = None
 EXPORTS = (
     "lacosmic_run", "lacosmic_workspace_bytes", "lacosmic_run_ws", "lacosmic_run_batch",
     "lacosmic_batch_workspace_bytes", "lacosmic_host_batch_workspace_bytes", "lacosmic_run_host_batch",
-    "lacosmic_host_workspace_bytes", "lacosmic_run_host", "lacosmic_run_host_u16", "lacosmic_run_host_sparse", "lacosmic_estimate_gain", "lacosmic_lplus",
+    "lacosmic_host_workspace_bytes", "lacosmic_run_host", "lacosmic_run_host_u16", "lacosmic_run_host_sparse", "lacosmic_run_host_stream_sparse", "lacosmic_estimate_gain", "lacosmic_lplus",
     "lacosmic_medfilt",
     "lacosmic_bitplane_pitch_words", "lacosmic_pack_bits", "lacosmic_unpack_bits",
     "lacosmic_dilate3", "lacosmic_masked_median", "lacosmic_strerror",
@@ -98,6 +98,7 @@ def load_library():
         "lacosmic_run_host": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp]),
         "lacosmic_run_host_u16": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp]),
         "lacosmic_run_host_sparse": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, vp, i, vp, sz, vp]),
+        "lacosmic_run_host_stream_sparse": (i, [vp, i, i, i, i, C.POINTER(_CParams), vp, vp, vp, vp, i, vp, sz, vp]),
         "lacosmic_estimate_gain": (i, [vp, i, i, vp, vp, vp, sz, vp]),
         "lacosmic_lplus": (i, [vp, vp, i, i, vp]),
         "lacosmic_medfilt": (i, [vp, vp, i, i, i, vp]),
@@ -322,6 +323,38 @@ def lacosmic_run_host_sparse(img_host, params=None, capacity=None, out=None, dev
                                     int(out["capacity"]), _dev(dev_workspace, torch.uint8, "dev_workspace"),
                                     dev_workspace.numel(), _stream(stream))
     _check(rc, "lacosmic_run_host_sparse")
+    return out
+
+
+def lacosmic_run_host_stream_sparse(imgs_host, params, capacity=None, out=None, dev_workspace=None,
+                                    device="cuda:0", stream=None, concurrency=3):
+    """Stream of host frames [n][h][w] (float32 or uint16), sparse results per frame: dict(maskbits int32
+    [n][h][pitch], idx int32 [n][capacity], val float32 [n][capacity], count int32 [n])."""
+    torch = _torch()
+    L = load_library()
+    if (not isinstance(imgs_host, torch.Tensor) or imgs_host.is_cuda or not imgs_host.is_contiguous()
+            or imgs_host.dim() != 3 or imgs_host.dtype not in (torch.float32, torch.uint16)):
+        raise TypeError("imgs_host must be a contiguous CPU float32 or uint16 tensor [n][h][w]")
+    n, h, w = imgs_host.shape
+    if len(params) != n:
+        raise ValueError("need one Params per frame")
+    arr = (_CParams * max(n, 1))(*[p._c() for p in params])
+    pitch = lacosmic_bitplane_pitch_words(w)
+    if out is None:
+        cap = int(capacity) if capacity is not None else max(1, (h * w) // 16)
+        out = dict(maskbits=torch.empty((n, h, pitch), dtype=torch.int32).pin_memory(),
+                   idx=torch.empty((n, max(cap, 1)), dtype=torch.int32).pin_memory(),
+                   val=torch.empty((n, max(cap, 1)), dtype=torch.float32).pin_memory(),
+                   count=torch.zeros(n, dtype=torch.int32).pin_memory(), capacity=cap)
+    if dev_workspace is None:
+        dev_workspace = torch.empty(max(lacosmic_host_batch_workspace_bytes(h, w, max(1, concurrency)), 256),
+                                    dtype=torch.uint8, device=device)
+    rc = L.lacosmic_run_host_stream_sparse(imgs_host.data_ptr(), int(imgs_host.dtype == torch.uint16), n, h, w, arr,
+                                           out["maskbits"].data_ptr(), out["idx"].data_ptr(), out["val"].data_ptr(),
+                                           out["count"].data_ptr(), int(out["capacity"]),
+                                           _dev(dev_workspace, torch.uint8, "dev_workspace"), dev_workspace.numel(),
+                                           _stream(stream))
+    _check(rc, "lacosmic_run_host_stream_sparse")
     return out
 
 

@@ -554,6 +554,7 @@ size_t lacosmic_host_workspace_bytes(int h, int w) {
     return align_up(P * 4, 256) * 2 + align_up(P, 256) + lacosmic_workspace_bytes(h, w);
 }
 
+extern "C++" {
 namespace {
 // uint16 -> fp32 (exact), 8 pixels per thread; src and dst must not overlap
 __global__ void __launch_bounds__(256) k_u16_to_f32(const uint16_t* __restrict__ src, float* __restrict__ dst, size_t n) {
@@ -574,31 +575,98 @@ __global__ void __launch_bounds__(256) k_u16_to_f32(const uint16_t* __restrict__
     }
 }
 
+// Host-side description of one frame: fp32 or uint16 input; dense results (mask + clean planes) or sparse
+// results (bit-plane mask, ascending list of flagged pixels with their replacement values, count).
+struct HostFrame {
+    const void* img;
+    bool u16;
+    uint8_t* mask;       // dense results (null: sparse)
+    float* clean;
+    uint32_t* maskbits;  // sparse results
+    int32_t* idx;
+    float* val;
+    int32_t* count;
+    int cap;
+};
+
 // one frame through a staging slot: H2D, the path, D2H (slot layout: img | clean | mask | workspace)
-int run_host_frame(const void* img_host, bool u16, int h, int w, const lacosmic_params& p, uint8_t* mask_out_host,
-                   float* clean_out_host, void* slot, cudaStream_t st) {
+int run_host_frame(const HostFrame& io, int h, int w, const lacosmic_params& p, void* slot, cudaStream_t st) {
     size_t P = (size_t)h * w, plane = align_up(P * 4, 256);
     char* base = (char*)slot;
     float* d_img = (float*)base;
     float* d_clean = (float*)(base + plane);
     uint8_t* d_mask = (uint8_t*)(base + 2 * plane);
-    void* ws = base + 2 * plane + align_up(P, 256);
-    if (u16) {
-        // the raw frame is staged in the mask slot's neighbour: the clean plane is dead until the path starts
+    Workspace ws = carve(base + 2 * plane + align_up(P, 256), h, w);
+    if (io.u16) {
+        // the raw frame is staged in the clean plane, which is dead until the path starts
         uint16_t* d_raw = (uint16_t*)d_clean;
-        CK(cudaMemcpyAsync(d_raw, img_host, P * 2, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(d_raw, io.img, P * 2, cudaMemcpyHostToDevice, st));
         k_u16_to_f32<<<(unsigned)((P + 2047) / 2048), 256, 0, st>>>(d_raw, d_img, P);
         LAUNCHED();
     } else {
-        CK(cudaMemcpyAsync(d_img, img_host, P * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(d_img, io.img, P * 4, cudaMemcpyHostToDevice, st));
     }
-    int rc = run_frame(d_img, h, w, p, d_mask, d_clean, carve(ws, h, w), nullptr, nullptr, st);
+    int rc = run_frame(d_img, h, w, p, io.mask ? d_mask : nullptr, d_clean, ws, nullptr, nullptr, st);
     if (rc) return rc;
-    CK(cudaMemcpyAsync(clean_out_host, d_clean, P * 4, cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(mask_out_host, d_mask, P, cudaMemcpyDeviceToHost, st));
+    if (io.mask) {
+        CK(cudaMemcpyAsync(io.clean, d_clean, P * 4, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(io.mask, d_mask, P, cudaMemcpyDeviceToHost, st));
+        return LACOSMIC_OK;
+    }
+    // sparse results.  The S plane, the candidate list and the quad list are dead now: values, indices, block sums
+    const int cap = (int)std::min<size_t>((size_t)io.cap, P);
+    const uint32_t* C = ws.C[p.niter & 1];
+    const int wpr = words_per_row(w), nwords = h * wpr;
+    const int nblocks = (nwords + lac::CP_WORDS_PER_CTA - 1) / lac::CP_WORDS_PER_CTA;
+    int* blocksum = ws.qlist;
+    if ((size_t)(nblocks + 1) > (size_t)h * ((w + 3) / 4)) blocksum = (int*)ws.G1;   // tiny frames: any dead plane
+    lac::k_popc_blocks<<<nblocks, 256, 0, st>>>(C, nwords, blocksum);
+    LAUNCHED();
+    lac::k_scan_blocks<<<1, 256, 0, st>>>(blocksum, nblocks);
+    LAUNCHED();
+    lac::k_emit_flagged<<<nblocks, 256, 0, st>>>(C, nwords, blocksum, d_clean, ws.clist, ws.S, cap, w, wpr);
+    LAUNCHED();
+    CK(cudaMemcpyAsync(io.maskbits, C, (size_t)nwords * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(io.count, blocksum + nblocks, 4, cudaMemcpyDeviceToHost, st));
+    if (cap > 0) {
+        CK(cudaMemcpyAsync(io.idx, ws.clist, (size_t)cap * 4, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(io.val, ws.S, (size_t)cap * 4, cudaMemcpyDeviceToHost, st));
+    }
     return LACOSMIC_OK;
 }
+
+// n host frames through k staging slots on the internal streams (fork / join around the caller's stream)
+template <class FrameOf>
+int run_host_stream(int n, int h, int w, const lacosmic_params* params, void* dev_workspace, size_t dev_workspace_bytes,
+                    cudaStream_t caller, FrameOf frame_of) {
+    const size_t slot = align_up(lacosmic_host_workspace_bytes(h, w), 256);
+    const int k = (int)std::min<size_t>(std::min(n, LACOSMIC_MAX_BATCH_STREAMS), dev_workspace_bytes / slot);
+    if (k < 1) return LACOSMIC_ERR_WORKSPACE;
+    BatchStreams* bs = nullptr;
+    if (k > 1) {
+        bs = batch_streams();
+        if (!bs) return LACOSMIC_ERR_CUDA;
+        CK(cudaEventRecord(bs->fork, caller));
+        for (int s = 0; s < k; ++s) CK(cudaStreamWaitEvent(bs->st[s], bs->fork, 0));
+    }
+    int rc = LACOSMIC_OK;
+    for (int f = 0; f < n; ++f) {
+        const int s = f % k;
+        rc = run_host_frame(frame_of(f), h, w, params[f], (char*)dev_workspace + (size_t)s * slot,
+                            k > 1 ? bs->st[s] : caller);
+        if (rc) break;
+    }
+    if (k > 1) {   // join, also after an error
+        for (int s = 0; s < k; ++s) {
+            if (!cuda_ok(cudaEventRecord(bs->join[s], bs->st[s])) ||
+                !cuda_ok(cudaStreamWaitEvent(caller, bs->join[s], 0)))
+                rc = rc ? rc : LACOSMIC_ERR_CUDA;
+        }
+    }
+    return rc;
+}
 }  // namespace
+}  // extern "C++"
 
 int lacosmic_run_host(const float* img_host, int h, int w, const lacosmic_params* p,
                       uint8_t* mask_out_host, float* clean_out_host, void* dev_workspace,
@@ -610,7 +678,8 @@ int lacosmic_run_host(const float* img_host, int h, int w, const lacosmic_params
     if ((rc = check_params(*p))) return rc;
     if ((uintptr_t)dev_workspace & 255) return LACOSMIC_ERR_ALIGN;
     if (dev_workspace_bytes < lacosmic_host_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
-    return run_host_frame(img_host, false, h, w, *p, mask_out_host, clean_out_host, dev_workspace, (cudaStream_t)stream);
+    return run_host_frame(HostFrame{img_host, false, mask_out_host, clean_out_host, nullptr, nullptr, nullptr, nullptr, 0},
+                          h, w, *p, dev_workspace, (cudaStream_t)stream);
 }
 
 int lacosmic_run_host_u16(const uint16_t* img_host, int h, int w, const lacosmic_params* p,
@@ -623,7 +692,8 @@ int lacosmic_run_host_u16(const uint16_t* img_host, int h, int w, const lacosmic
     if ((rc = check_params(*p))) return rc;
     if (((uintptr_t)dev_workspace & 255) || ((uintptr_t)img_host & 1)) return LACOSMIC_ERR_ALIGN;
     if (dev_workspace_bytes < lacosmic_host_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
-    return run_host_frame(img_host, true, h, w, *p, mask_out_host, clean_out_host, dev_workspace, (cudaStream_t)stream);
+    return run_host_frame(HostFrame{img_host, true, mask_out_host, clean_out_host, nullptr, nullptr, nullptr, nullptr, 0},
+                          h, w, *p, dev_workspace, (cudaStream_t)stream);
 }
 
 int lacosmic_run_host_sparse(const float* img_host, int h, int w, const lacosmic_params* p,
@@ -638,34 +708,32 @@ int lacosmic_run_host_sparse(const float* img_host, int h, int w, const lacosmic
     if (capacity < 0) return LACOSMIC_ERR_PARAM;
     if ((uintptr_t)dev_workspace & 255) return LACOSMIC_ERR_ALIGN;
     if (dev_workspace_bytes < lacosmic_host_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
-    const size_t P = (size_t)h * w, plane = align_up(P * 4, 256);
-    const int cap = (int)std::min<size_t>((size_t)capacity, P);
-    char* base = (char*)dev_workspace;
-    float* d_img = (float*)base;
-    float* d_clean = (float*)(base + plane);
-    Workspace ws = carve(base + 2 * plane + align_up(P, 256), h, w);
-    cudaStream_t st = (cudaStream_t)stream;
-    CK(cudaMemcpyAsync(d_img, img_host, P * 4, cudaMemcpyHostToDevice, st));
-    if ((rc = run_frame(d_img, h, w, *p, nullptr, d_clean, ws, nullptr, nullptr, st))) return rc;
-    // the S plane, the candidate list and the quad list are dead now: values, indices, block sums
-    const uint32_t* C = ws.C[p->niter & 1];
-    const int wpr = words_per_row(w), nwords = h * wpr;
-    const int nblocks = (nwords + lac::CP_WORDS_PER_CTA - 1) / lac::CP_WORDS_PER_CTA;
-    int* blocksum = ws.qlist;
-    if ((size_t)(nblocks + 1) > (size_t)h * ((w + 3) / 4)) blocksum = (int*)ws.G1;   // tiny frames: any dead plane
-    lac::k_popc_blocks<<<nblocks, 256, 0, st>>>(C, nwords, blocksum);
-    LAUNCHED();
-    lac::k_scan_blocks<<<1, 256, 0, st>>>(blocksum, nblocks);
-    LAUNCHED();
-    lac::k_emit_flagged<<<nblocks, 256, 0, st>>>(C, nwords, blocksum, d_clean, ws.clist, ws.S, cap, w, wpr);
-    LAUNCHED();
-    CK(cudaMemcpyAsync(maskbits_host, C, (size_t)nwords * 4, cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(count_host, blocksum + nblocks, 4, cudaMemcpyDeviceToHost, st));
-    if (cap > 0) {
-        CK(cudaMemcpyAsync(idx_host, ws.clist, (size_t)cap * 4, cudaMemcpyDeviceToHost, st));
-        CK(cudaMemcpyAsync(val_host, ws.S, (size_t)cap * 4, cudaMemcpyDeviceToHost, st));
-    }
-    return LACOSMIC_OK;
+    return run_host_frame(HostFrame{img_host, false, nullptr, nullptr, maskbits_host, idx_host, val_host, count_host, capacity},
+                          h, w, *p, dev_workspace, (cudaStream_t)stream);
+}
+
+int lacosmic_run_host_stream_sparse(const void* imgs_host, int input_is_u16, int n, int h, int w,
+                                    const lacosmic_params* params, uint32_t* maskbits_host, int32_t* idx_host,
+                                    float* val_host, int32_t* counts_host, int capacity, void* dev_workspace,
+                                    size_t dev_workspace_bytes, void* stream) {
+    g_launches = 0;
+    if (n < 0) return LACOSMIC_ERR_SHAPE;
+    if (n == 0) return LACOSMIC_OK;
+    if (!imgs_host || !params || !maskbits_host || !idx_host || !val_host || !counts_host || !dev_workspace)
+        return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    for (int f = 0; f < n; ++f)
+        if ((rc = check_params(params[f]))) return rc;
+    if (capacity < 0) return LACOSMIC_ERR_PARAM;
+    if (((uintptr_t)dev_workspace & 255) || (input_is_u16 && ((uintptr_t)imgs_host & 1))) return LACOSMIC_ERR_ALIGN;
+    const size_t P = (size_t)h * w, bw = (size_t)h * words_per_row(w);
+    return run_host_stream(n, h, w, params, dev_workspace, dev_workspace_bytes, (cudaStream_t)stream, [&](int f) {
+        const void* img = input_is_u16 ? (const void*)((const uint16_t*)imgs_host + f * P)
+                                       : (const void*)((const float*)imgs_host + f * P);
+        return HostFrame{img, input_is_u16 != 0, nullptr, nullptr, maskbits_host + f * bw,
+                         idx_host + (size_t)f * capacity, val_host + (size_t)f * capacity, counts_host + f, capacity};
+    });
 }
 
 size_t lacosmic_host_batch_workspace_bytes(int h, int w, int concurrency) {
@@ -685,32 +753,11 @@ int lacosmic_run_host_batch(const float* imgs_host, int n, int h, int w, const l
     for (int f = 0; f < n; ++f)
         if ((rc = check_params(params[f]))) return rc;
     if ((uintptr_t)dev_workspace & 255) return LACOSMIC_ERR_ALIGN;
-    const size_t slot = align_up(lacosmic_host_workspace_bytes(h, w), 256);
-    const int k = (int)std::min<size_t>(std::min(n, LACOSMIC_MAX_BATCH_STREAMS), dev_workspace_bytes / slot);
-    if (k < 1) return LACOSMIC_ERR_WORKSPACE;
     const size_t P = (size_t)h * w;
-    cudaStream_t caller = (cudaStream_t)stream;
-    BatchStreams* bs = nullptr;
-    if (k > 1) {
-        bs = batch_streams();
-        if (!bs) return LACOSMIC_ERR_CUDA;
-        CK(cudaEventRecord(bs->fork, caller));
-        for (int s = 0; s < k; ++s) CK(cudaStreamWaitEvent(bs->st[s], bs->fork, 0));
-    }
-    for (int f = 0; f < n; ++f) {
-        const int s = f % k;
-        rc = run_host_frame(imgs_host + f * P, false, h, w, params[f], masks_host + f * P, cleans_host + f * P,
-                            (char*)dev_workspace + (size_t)s * slot, k > 1 ? bs->st[s] : caller);
-        if (rc) break;
-    }
-    if (k > 1) {   // join, also after an error
-        for (int s = 0; s < k; ++s) {
-            if (!cuda_ok(cudaEventRecord(bs->join[s], bs->st[s])) ||
-                !cuda_ok(cudaStreamWaitEvent(caller, bs->join[s], 0)))
-                rc = rc ? rc : LACOSMIC_ERR_CUDA;
-        }
-    }
-    return rc;
+    return run_host_stream(n, h, w, params, dev_workspace, dev_workspace_bytes, (cudaStream_t)stream, [&](int f) {
+        return HostFrame{imgs_host + f * P, false, masks_host + f * P, cleans_host + f * P, nullptr, nullptr, nullptr,
+                         nullptr, 0};
+    });
 }
 
 // ---- single steps -----------------------------------------------------------------------------

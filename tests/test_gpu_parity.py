@@ -301,6 +301,37 @@ def test_host_sparse_results(lc, orc, shape):
     assert int(r0["count"][0]) == 0 and not r0["maskbits"].numpy().any()
 
 
+@pytest.mark.parametrize("u16", [False, True], ids=["f32", "u16"])
+@pytest.mark.parametrize("concurrency", [1, 3])
+def test_host_stream_sparse(lc, orc, u16, concurrency):
+    """lacosmic_run_host_stream_sparse: a stream of raw frames in, sparse results out, frames overlapped on the
+    internal streams; every frame's mask, index list and patched frame equal the oracle's."""
+    import torch
+    nf, h, w = 5, 120, 200
+    frames = [synth.make_frame(h, w, seed=3000 + j, n_star=8, n_cr=80, sp_frac=0.004).img for j in range(nf)]
+    if u16:
+        raws = [np.clip(np.rint(f), 0, 65535).astype(np.uint16) for f in frames]
+        frames = [r.astype(np.float32) for r in raws]
+        host = torch.from_numpy(np.stack(raws)).pin_memory()
+    else:
+        host = torch.from_numpy(np.stack(frames)).pin_memory()
+    ps = [dict(PARAMS, sigclip=(4.0, 4.5, 5.0)[j % 3]) for j in range(nf)]
+    r = lc.lacosmic_run_host_stream_sparse(host, [lc.Params(**p) for p in ps], capacity=h * w // 4,
+                                           concurrency=concurrency)
+    torch.cuda.synchronize()
+    for j in range(nf):
+        o = orc.run(frames[j], **ps[j])
+        n = int(r["count"][j])
+        assert n == int(o["mask"].sum()), j
+        bits = np.unpackbits(r["maskbits"][j].numpy().view(np.uint8), axis=1, bitorder="little")[:, :w]
+        assert np.array_equal(bits, o["mask"]), j
+        idx, val = r["idx"][j].numpy()[:n], r["val"][j].numpy()[:n]
+        assert np.array_equal(idx, np.flatnonzero(o["mask"])), j
+        clean = frames[j].copy()
+        clean.flat[idx] = val
+        assert np.array_equal(clean, o["clean"]), j
+
+
 @pytest.mark.parametrize("concurrency", [1, 3])
 def test_host_batch_pipeline(lc, orc, concurrency):
     """lacosmic_run_host_batch: frames in pinned host memory, H2D / kernels / D2H of different frames
