@@ -630,8 +630,8 @@ k_unpack_bits(const uint32_t* __restrict__ bits, uint8_t* __restrict__ u8, int h
         uint32_t o[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            const uint32_t nib = (half >> (4 * q)) & 0xfu;   // spread 4 bits into 4 bytes (0x01 each)
-            o[q] = (nib & 1u) | ((nib & 2u) << 7) | ((nib & 4u) << 14) | ((nib & 8u) << 21);
+            const uint32_t nib = (half >> (4 * q)) & 0xfu;   // spread 4 bits into 4 bytes (0x01 each): the four
+            o[q] = (nib * 0x00204081u) & 0x01010101u;        // shifted copies 0, 7, 14, 21 do not overlap
         }
         *reinterpret_cast<uint4*>(u8 + p0) = make_uint4(o[0], o[1], o[2], o[3]);
     } else {
