@@ -216,7 +216,9 @@ def run_cuda(args):
             fn()
             b.record(stream)
         barrier()
-        total_ms = replicas.max_over_ranks(sum(a.elapsed_time(b) for a, b in evs), world, dev)
+        per_step = [a.elapsed_time(b) for a, b in evs]
+        timed.last = dict(median=statistics.median(per_step), min=min(per_step), max=max(per_step))   # this rank
+        total_ms = replicas.max_over_ranks(sum(per_step), world, dev)
         return total_ms / steps
 
     def measure(mode):
@@ -232,9 +234,10 @@ def run_cuda(args):
         lc.lacosmic_kernel_timing_enable(False)
         launches = lc.lacosmic_last_launch_count()
         ms_nospans = timed(step, args.steps, 1)
+        spread = dict(timed.last)
         # `ms` (the headline) is the run WITHOUT the library's per-kernel event pairs (34 extra event records per
         # step cost ~0.1 ms); the per-kernel durations come from the identical K steps timed with them
-        return dict(ms=ms_nospans, ms_spans=ms, kt=kt, launches=launches,
+        return dict(ms=ms_nospans, ms_spans=ms, spread=spread, kt=kt, launches=launches,
                     counts=counts.cpu().numpy().tolist(), mask=mask.clone(), clean=clean.clone())
 
     # ---- device-resident timing (value): the production path, then the dense reference path
@@ -476,6 +479,7 @@ def run_cuda(args):
         kernels_ms_per_step=main_sum["kernels_ms_per_step"],
         kernel_share_of_step=main_sum["kernel_share_of_step"],
         ms_per_step_with_kernel_event_spans=res["ms_spans"],
+        ms_per_step_spread={k: round(v, 4) for k, v in res["spread"].items()},
         ref_comparisons_T_per_s=ref_cmp_rate,
         other_mode=dict(mode=other_mode, same_mask_clean_counts=modes_agree, roofline=roofline(res_other),
                         **summarise(res_other)),
