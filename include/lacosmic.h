@@ -82,7 +82,8 @@ typedef struct lacosmic_params {
  * uint8 0/1 for G1 = (S' > sigclip), G2 = (S' > sigfrac*sigclip) (both AND img < satlevel),
  * M1 (step 5), M2, M3 (step 6) and C (cumulative mask after the iteration).  LACOSMIC_MODE_LAZY never
  * forms Sp, m3, F and evaluates G2 only where step (6) reads it: those four planes are left untouched
- * there; every other plane is filled and identical in both modes. */
+ * there; every other plane is filled and identical in both modes.  An iteration that is skipped because an
+ * earlier one flagged nothing new (fixed point, R17) leaves the planes untouched. */
 typedef struct lacosmic_debug {
     int32_t iter;   /* iteration whose planes are dumped; -1: none (only `gains` is filled) */
     float *Lp, *N, *S, *Sp, *m3, *F;
