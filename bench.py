@@ -271,15 +271,15 @@ def run_cuda(args):
                                 want_gains=True)
         torch.cuda.synchronize()
         nsel = max(kt_est["gain_select"][1], 1)
-        # one clipping = 18 histogram passes over the residual plane (4 B/px each)
+        # one estimate = 18 histogram passes over the residual plane (4 B/px) + 3 over residual and med5 (8 B/px)
         sel_ms = kt_est["gain_select"][0] / nsel
         gain_est = dict(frames_per_s=world * 1e3 / ms_est, ms_per_step=ms_est,
                         gains=[float(v) for v in ge["gains"].cpu().numpy()],
                         new_cr_per_iteration=counts.cpu().numpy().tolist(),
                         select_ms_per_estimate=sel_ms,
-                        select_hbm_gbs=18 * npx * 4 / (sel_ms * 1e-3) / 1e9,
-                        select_hbm_frac=18 * npx * 4 / (sel_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                        note="gain = 0: residual plane + 3 rounds x 2 selections x 3 radix passes per iteration, "
+                        select_hbm_gbs=96 * npx / (sel_ms * 1e-3) / 1e9,
+                        select_hbm_frac=96 * npx / (sel_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                        note="gain = 0: residual plane + (3 rounds x 2 + 1) selections x 3 radix passes per iteration, "
                              "then every plane recomputed with the estimated gain (no incremental iterations)")
 
     # ---- configs[3] in small: a stream of independent frames with per-frame parameters, resident in HBM,

@@ -54,7 +54,8 @@ extern "C" {
 /* Parameters of one frame (PAPER.md:66-74 plus niter/satlevel of the north_star signature).
  * gain [e-/ADU] > 0, or 0 = "not supplied": it is then estimated at each iteration from that iteration's
  * input image (reading R21: residual over sqrt(med5), three rounds of rank-based
- * sigma clipping, gain = 1/s^2; every iteration then recomputes all planes); readnoise [e-] >= 0;
+ * sigma clipping, gain = the positive root of the noise model's variance equation; every iteration then
+ * recomputes all planes); readnoise [e-] >= 0;
  * sigclip > 0: detection limit in sigma; sigfrac in (0,1]: fractional limit for neighbours;
  * objlim >= 0: contrast limit L+/F; satlevel: pixels >= satlevel are never flagged (+INF disables);
  * niter in [0, LACOSMIC_MAX_NITER]: number of iterations (0: clean_out = img, mask_out = 0). */
@@ -192,11 +193,12 @@ int lacosmic_run_host_batch(const float *imgs_host, int n, int h, int w, const l
 /* ---- single steps (each is the kernel the whole path uses; exported for parity tests) -------- */
 
 /* R21 alone: the gain estimate of one image (what the whole path computes at the start of an iteration when
- * p->gain == 0).  gain_out: DEVICE pointer to one float; stats_out: nullable DEVICE pointer to 5 floats
- * {c, s, lo, hi, kept} of the last clipping round (centre, 1.4826 MAD, the interval the round started from,
- * number of pixels inside it).  workspace as for lacosmic_run_ws. */
-int lacosmic_estimate_gain(const float *img, int h, int w, float *gain_out, float *stats_out,
-                           void *workspace, size_t workspace_bytes, void *stream);
+ * p->gain == 0), for the given read noise [e-].  gain_out: DEVICE pointer to one float; stats_out: nullable
+ * DEVICE pointer to 6 floats {c, s, lo, hi, kept, mt}: centre, 1.4826 MAD, the interval the last clipping
+ * round started from, the number of pixels inside it, and the typical signal (rank-(kept-1)/2 element of
+ * max(med5, 1e-4) over those pixels).  workspace as for lacosmic_run_ws. */
+int lacosmic_estimate_gain(const float *img, int h, int w, float readnoise, float *gain_out,
+                           float *stats_out, void *workspace, size_t workspace_bytes, void *stream);
 
 /* Step (1): out = L+(in).  in/out fp32 [h][w], distinct. */
 int lacosmic_lplus(const float *in, float *out, int h, int w, void *stream);

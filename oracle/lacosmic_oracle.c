@@ -169,8 +169,8 @@ void orc_masked_median(const float *img, const uint8_t *mask, float *out, int h,
  * standard deviation 1/sqrt(gain).  sigma is estimated robustly and ORDER-INDEPENDENTLY (selection
  * only, no sums): three rounds of { c = median of r over the kept set, d = median of |r - c| over the
  * kept set, s = 1.4826 d, keep c - 5 s <= r <= c + 5 s (intersected with the previous interval) },
- * "median" = the element of 0-based rank (n-1)/2 of the ascending sort.  gain = 1/s^2 (1 if s is 0 or
- * not finite).  Read noise is not subtracted (stated bias, R21). */
+ * "median" = the element of 0-based rank (n-1)/2 of the ascending sort.  The gain then follows from s and
+ * the read noise through the noise model itself (orc_estimate_gain below). */
 static int cmp_float(const void *a, const void *b) {
     float x = *(const float *)a, y = *(const float *)b;
     return (x > y) - (x < y);
@@ -211,11 +211,17 @@ float orc_sigma_clip(const float *r, size_t n, int rounds, float *stats) {
 }
 
 /* gain estimate of one image (the `work` plane of an iteration).  stats: nullable float[5], see above. */
-int orc_estimate_gain(const float *work, int h, int w, float *gain_out, float *stats) {
-    if (!work || !gain_out || h < 1 || w < 1) return ORC_ERR_ARG;
+/* gain estimate of one image (the `work` plane of an iteration).  stats: nullable float[6] = the sigma-clip
+ * statistics above plus stats[5] = mt.  The noise model of O2 is var(work) = signal/gain + (rn/gain)^2, so
+ * with sigma^2 = var(r) = var(work)/signal:  sigma^2 gain^2 - gain - rn^2/mt = 0, mt = the typical signal =
+ * rank-(n-1)/2 element of max(med5, 1e-4) over the pixels the last clipping round kept.  The positive root,
+ * in this operation order (fp32):  s2 = s*s;  a = ((4*s2)*rn2)/mt;  gain = (1 + sqrt(1 + a)) / (2*s2).
+ * rn = 0 gives gain = 1/s2 exactly.  gain = 1 if s is 0 or the result is not finite and positive. */
+int orc_estimate_gain(const float *work, int h, int w, float readnoise, float *gain_out, float *stats) {
+    if (!work || !gain_out || h < 1 || w < 1 || !(readnoise >= 0.0f)) return ORC_ERR_ARG;
     size_t P = (size_t)h * (size_t)w;
-    float *m5 = malloc(P * 4), *r = malloc(P * 4);
-    if (!m5 || !r) { free(m5); free(r); return ORC_ERR_MEM; }
+    float *m5 = malloc(P * 4), *r = malloc(P * 4), *v = malloc(P * 4);
+    if (!m5 || !r || !v) { free(m5); free(r); free(v); return ORC_ERR_MEM; }
     orc_medfilt(work, m5, h, w, 5);
 #pragma omp parallel for schedule(static)
     for (size_t p = 0; p < P; ++p) {
@@ -223,10 +229,20 @@ int orc_estimate_gain(const float *work, int h, int w, float *gain_out, float *s
         float dev = work[p] - m5[p];
         r[p] = dev / sqrtf(m);
     }
-    float s = orc_sigma_clip(r, P, 3, stats);
+    float st[5];
+    float s = orc_sigma_clip(r, P, 3, st);
+    /* typical signal over the set the last round kept: st[2] <= r <= st[3] */
+    size_t m = 0;
+    for (size_t p = 0; p < P; ++p)
+        if (r[p] >= st[2] && r[p] <= st[3]) v[m++] = m5[p] > 1e-4f ? m5[p] : 1e-4f;
+    float mt = m ? lower_median(v, m) : 1.0f;
+    const float rn2 = readnoise * readnoise;
     float s2 = s * s;
-    *gain_out = (s > 0.0f && isfinite(s) && isfinite(1.0f / s2)) ? 1.0f / s2 : 1.0f;
-    free(m5); free(r);
+    float a = ((4.0f * s2) * rn2) / mt;
+    float g = (1.0f + sqrtf(1.0f + a)) / (2.0f * s2);
+    *gain_out = (s > 0.0f && isfinite(s) && isfinite(g) && g > 0.0f) ? g : 1.0f;
+    if (stats) { memcpy(stats, st, sizeof st); stats[5] = mt; }
+    free(m5); free(r); free(v);
     return ORC_OK;
 }
 
@@ -266,7 +282,7 @@ int orc_run(const float *img, int h, int w, float gain, float readnoise, float s
     for (int t = 0; t < niter; ++t) {
         if (dbg && dbg->iter == t) COPY_IF(dbg->work_in, work, P * 4);
         if (estimate) {   /* R21: estimated at each iteration, from the iteration's input image */
-            rc = orc_estimate_gain(work, h, w, &gain, NULL);
+            rc = orc_estimate_gain(work, h, w, readnoise, &gain, NULL);
             if (rc) goto done;
         }
         if (iter_gains) iter_gains[t] = gain;

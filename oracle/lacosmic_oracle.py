@@ -56,7 +56,7 @@ def lib():
         L.orc_masked_median.restype = None
         L.orc_run.argtypes = [fp, C.c_int, C.c_int] + [C.c_float] * 5 + [C.c_int, C.c_float,
                                                                         u8p, fp, i32p, C.c_void_p, fp]
-        L.orc_estimate_gain.argtypes = [fp, C.c_int, C.c_int, fp, fp]
+        L.orc_estimate_gain.argtypes = [fp, C.c_int, C.c_int, C.c_float, fp, fp]
         L.orc_estimate_gain.restype = C.c_int
         L.orc_sigma_clip.argtypes = [fp, C.c_size_t, C.c_int, fp]
         L.orc_sigma_clip.restype = C.c_float
@@ -130,12 +130,12 @@ def sigma_clip(r, rounds=3):
     return float(np.float32(s)), stats
 
 
-def estimate_gain(img):
-    """R21 gain estimate of one image.  Returns (gain fp32, stats)."""
+def estimate_gain(img, readnoise=0.0):
+    """R21 gain estimate of one image.  Returns (gain fp32, stats = [c, s, lo, hi, kept, mt])."""
     img = _f32(img)
     g = np.zeros(1, np.float32)
-    stats = np.zeros(5, np.float32)
-    rc = lib().orc_estimate_gain(_p(img), img.shape[0], img.shape[1], _p(g), _p(stats))
+    stats = np.zeros(6, np.float32)
+    rc = lib().orc_estimate_gain(_p(img), img.shape[0], img.shape[1], float(readnoise), _p(g), _p(stats))
     if rc != 0:
         raise ValueError("orc_estimate_gain failed with code %d" % rc)
     return np.float32(g[0]), stats

@@ -99,7 +99,7 @@ def load_library():
         "lacosmic_run_host_u16": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp]),
         "lacosmic_run_host_sparse": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, vp, i, vp, sz, vp]),
         "lacosmic_run_host_stream_sparse": (i, [vp, i, i, i, i, C.POINTER(_CParams), vp, vp, vp, vp, i, vp, sz, vp]),
-        "lacosmic_estimate_gain": (i, [vp, i, i, vp, vp, vp, sz, vp]),
+        "lacosmic_estimate_gain": (i, [vp, i, i, f, vp, vp, vp, sz, vp]),
         "lacosmic_lplus": (i, [vp, vp, i, i, vp]),
         "lacosmic_medfilt": (i, [vp, vp, i, i, i, vp]),
         "lacosmic_bitplane_pitch_words": (i, [i]),
@@ -390,16 +390,16 @@ def lacosmic_run_host_batch(imgs_host, params, masks_host=None, cleans_host=None
 
 
 # ----------------------------------------------------------------------------- single steps
-def lacosmic_estimate_gain(img, workspace=None, stream=None):
-    """R21 alone.  Returns (gain: device float tensor [1], stats: device float tensor [5] = c, s, lo, hi, kept)."""
+def lacosmic_estimate_gain(img, readnoise=0.0, workspace=None, stream=None):
+    """R21 alone.  Returns (gain: device float tensor [1], stats: device float tensor [6] = c, s, lo, hi, kept, mt)."""
     torch = _torch()
     h, w = img.shape
     if workspace is None:
         workspace = _workspace(h, w, img.device)
     gain = torch.zeros(1, dtype=torch.float32, device=img.device)
-    stats = torch.zeros(5, dtype=torch.float32, device=img.device)
+    stats = torch.zeros(6, dtype=torch.float32, device=img.device)
     _check(load_library().lacosmic_estimate_gain(
-        _dev(img, torch.float32, "img"), h, w, gain.data_ptr(), stats.data_ptr(),
+        _dev(img, torch.float32, "img"), h, w, float(readnoise), gain.data_ptr(), stats.data_ptr(),
         _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)), "lacosmic_estimate_gain")
     return gain, stats
 

@@ -208,16 +208,17 @@ int grow_replace(const lac::GrowArgs& ga, const int* prev, cudaStream_t st) {
     return LACOSMIC_OK;
 }
 
-// R21: sigma clipping of the residual plane R (select.cuh) -> *gain_out (device), stats (nullable, device)
+// R21: sigma clipping of the residual plane R, typical signal from the med5 plane M5 (select.cuh)
+// -> *gain_out (device), stats (nullable, device, 6 floats)
 template <int MODE, int PASS>
-int sel_step(const float* R, size_t npx, const Workspace& ws, int grid, int last, float* gain_out, float* stats,
-             const int* prev, cudaStream_t st) {
-    lac::k_sel_hist<MODE, PASS><<<grid, 256, 0, st>>>(R, npx, ws.sel, ws.hist, last, gain_out, stats, prev);
+int sel_step(const float* R, const float* M5, size_t npx, const Workspace& ws, int grid, int last, float rn2,
+             float* gain_out, float* stats, const int* prev, cudaStream_t st) {
+    lac::k_sel_hist<MODE, PASS><<<grid, 256, 0, st>>>(R, M5, npx, ws.sel, ws.hist, last, rn2, gain_out, stats, prev);
     LAUNCHED();
     return LACOSMIC_OK;
 }
-int sigma_clip_gain(const float* R, size_t npx, const Workspace& ws, float* gain_out, float* stats, const int* prev,
-                    cudaStream_t st) {
+int sigma_clip_gain(const float* R, const float* M5, size_t npx, const Workspace& ws, float rn2, float* gain_out,
+                    float* stats, const int* prev, cudaStream_t st) {
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
 #ifndef LAC_SEL_CTAS_PER_SM
@@ -228,16 +229,20 @@ int sigma_clip_gain(const float* R, size_t npx, const Workspace& ws, float* gain
     Span sp(KC_SELECT, st);
     lac::k_sel_init<<<1, 256, 0, st>>>(ws.sel, ws.hist, prev);
     LAUNCHED();
+    int rc;
     for (int j = 0; j < lac::SEL_ROUNDS; ++j) {
         const int last = j == lac::SEL_ROUNDS - 1;
-        int rc;
-        if ((rc = sel_step<0, 0>(R, npx, ws, grid, 0, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<0, 1>(R, npx, ws, grid, 0, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<0, 2>(R, npx, ws, grid, 0, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<1, 0>(R, npx, ws, grid, 0, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<1, 1>(R, npx, ws, grid, 0, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<1, 2>(R, npx, ws, grid, last, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<0, 0>(R, M5, npx, ws, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<0, 1>(R, M5, npx, ws, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<0, 2>(R, M5, npx, ws, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<1, 0>(R, M5, npx, ws, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<1, 1>(R, M5, npx, ws, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<1, 2>(R, M5, npx, ws, grid, last, rn2, gain_out, stats, prev, st))) return rc;
     }
+    // typical signal over the set the last round kept, then the gain
+    if ((rc = sel_step<2, 0>(R, M5, npx, ws, grid, 1, rn2, gain_out, stats, prev, st))) return rc;
+    if ((rc = sel_step<2, 1>(R, M5, npx, ws, grid, 1, rn2, gain_out, stats, prev, st))) return rc;
+    if ((rc = sel_step<2, 2>(R, M5, npx, ws, grid, 1, rn2, gain_out, stats, prev, st))) return rc;
     return LACOSMIC_OK;
 }
 
@@ -313,7 +318,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                               h, w, wpr, 1.0f, rn2, p.sigclip, siglow, p.satlevel, (float*)ws.clist, nullptr,
                               t == 0 ? zero_ptr : nullptr, zero_n};
             if ((rc = noise_pass(ne, src))) return rc;
-            if ((rc = sigma_clip_gain((const float*)ws.clist, P, ws, ws.gains + t, nullptr, prev, st))) return rc;
+            if ((rc = sigma_clip_gain((const float*)ws.clist, ws.S, P, ws, rn2, ws.gains + t, nullptr, prev, st))) return rc;
             src = work;
         }
         // lazy path, t >= 1: S, A1, A2 and the tests only change near the pixels the previous replacement
@@ -762,24 +767,25 @@ int lacosmic_run_host_batch(const float* imgs_host, int n, int h, int w, const l
 
 // ---- single steps -----------------------------------------------------------------------------
 
-int lacosmic_estimate_gain(const float* img, int h, int w, float* gain_out, float* stats_out, void* workspace,
-                           size_t workspace_bytes, void* stream) {
+int lacosmic_estimate_gain(const float* img, int h, int w, float readnoise, float* gain_out, float* stats_out,
+                           void* workspace, size_t workspace_bytes, void* stream) {
     g_launches = 0;
     if (!img || !gain_out || !workspace) return LACOSMIC_ERR_NULL;
     int rc = check_shape(h, w);
     if (rc) return rc;
+    if (!(readnoise >= 0.0f) || !std::isfinite(readnoise)) return LACOSMIC_ERR_PARAM;
     if (((uintptr_t)img & 15) || ((uintptr_t)workspace & 255)) return LACOSMIC_ERR_ALIGN;
     if (workspace_bytes < lacosmic_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
     Workspace ws = carve(workspace, h, w);
     cudaStream_t st = (cudaStream_t)stream;
     const size_t P = (size_t)h * w;
-    // the dense noise/S kernel (generic loader) with the residual plane switched on; S (gain 1) is scratch
+    // the dense noise/S kernel (generic loader) with the residual plane switched on: r -> clist, med5 -> S
     lac::NoiseArgs ne{ws.S, nullptr, nullptr, nullptr, nullptr, nullptr, h, w, words_per_row(w), 1.0f, 0.0f,
                       1.0f, 1.0f, 0.0f, (float*)ws.clist, nullptr};
     const int ntx = (w + lac::TW - 1) / lac::TW, nt = ntx * ((h + lac::NS_TH - 1) / lac::NS_TH);
     lac::k_noise_S<<<nt, lac::NT, 0, st>>>(img, ne, ntx, nullptr);
     LAUNCHED();
-    return sigma_clip_gain((const float*)ws.clist, P, ws, gain_out, stats_out, nullptr, st);
+    return sigma_clip_gain((const float*)ws.clist, ws.S, P, ws, readnoise * readnoise, gain_out, stats_out, nullptr, st);
 }
 
 int lacosmic_lplus(const float* in, float* out, int h, int w, void* stream) {

@@ -7,7 +7,8 @@
 // fixed (shared-memory histogram per CTA, flushed with atomics); the CTA that finishes last (atomic ticket)
 // then walks the 2048 counts to the bucket holding the wanted rank, so a pass is one launch.  One round of
 // the clipping is two selections over the kept set K = { lo <= r <= hi }: the centre c (rank (n-1)/2 of r)
-// and the MAD d (same rank of |r - c|).
+// and the MAD d (same rank of |r - c|).  A last selection gives the typical signal mt (same rank of max(med5,
+// 1e-4) over the set the last round kept), and the gain follows from the noise model (R21).
 #pragma once
 #include "common.cuh"
 
@@ -57,8 +58,8 @@ __global__ void k_sel_init(SelState* st, uint32_t* hist, const int* prev_count) 
 // follow with exactly the oracle's operations; the `last` round writes the gain instead (and the statistics
 // {c, s, lo, hi, kept} of the round when stats is given).
 template <int MODE, int PASS>
-__device__ __forceinline__ void sel_pick(SelState* st, uint32_t* hist, uint32_t* scan, int last, float* gain_out,
-                                         float* stats) {
+__device__ __forceinline__ void sel_pick(SelState* st, uint32_t* hist, uint32_t* scan, int last, float rn2,
+                                         float* gain_out, float* stats) {
     const int tid = threadIdx.x;
     constexpr int PER = SEL_BINS / 256;
     uint32_t loc[PER], sum = 0;
@@ -91,7 +92,7 @@ __device__ __forceinline__ void sel_pick(SelState* st, uint32_t* hist, uint32_t*
             const float v = sel_unkey(prefix);
             if (MODE == 0) {
                 st->c = v;
-            } else {
+            } else if (MODE == 1) {
                 const float s = __fmul_rn(1.4826f, v);
                 const float five_s = __fmul_rn(5.0f, s);
                 const float nlo = __fsub_rn(st->c, five_s), nhi = __fadd_rn(st->c, five_s);
@@ -99,13 +100,19 @@ __device__ __forceinline__ void sel_pick(SelState* st, uint32_t* hist, uint32_t*
                 if (!last) {   // the next round starts from the intersection
                     st->lo = nlo > st->lo ? nlo : st->lo;
                     st->hi = nhi < st->hi ? nhi : st->hi;
-                } else {
-                    const float g = __fdiv_rn(1.0f, __fmul_rn(s, s));
-                    const float INF = __int_as_float(0x7f800000);
-                    *gain_out = (s > 0.0f && s < INF && g < INF) ? g : 1.0f;
-                    if (stats) {
-                        stats[0] = st->c; stats[1] = s; stats[2] = st->lo; stats[3] = st->hi; stats[4] = (float)st->n;
-                    }
+                }
+            } else {
+                // v = mt, the typical signal.  sigma^2 gain^2 - gain - rn^2/mt = 0, positive root, in the
+                // oracle's operation order
+                const float s = st->s;
+                const float s2 = __fmul_rn(s, s);
+                const float a = __fdiv_rn(__fmul_rn(__fmul_rn(4.0f, s2), rn2), v);
+                const float g = __fdiv_rn(__fadd_rn(1.0f, __fsqrt_rn(__fadd_rn(1.0f, a))), __fmul_rn(2.0f, s2));
+                const float INF = __int_as_float(0x7f800000);
+                *gain_out = (s > 0.0f && s < INF && g > 0.0f && g < INF) ? g : 1.0f;
+                if (stats) {
+                    stats[0] = st->c; stats[1] = s; stats[2] = st->lo; stats[3] = st->hi; stats[4] = (float)st->n;
+                    stats[5] = v;
                 }
             }
             st->prefix = 0;
@@ -113,13 +120,14 @@ __device__ __forceinline__ void sel_pick(SelState* st, uint32_t* hist, uint32_t*
     }
 }
 
-// MODE 0: value = r; MODE 1: value = |r - c|.  PASS 0/1/2: key bits 31..21 / 20..10 / 9..0.
+// MODE 0: value = r; MODE 1: value = |r - c|; MODE 2: value = max(med5, 1e-4) (plane M5), all over the kept
+// set lo <= r <= hi.  PASS 0/1/2: key bits 31..21 / 20..10 / 9..0.
 template <int MODE, int PASS>
 __global__ void __launch_bounds__(256)
-k_sel_hist(const float* __restrict__ R, size_t npx, SelState* st, uint32_t* hist, int last, float* gain_out,
-           float* stats, const int* prev_count) {
+k_sel_hist(const float* __restrict__ R, const float* __restrict__ M5, size_t npx, SelState* st, uint32_t* hist,
+           int last, float rn2, float* gain_out, float* stats, const int* prev_count) {
     if (prev_count && *prev_count == 0) {          // fixed point (R17): same image, same estimate
-        if (MODE == 1 && PASS == 2 && last && blockIdx.x == 0 && threadIdx.x == 0) *gain_out = gain_out[-1];
+        if (MODE == 2 && PASS == 2 && blockIdx.x == 0 && threadIdx.x == 0) *gain_out = gain_out[-1];
         return;
     }
     __shared__ uint32_t sh[SEL_BINS];
@@ -139,31 +147,42 @@ k_sel_hist(const float* __restrict__ R, size_t npx, SelState* st, uint32_t* hist
     }
     const bool none = klo > khi;                    // empty intersection (cannot hold the wanted rank)
     const uint32_t span = khi - klo;
-    auto visit = [&](float r) {
+    auto visit = [&](float r, float m5) {
         uint32_t k;
         if (MODE == 0) {
             k = sel_key(r);
         } else {
             if (!(r >= lo && r <= hi)) return;
-            k = __float_as_uint(fabsf(__fsub_rn(r, c))) | 0x80000000u;   // non-negative value
+            const float v = MODE == 1 ? fabsf(__fsub_rn(r, c)) : (m5 > 1e-4f ? m5 : 1e-4f);
+            k = __float_as_uint(v) | 0x80000000u;   // non-negative value
         }
         if (!none && k - klo <= span) atomicAdd(&sh[(k >> SHIFT) & MASK], 1u);
     };
     const size_t nvec = npx / 4;
     const size_t stride = (size_t)gridDim.x * 256, end = nvec;
     size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
+    const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
     for (; i + 3 * stride < end; i += 4 * stride) {   // four independent 16-byte loads in flight per thread
-        float4 q[4];
+        float4 q[4], m[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) q[u] = __ldg(reinterpret_cast<const float4*>(R) + i + u * stride);
+        for (int u = 0; u < 4; ++u) {
+            q[u] = __ldg(reinterpret_cast<const float4*>(R) + i + u * stride);
+            m[u] = MODE == 2 ? __ldg(reinterpret_cast<const float4*>(M5) + i + u * stride) : zero4;
+        }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { visit(q[u].x); visit(q[u].y); visit(q[u].z); visit(q[u].w); }
+        for (int u = 0; u < 4; ++u) {
+            visit(q[u].x, m[u].x); visit(q[u].y, m[u].y); visit(q[u].z, m[u].z); visit(q[u].w, m[u].w);
+        }
     }
     for (; i < end; i += stride) {
         const float4 q = __ldg(reinterpret_cast<const float4*>(R) + i);
-        visit(q.x); visit(q.y); visit(q.z); visit(q.w);
+        const float4 m = MODE == 2 ? __ldg(reinterpret_cast<const float4*>(M5) + i) : zero4;
+        visit(q.x, m.x); visit(q.y, m.y); visit(q.z, m.z); visit(q.w, m.w);
     }
-    if (blockIdx.x == 0 && threadIdx.x < (int)(npx - nvec * 4)) visit(R[nvec * 4 + threadIdx.x]);
+    if (blockIdx.x == 0 && threadIdx.x < (int)(npx - nvec * 4)) {
+        const size_t t = nvec * 4 + threadIdx.x;
+        visit(R[t], MODE == 2 ? M5[t] : 0.0f);
+    }
     __syncthreads();
     for (int i = threadIdx.x; i < SEL_BINS; i += 256)
         if (sh[i]) atomicAdd(&hist[i], sh[i]);
@@ -175,7 +194,7 @@ k_sel_hist(const float* __restrict__ R, size_t npx, SelState* st, uint32_t* hist
     __syncthreads();
     if (!s_last) return;
     __threadfence();
-    sel_pick<MODE, PASS>(st, hist, sh, last, gain_out, stats);
+    sel_pick<MODE, PASS>(st, hist, sh, last, rn2, gain_out, stats);
     if (threadIdx.x == 0) st->ticket = 0;
 }
 

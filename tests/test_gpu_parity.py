@@ -358,11 +358,12 @@ def test_estimate_gain_bit_exact(lc, orc, shape):
     x = (300.0 + np.sqrt(300.0 / 1.9) * rng.standard_normal(shape)).astype(np.float32)
     if x.size > 50:
         x.flat[rng.integers(0, x.size, x.size // 40)] += 4000.0          # cosmic-ray-like outliers
-    g, st = lc.lacosmic_estimate_gain(_t(x))
-    torch.cuda.synchronize()
-    go, sto = orc.estimate_gain(x)
-    assert _n(g)[0] == go, (float(_n(g)[0]), float(go))
-    assert np.array_equal(_n(st), sto), (_n(st), sto)
+    for rn in (0.0, 7.5):
+        g, st = lc.lacosmic_estimate_gain(_t(x), readnoise=rn)
+        torch.cuda.synchronize()
+        go, sto = orc.estimate_gain(x, rn)
+        assert _n(g)[0] == go, (rn, float(_n(g)[0]), float(go))
+        assert np.array_equal(_n(st), sto), (rn, _n(st), sto)
 
 
 def test_estimate_gain_ties_and_degenerate(lc, orc):
@@ -370,9 +371,9 @@ def test_estimate_gain_ties_and_degenerate(lc, orc):
     for x in (np.full((40, 50), 77.0, np.float32),                          # sigma = 0 -> gain 1
               np.tile(np.array([10.0, 11.0], np.float32), (30, 20)),          # two values: massive ties
               -np.abs(_rng(3).standard_normal((50, 60))).astype(np.float32)):  # negative image: med5 floored
-        g, st = lc.lacosmic_estimate_gain(_t(x))
+        g, st = lc.lacosmic_estimate_gain(_t(x), readnoise=4.0)
         torch.cuda.synchronize()
-        go, sto = orc.estimate_gain(x)
+        go, sto = orc.estimate_gain(x, 4.0)
         assert _n(g)[0] == go and np.array_equal(_n(st), sto)
 
 

@@ -429,20 +429,35 @@ def test_p13_gain_of_pure_poisson_like_noise_is_recovered(orc, gain):
     g, stats = orc.estimate_gain(img)
     assert abs(g / gain - 1.0) < 0.12
     assert abs(stats[0]) < 0.05 / math.sqrt(gain)
+    assert g == np.float32(1.0) / (stats[1] * stats[1])          # no read noise: gain = 1/s^2 exactly
+    assert abs(stats[5] / B - 1.0) < 0.01                         # typical signal = the sky level
     # robust: 1 % of the pixels hit by cosmic rays barely moves the estimate
     hit = rng.random(img.shape) < 0.01
     g2, _ = orc.estimate_gain(np.where(hit, img + 5000.0, img).astype(np.float32))
     assert abs(g2 / g - 1.0) < 0.05
 
 
+@pytest.mark.parametrize("gain,rn,B", [(1.0, 10.0, 100.0), (2.0, 5.0, 400.0), (1.7, 20.0, 50.0), (0.6, 3.0, 30.0)])
+def test_p13_gain_is_recovered_with_read_noise(orc, gain, rn, B):
+    """The estimate must reproduce the noise model it feeds (O2): var(work) = B/gain + (rn/gain)^2.  Ignoring the
+    read-noise term would read gain 0.54 for a true 1.0 at rn = 10 e- on a 100 ADU sky."""
+    rng = np.random.default_rng(8)
+    img = (B + np.sqrt(B / gain + (rn / gain) ** 2) * rng.standard_normal((500, 620))).astype(np.float32)
+    g, _ = orc.estimate_gain(img, rn)
+    assert abs(g / gain - 1.0) < 0.12
+    g0, _ = orc.estimate_gain(img, 0.0)
+    assert g0 < g                                                  # the read-noise term only raises the estimate
+
+
 def test_p13_gain_scaling_is_exact(orc):
     """img -> 4 img scales every residual by exactly 2 (all operations scale by powers of two), hence
     gain -> gain / 4 bit for bit: pins the structure (difference over sqrt(median)) of the estimator."""
     f = synth.make_frame(96, 130, seed=4, n_star=5, n_cr=30, sp_frac=0.003)
-    g1, st1 = orc.estimate_gain(f.img)
-    g4, st4 = orc.estimate_gain(4.0 * f.img)
-    assert g4 * np.float32(4.0) == g1
-    assert st4[0] == 2 * st1[0] and st4[1] == 2 * st1[1] and st4[4] == st1[4]
+    for rn in (0.0, 10.0):       # read noise is in electrons: unchanged when the image is rescaled
+        g1, st1 = orc.estimate_gain(f.img, rn)
+        g4, st4 = orc.estimate_gain(4.0 * f.img, rn)
+        assert g4 * np.float32(4.0) == g1
+        assert st4[0] == 2 * st1[0] and st4[1] == 2 * st1[1] and st4[4] == st1[4] and st4[5] == 4 * st1[5]
 
 
 def test_p13_degenerate_and_whole_path(orc):
@@ -453,12 +468,12 @@ def test_p13_degenerate_and_whole_path(orc):
     assert est["gains"].shape == (PARAMS["niter"],) and np.all(est["gains"] > 0)
     # iteration 0 estimates from the input frame; feeding the estimates back as supplied gains, one
     # iteration at a time, reproduces the run: the estimate only enters through the noise model
-    g0, _ = orc.estimate_gain(f.img)
-    assert est["gains"][0] == g0
+    g0, _ = orc.estimate_gain(f.img, PARAMS["readnoise"])
+    assert est["gains"][0] == g0 and abs(g0 - 1.0) < 0.1                     # configs[0] was made with gain 1
     one = orc.run(f.img, **dict(PARAMS, gain=float(g0), niter=1))
     est1 = orc.run(f.img, **dict(PARAMS, gain=0.0, niter=1))
     assert np.array_equal(one["mask"], est1["mask"]) and np.array_equal(one["clean"], est1["clean"])
-    g1, _ = orc.estimate_gain(est1["clean"])
+    g1, _ = orc.estimate_gain(est1["clean"], PARAMS["readnoise"])
     assert est["gains"][1] == g1                                            # iteration 1 sees the cleaned frame
     fixed = orc.run(f.img, **PARAMS)
     assert np.all(fixed["gains"] == np.float32(PARAMS["gain"]))
