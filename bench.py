@@ -42,7 +42,7 @@ REF_COMPARISONS_PER_PX_ITER = 19 + 99 + 99 + 480
 # dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture
 # (profiles/; None until captured)
 NCU_TRAFFIC_BYTES = {"fine_gates": 238157312,      # dense mode: profiles/r01_v2_ncu_full.md
-                     "noise_S": 269300000}         # lazy mode (with the work = img_in copy): profiles/r01_v6_ncu_full.md
+                     "noise_S": 269300000}         # lazy mode (with the work = img_in copy): profiles/r01_v9_ncu_full.md
 
 
 def _peaks():
