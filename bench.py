@@ -41,7 +41,7 @@ FINE_GATES_MINMAX_PER_PX = None   # filled from the library's own accounting bel
 REF_COMPARISONS_PER_PX_ITER = 19 + 99 + 99 + 480
 # dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture
 # (profiles/; None until captured)
-NCU_TRAFFIC_BYTES = {"fine_gates": 238157312,      # dense mode: profiles/r01_v2_ncu_full.md
+NCU_TRAFFIC_BYTES = {"fine_gates": 239900000,      # dense mode: profiles/r01_v9_ncu_full_dense.md
                      "noise_S": 269300000}         # lazy mode (with the work = img_in copy): profiles/r01_v9_ncu_full.md
 
 
