@@ -6,21 +6,6 @@
 
 namespace lac {
 
-// Load policy of the listed-pixel / bit-plane device functions.  COH = false: the data was written by an EARLIER
-// launch (read-only path __ldg, or a plain load).  COH = true: the function runs inside the persistent kernel of
-// the incremental iterations (tail.cuh), where other CTAs rewrite the planes between grid-wide barriers: every
-// load of shared state goes to L2 (ld.global.cg), never through this SM's L1 or the read-only path.
-template <bool COH, class T>
-__device__ __forceinline__ T ldro(const T* p) {   // data that is read-only for the whole launch when !COH
-    if (COH) return __ldcg(p);
-    return __ldg(p);
-}
-template <bool COH, class T>
-__device__ __forceinline__ T ldpl(const T* p) {   // data this launch also writes (own words), plain when !COH
-    if (COH) return __ldcg(p);
-    return *p;
-}
-
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return min(max(v, lo), hi); }
 
 // compare-exchange: a <- min, b <- max (two FMNMX on the ALU pipe)

@@ -100,32 +100,36 @@ struct GrowArgs {
     float siglow;
 };
 
-// One strip (sx, sy) of nsx strip columns, by one warp.  s_plane: (WG_R + 4) * 32 words and s_list: WG_LCAP ints
-// of this warp's shared memory.  COH: see common.cuh (ldro / ldpl).
-template <bool COH>
-__device__ __forceinline__ void grow_replace_strip(const GrowArgs& a, const int* prev_count, int sx, int sy, int nsx,
-                                                   uint32_t* s_plane, int* s_list) {
-    const int lane = threadIdx.x & 31;
+#ifndef LAC_GROW_MINB
+#define LAC_GROW_MINB 3
+#endif
+__global__ void __launch_bounds__(32 * WG_WARPS, LAC_GROW_MINB)
+k_grow_replace(GrowArgs a, const int* prev_count) {
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const int h = a.h, w = a.w, wpr = a.wpr;
-    const int wxh = sx * WG_OWN - 1;                         // word column of lane 0
+    const int wxh = blockIdx.x * WG_OWN - 1;                 // word column of lane 0
     const int wx = wxh + lane;
-    const int ya = sy * WG_R;                                 // first own row
-    if (ya >= h) return;                                      // warp-uniform; no block barrier in here
+    const int ya = (blockIdx.y * WG_WARPS + wi) * WG_R;       // first own row
+    if (ya >= h) return;                                      // warp-uniform; the kernel has no block barrier
     const bool colok = wx >= 0 && wx < wpr;
     const bool own = lane >= 1 && lane <= WG_OWN && colok;
     const int wxc = clampi(wx, 0, wpr - 1);
+    __shared__ uint32_t s_plane_all[WG_WARPS][(WG_R + 4) * 32];   // G2, then C', rows ya-2 .. ya+WG_R+1
+    __shared__ int s_list_all[WG_WARPS][WG_LCAP];
+    uint32_t* s_plane = s_plane_all[wi];
+    int* s_list = s_list_all[wi];
     // word (row j, this lane's column) of a plane; 0 outside the frame.  Branch-free: clamped address.
-    auto ld = [&](const uint32_t* pl, int j) -> uint32_t {
+    auto ld = [&](const uint32_t* __restrict__ pl, int j) -> uint32_t {
         const int y = ya - 4 + j;
-        const uint32_t v = ldpl<COH>(pl + (size_t)clampi(y, 0, h - 1) * wpr + wxc);
+        const uint32_t v = pl[(size_t)clampi(y, 0, h - 1) * wpr + wxc];
         return (colok && y >= 0 && y < h) ? v : 0u;
     };
     auto qof = [&](int j) -> size_t { return (size_t)(ya - 4 + j) * wpr + wx; };
-    if (prev_count && ldpl<COH>(prev_count) == 0) {
+    if (prev_count && *prev_count == 0) {
         // fixed point (R17): nothing changes; carry C over to the plane the next reader expects
 #pragma unroll
         for (int j = 4; j < 4 + WG_R; ++j)
-            if (own && ya - 4 + j < h) a.Cnew[qof(j)] = ldpl<COH>(a.Cold + qof(j));
+            if (own && ya - 4 + j < h) a.Cnew[qof(j)] = a.Cold[qof(j)];
         return;
     }
     const bool lazy = a.A2 != nullptr;
@@ -135,15 +139,15 @@ __device__ __forceinline__ void grow_replace_strip(const GrowArgs& a, const int*
         // strip, so with no flagged strip among this one and its 8 neighbours nothing is fresh here.
         bool f = false;
         if (lane < 9) {
-            const int ny = sy - 1 + lane / 3, nx = sx - 1 + lane % 3;
-            if (ny >= 0 && ny < (h + WG_R - 1) / WG_R && nx >= 0 && nx < nsx)
-                f = ldpl<COH>(a.stripflag + ny * nsx + nx) != 0;
+            const int sy = blockIdx.y * WG_WARPS + wi - 1 + lane / 3, sx = (int)blockIdx.x - 1 + lane % 3;
+            if (sy >= 0 && sy < (h + WG_R - 1) / WG_R && sx >= 0 && sx < (int)gridDim.x)
+                f = a.stripflag[sy * gridDim.x + sx] != 0;
         }
         if (!__any_sync(FULL, f)) {
 #pragma unroll
             for (int j = 4; j < 4 + WG_R; ++j)
                 if (own && ya - 4 + j < h) {
-                    a.Cnew[qof(j)] = ldpl<COH>(a.Cold + qof(j));
+                    a.Cnew[qof(j)] = a.Cold[qof(j)];
                     a.NEED[qof(j)] = 0u;
                 }
             return;
@@ -200,7 +204,7 @@ __device__ __forceinline__ void grow_replace_strip(const GrowArgs& a, const int*
             warp_for_each_bit<2, WG_J - 2>(todo, s_list, lane, [&](int j, int sl, int bit) {
                 const int y = ya - 4 + j, x = (wxh + sl) * 32 + bit;
                 int c1, c2;
-                count_sp<COH>(a.S, y, x, h, w, a.siglow, a.siglow, c1, c2);
+                count_sp(a.S, y, x, h, w, a.siglow, a.siglow, c1, c2);
                 if (c2 >= 13) atomicOr(&s_plane[(j - 2) * 32 + sl], 1u << bit);
             });
 #pragma unroll
@@ -211,7 +215,7 @@ __device__ __forceinline__ void grow_replace_strip(const GrowArgs& a, const int*
             for (int j = 4; j < 4 + WG_R; ++j)
                 if (nb[j] && own && ya - 4 + j < h) {
                     a.G2[qof(j)] = g2[j];
-                    a.G2F[qof(j)] = ldpl<COH>(a.G2F + qof(j)) | (nb[j] & ~g2[j]);
+                    a.G2F[qof(j)] |= nb[j] & ~g2[j];
                 }
         }
     }
@@ -301,18 +305,6 @@ __device__ __forceinline__ void grow_replace_strip(const GrowArgs& a, const int*
     });
 }
 
-#ifndef LAC_GROW_MINB
-#define LAC_GROW_MINB 3
-#endif
-__global__ void __launch_bounds__(32 * WG_WARPS, LAC_GROW_MINB)
-k_grow_replace(GrowArgs a, const int* prev_count) {
-    __shared__ uint32_t s_plane_all[WG_WARPS][(WG_R + 4) * 32];   // G2, then C', rows ya-2 .. ya+WG_R+1
-    __shared__ int s_list_all[WG_WARPS][WG_LCAP];
-    const int wi = threadIdx.x >> 5;
-    grow_replace_strip<false>(a, prev_count, blockIdx.x, blockIdx.y * WG_WARPS + wi, gridDim.x, s_plane_all[wi],
-                              s_list_all[wi]);
-}
-
 // ------------------------------------------------------------------------------------------------
 // warp-aggregated append of the set bits of bits[J0..J1) (pixel index p0 + (j - J0) * w + bit) to a global
 // list: one atomicAdd per warp that has something to append
@@ -353,26 +345,16 @@ __device__ __forceinline__ void warp_append(const uint32_t (&bits)[WG_J], int p0
 //        structure test reads work within 4 px).  G1, G2, G2F, M1 are cleared inside R and the pixels of A1 in
 //        R outside the quads (their A1 is unchanged) go to the candidate list.
 // Same warp-autonomous layout as k_grow_replace.
-struct DirtyArgs {
-    const uint32_t *NEED, *A1;
-    uint32_t *G1, *G2, *G2F, *M1;
-    int *qlist, *nq, *clist, *nc;
-    uint8_t* stripflag;
-    int h, w, wpr;
-};
-
-template <bool COH>
-__device__ __forceinline__ void dirty_lists_strip(const DirtyArgs& d, const int* prev_count, int sx, int sy, int nsx) {
-    if (prev_count && ldpl<COH>(prev_count) == 0) return;
-    const uint32_t* NEED = d.NEED;
-    const uint32_t* A1 = d.A1;
-    uint32_t *G1 = d.G1, *G2 = d.G2, *G2F = d.G2F, *M1 = d.M1;
-    int *qlist = d.qlist, *nq = d.nq, *clist = d.clist, *nc = d.nc;
-    const int h = d.h, w = d.w, wpr = d.wpr;
-    const int lane = threadIdx.x & 31;
-    const int wx = sx * WG_OWN - 1 + lane;
-    const int ya = sy * WG_R;
-    if (ya >= h) return;                                      // warp-uniform; no block barrier in here
+__global__ void __launch_bounds__(32 * WG_WARPS, 3)
+k_dirty_lists(const uint32_t* __restrict__ NEED, const uint32_t* __restrict__ A1, uint32_t* __restrict__ G1,
+              uint32_t* __restrict__ G2, uint32_t* __restrict__ G2F, uint32_t* __restrict__ M1,
+              int* __restrict__ qlist, int* __restrict__ nq, int* __restrict__ clist, int* __restrict__ nc,
+              uint8_t* __restrict__ stripflag, int h, int w, int wpr, const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    const int wx = blockIdx.x * WG_OWN - 1 + lane;
+    const int ya = (blockIdx.y * WG_WARPS + wi) * WG_R;
+    if (ya >= h) return;                                      // warp-uniform; no block barrier in this kernel
     const bool colok = wx >= 0 && wx < wpr;
     const bool own = lane >= 1 && lane <= WG_OWN && colok;
     const int wxc = clampi(wx, 0, wpr - 1);
@@ -381,11 +363,11 @@ __device__ __forceinline__ void dirty_lists_strip(const DirtyArgs& d, const int*
 #pragma unroll
     for (int j = 0; j < WG_J; ++j) {
         const int y = ya - 4 + j;
-        const uint32_t v = ldpl<COH>(NEED + (size_t)clampi(y, 0, h - 1) * wpr + wxc);
+        const uint32_t v = NEED[(size_t)clampi(y, 0, h - 1) * wpr + wxc];
         h2[j] = (colok && y >= 0 && y < h) ? v : 0u;
         any |= h2[j] != 0;
     }
-    uint8_t* flag = d.stripflag + (size_t)sy * nsx + sx;
+    uint8_t* flag = stripflag + (size_t)(blockIdx.y * WG_WARPS + wi) * gridDim.x + blockIdx.x;
     if (!__any_sync(FULL, any)) {                             // nothing was rewritten near this strip
         if (lane == 0) *flag = 0;
         return;
@@ -396,8 +378,7 @@ __device__ __forceinline__ void dirty_lists_strip(const DirtyArgs& d, const int*
 #pragma unroll
     for (int k = 0; k < WG_R; ++k) {
         const size_t q = (size_t)min(ya + k, h - 1) * wpr + wxc;
-        a1[k] = ldpl<COH>(A1 + q); g1[k] = ldpl<COH>(G1 + q); g2[k] = ldpl<COH>(G2 + q); g2f[k] = ldpl<COH>(G2F + q);
-        m1[k] = ldpl<COH>(M1 + q);
+        a1[k] = A1[q]; g1[k] = G1[q]; g2[k] = G2[q]; g2f[k] = G2F[q]; m1[k] = M1[q];
     }
 #pragma unroll
     for (int j = 0; j < WG_J; ++j) {
@@ -444,11 +425,6 @@ __device__ __forceinline__ void dirty_lists_strip(const DirtyArgs& d, const int*
     const int p0 = ya * w + wx * 32;
     warp_append<4, 4 + WG_R>(quads, p0, w, qlist, nq, lane);
     warp_append<4, 4 + WG_R>(cand, p0, w, clist, nc, lane);
-}
-
-__global__ void __launch_bounds__(32 * WG_WARPS, 3)
-k_dirty_lists(DirtyArgs d, const int* prev_count) {
-    dirty_lists_strip<false>(d, prev_count, blockIdx.x, blockIdx.y * WG_WARPS + (threadIdx.x >> 5), gridDim.x);
 }
 
 }  // namespace lac

@@ -333,9 +333,8 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         if (incr) {
             {
                 Span sp(KC_LISTS, st);
-                lac::DirtyArgs da{ws.NEED, ws.A1, ws.G1, ws.G2, ws.G2F, ws.M1, ws.qlist, ws.nquad + t, ws.clist, ws.ncand + t,
-                                  ws.stripflag, h, w, wpr};
-                lac::k_dirty_lists<<<grow_grid(h, w), 32 * lac::WG_WARPS, 0, st>>>(da, prev);
+                lac::k_dirty_lists<<<grow_grid(h, w), 32 * lac::WG_WARPS, 0, st>>>(ws.NEED, ws.A1, ws.G1, ws.G2, ws.G2F, ws.M1, ws.qlist,
+                                                                   ws.nquad + t, ws.clist, ws.ncand + t, ws.stripflag, h, w, wpr, prev);
                 LAUNCHED();
             }
             {

@@ -171,17 +171,24 @@ __device__ __forceinline__ bool fine_bracket(float lp, float m3c, float objlim, 
 // Virtual 9x9 window V[r][c] = work<y-4+r, x-4+c>; the m3-plane tap (dy, dx) of the 7x7 window is med3x3
 // centred on the virtual position (cy(dy), cx(dx)), cy(dy) = clamp(y+dy) - y (R4: the STORED m3 plane is
 // replicated), whose own taps are V[cy+4+-1][cx+4+-1] (R3).
-template <bool COH>
-__device__ __forceinline__ void eval_candidate(const CandArgs& a, int p) {
+#ifndef LAC_EVAL_MINB
+#define LAC_EVAL_MINB 6
+#endif
+__global__ void __launch_bounds__(128, LAC_EVAL_MINB)
+k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restrict__ nlist,
+                  const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;
+    const int n = *nlist;
     const int h = a.h, w = a.w;
-    {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const int p = list[i];
         const int y = p / w, x = p - y * w;
         int c1, c2;
-        count_sp<COH>(a.S, y, x, h, w, a.sigclip, a.siglow, c1, c2);
+        count_sp(a.S, y, x, h, w, a.sigclip, a.siglow, c1, c2);
         const uint32_t bit = 1u << (x & 31);
         const size_t q = (size_t)y * a.wpr + (x >> 5);
         if (c2 >= 13) atomicOr(a.G2 + q, bit);
-        if (c1 < 13) return;
+        if (c1 < 13) continue;
         atomicOr(a.G1 + q, bit);
         uint32_t rows[9];   // bit c of rows[r] = P(V[r][c])
         float tlo, thi;
@@ -194,17 +201,17 @@ __device__ __forceinline__ void eval_candidate(const CandArgs& a, int p) {
             for (int r = 0; r < 3; ++r)
 #pragma unroll
                 for (int c = 0; c < 3; ++c)
-                    ctr[r][c] = ldro<COH>(a.work + (size_t)clampi(y + r - 1, 0, h - 1) * w + xx[3 + c]);
+                    ctr[r][c] = __ldg(a.work + (size_t)clampi(y + r - 1, 0, h - 1) * w + xx[3 + c]);
             const float lp = lplus_px(ctr[1][1], ctr[0][1], ctr[2][1], ctr[1][0], ctr[1][2]);
             const float m3c = med9(ctr[0][0], ctr[0][1], ctr[0][2], ctr[1][0], ctr[1][1], ctr[1][2], ctr[2][0],
                                    ctr[2][1], ctr[2][2]);
-            if (!fine_bracket(lp, m3c, a.objlim, tlo, thi)) return;
+            if (!fine_bracket(lp, m3c, a.objlim, tlo, thi)) continue;
 #pragma unroll 3
             for (int r = 0; r < 9; ++r) {
                 const float* row = a.work + (size_t)clampi(y + r - 4, 0, h - 1) * w;
                 float f[9];
 #pragma unroll
-                for (int c = 0; c < 9; ++c) f[c] = ldro<COH>(row + xx[c]);
+                for (int c = 0; c < 9; ++c) f[c] = __ldg(row + xx[c]);
                 const uint32_t m = fine_bits<9>(f, lp, m3c, a.objlim, tlo, thi);
 #pragma unroll
                 for (int k = 0; k < 9; ++k) rows[k] = (k == r) ? m : rows[k];
@@ -214,33 +221,18 @@ __device__ __forceinline__ void eval_candidate(const CandArgs& a, int p) {
     }
 }
 
-// the listed pixels, grid-stride
-template <bool COH>
-__device__ __forceinline__ void eval_candidates(const CandArgs& a, const int* list, int n) {
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
-        eval_candidate<COH>(a, ldpl<COH>(list + i));
-}
-
-#ifndef LAC_EVAL_MINB
-#define LAC_EVAL_MINB 6
-#endif
-__global__ void __launch_bounds__(128, LAC_EVAL_MINB)
-k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restrict__ nlist,
-                  const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;
-    eval_candidates<false>(a, list, *nlist);
-}
-
 // ------------------------------------------------------------------------------------------------
 // Incremental steps (1)-(3a) (iterations t >= 1): S, A1, A2 are recomputed only on the listed quads (aligned
 // groups of 4 pixels holding a pixel within 2 px of a rewritten one; k_dirty_lists), one quad per thread, with
 // the same window network and the same operations as the dense pass (kernels.cuh, noise_S_tile).  The
 // pixels of the quad with S > sigclip are appended to the candidate list (one atomic per CTA and round).
-template <bool COH>
-__device__ __forceinline__ void noise_S_quads(const float* work, const NoiseArgs& a, const int* qlist, int n,
-                                              int* clist, int* nc, int* s_warp, int* s_base_p) {
-    int& s_base = *s_base_p;
-    const int h = a.h, w = a.w;
+__global__ void __launch_bounds__(256, 4)
+k_noise_S_quads(const float* __restrict__ work, NoiseArgs a, const int* __restrict__ qlist,
+                const int* __restrict__ nq, int* __restrict__ clist, int* __restrict__ nc, const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;
+    __shared__ int s_warp[8];
+    __shared__ int s_base;
+    const int n = *nq, h = a.h, w = a.w;
     const int tid = threadIdx.x, lane = tid & 31, wi = tid >> 5;
     const bool vec = (w & 3) == 0;
     for (int base = blockIdx.x * 256; base < n; base += gridDim.x * 256) {   // uniform trip count per CTA
@@ -248,16 +240,16 @@ __device__ __forceinline__ void noise_S_quads(const float* work, const NoiseArgs
         uint32_t n1 = 0;
         int p = 0;
         if (i < n) {
-            p = ldpl<COH>(qlist + i);
+            p = qlist[i];
             const int y = p / w, x = p - y * w;
             float win[8][5];   // win[c][r] = work<y-2+r, x-2+c>
             if (vec && x >= 4 && x + 8 <= w && y >= 2 && y + 2 < h) {
 #pragma unroll
                 for (int r = 0; r < 5; ++r) {
                     const float* row = work + (size_t)(y - 2 + r) * w + (x - 4);
-                    const float4 q0 = ldpl<COH>(reinterpret_cast<const float4*>(row));
-                    const float4 q1 = ldpl<COH>(reinterpret_cast<const float4*>(row + 4));
-                    const float4 q2 = ldpl<COH>(reinterpret_cast<const float4*>(row + 8));
+                    const float4 q0 = *reinterpret_cast<const float4*>(row);
+                    const float4 q1 = *reinterpret_cast<const float4*>(row + 4);
+                    const float4 q2 = *reinterpret_cast<const float4*>(row + 8);
                     const float v[12] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w, q2.x, q2.y, q2.z, q2.w};
 #pragma unroll
                     for (int c = 0; c < 8; ++c) win[c][r] = v[2 + c];
@@ -270,7 +262,7 @@ __device__ __forceinline__ void noise_S_quads(const float* work, const NoiseArgs
                 for (int r = 0; r < 5; ++r) {
                     const float* row = work + (size_t)clampi(y - 2 + r, 0, h - 1) * w;
 #pragma unroll
-                    for (int c = 0; c < 8; ++c) win[c][r] = ldpl<COH>(row + xx[c]);
+                    for (int c = 0; c < 8; ++c) win[c][r] = row[xx[c]];
                 }
             }
             float m5[4], s[4];
@@ -288,7 +280,7 @@ __device__ __forceinline__ void noise_S_quads(const float* work, const NoiseArgs
             // this thread alone owns its nibble of the A1 / A2 words; the other nibbles change concurrently
             const size_t q = (size_t)y * a.wpr + (x >> 5);
             const int sh = x & 31;
-            const uint32_t o1 = (ldpl<COH>(a.A1 + q) >> sh) & 0xFu, o2 = (ldpl<COH>(a.A2 + q) >> sh) & 0xFu;
+            const uint32_t o1 = (a.A1[q] >> sh) & 0xFu, o2 = (a.A2[q] >> sh) & 0xFu;
             if (o1 != n1) atomicXor(a.A1 + q, (o1 ^ n1) << sh);
             if (o2 != n2) atomicXor(a.A2 + q, (o2 ^ n2) << sh);
         }
@@ -318,15 +310,6 @@ __device__ __forceinline__ void noise_S_quads(const float* work, const NoiseArgs
             if ((n1 >> j) & 1u) clist[o++] = p + j;
         __syncthreads();   // s_warp / s_base are rewritten in the next round
     }
-}
-
-__global__ void __launch_bounds__(256, 4)
-k_noise_S_quads(const float* __restrict__ work, NoiseArgs a, const int* __restrict__ qlist,
-                const int* __restrict__ nq, int* __restrict__ clist, int* __restrict__ nc, const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;
-    __shared__ int s_warp[8];
-    __shared__ int s_base;
-    noise_S_quads<false>(work, a, qlist, *nq, clist, nc, s_warp, &s_base);
 }
 
 }  // namespace lac

@@ -9,10 +9,9 @@ namespace lac {
 // Plain scalar taps: on B200 they beat covering each window row with aligned 16-byte vectors and selecting
 // the taps by a shift (fewer bytes per lane and no select chains; measured in k_eval_candidates and
 // k_grow_replace).
-template <bool COH = false>
-__device__ __forceinline__ void count_sp(const float* S, int y, int x, int h, int w, float sigclip,
+__device__ __forceinline__ void count_sp(const float* __restrict__ S, int y, int x, int h, int w, float sigclip,
                                          float siglow, int& c1, int& c2) {
-    const float sc = ldro<COH>(S + (size_t)y * w + x);
+    const float sc = __ldg(S + (size_t)y * w + x);
     int xx[5];
 #pragma unroll
     for (int d = 0; d < 5; ++d) xx[d] = clampi(x + d - 2, 0, w - 1);
@@ -23,7 +22,7 @@ __device__ __forceinline__ void count_sp(const float* S, int y, int x, int h, in
         const float* row = S + (size_t)clampi(y + dy - 2, 0, h - 1) * w;
 #pragma unroll
         for (int dx = 0; dx < 5; ++dx) {
-            const float sp = __fsub_rn(sc, ldro<COH>(row + xx[dx]));
+            const float sp = __fsub_rn(sc, __ldg(row + xx[dx]));
             c1 += sp > sigclip;
             c2 += sp > siglow;
         }
