@@ -119,15 +119,21 @@ def _workload(name):
 
 
 # ------------------------------------------------------------------------------------------- oracle legs
-def _oracle_sample(img, params, rows):
+def _oracle_sample(img, params, rows, threads=None):
     """Time the oracle, as it stands, on the top `rows` rows of the frame (a bounded sample)."""
     from oracle import lacosmic_oracle as orc   # allowed here: cpu_baseline / --impl reference legs
     orc.build()
     crop = np.ascontiguousarray(img[:rows])
+    allthreads = orc.max_threads()
+    if threads:
+        orc.set_threads(threads)
     t0 = time.perf_counter()
     orc.run(crop, **params)
     dt = time.perf_counter() - t0
-    return dt, crop.size, orc.max_threads()
+    used = orc.max_threads()
+    if threads:
+        orc.set_threads(allthreads)
+    return dt, crop.size, used
 
 
 def run_reference(args):
@@ -459,6 +465,10 @@ def run_cuda(args):
         cpu = dict(value=(px / npx) / dt, unit="frames/s", cores=cores, kind="oracle",
                    sample="top %d of %d rows of the same frame, one run, %.1f s; frames/s scaled by "
                           "pixel count" % (rows, h, dt))
+        rows1 = min(h, 100)                      # also one thread, on a smaller sample
+        dt1, px1, c1 = _oracle_sample(frame.img, params, rows1, threads=1)
+        cpu["single_thread"] = dict(value=(px1 / npx) / dt1, unit="frames/s", cores=c1,
+                                    sample="top %d rows, one run, %.1f s" % (rows1, dt1))
 
     main_sum = summarise(res)
     line = dict(
