@@ -640,3 +640,20 @@ def test_random_differential(lc, orc, seed):
             if np.all(o["counts"][:dbg_iter] > 0):     # the library skips iterations after a fixed point (R17)
                 for k in planes:
                     assert np.array_equal(_n(g[k]), o[k]), (seed, mode, k, p)
+
+
+@pytest.mark.parametrize("mode", [0, 1], ids=["lazy", "dense"])
+def test_maximum_niter(lc, orc, mode):
+    """niter = LACOSMIC_MAX_NITER (64): the library skips the iterations after the fixed point on the device
+    (R17), the oracle executes all of them; results and counts must agree, and niter + 1 is rejected."""
+    import torch
+    f = synth.make_frame(90, 124, seed=33, n_star=6, n_cr=60, n_hot=10, sp_frac=0.01)
+    p = dict(PARAMS, niter=64)
+    o = orc.run(f.img, **p)
+    g = lc.lacosmic_run_ws(_t(f.img), lc.Params(mode=mode, **p))
+    torch.cuda.synchronize()
+    assert np.array_equal(_n(g["mask"]), o["mask"]) and np.array_equal(_n(g["clean"]), o["clean"])
+    assert np.array_equal(_n(g["counts"])[:64], o["counts"]) and o["counts"][-1] == 0
+    with pytest.raises(lc.LacosmicError) as e:
+        lc.lacosmic_run_ws(_t(f.img), lc.Params(mode=mode, **dict(PARAMS, niter=65)))
+    assert e.value.code == -3
