@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     LacosmicError,
     Params,
     lacosmic_bitplane_pitch_words,
+    lacosmic_clean,
     lacosmic_dilate3,
     lacosmic_estimate_gain,
     lacosmic_host_workspace_bytes,

@@ -358,6 +358,27 @@ def lacosmic_run_host_stream_sparse(imgs_host, params, capacity=None, out=None, 
     return out
 
 
+def lacosmic_clean(image, gain=1.0, readnoise=10.0, sigclip=4.5, sigfrac=0.3, objlim=5.0, niter=4,
+                   satlevel=65535.0, device="cuda:0"):
+    """The user-level entry point of the paper (one call with objlim, sigfrac, sigclip and
+    optional gain / readnoise): a 2-D numpy array (float32, or the detector's uint16 counts) in, (mask bool
+    [h][w], cleaned float32 [h][w]) numpy arrays out.  gain=0 (or None): estimated at each iteration.  Every
+    step runs in the CUDA library (lacosmic_run_host*); this wrapper only stages pinned host buffers."""
+    import numpy as np
+    torch = _torch()
+    a = np.ascontiguousarray(image)
+    if a.ndim != 2:
+        raise ValueError("image must be 2-D")
+    if a.dtype != np.uint16:
+        a = a.astype(np.float32, copy=False)
+    p = Params(gain=0.0 if gain is None else float(gain), readnoise=readnoise, sigclip=sigclip, sigfrac=sigfrac,
+               objlim=objlim, satlevel=satlevel, niter=niter)
+    with torch.cuda.device(device):
+        r = lacosmic_run_host(torch.from_numpy(a).pin_memory(), p, device=device)
+        torch.cuda.current_stream().synchronize()
+    return r["mask"].numpy().astype(bool), r["clean"].numpy()
+
+
 def lacosmic_host_batch_workspace_bytes(h, w, concurrency):
     return int(load_library().lacosmic_host_batch_workspace_bytes(int(h), int(w), int(concurrency)))
 

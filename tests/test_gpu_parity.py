@@ -657,3 +657,16 @@ def test_maximum_niter(lc, orc, mode):
     with pytest.raises(lc.LacosmicError) as e:
         lc.lacosmic_run_ws(_t(f.img), lc.Params(mode=mode, **dict(PARAMS, niter=65)))
     assert e.value.code == -3
+
+
+def test_user_level_entry_point(lc, orc):
+    """lacosmic_clean: the paper's one-call interface on numpy arrays, fp32 and uint16 input,
+    supplied and estimated gain."""
+    f = synth.make_frame(150, 210, seed=44, n_star=10, n_cr=120, sp_frac=0.004)
+    for img, kw in ((f.img, {}), (f.img, dict(gain=None, sigclip=5.0)),
+                    (np.clip(np.rint(f.img), 0, 65535).astype(np.uint16), dict(objlim=4.0))):
+        mask, clean = lc.lacosmic_clean(img, **kw)
+        p = dict(PARAMS, **{k: (0.0 if v is None else v) for k, v in kw.items()})
+        o = orc.run(img.astype(np.float32), **p)
+        assert mask.dtype == bool and np.array_equal(mask, o["mask"].astype(bool))
+        assert clean.dtype == np.float32 and np.array_equal(clean, o["clean"])
