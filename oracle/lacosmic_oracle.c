@@ -210,7 +210,6 @@ float orc_sigma_clip(const float *r, size_t n, int rounds, float *stats) {
     return s;
 }
 
-/* gain estimate of one image (the `work` plane of an iteration).  stats: nullable float[5], see above. */
 /* gain estimate of one image (the `work` plane of an iteration).  stats: nullable float[6] = the sigma-clip
  * statistics above plus stats[5] = mt.  The noise model of O2 is var(work) = signal/gain + (rn/gain)^2, so
  * with sigma^2 = var(r) = var(work)/signal:  sigma^2 gain^2 - gain - rn^2/mt = 0, mt = the typical signal =

@@ -419,6 +419,42 @@ def test_p13_sigma_clip_is_order_independent_and_rank_based(orc):
     assert 0.9 < s0 < 1.1 and st0[4] <= 4001 + 1          # the 50-sigma cluster is clipped away, sigma ~ 1
 
 
+def _gain_cases():
+    cases, cur = [], None
+    for ln in open(os.path.join(GOLDEN, "gain_estimate_cases.txt")):
+        ln = ln.strip()
+        if not ln or ln.startswith("#"):
+            continue
+        key, _, rest = ln.partition(" ")
+        if key == "case":
+            cur = dict(name=rest, rows=[])
+            cases.append(cur)
+        elif key == "shape":
+            cur["shape"] = tuple(int(v) for v in rest.split())
+        elif key == "row":
+            cur["rows"].append([float(v) for v in rest.split()])
+        elif key == "rn":
+            cur["rn"] = float(rest)
+        elif key == "expect":
+            cur["expect"] = [float(v) for v in rest.split()]
+    return cases
+
+
+@pytest.mark.parametrize("case", _gain_cases(), ids=lambda c: c["name"])
+def test_p13_hand_computed_gain_estimate(orc, case):
+    """tests/golden/gain_estimate_cases.txt: a frame small enough to do on paper, rn > 0, one clipped outlier whose
+    med5 differs from the kept majority's.  Pins the read-noise root of R21 (the factor 4, the 2 s^2) and the
+    restriction of the typical signal mt to the set the last clipping round kept."""
+    img = np.array(case["rows"], np.float32)
+    assert img.shape == case["shape"]
+    g, st = orc.estimate_gain(img, case["rn"])
+    g_e, c_e, s_e, lo_e, hi_e, kept_e, mt_e = case["expect"]
+    assert st[0] == np.float32(c_e) and st[4] == kept_e and st[5] == np.float32(mt_e)
+    assert abs(st[1] - s_e) <= 1e-6 * s_e
+    assert abs(st[2] - lo_e) <= 1e-6 * abs(lo_e) and abs(st[3] - hi_e) <= 1e-6 * abs(hi_e)
+    assert abs(float(g) - g_e) <= 2e-6 * g_e, (float(g), g_e)
+
+
 @pytest.mark.parametrize("gain", [0.5, 2.0, 7.0])
 def test_p13_gain_of_pure_poisson_like_noise_is_recovered(orc, gain):
     """Closed form behind R21: var(work) = signal/gain => (work - med5)/sqrt(med5) has sigma 1/sqrt(gain).  The
