@@ -7,6 +7,7 @@ library raises LacosmicError (there is deliberately no fallback of any kind).
 from __future__ import annotations
 
 import ctypes as C
+import functools
 import os
 from dataclasses import dataclass
 
@@ -145,6 +146,29 @@ def _stream(stream):
     return getattr(stream, "cuda_stream", stream)
 
 
+def _scratch_on(t, stream):
+    """Scratch this module allocated itself is dropped when the wrapper returns, while the work enqueued on `stream`
+    still uses it.  The caching allocator only orders reuse against the stream a block was allocated on (torch's
+    current stream); for any other stream the block must be recorded on it, or it can be handed out again while
+    the kernels still run."""
+    if stream is None:
+        return t
+    torch = _torch()
+    st = stream if isinstance(stream, torch.cuda.Stream) else torch.cuda.ExternalStream(int(stream), device=t.device)
+    t.record_stream(st)
+    return t
+
+
+def _on_device(fn):
+    """Host-buffer entry points take device=...: make it the current device for the call (the library works on the
+    current device, and stream=None means that device's current stream)."""
+    @functools.wraps(fn)
+    def wrapped(*args, device="cuda:0", **kw):
+        with _torch().cuda.device(device):
+            return fn(*args, device=device, **kw)
+    return wrapped
+
+
 def _check(rc, where):
     if rc != 0:
         raise LacosmicError(rc, where)
@@ -213,7 +237,7 @@ def lacosmic_run_ws(img, params=None, mask_out=None, clean_out=None, workspace=N
     if clean_out is None:
         clean_out = torch.empty_like(img)
     if workspace is None:
-        workspace = _workspace(h, w, img.device)
+        workspace = _scratch_on(_workspace(h, w, img.device), stream)
     if iter_counts is None:
         iter_counts = torch.zeros(max(int(p.niter), 1), dtype=torch.int32, device=img.device)
     out = dict(mask=mask_out, clean=clean_out, counts=iter_counts)
@@ -257,8 +281,8 @@ def lacosmic_run_batch(imgs, params, masks_out=None, cleans_out=None, workspace=
     if cleans_out is None:
         cleans_out = torch.empty_like(imgs)
     if workspace is None:
-        workspace = torch.empty(max(lacosmic_batch_workspace_bytes(h, w, max(1, concurrency)), 256),
-                                dtype=torch.uint8, device=imgs.device)
+        workspace = _scratch_on(torch.empty(max(lacosmic_batch_workspace_bytes(h, w, max(1, concurrency)), 256),
+                                            dtype=torch.uint8, device=imgs.device), stream)
     if iter_counts is None:
         iter_counts = torch.zeros((max(n, 1), MAX_NITER), dtype=torch.int32, device=imgs.device)
     rc = L.lacosmic_run_batch(_dev(imgs, torch.float32, "imgs"), n, h, w, arr,
@@ -270,6 +294,7 @@ def lacosmic_run_batch(imgs, params, masks_out=None, cleans_out=None, workspace=
     return dict(mask=masks_out, clean=cleans_out, counts=iter_counts)
 
 
+@_on_device
 def lacosmic_run_host(img_host, params=None, mask_out_host=None, clean_out_host=None,
                       dev_workspace=None, device="cuda:0", stream=None, **kw):
     """End-to-end call with HOST (ideally pinned) torch CPU tensors; copies are part of the call.  img_host is
@@ -286,7 +311,7 @@ def lacosmic_run_host(img_host, params=None, mask_out_host=None, clean_out_host=
     if clean_out_host is None:
         clean_out_host = torch.empty((h, w), dtype=torch.float32).pin_memory()
     if dev_workspace is None:
-        dev_workspace = _workspace(h, w, device, host=True)
+        dev_workspace = _scratch_on(_workspace(h, w, device, host=True), stream)
     cp = p._c()
     fn = L.lacosmic_run_host_u16 if img_host.dtype == torch.uint16 else L.lacosmic_run_host
     rc = fn(img_host.data_ptr(), h, w, C.byref(cp), mask_out_host.data_ptr(),
@@ -296,6 +321,7 @@ def lacosmic_run_host(img_host, params=None, mask_out_host=None, clean_out_host=
     return dict(mask=mask_out_host, clean=clean_out_host)
 
 
+@_on_device
 def lacosmic_run_host_sparse(img_host, params=None, capacity=None, out=None, dev_workspace=None,
                              device="cuda:0", stream=None, **kw):
     """Sparse results (host tensors): dict(maskbits int32 [h][pitch], idx int32 [capacity], val float32
@@ -316,7 +342,7 @@ def lacosmic_run_host_sparse(img_host, params=None, capacity=None, out=None, dev
                    val=torch.empty(max(cap, 1), dtype=torch.float32).pin_memory(),
                    count=torch.zeros(1, dtype=torch.int32).pin_memory(), capacity=cap)
     if dev_workspace is None:
-        dev_workspace = _workspace(h, w, device, host=True)
+        dev_workspace = _scratch_on(_workspace(h, w, device, host=True), stream)
     cp = p._c()
     rc = L.lacosmic_run_host_sparse(img_host.data_ptr(), h, w, C.byref(cp), out["maskbits"].data_ptr(),
                                     out["idx"].data_ptr(), out["val"].data_ptr(), out["count"].data_ptr(),
@@ -326,6 +352,7 @@ def lacosmic_run_host_sparse(img_host, params=None, capacity=None, out=None, dev
     return out
 
 
+@_on_device
 def lacosmic_run_host_stream_sparse(imgs_host, params, capacity=None, out=None, dev_workspace=None,
                                     device="cuda:0", stream=None, concurrency=3):
     """Stream of host frames [n][h][w] (float32 or uint16), sparse results per frame: dict(maskbits int32
@@ -347,8 +374,8 @@ def lacosmic_run_host_stream_sparse(imgs_host, params, capacity=None, out=None, 
                    val=torch.empty((n, max(cap, 1)), dtype=torch.float32).pin_memory(),
                    count=torch.zeros(n, dtype=torch.int32).pin_memory(), capacity=cap)
     if dev_workspace is None:
-        dev_workspace = torch.empty(max(lacosmic_host_batch_workspace_bytes(h, w, max(1, concurrency)), 256),
-                                    dtype=torch.uint8, device=device)
+        dev_workspace = _scratch_on(torch.empty(max(lacosmic_host_batch_workspace_bytes(h, w, max(1, concurrency)), 256),
+                                                dtype=torch.uint8, device=device), stream)
     rc = L.lacosmic_run_host_stream_sparse(imgs_host.data_ptr(), int(imgs_host.dtype == torch.uint16), n, h, w, arr,
                                            out["maskbits"].data_ptr(), out["idx"].data_ptr(), out["val"].data_ptr(),
                                            out["count"].data_ptr(), int(out["capacity"]),
@@ -374,8 +401,10 @@ def lacosmic_clean(image, gain=1.0, readnoise=10.0, sigclip=4.5, sigfrac=0.3, ob
     p = Params(gain=0.0 if gain is None else float(gain), readnoise=readnoise, sigclip=sigclip, sigfrac=sigfrac,
                objlim=objlim, satlevel=satlevel, niter=niter)
     with torch.cuda.device(device):
-        r = lacosmic_run_host(torch.from_numpy(a).pin_memory(), p, device=device)
+        pinned = torch.from_numpy(a).pin_memory()          # stays referenced until the copy has completed
+        r = lacosmic_run_host(pinned, p, device=device)
         torch.cuda.current_stream().synchronize()
+    del pinned
     return r["mask"].numpy().astype(bool), r["clean"].numpy()
 
 
@@ -383,6 +412,7 @@ def lacosmic_host_batch_workspace_bytes(h, w, concurrency):
     return int(load_library().lacosmic_host_batch_workspace_bytes(int(h), int(w), int(concurrency)))
 
 
+@_on_device
 def lacosmic_run_host_batch(imgs_host, params, masks_host=None, cleans_host=None, dev_workspace=None,
                             device="cuda:0", stream=None, concurrency=3):
     """Stream of frames in HOST (ideally pinned) tensors [n][h][w]; params: list of n Params.  `concurrency`
@@ -401,8 +431,8 @@ def lacosmic_run_host_batch(imgs_host, params, masks_host=None, cleans_host=None
     if cleans_host is None:
         cleans_host = torch.empty((n, h, w), dtype=torch.float32).pin_memory()
     if dev_workspace is None:
-        dev_workspace = torch.empty(max(lacosmic_host_batch_workspace_bytes(h, w, max(1, concurrency)), 256),
-                                    dtype=torch.uint8, device=device)
+        dev_workspace = _scratch_on(torch.empty(max(lacosmic_host_batch_workspace_bytes(h, w, max(1, concurrency)), 256),
+                                                dtype=torch.uint8, device=device), stream)
     rc = L.lacosmic_run_host_batch(imgs_host.data_ptr(), n, h, w, arr, masks_host.data_ptr(),
                                    cleans_host.data_ptr(), _dev(dev_workspace, torch.uint8, "dev_workspace"),
                                    dev_workspace.numel(), _stream(stream))
@@ -416,7 +446,7 @@ def lacosmic_estimate_gain(img, readnoise=0.0, workspace=None, stream=None):
     torch = _torch()
     h, w = img.shape
     if workspace is None:
-        workspace = _workspace(h, w, img.device)
+        workspace = _scratch_on(_workspace(h, w, img.device), stream)
     gain = torch.zeros(1, dtype=torch.float32, device=img.device)
     stats = torch.zeros(6, dtype=torch.float32, device=img.device)
     _check(load_library().lacosmic_estimate_gain(
@@ -485,7 +515,7 @@ def lacosmic_masked_median(img, mask_u8, out=None, workspace=None, stream=None):
     if out is None:
         out = torch.empty_like(img)
     if workspace is None:
-        workspace = _workspace(h, w, img.device)
+        workspace = _scratch_on(_workspace(h, w, img.device), stream)
     _check(load_library().lacosmic_masked_median(
         _dev(img, torch.float32, "img"), _dev(mask_u8, torch.uint8, "mask_u8", (h, w)),
         _dev(out, torch.float32, "out", (h, w)), h, w, _dev(workspace, torch.uint8, "workspace"),

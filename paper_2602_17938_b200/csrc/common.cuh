@@ -8,6 +8,16 @@ namespace lac {
 
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return min(max(v, lo), hi); }
 
+// 2-D CTA coordinates out of a 1-D grid of nbx * nby CTAs: gridDim.y stops at 65535, which a tall, narrow frame
+// (rows on y) would exceed; gridDim.x reaches 2^31 - 1, enough for every shape the boundary accepts.
+struct BlockXY { int x, y; };
+__device__ __forceinline__ BlockXY block_xy(int nbx) {
+    BlockXY b;
+    b.y = (int)(blockIdx.x / (unsigned)nbx);
+    b.x = (int)(blockIdx.x - (unsigned)b.y * (unsigned)nbx);
+    return b;
+}
+
 // compare-exchange: a <- min, b <- max (two FMNMX on the ALU pipe)
 __device__ __forceinline__ void ce(float& a, float& b) {
     float t = fminf(a, b);

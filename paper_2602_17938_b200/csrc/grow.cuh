@@ -98,6 +98,7 @@ struct GrowArgs {
     const uint8_t* stripflag;     // nullable: per strip, set by k_dirty_lists when R is not empty in it
     int h, w, wpr;
     float siglow;
+    int nbx;                      // strips per row of strips = CTAs per row of CTAs (1-D grid, block_xy)
 };
 
 #ifndef LAC_GROW_MINB
@@ -107,9 +108,10 @@ __global__ void __launch_bounds__(32 * WG_WARPS, LAC_GROW_MINB)
 k_grow_replace(GrowArgs a, const int* prev_count) {
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const int h = a.h, w = a.w, wpr = a.wpr;
-    const int wxh = blockIdx.x * WG_OWN - 1;                 // word column of lane 0
+    const BlockXY bk = block_xy(a.nbx);
+    const int wxh = bk.x * WG_OWN - 1;                       // word column of lane 0
     const int wx = wxh + lane;
-    const int ya = (blockIdx.y * WG_WARPS + wi) * WG_R;       // first own row
+    const int ya = (bk.y * WG_WARPS + wi) * WG_R;             // first own row
     if (ya >= h) return;                                      // warp-uniform; the kernel has no block barrier
     const bool colok = wx >= 0 && wx < wpr;
     const bool own = lane >= 1 && lane <= WG_OWN && colok;
@@ -139,9 +141,9 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
         // strip, so with no flagged strip among this one and its 8 neighbours nothing is fresh here.
         bool f = false;
         if (lane < 9) {
-            const int sy = blockIdx.y * WG_WARPS + wi - 1 + lane / 3, sx = (int)blockIdx.x - 1 + lane % 3;
-            if (sy >= 0 && sy < (h + WG_R - 1) / WG_R && sx >= 0 && sx < (int)gridDim.x)
-                f = a.stripflag[sy * gridDim.x + sx] != 0;
+            const int sy = bk.y * WG_WARPS + wi - 1 + lane / 3, sx = bk.x - 1 + lane % 3;
+            if (sy >= 0 && sy < (h + WG_R - 1) / WG_R && sx >= 0 && sx < a.nbx)
+                f = a.stripflag[(size_t)sy * a.nbx + sx] != 0;
         }
         if (!__any_sync(FULL, f)) {
 #pragma unroll
@@ -349,11 +351,12 @@ __global__ void __launch_bounds__(32 * WG_WARPS, 3)
 k_dirty_lists(const uint32_t* __restrict__ NEED, const uint32_t* __restrict__ A1, uint32_t* __restrict__ G1,
               uint32_t* __restrict__ G2, uint32_t* __restrict__ G2F, uint32_t* __restrict__ M1,
               int* __restrict__ qlist, int* __restrict__ nq, int* __restrict__ clist, int* __restrict__ nc,
-              uint8_t* __restrict__ stripflag, int h, int w, int wpr, const int* prev_count) {
+              uint8_t* __restrict__ stripflag, int h, int w, int wpr, int nbx, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
-    const int wx = blockIdx.x * WG_OWN - 1 + lane;
-    const int ya = (blockIdx.y * WG_WARPS + wi) * WG_R;
+    const BlockXY bk = block_xy(nbx);
+    const int wx = bk.x * WG_OWN - 1 + lane;
+    const int ya = (bk.y * WG_WARPS + wi) * WG_R;
     if (ya >= h) return;                                      // warp-uniform; no block barrier in this kernel
     const bool colok = wx >= 0 && wx < wpr;
     const bool own = lane >= 1 && lane <= WG_OWN && colok;
@@ -367,7 +370,7 @@ k_dirty_lists(const uint32_t* __restrict__ NEED, const uint32_t* __restrict__ A1
         h2[j] = (colok && y >= 0 && y < h) ? v : 0u;
         any |= h2[j] != 0;
     }
-    uint8_t* flag = stripflag + (size_t)(blockIdx.y * WG_WARPS + wi) * gridDim.x + blockIdx.x;
+    uint8_t* flag = stripflag + (size_t)(bk.y * WG_WARPS + wi) * nbx + bk.x;
     if (!__any_sync(FULL, any)) {                             // nothing was rewritten near this strip
         if (lane == 0) *flag = 0;
         return;

@@ -76,11 +76,12 @@ __device__ __forceinline__ void store4q(float* __restrict__ dst, size_t row_off,
 // kernels.  Each thread produces 4 adjacent outputs from a (k+3) x k register window.
 template <int K>
 __global__ void __launch_bounds__(NT) k_medfilt(const float* __restrict__ in, float* __restrict__ out,
-                                               int h, int w) {
+                                               int h, int w, int nbx) {
     constexpr int R = K / 2, MX = 4, PITCH = TW + 2 * MX;
     __shared__ __align__(16) float sm[(TH + 2 * R) * PITCH];
     const int tid = threadIdx.x, lane = tid & 31, wi = tid >> 5;
-    const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
+    const BlockXY bk = block_xy(nbx);
+    const int x0 = bk.x * TW, y0 = bk.y * TH;
     load_tile<MX, R, PITCH>(sm, in, h, w, y0, x0, tid);
     __syncthreads();
 #pragma unroll 1
@@ -96,8 +97,9 @@ __global__ void __launch_bounds__(NT) k_medfilt(const float* __restrict__ in, fl
 
 // Standalone L+ (lacosmic_lplus).
 __global__ void __launch_bounds__(NT) k_lplus(const float* __restrict__ in, float* __restrict__ out,
-                                             int h, int w) {
-    int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
+                                             int h, int w, int nbx) {
+    const BlockXY bk = block_xy(nbx);
+    int x = bk.x * 32 + (threadIdx.x & 31), y = bk.y * 8 + (threadIdx.x >> 5);
     if (x >= w || y >= h) return;
     const float* row = in + (size_t)y * w;
     float c = row[x];
@@ -331,14 +333,15 @@ __device__ __forceinline__ void fine_gates_tile(const float* smA, float* smB, co
 
 // generic path (any w): one tile per CTA, tiles loaded with clamped scalar loads
 __global__ void __launch_bounds__(NT)
-k_fine_gates(const float* __restrict__ work, const float* __restrict__ S, FineArgs a,
+k_fine_gates(const float* __restrict__ work, const float* __restrict__ S, FineArgs a, int nbx,
              const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     __shared__ __align__(16) float smA[FG_AROWS * FG_PA];
     __shared__ __align__(16) float smB[FG_BROWS * FG_PB];
     __shared__ __align__(16) float smS[FG_SROWS * FG_PS];
     const int tid = threadIdx.x;
-    const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
+    const BlockXY bk = block_xy(nbx);
+    const int x0 = bk.x * TW, y0 = bk.y * TH;
     load_tile<FG_AX, FG_AY, FG_PA>(smA, work, a.h, a.w, y0, x0, tid);
     load_tile<FG_SX, FG_SY, FG_PS>(smS, S, a.h, a.w, y0, x0, tid);
     __syncthreads();
@@ -500,12 +503,13 @@ __device__ __forceinline__ float one_S_px(float c, float U, float D, float Lf, f
 // consecutive rows in registers (sliding down), horizontal neighbours come from the adjacent lanes.
 constexpr int SM5_ROWS = 16;
 __global__ void __launch_bounds__(256)
-k_S_from_m5(const float* __restrict__ work, NoiseArgs a, const int* prev_count) {
+k_S_from_m5(const float* __restrict__ work, NoiseArgs a, int nbx, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const int h = a.h, w = a.w;
-    const int x = blockIdx.x * 128 + 4 * lane;
-    const int ya = (blockIdx.y * 8 + wi) * SM5_ROWS;
+    const BlockXY bk = block_xy(nbx);
+    const int x = bk.x * 128 + 4 * lane;
+    const int ya = (bk.y * 8 + wi) * SM5_ROWS;
     if (ya >= h) return;                          // warp-uniform
     const bool inx = x < w;                       // w % 4 == 0: a quad is inside or outside as a whole
     const int xc = inx ? x : w - 4;               // out-of-frame lanes read a valid quad; results unused
@@ -548,11 +552,12 @@ k_S_from_m5(const float* __restrict__ work, NoiseArgs a, const int* prev_count) 
 
 // any w: one thread per aligned group of 4 pixels, clamped scalar loads
 __global__ void __launch_bounds__(256)
-k_S_from_m5_generic(const float* __restrict__ work, NoiseArgs a, const int* prev_count) {
+k_S_from_m5_generic(const float* __restrict__ work, NoiseArgs a, int nbx, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const int h = a.h, w = a.w;
-    const int x = blockIdx.x * 128 + 4 * lane, y = blockIdx.y * 8 + wi;
+    const BlockXY bk = block_xy(nbx);
+    const int x = bk.x * 128 + 4 * lane, y = bk.y * 8 + wi;
     if (y >= h) return;                           // warp-uniform
     const float gain = a.gain_dev ? __ldg(a.gain_dev) : a.gain;
     const float* rc = work + (size_t)y * w;
@@ -587,9 +592,10 @@ k_S_from_m5_generic(const float* __restrict__ work, NoiseArgs a, const int* prev
 // common.cuh (8 words of one column of words per thread; the horizontally dilated rows are shared between
 // them).  The whole path runs the same word arithmetic inside k_grow_replace (grow.cuh).
 __global__ void __launch_bounds__(256)
-k_dilate3(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, int h, int w, int wpr) {
+k_dilate3(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, int h, int w, int wpr, int nbx) {
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
-    const int wx = blockIdx.x * 32 + lane, y0 = blockIdx.y * BW_CTA_ROWS + wi * BW_ROWS;
+    const BlockXY bk = block_xy(nbx);
+    const int wx = bk.x * 32 + lane, y0 = bk.y * BW_CTA_ROWS + wi * BW_ROWS;
     if (wx >= wpr || y0 >= h) return;
     uint32_t res[BW_ROWS];
     dilate_rows<1>(in, y0, wx, h, wpr, res);
@@ -644,8 +650,9 @@ k_unpack_bits(const uint32_t* __restrict__ bits, uint8_t* __restrict__ u8, int h
 }
 
 __global__ void __launch_bounds__(256)
-k_pack_bits(const uint8_t* __restrict__ u8, uint32_t* __restrict__ bits, int h, int w, int wpr) {
-    int x = blockIdx.x * 256 + threadIdx.x, y = blockIdx.y;
+k_pack_bits(const uint8_t* __restrict__ u8, uint32_t* __restrict__ bits, int h, int w, int wpr, int nbx) {
+    const BlockXY bk = block_xy(nbx);
+    int x = bk.x * 256 + threadIdx.x, y = bk.y;
     bool b = (x < w) && (u8[(size_t)y * w + x] != 0);
     uint32_t word = __ballot_sync(0xffffffffu, b);
     if ((threadIdx.x & 31) == 0 && (x >> 5) < wpr) bits[(size_t)y * wpr + (x >> 5)] = word;

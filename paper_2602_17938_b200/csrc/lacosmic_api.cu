@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <mutex>
 
 #include "kernels.cuh"
 #include "lazy.cuh"
@@ -93,26 +94,32 @@ struct DeviceInfo {
     bool ok = false;
 };
 
-const DeviceInfo& device_info() {
-    static DeviceInfo info = []() {
-        DeviceInfo d;
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return d;
-        if (cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return d;
-        if (cudaFuncSetAttribute(lac::k_fine_gates_tma, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 lac::FG_SMEM_BYTES) != cudaSuccess) return d;
-        if (cudaFuncSetAttribute(lac::k_noise_S_tma, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 lac::NS_SMEM_BYTES) != cudaSuccess) return d;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_fine, lac::k_fine_gates_tma, lac::NT,
-                                                          lac::FG_SMEM_BYTES) != cudaSuccess) return d;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_noise, lac::k_noise_S_tma, lac::NT,
-                                                          lac::NS_SMEM_BYTES) != cudaSuccess) return d;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_quads, lac::k_noise_S_quads, 256, 0) != cudaSuccess) return d;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_eval, lac::k_eval_candidates, 128, 0) != cudaSuccess) return d;
-        d.ok = d.sms > 0 && d.occ_fine > 0 && d.occ_noise > 0 && d.occ_quads > 0 && d.occ_eval > 0;
-        return d;
-    }();
-    return info;
+// Per-device: the SM count, the occupancy of the persistent kernels and the opt-in to > 48 KB of dynamic shared
+// memory (a per-device function attribute) belong to the CURRENT device, which may differ from call to call.
+constexpr int MAX_DEVICES = 64;
+DeviceInfo device_info() {
+    static DeviceInfo infos[MAX_DEVICES];
+    static std::mutex mu;
+    const DeviceInfo bad;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEVICES) return bad;
+    std::lock_guard<std::mutex> lock(mu);
+    DeviceInfo& d = infos[dev];
+    if (d.ok) return d;
+    d = DeviceInfo();
+    if (cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return d;
+    if (cudaFuncSetAttribute(lac::k_fine_gates_tma, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             lac::FG_SMEM_BYTES) != cudaSuccess) return d;
+    if (cudaFuncSetAttribute(lac::k_noise_S_tma, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             lac::NS_SMEM_BYTES) != cudaSuccess) return d;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_fine, lac::k_fine_gates_tma, lac::NT,
+                                                      lac::FG_SMEM_BYTES) != cudaSuccess) return d;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_noise, lac::k_noise_S_tma, lac::NT,
+                                                      lac::NS_SMEM_BYTES) != cudaSuccess) return d;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_quads, lac::k_noise_S_quads, 256, 0) != cudaSuccess) return d;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_eval, lac::k_eval_candidates, 128, 0) != cudaSuccess) return d;
+    d.ok = d.sms > 0 && d.occ_fine > 0 && d.occ_noise > 0 && d.occ_quads > 0 && d.occ_eval > 0;
+    return d;
 }
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -193,11 +200,14 @@ int unpack(const uint32_t* bits, uint8_t* u8, int h, int w, cudaStream_t st, con
 }
 
 // grid of the bit-plane list kernels: 32 words x 64 rows per CTA (common.cuh)
-inline dim3 bit_grid(int h, int w) { return dim3((words_per_row(w) + 31) / 32, (h + lac::BW_CTA_ROWS - 1) / lac::BW_CTA_ROWS); }
+// (1-D grids of nbx * nby CTAs, block_xy in common.cuh: rows on gridDim.y would stop at 65535 rows of CTAs)
+inline int bit_nbx(int w) { return (words_per_row(w) + 31) / 32; }
+inline unsigned bit_grid(int h, int w) { return (unsigned)bit_nbx(w) * (unsigned)((h + lac::BW_CTA_ROWS - 1) / lac::BW_CTA_ROWS); }
 // grid of k_grow_replace / k_dirty_lists: 30 words x 64 rows per CTA, one 30 x 8 strip per warp (grow.cuh)
-inline dim3 grow_grid(int h, int w) {
+inline int grow_nbx(int w) { return (words_per_row(w) + lac::WG_OWN - 1) / lac::WG_OWN; }
+inline unsigned grow_grid(int h, int w) {
     const int rows = lac::WG_R * lac::WG_WARPS;
-    return dim3((words_per_row(w) + lac::WG_OWN - 1) / lac::WG_OWN, (h + rows - 1) / rows);
+    return (unsigned)grow_nbx(w) * (unsigned)((h + rows - 1) / rows);
 }
 
 // steps (6)-(7) of one iteration, fused (grow.cuh)
@@ -274,10 +284,11 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     const float siglow = p.sigfrac * p.sigclip;   // R9: one fp32 multiply on the host
     const float rn2 = p.readnoise * p.readnoise;
     lac::GateParams gp{p.sigclip, siglow, p.objlim, p.satlevel};
-    dim3 tb(lac::NT), tg((w + lac::TW - 1) / lac::TW, (h + lac::TH - 1) / lac::TH);
+    dim3 tb(lac::NT);
+    const int tgx = (w + lac::TW - 1) / lac::TW, tgy = (h + lac::TH - 1) / lac::TH;
     // TMA path needs 16-byte row pitch; other widths take the generic tile loader
     const bool tma = (w % 4 == 0);
-    const int ntx = (int)tg.x, ntiles = (int)(tg.x * tg.y);
+    const int ntx = tgx, ntiles = tgx * tgy;
     const int ntilesNS = ntx * ((h + lac::NS_TH - 1) / lac::NS_TH);   // tiles of the noise/S pass
     CUtensorMap mapWorkNS, mapImgNS, mapWorkFG, mapS;
     int gridNS = 0, gridFG = 0, gridQ = 1184, gridE = 2368;
@@ -334,7 +345,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
             {
                 Span sp(KC_LISTS, st);
                 lac::k_dirty_lists<<<grow_grid(h, w), 32 * lac::WG_WARPS, 0, st>>>(ws.NEED, ws.A1, ws.G1, ws.G2, ws.G2F, ws.M1, ws.qlist,
-                                                                   ws.nquad + t, ws.clist, ws.ncand + t, ws.stripflag, h, w, wpr, prev);
+                                                                   ws.nquad + t, ws.clist, ws.ncand + t, ws.stripflag, h, w, wpr, grow_nbx(w), prev);
                 LAUNCHED();
             }
             {
@@ -346,8 +357,9 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
             if (estimate) {
                 // the residual pass left med5(work) in the S plane: S, A1, A2 follow elementwise (HBM bound)
                 Span sp(KC_NOISE_S, st);
-                if (tma) lac::k_S_from_m5<<<dim3((w + 127) / 128, (h + 8 * lac::SM5_ROWS - 1) / (8 * lac::SM5_ROWS)), 256, 0, st>>>(work, na, prev);
-                else lac::k_S_from_m5_generic<<<dim3((w + 127) / 128, (h + 7) / 8), 256, 0, st>>>(work, na, prev);
+                const unsigned nbx = (unsigned)((w + 127) / 128);
+                if (tma) lac::k_S_from_m5<<<nbx * (unsigned)((h + 8 * lac::SM5_ROWS - 1) / (8 * lac::SM5_ROWS)), 256, 0, st>>>(work, na, (int)nbx, prev);
+                else lac::k_S_from_m5_generic<<<nbx * (unsigned)((h + 7) / 8), 256, 0, st>>>(work, na, (int)nbx, prev);
                 LAUNCHED();
             } else if ((rc = noise_pass(na, src))) {
                 return rc;
@@ -355,7 +367,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
             if (lazy) {
                 Span sp(KC_LISTS, st);
                 lac::k_list_candidates<<<bit_grid(h, w), 256, 0, st>>>(ws.A1, (t > 0 && !estimate) ? ws.NEED : nullptr, ws.G1, ws.G2, ws.G2F, ws.M1,
-                                                                      ws.clist, ws.ncand + t, t == 0 ? ws.C[0] : nullptr, h, w, wpr, prev);
+                                                                      ws.clist, ws.ncand + t, t == 0 ? ws.C[0] : nullptr, h, w, wpr, bit_nbx(w), prev);
                 LAUNCHED();
             }
         }
@@ -370,14 +382,14 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                              d ? dbg->F : nullptr, h, w, wpr, gp};
             Span sp(KC_FINE_GATES, st);
             if (tma) lac::k_fine_gates_tma<<<gridFG, tb, lac::FG_SMEM_BYTES, st>>>(mapWorkFG, mapS, fa, ntx, ntiles, prev);
-            else lac::k_fine_gates<<<tg, tb, 0, st>>>(work, ws.S, fa, prev);
+            else lac::k_fine_gates<<<(unsigned)ntiles, tb, 0, st>>>(work, ws.S, fa, ntx, prev);
             LAUNCHED();
         }
         if (d && dbg->S) CK(cudaMemcpyAsync(dbg->S, ws.S, P * 4, cudaMemcpyDeviceToDevice, st));
         // steps (6)-(7), fused; in the lazy path G2 is completed on the pixels the second growth reaches
         lac::GrowArgs ga{ws.M1, ws.G1, ws.G2, ws.G2F, lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
                          ws.C[t & 1], ws.C[(t + 1) & 1], ws.NEED, d ? ws.M2 : nullptr, d ? ws.M3 : nullptr,
-                         ws.S, img, work, ws.counts + t, incr ? ws.stripflag : nullptr, h, w, wpr, siglow};
+                         ws.S, img, work, ws.counts + t, incr ? ws.stripflag : nullptr, h, w, wpr, siglow, grow_nbx(w)};
         if ((rc = grow_replace(ga, prev, st))) return rc;
         if (d) {
             // lazy path: G2 is only evaluated where step (6) needs it, so it is not dumped
@@ -793,8 +805,8 @@ int lacosmic_lplus(const float* in, float* out, int h, int w, void* stream) {
     int rc = check_shape(h, w);
     if (rc) return rc;
     if (overlap(in, (size_t)h * w * 4, out, (size_t)h * w * 4)) return LACOSMIC_ERR_ALIAS;
-    dim3 g((w + 31) / 32, (h + 7) / 8), b(256);
-    lac::k_lplus<<<g, b, 0, (cudaStream_t)stream>>>(in, out, h, w);
+    const unsigned nbx = (unsigned)((w + 31) / 32);
+    lac::k_lplus<<<nbx * (unsigned)((h + 7) / 8), 256, 0, (cudaStream_t)stream>>>(in, out, h, w, (int)nbx);
     LAUNCHED();
     return LACOSMIC_OK;
 }
@@ -805,11 +817,13 @@ int lacosmic_medfilt(const float* in, float* out, int h, int w, int k, void* str
     if (rc) return rc;
     if (k != 3 && k != 5 && k != 7) return LACOSMIC_ERR_PARAM;
     if (overlap(in, (size_t)h * w * 4, out, (size_t)h * w * 4)) return LACOSMIC_ERR_ALIAS;
-    dim3 tb(lac::NT), tg((w + lac::TW - 1) / lac::TW, (h + lac::TH - 1) / lac::TH);
+    const int nbx = (w + lac::TW - 1) / lac::TW;
+    const unsigned tg = (unsigned)nbx * (unsigned)((h + lac::TH - 1) / lac::TH);
+    dim3 tb(lac::NT);
     cudaStream_t st = (cudaStream_t)stream;
-    if (k == 3) lac::k_medfilt<3><<<tg, tb, 0, st>>>(in, out, h, w);
-    else if (k == 5) lac::k_medfilt<5><<<tg, tb, 0, st>>>(in, out, h, w);
-    else lac::k_medfilt<7><<<tg, tb, 0, st>>>(in, out, h, w);
+    if (k == 3) lac::k_medfilt<3><<<tg, tb, 0, st>>>(in, out, h, w, nbx);
+    else if (k == 5) lac::k_medfilt<5><<<tg, tb, 0, st>>>(in, out, h, w, nbx);
+    else lac::k_medfilt<7><<<tg, tb, 0, st>>>(in, out, h, w, nbx);
     LAUNCHED();
     return LACOSMIC_OK;
 }
@@ -820,8 +834,8 @@ int lacosmic_pack_bits(const uint8_t* mask_u8, uint32_t* bits, int h, int w, voi
     if (!mask_u8 || !bits) return LACOSMIC_ERR_NULL;
     int rc = check_shape(h, w);
     if (rc) return rc;
-    dim3 g((w + 255) / 256, h);
-    lac::k_pack_bits<<<g, 256, 0, (cudaStream_t)stream>>>(mask_u8, bits, h, w, words_per_row(w));
+    const unsigned nbx = (unsigned)((w + 255) / 256);
+    lac::k_pack_bits<<<nbx * (unsigned)h, 256, 0, (cudaStream_t)stream>>>(mask_u8, bits, h, w, words_per_row(w), (int)nbx);
     LAUNCHED();
     return LACOSMIC_OK;
 }
@@ -839,7 +853,7 @@ int lacosmic_dilate3(const uint32_t* bits_in, uint32_t* bits_out, int h, int w, 
     if (rc) return rc;
     int wpr = words_per_row(w);
     if (overlap(bits_in, (size_t)h * wpr * 4, bits_out, (size_t)h * wpr * 4)) return LACOSMIC_ERR_ALIAS;
-    lac::k_dilate3<<<bit_grid(h, w), 256, 0, (cudaStream_t)stream>>>(bits_in, bits_out, h, w, wpr);
+    lac::k_dilate3<<<bit_grid(h, w), 256, 0, (cudaStream_t)stream>>>(bits_in, bits_out, h, w, wpr, bit_nbx(w));
     LAUNCHED();
     return LACOSMIC_OK;
 }
@@ -863,7 +877,7 @@ int lacosmic_masked_median(const float* img, const uint8_t* mask_u8, float* out,
     CK(cudaMemsetAsync(ws.C[0], 0, (size_t)h * wpr * 4, st));
     CK(cudaMemsetAsync(ws.counts, 0, 4, st));
     lac::GrowArgs ga{ws.M1, ws.M1, ws.M1, nullptr, nullptr, nullptr, ws.C[0], ws.C[1], ws.NEED, nullptr, nullptr,
-                     nullptr, img, out, ws.counts, nullptr, h, w, wpr, 0.0f};
+                     nullptr, img, out, ws.counts, nullptr, h, w, wpr, 0.0f, grow_nbx(w)};
     return grow_replace(ga, nullptr, st);
 }
 

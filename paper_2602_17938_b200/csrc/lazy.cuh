@@ -34,10 +34,11 @@ namespace lac {
 __global__ void __launch_bounds__(256)
 k_list_candidates(const uint32_t* __restrict__ A1, const uint32_t* __restrict__ dirty, uint32_t* __restrict__ G1,
                   uint32_t* __restrict__ G2, uint32_t* __restrict__ G2F, uint32_t* __restrict__ M1, int* __restrict__ list,
-                  int* __restrict__ nlist, uint32_t* __restrict__ Czero, int h, int w, int wpr, const int* prev_count) {
+                  int* __restrict__ nlist, uint32_t* __restrict__ Czero, int h, int w, int wpr, int nbx, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
-    const int wx = blockIdx.x * 32 + lane, y0 = blockIdx.y * BW_CTA_ROWS + wi * BW_ROWS;
+    const BlockXY bk = block_xy(nbx);
+    const int wx = bk.x * 32 + lane, y0 = bk.y * BW_CTA_ROWS + wi * BW_ROWS;
     uint32_t bits[BW_ROWS];
 #pragma unroll
     for (int i = 0; i < BW_ROWS; ++i) bits[i] = 0;

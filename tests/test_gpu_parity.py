@@ -216,6 +216,73 @@ def test_dense_candidates_low_thresholds(lc, orc, mode):
     _compare_run(lc, orc, np.round(f.img / 8) * 8, dict(PARAMS, sigclip=1.0, objlim=1.0), 1, "quantised", mode)
 
 
+@pytest.mark.parametrize("shape", [(70001, 5), (3, 300007), (1100000, 1)])
+def test_very_tall_and_very_wide_frames(lc, orc, shape):
+    """Row counts beyond what gridDim.y can hold (65535 rows of CTAs): every kernel takes its rows from a 1-D grid.
+    Whole path in both modes, the single steps, bit packing with more than 65535 rows."""
+    import torch
+    h, w = shape
+    rng = _rng(88)
+    img = (100.0 + 10.0 * rng.standard_normal(shape)).astype(np.float32)
+    hits = rng.integers(0, h * w, h * w // 200)
+    img.flat[hits] += rng.uniform(300, 5000, hits.size).astype(np.float32)
+    for mode in MODES:
+        _compare_run(lc, orc, img, PARAMS, None, str(shape), mode)
+    m = (rng.random(shape) < 0.02).astype(np.uint8)
+    bits = lc.lacosmic_pack_bits(_t(m))
+    assert np.array_equal(_n(bits), _pack_np(m))
+    assert np.array_equal(_n(lc.lacosmic_unpack_bits(lc.lacosmic_dilate3(bits, h, w), h, w)), orc.dilate3(m))
+    assert np.array_equal(_n(lc.lacosmic_masked_median(_t(img), _t(m))), orc.masked_median(img, m))
+    assert np.array_equal(_n(lc.lacosmic_lplus(_t(img))), orc.lplus(img))
+    assert np.array_equal(_n(lc.lacosmic_medfilt(_t(img), 5)), orc.medfilt(img, 5))
+    g, st = lc.lacosmic_estimate_gain(_t(img), readnoise=5.0)
+    torch.cuda.synchronize()
+    go, sto = orc.estimate_gain(img, 5.0)
+    assert _n(g)[0] == go and np.array_equal(_n(st), sto)
+
+
+def test_explicit_stream_with_internal_scratch(lc, orc):
+    """stream= other than torch's current stream: the scratch the wrapper allocates itself must stay valid until the
+    work enqueued on that stream has run (binding._scratch_on records it on the stream)."""
+    import torch
+    f = synth.make_frame(300, 420, seed=23, n_star=10, n_cr=200, sp_frac=0.004)
+    o = orc.run(f.img, **PARAMS)
+    side = torch.cuda.Stream()
+    img = _t(f.img)
+    torch.cuda.synchronize()
+    outs = []
+    for _ in range(4):
+        outs.append(lc.lacosmic_run_ws(img, lc.Params(**PARAMS), stream=side))
+        junk = torch.empty(lc.lacosmic_workspace_bytes(300, 420), dtype=torch.uint8, device="cuda").fill_(255)
+        del junk
+    side.synchronize()
+    torch.cuda.synchronize()
+    for g in outs:
+        assert np.array_equal(_n(g["mask"]), o["mask"]) and np.array_equal(_n(g["clean"]), o["clean"])
+    r = lc.lacosmic_run_host(torch.from_numpy(f.img).pin_memory(), lc.Params(**PARAMS), stream=side.cuda_stream)
+    side.synchronize()
+    assert np.array_equal(r["mask"].numpy(), o["mask"]) and np.array_equal(r["clean"].numpy(), o["clean"])
+
+
+def test_second_device_in_one_process(lc, orc):
+    """Per-device state (SM count, occupancy, the > 48 KB shared-memory opt-in of k_fine_gates_tma) must follow the
+    current device: dense mode on cuda:1 after cuda:0 in the same process."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    f = synth.make_frame(200, 264, seed=24, n_star=8, n_cr=100, sp_frac=0.004)
+    o = orc.run(f.img, **PARAMS)
+    for dev in ("cuda:0", "cuda:1"):
+        with torch.cuda.device(dev):
+            for mode in (lc.MODE_DENSE, lc.MODE_LAZY):
+                g = lc.lacosmic_run_ws(torch.from_numpy(f.img).to(dev), lc.Params(mode=mode, **PARAMS))
+                torch.cuda.synchronize()
+                assert np.array_equal(_n(g["mask"]), o["mask"]) and np.array_equal(_n(g["clean"]), o["clean"])
+        r = lc.lacosmic_run_host(torch.from_numpy(f.img).pin_memory(), lc.Params(**PARAMS), device=dev)
+        torch.cuda.synchronize(dev)
+        assert np.array_equal(r["mask"].numpy(), o["mask"])
+
+
 def test_rot180_invariance_on_gpu(lc):
     f = synth.make_frame(150, 170, seed=21, n_star=10, n_cr=60, n_hot=20, sp_frac=0.003)
     a = lc.lacosmic_run_ws(_t(f.img), lc.Params(**PARAMS))
@@ -366,6 +433,21 @@ def test_estimate_gain_bit_exact(lc, orc, shape):
         assert np.array_equal(_n(st), sto), (rn, _n(st), sto)
 
 
+def test_estimate_gain_hand_computed_cases(lc, orc):
+    """The hand-worked frames of tests/golden/gain_estimate_cases.txt (one clipped outlier whose med5 differs, rn > 0):
+    the GPU estimate against the file's values and, bit for bit, against the oracle."""
+    import torch
+    from test_oracle_pins import _gain_cases
+    for case in _gain_cases():
+        x = np.array(case["rows"], np.float32)
+        g, st = lc.lacosmic_estimate_gain(_t(x), readnoise=case["rn"])
+        torch.cuda.synchronize()
+        go, sto = orc.estimate_gain(x, case["rn"])
+        assert _n(g)[0] == go and np.array_equal(_n(st), sto), case["name"]
+        assert abs(float(_n(g)[0]) - case["expect"][0]) <= 2e-6 * case["expect"][0]
+        assert _n(st)[4] == case["expect"][5] and _n(st)[5] == case["expect"][6]
+
+
 def test_estimate_gain_ties_and_degenerate(lc, orc):
     import torch
     for x in (np.full((40, 50), 77.0, np.float32),                          # sigma = 0 -> gain 1
@@ -432,53 +514,46 @@ def _windows(h, w, size=192):
     return [(y, x, size) for y in ys for x in xs]
 
 
-def _check_full_frame(lc, orc, img, p, label, mode="lazy"):
-    """Sampled windows the oracle can compute one by one: the result inside a window depends only on
-    input within HALO pixels (4 iterations x radius 8 + 6), so the oracle run on the haloed crop is
-    exact on the window interior (crop edges that coincide with frame edges replicate identically)."""
+def _check_full_frame(lc, orc, img, p, label, modes=("lazy", "dense")):
+    """Whole frame, element by element, against ONE oracle run of the whole frame (about 11 s on 16 host cores for
+    26 Mpx): mask, cleaned frame and per-iteration counts must be equal over every pixel, in every requested mode,
+    in the launch configuration bench.py times."""
     import torch
-    h, w = img.shape
-    g = lc.lacosmic_run_ws(_t(img), lc.Params(mode=lc.MODE_LAZY if mode == "lazy" else lc.MODE_DENSE, **p))
-    torch.cuda.synchronize()
-    gm, gc, counts = _n(g["mask"]), _n(g["clean"]), _n(g["counts"])
-    nmask = 0
-    for (y0, x0, s) in _windows(h, w):
-        ya, yb, xa, xb = max(y0 - HALO, 0), min(y0 + s + HALO, h), max(x0 - HALO, 0), min(x0 + s + HALO, w)
-        o = orc.run(np.ascontiguousarray(img[ya:yb, xa:xb]), **p)
-        sl = (slice(y0 - ya, y0 - ya + s), slice(x0 - xa, x0 - xa + s))
-        assert np.array_equal(gm[y0:y0 + s, x0:x0 + s], o["mask"][sl]), (label, y0, x0)
-        assert np.array_equal(gc[y0:y0 + s, x0:x0 + s], o["clean"][sl]), (label, y0, x0)
-        nmask += int(o["mask"][sl].sum())
-    assert nmask > 0
-    # properties that hold at any size (P7, R11): clean is the masked median of (img, final mask);
-    # unmasked pixels untouched; counts add up to the mask size
-    assert set(np.unique(gm)) <= {0, 1}
-    assert np.array_equal(gc, orc.masked_median(img, gm))
-    assert int(counts[:p["niter"]].sum()) == int(gm.sum())
-    print(label, "mask fraction %.4f, new per iteration %s" % (gm.mean(), counts[:p["niter"]]))
+    o = orc.run(img, **p)
+    gm = None
+    for mode in modes:
+        g = lc.lacosmic_run_ws(_t(img), lc.Params(mode=lc.MODE_LAZY if mode == "lazy" else lc.MODE_DENSE, **p))
+        torch.cuda.synchronize()
+        gm, gc, counts = _n(g["mask"]), _n(g["clean"]), _n(g["counts"])
+        ndiff = int((gm != o["mask"]).sum())
+        assert ndiff == 0, "%s [%s]: %d of %d mask pixels differ" % (label, mode, ndiff, gm.size)
+        assert np.array_equal(gc, o["clean"]), (label, mode)
+        assert np.array_equal(counts[:p["niter"]], o["counts"]), (label, mode)
+        del g
+    assert int(o["counts"].sum()) == int(o["mask"].sum()) and o["mask"].sum() > 0
+    print(label, "whole frame == oracle (%d px, modes %s): mask fraction %.4f, new per iteration %s" % (
+        gm.size, "/".join(modes), gm.mean(), o["counts"]))
     return gm
 
 
-def test_config2_full_size_windows(lc, orc):
-    """Both modes in the launch configuration bench.py times; they must also agree on the whole frame."""
+def test_config2_full_size_whole_frame(lc, orc):
+    """configs[2] (the bench frame), both modes, every one of the 26 M pixels against the oracle."""
     f = synth.make_config(2)
-    gm = _check_full_frame(lc, orc, f.img, PARAMS, "configs[2]", "lazy")
+    gm = _check_full_frame(lc, orc, f.img, PARAMS, "configs[2]")
     assert gm[f.cr_truth].mean() > 0.95
-    gd = _check_full_frame(lc, orc, f.img, PARAMS, "configs[2]", "dense")
-    assert np.array_equal(gm, gd)
 
 
-def test_config4_saturation_stress_full_size(lc, orc):
+def test_config4_saturation_stress_whole_frame(lc, orc):
     f = synth.make_config(4)
     assert f.sat_truth.sum() > 1000
     gm = _check_full_frame(lc, orc, f.img, PARAMS, "configs[4]")
     assert not (gm.astype(bool) & (f.img >= np.float32(65535.0))).any(), "saturated core flagged"
 
 
-def test_transposed_orientation_windows(lc, orc):
+def test_transposed_orientation_whole_frame(lc, orc):
     """R19: PAPER.md:31 says 4000x6500 without naming the axis order; exercise 6500 rows x 4000 cols."""
     f = synth.make_frame(6500, 4000, seed=3, n_star=8000, n_cr=30000, sp_frac=0.005)
-    _check_full_frame(lc, orc, f.img, PARAMS, "6500x4000")
+    _check_full_frame(lc, orc, f.img, PARAMS, "6500x4000", modes=("lazy",))
 
 
 def test_maximum_frame_size(lc, orc):
@@ -565,8 +640,8 @@ def test_cuda_graph_capture_and_replay(lc, orc):
 def test_config3_stream_full_size(lc, orc):
     """configs[3] at full frame size, shortened to 8 frames (seeds 1000..1007, sigclip cycling 4.0/4.5/5.0 by
     seed: per-frame parameters): lacosmic_run_batch with 4 frames in flight, in the configuration bench.py's
-    stream leg times.  Frames 0, 3 and 7 are compared with the oracle on nine windows each; every frame must
-    equal the single-frame call and satisfy the size-independent properties."""
+    stream leg times.  Frames 0 and 7 are compared with the oracle over the whole frame; every frame must equal the
+    single-frame call and satisfy the size-independent properties."""
     import torch
     nf = 8
     cfg = synth.stream_config(nf)
@@ -577,7 +652,7 @@ def test_config3_stream_full_size(lc, orc):
     for j, (kw, _) in enumerate(cfg):
         f = synth.make_frame(**kw)
         imgs[j].copy_(torch.from_numpy(f.img))
-        if j in (0, 3, 7):
+        if j in (0, 7):
             host[j] = f.img
     plist = [lc.Params(**p) for _, p in cfg]
     g = lc.lacosmic_run_batch(imgs, plist, concurrency=4)
@@ -589,14 +664,10 @@ def test_config3_stream_full_size(lc, orc):
         assert np.array_equal(_n(one["counts"])[:4], _n(g["counts"][j])[:4]), j
         assert int(g["counts"][j][:4].sum()) == int(g["mask"][j].sum(dtype=torch.int64)), j
     for j, img in host.items():
-        p = cfg[j][1]
-        gm, gc = _n(g["mask"][j]), _n(g["clean"][j])
-        for (y0, x0, s) in _windows(h, w):
-            ya, yb, xa, xb = max(y0 - HALO, 0), min(y0 + s + HALO, h), max(x0 - HALO, 0), min(x0 + s + HALO, w)
-            o = orc.run(np.ascontiguousarray(img[ya:yb, xa:xb]), **p)
-            sl = (slice(y0 - ya, y0 - ya + s), slice(x0 - xa, x0 - xa + s))
-            assert np.array_equal(gm[y0:y0 + s, x0:x0 + s], o["mask"][sl]), (j, y0, x0)
-            assert np.array_equal(gc[y0:y0 + s, x0:x0 + s], o["clean"][sl]), (j, y0, x0)
+        o = orc.run(img, **cfg[j][1])
+        assert np.array_equal(_n(g["mask"][j]), o["mask"]), j
+        assert np.array_equal(_n(g["clean"][j]), o["clean"]), j
+        assert np.array_equal(_n(g["counts"][j])[:4], o["counts"]), j
 
 
 @pytest.mark.parametrize("seed", range(24))
