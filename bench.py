@@ -4,6 +4,11 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config2|config1|config0|stream]
     python bench.py --impl reference ...        # the CPU oracle on the host cores, same metric
 
+--gpus N > 1 outside a torchrun environment re-executes itself under `python -m torch.distributed.run
+--nproc-per-node N` (one rank per GPU); under torchrun the ranks come from the environment.
+--workload stream: BASELINE.json configs[3], 64 independent frames with per-frame parameters, frame i on rank
+i mod N (replicas.shard), each rank through lacosmic_run_batch; whole-job frames/s, "scaling": "strong".
+
 One "step" = one whole pass of the hot path (all section-8(a) rows: niter = 4 iterations of steps
 (1)-(7) plus frame prologue/epilogue) over one synthetic 4000x6500 fp32 frame (BASELINE.json
 configs[2]).  `value` = frames/s with the frame resident in HBM (CUDA events around each step, L2
@@ -119,42 +124,69 @@ def _workload(name):
 
 
 # ------------------------------------------------------------------------------------------- oracle legs
-def _oracle_sample(img, params, rows, threads=None):
-    """Time the oracle, as it stands, on the top `rows` rows of the frame (a bounded sample)."""
+def _oracle_frame(img, params, threads=None):
+    """Time the oracle, as it stands, on one WHOLE frame.  Returns (seconds, threads used)."""
     from oracle import lacosmic_oracle as orc   # allowed here: cpu_baseline / --impl reference legs
     orc.build()
-    crop = np.ascontiguousarray(img[:rows])
     allthreads = orc.max_threads()
     if threads:
         orc.set_threads(threads)
-    t0 = time.perf_counter()
-    orc.run(crop, **params)
-    dt = time.perf_counter() - t0
     used = orc.max_threads()
+    t0 = time.perf_counter()
+    orc.run(img, **params)
+    dt = time.perf_counter() - t0
     if threads:
         orc.set_threads(allthreads)
-    return dt, crop.size, used
+    return dt, used
+
+
+def oracle_baseline(frame_img, params):
+    """the oracle on whole frames of configs[0], [1], [2] at all host threads, and of configs[0],
+    [1] on one thread (a 26-Mpx frame takes minutes single-threaded).  The headline value is configs[2]'s."""
+    out = {}
+    for i in (0, 1):
+        f = synth.make_config(i).img
+        dt, cores = _oracle_frame(f, params)
+        dt1, _ = _oracle_frame(f, params, threads=1)
+        out["configs[%d]" % i] = dict(shape=list(f.shape), s_per_frame=dt, cores=cores, s_per_frame_1_thread=dt1,
+                                      mpix_per_s=f.size / dt / 1e6, mpix_per_s_1_thread=f.size / dt1 / 1e6)
+    dt, cores = _oracle_frame(frame_img, params)
+    out["configs[2]"] = dict(shape=list(frame_img.shape), s_per_frame=dt, cores=cores,
+                             mpix_per_s=frame_img.size / dt / 1e6)
+    return dict(value=1.0 / dt, unit="frames/s", cores=cores, kind="oracle",
+                sample="one whole frame of the bench workload (%dx%d, niter=%d), one run, %.1f s wall clock; "
+                       "whole_frames: configs[0], [1] also on one thread" % (frame_img.shape[0], frame_img.shape[1],
+                                                                            params["niter"], dt),
+                whole_frames=out)
+
+
+REFERENCE_MAX_STEPS = 5      # the oracle takes ~11 s per 26-Mpx frame on 16 cores: bound the run to about a minute
 
 
 def run_reference(args):
     rank, _, _ = replicas.env_rank_world()
     if rank != 0:                            # under torchrun rank 0 alone runs the oracle; the others exit 0
         return 0
-    wl = _workload(args.workload)
+    wl = _workload(args.workload if args.workload != "stream" else "config2")
     frame = synth.make_config(wl["cfg"])
     params = dict(synth.DEFAULT_PARAMS)
     h, w = frame.img.shape
-    rows = min(h, max(64, h // 8))          # 1/8 of the frame per step: a few seconds per step
-    times = []
-    for i in range(args.warmup + args.steps):
-        dt, px, cores = _oracle_sample(frame.img, params, rows)
-        if i >= args.warmup:
+    # every step is one WHOLE frame; the step counts are capped so that the run ends within a few minutes, and the
+    # line reports the counts actually executed (ms_per_step is a measured frame, not an extrapolation)
+    warmup = min(args.warmup, 1)
+    steps = max(1, min(args.steps, REFERENCE_MAX_STEPS))
+    times, cores = [], 0
+    for i in range(warmup + steps):
+        dt, cores = _oracle_frame(frame.img, params)
+        if i >= warmup:
             times.append(dt)
-    per_frame = statistics.mean(times) * (h * w) / px
+    per_frame = statistics.mean(times)
     value = 1.0 / per_frame
-    sample = "top %d of %d rows of the frame per step, time scaled by pixel count" % (rows, h)
+    sample = "one whole %dx%d frame per step, %d timed steps after %d warm-up (requested %d/%d)" % (
+        h, w, steps, warmup, args.steps, args.warmup)
     line = dict(impl="reference", metric=METRIC, value=value, unit="frames/s", n_gpus=args.gpus,
-                steps=args.steps, warmup=args.warmup, ms_per_step=per_frame * 1e3,
+                steps=steps, warmup=warmup, steps_requested=args.steps, warmup_requested=args.warmup,
+                ms_per_step=per_frame * 1e3,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
                 config=dict(workload=wl["label"], h=h, w=w, niter=params["niter"], sigclip=params["sigclip"],
                             sigfrac=params["sigfrac"], objlim=params["objlim"],
@@ -410,6 +442,8 @@ def run_cuda(args):
         e2e_stream["sparse_results"] = dict(call="lacosmic_run_host_stream_sparse (%d frames, %d staging slots)" % (nh, kslots),
                                             **prod)
         del imgs_h, hbws, src
+    # ---- the "alu" roofline's peak, measured in this run: fp32 min/max issue rate of this GPU (probe.cuh)
+    probe = dict(fmnmx=lc.lacosmic_probe_minmax_rate(0) / 1e12, fmnmx3=lc.lacosmic_probe_minmax_rate(1) / 1e12)
     clocks = sampler.stop() if rank == 0 else None
 
     if rank != 0:
@@ -443,8 +477,11 @@ def run_cuda(args):
         achieved = npx * ops_px / (dom_avg_ms * 1e-3) / 1e12
         return dict(bound="alu", kernel=dom, achieved=achieved, peak=alu_peak, unit="T min/max instr/s",
                     frac=achieved / alu_peak, traffic=(NCU_TRAFFIC_BYTES or {}).get(dom),
-                    peak_source="148 SM x 64 ALU lanes/clk x %.0f MHz (DESIGN.md section 5; lanes/clk "
-                                "measured in profiles/r01_alu_minmax_microbench.txt)" % sm_max,
+                    peak_source="derived: 148 SM x 64 ALU lanes/clk x %.0f MHz (DESIGN.md section 5)" % sm_max,
+                    peak_measured=probe["fmnmx"], peak_measured_fmnmx3=probe["fmnmx3"],
+                    peak_measured_source="lacosmic_probe_minmax_rate in this run (csrc/probe.cuh: register-only "
+                                         "FMNMX / FMNMX3 chains, ILP 8, 2 x 1024 threads per SM)",
+                    frac_of_measured_peak=achieved / probe["fmnmx"],
                     minmax_instr_per_px=ops_px, avg_launch_ms=dom_avg_ms, launches_timed=dom_spans)
 
     frames_per_s = world * 1e3 / res["ms"]
@@ -457,18 +494,10 @@ def run_cuda(args):
                frac=hbm_bytes_step / (res["ms"] * 1e-3) / 1e9 / peaks["hbm_gbs"])
     ref_cmp_rate = npx * REF_COMPARISONS_PER_PX_ITER * niter / (res["ms"] * 1e-3) / 1e12
 
-    # ---- the oracle on the host cores: a bounded sample of the same frame
+    # ---- the oracle on the host cores, whole frames
     cpu = None
     if not args.no_cpu_baseline:
-        rows = min(h, 1000)
-        dt, px, cores = _oracle_sample(frame.img, params, rows)
-        cpu = dict(value=(px / npx) / dt, unit="frames/s", cores=cores, kind="oracle",
-                   sample="top %d of %d rows of the same frame, one run, %.1f s; frames/s scaled by "
-                          "pixel count" % (rows, h, dt))
-        rows1 = min(h, 100)                      # also one thread, on a smaller sample
-        dt1, px1, c1 = _oracle_sample(frame.img, params, rows1, threads=1)
-        cpu["single_thread"] = dict(value=(px1 / npx) / dt1, unit="frames/s", cores=c1,
-                                    sample="top %d rows, one run, %.1f s" % (rows1, dt1))
+        cpu = oracle_baseline(frame.img, params)
 
     main_sum = summarise(res)
     line = dict(
@@ -505,6 +534,116 @@ def run_cuda(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------- configs[3] stream
+def stream_job(n_frames, rank, world, run_shard, device=None):
+    """The sharded stream workload (30 arrays x >1200 frames a night): frame i
+    belongs to rank i mod world (replicas.shard), every rank runs `run_shard(indices) -> (frames done, device ms)` on
+    its own frames with NO data-path collective, and the whole-job rate is the frames all ranks did over the slowest
+    rank's time (SUM and MAX over ranks).  tests/test_replicas_gloo.py runs this with world_size 2 on gloo."""
+    mine = replicas.shard(n_frames, rank, world)
+    done, ms = run_shard(mine)
+    total = replicas.sum_over_ranks(done, world, device)
+    slowest = replicas.max_over_ranks(ms, world, device)
+    fps = replicas.job_throughput(done, ms, world, device)
+    return dict(frames_per_s=fps, frames_total=int(round(total)), ms_slowest_rank=slowest,
+                frames_this_rank=len(mine), ms_this_rank=ms, indices_this_rank=mine)
+
+
+def run_stream(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2602_17938_b200 as lc
+
+    rank, local_rank, world = replicas.env_rank_world()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    lc.load_library()
+    nf = args.stream_total
+    cfg = synth.stream_config(nf)
+    h, w = cfg[0][0]["h"], cfg[0][0]["w"]
+    npx = h * w
+    kc = max(1, args.stream_concurrency)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    sampler = ClockSampler(local_rank)
+    state = {}
+
+    def run_shard(mine):
+        n = len(mine)
+        if n == 0:
+            return 0, 0.0
+        imgs = torch.empty((n, h, w), dtype=torch.float32, device=dev)
+        for j, i in enumerate(mine):
+            imgs[j].copy_(torch.from_numpy(synth.make_frame(**cfg[i][0]).img))
+        plist = [lc.Params(mode=lc.MODE_LAZY, **cfg[i][1]) for i in mine]
+        masks = torch.empty((n, h, w), dtype=torch.uint8, device=dev)
+        cleans = torch.empty_like(imgs)
+        bcounts = torch.zeros((n, lc.MAX_NITER), dtype=torch.int32, device=dev)
+        bws = torch.empty(lc.lacosmic_batch_workspace_bytes(h, w, kc), dtype=torch.uint8, device=dev)
+
+        def step():
+            lc.lacosmic_run_batch(imgs, plist, masks_out=masks, cleans_out=cleans, workspace=bws, iter_counts=bcounts)
+        for _ in range(args.warmup):
+            step()
+        state["launches"] = lc.lacosmic_last_launch_count()
+        replicas.barrier(world, torch.cuda.synchronize)
+        if rank == 0:
+            sampler.start()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for a, b in evs:
+            flush.zero_()
+            a.record(stream)
+            step()
+            b.record(stream)
+        replicas.barrier(world, torch.cuda.synchronize)
+        state["clocks"] = sampler.stop() if rank == 0 else None
+        state["flagged"] = int(masks.sum(dtype=torch.int64).item())
+        state["new0"] = bcounts[:, 0].cpu().numpy().tolist()
+        return n * args.steps, sum(a.elapsed_time(b) for a, b in evs)
+
+    job = stream_job(nf, rank, world, run_shard, dev)
+    if world > 1:
+        dist.destroy_process_group()
+    if rank != 0:
+        return 0
+    fps = job["frames_per_s"]
+    line = dict(metric=METRIC, value=fps, unit="frames/s", n_gpus=world, steps=args.steps, warmup=args.warmup,
+                ms_per_step=job["ms_slowest_rank"] / args.steps, higher_is_better=True, scaling="strong",
+                vs_baseline=None, dtype="f32", data="synthetic",
+                config=dict(workload="configs[3]: stream of %d independent 4000x6500 fp32 frames (seeds 1000.., sigclip "
+                                     "cycling 4.0/4.5/5.0), resident in HBM, frame i on rank i mod %d" % (nf, world),
+                            h=h, w=w, niter=cfg[0][1]["niter"], frames=nf, frames_in_flight_per_gpu=kc, mode="lazy",
+                            l2="flushed between steps (256 MiB write outside the event pair); a step's input (%d frames "
+                               "x 104 MB per rank) exceeds the 126 MB L2" % job["frames_this_rank"],
+                            parallelism="replicas: frames sharded over ranks, no data-path collective"),
+                mpix_per_s=fps * npx / 1e6, ms_per_frame=job["ms_slowest_rank"] / max(job["frames_total"] / world, 1),
+                frames_per_step=nf, frames_rank0=job["frames_this_rank"],
+                gpu_launches=state.get("launches", 0) * args.steps, launches_per_step=state.get("launches", 0),
+                flagged_pixels_rank0=state.get("flagged"), clocks=state.get("clocks"),
+                e2e=None, roofline=None, cpu_baseline=None,
+                note="sharded stream leg; the roofline, e2e and cpu_baseline objects belong to the default workload "
+                     "(python bench.py)")
+    print(json.dumps(line))
+    return 0
+
+
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` (N > 1) outside a torchrun environment: start N ranks, one per GPU, the way the
+    driver does (python -m torch.distributed.run --nnodes=1 --nproc-per-node N, rendezvous on 127.0.0.1)."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 # ALU-pipe min/max instructions per output pixel of each kernel class (DESIGN.md section 5; static SASS
 # count of FMNMX/FMNMX3 per pixel, halo recomputation included) -- the per-unit figure behind
 # roofline.achieved.
@@ -526,7 +665,9 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="config2", choices=["config2", "config1", "config0"])
+    ap.add_argument("--workload", default="config2", choices=["config2", "config1", "config0", "stream"])
+    ap.add_argument("--stream-total", type=int, default=64,
+                    help="--workload stream: frames of the configs[3] stream, sharded over the ranks")
     ap.add_argument("--mode", default="lazy", choices=["lazy", "dense"],
                     help="which evaluation mode is the headline (the other is measured and reported too)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -540,6 +681,10 @@ def main():
         args.warmup = 3                          # timing rule: at least 3 warm-up steps
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "RANK" not in os.environ and "WORLD_SIZE" not in os.environ:
+        return respawn_under_torchrun(args)
+    if args.workload == "stream":
+        return run_stream(args)
     return run_cuda(args)
 
 

@@ -239,6 +239,13 @@ const char *lacosmic_version(void);
  * LACOSMIC_NUM_KERNEL_CLASSES, the summed device time ms_sum[c] and the number of spans[c] (HOST
  * arrays), and clears the record.  Class names: lacosmic_kernel_class_name(c); the last class is the
  * whole frame (copies included). */
+/* Measured peak of the "alu" roofline (the medians of PAPER.md:23,64 are fp32 min/max selection
+ * networks, bound by the rate at which the SMs issue FMNMX).  Runs a register-only kernel of independent min/max chains
+ * (kind 0: two-input FMNMX; kind 1: three-input FMNMX3) on every SM of the current device and writes the achieved
+ * thread-level instructions per second to *instr_per_s_host (HOST pointer).  Unlike every other entry point this
+ * diagnostic allocates 256 bytes of device memory, SYNCHRONISES `stream` and takes about 10 ms. */
+int lacosmic_probe_minmax_rate(int kind, double *instr_per_s_host, void *stream);
+
 #define LACOSMIC_NUM_KERNEL_CLASSES 9
 int lacosmic_kernel_timing_enable(int enable);
 int lacosmic_kernel_timing_read(float *ms_sum, int32_t *spans);

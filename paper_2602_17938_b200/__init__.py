@@ -22,6 +22,7 @@ from .binding import (  # noqa: F401
     lacosmic_masked_median,
     lacosmic_medfilt,
     lacosmic_pack_bits,
+    lacosmic_probe_minmax_rate,
     lacosmic_run,
     lacosmic_run_batch,
     lacosmic_run_host,

@@ -25,6 +25,7 @@ EXPORTS = (
     "lacosmic_dilate3", "lacosmic_masked_median", "lacosmic_strerror",
     "lacosmic_last_cuda_error", "lacosmic_last_launch_count", "lacosmic_version",
     "lacosmic_kernel_timing_enable", "lacosmic_kernel_timing_read", "lacosmic_kernel_class_name",
+    "lacosmic_probe_minmax_rate",
 )
 NUM_KERNEL_CLASSES = 9
 MODE_LAZY, MODE_DENSE = 0, 1
@@ -115,6 +116,7 @@ def load_library():
         "lacosmic_kernel_timing_enable": (i, [i]),
         "lacosmic_kernel_timing_read": (i, [vp, vp]),
         "lacosmic_kernel_class_name": (C.c_char_p, [i]),
+        "lacosmic_probe_minmax_rate": (i, [i, vp, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)      # AttributeError if the header and the library disagree
@@ -538,6 +540,15 @@ def lacosmic_version():
 def lacosmic_kernel_timing_enable(enable=True):
     _check(load_library().lacosmic_kernel_timing_enable(1 if enable else 0),
            "lacosmic_kernel_timing_enable")
+
+
+def lacosmic_probe_minmax_rate(kind=0, stream=None):
+    """Measured fp32 min/max issue rate of the current device in instructions/s (kind 0: FMNMX, 1: FMNMX3).
+    Synchronises the stream."""
+    out = C.c_double(0.0)
+    _check(load_library().lacosmic_probe_minmax_rate(int(kind), C.byref(out), _stream(stream)),
+           "lacosmic_probe_minmax_rate")
+    return float(out.value)
 
 
 def lacosmic_kernel_timing_read():

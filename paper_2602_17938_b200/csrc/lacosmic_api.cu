@@ -12,6 +12,7 @@
 #include "grow.cuh"
 #include "select.cuh"
 #include "compact.cuh"
+#include "probe.cuh"
 
 namespace {
 
@@ -924,6 +925,45 @@ const char* lacosmic_kernel_class_name(int cls) {
     static const char* names[KC_COUNT] = {"noise_S", "fine_gates", "grow_replace", "lists", "bits",
                                           "eval_candidates", "noise_S_quads", "gain_select", "whole_frame"};
     return (cls >= 0 && cls < KC_COUNT) ? names[cls] : "?";
+}
+
+int lacosmic_probe_minmax_rate(int kind, double* instr_per_s_host, void* stream) {
+    if (!instr_per_s_host) return LACOSMIC_ERR_NULL;
+    if (kind != 0 && kind != 1) return LACOSMIC_ERR_PARAM;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    float* sink = nullptr;
+    CK(cudaMalloc(&sink, 256));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = LACOSMIC_OK;
+    const int iters = 4096, reps = 3, grid = sms * lac::PROBE_CTAS_PER_SM;
+    auto launch = [&]() {
+        if (kind == 0) lac::k_probe_minmax<0><<<grid, lac::PROBE_THREADS, 0, st>>>(sink, iters, 1.0009765625f);
+        else lac::k_probe_minmax<1><<<grid, lac::PROBE_THREADS, 0, st>>>(sink, iters, 1.0009765625f);
+    };
+    double best_ms = 0.0;
+    if (!cuda_ok(cudaEventCreate(&e0)) || !cuda_ok(cudaEventCreate(&e1))) rc = LACOSMIC_ERR_CUDA;
+    if (!rc) launch();   // warm-up
+    for (int r = 0; r < reps && !rc; ++r) {
+        float ms = 0.0f;
+        if (!cuda_ok(cudaEventRecord(e0, st))) { rc = LACOSMIC_ERR_CUDA; break; }
+        launch();
+        if (!cuda_ok(cudaGetLastError()) || !cuda_ok(cudaEventRecord(e1, st)) || !cuda_ok(cudaEventSynchronize(e1)) ||
+            !cuda_ok(cudaEventElapsedTime(&ms, e0, e1))) { rc = LACOSMIC_ERR_CUDA; break; }
+        if (r == 0 || ms < best_ms) best_ms = ms;
+    }
+    if (!rc && best_ms > 0.0) {
+        const double instr = (double)grid * lac::PROBE_THREADS * (double)iters * lac::PROBE_STAGES_PER_ITER * 8.0;
+        *instr_per_s_host = instr / (best_ms * 1e-3);
+    } else if (!rc) {
+        rc = LACOSMIC_ERR_CUDA;
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(sink);
+    return rc;
 }
 
 int lacosmic_last_cuda_error(void) { return g_last_cuda_error; }
