@@ -351,3 +351,214 @@ done:
     free(G1); free(G2); free(M1); free(D); free(M2); free(M3);
     return rc;
 }
+
+/* ======================================================================================================
+ * SURVEY.md 8(f)-3 / 8(f)-4 variants (readings R22-R26).  Everything above is untouched: orc_run
+ * stays the definition of the north-star path; orc_run_ex below restates the same loop with the variant
+ * branches written in, and a pin checks that with no variant selected it equals orc_run bit for bit.
+ * ====================================================================================================== */
+
+/* R26: separable k x k median (the approximation PAPER.md:29,37 argues AGAINST; comparison only):
+ * T[y][x] = middle element of the k values X<y, x+dx>, |dx| <= (k-1)/2 (row pass);
+ * out[y][x] = middle element of the k values T<y+dy, x>, |dy| <= (k-1)/2 (column pass on the stored T plane). */
+int orc_sepmedfilt(const float *X, float *out, int h, int w, int k) {
+    if (!(k == 3 || k == 5 || k == 7) || h < 1 || w < 1) return ORC_ERR_ARG;
+    int r = (k - 1) / 2;
+    float *T = malloc((size_t)h * w * 4);
+    if (!T) return ORC_ERR_MEM;
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < h; ++y) {
+        float v[7];
+        for (int x = 0; x < w; ++x) {
+            for (int dx = -r; dx <= r; ++dx) v[dx + r] = rd(X, h, w, y, x + dx);
+            sort_ascending(v, k);
+            T[(size_t)y * w + x] = v[r];
+        }
+    }
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < h; ++y) {
+        float v[7];
+        for (int x = 0; x < w; ++x) {
+            for (int dy = -r; dy <= r; ++dy) v[dy + r] = rd(T, h, w, y + dy, x);
+            sort_ascending(v, k);
+            out[(size_t)y * w + x] = v[r];
+        }
+    }
+    free(T);
+    return ORC_OK;
+}
+
+/* R25: extended saturated-star mask.  core = (med5(img) >= satlevel): the pixels whose 5x5 edge-replicated
+ * neighbourhood is saturated in its majority (an isolated saturated pixel, e.g. a strong cosmic-ray hit, is not a
+ * core); out = core dilated `grow` times by the 3x3 square (grow = 0: the core itself). */
+int orc_satstar_mask(const float *img, int h, int w, float satlevel, int grow, uint8_t *out) {
+    if (!img || !out || h < 1 || w < 1 || grow < 0) return ORC_ERR_ARG;
+    size_t P = (size_t)h * w;
+    float *m5 = malloc(P * 4);
+    uint8_t *tmp = malloc(P);
+    if (!m5 || !tmp) { free(m5); free(tmp); return ORC_ERR_MEM; }
+    orc_medfilt(img, m5, h, w, 5);
+    for (size_t p = 0; p < P; ++p) out[p] = (uint8_t)(m5[p] >= satlevel);
+    for (int j = 0; j < grow; ++j) {
+        orc_dilate3(out, tmp, h, w);
+        memcpy(out, tmp, P);
+    }
+    free(m5); free(tmp);
+    return ORC_OK;
+}
+
+/* O7 with an input bad-pixel mask (R23): as orc_masked_median, but a tap is a donor iff its (clamped) pixel is
+ * neither in `mask` nor in `bpm`; no donor -> plain median of all 25 taps (R15).  bpm == NULL: orc_masked_median. */
+void orc_masked_median_bpm(const float *img, const uint8_t *mask, const uint8_t *bpm, float *out, int h, int w) {
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < h; ++y) {
+        float v[25];
+        for (int x = 0; x < w; ++x) {
+            size_t p = (size_t)y * w + x;
+            if (!mask[p]) { out[p] = img[p]; continue; }
+            int k = 0;
+            for (int dy = -2; dy <= 2; ++dy)
+                for (int dx = -2; dx <= 2; ++dx) {
+                    size_t q = (size_t)clampi(y + dy, 0, h - 1) * w + (size_t)clampi(x + dx, 0, w - 1);
+                    if (!mask[q] && !(bpm && bpm[q])) v[k++] = img[q];
+                }
+            if (k == 0)
+                for (int dy = -2; dy <= 2; ++dy)
+                    for (int dx = -2; dx <= 2; ++dx) v[k++] = rd(img, h, w, y + dy, x + dx);
+            sort_ascending(v, k);
+            out[p] = (k & 1) ? v[k / 2] : (v[k / 2 - 1] + v[k / 2]) * 0.5f;
+        }
+    }
+}
+
+typedef struct {
+    int fsmode;          /* 0: R7, the north-star test L+/F > objlim with F in ADU;
+                            1: R22, noise-normalised fine structure: Fn = max((m3 - m7)/N, 0.01), test S'/Fn > objlim */
+    int satgrow;         /* < 0: off; k >= 0: R25, pixels of orc_satstar_mask(img_in, satlevel, k) are never flagged */
+    int sepmed;          /* 0: true medians; 1: R26, every median of O2-O4 replaced by orc_sepmedfilt (comparison) */
+    const uint8_t *bpm;  /* nullable [h][w], R23: != 0 = bad pixel: never flagged, never a donor */
+    const float *var;    /* nullable [h][w], R24: variance plane [ADU^2]: N = sqrt(max(var, 1e-8)), replaces O2 */
+} orc_variant;
+
+static int medfilt_v(const float *X, float *out, int h, int w, int k, int sepmed) {
+    return sepmed ? orc_sepmedfilt(X, out, h, w, k) : orc_medfilt(X, out, h, w, k);
+}
+
+/* The whole path with the variants of R22-R26.  v == NULL or all-default: identical to orc_run.
+ * R23/R25: nok = bpm OR satstar; O5's `ok` becomes (work < satlevel) AND NOT nok, so such pixels are never candidates
+ * and never added by growth (hence never in C, never replaced).  R23 also removes bad pixels from the donors of O7.
+ * R24: with a variance plane O2 is replaced by N = sqrt(max(var, 1e-8)); the gain is then not used (never estimated).
+ * The dumped F plane is Fn when fsmode == 1. */
+int orc_run_ex(const float *img, int h, int w, float gain, float readnoise, float sigclip, float sigfrac,
+               float objlim, int niter, float satlevel, const orc_variant *v, uint8_t *mask_out, float *clean_out,
+               int32_t *iter_counts, orc_debug *dbg, float *iter_gains) {
+    static const orc_variant none = {0, -1, 0, NULL, NULL};
+    if (!v) v = &none;
+    if (!img || !mask_out || !clean_out || h < 1 || w < 1 || niter < 0) return ORC_ERR_ARG;
+    if (!(v->fsmode == 0 || v->fsmode == 1) || !(v->sepmed == 0 || v->sepmed == 1)) return ORC_ERR_ARG;
+    const int estimate = (gain == 0.0f) && !v->var;
+    if (!(gain >= 0.0f) || !(readnoise >= 0.0f) || !(sigclip > 0.0f) || !(sigfrac > 0.0f) || !(objlim >= 0.0f))
+        return ORC_ERR_ARG;
+    size_t P = (size_t)h * (size_t)w;
+    float *work = clean_out;
+    float *Lp = malloc(P * 4), *m5 = malloc(P * 4), *N = malloc(P * 4), *S = malloc(P * 4);
+    float *mS = malloc(P * 4), *Sp = malloc(P * 4), *m3 = malloc(P * 4), *m7 = malloc(P * 4);
+    float *F = malloc(P * 4);
+    uint8_t *G1 = malloc(P), *G2 = malloc(P), *M1 = malloc(P), *D = malloc(P), *M2 = malloc(P);
+    uint8_t *M3 = malloc(P), *nok = malloc(P), *C = mask_out;
+    int rc = ORC_OK;
+    if (!Lp || !m5 || !N || !S || !mS || !Sp || !m3 || !m7 || !F || !G1 || !G2 || !M1 || !D || !M2 || !M3 || !nok) {
+        rc = ORC_ERR_MEM;
+        goto done;
+    }
+    memset(C, 0, P);
+    memcpy(work, img, P * 4);
+    const float siglow = sigfrac * sigclip;
+    const float rn2 = readnoise * readnoise;
+    /* R23 / R25: the pixels that may never be flagged, fixed for the frame (from img_in) */
+    memset(nok, 0, P);
+    if (v->satgrow >= 0) {
+        rc = orc_satstar_mask(img, h, w, satlevel, v->satgrow, nok);
+        if (rc) goto done;
+    }
+    if (v->bpm)
+        for (size_t p = 0; p < P; ++p) nok[p] = (uint8_t)(nok[p] || v->bpm[p]);
+
+    for (int t = 0; t < niter; ++t) {
+        if (dbg && dbg->iter == t) COPY_IF(dbg->work_in, work, P * 4);
+        if (estimate) {
+            rc = orc_estimate_gain(work, h, w, readnoise, &gain, NULL);
+            if (rc) goto done;
+        }
+        if (iter_gains) iter_gains[t] = gain;
+        orc_lplus(work, Lp, h, w);                                                /* O1 */
+        if (v->var) {                                                             /* R24 */
+#pragma omp parallel for schedule(static)
+            for (size_t p = 0; p < P; ++p) {
+                float vv = v->var[p] > 1e-8f ? v->var[p] : 1e-8f;
+                N[p] = sqrtf(vv);
+            }
+        } else {                                                                  /* O2 */
+            rc = medfilt_v(work, m5, h, w, 5, v->sepmed);
+            if (rc) goto done;
+#pragma omp parallel for schedule(static)
+            for (size_t p = 0; p < P; ++p) {
+                float m = m5[p] > 1e-4f ? m5[p] : 1e-4f;
+                float gm = gain * m;
+                float var = gm + rn2;
+                N[p] = sqrtf(var) / gain;
+            }
+        }
+#pragma omp parallel for schedule(static)
+        for (size_t p = 0; p < P; ++p) {                                          /* O3 */
+            float twoN = 2.0f * N[p];
+            S[p] = Lp[p] / twoN;
+        }
+        rc = medfilt_v(S, mS, h, w, 5, v->sepmed);
+        if (rc) goto done;
+#pragma omp parallel for schedule(static)
+        for (size_t p = 0; p < P; ++p) Sp[p] = S[p] - mS[p];
+        rc = medfilt_v(work, m3, h, w, 3, v->sepmed);                             /* O4 */
+        if (rc) goto done;
+        rc = medfilt_v(m3, m7, h, w, 7, v->sepmed);
+        if (rc) goto done;
+#pragma omp parallel for schedule(static)
+        for (size_t p = 0; p < P; ++p) {
+            float f = m3[p] - m7[p];
+            if (v->fsmode == 1) f = f / N[p];                                     /* R22: in units of the noise */
+            F[p] = f > 0.01f ? f : 0.01f;
+        }
+#pragma omp parallel for schedule(static)
+        for (size_t p = 0; p < P; ++p) {                                          /* O5, R12, R23, R25 */
+            int ok = (work[p] < satlevel) && !nok[p];
+            G1[p] = (uint8_t)(ok && (Sp[p] > sigclip));
+            G2[p] = (uint8_t)(ok && (Sp[p] > siglow));
+            float ratio = (v->fsmode == 1 ? Sp[p] : Lp[p]) / F[p];                /* R22: S'/Fn; R7: L+/F */
+            M1[p] = (uint8_t)(G1[p] && (ratio > objlim));
+        }
+        orc_dilate3(M1, D, h, w);                                                 /* O6 */
+#pragma omp parallel for schedule(static)
+        for (size_t p = 0; p < P; ++p) M2[p] = (uint8_t)(D[p] && G1[p]);
+        orc_dilate3(M2, D, h, w);
+        int64_t newc = 0;
+#pragma omp parallel for schedule(static) reduction(+ : newc)
+        for (size_t p = 0; p < P; ++p) {
+            M3[p] = (uint8_t)(D[p] && G2[p]);
+            if (M3[p] && !C[p]) ++newc;
+            C[p] = (uint8_t)(C[p] || M3[p]);
+        }
+        if (iter_counts) iter_counts[t] = (int32_t)newc;
+        orc_masked_median_bpm(img, C, v->bpm, work, h, w);                        /* O7, R23 */
+
+        if (dbg && dbg->iter == t) {
+            COPY_IF(dbg->Lp, Lp, P * 4); COPY_IF(dbg->N, N, P * 4); COPY_IF(dbg->S, S, P * 4);
+            COPY_IF(dbg->Sp, Sp, P * 4); COPY_IF(dbg->m3, m3, P * 4); COPY_IF(dbg->F, F, P * 4);
+            COPY_IF(dbg->G1, G1, P); COPY_IF(dbg->G2, G2, P); COPY_IF(dbg->M1, M1, P);
+            COPY_IF(dbg->M2, M2, P); COPY_IF(dbg->M3, M3, P); COPY_IF(dbg->C, C, P);
+        }
+    }
+done:
+    free(Lp); free(m5); free(N); free(S); free(mS); free(Sp); free(m3); free(m7); free(F);
+    free(G1); free(G2); free(M1); free(D); free(M2); free(M3); free(nok);
+    return rc;
+}

@@ -61,6 +61,15 @@ def lib():
         L.orc_sigma_clip.argtypes = [fp, C.c_size_t, C.c_int, fp]
         L.orc_sigma_clip.restype = C.c_float
         L.orc_run.restype = C.c_int
+        L.orc_sepmedfilt.argtypes = [fp, fp, C.c_int, C.c_int, C.c_int]
+        L.orc_sepmedfilt.restype = C.c_int
+        L.orc_satstar_mask.argtypes = [fp, C.c_int, C.c_int, C.c_float, C.c_int, u8p]
+        L.orc_satstar_mask.restype = C.c_int
+        L.orc_masked_median_bpm.argtypes = [fp, u8p, u8p, fp, C.c_int, C.c_int]
+        L.orc_masked_median_bpm.restype = None
+        L.orc_run_ex.argtypes = [fp, C.c_int, C.c_int] + [C.c_float] * 5 + [C.c_int, C.c_float, C.c_void_p,
+                                                                           u8p, fp, i32p, C.c_void_p, fp]
+        L.orc_run_ex.restype = C.c_int
         L.orc_set_threads.argtypes = [C.c_int]
         L.orc_get_max_threads.restype = C.c_int
         _lib = L
@@ -122,6 +131,40 @@ def masked_median(img, mask):
     return out
 
 
+def sepmedfilt(img, k):
+    """R26: separable k x k median (row pass, then column pass); comparison only."""
+    img = _f32(img)
+    out = np.empty_like(img)
+    rc = lib().orc_sepmedfilt(_p(img), _p(out), img.shape[0], img.shape[1], int(k))
+    if rc != 0:
+        raise ValueError("orc_sepmedfilt: bad argument")
+    return out
+
+
+def satstar_mask(img, satlevel=65535.0, grow=0):
+    """R25: (med5(img) >= satlevel) dilated `grow` times by the 3x3 square."""
+    img = _f32(img)
+    out = np.empty(img.shape, np.uint8)
+    rc = lib().orc_satstar_mask(_p(img), img.shape[0], img.shape[1], float(satlevel), int(grow), _p(out))
+    if rc != 0:
+        raise ValueError("orc_satstar_mask: bad argument")
+    return out
+
+
+def masked_median_bpm(img, mask, bpm=None):
+    """O7 with bad pixels removed from the donors (R23)."""
+    img, mask = _f32(img), _u8(mask)
+    out = np.empty_like(img)
+    b = None if bpm is None else _u8(bpm)
+    lib().orc_masked_median_bpm(_p(img), _p(mask), None if b is None else _p(b), _p(out), *img.shape)
+    return out
+
+
+class _Variant(C.Structure):
+    _fields_ = [("fsmode", C.c_int), ("satgrow", C.c_int), ("sepmed", C.c_int), ("bpm", C.c_void_p),
+                ("var", C.c_void_p)]
+
+
 def sigma_clip(r, rounds=3):
     """R21 sigma clipping of a 1-D fp32 vector.  Returns (s, stats = [c, s, lo, hi, kept] of the last round)."""
     r = np.ascontiguousarray(r, dtype=np.float32).ravel()
@@ -142,9 +185,11 @@ def estimate_gain(img, readnoise=0.0):
 
 
 def run(img, gain=1.0, readnoise=10.0, sigclip=4.5, sigfrac=0.3, objlim=5.0, niter=4,
-        satlevel=65535.0, debug_iter=None):
+        satlevel=65535.0, debug_iter=None, fsmode=None, satgrow=None, sepmed=None, bpm=None, var=None):
     """Whole path (O0-O7).  gain = 0: estimated at each iteration (R21).  Returns dict(mask=u8, clean=f32,
-    counts=int32[niter], gains=f32[niter] (the gain each iteration used), [debug planes])."""
+    counts=int32[niter], gains=f32[niter] (the gain each iteration used), [debug planes]).
+    Any of fsmode / satgrow / sepmed / bpm / var given: orc_run_ex with those variants (R22-R26); none given:
+    orc_run, the north-star path."""
     img = _f32(img)
     h, w = img.shape
     mask = np.empty((h, w), np.uint8)
@@ -163,8 +208,17 @@ def run(img, gain=1.0, readnoise=10.0, sigclip=4.5, sigfrac=0.3, objlim=5.0, nit
             setattr(dbg, n, out[n].ctypes.data)
         dbg_ref = C.byref(dbg)
     gains = np.zeros(max(niter, 1), np.float32)
-    rc = lib().orc_run(_p(img), h, w, gain, readnoise, sigclip, sigfrac, objlim, int(niter),
-                       satlevel, _p(mask), _p(clean), _p(counts), dbg_ref, _p(gains))
+    if all(a is None for a in (fsmode, satgrow, sepmed, bpm, var)):
+        rc = lib().orc_run(_p(img), h, w, gain, readnoise, sigclip, sigfrac, objlim, int(niter),
+                           satlevel, _p(mask), _p(clean), _p(counts), dbg_ref, _p(gains))
+    else:
+        b = None if bpm is None else _u8(bpm)
+        vp = None if var is None else _f32(var)
+        assert (b is None or b.shape == img.shape) and (vp is None or vp.shape == img.shape)
+        v = _Variant(int(fsmode or 0), -1 if satgrow is None else int(satgrow), int(bool(sepmed)),
+                     None if b is None else b.ctypes.data, None if vp is None else vp.ctypes.data)
+        rc = lib().orc_run_ex(_p(img), h, w, gain, readnoise, sigclip, sigfrac, objlim, int(niter),
+                              satlevel, C.byref(v), _p(mask), _p(clean), _p(counts), dbg_ref, _p(gains))
     if rc != 0:
         raise ValueError("orc_run failed with code %d" % rc)
     out.update(mask=mask, clean=clean, counts=counts[:niter].copy(), gains=gains[:niter].copy())
