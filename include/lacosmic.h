@@ -118,6 +118,49 @@ int lacosmic_run_ws(const float *img, int h, int w, const lacosmic_params *p, ui
                     float *clean_out, void *workspace, size_t workspace_bytes, int32_t *iter_counts,
                     const lacosmic_debug *dbg, void *stream);
 
+/* ---- fidelity variants (readings R22-R25) ------------------------------ */
+
+#define LACOSMIC_FS_ADU 0          /* R7, the north-star test: L+/F > objlim, F = max(med3 - med7(med3), 0.01) in ADU */
+#define LACOSMIC_FS_NORMALISED 1   /* R22: Fn = max((med3 - med7(med3))/N, 0.01), test S'/Fn > objlim */
+#define LACOSMIC_MAX_SATGROW 16
+
+/* Optional variants of one frame; a NULL pointer or {LACOSMIC_FS_ADU, -1, NULL, NULL} is the north-star path.
+ *   fsmode : which quantity the object test of step (5) compares (above).
+ *   satgrow: -1 = off; k in [0, LACOSMIC_MAX_SATGROW] = extended saturated-star mask (R25): the pixels of
+ *            dil3^k(med5(img) >= satlevel), computed once from the input frame, are never flagged (they stay donors).
+ *   bpm    : nullable DEVICE uint8 [h][w], != 0 = bad pixel (R23): never flagged, never rewritten, never a donor of
+ *            the replacement; its value still enters the filters.
+ *   var    : nullable DEVICE fp32 [h][w] (16-byte aligned), variance in ADU^2 (R24): N = sqrt(max(var, 1e-8)) replaces
+ *            the noise model of step (2); gain and readnoise are then unused (gain = 0 does not trigger the estimate).
+ * bpm / var are read during the call's stream work and must not overlap the outputs. */
+typedef struct lacosmic_variant {
+    int32_t fsmode;
+    int32_t satgrow;
+    const uint8_t *bpm;
+    const float *var;
+} lacosmic_variant;
+
+/* lacosmic_run_ws with variants (v: nullable HOST struct, read during the call).  Same outputs, same modes: both
+ * LACOSMIC_MODE_LAZY and LACOSMIC_MODE_DENSE implement every variant and agree bit for bit.  With fsmode =
+ * LACOSMIC_FS_NORMALISED the debug plane F holds Fn. */
+int lacosmic_run_ex(const float *img, int h, int w, const lacosmic_params *p, const lacosmic_variant *v,
+                    uint8_t *mask_out, float *clean_out, void *workspace, size_t workspace_bytes,
+                    int32_t *iter_counts, const lacosmic_debug *dbg, void *stream);
+
+/* ---- separable-median COMPARISON path (R26) ---------------------------- */
+
+/* PAPER.md:29,37 argue that the separable median (row pass, then column pass) "can result in the incorrect removal of
+ * cosmic rays by incorrectly classifying the center of near-saturated or saturated stars as cosmic rays".  This entry
+ * point exists to show that difference: it runs O0-O7 with med5(img), med5(S), med3 and med7 all replaced by the
+ * separable median and is otherwise lacosmic_run_ws (p->mode is ignored; p->gain must be > 0).  It is NOT a product
+ * path: nothing else in the library calls it.  workspace: lacosmic_sepmed_workspace_bytes(h, w) bytes. */
+size_t lacosmic_sepmed_workspace_bytes(int h, int w);
+int lacosmic_run_sepmed_compare(const float *img, int h, int w, const lacosmic_params *p, uint8_t *mask_out,
+                                float *clean_out, void *workspace, size_t workspace_bytes, int32_t *iter_counts,
+                                const lacosmic_debug *dbg, void *stream);
+/* out = separable k x k median of in (k in {3,5,7}); tmp: a third fp32 [h][w] plane (receives the row pass). */
+int lacosmic_sepmedfilt(const float *in, float *out, float *tmp, int h, int w, int k, void *stream);
+
 /* n independent frames ("batch processing"; BASELINE.json configs[3]).
  * imgs/masks_out/cleans_out are [n][h][w]; params is a HOST array of n structs (per-frame
  * parameters, read during the call); iter_counts: nullable device array [n][LACOSMIC_MAX_NITER].
@@ -222,6 +265,14 @@ int lacosmic_dilate3(const uint32_t *bits_in, uint32_t *bits_out, int h, int w, 
  * for lacosmic_run_ws. */
 int lacosmic_masked_median(const float *img, const uint8_t *mask_u8, float *out, int h, int w,
                            void *workspace, size_t workspace_bytes, void *stream);
+
+/* Step (7) with bad pixels removed from the donors (R23); bpm_u8 nullable (then lacosmic_masked_median). */
+int lacosmic_masked_median_bpm(const float *img, const uint8_t *mask_u8, const uint8_t *bpm_u8, float *out, int h,
+                               int w, void *workspace, size_t workspace_bytes, void *stream);
+
+/* R25 alone: out_u8[h][w] = 1 on dil3^grow(med5(img) >= satlevel), else 0.  workspace as for lacosmic_run_ws. */
+int lacosmic_satstar_mask(const float *img, int h, int w, float satlevel, int grow, uint8_t *out_u8, void *workspace,
+                          size_t workspace_bytes, void *stream);
 
 /* ---- diagnostics ---------------------------------------------------------------------------- */
 const char *lacosmic_strerror(int code);

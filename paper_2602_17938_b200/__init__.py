@@ -8,6 +8,8 @@ from .binding import (  # noqa: F401
     MAX_NITER,
     MODE_DENSE,
     MODE_LAZY,
+    FS_ADU,
+    FS_NORMALISED,
     LacosmicError,
     Params,
     lacosmic_bitplane_pitch_words,
@@ -27,6 +29,12 @@ from .binding import (  # noqa: F401
     lacosmic_run_batch,
     lacosmic_run_host,
     lacosmic_run_ws,
+    lacosmic_run_ex,
+    lacosmic_run_sepmed_compare,
+    lacosmic_sepmed_workspace_bytes,
+    lacosmic_sepmedfilt,
+    lacosmic_satstar_mask,
+    lacosmic_masked_median_bpm,
     lacosmic_strerror,
     lacosmic_unpack_bits,
     lacosmic_version,
@@ -42,4 +50,5 @@ from .binding import (  # noqa: F401
 
 __all__ = [n for n in dir() if n.startswith("lacosmic_")] + ["LacosmicError", "Params",
                                                               "library_path", "load_library",
-                                                              "MODE_LAZY", "MODE_DENSE", "MAX_NITER"]
+                                                              "MODE_LAZY", "MODE_DENSE", "MAX_NITER",
+                                                              "FS_ADU", "FS_NORMALISED"]

@@ -26,9 +26,12 @@ EXPORTS = (
     "lacosmic_last_cuda_error", "lacosmic_last_launch_count", "lacosmic_version",
     "lacosmic_kernel_timing_enable", "lacosmic_kernel_timing_read", "lacosmic_kernel_class_name",
     "lacosmic_probe_minmax_rate",
+    "lacosmic_run_ex", "lacosmic_sepmed_workspace_bytes", "lacosmic_run_sepmed_compare", "lacosmic_sepmedfilt",
+    "lacosmic_masked_median_bpm", "lacosmic_satstar_mask",
 )
 NUM_KERNEL_CLASSES = 9
 MODE_LAZY, MODE_DENSE = 0, 1
+FS_ADU, FS_NORMALISED = 0, 1
 
 
 class LacosmicError(RuntimeError):
@@ -43,6 +46,10 @@ class LacosmicError(RuntimeError):
 class _CParams(C.Structure):
     _fields_ = [(n, C.c_float) for n in ("gain", "readnoise", "sigclip", "sigfrac", "objlim",
                                          "satlevel")] + [("niter", C.c_int32), ("mode", C.c_int32)]
+
+
+class _CVariant(C.Structure):
+    _fields_ = [("fsmode", C.c_int32), ("satgrow", C.c_int32), ("bpm", C.c_void_p), ("var", C.c_void_p)]
 
 
 class _CDebug(C.Structure):
@@ -117,6 +124,13 @@ def load_library():
         "lacosmic_kernel_timing_read": (i, [vp, vp]),
         "lacosmic_kernel_class_name": (C.c_char_p, [i]),
         "lacosmic_probe_minmax_rate": (i, [i, vp, vp]),
+        "lacosmic_run_ex": (i, [vp, i, i, C.POINTER(_CParams), C.POINTER(_CVariant), vp, vp, vp, sz, vp,
+                                C.POINTER(_CDebug), vp]),
+        "lacosmic_sepmed_workspace_bytes": (sz, [i, i]),
+        "lacosmic_run_sepmed_compare": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp, C.POINTER(_CDebug), vp]),
+        "lacosmic_sepmedfilt": (i, [vp, vp, vp, i, i, i, vp]),
+        "lacosmic_masked_median_bpm": (i, [vp, vp, vp, vp, i, i, vp, sz, vp]),
+        "lacosmic_satstar_mask": (i, [vp, i, i, f, i, vp, vp, sz, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)      # AttributeError if the header and the library disagree
@@ -224,12 +238,18 @@ def lacosmic_run(img, gain=1.0, readnoise=10.0, sigclip=4.5, sigfrac=0.3, objlim
 
 
 def lacosmic_run_ws(img, params=None, mask_out=None, clean_out=None, workspace=None,
-                    iter_counts=None, debug_iter=None, debug_planes=None, want_gains=False, stream=None, **kw):
+                    iter_counts=None, debug_iter=None, debug_planes=None, want_gains=False, stream=None,
+                    fsmode=None, satgrow=None, bpm=None, var=None, sepmed_compare=False, **kw):
     """Timed entry point.  Returns dict(mask, clean, counts[, debug planes of iteration debug_iter][, gains =
-    the gain each iteration used, when want_gains])."""
+    the gain each iteration used, when want_gains]).  Any of fsmode / satgrow / bpm (uint8 CUDA tensor) / var (float32
+    CUDA tensor) given: lacosmic_run_ex with those variants (R22-R25).  sepmed_compare=True:
+    lacosmic_run_sepmed_compare, the separable-median comparison path (R26)."""
     torch = _torch()
     L = load_library()
     p = _params(params, **kw)
+    variant = not all(a is None for a in (fsmode, satgrow, bpm, var))
+    if variant and sepmed_compare:
+        raise ValueError("the separable-median comparison path takes no variants")
     if img.dim() != 2:
         raise ValueError("img must be [h][w]")
     h, w = img.shape
@@ -239,7 +259,8 @@ def lacosmic_run_ws(img, params=None, mask_out=None, clean_out=None, workspace=N
     if clean_out is None:
         clean_out = torch.empty_like(img)
     if workspace is None:
-        workspace = _scratch_on(_workspace(h, w, img.device), stream)
+        nbytes = lacosmic_sepmed_workspace_bytes(h, w) if sepmed_compare else lacosmic_workspace_bytes(h, w)
+        workspace = _scratch_on(torch.empty(nbytes, dtype=torch.uint8, device=img.device), stream)
     if iter_counts is None:
         iter_counts = torch.zeros(max(int(p.niter), 1), dtype=torch.int32, device=img.device)
     out = dict(mask=mask_out, clean=clean_out, counts=iter_counts)
@@ -258,11 +279,56 @@ def lacosmic_run_ws(img, params=None, mask_out=None, clean_out=None, workspace=N
             dbg.gains = out["gains"].data_ptr()
         dbg_ref = C.byref(dbg)
     cp = p._c()
-    rc = L.lacosmic_run_ws(ip, h, w, C.byref(cp), _dev(mask_out, torch.uint8, "mask_out", (h, w)),
-                           _dev(clean_out, torch.float32, "clean_out", (h, w)),
-                           _dev(workspace, torch.uint8, "workspace"), workspace.numel(),
-                           _dev(iter_counts, torch.int32, "iter_counts"), dbg_ref, _stream(stream))
-    _check(rc, "lacosmic_run_ws")
+    tail = (_dev(mask_out, torch.uint8, "mask_out", (h, w)), _dev(clean_out, torch.float32, "clean_out", (h, w)),
+            _dev(workspace, torch.uint8, "workspace"), workspace.numel(),
+            _dev(iter_counts, torch.int32, "iter_counts"), dbg_ref, _stream(stream))
+    if sepmed_compare:
+        _check(L.lacosmic_run_sepmed_compare(ip, h, w, C.byref(cp), *tail), "lacosmic_run_sepmed_compare")
+    elif variant:
+        cv = _CVariant(int(fsmode or 0), -1 if satgrow is None else int(satgrow),
+                       None if bpm is None else _dev(bpm, torch.uint8, "bpm", (h, w)),
+                       None if var is None else _dev(var, torch.float32, "var", (h, w)))
+        _check(L.lacosmic_run_ex(ip, h, w, C.byref(cp), C.byref(cv), *tail), "lacosmic_run_ex")
+    else:
+        _check(L.lacosmic_run_ws(ip, h, w, C.byref(cp), *tail), "lacosmic_run_ws")
+    return out
+
+
+def lacosmic_run_ex(img, params=None, fsmode=FS_ADU, satgrow=-1, bpm=None, var=None, **kw):
+    """lacosmic_run_ws with the variants of DESIGN.md R22-R25 (always through the lacosmic_run_ex entry point)."""
+    return lacosmic_run_ws(img, params, fsmode=fsmode, satgrow=satgrow, bpm=bpm, var=var, **kw)
+
+
+def lacosmic_run_sepmed_compare(img, params=None, **kw):
+    """The separable-median comparison path (R26).  Not a product path."""
+    return lacosmic_run_ws(img, params, sepmed_compare=True, **kw)
+
+
+def lacosmic_sepmed_workspace_bytes(h, w):
+    return int(load_library().lacosmic_sepmed_workspace_bytes(int(h), int(w)))
+
+
+def lacosmic_sepmedfilt(img, k, out=None, stream=None):
+    torch = _torch()
+    h, w = img.shape
+    if out is None:
+        out = torch.empty_like(img)
+    tmp = _scratch_on(torch.empty_like(img), stream)
+    _check(load_library().lacosmic_sepmedfilt(_dev(img, torch.float32, "img"), _dev(out, torch.float32, "out", (h, w)),
+                                              tmp.data_ptr(), h, w, int(k), _stream(stream)), "lacosmic_sepmedfilt")
+    return out
+
+
+def lacosmic_satstar_mask(img, satlevel=65535.0, grow=0, workspace=None, stream=None):
+    """R25 alone: uint8 [h][w], 1 on dil3^grow(med5(img) >= satlevel)."""
+    torch = _torch()
+    h, w = img.shape
+    out = torch.empty((h, w), dtype=torch.uint8, device=img.device)
+    if workspace is None:
+        workspace = _scratch_on(_workspace(h, w, img.device), stream)
+    _check(load_library().lacosmic_satstar_mask(_dev(img, torch.float32, "img"), h, w, float(satlevel), int(grow),
+                                                out.data_ptr(), _dev(workspace, torch.uint8, "workspace"),
+                                                workspace.numel(), _stream(stream)), "lacosmic_satstar_mask")
     return out
 
 
@@ -511,18 +577,27 @@ def lacosmic_dilate3(bits, h, w, stream=None):
     return out
 
 
-def lacosmic_masked_median(img, mask_u8, out=None, workspace=None, stream=None):
+def lacosmic_masked_median(img, mask_u8, out=None, workspace=None, stream=None, bpm=None):
+    """Step (7).  bpm (uint8 CUDA tensor): bad pixels removed from the donors (R23, lacosmic_masked_median_bpm)."""
     torch = _torch()
     h, w = img.shape
     if out is None:
         out = torch.empty_like(img)
     if workspace is None:
         workspace = _scratch_on(_workspace(h, w, img.device), stream)
-    _check(load_library().lacosmic_masked_median(
-        _dev(img, torch.float32, "img"), _dev(mask_u8, torch.uint8, "mask_u8", (h, w)),
-        _dev(out, torch.float32, "out", (h, w)), h, w, _dev(workspace, torch.uint8, "workspace"),
-        workspace.numel(), _stream(stream)), "lacosmic_masked_median")
+    L = load_library()
+    args = (_dev(out, torch.float32, "out", (h, w)), h, w, _dev(workspace, torch.uint8, "workspace"),
+            workspace.numel(), _stream(stream))
+    if bpm is None:
+        _check(L.lacosmic_masked_median(_dev(img, torch.float32, "img"), _dev(mask_u8, torch.uint8, "mask_u8", (h, w)),
+                                        *args), "lacosmic_masked_median")
+    else:
+        _check(L.lacosmic_masked_median_bpm(_dev(img, torch.float32, "img"), _dev(mask_u8, torch.uint8, "mask_u8", (h, w)),
+                                            _dev(bpm, torch.uint8, "bpm", (h, w)), *args), "lacosmic_masked_median_bpm")
     return out
+
+
+lacosmic_masked_median_bpm = lacosmic_masked_median
 
 
 def lacosmic_strerror(code):

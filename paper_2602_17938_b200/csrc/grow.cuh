@@ -99,6 +99,7 @@ struct GrowArgs {
     int h, w, wpr;
     float siglow;
     int nbx;                      // strips per row of strips = CTAs per row of CTAs (1-D grid, block_xy)
+    const uint32_t* donx;         // nullable (R23): bad pixels, never donors of the replacement
 };
 
 #ifndef LAC_GROW_MINB
@@ -261,8 +262,9 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
     if (!__any_sync(FULL, anyneed)) return;
     // ---- step (7) at those pixels: 25 clamped taps of img_in, +inf where the tap's pixel is in C', 25-input
     // sorting network, middle element(s) of the k donors (R13-R16)
+    // s_plane: the pixels that are no donors = C' (R13), plus the bad pixels (R23)
 #pragma unroll
-    for (int j = 2; j < WG_J - 2; ++j) s_plane[(j - 2) * 32 + lane] = cn[j];
+    for (int j = 2; j < WG_J - 2; ++j) s_plane[(j - 2) * 32 + lane] = cn[j] | (a.donx ? ld(a.donx, j) : 0u);
     __syncwarp();
     const float INF = __int_as_float(0x7f800000);
     warp_for_each_bit<4, 4 + WG_R>(need, s_list, lane, [&](int j, int sl, int bit) {

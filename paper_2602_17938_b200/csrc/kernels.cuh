@@ -131,7 +131,13 @@ struct NoiseArgs {
     const float* gain_dev;   // nullable (R21): the gain of this iteration, estimated on the device
     int* zero_ptr;           // nullable: the frame's counter block, cleared by the first launch of a frame
     int zero_n;              // (nothing reads or adds to it before the next launch)
+    const uint32_t* nok;     // nullable (R23, R25): bit-plane of the pixels that may never be flagged (bad pixels,
+                             // extended saturated-star mask); cleared from A1 / A2
+    const float* var;        // nullable (R24): variance plane; N = sqrt(max(var, 1e-8)) replaces the noise model
 };
+
+// R24: N from a variance entry
+__device__ __forceinline__ float noise_from_var(float v) { return __fsqrt_rn(v > 1e-8f ? v : 1e-8f); }
 
 __device__ __forceinline__ void zero_counters(const NoiseArgs& a) {
     if (a.zero_ptr)
@@ -198,8 +204,9 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
             const uint32_t b1 = nibbles_to_word(n1, lane), b2 = nibbles_to_word(n2, lane);
             if (lx == 0 && y < a.h) {
                 size_t q = (size_t)y * a.wpr + (xu >> 5);
-                a.A1[q] = b1;
-                a.A2[q] = b2;
+                const uint32_t keep = a.nok ? ~a.nok[q] : 0xffffffffu;
+                a.A1[q] = b1 & keep;
+                a.A2[q] = b2 & keep;
             }
         }
     }
@@ -231,6 +238,8 @@ struct FineArgs {
     float *dbgSp, *dbgM3, *dbgF;
     int h, w, wpr;
     GateParams gp;
+    const float* N;          // R22 (fsmode 1): the noise plane the noise/S pass stored; null: R7 (L+/F, F in ADU)
+    const uint32_t* nok;     // nullable (R23, R25): pixels that may never be flagged
 };
 
 // smA / smS: edge-replicated work / S tiles; smB: scratch for the m3 tile.  Contains block barriers.
@@ -293,6 +302,7 @@ __device__ __forceinline__ void fine_gates_tile(const float* smA, float* smB, co
                 for (int j = 0; j < 4; ++j) {
                     m3[j] = win[3 + j][3];
                     float d = __fsub_rn(m3[j], m7[j]);
+                    if (a.N) d = __fdiv_rn(d, a.N[(size_t)y * w + min(x + j, w - 1)]);   // R22: in units of the noise
                     f[j] = d > 0.01f ? d : 0.01f;
                 }
             }
@@ -310,7 +320,8 @@ __device__ __forceinline__ void fine_gates_tile(const float* smA, float* smB, co
                 bool ok = (x + j < w) && (ctr[1 + j] < a.gp.satlevel);            // R12
                 bool g1 = ok && (sp[j] > a.gp.sigclip);
                 bool g2 = ok && (sp[j] > a.gp.siglow);
-                bool m1 = g1 && (fdiv_nn(lp, f[j]) > a.gp.objlim);               // R8
+                // R8; R22 compares S' (positive where G1 holds) instead of L+
+                bool m1 = g1 && ((a.N ? __fdiv_rn(sp[j], f[j]) : fdiv_nn(lp, f[j])) > a.gp.objlim);
                 n1 |= (uint32_t)g1 << j;
                 n2 |= (uint32_t)g2 << j;
                 n3 |= (uint32_t)m1 << j;
@@ -324,9 +335,10 @@ __device__ __forceinline__ void fine_gates_tile(const float* smA, float* smB, co
         int wx = (x0 >> 5) + (lane >> 3);
         if ((lane & 7) == 0 && y < h && wx < a.wpr) {
             size_t q = (size_t)y * a.wpr + wx;
-            a.G1[q] = b1;
-            a.G2[q] = b2;
-            a.M1[q] = b3;
+            const uint32_t keep = a.nok ? ~a.nok[q] : 0xffffffffu;
+            a.G1[q] = b1 & keep;
+            a.G2[q] = b2 & keep;
+            a.M1[q] = b3 & keep;
         }
     }
 }
@@ -491,7 +503,7 @@ __device__ __forceinline__ float one_S_px(float c, float U, float D, float Lf, f
                                           const NoiseArgs& a, bool inframe, int j, uint32_t& n1, uint32_t& n2,
                                           float& lp, float& nn) {
     lp = lplus_px(c, U, D, Lf, R);
-    nn = noise_px(m5, gain, a.rn2);
+    nn = a.var ? noise_from_var(m5) : noise_px(m5, gain, a.rn2);   // R24: the plane holds the variance
     const float s = fdiv_nn(lp, __fmul_rn(2.0f, nn));
     const bool ok = inframe && (c < a.satlevel);                                         // R12
     n1 |= (uint32_t)(ok && s > a.sigclip) << j;
@@ -505,6 +517,7 @@ constexpr int SM5_ROWS = 16;
 __global__ void __launch_bounds__(256)
 k_S_from_m5(const float* __restrict__ work, NoiseArgs a, int nbx, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
+    zero_counters(a);
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const int h = a.h, w = a.w;
     const BlockXY bk = block_xy(nbx);
@@ -522,7 +535,7 @@ k_S_from_m5(const float* __restrict__ work, NoiseArgs a, int nbx, const int* pre
     for (int y = ya; y < yend; ++y) {
         dn = ldrow(y + 1);
         const size_t o = (size_t)y * w + xc;
-        const float4 m5 = *reinterpret_cast<const float4*>(a.S + o);
+        const float4 m5 = *reinterpret_cast<const float4*>((a.var ? a.var : a.S) + o);
         float lf = __shfl_up_sync(0xffffffffu, cur.w, 1);          // R3: clamped at the frame edge
         float rt = __shfl_down_sync(0xffffffffu, cur.x, 1);
         if (lane == 0) lf = x > 0 ? __ldg(work + (size_t)y * w + x - 1) : cur.x;
@@ -537,12 +550,14 @@ k_S_from_m5(const float* __restrict__ work, NoiseArgs a, int nbx, const int* pre
         const uint32_t b1 = nibbles_to_word(n1, lane), b2 = nibbles_to_word(n2, lane);
         if (inx) {
             *reinterpret_cast<float4*>(a.S + o) = make_float4(s[0], s[1], s[2], s[3]);
+            if (a.copy_out) *reinterpret_cast<float4*>(a.copy_out + o) = cur;
             if (a.dbgLp) store4(a.dbgLp, (size_t)y * w, x, w, lp);
             if (a.dbgN) store4(a.dbgN, (size_t)y * w, x, w, nn);
             if (a.A1 && (lane & 7) == 0) {
                 const size_t q = (size_t)y * a.wpr + (x >> 5);
-                a.A1[q] = b1;
-                a.A2[q] = b2;
+                const uint32_t keep = a.nok ? ~a.nok[q] : 0xffffffffu;
+                a.A1[q] = b1 & keep;
+                a.A2[q] = b2 & keep;
             }
         }
         up = cur;
@@ -554,6 +569,7 @@ k_S_from_m5(const float* __restrict__ work, NoiseArgs a, int nbx, const int* pre
 __global__ void __launch_bounds__(256)
 k_S_from_m5_generic(const float* __restrict__ work, NoiseArgs a, int nbx, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
+    zero_counters(a);
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const int h = a.h, w = a.w;
     const BlockXY bk = block_xy(nbx);
@@ -571,18 +587,21 @@ k_S_from_m5_generic(const float* __restrict__ work, NoiseArgs a, int nbx, const 
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const int xj = min(x + j, w - 1);
-        s[j] = one_S_px(c[1 + j], __ldg(ru + xj), __ldg(rd + xj), c[j], c[2 + j], a.S[(size_t)y * w + xj], gain, a,
-                        x + j < w, j, n1, n2, lp[j], nn[j]);
+        s[j] = one_S_px(c[1 + j], __ldg(ru + xj), __ldg(rd + xj), c[j], c[2 + j],
+                        (a.var ? a.var : a.S)[(size_t)y * w + xj], gain, a, x + j < w, j, n1, n2, lp[j], nn[j]);
     }
     const uint32_t b1 = nibbles_to_word(n1, lane), b2 = nibbles_to_word(n2, lane);
     if (x < w) {
+        const float ctr[4] = {c[1], c[2], c[3], c[4]};
         store4(a.S, (size_t)y * w, x, w, s);
+        if (a.copy_out) store4(a.copy_out, (size_t)y * w, x, w, ctr);
         if (a.dbgLp) store4(a.dbgLp, (size_t)y * w, x, w, lp);
         if (a.dbgN) store4(a.dbgN, (size_t)y * w, x, w, nn);
         if (a.A1 && (lane & 7) == 0) {
             const size_t q = (size_t)y * a.wpr + (x >> 5);
-            a.A1[q] = b1;
-            a.A2[q] = b2;
+            const uint32_t keep = a.nok ? ~a.nok[q] : 0xffffffffu;
+            a.A1[q] = b1 & keep;
+            a.A2[q] = b2 & keep;
         }
     }
 }
@@ -650,12 +669,60 @@ k_unpack_bits(const uint32_t* __restrict__ bits, uint8_t* __restrict__ u8, int h
 }
 
 __global__ void __launch_bounds__(256)
-k_pack_bits(const uint8_t* __restrict__ u8, uint32_t* __restrict__ bits, int h, int w, int wpr, int nbx) {
+k_pack_bits(const uint8_t* __restrict__ u8, uint32_t* __restrict__ bits, int h, int w, int wpr, int nbx,
+            uint32_t* __restrict__ or_into) {
     const BlockXY bk = block_xy(nbx);
     int x = bk.x * 256 + threadIdx.x, y = bk.y;
     bool b = (x < w) && (u8[(size_t)y * w + x] != 0);
     uint32_t word = __ballot_sync(0xffffffffu, b);
+    if ((threadIdx.x & 31) == 0 && (x >> 5) < wpr) {
+        bits[(size_t)y * wpr + (x >> 5)] = word;
+        if (or_into) or_into[(size_t)y * wpr + (x >> 5)] |= word;      // R23: bad pixels join the never-flag plane
+    }
+}
+
+// bits = (img >= level) (R25: the saturated pixels of the input frame)
+__global__ void __launch_bounds__(256)
+k_pack_ge(const float* __restrict__ img, float level, uint32_t* __restrict__ bits, int h, int w, int wpr, int nbx) {
+    const BlockXY bk = block_xy(nbx);
+    int x = bk.x * 256 + threadIdx.x, y = bk.y;
+    bool b = (x < w) && (img[(size_t)y * w + x] >= level);
+    uint32_t word = __ballot_sync(0xffffffffu, b);
     if ((threadIdx.x & 31) == 0 && (x >> 5) < wpr) bits[(size_t)y * wpr + (x >> 5)] = word;
+}
+
+// R25: core = (med5(img) >= satlevel) from the bit-plane sat = (img >= satlevel): the median of the 25 clamped taps
+// reaches the level iff at least 13 of them do.  One thread per word; a word with no saturated pixel within two rows and
+// one word of it (almost every word of a frame) is zero without looking at single pixels.
+__global__ void __launch_bounds__(256)
+k_satcore(const uint32_t* __restrict__ sat, uint32_t* __restrict__ core, int h, int w, int wpr, int nbx) {
+    const BlockXY bk = block_xy(nbx);
+    const int wx = bk.x * 256 + threadIdx.x, y = bk.y;
+    if (wx >= wpr) return;
+    const int wl = max(wx - 1, 0), wr = min(wx + 1, wpr - 1);
+    uint32_t any = 0;
+#pragma unroll
+    for (int dy = -2; dy <= 2; ++dy) {
+        const uint32_t* row = sat + (size_t)clampi(y + dy, 0, h - 1) * wpr;
+        any |= row[wl] | row[wx] | row[wr];
+    }
+    uint32_t out = 0;
+    if (any) {
+        for (int b = 0; b < 32; ++b) {
+            const int x = wx * 32 + b;
+            if (x >= w) break;
+            int cnt = 0;
+            for (int dy = -2; dy <= 2; ++dy) {
+                const uint32_t* row = sat + (size_t)clampi(y + dy, 0, h - 1) * wpr;
+                for (int dx = -2; dx <= 2; ++dx) {
+                    const int xx = clampi(x + dx, 0, w - 1);
+                    cnt += (row[xx >> 5] >> (xx & 31)) & 1u;
+                }
+            }
+            out |= (uint32_t)(cnt >= 13) << b;
+        }
+    }
+    core[(size_t)y * wpr + wx] = out;
 }
 
 }  // namespace lac

@@ -13,6 +13,7 @@
 #include "select.cuh"
 #include "compact.cuh"
 #include "probe.cuh"
+#include "sepmed.cuh"
 
 namespace {
 
@@ -118,7 +119,7 @@ DeviceInfo device_info() {
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_noise, lac::k_noise_S_tma, lac::NT,
                                                       lac::NS_SMEM_BYTES) != cudaSuccess) return d;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_quads, lac::k_noise_S_quads, 256, 0) != cudaSuccess) return d;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_eval, lac::k_eval_candidates, 128, 0) != cudaSuccess) return d;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_eval, lac::k_eval_candidates<0>, 128, 0) != cudaSuccess) return d;
     d.ok = d.sms > 0 && d.occ_fine > 0 && d.occ_noise > 0 && d.occ_quads > 0 && d.occ_eval > 0;
     return d;
 }
@@ -154,6 +155,7 @@ struct Workspace {
     int32_t* clist;    // compacted candidate pixel list (capacity h*w)
     int32_t* qlist;    // compacted quad list of the incremental noise/S pass (capacity h*ceil(w/4))
     uint32_t *G1, *G2, *G2F, *M1, *M2, *M3, *C[2], *A1, *A2, *NEED;
+    uint32_t *NOK, *DONX;  // R23 / R25: pixels never flagged (bad pixels | extended saturated-star mask); bad pixels
     int32_t* counts;   // per iteration: newly flagged pixels
     int32_t* ncand;    // per iteration (lazy path): candidate pixels evaluated
     int32_t* nquad;    // per iteration (lazy path): quads the incremental noise/S pass recomputed
@@ -175,7 +177,8 @@ Workspace carve(void* base, int h, int w) {
     ws.S = (float*)(p + off); off += plane;
     ws.clist = (int32_t*)(p + off); off += plane;
     ws.qlist = (int32_t*)(p + off); off += align_up((size_t)h * ((w + 3) / 4) * 4, 256);
-    uint32_t** planes[] = {&ws.G1, &ws.G2, &ws.G2F, &ws.M1, &ws.M2, &ws.M3, &ws.C[0], &ws.C[1], &ws.A1, &ws.A2, &ws.NEED};
+    uint32_t** planes[] = {&ws.G1, &ws.G2, &ws.G2F, &ws.M1, &ws.M2, &ws.M3, &ws.C[0], &ws.C[1], &ws.A1, &ws.A2, &ws.NEED,
+                           &ws.NOK, &ws.DONX};
     for (uint32_t** pl : planes) { *pl = (uint32_t*)(p + off); off += bp; }
     ws.stripflag = (uint8_t*)(p + off);
     off += align_up((size_t)((words_per_row(w) + lac::WG_OWN - 1) / lac::WG_OWN) * ((h + lac::WG_R - 1) / lac::WG_R + lac::WG_WARPS), 256);
@@ -261,17 +264,68 @@ __global__ void k_fill_floats(float* dst, int n, float v) {
     for (int i = threadIdx.x; i < n; i += blockDim.x) dst[i] = v;
 }
 
-// The iteration loop (O0-O7) for one frame.
+int pack_bits(const uint8_t* mask_u8, uint32_t* bits, int h, int w, uint32_t* or_into, cudaStream_t st) {
+    const unsigned nbx = (unsigned)((w + 255) / 256);
+    lac::k_pack_bits<<<nbx * (unsigned)h, 256, 0, st>>>(mask_u8, bits, h, w, words_per_row(w), (int)nbx, or_into);
+    LAUNCHED();
+    return LACOSMIC_OK;
+}
+
+// R25: out = (med5(img) >= satlevel) dilated `grow` times (3x3); tmp: a second bit-plane
+int satstar_bits(const float* img, int h, int w, float satlevel, int grow, uint32_t* out, uint32_t* tmp, cudaStream_t st) {
+    const int wpr = words_per_row(w);
+    const unsigned nbx = (unsigned)((w + 255) / 256), nbw = (unsigned)((wpr + 255) / 256);
+    // the plane that ends up in `out` after `grow` ping-pong dilations
+    uint32_t* a = (grow & 1) ? tmp : out;
+    uint32_t* b = (grow & 1) ? out : tmp;
+    lac::k_pack_ge<<<nbx * (unsigned)h, 256, 0, st>>>(img, satlevel, b, h, w, wpr, (int)nbx);
+    LAUNCHED();
+    lac::k_satcore<<<nbw * (unsigned)h, 256, 0, st>>>(b, a, h, w, wpr, (int)nbw);
+    LAUNCHED();
+    for (int j = 0; j < grow; ++j) {
+        lac::k_dilate3<<<bit_grid(h, w), 256, 0, st>>>(a, b, h, w, wpr, bit_nbx(w));
+        LAUNCHED();
+        std::swap(a, b);
+    }
+    return LACOSMIC_OK;   // a == out
+}
+
+inline int check_variant(const lacosmic_variant* v) {
+    if (!v) return LACOSMIC_OK;
+    if (v->fsmode != LACOSMIC_FS_ADU && v->fsmode != LACOSMIC_FS_NORMALISED) return LACOSMIC_ERR_PARAM;
+    if (v->satgrow < -1 || v->satgrow > LACOSMIC_MAX_SATGROW) return LACOSMIC_ERR_PARAM;
+    if ((uintptr_t)v->var & 15) return LACOSMIC_ERR_ALIGN;
+    return LACOSMIC_OK;
+}
+
+// The iteration loop (O0-O7) for one frame.  vr: nullable variants (R22-R25).
 int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t* mask_out,
               float* clean_out, const Workspace& ws, int32_t* iter_counts, const lacosmic_debug* dbg,
-              cudaStream_t st) {
+              cudaStream_t st, const lacosmic_variant* vr = nullptr) {
     const size_t P = (size_t)h * w;
     const int wpr = words_per_row(w);
     const size_t bp_bytes = (size_t)h * wpr * 4;
     float* work = clean_out;
     Span whole(KC_STEP, st);   // the whole frame, copies included
     const bool lazy = p.mode == LACOSMIC_MODE_LAZY;
-    const bool estimate = p.gain == 0.0f;   // R21: no gain supplied
+    const float* var = vr ? vr->var : nullptr;                        // R24
+    const bool fs1 = vr && vr->fsmode == LACOSMIC_FS_NORMALISED;      // R22
+    const bool estimate = p.gain == 0.0f && !var;   // R21: no gain supplied (a variance plane replaces the noise model)
+    // R23 / R25: the planes of the pixels never flagged / never donors, fixed for the frame
+    const uint32_t *nok = nullptr, *donx = nullptr;
+    if (vr && p.niter > 0 && (vr->bpm || vr->satgrow >= 0)) {
+        int rc;
+        if (vr->satgrow >= 0) {
+            if ((rc = satstar_bits(img, h, w, p.satlevel, vr->satgrow, ws.NOK, ws.M2, st))) return rc;
+        } else {
+            CK(cudaMemsetAsync(ws.NOK, 0, bp_bytes, st));
+        }
+        if (vr->bpm) {
+            if ((rc = pack_bits(vr->bpm, ws.DONX, h, w, ws.NOK, st))) return rc;
+            donx = ws.DONX;
+        }
+        nok = ws.NOK;
+    }
     // O0.  The lazy path fuses work = img_in into its first pass (which then reads img_in itself).
     const bool fused_copy = lazy && p.niter > 0;
     if (!fused_copy) CK(cudaMemcpyAsync(work, img, P * 4, cudaMemcpyDeviceToDevice, st));
@@ -337,11 +391,15 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         // rewrote (ws.NEED); a debug dump recomputes the planes everywhere, and so does an estimated gain
         // (it changes with every iteration, and S with it)
         const bool incr = lazy && t > 0 && !d && !estimate;
-        lac::NoiseArgs na{ws.S, d ? dbg->Lp : nullptr, d ? dbg->N : nullptr,
+        // R22 in the dense path: the gate kernel reads the noise plane, which the noise/S pass stores in the
+        // candidate list's storage (not used by the dense path; free again once a gain estimate has been selected)
+        float* const nplane = (d && dbg->N) ? dbg->N : ((fs1 && !lazy) ? (float*)ws.clist : nullptr);
+        lac::NoiseArgs na{ws.S, d ? dbg->Lp : nullptr, nplane,
                           lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
                           (fused_copy && t == 0 && !estimate) ? work : nullptr,
                           h, w, wpr, p.gain, rn2, p.sigclip, siglow, p.satlevel, nullptr,
-                          estimate ? ws.gains + t : nullptr, (t == 0 && !estimate) ? zero_ptr : nullptr, zero_n};
+                          estimate ? ws.gains + t : nullptr, (t == 0 && !estimate) ? zero_ptr : nullptr, zero_n,
+                          nok, var};
         if (incr) {
             {
                 Span sp(KC_LISTS, st);
@@ -355,12 +413,13 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                 LAUNCHED();
             }
         } else {
-            if (estimate) {
-                // the residual pass left med5(work) in the S plane: S, A1, A2 follow elementwise (HBM bound)
+            if (estimate || var) {
+                // the residual pass left med5(work) in the S plane (R21), or N comes from the variance plane (R24):
+                // S, A1, A2 follow elementwise (HBM bound)
                 Span sp(KC_NOISE_S, st);
                 const unsigned nbx = (unsigned)((w + 127) / 128);
-                if (tma) lac::k_S_from_m5<<<nbx * (unsigned)((h + 8 * lac::SM5_ROWS - 1) / (8 * lac::SM5_ROWS)), 256, 0, st>>>(work, na, (int)nbx, prev);
-                else lac::k_S_from_m5_generic<<<nbx * (unsigned)((h + 7) / 8), 256, 0, st>>>(work, na, (int)nbx, prev);
+                if (tma) lac::k_S_from_m5<<<nbx * (unsigned)((h + 8 * lac::SM5_ROWS - 1) / (8 * lac::SM5_ROWS)), 256, 0, st>>>(src, na, (int)nbx, prev);
+                else lac::k_S_from_m5_generic<<<nbx * (unsigned)((h + 7) / 8), 256, 0, st>>>(src, na, (int)nbx, prev);
                 LAUNCHED();
             } else if ((rc = noise_pass(na, src))) {
                 return rc;
@@ -374,13 +433,15 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         }
         if (lazy) {
             // steps (3b)-(5) on the listed candidates only (lazy.cuh)
-            lac::CandArgs ca{ws.S, work, ws.G1, ws.G2, ws.M1, h, w, wpr, p.sigclip, siglow, p.objlim};
+            lac::CandArgs ca{ws.S, work, ws.G1, ws.G2, ws.M1, h, w, wpr, p.sigclip, siglow, p.objlim,
+                             p.gain, rn2, estimate ? ws.gains + t : nullptr, var};
             Span sp(KC_EVAL, st);
-            lac::k_eval_candidates<<<gridE, 128, 0, st>>>(ca, ws.clist, ws.ncand + t, prev);
+            if (fs1) lac::k_eval_candidates<1><<<gridE, 128, 0, st>>>(ca, ws.clist, ws.ncand + t, prev);
+            else lac::k_eval_candidates<0><<<gridE, 128, 0, st>>>(ca, ws.clist, ws.ncand + t, prev);
             LAUNCHED();
         } else {
             lac::FineArgs fa{ws.G1, ws.G2, ws.M1, d ? dbg->Sp : nullptr, d ? dbg->m3 : nullptr,
-                             d ? dbg->F : nullptr, h, w, wpr, gp};
+                             d ? dbg->F : nullptr, h, w, wpr, gp, fs1 ? nplane : nullptr, nok};
             Span sp(KC_FINE_GATES, st);
             if (tma) lac::k_fine_gates_tma<<<gridFG, tb, lac::FG_SMEM_BYTES, st>>>(mapWorkFG, mapS, fa, ntx, ntiles, prev);
             else lac::k_fine_gates<<<(unsigned)ntiles, tb, 0, st>>>(work, ws.S, fa, ntx, prev);
@@ -390,7 +451,8 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         // steps (6)-(7), fused; in the lazy path G2 is completed on the pixels the second growth reaches
         lac::GrowArgs ga{ws.M1, ws.G1, ws.G2, ws.G2F, lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
                          ws.C[t & 1], ws.C[(t + 1) & 1], ws.NEED, d ? ws.M2 : nullptr, d ? ws.M3 : nullptr,
-                         ws.S, img, work, ws.counts + t, incr ? ws.stripflag : nullptr, h, w, wpr, siglow, grow_nbx(w)};
+                         ws.S, img, work, ws.counts + t, incr ? ws.stripflag : nullptr, h, w, wpr, siglow, grow_nbx(w),
+                         donx};
         if ((rc = grow_replace(ga, prev, st))) return rc;
         if (d) {
             // lazy path: G2 is only evaluated where step (6) needs it, so it is not dumped
@@ -416,6 +478,72 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         CK(cudaMemcpyAsync(dbg->gains, ws.gains, (size_t)p.niter * 4, cudaMemcpyDeviceToDevice, st));
     }
     return LACOSMIC_OK;
+}
+
+// R26 (comparison only): out = sepmedK(in), tmp = the row pass
+int sepmed(const float* in, float* out, float* tmp, int h, int w, int k, cudaStream_t st) {
+    const unsigned g = (unsigned)(((size_t)h * w + 255) / 256);
+    if (k == 3) { lac::k_sepmed_pass<3, true><<<g, 256, 0, st>>>(in, tmp, h, w); lac::k_sepmed_pass<3, false><<<g, 256, 0, st>>>(tmp, out, h, w); }
+    else if (k == 5) { lac::k_sepmed_pass<5, true><<<g, 256, 0, st>>>(in, tmp, h, w); lac::k_sepmed_pass<5, false><<<g, 256, 0, st>>>(tmp, out, h, w); }
+    else { lac::k_sepmed_pass<7, true><<<g, 256, 0, st>>>(in, tmp, h, w); lac::k_sepmed_pass<7, false><<<g, 256, 0, st>>>(tmp, out, h, w); }
+    g_launches += 1;
+    LAUNCHED();
+    return LACOSMIC_OK;
+}
+
+// O0-O7 with every median replaced by the separable one (R26).  Planes: A = ws.S, B = the candidate list's storage,
+// C3 = `third` (the extra plane of lacosmic_sepmed_workspace_bytes).
+int run_sepmed_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t* mask_out, float* clean_out,
+                     const Workspace& ws, float* third, int32_t* iter_counts, const lacosmic_debug* dbg, cudaStream_t st) {
+    const size_t P = (size_t)h * w;
+    const int wpr = words_per_row(w);
+    const size_t bp_bytes = (size_t)h * wpr * 4;
+    float *work = clean_out, *A = ws.S, *B = (float*)ws.clist, *C3 = third;
+    CK(cudaMemcpyAsync(work, img, P * 4, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemsetAsync(ws.C[0], 0, bp_bytes, st));
+    CK(cudaMemsetAsync((char*)ws.S + ws.zero_off, 0, ws.zero_bytes, st));
+    const float siglow = p.sigfrac * p.sigclip, rn2 = p.readnoise * p.readnoise;
+    const unsigned gw = (unsigned)(((size_t)h * wpr + 7) / 8);
+    for (int t = 0; t < p.niter; ++t) {
+        const int* prev = t > 0 ? ws.counts + (t - 1) : nullptr;
+        const bool d = dbg && dbg->iter == t;
+        int rc;
+        // O2, O3a: A = sepmed5(work), then S in place (with L+ and N)
+        if ((rc = sepmed(work, A, B, h, w, 5, st))) return rc;
+        lac::NoiseArgs na{A, d ? dbg->Lp : nullptr, d ? dbg->N : nullptr, nullptr, nullptr, nullptr, h, w, wpr,
+                          p.gain, rn2, p.sigclip, siglow, p.satlevel, nullptr, nullptr, nullptr, 0};
+        const unsigned nbx = (unsigned)((w + 127) / 128);
+        lac::k_S_from_m5_generic<<<nbx * (unsigned)((h + 7) / 8), 256, 0, st>>>(work, na, (int)nbx, nullptr);
+        LAUNCHED();
+        if (d && dbg->S) CK(cudaMemcpyAsync(dbg->S, A, P * 4, cudaMemcpyDeviceToDevice, st));
+        // O3b, O5: C3 = sepmed5(S); G1, G2
+        if ((rc = sepmed(A, C3, B, h, w, 5, st))) return rc;
+        lac::SepGateArgs ga{work, A, C3, nullptr, nullptr, ws.G1, ws.G2, ws.M1, d ? dbg->Sp : nullptr, d ? dbg->F : nullptr,
+                            h, w, wpr, p.sigclip, siglow, p.objlim, p.satlevel};
+        lac::k_sep_gates<0><<<gw, 256, 0, st>>>(ga);
+        LAUNCHED();
+        // O4, O5: A = m3 = sepmed3(work); C3 = sepmed7(m3); M1
+        if ((rc = sepmed(work, A, B, h, w, 3, st))) return rc;
+        if (d && dbg->m3) CK(cudaMemcpyAsync(dbg->m3, A, P * 4, cudaMemcpyDeviceToDevice, st));
+        if ((rc = sepmed(A, C3, B, h, w, 7, st))) return rc;
+        ga.m3 = A;
+        ga.m7 = C3;
+        lac::k_sep_gates<1><<<gw, 256, 0, st>>>(ga);
+        LAUNCHED();
+        // O6, O7: the product kernel (G2 complete, as in the dense path)
+        lac::GrowArgs gr{ws.M1, ws.G1, ws.G2, ws.G2F, nullptr, nullptr, ws.C[t & 1], ws.C[(t + 1) & 1], ws.NEED,
+                         d ? ws.M2 : nullptr, d ? ws.M3 : nullptr, A, img, work, ws.counts + t, nullptr, h, w, wpr, siglow,
+                         grow_nbx(w), nullptr};
+        if ((rc = grow_replace(gr, prev, st))) return rc;
+        if (d) {
+            struct { const uint32_t* b; uint8_t* o; } planes[] = {{ws.G1, dbg->G1}, {ws.G2, dbg->G2}, {ws.M1, dbg->M1},
+                                                                 {ws.M2, dbg->M2}, {ws.M3, dbg->M3}, {ws.C[(t + 1) & 1], dbg->C}};
+            for (auto& pl : planes)
+                if (pl.o && (rc = unpack(pl.b, pl.o, h, w, st))) return rc;
+        }
+    }
+    const bool want_counts = iter_counts && p.niter > 0;
+    return unpack(ws.C[p.niter & 1], mask_out, h, w, st, ws.counts, want_counts ? iter_counts : nullptr, p.niter);
 }
 
 // Internal streams of lacosmic_run_batch (per calling thread and device, created on first use, kept for the
@@ -482,6 +610,25 @@ int lacosmic_run_ws(const float* img, int h, int w, const lacosmic_params* p, ui
             if ((uintptr_t)pl & 15) return LACOSMIC_ERR_ALIGN;
     return run_frame(img, h, w, *p, mask_out, clean_out, carve(workspace, h, w), iter_counts, dbg,
                      (cudaStream_t)stream);
+}
+
+int lacosmic_run_ex(const float* img, int h, int w, const lacosmic_params* p, const lacosmic_variant* v,
+                    uint8_t* mask_out, float* clean_out, void* workspace, size_t workspace_bytes,
+                    int32_t* iter_counts, const lacosmic_debug* dbg, void* stream) {
+    g_launches = 0;
+    int rc = check_frame_args(img, h, w, p, mask_out, clean_out, workspace, workspace_bytes);
+    if (rc) return rc;
+    if ((rc = check_variant(v))) return rc;
+    if (dbg && (dbg->iter < -1 || dbg->iter >= LACOSMIC_MAX_NITER)) return LACOSMIC_ERR_PARAM;
+    if (dbg)
+        for (const float* pl : {dbg->Lp, dbg->N, dbg->S, dbg->Sp, dbg->m3, dbg->F})
+            if ((uintptr_t)pl & 15) return LACOSMIC_ERR_ALIGN;
+    const size_t P = (size_t)h * w;
+    if (v && ((v->bpm && (overlap(v->bpm, P, clean_out, P * 4) || overlap(v->bpm, P, mask_out, P))) ||
+              (v->var && (overlap(v->var, P * 4, clean_out, P * 4) || overlap(v->var, P * 4, mask_out, P)))))
+        return LACOSMIC_ERR_ALIAS;
+    return run_frame(img, h, w, *p, mask_out, clean_out, carve(workspace, h, w), iter_counts, dbg,
+                     (cudaStream_t)stream, v);
 }
 
 int lacosmic_run(const float* img, int h, int w, float gain, float readnoise, float sigclip,
@@ -835,10 +982,7 @@ int lacosmic_pack_bits(const uint8_t* mask_u8, uint32_t* bits, int h, int w, voi
     if (!mask_u8 || !bits) return LACOSMIC_ERR_NULL;
     int rc = check_shape(h, w);
     if (rc) return rc;
-    const unsigned nbx = (unsigned)((w + 255) / 256);
-    lac::k_pack_bits<<<nbx * (unsigned)h, 256, 0, (cudaStream_t)stream>>>(mask_u8, bits, h, w, words_per_row(w), (int)nbx);
-    LAUNCHED();
-    return LACOSMIC_OK;
+    return pack_bits(mask_u8, bits, h, w, nullptr, (cudaStream_t)stream);
 }
 
 int lacosmic_unpack_bits(const uint32_t* bits, uint8_t* mask_u8, int h, int w, void* stream) {
@@ -861,6 +1005,59 @@ int lacosmic_dilate3(const uint32_t* bits_in, uint32_t* bits_out, int h, int w, 
 
 int lacosmic_masked_median(const float* img, const uint8_t* mask_u8, float* out, int h, int w,
                            void* workspace, size_t workspace_bytes, void* stream) {
+    return lacosmic_masked_median_bpm(img, mask_u8, nullptr, out, h, w, workspace, workspace_bytes, stream);
+}
+
+int lacosmic_satstar_mask(const float* img, int h, int w, float satlevel, int grow, uint8_t* out_u8, void* workspace,
+                          size_t workspace_bytes, void* stream) {
+    g_launches = 0;
+    if (!img || !out_u8 || !workspace) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    if (std::isnan(satlevel) || grow < 0 || grow > LACOSMIC_MAX_SATGROW) return LACOSMIC_ERR_PARAM;
+    if ((uintptr_t)workspace & 255) return LACOSMIC_ERR_ALIGN;
+    if (workspace_bytes < lacosmic_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
+    Workspace ws = carve(workspace, h, w);
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = satstar_bits(img, h, w, satlevel, grow, ws.NOK, ws.M2, st))) return rc;
+    return unpack(ws.NOK, out_u8, h, w, st);
+}
+
+int lacosmic_sepmedfilt(const float* in, float* out, float* tmp, int h, int w, int k, void* stream) {
+    g_launches = 0;
+    if (!in || !out || !tmp) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    if (k != 3 && k != 5 && k != 7) return LACOSMIC_ERR_PARAM;
+    const size_t B = (size_t)h * w * 4;
+    if (overlap(in, B, out, B) || overlap(in, B, tmp, B) || overlap(out, B, tmp, B)) return LACOSMIC_ERR_ALIAS;
+    return sepmed(in, out, tmp, h, w, k, (cudaStream_t)stream);
+}
+
+size_t lacosmic_sepmed_workspace_bytes(int h, int w) {
+    if (check_shape(h, w)) return 0;
+    return align_up(lacosmic_workspace_bytes(h, w), 256) + align_up((size_t)h * w * 4, 256);
+}
+
+int lacosmic_run_sepmed_compare(const float* img, int h, int w, const lacosmic_params* p, uint8_t* mask_out,
+                                float* clean_out, void* workspace, size_t workspace_bytes, int32_t* iter_counts,
+                                const lacosmic_debug* dbg, void* stream) {
+    g_launches = 0;
+    int rc = check_frame_args(img, h, w, p, mask_out, clean_out, workspace, lacosmic_workspace_bytes(h, w));
+    if (rc) return rc;
+    if (p->gain == 0.0f) return LACOSMIC_ERR_PARAM;      // the comparison path takes a supplied gain only
+    if (workspace_bytes < lacosmic_sepmed_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
+    if (dbg && (dbg->iter < -1 || dbg->iter >= LACOSMIC_MAX_NITER)) return LACOSMIC_ERR_PARAM;
+    const size_t P = (size_t)h * w, need = lacosmic_sepmed_workspace_bytes(h, w);
+    if (overlap(workspace, need, img, P * 4) || overlap(workspace, need, clean_out, P * 4) || overlap(workspace, need, mask_out, P))
+        return LACOSMIC_ERR_ALIAS;
+    Workspace ws = carve(workspace, h, w);
+    float* third = (float*)((char*)workspace + align_up(ws.bytes, 256));
+    return run_sepmed_frame(img, h, w, *p, mask_out, clean_out, ws, third, iter_counts, dbg, (cudaStream_t)stream);
+}
+
+int lacosmic_masked_median_bpm(const float* img, const uint8_t* mask_u8, const uint8_t* bpm_u8, float* out, int h, int w,
+                               void* workspace, size_t workspace_bytes, void* stream) {
     if (!img || !mask_u8 || !out || !workspace) return LACOSMIC_ERR_NULL;
     int rc = check_shape(h, w);
     if (rc) return rc;
@@ -874,11 +1071,12 @@ int lacosmic_masked_median(const float* img, const uint8_t* mask_u8, float* out,
     // the fused growth/replacement kernel with M1 = G1 = G2 = mask and C = 0 flags exactly the mask
     // (M2 = dil3(mask) & mask, M3 likewise) and replaces every pixel of it
     if ((rc = lacosmic_pack_bits(mask_u8, ws.M1, h, w, stream))) return rc;
+    if (bpm_u8 && (rc = lacosmic_pack_bits(bpm_u8, ws.DONX, h, w, stream))) return rc;
     CK(cudaMemcpyAsync(out, img, P * 4, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemsetAsync(ws.C[0], 0, (size_t)h * wpr * 4, st));
     CK(cudaMemsetAsync(ws.counts, 0, 4, st));
     lac::GrowArgs ga{ws.M1, ws.M1, ws.M1, nullptr, nullptr, nullptr, ws.C[0], ws.C[1], ws.NEED, nullptr, nullptr,
-                     nullptr, img, out, ws.counts, nullptr, h, w, wpr, 0.0f, grow_nbx(w)};
+                     nullptr, img, out, ws.counts, nullptr, h, w, wpr, 0.0f, grow_nbx(w), bpm_u8 ? ws.DONX : nullptr};
     return grow_replace(ga, nullptr, st);
 }
 

@@ -90,13 +90,19 @@ struct CandArgs {
     uint32_t *G1, *G2, *M1;
     int h, w, wpr;
     float sigclip, siglow, objlim;
+    // R22 (fsmode 1) only: what N at the candidate is made of
+    float gain, rn2;
+    const float* gain_dev;   // nullable (R21)
+    const float* var;        // nullable (R24)
 };
 
-// P(v) of the header comment, with exactly the operations of O4/O5
-__device__ __forceinline__ bool fine_test(float lp, float m3c, float v, float objlim) {
-    const float d = __fsub_rn(m3c, v);
+// P(v) of the header comment, with exactly the operations of O4/O5.  nn == 0: R7 (num = L+, F in ADU); nn > 0: R22
+// (num = S', F divided by the noise nn) -- non-decreasing in v in both forms because num > 0 wherever it is evaluated.
+__device__ __forceinline__ bool fine_test(float num, float m3c, float v, float objlim, float nn = 0.0f) {
+    float d = __fsub_rn(m3c, v);
+    if (nn > 0.0f) d = __fdiv_rn(d, nn);
     const float f = d > 0.01f ? d : 0.01f;
-    return __fdiv_rn(lp, f) > objlim;
+    return __fdiv_rn(num, f) > objlim;
 }
 
 // bit k = P(e[k]).  P is non-decreasing in v and (tlo, thi) brackets its switch point: P(v) is false for
@@ -104,7 +110,7 @@ __device__ __forceinline__ bool fine_test(float lp, float m3c, float v, float ob
 // inside the bracket need the division.  tlo = -inf, thi = +inf evaluates every value exactly.
 template <int N>
 __device__ __forceinline__ uint32_t fine_bits(const float (&e)[N], float lp, float m3c, float objlim, float tlo,
-                                              float thi) {
+                                              float thi, float nn = 0.0f) {
     uint32_t m = 0, amb = 0;
 #pragma unroll
     for (int k = 0; k < N; ++k) {
@@ -114,7 +120,7 @@ __device__ __forceinline__ uint32_t fine_bits(const float (&e)[N], float lp, flo
     if (amb) {
 #pragma unroll
         for (int k = 0; k < N; ++k)
-            if ((amb >> k) & 1u) m |= (uint32_t)fine_test(lp, m3c, e[k], objlim) << k;
+            if ((amb >> k) & 1u) m |= (uint32_t)fine_test(lp, m3c, e[k], objlim, nn) << k;
     }
     return m;
 }
@@ -175,6 +181,10 @@ __device__ __forceinline__ bool fine_bracket(float lp, float m3c, float objlim, 
 #ifndef LAC_EVAL_MINB
 #define LAC_EVAL_MINB 6
 #endif
+// FS = 1 (R22): the test compares S' = S - med5(S) with objlim * Fn, Fn = F / N: med5(S) and med5(work) (for N) are
+// selected exactly at the candidate (25-input network), then the same counting over the 9x9 window decides, every
+// tap evaluated with the exact operations (no bracket).
+template <int FS>
 __global__ void __launch_bounds__(128, LAC_EVAL_MINB)
 k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restrict__ nlist,
                   const int* prev_count) {
@@ -203,17 +213,43 @@ k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restric
 #pragma unroll
                 for (int c = 0; c < 3; ++c)
                     ctr[r][c] = __ldg(a.work + (size_t)clampi(y + r - 1, 0, h - 1) * w + xx[3 + c]);
-            const float lp = lplus_px(ctr[1][1], ctr[0][1], ctr[2][1], ctr[1][0], ctr[1][2]);
+            float lp = lplus_px(ctr[1][1], ctr[0][1], ctr[2][1], ctr[1][0], ctr[1][2]);
             const float m3c = med9(ctr[0][0], ctr[0][1], ctr[0][2], ctr[1][0], ctr[1][1], ctr[1][2], ctr[2][0],
                                    ctr[2][1], ctr[2][2]);
-            if (!fine_bracket(lp, m3c, a.objlim, tlo, thi)) continue;
+            float nn = 0.0f;
+            if (FS == 1) {
+                float v[25], srt[25];
+#pragma unroll
+                for (int dy = 0; dy < 5; ++dy)
+#pragma unroll
+                    for (int dx = 0; dx < 5; ++dx)
+                        v[5 * dy + dx] = __ldg(a.S + (size_t)clampi(y + dy - 2, 0, h - 1) * w + xx[2 + dx]);
+                const float sc = v[12];
+                sort25(v, srt);
+                lp = __fsub_rn(sc, srt[12]);                  // the numerator of R22 is S'
+                if (a.var) {
+                    nn = noise_from_var(__ldg(a.var + (size_t)y * w + x));
+                } else {
+#pragma unroll
+                    for (int dy = 0; dy < 5; ++dy)
+#pragma unroll
+                        for (int dx = 0; dx < 5; ++dx)
+                            v[5 * dy + dx] = __ldg(a.work + (size_t)clampi(y + dy - 2, 0, h - 1) * w + xx[2 + dx]);
+                    sort25(v, srt);
+                    nn = noise_px(srt[12], a.gain_dev ? __ldg(a.gain_dev) : a.gain, a.rn2);
+                }
+                tlo = -__int_as_float(0x7f800000);
+                thi = __int_as_float(0x7f800000);
+            } else if (!fine_bracket(lp, m3c, a.objlim, tlo, thi)) {
+                continue;
+            }
 #pragma unroll 3
             for (int r = 0; r < 9; ++r) {
                 const float* row = a.work + (size_t)clampi(y + r - 4, 0, h - 1) * w;
                 float f[9];
 #pragma unroll
                 for (int c = 0; c < 9; ++c) f[c] = __ldg(row + xx[c]);
-                const uint32_t m = fine_bits<9>(f, lp, m3c, a.objlim, tlo, thi);
+                const uint32_t m = fine_bits<9>(f, lp, m3c, a.objlim, tlo, thi, nn);
 #pragma unroll
                 for (int k = 0; k < 9; ++k) rows[k] = (k == r) ? m : rows[k];
             }
@@ -267,12 +303,19 @@ k_noise_S_quads(const float* __restrict__ work, NoiseArgs a, const int* __restri
                 }
             }
             float m5[4], s[4];
-            median5x5_x4(win, m5);
+            if (a.var) {                                   // R24: N comes from the variance plane, no median
+#pragma unroll
+                for (int j = 0; j < 4; ++j) m5[j] = __ldg(a.var + (size_t)y * w + min(x + j, w - 1));
+            } else {
+                median5x5_x4(win, m5);
+            }
             uint32_t n2 = 0;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const float lp = lplus_px(win[2 + j][2], win[2 + j][1], win[2 + j][3], win[1 + j][2], win[3 + j][2]);
-                s[j] = fdiv_nn(lp, __fmul_rn(2.0f, noise_px(m5[j], a.gain_dev ? __ldg(a.gain_dev) : a.gain, a.rn2)));
+                const float nn = a.var ? noise_from_var(m5[j])
+                                       : noise_px(m5[j], a.gain_dev ? __ldg(a.gain_dev) : a.gain, a.rn2);
+                s[j] = fdiv_nn(lp, __fmul_rn(2.0f, nn));
                 const bool ok = (x + j < w) && (win[2 + j][2] < a.satlevel);                    // R12
                 n1 |= (uint32_t)(ok && s[j] > a.sigclip) << j;
                 n2 |= (uint32_t)(ok && s[j] > a.siglow) << j;
@@ -281,6 +324,11 @@ k_noise_S_quads(const float* __restrict__ work, NoiseArgs a, const int* __restri
             // this thread alone owns its nibble of the A1 / A2 words; the other nibbles change concurrently
             const size_t q = (size_t)y * a.wpr + (x >> 5);
             const int sh = x & 31;
+            if (a.nok) {                                   // R23 / R25: never flagged
+                const uint32_t nk = (a.nok[q] >> sh) & 0xFu;
+                n1 &= ~nk;
+                n2 &= ~nk;
+            }
             const uint32_t o1 = (a.A1[q] >> sh) & 0xFu, o2 = (a.A2[q] >> sh) & 0xFu;
             if (o1 != n1) atomicXor(a.A1 + q, (o1 ^ n1) << sh);
             if (o2 != n2) atomicXor(a.A2 + q, (o2 ^ n2) << sh);

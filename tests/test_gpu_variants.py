@@ -1,0 +1,250 @@
+"""GPU parity tests (-m gpu) of the variants of DESIGN.md R22-R26: the CUDA path through the
+C ABI (lacosmic_run_ex, lacosmic_run_sepmed_compare, single steps) against the oracle's orc_run_ex, bit for bit, in both
+evaluation modes."""
+import numpy as np
+import pytest
+
+from paper_2602_17938_b200 import synth
+
+pytestmark = pytest.mark.gpu
+PARAMS = dict(synth.DEFAULT_PARAMS)
+MODES = ["lazy", "dense"]
+LAZY_SKIPS = ("Sp", "m3", "F", "G2")
+
+
+@pytest.fixture(scope="module")
+def lc():
+    import torch
+    assert torch.cuda.is_available(), "-m gpu tests need a CUDA device"
+    import paper_2602_17938_b200 as lc
+    lc.load_library()
+    return lc
+
+
+def _t(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _n(t):
+    return t.cpu().numpy()
+
+
+def _rng(seed):
+    return np.random.Generator(np.random.Philox(seed))
+
+
+def _compare(lc, orc, img, p, mode, debug_iter=None, label="", **variant):
+    import torch
+    o = orc.run(img, debug_iter=debug_iter, **variant, **p)
+    kw = {k: (_t(v) if isinstance(v, np.ndarray) else v) for k, v in variant.items()}
+    g = lc.lacosmic_run_ex(_t(img), lc.Params(mode=lc.MODE_LAZY if mode == "lazy" else lc.MODE_DENSE, **p),
+                           debug_iter=debug_iter, want_gains=True, **kw)
+    torch.cuda.synchronize()
+    tag = "%s [%s] %s" % (label, mode, {k: (v if not isinstance(v, np.ndarray) else "plane") for k, v in variant.items()})
+    assert np.array_equal(_n(g["mask"]), o["mask"]), tag
+    assert np.array_equal(_n(g["clean"]), o["clean"]), tag
+    assert np.array_equal(_n(g["counts"])[:p["niter"]], o["counts"]), tag
+    if debug_iter is not None and debug_iter < p["niter"] and np.all(o["counts"][:debug_iter] > 0):
+        for name in ("Lp", "N", "S", "Sp", "m3", "F", "G1", "G2", "M1", "M2", "M3", "C"):
+            if mode == "lazy" and name in LAZY_SKIPS:
+                continue
+            assert np.array_equal(_n(g[name]), o[name]), (tag, name)
+    return o, g
+
+
+def _frame(h=170, w=230, seed=81, n_sat=6):
+    return synth.make_frame(h, w, seed=seed, n_star=12, n_cr=160, n_hot=30, sp_frac=0.006, n_sat=n_sat)
+
+
+# ---------------------------------------------------------------- R22: noise-normalised fine structure
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("shape", [(170, 230), (97, 131), (1, 40), (5, 3), (64, 128)])
+def test_normalised_fine_structure(lc, orc, mode, shape):
+    f = _frame(*shape)
+    for dbg in (0, 1, None):
+        _compare(lc, orc, f.img, PARAMS, mode, dbg, "R22", fsmode=1)
+    _compare(lc, orc, f.img, dict(PARAMS, gain=2.3, readnoise=4.0, objlim=2.0), mode, 0, "R22 gain", fsmode=1)
+    _compare(lc, orc, f.img, dict(PARAMS, gain=0.0), mode, 1, "R22 estimated gain", fsmode=1)
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_normalised_fine_structure_worked_frame(lc, orc, mode):
+    """The decision table of tests/test_oracle_variants.py (spikes on 5x5 plateaus): R7 flags four, R22 three."""
+    img = np.full((40, 120), 100.0, np.float32)
+    for i, A in enumerate([100.0, 150.0, 250.0, 400.0, 1000.0]):
+        x0 = 10 + 22 * i
+        img[18:23, x0:x0 + 5] += 40.0
+        img[20, x0 + 2] += A
+    o0, _ = _compare(lc, orc, img, PARAMS, mode, 0, "worked", fsmode=0)
+    o1, _ = _compare(lc, orc, img, PARAMS, mode, 0, "worked", fsmode=1)
+    assert [int(o0["M1"][20, 12 + 22 * i]) for i in range(5)] == [0, 1, 1, 1, 1]
+    assert [int(o1["M1"][20, 12 + 22 * i]) for i in range(5)] == [0, 0, 1, 1, 1]
+
+
+# ---------------------------------------------------------------- R23: bad pixels
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("shape", [(170, 230), (97, 131), (3, 70), (64, 128)])
+def test_bad_pixel_mask(lc, orc, mode, shape):
+    f = _frame(*shape)
+    base = orc.run(f.img, **PARAMS)
+    bpm = (_rng(7).random(shape) < 0.02).astype(np.uint8)
+    ys, xs = np.nonzero(base["mask"])
+    bpm[ys[::3], xs[::3]] = 1
+    for dbg in (0, 2, None):
+        o, _ = _compare(lc, orc, f.img, PARAMS, mode, dbg, "R23", bpm=bpm)
+    assert not (o["mask"] & bpm).any()
+    _compare(lc, orc, f.img, PARAMS, mode, None, "R23 all bad", bpm=np.ones(shape, np.uint8))
+    _compare(lc, orc, f.img, PARAMS, mode, None, "R23 none bad", bpm=np.zeros(shape, np.uint8))
+
+
+@pytest.mark.parametrize("shape", [(1, 1), (7, 33), (70, 131), (64, 128)])
+def test_masked_median_with_bad_pixels_step(lc, orc, shape):
+    rng = _rng(44)
+    x = rng.standard_normal(shape).astype(np.float32)
+    m = (rng.random(shape) < 0.3).astype(np.uint8)
+    b = ((rng.random(shape) < 0.4) & (m == 0)).astype(np.uint8)
+    if shape[0] > 8 and shape[1] > 8:
+        m[0:4, 0:4] = 1
+        b[0:7, 0:7] |= (m[0:7, 0:7] == 0)                      # zero-donor pixels
+    assert np.array_equal(_n(lc.lacosmic_masked_median(_t(x), _t(m), bpm=_t(b))), orc.masked_median_bpm(x, m, b))
+
+
+def test_masked_median_with_bad_pixels_golden(lc):
+    from test_oracle_variants import _bpm_cases
+    img = (10 * np.arange(7)[:, None] + np.arange(7)[None, :]).astype(np.float32)
+    for case in _bpm_cases():
+        out = _n(lc.lacosmic_masked_median(_t(img), _t(case["mask"]), bpm=_t(case["bpm"])))
+        for y, x, v in case["expect"]:
+            assert out[y, x] == np.float32(v), (case["name"], y, x)
+
+
+# ---------------------------------------------------------------- R24: variance plane
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("shape", [(170, 230), (97, 131), (2, 50), (64, 128)])
+def test_variance_plane(lc, orc, mode, shape):
+    f = _frame(*shape)
+    rng = _rng(9)
+    var = (np.maximum(f.img, 0.0) + 100.0 + 20.0 * rng.random(shape)).astype(np.float32)
+    var[rng.random(shape) < 0.01] = 0.0                           # floored entries
+    var[rng.random(shape) < 0.01] = -5.0
+    for dbg in (0, 1, None):
+        _compare(lc, orc, f.img, PARAMS, mode, dbg, "R24", var=var)
+    _compare(lc, orc, f.img, dict(PARAMS, gain=0.0), mode, 0, "R24 gain 0 is not estimated", var=var)
+    _compare(lc, orc, f.img, PARAMS, mode, 1, "R24 + R22", var=var, fsmode=1)
+
+
+# ---------------------------------------------------------------- R25: extended saturated-star mask
+@pytest.mark.parametrize("grow", [0, 1, 2, 5])
+@pytest.mark.parametrize("shape", [(150, 180), (33, 47), (1, 64), (64, 1), (70, 131)])
+def test_satstar_mask_step(lc, orc, grow, shape):
+    f = synth.make_frame(shape[0], shape[1], seed=62, n_star=4, n_cr=30, sp_frac=0.005, n_sat=8)
+    img = f.img.copy()
+    img[: min(3, shape[0]), : min(4, shape[1])] = 65535.0         # a saturated frame corner (clamped taps)
+    got = _n(lc.lacosmic_satstar_mask(_t(img), 65535.0, grow))
+    assert np.array_equal(got, orc.satstar_mask(img, 65535.0, grow)) and got.sum() > 0
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_satstar_mask_whole_path(lc, orc, mode):
+    f = synth.make_frame(200, 240, seed=66, n_star=10, n_cr=150, sp_frac=0.01, n_sat=16)
+    p = dict(PARAMS, satlevel=60000.0)
+    for grow in (0, 2):
+        o, _ = _compare(lc, orc, f.img, p, mode, 0, "R25", satgrow=grow)
+        assert not (o["mask"] & orc.satstar_mask(f.img, 60000.0, grow)).any()
+    bpm = (_rng(3).random(f.img.shape) < 0.01).astype(np.uint8)
+    _compare(lc, orc, f.img, p, mode, 1, "R25 + R23 + R22", satgrow=1, bpm=bpm, fsmode=1)
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_random_variant_combinations(lc, orc, seed):
+    """Seeded differential test over random shapes, parameters and variant combinations, both modes."""
+    rng = _rng(7000 + seed)
+    h, w = int(rng.integers(1, 100)), int(rng.integers(1, 150))
+    img = 100.0 + rng.standard_normal((h, w)) * 12.0
+    nhit = int(rng.integers(0, max(2, h * w // 10)))
+    img.flat[rng.integers(0, h * w, nhit)] += rng.uniform(30, 6000, nhit)
+    if seed % 3 == 0:
+        img = np.round(img / 4.0) * 4.0
+    if seed % 2 == 0:
+        img[rng.random((h, w)) < 0.03] = 65535.0
+    img = img.astype(np.float32)
+    variant = dict(fsmode=int(rng.integers(0, 2)))
+    if rng.random() < 0.6:
+        variant["bpm"] = (rng.random((h, w)) < 0.05).astype(np.uint8)
+    if rng.random() < 0.5:
+        variant["var"] = (100.0 + 300.0 * rng.random((h, w))).astype(np.float32)
+    if rng.random() < 0.6:
+        variant["satgrow"] = int(rng.integers(0, 4))
+    p = dict(PARAMS, gain=float(rng.choice([0.0, 1.0, 1.8])), sigclip=float(rng.uniform(2.5, 6.0)),
+             objlim=float(rng.choice([0.5, 2.0, 5.0])), niter=int(rng.integers(1, 5)),
+             sigfrac=float(rng.choice([0.3, 0.7])))
+    for mode in MODES:
+        _compare(lc, orc, img, p, mode, int(rng.integers(0, p["niter"])), "random %d" % seed, **variant)
+
+
+# ---------------------------------------------------------------- R26: separable-median comparison
+@pytest.mark.parametrize("k", [3, 5, 7])
+@pytest.mark.parametrize("shape", [(1, 1), (1, 9), (9, 1), (33, 47), (70, 131)])
+def test_sepmedfilt_step(lc, orc, k, shape):
+    x = _rng(30 + k).integers(0, 5, shape).astype(np.float32) if shape[0] % 2 else \
+        _rng(30 + k).standard_normal(shape).astype(np.float32)
+    assert np.array_equal(_n(lc.lacosmic_sepmedfilt(_t(x), k)), orc.sepmedfilt(x, k))
+
+
+@pytest.mark.parametrize("shape", [(130, 160), (97, 131), (3, 50), (64, 128)])
+def test_sepmed_compare_whole_path(lc, orc, shape):
+    import torch
+    f = _frame(*shape, seed=67, n_sat=3)
+    for dbg in (0, 1, None):
+        o = orc.run(f.img, debug_iter=dbg, sepmed=1, **PARAMS)
+        g = lc.lacosmic_run_sepmed_compare(_t(f.img), lc.Params(**PARAMS), debug_iter=dbg)
+        torch.cuda.synchronize()
+        assert np.array_equal(_n(g["mask"]), o["mask"]) and np.array_equal(_n(g["clean"]), o["clean"])
+        assert np.array_equal(_n(g["counts"])[:4], o["counts"])
+        if dbg is not None:
+            for name in ("Lp", "N", "S", "Sp", "m3", "F", "G1", "G2", "M1", "M2", "M3", "C"):
+                assert np.array_equal(_n(g[name]), o[name]), name
+    with pytest.raises(lc.LacosmicError):
+        lc.lacosmic_run_sepmed_compare(_t(f.img), lc.Params(**dict(PARAMS, gain=0.0)))
+
+
+def test_sepmed_flags_star_cores_on_config4(lc, orc):
+    """configs[4] at full size: the paper's argument in numbers -- pixels of (near-)saturated star cores
+    (>= 40000 ADU) flagged by the true median vs by the separable median, saturation gate on and off.  The CUDA comparison
+    path equals the oracle's over the whole frame."""
+    import torch
+    f = synth.make_config(4)
+    bright = f.img >= np.float32(40000.0)
+    img = _t(f.img)
+    for sat in (65535.0, float("inf")):
+        p = dict(PARAMS, satlevel=sat)
+        t = lc.lacosmic_run_ws(img, lc.Params(**p))
+        s = lc.lacosmic_run_sepmed_compare(img, lc.Params(**p))
+        torch.cuda.synchronize()
+        tm, sm = _n(t["mask"]).astype(bool), _n(s["mask"]).astype(bool)
+        print("configs[4], satlevel %s: star-core pixels (>= 40000 ADU, %d in all) flagged: true median %d, separable "
+              "median %d; whole mask %d vs %d" % (sat, bright.sum(), (tm & bright).sum(), (sm & bright).sum(),
+                                                  tm.sum(), sm.sum()))
+        assert (tm & bright).sum() == 0 and (sm & bright).sum() > 0
+        if sat == 65535.0:
+            o = orc.run(f.img, sepmed=1, **p)
+            assert np.array_equal(_n(s["mask"]), o["mask"]) and np.array_equal(_n(s["clean"]), o["clean"])
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_variants_full_size_whole_frame(lc, orc, mode):
+    """configs[4] at full size with every variant switched on, whole frame against the oracle."""
+    f = synth.make_config(4)
+    rng = _rng(12)
+    bpm = (rng.random(f.img.shape) < 0.002).astype(np.uint8)
+    _compare(lc, orc, f.img, PARAMS, mode, None, "configs[4] R22+R23+R25", fsmode=1, bpm=bpm, satgrow=2)
+
+
+def test_variant_argument_errors(lc):
+    import torch
+    img = torch.zeros((16, 16), device="cuda")
+    for kw in (dict(fsmode=2), dict(satgrow=-2), dict(satgrow=17)):
+        with pytest.raises(lc.LacosmicError) as e:
+            lc.lacosmic_run_ex(img, lc.Params(), **kw)
+        assert e.value.code == -3
