@@ -28,19 +28,16 @@ constexpr int WG_J = WG_R + 8;                // register rows: y = ya - 4 + j, 
 constexpr int WG_LCAP = 128;                  // per-warp pixel list capacity of one round
 constexpr unsigned FULL = 0xffffffffu;
 
-__device__ __forceinline__ uint32_t lane_left(uint32_t v, int lane) {
-    const uint32_t t = __shfl_up_sync(FULL, v, 1);
-    return lane > 0 ? t : 0u;
-}
-__device__ __forceinline__ uint32_t lane_right(uint32_t v, int lane) {
-    const uint32_t t = __shfl_down_sync(FULL, v, 1);
-    return lane < 31 ? t : 0u;
-}
-// horizontal dilation of a row held one word per lane; lanes 0 / 31 miss their outer neighbour, which only
-// affects their outer bits, and no result of the own columns depends on those
+// horizontal dilation of a row held one word per lane.  Lanes 0 / 31 have no outer neighbour (the shuffle hands them
+// their own word): that only spoils their outer R bits per stage -- at most 4 bits over the three chained stages of
+// k_grow_replace, 4 in k_dirty_lists -- and the own columns (lanes 1..30) only ever read the INNER 4 bits of a halo word.
 template <int R>
 __device__ __forceinline__ uint32_t hdil_w(uint32_t v, int lane) {
-    return hdil<R>(lane_left(v, lane), v, lane_right(v, lane));
+    const uint32_t vl = __shfl_up_sync(FULL, v, 1), vr = __shfl_down_sync(FULL, v, 1);
+    uint32_t o = v;
+#pragma unroll
+    for (int k = 1; k <= R; ++k) o |= __funnelshift_l(vl, v, k) | __funnelshift_r(v, vr, k);
+    return o;
 }
 
 // Warp-cooperative loop over every set bit of bits[J0..J1) of every lane: the bits are compacted into the
@@ -95,11 +92,12 @@ struct GrowArgs {
     const float* img;             // img_in: donor values (R13)
     float* work;
     int* count;                   // += |M3 & ~C|
-    const uint8_t* stripflag;     // nullable: per strip, set by k_dirty_lists when R is not empty in it
+    int incremental;              // t >= 1 of the lazy path: M1 holds this iteration's new detections only
     int h, w, wpr;
     float siglow;
     int nbx;                      // strips per row of strips = CTAs per row of CTAs (1-D grid, block_xy)
     const uint32_t* donx;         // nullable (R23): bad pixels, never donors of the replacement
+    int backwards;                // strips are taken bottom to top (after a dense top-to-bottom pass: L2 holds the end)
 };
 
 #ifndef LAC_GROW_MINB
@@ -109,25 +107,23 @@ __global__ void __launch_bounds__(32 * WG_WARPS, LAC_GROW_MINB)
 k_grow_replace(GrowArgs a, const int* prev_count) {
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const int h = a.h, w = a.w, wpr = a.wpr;
-    const BlockXY bk = block_xy(a.nbx);
+    BlockXY bk = block_xy(a.nbx);
+    if (a.backwards) bk.y = (int)(gridDim.x / (unsigned)a.nbx) - 1 - bk.y;
     const int wxh = bk.x * WG_OWN - 1;                       // word column of lane 0
     const int wx = wxh + lane;
     const int ya = (bk.y * WG_WARPS + wi) * WG_R;             // first own row
     if (ya >= h) return;                                      // warp-uniform; the kernel has no block barrier
     const bool colok = wx >= 0 && wx < wpr;
     const bool own = lane >= 1 && lane <= WG_OWN && colok;
-    const int wxc = clampi(wx, 0, wpr - 1);
     __shared__ uint32_t s_plane_all[WG_WARPS][(WG_R + 4) * 32];   // G2, then C', rows ya-2 .. ya+WG_R+1
     __shared__ int s_list_all[WG_WARPS][WG_LCAP];
     uint32_t* s_plane = s_plane_all[wi];
     int* s_list = s_list_all[wi];
-    // word (row j, this lane's column) of a plane; 0 outside the frame.  Branch-free: clamped address.
-    auto ld = [&](const uint32_t* __restrict__ pl, int j) -> uint32_t {
-        const int y = ya - 4 + j;
-        const uint32_t v = pl[(size_t)clampi(y, 0, h - 1) * wpr + wxc];
-        return (colok && y >= 0 && y < h) ? v : 0u;
-    };
-    auto qof = [&](int j) -> size_t { return (size_t)(ya - 4 + j) * wpr + wx; };
+    // word (row j, this lane's column) of a plane sits at base + j * wpr; rows / columns outside the frame read as 0
+    // (predicated loads: the address is never formed into an access there)
+    const int base = (ya - 4) * wpr + wx;
+    auto rowok = [&](int j) -> bool { return colok && (unsigned)(ya - 4 + j) < (unsigned)h; };
+    auto qof = [&](int j) -> int { return base + j * wpr; };
     if (prev_count && *prev_count == 0) {
         // fixed point (R17): nothing changes; carry C over to the plane the next reader expects
 #pragma unroll
@@ -136,39 +132,41 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
         return;
     }
     const bool lazy = a.A2 != nullptr;
-    if (a.stripflag) {
-        // incremental iteration: M1, G1, G2 only changed inside the strips k_dirty_lists flagged.  A pixel is
-        // fresh only if one of them changed within 2 px of it, and `need` reads fresh within 2 px of the own
-        // strip, so with no flagged strip among this one and its 8 neighbours nothing is fresh here.
-        bool f = false;
-        if (lane < 9) {
-            const int sy = bk.y * WG_WARPS + wi - 1 + lane / 3, sx = bk.x - 1 + lane % 3;
-            if (sy >= 0 && sy < (h + WG_R - 1) / WG_R && sx >= 0 && sx < a.nbx)
-                f = a.stripflag[(size_t)sy * a.nbx + sx] != 0;
-        }
-        if (!__any_sync(FULL, f)) {
+    // M1 first.  In an incremental iteration (t >= 1) M1 only holds the new detections of this iteration, so most
+    // strips see none within their 16 rows: then M2 = M3 = 0, nothing is fresh and nothing needs a replacement --
+    // the strip carries C over and is done after 24 words instead of the ~100 of all planes (the bit-plane
+    // traffic of all strips at once, not the arithmetic, is what these launches cost).
+    uint32_t m1[WG_J];
+    bool anym1 = false;
 #pragma unroll
-            for (int j = 4; j < 4 + WG_R; ++j)
-                if (own && ya - 4 + j < h) {
-                    a.Cnew[qof(j)] = a.Cold[qof(j)];
-                    a.NEED[qof(j)] = 0u;
-                }
-            return;
-        }
+    for (int j = 0; j < WG_J; ++j) {
+        m1[j] = rowok(j) ? a.M1[qof(j)] : 0u;
+        anym1 |= m1[j] != 0;
     }
-    // every word the strip can need, requested up front (independent loads, one round trip)
+    if (a.incremental && !__any_sync(FULL, anym1)) {
+#pragma unroll
+        for (int j = 4; j < 4 + WG_R; ++j)
+            if (own && ya - 4 + j < h) {
+                a.Cnew[qof(j)] = a.Cold[qof(j)];
+                a.NEED[qof(j)] = 0u;
+            }
+        return;
+    }
+    // every other word the strip can need, requested together (independent loads, one round trip), row by row so
+    // that one offset and one predicate serve all planes of a row
     uint32_t m2[WG_J], g2[WG_J], nbm[WG_J], cold[WG_J];
     {
-        uint32_t m1[WG_J], g1[WG_J];
+        uint32_t g1[WG_J];
 #pragma unroll
-        for (int j = 0; j < WG_J; ++j) m1[j] = ld(a.M1, j);
-#pragma unroll
-        for (int j = 1; j < WG_J - 1; ++j) g1[j] = ld(a.G1, j);
-#pragma unroll
-        for (int j = 2; j < WG_J - 2; ++j) {
-            g2[j] = ld(a.G2, j);
-            cold[j] = ld(a.Cold, j);
-            nbm[j] = lazy ? (ld(a.A2, j) & ~ld(a.A1, j) & ~ld(a.G2F, j)) : 0u;
+        for (int j = 1; j < WG_J - 1; ++j) {
+            const bool ok = rowok(j);
+            const int q = qof(j);
+            g1[j] = ok ? a.G1[q] : 0u;
+            if (j >= 2 && j < WG_J - 2) {
+                g2[j] = ok ? a.G2[q] : 0u;
+                cold[j] = ok ? a.Cold[q] : 0u;
+                nbm[j] = (lazy && ok) ? (a.A2[q] & ~a.A1[q] & ~a.G2F[q]) : 0u;
+            }
         }
         // ---- M2 = dil3(M1) & G1, rows 1 .. WG_J-2
 #pragma unroll
@@ -264,7 +262,7 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
     // sorting network, middle element(s) of the k donors (R13-R16)
     // s_plane: the pixels that are no donors = C' (R13), plus the bad pixels (R23)
 #pragma unroll
-    for (int j = 2; j < WG_J - 2; ++j) s_plane[(j - 2) * 32 + lane] = cn[j] | (a.donx ? ld(a.donx, j) : 0u);
+    for (int j = 2; j < WG_J - 2; ++j) s_plane[(j - 2) * 32 + lane] = cn[j] | ((a.donx && rowok(j)) ? a.donx[qof(j)] : 0u);
     __syncwarp();
     const float INF = __int_as_float(0x7f800000);
     warp_for_each_bit<4, 4 + WG_R>(need, s_list, lane, [&](int j, int sl, int bit) {
@@ -349,11 +347,14 @@ __device__ __forceinline__ void warp_append(const uint32_t (&bits)[WG_J], int p0
 //        structure test reads work within 4 px).  G1, G2, G2F, M1 are cleared inside R and the pixels of A1 in
 //        R outside the quads (their A1 is unchanged) go to the candidate list.
 // Same warp-autonomous layout as k_grow_replace.
-__global__ void __launch_bounds__(32 * WG_WARPS, 3)
+#ifndef LAC_DIRTY_MINB
+#define LAC_DIRTY_MINB 2
+#endif
+__global__ void __launch_bounds__(32 * WG_WARPS, LAC_DIRTY_MINB)
 k_dirty_lists(const uint32_t* __restrict__ NEED, const uint32_t* __restrict__ A1, uint32_t* __restrict__ G1,
               uint32_t* __restrict__ G2, uint32_t* __restrict__ G2F, uint32_t* __restrict__ M1,
               int* __restrict__ qlist, int* __restrict__ nq, int* __restrict__ clist, int* __restrict__ nc,
-              uint8_t* __restrict__ stripflag, int h, int w, int wpr, int nbx, const int* prev_count) {
+              int h, int w, int wpr, int nbx, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const BlockXY bk = block_xy(nbx);
@@ -362,45 +363,38 @@ k_dirty_lists(const uint32_t* __restrict__ NEED, const uint32_t* __restrict__ A1
     if (ya >= h) return;                                      // warp-uniform; no block barrier in this kernel
     const bool colok = wx >= 0 && wx < wpr;
     const bool own = lane >= 1 && lane <= WG_OWN && colok;
-    const int wxc = clampi(wx, 0, wpr - 1);
+    const int base = (ya - 4) * wpr + wx;           // word (row ya - 4 + j, this lane's column) = base + j * wpr
     uint32_t h2[WG_J], h4[WG_J];
     bool any = false;
 #pragma unroll
     for (int j = 0; j < WG_J; ++j) {
-        const int y = ya - 4 + j;
-        const uint32_t v = NEED[(size_t)clampi(y, 0, h - 1) * wpr + wxc];
-        h2[j] = (colok && y >= 0 && y < h) ? v : 0u;
+        h2[j] = (colok && (unsigned)(ya - 4 + j) < (unsigned)h) ? NEED[base + j * wpr] : 0u;
         any |= h2[j] != 0;
     }
-    uint8_t* flag = stripflag + (size_t)(bk.y * WG_WARPS + wi) * nbx + bk.x;
-    if (!__any_sync(FULL, any)) {                             // nothing was rewritten near this strip
-        if (lane == 0) *flag = 0;
-        return;
-    }
-    // the words of the own rows, requested up front (R is not known yet, but a dependent load per row would
-    // serialise eight round trips)
-    uint32_t a1[WG_R], g1[WG_R], g2[WG_R], g2f[WG_R], m1[WG_R];
-#pragma unroll
-    for (int k = 0; k < WG_R; ++k) {
-        const size_t q = (size_t)min(ya + k, h - 1) * wpr + wxc;
-        a1[k] = A1[q]; g1[k] = G1[q]; g2[k] = G2[q]; g2f[k] = G2F[q]; m1[k] = M1[q];
-    }
+    if (!__any_sync(FULL, any)) return;                       // nothing was rewritten near this strip
 #pragma unroll
     for (int j = 0; j < WG_J; ++j) {
-        const uint32_t vl = lane_left(h2[j], lane), vc = h2[j], vr = lane_right(h2[j], lane);
-        h2[j] = hdil<2>(vl, vc, vr);
-        h4[j] = hdil<4>(vl, vc, vr);
+        // (halo lanes 0 / 31 have no outer neighbour: see hdil_w)
+        const uint32_t vl = __shfl_up_sync(FULL, h2[j], 1), vc = h2[j], vr = __shfl_down_sync(FULL, h2[j], 1);
+        uint32_t o2 = vc;
+#pragma unroll
+        for (int k = 1; k <= 2; ++k) o2 |= __funnelshift_l(vl, vc, k) | __funnelshift_r(vc, vr, k);
+        uint32_t o4 = o2;
+#pragma unroll
+        for (int k = 3; k <= 4; ++k) o4 |= __funnelshift_l(vl, vc, k) | __funnelshift_r(vc, vr, k);
+        h2[j] = o2;
+        h4[j] = o4;
     }
-    uint32_t quads[WG_J], cand[WG_J];
-    bool anyR = false;
+    uint32_t quads[WG_J], cand[WG_J], Rr[WG_R], dqr[WG_R];
     const int rem = w - wx * 32;
     const uint32_t valid = rem >= 32 ? 0xffffffffu : rem > 0 ? ((1u << rem) - 1u) : 0u;
 #pragma unroll
     for (int j = 0; j < WG_J; ++j) quads[j] = cand[j] = 0;
 #pragma unroll
-    for (int j = 4; j < 4 + WG_R; ++j) {
-        const int y = ya - 4 + j;
-        if (own && y < h) {
+    for (int k = 0; k < WG_R; ++k) {
+        const int j = k + 4;
+        Rr[k] = dqr[k] = 0;
+        if (own && ya + k < h) {
             uint32_t d5 = 0, r9 = 0;
 #pragma unroll
             for (int d = -2; d <= 2; ++d) d5 |= h2[j + d];
@@ -410,23 +404,33 @@ k_dirty_lists(const uint32_t* __restrict__ NEED, const uint32_t* __restrict__ A1
             uint32_t t = d5 | (d5 >> 1);
             t |= t >> 2;
             t &= 0x11111111u;                       // bit 4k: quad k of this word holds a pixel of D5
-            const uint32_t dq = t * 0xFu;           // all four pixels of those quads
-            const uint32_t R = (r9 | dq) & valid;
+            dqr[k] = t * 0xFu;                      // all four pixels of those quads
+            Rr[k] = (r9 | dqr[k]) & valid;
             quads[j] = t;
-            if (R) {
-                const size_t q = (size_t)y * wpr + wx;
-                const int k = j - 4;
-                anyR = true;
-                cand[j] = a1[k] & R & ~dq;
-                if (g1[k] & R) G1[q] = g1[k] & ~R;
-                if (g2[k] & R) G2[q] = g2[k] & ~R;
-                if (g2f[k] & R) G2F[q] = g2f[k] & ~R;
-                if (m1[k] & R) M1[q] = m1[k] & ~R;
-            }
         }
     }
-    anyR = __any_sync(FULL, anyR);
-    if (lane == 0) *flag = anyR ? 1 : 0;
+    // the gate planes are only read (and rewritten) in the words that hold a pixel of R: late iterations touch a
+    // few words per strip, and the bit-plane traffic of all strips at once is what this launch costs
+    uint32_t a1[WG_R], g1[WG_R], g2[WG_R], g2f[WG_R], m1[WG_R];
+#pragma unroll
+    for (int k = 0; k < WG_R; ++k) {
+        const bool rd = Rr[k] != 0;
+        const int q = base + (4 + k) * wpr;
+        a1[k] = rd ? A1[q] : 0u; g1[k] = rd ? G1[q] : 0u; g2[k] = rd ? G2[q] : 0u;
+        g2f[k] = rd ? G2F[q] : 0u; m1[k] = rd ? M1[q] : 0u;
+    }
+#pragma unroll
+    for (int k = 0; k < WG_R; ++k) {
+        const uint32_t R = Rr[k];
+        if (R) {
+            const int q = base + (4 + k) * wpr;
+            cand[k + 4] = a1[k] & R & ~dqr[k];
+            if (g1[k] & R) G1[q] = g1[k] & ~R;
+            if (g2[k] & R) G2[q] = g2[k] & ~R;
+            if (g2f[k] & R) G2F[q] = g2f[k] & ~R;
+            if (m1[k] & R) M1[q] = m1[k] & ~R;
+        }
+    }
     const int p0 = ya * w + wx * 32;
     warp_append<4, 4 + WG_R>(quads, p0, w, qlist, nq, lane);
     warp_append<4, 4 + WG_R>(cand, p0, w, clist, nc, lane);

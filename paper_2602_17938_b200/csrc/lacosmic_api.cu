@@ -162,7 +162,6 @@ struct Workspace {
     float* gains;      // per iteration: the gain the noise model used (R21: estimated when p.gain == 0)
     lac::SelState* sel; // radix selection state and histogram of the gain estimation (select.cuh)
     uint32_t* hist;
-    uint8_t* stripflag; // per 30-word x 8-row strip of the bit-planes (grow.cuh): R not empty in it
     size_t bytes;      // total
     size_t zero_off, zero_bytes;   // region cleared at the start of a frame: the counters
 };
@@ -180,8 +179,6 @@ Workspace carve(void* base, int h, int w) {
     uint32_t** planes[] = {&ws.G1, &ws.G2, &ws.G2F, &ws.M1, &ws.M2, &ws.M3, &ws.C[0], &ws.C[1], &ws.A1, &ws.A2, &ws.NEED,
                            &ws.NOK, &ws.DONX};
     for (uint32_t** pl : planes) { *pl = (uint32_t*)(p + off); off += bp; }
-    ws.stripflag = (uint8_t*)(p + off);
-    off += align_up((size_t)((words_per_row(w) + lac::WG_OWN - 1) / lac::WG_OWN) * ((h + lac::WG_R - 1) / lac::WG_R + lac::WG_WARPS), 256);
     ws.zero_off = off;
     ws.counts = (int32_t*)(p + off); off += align_up(NCOUNTERS * 4, 256);
     ws.ncand = ws.counts + LACOSMIC_MAX_NITER;
@@ -391,6 +388,11 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         // rewrote (ws.NEED); a debug dump recomputes the planes everywhere, and so does an estimated gain
         // (it changes with every iteration, and S with it)
         const bool incr = lazy && t > 0 && !d && !estimate;
+#ifndef LAC_BACKWARDS
+#define LAC_BACKWARDS 1
+#endif
+        // after a dense pass over the frame the sparse kernels walk it from the end (what the L2 still holds)
+        const int backwards = (LAC_BACKWARDS && !incr) ? 1 : 0;
         // R22 in the dense path: the gate kernel reads the noise plane, which the noise/S pass stores in the
         // candidate list's storage (not used by the dense path; free again once a gain estimate has been selected)
         float* const nplane = (d && dbg->N) ? dbg->N : ((fs1 && !lazy) ? (float*)ws.clist : nullptr);
@@ -404,7 +406,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
             {
                 Span sp(KC_LISTS, st);
                 lac::k_dirty_lists<<<grow_grid(h, w), 32 * lac::WG_WARPS, 0, st>>>(ws.NEED, ws.A1, ws.G1, ws.G2, ws.G2F, ws.M1, ws.qlist,
-                                                                   ws.nquad + t, ws.clist, ws.ncand + t, ws.stripflag, h, w, wpr, grow_nbx(w), prev);
+                                                                   ws.nquad + t, ws.clist, ws.ncand + t, h, w, wpr, grow_nbx(w), prev);
                 LAUNCHED();
             }
             {
@@ -436,8 +438,8 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
             lac::CandArgs ca{ws.S, work, ws.G1, ws.G2, ws.M1, h, w, wpr, p.sigclip, siglow, p.objlim,
                              p.gain, rn2, estimate ? ws.gains + t : nullptr, var};
             Span sp(KC_EVAL, st);
-            if (fs1) lac::k_eval_candidates<1><<<gridE, 128, 0, st>>>(ca, ws.clist, ws.ncand + t, prev);
-            else lac::k_eval_candidates<0><<<gridE, 128, 0, st>>>(ca, ws.clist, ws.ncand + t, prev);
+            if (fs1) lac::k_eval_candidates<1><<<gridE, 128, 0, st>>>(ca, ws.clist, ws.ncand + t, prev, backwards);
+            else lac::k_eval_candidates<0><<<gridE, 128, 0, st>>>(ca, ws.clist, ws.ncand + t, prev, backwards);
             LAUNCHED();
         } else {
             lac::FineArgs fa{ws.G1, ws.G2, ws.M1, d ? dbg->Sp : nullptr, d ? dbg->m3 : nullptr,
@@ -451,8 +453,8 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         // steps (6)-(7), fused; in the lazy path G2 is completed on the pixels the second growth reaches
         lac::GrowArgs ga{ws.M1, ws.G1, ws.G2, ws.G2F, lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
                          ws.C[t & 1], ws.C[(t + 1) & 1], ws.NEED, d ? ws.M2 : nullptr, d ? ws.M3 : nullptr,
-                         ws.S, img, work, ws.counts + t, incr ? ws.stripflag : nullptr, h, w, wpr, siglow, grow_nbx(w),
-                         donx};
+                         ws.S, img, work, ws.counts + t, incr ? 1 : 0, h, w, wpr, siglow, grow_nbx(w),
+                         donx, backwards};
         if ((rc = grow_replace(ga, prev, st))) return rc;
         if (d) {
             // lazy path: G2 is only evaluated where step (6) needs it, so it is not dumped
@@ -532,8 +534,8 @@ int run_sepmed_frame(const float* img, int h, int w, const lacosmic_params& p, u
         LAUNCHED();
         // O6, O7: the product kernel (G2 complete, as in the dense path)
         lac::GrowArgs gr{ws.M1, ws.G1, ws.G2, ws.G2F, nullptr, nullptr, ws.C[t & 1], ws.C[(t + 1) & 1], ws.NEED,
-                         d ? ws.M2 : nullptr, d ? ws.M3 : nullptr, A, img, work, ws.counts + t, nullptr, h, w, wpr, siglow,
-                         grow_nbx(w), nullptr};
+                         d ? ws.M2 : nullptr, d ? ws.M3 : nullptr, A, img, work, ws.counts + t, 0, h, w, wpr, siglow,
+                         grow_nbx(w), nullptr, 0};
         if ((rc = grow_replace(gr, prev, st))) return rc;
         if (d) {
             struct { const uint32_t* b; uint8_t* o; } planes[] = {{ws.G1, dbg->G1}, {ws.G2, dbg->G2}, {ws.M1, dbg->M1},
@@ -1076,7 +1078,7 @@ int lacosmic_masked_median_bpm(const float* img, const uint8_t* mask_u8, const u
     CK(cudaMemsetAsync(ws.C[0], 0, (size_t)h * wpr * 4, st));
     CK(cudaMemsetAsync(ws.counts, 0, 4, st));
     lac::GrowArgs ga{ws.M1, ws.M1, ws.M1, nullptr, nullptr, nullptr, ws.C[0], ws.C[1], ws.NEED, nullptr, nullptr,
-                     nullptr, img, out, ws.counts, nullptr, h, w, wpr, 0.0f, grow_nbx(w), bpm_u8 ? ws.DONX : nullptr};
+                     nullptr, img, out, ws.counts, 0, h, w, wpr, 0.0f, grow_nbx(w), bpm_u8 ? ws.DONX : nullptr, 0};
     return grow_replace(ga, nullptr, st);
 }
 

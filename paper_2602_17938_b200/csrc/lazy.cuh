@@ -187,12 +187,14 @@ __device__ __forceinline__ bool fine_bracket(float lp, float m3c, float objlim, 
 template <int FS>
 __global__ void __launch_bounds__(128, LAC_EVAL_MINB)
 k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restrict__ nlist,
-                  const int* prev_count) {
+                  const int* prev_count, int backwards) {
     if (prev_count && *prev_count == 0) return;
     const int n = *nlist;
     const int h = a.h, w = a.w;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        const int p = list[i];
+        // backwards: the list is in frame order and the dense pass before it ran top to bottom, so the END of the
+        // planes is what the L2 still holds -- start there
+        const int p = list[backwards ? n - 1 - i : i];
         const int y = p / w, x = p - y * w;
         int c1, c2;
         count_sp(a.S, y, x, h, w, a.sigclip, a.siglow, c1, c2);
