@@ -383,10 +383,15 @@ def run_cuda(args):
 
     def step_host_sparse():
         lc.lacosmic_run_host_sparse(img_h, P[main_mode], out=sp_out, dev_workspace=hws)
-    ms_sp = timed(step_host_sparse, max(3, args.steps // 2), 1)
+    ms_sp = timed(step_host_sparse, args.steps, max(1, args.warmup // 2))
     nsp = int(sp_out["count"][0])
     sp_idx = sp_out["idx"].numpy()[:nsp]
-    sp_ok = bool(nsp == int(res["mask"].sum().item()) and nsp <= sp_out["capacity"] and
+    ref_mask = res["mask"].cpu().numpy()
+    sp_bits = np.unpackbits(sp_out["maskbits"].numpy().view(np.uint8), axis=1, bitorder="little")[:, :w]
+    # the sparse results reproduce the device-resident path: same mask, ascending indices of exactly its pixels, and the
+    # listed values are the cleaned frame's
+    sp_ok = bool(nsp == int(ref_mask.sum()) and nsp <= sp_out["capacity"] and np.array_equal(sp_bits, ref_mask) and
+                 np.array_equal(sp_idx, np.flatnonzero(ref_mask)) and
                  (sp_out["val"].numpy()[:nsp] == res["clean"].cpu().numpy().ravel()[sp_idx]).all())
     e2e_sparse = dict(value=world * 1e3 / ms_sp, unit="frames/s", ms_per_step=ms_sp, h2d_bytes_per_step=npx * 4,
                       d2h_bytes_per_step=int(sp_out["maskbits"].numel() * 4 + 8 * sp_out["capacity"] + 4),
@@ -442,6 +447,12 @@ def run_cuda(args):
         e2e_stream["sparse_results"] = dict(call="lacosmic_run_host_stream_sparse (%d frames, %d staging slots)" % (nh, kslots),
                                             **prod)
         del imgs_h, hbws, src
+    # ---- work counters of one frame (untimed run with the library's statistics switched on): the data-dependent
+    # terms of the whole-step roofline
+    lc.lacosmic_stats_enable(True)
+    make_step(main_mode)()
+    frame_stats = lc.lacosmic_frame_stats(ws, h, w)
+    lc.lacosmic_stats_enable(False)
     # ---- the "alu" roofline's peak, measured in this run: fp32 min/max issue rate of this GPU (probe.cuh)
     probe = dict(fmnmx=lc.lacosmic_probe_minmax_rate(0) / 1e12, fmnmx3=lc.lacosmic_probe_minmax_rate(1) / 1e12)
     clocks = sampler.stop() if rank == 0 else None
@@ -484,14 +495,69 @@ def run_cuda(args):
                     frac_of_measured_peak=achieved / probe["fmnmx"],
                     minmax_instr_per_px=ops_px, avg_launch_ms=dom_avg_ms, launches_timed=dom_spans)
 
+    def step_roofline(ms_step):
+        """sum over the kernels of a step of max(bytes_k / BW, minmax_k / ALU_peak), over the measured
+        step time.  bytes_k = ALGORITHMIC bytes (what the kernel's inputs and outputs amount to; gathers counted per
+        tap, not per sector), minmax_k = the kernel's own min/max instruction count (DESIGN.md section 5 table)."""
+        if main_mode != "lazy":
+            return None
+        bw = peaks["hbm_gbs"] * 1e9
+        alu = probe["fmnmx"] * 1e12
+        bp = npx / 8.0                               # one bit-plane
+        plane = npx * 4.0                            # one fp32 plane
+        st = frame_stats
+        terms = []
+
+        def add(name, t, nbytes, minmax):
+            terms.append(dict(kernel=name, iteration=t, bytes=int(nbytes), minmax=int(minmax),
+                              t_hbm_us=nbytes / bw * 1e6, t_alu_us=minmax / alu * 1e6))
+        for t in range(niter):
+            if t > 0 and st["new"][t - 1] == 0:
+                break
+            ncand, nq, nrep, nfine = st["candidates"][t], st["quads"][t], st["replaced"][t], st["fine_tests"][t]
+            if t == 0:
+                # read img 4, write S 4 + work 4, A1/A2; med5 network 326 + 16 clip min/max per 4 pixels
+                add("noise_S", t, npx * 12 + 2 * bp, npx * KERNEL_MINMAX_PER_PX["noise_S"])
+                add("list_candidates", t, bp + 5 * bp + 4 * ncand, 0)       # A1 read, G1/G2/G2F/M1/C cleared, list
+            else:
+                add("dirty_lists", t, bp + 4 * nq + 4 * ncand, 0)           # NEED read, lists written
+                # per quad: its 8 x 5 window of work read (never more than the plane: windows overlap), 4 S written,
+                # A1/A2 nibbles; the x4 network
+                add("noise_S_quads", t, min(nq * 160, plane) + nq * 18, nq * 4 * KERNEL_MINMAX_PER_PX["noise_S"])
+            # per candidate: list entry, 25 taps of S, gate bits; per fine test: 81 taps of work, med3x3 (30 min/max);
+            # taps of neighbouring candidates overlap, so neither sum can exceed its plane
+            add("eval_candidates", t, ncand * 5 + min(ncand * 100, plane) + min(nfine * 324, plane), nfine * 30)
+            # bit-planes M1 G1 G2 C A1 A2 G2F read, C' NEED written (t = 0; later iterations M1 + C carried over); per
+            # replaced pixel 25 taps + 1 store and the 25-input sorting network (276 min/max)
+            planes = 9 * bp if t == 0 else 4 * bp
+            add("grow_replace", t, planes + min(nrep * 100, plane) + nrep * 4, nrep * 276)
+        add("unpack_bits", niter, bp + npx, 0)
+        total_us = sum(max(x["t_hbm_us"], x["t_alu_us"]) for x in terms)
+        return dict(step_frac=total_us / (ms_step * 1e3), bound_us=total_us, step_us=ms_step * 1e3,
+                    bw_gbs=peaks["hbm_gbs"], alu_peak_T=probe["fmnmx"],
+                    definition="sum_k max(bytes_k / BW, minmax_k / ALU_peak) / T_step (SURVEY.md 8(d)); BW = measured "
+                               "copy rate, ALU_peak = the min/max issue rate measured in this run",
+                    frame_stats={k: v[:niter] for k, v in st.items()}, terms=terms)
+
     frames_per_s = world * 1e3 / res["ms"]
     e2e_fps = world * 1e3 / ms_e2e
     bytes_iter = HBM_BYTES_PER_PX_ITER[main_mode]
     hbm_bytes_step = npx * (bytes_iter * niter + HBM_BYTES_PER_PX_FRAME)
+    def hbm_frac(bytes_px_iter):
+        b = npx * (bytes_px_iter * niter + HBM_BYTES_PER_PX_FRAME)
+        return dict(bytes_per_px_iter=bytes_px_iter, bytes_per_step=int(b),
+                    achieved_gbs=b / (res["ms"] * 1e-3) / 1e9, frac=b / (res["ms"] * 1e-3) / 1e9 / peaks["hbm_gbs"])
+    # the HBM-only fraction of the step against each byte figure of SURVEY.md 8(a) -- `frac` below uses this path's own
     hbm = dict(algorithmic_bytes_per_step=hbm_bytes_step,
                achieved_gbs=hbm_bytes_step / (res["ms"] * 1e-3) / 1e9,
                peak_gbs=peaks["hbm_gbs"], peak_source=peaks["source"],
-               frac=hbm_bytes_step / (res["ms"] * 1e-3) / 1e9 / peaks["hbm_gbs"])
+               frac=hbm_bytes_step / (res["ms"] * 1e-3) / 1e9 / peaks["hbm_gbs"],
+               frac_uses="own fusion: %.2f B/px/iteration (%s mode, DESIGN.md section 5) + %.3f B/px per frame"
+                         % (bytes_iter, main_mode, HBM_BYTES_PER_PX_FRAME),
+               against_survey_8a=dict(floor_4p5=hbm_frac(4.5), pragmatic_fusion_31p5=hbm_frac(31.5),
+                                      fully_materialised_77=hbm_frac(77.0)),
+               note="the lazy path never moves the 31.5 / 77 B per pixel of SURVEY 8(a): those fractions only say how "
+                    "the step time compares with what a dense implementation would have to move")
     ref_cmp_rate = npx * REF_COMPARISONS_PER_PX_ITER * niter / (res["ms"] * 1e-3) / 1e12
 
     # ---- the oracle on the host cores, whole frames (SURVEY.md 8(d))
@@ -509,12 +575,16 @@ def run_cuda(args):
                     l2="flushed between steps (256 MiB write outside the event pair)",
                     parallelism="replicas (one frame per GPU, no collective)"),
         mpix_per_s=frames_per_s * npx / 1e6,
-        e2e=dict(value=e2e_fps, unit="frames/s", h2d_bytes_per_step=npx * 4,
-                 d2h_bytes_per_step=npx * 5, ms_per_step=ms_e2e, matches_device_path=same,
-                 call="lacosmic_run_host (pinned host buffers)"),
+        # e2e leads with the sparse-result call: the cleaned frame equals the input outside the mask,
+        # so the host call that returns the mask bit-plane + the replaced pixels moves 114 MB instead of 234 MB over PCIe;
+        # the dense-result call (mask and cleaned planes copied back in full) is reported beside it
+        e2e=dict(e2e_sparse, note="results = mask bit-plane + ascending list of replaced pixels with their values"),
+        e2e_dense=dict(value=e2e_fps, unit="frames/s", h2d_bytes_per_step=npx * 4,
+                       d2h_bytes_per_step=npx * 5, ms_per_step=ms_e2e, matches_device_path=same,
+                       call="lacosmic_run_host (pinned host buffers; mask uint8 + cleaned fp32 planes copied back)"),
         gpu_launches=res["launches"] * args.steps,
         launches_per_step=res["launches"],
-        roofline=roofline(res), hbm=hbm,
+        roofline=dict(roofline(res), step=step_roofline(res["ms"])), hbm=hbm,
         kernels_ms_per_step=main_sum["kernels_ms_per_step"],
         kernel_share_of_step=main_sum["kernel_share_of_step"],
         ms_per_step_with_kernel_event_spans=res["ms_spans"],
@@ -522,7 +592,7 @@ def run_cuda(args):
         ref_comparisons_T_per_s=ref_cmp_rate,
         other_mode=dict(mode=other_mode, same_mask_clean_counts=modes_agree, roofline=roofline(res_other),
                         **summarise(res_other)),
-        stream=stream_res, e2e_stream=e2e_stream, e2e_u16=e2e_u16, e2e_sparse=e2e_sparse, gain_estimation=gain_est,
+        stream=stream_res, e2e_stream=e2e_stream, e2e_u16=e2e_u16, gain_estimation=gain_est,
         new_cr_per_iteration=res["counts"], mask_fraction=mask_frac,
         clocks=clocks, cpu_baseline=cpu,
         context="paper (PAPER.md:31,47): 55 s/frame dfcosmic C++ at 2 threads on AWS; GPU variant on an "
@@ -650,7 +720,7 @@ def respawn_under_torchrun(args):
 KERNEL_MINMAX_PER_PX = {
     # generated networks (median_networks.cuh): med7 764/4, med5 326/4, med3 76/4 x 1.46 (haloed m3 tile)
     "fine_gates": 764 / 4 + 326 / 4 + 1.46 * 76 / 4,
-    "noise_S": 326 / 4 + 13 / 4,                     # med5 + the clamp/floor selects of L+ and N
+    "noise_S": 326 / 4 + 16 / 4,                     # med5 network + the four clips of L+ (FMNMX) per pixel
 }
 # HBM bytes per pixel per iteration the path must move with the current fusion:
 # noise_S: read work 4 + write S 4; dense fine_gates: read work 4 + S 4 + 0.375 bit-planes; lazy: A1/A2

@@ -290,6 +290,18 @@ const char *lacosmic_version(void);
  * LACOSMIC_NUM_KERNEL_CLASSES, the summed device time ms_sum[c] and the number of spans[c] (HOST
  * arrays), and clears the record.  Class names: lacosmic_kernel_class_name(c); the last class is the
  * whole frame (copies included). */
+/* Work counters of the last frame that ran in `workspace` (the lazy path's data-dependent work; bench.py turns them into
+ * the per-kernel terms of the whole-step roofline).  stats_host: HOST array
+ * [LACOSMIC_NUM_FRAME_STATS][LACOSMIC_MAX_NITER] of int32, row r, iteration t:
+ *   0 newly flagged pixels; 1 candidates evaluated (pixels with S > sigclip listed for the tests); 2 quads (aligned groups
+ *   of 4 pixels) whose S the incremental pass recomputed; and, only for frames run after lacosmic_stats_enable(1) on the
+ *   calling thread (two extra atomics per warp, so off by default): 3 pixels whose replacement value was computed;
+ *   4 candidates that passed S' > sigclip and took the fine-structure test.
+ * Copies 5 * 64 * 4 bytes device-to-host and SYNCHRONISES `stream`. */
+#define LACOSMIC_NUM_FRAME_STATS 5
+int lacosmic_stats_enable(int enable);
+int lacosmic_frame_stats(const void *workspace, int h, int w, int32_t *stats_host, void *stream);
+
 /* Measured peak of the "alu" roofline (the medians of PAPER.md:23,64 are fp32 min/max selection
  * networks, bound by the rate at which the SMs issue FMNMX).  Runs a register-only kernel of independent min/max chains
  * (kind 0: two-input FMNMX; kind 1: three-input FMNMX3) on every SM of the current device and writes the achieved

@@ -25,7 +25,7 @@ EXPORTS = (
     "lacosmic_dilate3", "lacosmic_masked_median", "lacosmic_strerror",
     "lacosmic_last_cuda_error", "lacosmic_last_launch_count", "lacosmic_version",
     "lacosmic_kernel_timing_enable", "lacosmic_kernel_timing_read", "lacosmic_kernel_class_name",
-    "lacosmic_probe_minmax_rate",
+    "lacosmic_probe_minmax_rate", "lacosmic_stats_enable", "lacosmic_frame_stats",
     "lacosmic_run_ex", "lacosmic_sepmed_workspace_bytes", "lacosmic_run_sepmed_compare", "lacosmic_sepmedfilt",
     "lacosmic_masked_median_bpm", "lacosmic_satstar_mask",
 )
@@ -124,6 +124,8 @@ def load_library():
         "lacosmic_kernel_timing_read": (i, [vp, vp]),
         "lacosmic_kernel_class_name": (C.c_char_p, [i]),
         "lacosmic_probe_minmax_rate": (i, [i, vp, vp]),
+        "lacosmic_stats_enable": (i, [i]),
+        "lacosmic_frame_stats": (i, [vp, i, i, vp, vp]),
         "lacosmic_run_ex": (i, [vp, i, i, C.POINTER(_CParams), C.POINTER(_CVariant), vp, vp, vp, sz, vp,
                                 C.POINTER(_CDebug), vp]),
         "lacosmic_sepmed_workspace_bytes": (sz, [i, i]),
@@ -624,6 +626,20 @@ def lacosmic_probe_minmax_rate(kind=0, stream=None):
     _check(load_library().lacosmic_probe_minmax_rate(int(kind), C.byref(out), _stream(stream)),
            "lacosmic_probe_minmax_rate")
     return float(out.value)
+
+
+def lacosmic_stats_enable(enable=True):
+    _check(load_library().lacosmic_stats_enable(1 if enable else 0), "lacosmic_stats_enable")
+
+
+def lacosmic_frame_stats(workspace, h, w, stream=None):
+    """{name: [per-iteration int]} of the last frame that ran in `workspace` (synchronises the stream)."""
+    torch = _torch()
+    buf = (C.c_int32 * (5 * MAX_NITER))()
+    _check(load_library().lacosmic_frame_stats(_dev(workspace, torch.uint8, "workspace"), int(h), int(w), buf,
+                                               _stream(stream)), "lacosmic_frame_stats")
+    names = ("new", "candidates", "quads", "replaced", "fine_tests")
+    return {n: [int(buf[r * MAX_NITER + t]) for t in range(MAX_NITER)] for r, n in enumerate(names)}
 
 
 def lacosmic_kernel_timing_read():

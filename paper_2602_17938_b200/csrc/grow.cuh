@@ -97,7 +97,7 @@ struct GrowArgs {
     float siglow;
     int nbx;                      // strips per row of strips = CTAs per row of CTAs (1-D grid, block_xy)
     const uint32_t* donx;         // nullable (R23): bad pixels, never donors of the replacement
-    int backwards;                // strips are taken bottom to top (after a dense top-to-bottom pass: L2 holds the end)
+    int* nneed;                   // nullable (lacosmic_stats_enable): += pixels whose replacement value is (re)computed
 };
 
 #ifndef LAC_GROW_MINB
@@ -107,8 +107,7 @@ __global__ void __launch_bounds__(32 * WG_WARPS, LAC_GROW_MINB)
 k_grow_replace(GrowArgs a, const int* prev_count) {
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const int h = a.h, w = a.w, wpr = a.wpr;
-    BlockXY bk = block_xy(a.nbx);
-    if (a.backwards) bk.y = (int)(gridDim.x / (unsigned)a.nbx) - 1 - bk.y;
+    const BlockXY bk = block_xy(a.nbx);
     const int wxh = bk.x * WG_OWN - 1;                       // word column of lane 0
     const int wx = wxh + lane;
     const int ya = (bk.y * WG_WARPS + wi) * WG_R;             // first own row
@@ -258,6 +257,13 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
 #pragma unroll
     for (int j = 4; j < 4 + WG_R; ++j) anyneed |= need[j] != 0;
     if (!__any_sync(FULL, anyneed)) return;
+    if (a.nneed) {                                            // statistics only (off in timed runs)
+        int nn = 0;
+#pragma unroll
+        for (int j = 4; j < 4 + WG_R; ++j) nn += __popc(need[j]);
+        nn = __reduce_add_sync(FULL, nn);
+        if (lane == 0) atomicAdd(a.nneed, nn);
+    }
     // ---- step (7) at those pixels: 25 clamped taps of img_in, +inf where the tap's pixel is in C', 25-input
     // sorting network, middle element(s) of the k donors (R13-R16)
     // s_plane: the pixels that are no donors = C' (R13), plus the bad pixels (R23)

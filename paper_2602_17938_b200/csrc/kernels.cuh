@@ -159,11 +159,19 @@ constexpr int UW = 32, UH = 4;
 
 // sm: work tile with margins (NS_MX, NS_MY), edge-replicated
 // W4: w % 4 == 0 and 16-byte aligned planes (the TMA path): quads are whole and every store is one vector
-template <bool W4>
+// CFG >= 0: the nullable outputs are known at compile time (bit 0: copy_out, bit 1: A1 / A2; no debug plane, no residual
+// plane, no device-side gain), which takes their tests out of the unit loop; CFG < 0: decided at run time.
+// The threshold tests and their packing run on the FMA pipe: for finite a, b the sign of fsub(a, b) is set iff a < b
+// (a difference of two floats never rounds to zero unless they are equal: gradual underflow), so
+// (s > thr) = sign(thr - s), (c < satlevel) = sign(c - satlevel), and the nibble is a sum of sign bits times 2^j.
+template <bool W4, int CFG>
 __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a, int x0, int y0, int lane,
                                              int wi) {
     const int lx = lane & 7, lr = lane >> 3;
-    const float gain = a.gain_dev ? __ldg(a.gain_dev) : a.gain;
+    const bool has_copy = CFG < 0 ? a.copy_out != nullptr : (CFG & 1) != 0;
+    const bool has_A = CFG < 0 ? a.A1 != nullptr : (CFG & 2) != 0;
+    const bool has_lp = CFG < 0 && a.dbgLp != nullptr, has_n = CFG < 0 && a.dbgN != nullptr, has_R = CFG < 0 && a.R != nullptr;
+    const float gain = (CFG < 0 && a.gain_dev) ? __ldg(a.gain_dev) : a.gain;
 #pragma unroll 1
     for (int u = wi; u < (TW / UW) * (NS_TH / UH); u += NWARP) {
         const int xu = x0 + (u & 3) * UW, lyu = (u >> 2) * UH, yu = y0 + lyu;
@@ -174,23 +182,26 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
             float win[8][5], m5[4], s[4], lp[4], n[4], ctr[4];
             load_window<5, NS_PITCH>(sm + ly * NS_PITCH + (x - x0), win);
             median5x5_x4(win, m5);
+            uint32_t nok = 0;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 ctr[j] = win[2 + j][2];
                 lp[j] = lplus_px(win[2 + j][2], win[2 + j][1], win[2 + j][3], win[1 + j][2], win[3 + j][2]);
                 n[j] = noise_px(m5[j], gain, a.rn2);
                 s[j] = fdiv_nn(lp[j], __fmul_rn(2.0f, n[j]));
-                const bool ok = (W4 || x + j < a.w) && (win[2 + j][2] < a.satlevel);            // R12
-                n1 |= (uint32_t)(ok && s[j] > a.sigclip) << j;
-                n2 |= (uint32_t)(ok && s[j] > a.siglow) << j;
+                n1 += sign01(__fsub_rn(a.sigclip, s[j])) << j;                            // S > sigclip
+                n2 += sign01(__fsub_rn(a.siglow, s[j])) << j;                             // S > siglow
+                nok += ((W4 || x + j < a.w) ? sign01(__fsub_rn(ctr[j], a.satlevel)) : 0u) << j;   // R12: c < satlevel
             }
+            n1 &= nok;
+            n2 &= nok;
             size_t ro = (size_t)y * a.w;
-            if (a.R) store4q<W4>(a.S, ro, x, a.w, m5);
+            if (has_R) store4q<W4>(a.S, ro, x, a.w, m5);
             else store4q<W4>(a.S, ro, x, a.w, s);
-            if (a.dbgLp) store4q<W4>(a.dbgLp, ro, x, a.w, lp);
-            if (a.dbgN) store4q<W4>(a.dbgN, ro, x, a.w, n);
-            if (a.copy_out) store4q<W4>(a.copy_out, ro, x, a.w, ctr);
-            if (a.R) {   // R21: residual in units of sqrt(signal)
+            if (has_lp) store4q<W4>(a.dbgLp, ro, x, a.w, lp);
+            if (has_n) store4q<W4>(a.dbgN, ro, x, a.w, n);
+            if (has_copy) store4q<W4>(a.copy_out, ro, x, a.w, ctr);
+            if (has_R) {   // R21: residual in units of sqrt(signal)
                 float r[4];
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
@@ -200,7 +211,7 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
                 store4q<W4>(a.R, ro, x, a.w, r);
             }
         }
-        if (a.A1) {
+        if (has_A) {
             const uint32_t b1 = nibbles_to_word(n1, lane), b2 = nibbles_to_word(n2, lane);
             if (lx == 0 && y < a.h) {
                 size_t q = (size_t)y * a.wpr + (xu >> 5);
@@ -224,7 +235,7 @@ k_noise_S(const float* __restrict__ work, NoiseArgs a, int ntx, const int* prev_
     const int x0 = tx * TW, y0 = ty * NS_TH;
     load_tile<NS_MX, NS_MY, NS_PITCH, NS_TH>(sm, work, a.h, a.w, y0, x0, tid);
     __syncthreads();
-    noise_S_tile<false>(sm, a, x0, y0, tid & 31, tid >> 5);
+    noise_S_tile<false, -1>(sm, a, x0, y0, tid & 31, tid >> 5);
 }
 
 // K_B: steps (3b)-(5).  S' = S - med5(S); m3 = med3(work) (tile in shared memory, replicated at the
@@ -404,6 +415,7 @@ __device__ __forceinline__ void replicate_fix(float* sm, int oy, int ox, int h, 
 #ifndef LAC_NS_MINB
 #define LAC_NS_MINB 4
 #endif
+template <int CFG>
 __global__ void __launch_bounds__(NT, LAC_NS_MINB)
 k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx, int ntiles,
               const int* prev_count) {
@@ -441,7 +453,7 @@ k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx,
             fence_proxy_async();
             __syncthreads();
         }
-        noise_S_tile<true>(buf(st), a, x0, y0, tid & 31, tid >> 5);
+        noise_S_tile<true, CFG>(buf(st), a, x0, y0, tid & 31, tid >> 5);
         __syncthreads();   // stage st is free for the load issued at the top of the next iteration
     }
 }

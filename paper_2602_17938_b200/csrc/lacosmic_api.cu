@@ -19,6 +19,7 @@ namespace {
 
 thread_local int g_last_cuda_error = 0;
 thread_local int g_launches = 0;
+thread_local bool g_stats = false;   // lacosmic_stats_enable: per-iteration work counters for bench.py's roofline terms
 
 inline bool cuda_ok(cudaError_t e) {
     if (e != cudaSuccess) {
@@ -112,11 +113,13 @@ DeviceInfo device_info() {
     if (cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return d;
     if (cudaFuncSetAttribute(lac::k_fine_gates_tma, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              lac::FG_SMEM_BYTES) != cudaSuccess) return d;
-    if (cudaFuncSetAttribute(lac::k_noise_S_tma, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             lac::NS_SMEM_BYTES) != cudaSuccess) return d;
+    if (cudaFuncSetAttribute(lac::k_noise_S_tma<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(lac::k_noise_S_tma<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(lac::k_noise_S_tma<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess)
+        return d;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_fine, lac::k_fine_gates_tma, lac::NT,
                                                       lac::FG_SMEM_BYTES) != cudaSuccess) return d;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_noise, lac::k_noise_S_tma, lac::NT,
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_noise, lac::k_noise_S_tma<3>, lac::NT,
                                                       lac::NS_SMEM_BYTES) != cudaSuccess) return d;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_quads, lac::k_noise_S_quads, 256, 0) != cudaSuccess) return d;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_eval, lac::k_eval_candidates<0>, 128, 0) != cudaSuccess) return d;
@@ -159,13 +162,14 @@ struct Workspace {
     int32_t* counts;   // per iteration: newly flagged pixels
     int32_t* ncand;    // per iteration (lazy path): candidate pixels evaluated
     int32_t* nquad;    // per iteration (lazy path): quads the incremental noise/S pass recomputed
+    int32_t *nneed, *nfine;   // per iteration, only with lacosmic_stats_enable: replacement values computed; fine tests
     float* gains;      // per iteration: the gain the noise model used (R21: estimated when p.gain == 0)
     lac::SelState* sel; // radix selection state and histogram of the gain estimation (select.cuh)
     uint32_t* hist;
     size_t bytes;      // total
     size_t zero_off, zero_bytes;   // region cleared at the start of a frame: the counters
 };
-constexpr int NCOUNTERS = 3 * LACOSMIC_MAX_NITER;
+constexpr int NCOUNTERS = LACOSMIC_NUM_FRAME_STATS * LACOSMIC_MAX_NITER;
 
 Workspace carve(void* base, int h, int w) {
     Workspace ws;
@@ -183,6 +187,8 @@ Workspace carve(void* base, int h, int w) {
     ws.counts = (int32_t*)(p + off); off += align_up(NCOUNTERS * 4, 256);
     ws.ncand = ws.counts + LACOSMIC_MAX_NITER;
     ws.nquad = ws.counts + 2 * LACOSMIC_MAX_NITER;
+    ws.nneed = ws.counts + 3 * LACOSMIC_MAX_NITER;
+    ws.nfine = ws.counts + 4 * LACOSMIC_MAX_NITER;
     ws.gains = (float*)(p + off); off += align_up(LACOSMIC_MAX_NITER * 4, 256);
     ws.sel = (lac::SelState*)(p + off); off += 256;
     ws.hist = (uint32_t*)(p + off); off += align_up(lac::SEL_BINS * 4, 256);
@@ -368,7 +374,14 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         const float* src = (fused_copy && t == 0) ? img : work;
         auto noise_pass = [&](const lac::NoiseArgs& na, const float* from) -> int {
             Span sp(KC_NOISE_S, st);
-            if (tma) lac::k_noise_S_tma<<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(from == img ? mapImgNS : mapWorkNS, na, ntx, ntilesNS, prev);
+            if (tma) {
+                // the two configurations of a plain frame are compiled without the tests of the nullable outputs
+                const CUtensorMap& map = from == img ? mapImgNS : mapWorkNS;
+                const bool plain = !na.dbgLp && !na.dbgN && !na.R && !na.gain_dev;
+                if (plain && na.copy_out && na.A1) lac::k_noise_S_tma<3><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
+                else if (plain && !na.copy_out && !na.A1) lac::k_noise_S_tma<0><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
+                else lac::k_noise_S_tma<-1><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
+            }
             else lac::k_noise_S<<<ntilesNS, tb, 0, st>>>(from, na, ntx, prev);
             LAUNCHED();
             return LACOSMIC_OK;
@@ -388,11 +401,6 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         // rewrote (ws.NEED); a debug dump recomputes the planes everywhere, and so does an estimated gain
         // (it changes with every iteration, and S with it)
         const bool incr = lazy && t > 0 && !d && !estimate;
-#ifndef LAC_BACKWARDS
-#define LAC_BACKWARDS 1
-#endif
-        // after a dense pass over the frame the sparse kernels walk it from the end (what the L2 still holds)
-        const int backwards = (LAC_BACKWARDS && !incr) ? 1 : 0;
         // R22 in the dense path: the gate kernel reads the noise plane, which the noise/S pass stores in the
         // candidate list's storage (not used by the dense path; free again once a gain estimate has been selected)
         float* const nplane = (d && dbg->N) ? dbg->N : ((fs1 && !lazy) ? (float*)ws.clist : nullptr);
@@ -436,10 +444,10 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         if (lazy) {
             // steps (3b)-(5) on the listed candidates only (lazy.cuh)
             lac::CandArgs ca{ws.S, work, ws.G1, ws.G2, ws.M1, h, w, wpr, p.sigclip, siglow, p.objlim,
-                             p.gain, rn2, estimate ? ws.gains + t : nullptr, var};
+                             p.gain, rn2, estimate ? ws.gains + t : nullptr, var, g_stats ? ws.nfine + t : nullptr};
             Span sp(KC_EVAL, st);
-            if (fs1) lac::k_eval_candidates<1><<<gridE, 128, 0, st>>>(ca, ws.clist, ws.ncand + t, prev, backwards);
-            else lac::k_eval_candidates<0><<<gridE, 128, 0, st>>>(ca, ws.clist, ws.ncand + t, prev, backwards);
+            if (fs1) lac::k_eval_candidates<1><<<gridE, 128, 0, st>>>(ca, ws.clist, ws.ncand + t, prev);
+            else lac::k_eval_candidates<0><<<gridE, 128, 0, st>>>(ca, ws.clist, ws.ncand + t, prev);
             LAUNCHED();
         } else {
             lac::FineArgs fa{ws.G1, ws.G2, ws.M1, d ? dbg->Sp : nullptr, d ? dbg->m3 : nullptr,
@@ -454,7 +462,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         lac::GrowArgs ga{ws.M1, ws.G1, ws.G2, ws.G2F, lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
                          ws.C[t & 1], ws.C[(t + 1) & 1], ws.NEED, d ? ws.M2 : nullptr, d ? ws.M3 : nullptr,
                          ws.S, img, work, ws.counts + t, incr ? 1 : 0, h, w, wpr, siglow, grow_nbx(w),
-                         donx, backwards};
+                         donx, g_stats ? ws.nneed + t : nullptr};
         if ((rc = grow_replace(ga, prev, st))) return rc;
         if (d) {
             // lazy path: G2 is only evaluated where step (6) needs it, so it is not dumped
@@ -535,7 +543,7 @@ int run_sepmed_frame(const float* img, int h, int w, const lacosmic_params& p, u
         // O6, O7: the product kernel (G2 complete, as in the dense path)
         lac::GrowArgs gr{ws.M1, ws.G1, ws.G2, ws.G2F, nullptr, nullptr, ws.C[t & 1], ws.C[(t + 1) & 1], ws.NEED,
                          d ? ws.M2 : nullptr, d ? ws.M3 : nullptr, A, img, work, ws.counts + t, 0, h, w, wpr, siglow,
-                         grow_nbx(w), nullptr, 0};
+                         grow_nbx(w), nullptr, nullptr};
         if ((rc = grow_replace(gr, prev, st))) return rc;
         if (d) {
             struct { const uint32_t* b; uint8_t* o; } planes[] = {{ws.G1, dbg->G1}, {ws.G2, dbg->G2}, {ws.M1, dbg->M1},
@@ -1078,7 +1086,7 @@ int lacosmic_masked_median_bpm(const float* img, const uint8_t* mask_u8, const u
     CK(cudaMemsetAsync(ws.C[0], 0, (size_t)h * wpr * 4, st));
     CK(cudaMemsetAsync(ws.counts, 0, 4, st));
     lac::GrowArgs ga{ws.M1, ws.M1, ws.M1, nullptr, nullptr, nullptr, ws.C[0], ws.C[1], ws.NEED, nullptr, nullptr,
-                     nullptr, img, out, ws.counts, 0, h, w, wpr, 0.0f, grow_nbx(w), bpm_u8 ? ws.DONX : nullptr, 0};
+                     nullptr, img, out, ws.counts, 0, h, w, wpr, 0.0f, grow_nbx(w), bpm_u8 ? ws.DONX : nullptr, nullptr};
     return grow_replace(ga, nullptr, st);
 }
 
@@ -1164,6 +1172,23 @@ int lacosmic_probe_minmax_rate(int kind, double* instr_per_s_host, void* stream)
     if (e1) cudaEventDestroy(e1);
     cudaFree(sink);
     return rc;
+}
+
+int lacosmic_stats_enable(int enable) {
+    g_stats = enable != 0;
+    return LACOSMIC_OK;
+}
+
+int lacosmic_frame_stats(const void* workspace, int h, int w, int32_t* stats_host, void* stream) {
+    if (!workspace || !stats_host) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    if ((uintptr_t)workspace & 255) return LACOSMIC_ERR_ALIGN;
+    Workspace ws = carve(const_cast<void*>(workspace), h, w);
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaMemcpyAsync(stats_host, ws.counts, (size_t)NCOUNTERS * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return LACOSMIC_OK;
 }
 
 int lacosmic_last_cuda_error(void) { return g_last_cuda_error; }

@@ -94,6 +94,7 @@ struct CandArgs {
     float gain, rn2;
     const float* gain_dev;   // nullable (R21)
     const float* var;        // nullable (R24)
+    int* nfine;              // nullable (lacosmic_stats_enable): += candidates that pass G1 and take the fine-structure test
 };
 
 // P(v) of the header comment, with exactly the operations of O4/O5.  nn == 0: R7 (num = L+, F in ADU); nn > 0: R22
@@ -187,20 +188,19 @@ __device__ __forceinline__ bool fine_bracket(float lp, float m3c, float objlim, 
 template <int FS>
 __global__ void __launch_bounds__(128, LAC_EVAL_MINB)
 k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restrict__ nlist,
-                  const int* prev_count, int backwards) {
+                  const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     const int n = *nlist;
     const int h = a.h, w = a.w;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        // backwards: the list is in frame order and the dense pass before it ran top to bottom, so the END of the
-        // planes is what the L2 still holds -- start there
-        const int p = list[backwards ? n - 1 - i : i];
+        const int p = list[i];
         const int y = p / w, x = p - y * w;
         int c1, c2;
         count_sp(a.S, y, x, h, w, a.sigclip, a.siglow, c1, c2);
         const uint32_t bit = 1u << (x & 31);
         const size_t q = (size_t)y * a.wpr + (x >> 5);
         if (c2 >= 13) atomicOr(a.G2 + q, bit);
+        if (a.nfine && c1 >= 13) atomicAdd(a.nfine, 1);      // statistics only (off in timed runs)
         if (c1 < 13) continue;
         atomicOr(a.G1 + q, bit);
         uint32_t rows[9];   // bit c of rows[r] = P(V[r][c])
@@ -318,9 +318,10 @@ k_noise_S_quads(const float* __restrict__ work, NoiseArgs a, const int* __restri
                 const float nn = a.var ? noise_from_var(m5[j])
                                        : noise_px(m5[j], a.gain_dev ? __ldg(a.gain_dev) : a.gain, a.rn2);
                 s[j] = fdiv_nn(lp, __fmul_rn(2.0f, nn));
-                const bool ok = (x + j < w) && (win[2 + j][2] < a.satlevel);                    // R12
-                n1 |= (uint32_t)(ok && s[j] > a.sigclip) << j;
-                n2 |= (uint32_t)(ok && s[j] > a.siglow) << j;
+                // threshold tests as sign bits on the FMA pipe (see noise_S_tile)
+                const uint32_t ok = (x + j < w) ? sign01(__fsub_rn(win[2 + j][2], a.satlevel)) : 0u;   // R12
+                n1 += (ok & sign01(__fsub_rn(a.sigclip, s[j]))) << j;
+                n2 += (ok & sign01(__fsub_rn(a.siglow, s[j]))) << j;
             }
             store4(a.S, (size_t)y * w, x, w, s);
             // this thread alone owns its nibble of the A1 / A2 words; the other nibbles change concurrently
