@@ -23,7 +23,10 @@ namespace lac {
 
 constexpr int WG_OWN = 30;                    // own word columns of a warp (lanes 1..30)
 constexpr int WG_R = 8;                       // own rows of a warp
-constexpr int WG_WARPS = 8;                   // warps per CTA, stacked vertically
+#ifndef LAC_WG_WARPS
+#define LAC_WG_WARPS 8
+#endif
+constexpr int WG_WARPS = LAC_WG_WARPS;        // warps per CTA, stacked vertically
 constexpr int WG_J = WG_R + 8;                // register rows: y = ya - 4 + j, j < WG_J
 constexpr int WG_LCAP = 128;                  // per-warp pixel list capacity of one round
 constexpr unsigned FULL = 0xffffffffu;
