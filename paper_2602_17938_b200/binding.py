@@ -456,11 +456,18 @@ def lacosmic_run_host_stream_sparse(imgs_host, params, capacity=None, out=None, 
 
 
 def lacosmic_clean(image, gain=1.0, readnoise=10.0, sigclip=4.5, sigfrac=0.3, objlim=5.0, niter=4,
-                   satlevel=65535.0, device="cuda:0"):
+                   satlevel=65535.0, device="cuda:0", fsmode=FS_ADU, satgrow=None, bpm=None, var=None):
     """The user-level entry point of the paper (one call with objlim, sigfrac, sigclip and
     optional gain / readnoise): a 2-D numpy array (float32, or the detector's uint16 counts) in, (mask bool
     [h][w], cleaned float32 [h][w]) numpy arrays out.  gain=0 (or None): estimated at each iteration.  Every
-    step runs in the CUDA library (lacosmic_run_host*); this wrapper only stages pinned host buffers."""
+    step runs in the CUDA library; this wrapper only stages buffers.
+
+    Fidelity note.  The default object test is the north-star text's (R7): L+/F > objlim with the fine
+    structure F in ADU.  van Dokkum's original form, which dfcosmic ports, compares S' with the fine structure in units
+    of the noise: fsmode=FS_NORMALISED (R22) selects it -- there the same objlim is about twice as strict (S'/Fn is
+    (L+/F)/2 where med5(S) = 0), so masks differ between the two settings.  satgrow=k protects (near-)saturated star
+    cores (R25), bpm / var are an input bad-pixel mask and a variance plane (R23, R24).  None of these readings could be
+    checked against dfcosmic's code or the IRAF masks (not available): expect differences in detail on real data."""
     import numpy as np
     torch = _torch()
     a = np.ascontiguousarray(image)
@@ -470,7 +477,19 @@ def lacosmic_clean(image, gain=1.0, readnoise=10.0, sigclip=4.5, sigfrac=0.3, ob
         a = a.astype(np.float32, copy=False)
     p = Params(gain=0.0 if gain is None else float(gain), readnoise=readnoise, sigclip=sigclip, sigfrac=sigfrac,
                objlim=objlim, satlevel=satlevel, niter=niter)
+    variant = fsmode != FS_ADU or satgrow is not None or bpm is not None or var is not None
     with torch.cuda.device(device):
+        if variant:      # the variants take device planes (lacosmic_run_ex)
+            dev = torch.device(device)
+            img = torch.from_numpy(a.astype(np.float32, copy=False)).to(dev)
+            kw = dict(fsmode=fsmode, satgrow=-1 if satgrow is None else satgrow)
+            if bpm is not None:
+                kw["bpm"] = torch.from_numpy(np.ascontiguousarray(bpm).astype(np.uint8)).to(dev)
+            if var is not None:
+                kw["var"] = torch.from_numpy(np.ascontiguousarray(var, dtype=np.float32)).to(dev)
+            r = lacosmic_run_ex(img, p, **kw)
+            torch.cuda.current_stream().synchronize()
+            return r["mask"].cpu().numpy().astype(bool), r["clean"].cpu().numpy()
         pinned = torch.from_numpy(a).pin_memory()          # stays referenced until the copy has completed
         r = lacosmic_run_host(pinned, p, device=device)
         torch.cuda.current_stream().synchronize()

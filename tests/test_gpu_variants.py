@@ -252,3 +252,11 @@ def test_variant_argument_errors(lc):
         with pytest.raises(lc.LacosmicError) as e:
             lc.lacosmic_run_ex(img, lc.Params(), **kw)
         assert e.value.code == -3
+
+
+def test_user_level_entry_point_with_variants(lc, orc):
+    f = _frame(150, 210, seed=45)
+    bpm = (_rng(4).random(f.img.shape) < 0.01).astype(np.uint8)
+    mask, clean = lc.lacosmic_clean(f.img, fsmode=lc.FS_NORMALISED, satgrow=1, bpm=bpm)
+    o = orc.run(f.img, fsmode=1, satgrow=1, bpm=bpm, **PARAMS)
+    assert np.array_equal(mask, o["mask"].astype(bool)) and np.array_equal(clean, o["clean"])
