@@ -101,6 +101,8 @@ struct GrowArgs {
     int nbx;                      // strips per row of strips = CTAs per row of CTAs (1-D grid, block_xy)
     const uint32_t* donx;         // nullable (R23): bad pixels, never donors of the replacement
     int* nneed;                   // nullable (lacosmic_stats_enable): += pixels whose replacement value is (re)computed
+    uint8_t* mask_u8;             // nullable: the frame's uint8 mask (cleared by the first pass): every pixel whose
+                                  // replacement is computed is in C', so it is set here
 };
 
 #ifndef LAC_GROW_MINB
@@ -313,6 +315,7 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
             hi = (q == ihi) ? s[q] : hi;
         }
         a.work[(size_t)y * w + x] = (k & 1) ? hi : __fmul_rn(__fadd_rn(lo, hi), 0.5f);   // R14
+        if (a.mask_u8) a.mask_u8[(size_t)y * w + x] = 1;
     });
 }
 

@@ -134,6 +134,8 @@ struct NoiseArgs {
     const uint32_t* nok;     // nullable (R23, R25): bit-plane of the pixels that may never be flagged (bad pixels,
                              // extended saturated-star mask); cleared from A1 / A2
     const float* var;        // nullable (R24): variance plane; N = sqrt(max(var, 1e-8)) replaces the noise model
+    uint8_t* mask_zero;      // nullable: the frame's uint8 mask, cleared by this pass (k_grow_replace then sets the flagged
+                             // pixels directly, and the frame needs no bit-plane -> uint8 expansion at its end)
 };
 
 // R24: N from a variance entry
@@ -159,8 +161,8 @@ constexpr int UW = 32, UH = 4;
 
 // sm: work tile with margins (NS_MX, NS_MY), edge-replicated
 // W4: w % 4 == 0 and 16-byte aligned planes (the TMA path): quads are whole and every store is one vector
-// CFG >= 0: the nullable outputs are known at compile time (bit 0: copy_out, bit 1: A1 / A2; no debug plane, no residual
-// plane, no device-side gain), which takes their tests out of the unit loop; CFG < 0: decided at run time.
+// CFG >= 0: the nullable outputs are known at compile time (bit 0: copy_out, bit 1: A1 / A2, bit 2: mask_zero; no debug
+// plane, no residual plane, no device-side gain), which takes their tests out of the unit loop; CFG < 0: decided at run time.
 // The threshold tests and their packing run on the FMA pipe: for finite a, b the sign of fsub(a, b) is set iff a < b
 // (a difference of two floats never rounds to zero unless they are equal: gradual underflow), so
 // (s > thr) = sign(thr - s), (c < satlevel) = sign(c - satlevel), and the nibble is a sum of sign bits times 2^j.
@@ -170,6 +172,7 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
     const int lx = lane & 7, lr = lane >> 3;
     const bool has_copy = CFG < 0 ? a.copy_out != nullptr : (CFG & 1) != 0;
     const bool has_A = CFG < 0 ? a.A1 != nullptr : (CFG & 2) != 0;
+    const bool has_mz = CFG < 0 ? a.mask_zero != nullptr : (CFG & 4) != 0;
     const bool has_lp = CFG < 0 && a.dbgLp != nullptr, has_n = CFG < 0 && a.dbgN != nullptr, has_R = CFG < 0 && a.R != nullptr;
     const float gain = (CFG < 0 && a.gain_dev) ? __ldg(a.gain_dev) : a.gain;
 #pragma unroll 1
@@ -201,6 +204,15 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
             if (has_lp) store4q<W4>(a.dbgLp, ro, x, a.w, lp);
             if (has_n) store4q<W4>(a.dbgN, ro, x, a.w, n);
             if (has_copy) store4q<W4>(a.copy_out, ro, x, a.w, ctr);
+            if (has_mz) {
+                if (W4) {
+                    *reinterpret_cast<uint32_t*>(a.mask_zero + ro + x) = 0u;     // 4 pixels; the API checks the alignment
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        if (x + j < a.w) a.mask_zero[ro + x + j] = 0;
+                }
+            }
             if (has_R) {   // R21: residual in units of sqrt(signal)
                 float r[4];
 #pragma unroll

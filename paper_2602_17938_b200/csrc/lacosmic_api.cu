@@ -121,7 +121,8 @@ DeviceInfo device_info() {
                              lac::FG_SMEM_BYTES) != cudaSuccess) return d;
     if (cudaFuncSetAttribute(lac::k_noise_S_tma<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(lac::k_noise_S_tma<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess ||
-        cudaFuncSetAttribute(lac::k_noise_S_tma<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess)
+        cudaFuncSetAttribute(lac::k_noise_S_tma<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(lac::k_noise_S_tma<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess)
         return d;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_fine, lac::k_fine_gates_tma, lac::NT,
                                                       lac::FG_SMEM_BYTES) != cudaSuccess) return d;
@@ -338,6 +339,9 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     // O0.  The lazy path fuses work = img_in into its first pass (which then reads img_in itself).
     const bool fused_copy = lazy && p.niter > 0;
     if (!fused_copy) CK(cudaMemcpyAsync(work, img, P * 4, cudaMemcpyDeviceToDevice, st));
+    // Lazy frames whose first launch is the noise/S kernel itself: that pass clears the uint8 mask and k_grow_replace
+    // sets the flagged pixels in it, which saves the bit-plane -> uint8 expansion (a launch and 29 MB) at the frame's end
+    const bool direct_mask = fused_copy && mask_out && !estimate && !var && ((uintptr_t)mask_out & 3) == 0;
     // C = 0 and the counter block: cleared by the first kernels of the frame (k_list_candidates clears C in the
     // lazy path, the first noise pass clears the counters); plain memsets where those kernels do not run
     const bool fused_zero = p.niter > 0;
@@ -387,8 +391,9 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                 // the two configurations of a plain frame are compiled without the tests of the nullable outputs
                 const CUtensorMap& map = from == img ? mapImgNS : mapWorkNS;
                 const bool plain = !na.dbgLp && !na.dbgN && !na.R && !na.gain_dev;
-                if (plain && na.copy_out && na.A1) lac::k_noise_S_tma<3><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
-                else if (plain && !na.copy_out && !na.A1) lac::k_noise_S_tma<0><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
+                if (plain && na.copy_out && na.A1 && na.mask_zero) lac::k_noise_S_tma<7><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
+                else if (plain && na.copy_out && na.A1 && !na.mask_zero) lac::k_noise_S_tma<3><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
+                else if (plain && !na.copy_out && !na.A1 && !na.mask_zero) lac::k_noise_S_tma<0><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
                 else lac::k_noise_S_tma<-1><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
             }
             else lac::k_noise_S<<<ntilesNS, tb, 0, st>>>(from, na, ntx, prev);
@@ -418,7 +423,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                           (fused_copy && t == 0 && !estimate) ? work : nullptr,
                           h, w, wpr, p.gain, rn2, p.sigclip, siglow, p.satlevel, nullptr,
                           estimate ? ws.gains + t : nullptr, (t == 0 && !estimate) ? zero_ptr : nullptr, zero_n,
-                          nok, var};
+                          nok, var, (direct_mask && t == 0) ? mask_out : nullptr};
         if (incr) {
             {
                 Span sp(KC_LISTS, st);
@@ -471,7 +476,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         lac::GrowArgs ga{ws.M1, ws.G1, ws.G2, ws.G2F, lazy ? ws.A1 : nullptr, lazy ? ws.A2 : nullptr,
                          ws.C[t & 1], ws.C[(t + 1) & 1], ws.NEED, d ? ws.M2 : nullptr, d ? ws.M3 : nullptr,
                          ws.S, img, work, ws.counts + t, incr ? 1 : 0, h, w, wpr, siglow, grow_nbx(w),
-                         donx, g_stats ? ws.nneed + t : nullptr};
+                         donx, g_stats ? ws.nneed + t : nullptr, direct_mask ? mask_out : nullptr};
         if ((rc = grow_replace(ga, prev, st))) return rc;
         if (d) {
             // lazy path: G2 is only evaluated where step (6) needs it, so it is not dumped
@@ -484,10 +489,11 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
     }
     const bool want_counts = iter_counts && p.niter > 0;
     // mask_out null: the caller reads the bit-plane.  The iteration counts ride along with the unpack launch.
-    int rc = mask_out ? unpack(ws.C[p.niter & 1], mask_out, h, w, st, ws.counts, want_counts ? iter_counts : nullptr, p.niter)
-                      : LACOSMIC_OK;
+    int rc = (mask_out && !direct_mask)
+                 ? unpack(ws.C[p.niter & 1], mask_out, h, w, st, ws.counts, want_counts ? iter_counts : nullptr, p.niter)
+                 : LACOSMIC_OK;
     if (rc) return rc;
-    if (want_counts && !mask_out)
+    if (want_counts && (!mask_out || direct_mask))
         CK(cudaMemcpyAsync(iter_counts, ws.counts, (size_t)p.niter * 4, cudaMemcpyDeviceToDevice, st));
     if (dbg && dbg->gains && p.niter > 0) {
         if (!estimate) {
@@ -552,7 +558,7 @@ int run_sepmed_frame(const float* img, int h, int w, const lacosmic_params& p, u
         // O6, O7: the product kernel (G2 complete, as in the dense path)
         lac::GrowArgs gr{ws.M1, ws.G1, ws.G2, ws.G2F, nullptr, nullptr, ws.C[t & 1], ws.C[(t + 1) & 1], ws.NEED,
                          d ? ws.M2 : nullptr, d ? ws.M3 : nullptr, A, img, work, ws.counts + t, 0, h, w, wpr, siglow,
-                         grow_nbx(w), nullptr, nullptr};
+                         grow_nbx(w), nullptr, nullptr, nullptr};
         if ((rc = grow_replace(gr, prev, st))) return rc;
         if (d) {
             struct { const uint32_t* b; uint8_t* o; } planes[] = {{ws.G1, dbg->G1}, {ws.G2, dbg->G2}, {ws.M1, dbg->M1},
@@ -1095,7 +1101,7 @@ int lacosmic_masked_median_bpm(const float* img, const uint8_t* mask_u8, const u
     CK(cudaMemsetAsync(ws.C[0], 0, (size_t)h * wpr * 4, st));
     CK(cudaMemsetAsync(ws.counts, 0, 4, st));
     lac::GrowArgs ga{ws.M1, ws.M1, ws.M1, nullptr, nullptr, nullptr, ws.C[0], ws.C[1], ws.NEED, nullptr, nullptr,
-                     nullptr, img, out, ws.counts, 0, h, w, wpr, 0.0f, grow_nbx(w), bpm_u8 ? ws.DONX : nullptr, nullptr};
+                     nullptr, img, out, ws.counts, 0, h, w, wpr, 0.0f, grow_nbx(w), bpm_u8 ? ws.DONX : nullptr, nullptr, nullptr};
     return grow_replace(ga, nullptr, st);
 }
 
