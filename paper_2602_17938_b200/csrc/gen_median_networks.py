@@ -432,7 +432,7 @@ def emit_sort(n, name):
 
 CONFIGS = [  # (k, T, function name)
     (3, 2, "median3x3_x2"), (3, 4, "median3x3_x4"),
-    (5, 2, "median5x5_x2"), (5, 4, "median5x5_x4"),
+    (5, 2, "median5x5_x2"), (5, 4, "median5x5_x4"), (5, 8, "median5x5_x8"),
     (7, 2, "median7x7_x2"), (7, 4, "median7x7_x4"),
 ]
 

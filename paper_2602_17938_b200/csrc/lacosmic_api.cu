@@ -93,7 +93,7 @@ bool make_map(CUtensorMap* m, const float* base, int h, int w, int boxW, int box
 }
 
 #ifndef LAC_NS_WAVES
-#define LAC_NS_WAVES 6
+#define LAC_NS_WAVES 8
 #endif
 #ifndef LAC_FG_WAVES
 #define LAC_FG_WAVES 6
