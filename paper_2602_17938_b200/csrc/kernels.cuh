@@ -113,8 +113,11 @@ __global__ void __launch_bounds__(NT) k_lplus(const float* __restrict__ in, floa
 // ------------------------------------------------------------------------------------------------
 // K_A: steps (1)-(3a).  work -> L+ (recomputed later, not stored), N = sqrt(gain*med5+rn^2)/gain,
 // S = L+/(2N).  Writes S; Lp/N only when a debug plane is requested.
+// Tile height 32: 128x64 tiles are 1 % faster for a single frame (0.640 vs 0.647 ms) but their two 38 KB stages x 3 CTAs
+// fill the SM's shared memory, and frames in flight on other streams can no longer interleave their kernels
+// (configs[3] with 4 frames in flight: 1321 frames/s against 1923 with 128x32 tiles; B200)
 #ifndef LAC_NS_TH
-#define LAC_NS_TH 64
+#define LAC_NS_TH 32
 #endif
 constexpr int NS_TH = LAC_NS_TH;   // tile height of the noise/S pass (own constant: its tile is much lighter than K_B's)
 // pitch 140 = 128 + 4 (left margin) + 8: the tile needs 136 columns; 140 (35 x 16 bytes) makes consecutive rows start 48
