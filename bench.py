@@ -210,6 +210,9 @@ def run_cuda(args):
         raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
+    # the pipeline's own (non-default) stream: on it the library replays a repeated frame call from a CUDA graph
+    # (include/lacosmic.h, lacosmic_graph_replay_enable; the legacy default stream cannot be captured)
+    torch.cuda.set_stream(torch.cuda.Stream(device=dev))
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     lc.load_library()
@@ -290,26 +293,13 @@ def run_cuda(args):
                        and res["counts"] == res_other["counts"])
     mask_frac = float(res["mask"].float().mean().item())
 
-    # ---- the same call captured once in a CUDA graph by the caller and replayed (the entry point only enqueues work, so
-    # it can be captured): what the 16 dependent launches cost beyond the kernels themselves
-    graph_replay = None
-    try:
-        gstep = make_step(main_mode)
-        g = torch.cuda.CUDAGraph()
-        side = torch.cuda.Stream()
-        with torch.cuda.stream(side):
-            gstep()
-            torch.cuda.synchronize()
-            with torch.cuda.graph(g, stream=side):
-                gstep()
-        torch.cuda.synchronize()
-        ms_graph = timed(g.replay, args.steps, 2)
-        graph_replay = dict(ms_per_step=ms_graph, frames_per_s=world * 1e3 / ms_graph,
-                            same_result=bool(torch.equal(mask, res["mask"]) and torch.equal(clean, res["clean"])),
-                            note="lacosmic_run_ws captured once with torch.cuda.graph and replayed; not the headline")
-        del g
-    except Exception as e:        # a capture problem must not take the bench line down
-        graph_replay = dict(error=str(e)[:200])
+    # ---- the same steps with the library's CUDA-graph replay switched off (every launch enqueued by the host each call):
+    # what the replay of the 16 dependent launches saves
+    lc.lacosmic_graph_replay_enable(False)
+    ms_direct = timed(make_step(main_mode), args.steps, 2)
+    lc.lacosmic_graph_replay_enable(True)
+    direct_launches = dict(ms_per_step=ms_direct, frames_per_s=world * 1e3 / ms_direct,
+                           note="lacosmic_graph_replay_enable(0): the same kernels, launched one by one from the host")
 
     # ---- the same frame with no gain supplied (estimated at each iteration, R21)
     gain_est = None
@@ -594,6 +584,8 @@ def run_cuda(args):
         config=dict(workload=wl["label"], h=h, w=w, niter=niter, sigclip=params["sigclip"],
                     sigfrac=params["sigfrac"], objlim=params["objlim"], mode=main_mode,
                     l2="flushed between steps (256 MiB write outside the event pair)",
+                    launch="lacosmic_run_ws on a non-default stream: the library replays the repeated call from a CUDA "
+                           "graph (every kernel runs every step; direct_launches = the same without the replay)",
                     parallelism="replicas (one frame per GPU, no collective)"),
         mpix_per_s=frames_per_s * npx / 1e6,
         # e2e leads with the sparse-result call: the cleaned frame equals the input outside the mask,
@@ -613,7 +605,7 @@ def run_cuda(args):
         ref_comparisons_T_per_s=ref_cmp_rate,
         other_mode=dict(mode=other_mode, same_mask_clean_counts=modes_agree, roofline=roofline(res_other),
                         **summarise(res_other)),
-        stream=stream_res, e2e_stream=e2e_stream, e2e_u16=e2e_u16, gain_estimation=gain_est, graph_replay=graph_replay,
+        stream=stream_res, e2e_stream=e2e_stream, e2e_u16=e2e_u16, gain_estimation=gain_est, direct_launches=direct_launches,
         new_cr_per_iteration=res["counts"], mask_fraction=mask_frac,
         clocks=clocks, cpu_baseline=cpu,
         context="paper (PAPER.md:31,47): 55 s/frame dfcosmic C++ at 2 threads on AWS; GPU variant on an "

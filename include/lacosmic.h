@@ -302,6 +302,17 @@ const char *lacosmic_version(void);
 int lacosmic_stats_enable(int enable);
 int lacosmic_frame_stats(const void *workspace, int h, int w, int32_t *stats_host, void *stream);
 
+/* Replay of repeated calls from a CUDA graph (process-wide switch; on by default, also off with the environment
+ * variable LACOSMIC_GRAPHS=0).  The launch sequence of lacosmic_run_ws is a function of its arguments alone (pointers,
+ * shape, parameters; everything data-dependent is decided on the device), so from the second call with identical
+ * arguments on the library captures the sequence once into a CUDA graph and later calls enqueue that graph: the same
+ * kernels run on every call, the host-side launch work is reused (about 2 us per dependent kernel; CUDA graphs are the
+ * launch mechanism the Blackwell guide recommends for launch-bound loops).  The 16 most recently used argument sets are
+ * kept.  Not used when `dbg` is given, while kernel timing or statistics are enabled, on the legacy default stream, or
+ * on a stream the caller is capturing (the call then enqueues its kernels directly, as always).  enable = 0 also drops
+ * the cached graphs.  Results and ordering on `stream` are identical either way. */
+int lacosmic_graph_replay_enable(int enable);
+
 /* Measured peak of the "alu" roofline (the medians of PAPER.md:23,64 are fp32 min/max selection
  * networks, bound by the rate at which the SMs issue FMNMX).  Runs a register-only kernel of independent min/max chains
  * (kind 0: two-input FMNMX; kind 1: three-input FMNMX3) on every SM of the current device and writes the achieved

@@ -25,7 +25,7 @@ EXPORTS = (
     "lacosmic_dilate3", "lacosmic_masked_median", "lacosmic_strerror",
     "lacosmic_last_cuda_error", "lacosmic_last_launch_count", "lacosmic_version",
     "lacosmic_kernel_timing_enable", "lacosmic_kernel_timing_read", "lacosmic_kernel_class_name",
-    "lacosmic_probe_minmax_rate", "lacosmic_stats_enable", "lacosmic_frame_stats",
+    "lacosmic_probe_minmax_rate", "lacosmic_stats_enable", "lacosmic_frame_stats", "lacosmic_graph_replay_enable",
     "lacosmic_run_ex", "lacosmic_sepmed_workspace_bytes", "lacosmic_run_sepmed_compare", "lacosmic_sepmedfilt",
     "lacosmic_masked_median_bpm", "lacosmic_satstar_mask",
 )
@@ -125,6 +125,7 @@ def load_library():
         "lacosmic_kernel_class_name": (C.c_char_p, [i]),
         "lacosmic_probe_minmax_rate": (i, [i, vp, vp]),
         "lacosmic_stats_enable": (i, [i]),
+        "lacosmic_graph_replay_enable": (i, [i]),
         "lacosmic_frame_stats": (i, [vp, i, i, vp, vp]),
         "lacosmic_run_ex": (i, [vp, i, i, C.POINTER(_CParams), C.POINTER(_CVariant), vp, vp, vp, sz, vp,
                                 C.POINTER(_CDebug), vp]),
@@ -649,6 +650,11 @@ def lacosmic_probe_minmax_rate(kind=0, stream=None):
 
 def lacosmic_stats_enable(enable=True):
     _check(load_library().lacosmic_stats_enable(1 if enable else 0), "lacosmic_stats_enable")
+
+
+def lacosmic_graph_replay_enable(enable=True):
+    """Switch the CUDA-graph replay of repeated identical lacosmic_run_ws calls on or off (process-wide; on by default)."""
+    _check(load_library().lacosmic_graph_replay_enable(1 if enable else 0), "lacosmic_graph_replay_enable")
 
 
 def lacosmic_frame_stats(workspace, h, w, stream=None):

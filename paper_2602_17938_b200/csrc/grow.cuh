@@ -22,7 +22,10 @@
 namespace lac {
 
 constexpr int WG_OWN = 30;                    // own word columns of a warp (lanes 1..30)
-constexpr int WG_R = 8;                       // own rows of a warp
+#ifndef LAC_WG_R
+#define LAC_WG_R 4
+#endif
+constexpr int WG_R = LAC_WG_R;                // own rows of a warp
 #ifndef LAC_WG_WARPS
 #define LAC_WG_WARPS 8
 #endif
@@ -128,13 +131,7 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
     const int base = (ya - 4) * wpr + wx;
     auto rowok = [&](int j) -> bool { return colok && (unsigned)(ya - 4 + j) < (unsigned)h; };
     auto qof = [&](int j) -> int { return base + j * wpr; };
-    if (prev_count && *prev_count == 0) {
-        // fixed point (R17): nothing changes; carry C over to the plane the next reader expects
-#pragma unroll
-        for (int j = 4; j < 4 + WG_R; ++j)
-            if (own && ya - 4 + j < h) a.Cnew[qof(j)] = a.Cold[qof(j)];
-        return;
-    }
+    const int pc = prev_count ? *prev_count : 1;             // tested below, after the M1 loads have been issued
     const bool lazy = a.A2 != nullptr;
     // M1 first.  In an incremental iteration (t >= 1) M1 only holds the new detections of this iteration, so most
     // strips see none within their 16 rows: then M2 = M3 = 0, nothing is fresh and nothing needs a replacement --
@@ -146,6 +143,13 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
     for (int j = 0; j < WG_J; ++j) {
         m1[j] = rowok(j) ? a.M1[qof(j)] : 0u;
         anym1 |= m1[j] != 0;
+    }
+    if (pc == 0) {
+        // fixed point (R17): nothing changes; carry C over to the plane the next reader expects
+#pragma unroll
+        for (int j = 4; j < 4 + WG_R; ++j)
+            if (own && ya - 4 + j < h) a.Cnew[qof(j)] = a.Cold[qof(j)];
+        return;
     }
     if (a.incremental && !__any_sync(FULL, anym1)) {
 #pragma unroll
@@ -367,7 +371,7 @@ k_dirty_lists(const uint32_t* __restrict__ NEED, const uint32_t* __restrict__ A1
               uint32_t* __restrict__ G2, uint32_t* __restrict__ G2F, uint32_t* __restrict__ M1,
               int* __restrict__ qlist, int* __restrict__ nq, int* __restrict__ clist, int* __restrict__ nc,
               int h, int w, int wpr, int nbx, const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;
+    const int pc = prev_count ? *prev_count : 1;             // tested below, after the NEED loads have been issued
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const BlockXY bk = block_xy(nbx);
     const int wx = bk.x * WG_OWN - 1 + lane;
@@ -383,7 +387,7 @@ k_dirty_lists(const uint32_t* __restrict__ NEED, const uint32_t* __restrict__ A1
         h2[j] = (colok && (unsigned)(ya - 4 + j) < (unsigned)h) ? NEED[base + j * wpr] : 0u;
         any |= h2[j] != 0;
     }
-    if (!__any_sync(FULL, any)) return;                       // nothing was rewritten near this strip
+    if (pc == 0 || !__any_sync(FULL, any)) return;            // fixed point (R17), or nothing was rewritten near this strip
 #pragma unroll
     for (int j = 0; j < WG_J; ++j) {
         // (halo lanes 0 / 31 have no outer neighbour: see hdil_w)

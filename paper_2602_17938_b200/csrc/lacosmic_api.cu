@@ -4,6 +4,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 
@@ -623,6 +624,61 @@ size_t lacosmic_workspace_bytes(int h, int w) {
     return carve(nullptr, h, w).bytes;
 }
 
+extern "C++" {
+namespace {
+// ---- replay of a repeated frame call from a CUDA graph ------------------------------------------
+// The launch sequence of a frame is a pure function of the call's arguments (pointers, shape, parameters): what
+// the kernels do with the data is decided on the device.  A pipeline that cleans frame after frame through the
+// same buffers therefore enqueues the same 16 launches every time; from the second identical call on, the
+// sequence is captured once into a CUDA graph and later calls replay it (one graph launch instead of 16 kernel
+// launches: ~2 us less launch latency per dependent kernel, 0.03 ms per 4000x6500 frame on B200).  Every kernel
+// still runs on every call -- only the host-side launch work is reused.  Not used with a debug dump, with kernel
+// timing or statistics on, on the legacy default stream or on a stream that is being captured by the caller.
+struct GraphKey {
+    int dev, h, w;
+    const void *img, *mask, *clean, *ws, *counts;
+    size_t ws_bytes;
+    lacosmic_params p;
+    bool operator==(const GraphKey& o) const {
+        return dev == o.dev && h == o.h && w == o.w && img == o.img && mask == o.mask && clean == o.clean &&
+               ws == o.ws && counts == o.counts && ws_bytes == o.ws_bytes && std::memcmp(&p, &o.p, sizeof p) == 0;
+    }
+};
+struct GraphEntry {
+    GraphKey key;
+    cudaGraphExec_t exec = nullptr;
+    int launches = 0;
+    int seen = 0;             // calls with this key so far
+    bool failed = false;      // capture or instantiation failed once: this key always takes the direct path
+    unsigned long long used = 0;
+};
+constexpr int GRAPH_CACHE = 16;
+GraphEntry g_graphs[GRAPH_CACHE];
+std::mutex g_graph_mu;
+unsigned long long g_graph_clock = 0;
+int g_graphs_on = -1;         // -1: not decided yet (environment LACOSMIC_GRAPHS=0 switches the replay off)
+
+bool graphs_enabled() {
+    if (g_graphs_on < 0) {
+        const char* e = std::getenv("LACOSMIC_GRAPHS");
+        g_graphs_on = (e && e[0] == '0') ? 0 : 1;
+    }
+    return g_graphs_on == 1;
+}
+}  // namespace
+}
+
+int lacosmic_graph_replay_enable(int enable) {
+    std::lock_guard<std::mutex> lock(g_graph_mu);
+    g_graphs_on = enable ? 1 : 0;
+    if (!enable)
+        for (GraphEntry& e : g_graphs) {
+            if (e.exec) cudaGraphExecDestroy(e.exec);
+            e = GraphEntry();
+        }
+    return LACOSMIC_OK;
+}
+
 int lacosmic_run_ws(const float* img, int h, int w, const lacosmic_params* p, uint8_t* mask_out,
                     float* clean_out, void* workspace, size_t workspace_bytes, int32_t* iter_counts,
                     const lacosmic_debug* dbg, void* stream) {
@@ -633,8 +689,68 @@ int lacosmic_run_ws(const float* img, int h, int w, const lacosmic_params* p, ui
     if (dbg)   // fp32 debug planes are written with 16-byte vectors
         for (const float* pl : {dbg->Lp, dbg->N, dbg->S, dbg->Sp, dbg->m3, dbg->F})
             if ((uintptr_t)pl & 15) return LACOSMIC_ERR_ALIGN;
-    return run_frame(img, h, w, *p, mask_out, clean_out, carve(workspace, h, w), iter_counts, dbg,
-                     (cudaStream_t)stream);
+    cudaStream_t st = (cudaStream_t)stream;
+    const Workspace ws = carve(workspace, h, w);
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    const bool replayable = !dbg && !g_kt.enabled && !g_stats && p->niter > 0 && st != nullptr && st != cudaStreamLegacy &&
+                            cudaStreamIsCapturing(st, &cap) == cudaSuccess && cap == cudaStreamCaptureStatusNone;
+    if (!replayable) {
+        cudaGetLastError();     // cudaStreamIsCapturing on the legacy stream during someone else's capture reports an error
+        return run_frame(img, h, w, *p, mask_out, clean_out, ws, iter_counts, dbg, st);
+    }
+    std::unique_lock<std::mutex> lock(g_graph_mu);
+    if (!graphs_enabled()) {
+        lock.unlock();
+        return run_frame(img, h, w, *p, mask_out, clean_out, ws, iter_counts, dbg, st);
+    }
+    GraphKey key;
+    std::memset(&key, 0, sizeof key);
+    cudaGetDevice(&key.dev);
+    key.h = h; key.w = w; key.img = img; key.mask = mask_out; key.clean = clean_out; key.ws = workspace;
+    key.counts = iter_counts; key.ws_bytes = workspace_bytes; key.p = *p;
+    GraphEntry* e = nullptr;
+    GraphEntry* lru = &g_graphs[0];
+    for (GraphEntry& g : g_graphs) {
+        if (g.seen && g.key == key) { e = &g; break; }
+        if (g.used < lru->used) lru = &g;
+    }
+    if (!e) {                   // first call with these arguments: remember them, run directly
+        if (lru->exec) cudaGraphExecDestroy(lru->exec);
+        *lru = GraphEntry();
+        lru->key = key;
+        lru->seen = 1;
+        lru->used = ++g_graph_clock;
+        lock.unlock();
+        return run_frame(img, h, w, *p, mask_out, clean_out, ws, iter_counts, dbg, st);
+    }
+    e->used = ++g_graph_clock;
+    ++e->seen;
+    if (!e->exec && !e->failed) {   // second call: capture the sequence
+        cudaGraph_t graph = nullptr;
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            rc = run_frame(img, h, w, *p, mask_out, clean_out, ws, iter_counts, dbg, st);
+            const cudaError_t ce = cudaStreamEndCapture(st, &graph);
+            if (rc == LACOSMIC_OK && ce == cudaSuccess && graph &&
+                cudaGraphInstantiate(&e->exec, graph, 0) == cudaSuccess) {
+                e->launches = g_launches;
+            } else {
+                e->exec = nullptr;
+                e->failed = true;
+            }
+            if (graph) cudaGraphDestroy(graph);
+        } else {
+            e->failed = true;
+        }
+        cudaGetLastError();
+    }
+    if (e->exec) {
+        g_launches = e->launches;
+        CK(cudaGraphLaunch(e->exec, st));
+        return LACOSMIC_OK;
+    }
+    lock.unlock();
+    g_launches = 0;
+    return run_frame(img, h, w, *p, mask_out, clean_out, ws, iter_counts, dbg, st);
 }
 
 int lacosmic_run_ex(const float* img, int h, int w, const lacosmic_params* p, const lacosmic_variant* v,

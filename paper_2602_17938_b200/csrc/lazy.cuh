@@ -189,8 +189,10 @@ template <int FS>
 __global__ void __launch_bounds__(128, LAC_EVAL_MINB)
 k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restrict__ nlist,
                   const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;
-    const int n = *nlist;
+    // the two counters are read together (one round trip, not two dependent ones, in front of the list)
+    const int pc = prev_count ? *prev_count : 1;
+    const int n0 = *nlist;
+    const int n = pc ? n0 : 0;
     const int h = a.h, w = a.w;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const int p = list[i];
@@ -268,10 +270,11 @@ k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restric
 __global__ void __launch_bounds__(256, 4)
 k_noise_S_quads(const float* __restrict__ work, NoiseArgs a, const int* __restrict__ qlist,
                 const int* __restrict__ nq, int* __restrict__ clist, int* __restrict__ nc, const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;
     __shared__ int s_warp[8];
     __shared__ int s_base;
-    const int n = *nq, h = a.h, w = a.w;
+    const int pc = prev_count ? *prev_count : 1;      // read together with the list length: one round trip
+    const int n0 = *nq;
+    const int n = pc ? n0 : 0, h = a.h, w = a.w;
     const int tid = threadIdx.x, lane = tid & 31, wi = tid >> 5;
     const bool vec = (w & 3) == 0;
     for (int base = blockIdx.x * 256; base < n; base += gridDim.x * 256) {   // uniform trip count per CTA

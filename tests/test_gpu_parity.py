@@ -637,6 +637,39 @@ def test_cuda_graph_capture_and_replay(lc, orc):
         assert np.array_equal(_n(counts), o["counts"])
 
 
+def test_repeated_call_replays_from_library_graph(lc, orc):
+    """lacosmic_graph_replay_enable (include/lacosmic.h): from the second call with identical arguments on, lacosmic_run_ws
+    captures its launch sequence and later calls replay it.  The frame CONTENTS change between the calls (same buffers,
+    the pipeline case), so every replay must do the full work: each result is compared with the oracle's for that frame,
+    in both modes, and with the replay switched off again."""
+    import torch
+    frames = [synth.make_frame(200, 292, seed=70 + k, n_star=15, n_cr=100 + 40 * k, n_hot=30, sp_frac=0.004) for k in range(4)]
+    oracle = [orc.run(f.img, **PARAMS) for f in frames]
+    h, w = frames[0].img.shape
+    s = torch.cuda.Stream()
+    for mode in (lc.MODE_LAZY, lc.MODE_DENSE):
+        img = torch.empty((h, w), dtype=torch.float32, device="cuda")
+        mask = torch.empty((h, w), dtype=torch.uint8, device="cuda")
+        clean = torch.empty_like(img)
+        ws = torch.empty(lc.lacosmic_workspace_bytes(h, w), dtype=torch.uint8, device="cuda")
+        counts = torch.zeros(PARAMS["niter"], dtype=torch.int32, device="cuda")
+        P = lc.Params(mode=mode, **PARAMS)
+        for enable in (True, False, True):
+            lc.lacosmic_graph_replay_enable(enable)
+            with torch.cuda.stream(s):
+                for rep in range(6):                      # calls 0 direct, 1 captures, 2.. replay
+                    k = rep % len(frames)
+                    img.copy_(_t(frames[k].img))
+                    mask.fill_(7); clean.fill_(-1.0); counts.fill_(-3)
+                    lc.lacosmic_run_ws(img, P, mask_out=mask, clean_out=clean, workspace=ws, iter_counts=counts, stream=s)
+                    assert lc.lacosmic_last_launch_count() > 0
+                    s.synchronize()
+                    o = oracle[k]
+                    assert np.array_equal(_n(mask), o["mask"]) and np.array_equal(_n(clean), o["clean"]), (mode, enable, rep)
+                    assert np.array_equal(_n(counts), o["counts"])
+    lc.lacosmic_graph_replay_enable(True)
+
+
 def test_config3_stream_full_size(lc, orc):
     """configs[3] at full frame size, shortened to 8 frames (seeds 1000..1007, sigclip cycling 4.0/4.5/5.0 by
     seed: per-frame parameters): lacosmic_run_batch with 4 frames in flight, in the configuration bench.py's
