@@ -237,11 +237,28 @@ int lacosmic_run_host_batch(const float *imgs_host, int n, int h, int w, const l
 
 /* R21 alone: the gain estimate of one image (what the whole path computes at the start of an iteration when
  * p->gain == 0), for the given read noise [e-].  gain_out: DEVICE pointer to one float; stats_out: nullable
- * DEVICE pointer to 6 floats {c, s, lo, hi, kept, mt}: centre, 1.4826 MAD, the interval the last clipping
- * round started from, the number of pixels inside it, and the typical signal (rank-(kept-1)/2 element of
- * max(med5, 1e-4) over those pixels).  workspace as for lacosmic_run_ws. */
+ * DEVICE pointer to 7 floats {c, s, lo, hi, kept, mt, fast}: centre, 1.4826 MAD, the interval the last clipping
+ * round started from, the number of pixels inside it, the typical signal (rank-(kept-1)/2 element of
+ * max(med5, 1e-4) over those pixels), and 1 if the three clipping rounds were resolved on the zone lists
+ * (two reads of the residual plane, csrc/selectz.cuh), 0 if by radix passes over the plane (csrc/select.cuh;
+ * taken when the fast path is switched off, on frames of a few pixels or of few distinct values, or when a
+ * check of the fast path fails) -- the values are the same bits either way.  workspace as for lacosmic_run_ws. */
 int lacosmic_estimate_gain(const float *img, int h, int w, float readnoise, float *gain_out,
                            float *stats_out, void *workspace, size_t workspace_bytes, void *stream);
+
+/* Diagnostic: the plan of the last gain estimate that ran in `workspace` (csrc/selectz.cuh, struct SelZone), copied to
+ * the HOST array info_host[LACOSMIC_GAIN_ZONE_WORDS] as 32-bit words after synchronising `stream`:
+ *   0-1 base, scale of the bucket grid (float bits); 2-7 bucket ranges of Z0, Z-, Z+ (lo, hi each); 8-9 last bucket of
+ *   OUT-, first of OUT+; 10 values below Z0; 11-13 values in Z0, Z-, Z+; 14 values between Z- and Z+; 15-16 values in
+ *   OUT-, OUT+; 17 pixels; 18-22 list cursors; 23 plan made; 24 rounds resolved on the lists; 25 where the fast path
+ *   stopped (0 it did not; 1 off / no grid; 2-4 plan; 10 j + 1..4: round j, bounds / centre / MAD rank / MAD); 26 the
+ *   residuals that are exactly +0. */
+#define LACOSMIC_GAIN_ZONE_WORDS 32
+int lacosmic_gain_zone_info(const void *workspace, int h, int w, int32_t *info_host, void *stream);
+
+/* Switches the fast path of the gain estimate on (default; environment LACOSMIC_GAIN_FAST=0 starts with it off)
+ * or off, for the whole process.  Results do not depend on it. */
+int lacosmic_gain_fast_path_enable(int enable);
 
 /* Step (1): out = L+(in).  in/out fp32 [h][w], distinct. */
 int lacosmic_lplus(const float *in, float *out, int h, int w, void *stream);

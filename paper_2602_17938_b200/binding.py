@@ -25,7 +25,7 @@ EXPORTS = (
     "lacosmic_dilate3", "lacosmic_masked_median", "lacosmic_strerror",
     "lacosmic_last_cuda_error", "lacosmic_last_launch_count", "lacosmic_version",
     "lacosmic_kernel_timing_enable", "lacosmic_kernel_timing_read", "lacosmic_kernel_class_name",
-    "lacosmic_probe_minmax_rate", "lacosmic_stats_enable", "lacosmic_frame_stats", "lacosmic_graph_replay_enable",
+    "lacosmic_probe_minmax_rate", "lacosmic_stats_enable", "lacosmic_frame_stats", "lacosmic_graph_replay_enable", "lacosmic_gain_fast_path_enable", "lacosmic_gain_zone_info",
     "lacosmic_run_ex", "lacosmic_sepmed_workspace_bytes", "lacosmic_run_sepmed_compare", "lacosmic_sepmedfilt",
     "lacosmic_masked_median_bpm", "lacosmic_satstar_mask",
 )
@@ -125,6 +125,8 @@ def load_library():
         "lacosmic_kernel_class_name": (C.c_char_p, [i]),
         "lacosmic_probe_minmax_rate": (i, [i, vp, vp]),
         "lacosmic_stats_enable": (i, [i]),
+        "lacosmic_gain_fast_path_enable": (i, [i]),
+        "lacosmic_gain_zone_info": (i, [vp, i, i, vp, vp]),
         "lacosmic_graph_replay_enable": (i, [i]),
         "lacosmic_frame_stats": (i, [vp, i, i, vp, vp]),
         "lacosmic_run_ex": (i, [vp, i, i, C.POINTER(_CParams), C.POINTER(_CVariant), vp, vp, vp, sz, vp,
@@ -531,18 +533,35 @@ def lacosmic_run_host_batch(imgs_host, params, masks_host=None, cleans_host=None
 
 
 # ----------------------------------------------------------------------------- single steps
-def lacosmic_estimate_gain(img, readnoise=0.0, workspace=None, stream=None):
-    """R21 alone.  Returns (gain: device float tensor [1], stats: device float tensor [6] = c, s, lo, hi, kept, mt)."""
+def lacosmic_gain_zone_info(workspace, h, w, stream=None):
+    """Diagnostic: the plan of the last gain estimate run in `workspace` as 32 int32 words (include/lacosmic.h)."""
+    import numpy as np
+    torch = _torch()
+    buf = np.zeros(32, np.int32)
+    _check(load_library().lacosmic_gain_zone_info(_dev(workspace, torch.uint8, "workspace"), int(h), int(w),
+                                                  buf.ctypes.data, _stream(stream)), "lacosmic_gain_zone_info")
+    return buf
+
+
+def lacosmic_gain_fast_path_enable(enable=True):
+    _check(load_library().lacosmic_gain_fast_path_enable(1 if enable else 0), "lacosmic_gain_fast_path_enable")
+
+
+def lacosmic_estimate_gain(img, readnoise=0.0, workspace=None, stream=None, want_path=False):
+    """R21 alone.  Returns (gain: device float tensor [1], stats: device float tensor [6] = c, s, lo, hi, kept, mt);
+    with want_path also a device float tensor [1]: 1 if the clipping rounds ran on the zone lists, 0 if on the plane."""
     torch = _torch()
     h, w = img.shape
     if workspace is None:
         workspace = _scratch_on(_workspace(h, w, img.device), stream)
     gain = torch.zeros(1, dtype=torch.float32, device=img.device)
-    stats = torch.zeros(6, dtype=torch.float32, device=img.device)
+    stats = torch.zeros(7, dtype=torch.float32, device=img.device)
     _check(load_library().lacosmic_estimate_gain(
         _dev(img, torch.float32, "img"), h, w, float(readnoise), gain.data_ptr(), stats.data_ptr(),
         _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)), "lacosmic_estimate_gain")
-    return gain, stats
+    if want_path:
+        return gain, stats[:6], stats[6:7]
+    return gain, stats[:6]
 
 
 def lacosmic_lplus(img, out=None, stream=None):

@@ -12,6 +12,7 @@
 #include "lazy.cuh"
 #include "grow.cuh"
 #include "select.cuh"
+#include "selectz.cuh"
 #include "compact.cuh"
 #include "probe.cuh"
 #include "sepmed.cuh"
@@ -174,6 +175,8 @@ struct Workspace {
     float* gains;      // per iteration: the gain the noise model used (R21: estimated when p.gain == 0)
     lac::SelState* sel; // radix selection state and histogram of the gain estimation (select.cuh)
     uint32_t* hist;
+    lac::SelZone* zone; // fast path of the gain estimation (selectz.cuh): plan, bucket counts, zone id of every bucket
+    uint32_t* histz;
     size_t bytes;      // total
     size_t zero_off, zero_bytes;   // region cleared at the start of a frame: the counters
 };
@@ -200,6 +203,8 @@ Workspace carve(void* base, int h, int w) {
     ws.gains = (float*)(p + off); off += align_up(LACOSMIC_MAX_NITER * 4, 256);
     ws.sel = (lac::SelState*)(p + off); off += 256;
     ws.hist = (uint32_t*)(p + off); off += align_up(lac::SEL_BINS * 4, 256);
+    ws.zone = (lac::SelZone*)(p + off); off += align_up(sizeof(lac::SelZone), 256);
+    ws.histz = (uint32_t*)(p + off); off += align_up(lac::SELZ_NB * 4, 256);
     ws.zero_bytes = off - ws.zero_off;
     ws.bytes = off;
     return ws;
@@ -233,17 +238,28 @@ int grow_replace(const lac::GrowArgs& ga, const int* prev, cudaStream_t st) {
     return LACOSMIC_OK;
 }
 
-// R21: sigma clipping of the residual plane R, typical signal from the med5 plane M5 (select.cuh)
-// -> *gain_out (device), stats (nullable, device, 6 floats)
+// R21: sigma clipping of the residual plane R, typical signal from the med5 plane M5 (select.cuh, selectz.cuh)
+// -> *gain_out (device), stats (nullable, device, 7 floats).  `lists`: storage of the fast path's lists (list_words
+// 32-bit words: the quad list and the planes G1, G2, G2F, M1, M2, M3 behind it, which hold nothing at this point of an
+// iteration that estimates the gain -- such an iteration is never incremental and rewrites them all).
+int g_gain_fast = -1;          // -1: not decided yet (environment LACOSMIC_GAIN_FAST=0 switches the fast path off)
+bool gain_fast_enabled() {
+    if (g_gain_fast < 0) {
+        const char* e = std::getenv("LACOSMIC_GAIN_FAST");
+        g_gain_fast = (e && e[0] == '0') ? 0 : 1;
+    }
+    return g_gain_fast == 1;
+}
 template <int MODE, int PASS>
-int sel_step(const float* R, const float* M5, size_t npx, const Workspace& ws, int grid, int last, float rn2,
-             float* gain_out, float* stats, const int* prev, cudaStream_t st) {
-    lac::k_sel_hist<MODE, PASS><<<grid, 256, 0, st>>>(R, M5, npx, ws.sel, ws.hist, last, rn2, gain_out, stats, prev);
+int sel_step(const float* R, const float* M5, size_t npx, const Workspace& ws, const float2* olist, int grid, int last,
+             float rn2, float* gain_out, float* stats, const int* prev, cudaStream_t st) {
+    lac::k_sel_hist<MODE, PASS><<<grid, 256, 0, st>>>(R, M5, npx, ws.sel, ws.hist, last, rn2, gain_out, stats, prev,
+                                                      &ws.zone->done, &ws.zone->no, olist);
     LAUNCHED();
     return LACOSMIC_OK;
 }
-int sigma_clip_gain(const float* R, const float* M5, size_t npx, const Workspace& ws, float rn2, float* gain_out,
-                    float* stats, const int* prev, cudaStream_t st) {
+int sigma_clip_gain(const float* R, const float* M5, size_t npx, const Workspace& ws, void* lists, size_t list_words,
+                    float rn2, float* gain_out, float* stats, const int* prev, cudaStream_t st) {
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
 #ifndef LAC_SEL_CTAS_PER_SM
@@ -251,23 +267,41 @@ int sigma_clip_gain(const float* R, const float* M5, size_t npx, const Workspace
 #endif
     // full occupancy measured best on B200 (8 > 4 > 2 > 1 CTAs per SM): the pass is a streaming read
     const int grid = (int)std::min<size_t>((size_t)sms * LAC_SEL_CTAS_PER_SM, (npx / 4 + 255) / 256 + 1);
+    // the lists of the fast path (selectz.cuh) live in the quad list's storage
+    const float2* olist = lac::selz_carve(lists, list_words).o;
+    const int grid_h = (int)std::min<size_t>((size_t)sms * 2, (npx / 4 + 4 * lac::SELZ_HT - 1) / (4 * lac::SELZ_HT) + 1);
+    if (lac::SELZ_CLUSTER > 8) {              // once per device: clusters of 16 CTAs are a non-portable size
+        static bool allowed[MAX_DEVICES] = {};
+        if (dev >= 0 && dev < MAX_DEVICES && !allowed[dev]) {
+            CK(cudaFuncSetAttribute(lac::k_selz_resolve, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+            allowed[dev] = true;
+        }
+    }
     Span sp(KC_SELECT, st);
-    lac::k_sel_init<<<1, 256, 0, st>>>(ws.sel, ws.hist, prev);
+    lac::k_selz_init<<<1, lac::SELZ_SAMPLE, 0, st>>>(R, npx, ws.sel, ws.zone, ws.hist, ws.histz, gain_fast_enabled() ? 0 : 1, prev);
+    LAUNCHED();
+    lac::k_selz_hist<<<grid_h, lac::SELZ_HT, 0, st>>>(R, npx, ws.sel, ws.zone, ws.histz, lists, list_words, prev);
+    LAUNCHED();
+    lac::k_selz_compact<<<grid, 256, 0, st>>>(R, M5, npx, ws.zone, lists, list_words, prev);
+    LAUNCHED();
+    lac::k_selz_resolve<<<lac::SELZ_CLUSTER, lac::SELZ_RT, 0, st>>>(ws.sel, ws.zone, ws.histz, lists, list_words,
+                                                                    stats ? stats + 6 : nullptr, prev);
     LAUNCHED();
     int rc;
+    // (these return at once when the fast path resolved the three rounds)
     for (int j = 0; j < lac::SEL_ROUNDS; ++j) {
         const int last = j == lac::SEL_ROUNDS - 1;
-        if ((rc = sel_step<0, 0>(R, M5, npx, ws, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<0, 1>(R, M5, npx, ws, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<0, 2>(R, M5, npx, ws, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<1, 0>(R, M5, npx, ws, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<1, 1>(R, M5, npx, ws, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<1, 2>(R, M5, npx, ws, grid, last, rn2, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<0, 0>(R, M5, npx, ws, olist, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<0, 1>(R, M5, npx, ws, olist, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<0, 2>(R, M5, npx, ws, olist, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<1, 0>(R, M5, npx, ws, olist, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<1, 1>(R, M5, npx, ws, olist, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
+        if ((rc = sel_step<1, 2>(R, M5, npx, ws, olist, grid, last, rn2, gain_out, stats, prev, st))) return rc;
     }
     // typical signal over the set the last round kept, then the gain
-    if ((rc = sel_step<2, 0>(R, M5, npx, ws, grid, 1, rn2, gain_out, stats, prev, st))) return rc;
-    if ((rc = sel_step<2, 1>(R, M5, npx, ws, grid, 1, rn2, gain_out, stats, prev, st))) return rc;
-    if ((rc = sel_step<2, 2>(R, M5, npx, ws, grid, 1, rn2, gain_out, stats, prev, st))) return rc;
+    if ((rc = sel_step<2, 0>(R, M5, npx, ws, olist, grid, 1, rn2, gain_out, stats, prev, st))) return rc;
+    if ((rc = sel_step<2, 1>(R, M5, npx, ws, olist, grid, 1, rn2, gain_out, stats, prev, st))) return rc;
+    if ((rc = sel_step<2, 2>(R, M5, npx, ws, olist, grid, 1, rn2, gain_out, stats, prev, st))) return rc;
     return LACOSMIC_OK;
 }
 
@@ -409,7 +443,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                               h, w, wpr, 1.0f, rn2, p.sigclip, siglow, p.satlevel, (float*)ws.clist, nullptr,
                               t == 0 ? zero_ptr : nullptr, zero_n};
             if ((rc = noise_pass(ne, src))) return rc;
-            if ((rc = sigma_clip_gain((const float*)ws.clist, ws.S, P, ws, rn2, ws.gains + t, nullptr, prev, st))) return rc;
+            if ((rc = sigma_clip_gain((const float*)ws.clist, ws.S, P, ws, ws.qlist, (size_t)((char*)ws.C[0] - (char*)ws.qlist) / 4, rn2, ws.gains + t, nullptr, prev, st))) return rc;
             src = work;
         }
         // lazy path, t >= 1: S, A1, A2 and the tests only change near the pixels the previous replacement
@@ -1086,7 +1120,13 @@ int lacosmic_estimate_gain(const float* img, int h, int w, float readnoise, floa
     const int ntx = (w + lac::TW - 1) / lac::TW, nt = ntx * ((h + lac::NS_TH - 1) / lac::NS_TH);
     lac::k_noise_S<<<nt, lac::NT, 0, st>>>(img, ne, ntx, nullptr);
     LAUNCHED();
-    return sigma_clip_gain((const float*)ws.clist, ws.S, P, ws, readnoise * readnoise, gain_out, stats_out, nullptr, st);
+    return sigma_clip_gain((const float*)ws.clist, ws.S, P, ws, ws.qlist, (size_t)((char*)ws.C[0] - (char*)ws.qlist) / 4, readnoise * readnoise, gain_out, stats_out,
+                           nullptr, st);
+}
+
+int lacosmic_gain_fast_path_enable(int enable) {
+    g_gain_fast = enable ? 1 : 0;
+    return LACOSMIC_OK;
 }
 
 int lacosmic_lplus(const float* in, float* out, int h, int w, void* stream) {
@@ -1318,6 +1358,20 @@ int lacosmic_frame_stats(const void* workspace, int h, int w, int32_t* stats_hos
     Workspace ws = carve(const_cast<void*>(workspace), h, w);
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaMemcpyAsync(stats_host, ws.counts, (size_t)NCOUNTERS * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return LACOSMIC_OK;
+}
+
+int lacosmic_gain_zone_info(const void* workspace, int h, int w, int32_t* info_host, void* stream) {
+    if (!workspace || !info_host) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    if ((uintptr_t)workspace & 255) return LACOSMIC_ERR_ALIGN;
+    Workspace ws = carve(const_cast<void*>(workspace), h, w);
+    static_assert(sizeof(lac::SelZone) <= LACOSMIC_GAIN_ZONE_WORDS * 4, "header and library disagree");
+    cudaStream_t st = (cudaStream_t)stream;
+    std::memset(info_host, 0, LACOSMIC_GAIN_ZONE_WORDS * 4);
+    CK(cudaMemcpyAsync(info_host, ws.zone, sizeof(lac::SelZone), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     return LACOSMIC_OK;
 }

@@ -37,6 +37,63 @@ __device__ __forceinline__ float sel_unkey(uint32_t k) {
     return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
 }
 
+// inclusive prefix sums over the 256 threads of a CTA (scan: 256 words of shared memory); returns this thread's
+__device__ __forceinline__ uint32_t sel_scan256(uint32_t sum, uint32_t* scan) {
+    const int tid = threadIdx.x;
+    scan[tid] = sum;
+    __syncthreads();
+    for (int d = 1; d < 256; d <<= 1) {
+        const uint32_t v = tid >= d ? scan[tid - d] : 0u;
+        __syncthreads();
+        scan[tid] += v;
+        __syncthreads();
+    }
+    return scan[tid];
+}
+
+// Visits the plane R (and M5 when WITH_M5) in chunks of 16 values per thread of an NT-thread CTA: f(r, m5, valid, index) is
+// called by ALL threads of the CTA the same number of times (valid = false past the end), so f may use warp votes.
+template <bool WITH_M5, int NT, class F>
+__device__ __forceinline__ void sel_visit_plane(const float* __restrict__ R, const float* __restrict__ M5, size_t npx, F f) {
+    const size_t nvec = npx / 4;
+    const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (size_t b0 = (size_t)blockIdx.x * (4 * NT); b0 < nvec; b0 += (size_t)gridDim.x * (4 * NT)) {
+        float4 q[4], m[4];
+        bool ok[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {     // four independent 16-byte loads in flight per thread
+            const size_t i = b0 + u * NT + threadIdx.x;
+            ok[u] = i < nvec;
+            q[u] = ok[u] ? __ldg(reinterpret_cast<const float4*>(R) + i) : zero4;
+            m[u] = (WITH_M5 && ok[u]) ? __ldg(reinterpret_cast<const float4*>(M5) + i) : zero4;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const size_t i4 = 4 * (b0 + u * NT + threadIdx.x);
+            f(q[u].x, m[u].x, ok[u], i4); f(q[u].y, m[u].y, ok[u], i4 + 1); f(q[u].z, m[u].z, ok[u], i4 + 2);
+            f(q[u].w, m[u].w, ok[u], i4 + 3);
+        }
+    }
+    if (blockIdx.x == 0) {                // the last npx % 4 values
+        const size_t t = nvec * 4 + threadIdx.x;
+        const bool ok = t < npx;
+        f(ok ? R[t] : 0.0f, (WITH_M5 && ok) ? M5[t] : 0.0f, ok, t);
+    }
+}
+
+// shared-memory histogram increment with the warp's votes for the leader's bucket combined into one atomic
+// (values that are smooth over the frame, or a list of equal keys, put a whole warp on one address).  All 32
+// lanes call.
+__device__ __forceinline__ void sel_hist_add(uint32_t* sh, bool valid, uint32_t bin) {
+    const unsigned m = __ballot_sync(0xffffffffu, valid);
+    if (m == 0) return;
+    const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
+    const uint32_t b0 = __shfl_sync(0xffffffffu, bin, leader);
+    const unsigned same = __ballot_sync(0xffffffffu, valid && bin == b0);
+    if (lane == leader) atomicAdd(&sh[b0], (uint32_t)__popc(same));
+    else if (valid && bin != b0) atomicAdd(&sh[bin], 1u);
+}
+
 __global__ void k_sel_init(SelState* st, uint32_t* hist, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     for (int i = threadIdx.x; i < SEL_BINS; i += blockDim.x) hist[i] = 0;
@@ -125,11 +182,17 @@ __device__ __forceinline__ void sel_pick(SelState* st, uint32_t* hist, uint32_t*
 template <int MODE, int PASS>
 __global__ void __launch_bounds__(256)
 k_sel_hist(const float* __restrict__ R, const float* __restrict__ M5, size_t npx, SelState* st, uint32_t* hist,
-           int last, float rn2, float* gain_out, float* stats, const int* prev_count) {
+           int last, float rn2, float* gain_out, float* stats, const int* prev_count, const uint32_t* zdone,
+           const uint32_t* zno, const float2* __restrict__ olist) {
     if (prev_count && *prev_count == 0) {          // fixed point (R17): same image, same estimate
         if (MODE == 2 && PASS == 2 && blockIdx.x == 0 && threadIdx.x == 0) *gain_out = gain_out[-1];
         return;
     }
+    // selectz.cuh: the three rounds were resolved on the zone lists.  The passes over r and |r - c| then have
+    // nothing to do, and the typical signal is selected over ALL pixels of the med5 plane minus the listed pixels
+    // outside the kept interval (every such pixel is in the OUT list), so that the residual plane is not read again.
+    const bool fast = zdone && *zdone;
+    if (MODE != 2 && fast) return;
     __shared__ uint32_t sh[SEL_BINS];
     for (int i = threadIdx.x; i < SEL_BINS; i += 256) sh[i] = 0;
     __syncthreads();
@@ -152,7 +215,7 @@ k_sel_hist(const float* __restrict__ R, const float* __restrict__ M5, size_t npx
         if (MODE == 0) {
             k = sel_key(r);
         } else {
-            if (!(r >= lo && r <= hi)) return;
+            if (!(MODE == 2 && fast) && !(r >= lo && r <= hi)) return;
             const float v = MODE == 1 ? fabsf(__fsub_rn(r, c)) : (m5 > 1e-4f ? m5 : 1e-4f);
             k = __float_as_uint(v) | 0x80000000u;   // non-negative value
         }
@@ -162,12 +225,14 @@ k_sel_hist(const float* __restrict__ R, const float* __restrict__ M5, size_t npx
     const size_t stride = (size_t)gridDim.x * 256, end = nvec;
     size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
     const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    const bool one = MODE == 2 && fast;             // only the med5 plane is read
+    const float* P0 = one ? M5 : R;
     for (; i + 3 * stride < end; i += 4 * stride) {   // four independent 16-byte loads in flight per thread
         float4 q[4], m[4];
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-            q[u] = __ldg(reinterpret_cast<const float4*>(R) + i + u * stride);
-            m[u] = MODE == 2 ? __ldg(reinterpret_cast<const float4*>(M5) + i + u * stride) : zero4;
+            q[u] = __ldg(reinterpret_cast<const float4*>(P0) + i + u * stride);
+            m[u] = (MODE == 2 && !one) ? __ldg(reinterpret_cast<const float4*>(M5) + i + u * stride) : MODE == 2 ? q[u] : zero4;
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
@@ -175,13 +240,23 @@ k_sel_hist(const float* __restrict__ R, const float* __restrict__ M5, size_t npx
         }
     }
     for (; i < end; i += stride) {
-        const float4 q = __ldg(reinterpret_cast<const float4*>(R) + i);
-        const float4 m = MODE == 2 ? __ldg(reinterpret_cast<const float4*>(M5) + i) : zero4;
+        const float4 q = __ldg(reinterpret_cast<const float4*>(P0) + i);
+        const float4 m = (MODE == 2 && !one) ? __ldg(reinterpret_cast<const float4*>(M5) + i) : MODE == 2 ? q : zero4;
         visit(q.x, m.x); visit(q.y, m.y); visit(q.z, m.z); visit(q.w, m.w);
     }
     if (blockIdx.x == 0 && threadIdx.x < (int)(npx - nvec * 4)) {
         const size_t t = nvec * 4 + threadIdx.x;
-        visit(R[t], MODE == 2 ? M5[t] : 0.0f);
+        visit(P0[t], MODE == 2 ? M5[t] : 0.0f);
+    }
+    if (one) {                                      // take the listed pixels outside the kept interval out again
+        const uint32_t no = *zno;
+        for (uint32_t j = blockIdx.x * 256 + threadIdx.x; j < no; j += gridDim.x * 256) {
+            const float2 e = olist[j];
+            if (e.x >= lo && e.x <= hi) continue;
+            const float v = e.y > 1e-4f ? e.y : 1e-4f;
+            const uint32_t k = __float_as_uint(v) | 0x80000000u;
+            if (!none && k - klo <= span) atomicSub(&sh[(k >> SHIFT) & MASK], 1u);   // (wraps; the global sum is exact)
+        }
     }
     __syncthreads();
     for (int i = threadIdx.x; i < SEL_BINS; i += 256)

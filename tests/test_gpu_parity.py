@@ -459,6 +459,44 @@ def test_estimate_gain_ties_and_degenerate(lc, orc):
         assert _n(g)[0] == go and np.array_equal(_n(st), sto)
 
 
+@pytest.mark.parametrize("kind", ["frame", "integer", "gain4", "gain0p2", "skewed", "coarse"])
+def test_estimate_gain_fast_path_equals_oracle_and_plane_path(lc, orc, kind):
+    """The fast path of the estimate (two reads of the residual plane, rounds resolved on zone lists, csrc/selectz.cuh)
+    and the radix passes over the plane (csrc/select.cuh) give the oracle's bits; on frames like the paper's the fast
+    path is the one that runs (stats[6] = 1), on a frame of few distinct values it hands over to the plane passes."""
+    import torch
+    rng = _rng(77)
+    if kind == "frame":
+        x = synth.make_frame(700, 900, seed=5, n_star=60, n_cr=700, n_hot=150, sp_frac=0.005).img
+    elif kind == "integer":            # raw counts: heavy ties in the residuals
+        x = np.rint(synth.make_frame(600, 800, seed=6, n_star=40, n_cr=500, sp_frac=0.004).img).astype(np.float32)
+    elif kind == "gain4":              # narrow residuals (sigma_r = 0.5)
+        x = (400.0 + np.sqrt(400.0 / 4.0) * rng.standard_normal((640, 720))).astype(np.float32)
+    elif kind == "gain0p2":            # wide residuals (sigma_r = 2.2)
+        x = (400.0 + np.sqrt(400.0 / 0.2) * rng.standard_normal((640, 720))).astype(np.float32)
+    elif kind == "skewed":             # 8 % of the pixels far above the rest: the centre moves between the rounds
+        x = (200.0 + 12.0 * rng.standard_normal((600, 700))).astype(np.float32)
+        x.flat[rng.integers(0, x.size, x.size // 12)] += rng.uniform(100.0, 3000.0, x.size // 12).astype(np.float32)
+    else:                              # 16 distinct values only
+        x = (100.0 + 4.0 * rng.integers(0, 16, (500, 640))).astype(np.float32)
+    go, sto = orc.estimate_gain(x, 6.0)
+    paths = {}
+    try:
+        for fast in (True, False):
+            lc.lacosmic_gain_fast_path_enable(fast)
+            g, st, path = lc.lacosmic_estimate_gain(_t(x), readnoise=6.0, want_path=True)
+            torch.cuda.synchronize()
+            assert _n(g)[0] == go, (kind, fast, float(_n(g)[0]), float(go))
+            assert np.array_equal(_n(st), sto), (kind, fast, _n(st), sto)
+            paths[fast] = float(_n(path)[0])
+    finally:
+        lc.lacosmic_gain_fast_path_enable(True)
+    assert paths[False] == 0.0
+    print("estimate_gain[%s]: fast path taken = %s" % (kind, paths[True]))
+    if kind in ("frame", "gain4", "gain0p2"):
+        assert paths[True] == 1.0, kind
+
+
 @pytest.mark.parametrize("mode", [0, 1], ids=["lazy", "dense"])
 @pytest.mark.parametrize("cfg", [dict(h=200, w=264, seed=71, n_star=12, n_cr=150, n_hot=30, sp_frac=0.004),
                                  dict(h=131, w=97, seed=72, n_star=4, n_cr=60, sp_frac=0.0)])
