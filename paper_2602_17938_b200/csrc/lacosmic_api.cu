@@ -288,15 +288,21 @@ int sigma_clip_gain(const float* R, const float* M5, size_t npx, const Workspace
                                                                     stats ? stats + 6 : nullptr, prev);
     LAUNCHED();
     int rc;
-    // (these return at once when the fast path resolved the three rounds)
-    for (int j = 0; j < lac::SEL_ROUNDS; ++j) {
-        const int last = j == lac::SEL_ROUNDS - 1;
-        if ((rc = sel_step<0, 0>(R, M5, npx, ws, olist, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<0, 1>(R, M5, npx, ws, olist, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<0, 2>(R, M5, npx, ws, olist, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<1, 0>(R, M5, npx, ws, olist, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<1, 1>(R, M5, npx, ws, olist, grid, 0, rn2, gain_out, stats, prev, st))) return rc;
-        if ((rc = sel_step<1, 2>(R, M5, npx, ws, olist, grid, last, rn2, gain_out, stats, prev, st))) return rc;
+    {
+        // the rounds by radix passes over the plane: one cooperative launch, which returns at once when the fast path
+        // has resolved them.  Its grid must be resident as a whole.
+        static int per_sm[MAX_DEVICES] = {};
+        if (dev < 0 || dev >= MAX_DEVICES) return LACOSMIC_ERR_CUDA;
+        if (!per_sm[dev]) {
+            int n = 0;
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, lac::k_sel_rounds, 256, 0));
+            per_sm[dev] = std::max(1, std::min(n, LAC_SEL_CTAS_PER_SM));
+        }
+        const int grid_c = std::min(grid, sms * per_sm[dev]);
+        const uint32_t* zdone = &ws.zone->done;
+        void* args[] = {(void*)&R, (void*)&npx, (void*)&ws.sel, (void*)&ws.hist, (void*)&prev, (void*)&zdone};
+        CK(cudaLaunchCooperativeKernel((const void*)lac::k_sel_rounds, dim3((unsigned)grid_c), dim3(256), args, 0, st));
+        LAUNCHED();
     }
     // typical signal over the set the last round kept, then the gain
     if ((rc = sel_step<2, 0>(R, M5, npx, ws, olist, grid, 1, rn2, gain_out, stats, prev, st))) return rc;

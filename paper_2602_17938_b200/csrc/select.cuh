@@ -10,6 +10,8 @@
 // and the MAD d (same rank of |r - c|).  A last selection gives the typical signal mt (same rank of max(med5,
 // 1e-4) over the set the last round kept), and the gain follows from the noise model (R21).
 #pragma once
+#include <cooperative_groups.h>
+
 #include "common.cuh"
 
 namespace lac {
@@ -135,13 +137,13 @@ __device__ __forceinline__ void sel_pick(SelState* st, uint32_t* hist, uint32_t*
         __syncthreads();
     }
     const uint32_t incl = scan[tid], excl = incl - sum, n = scan[255];
-    const uint32_t kth = PASS == 0 ? (n - 1u) / 2u : st->kth;
+    const uint32_t kth = PASS == 0 ? (n - 1u) / 2u : __ldcg(&st->kth);
     if (kth >= excl && kth < incl) {      // exactly one thread: the group that holds the rank
         uint32_t acc = excl;
         int i = 0;
         while (i < PER - 1 && acc + loc[i] <= kth) acc += loc[i++];
         const uint32_t digit = (uint32_t)(tid * PER + i);
-        const uint32_t prefix = PASS == 0 ? digit : PASS == 1 ? ((st->prefix << 11) | digit) : ((st->prefix << 10) | digit);
+        const uint32_t prefix = PASS == 0 ? digit : PASS == 1 ? ((__ldcg(&st->prefix) << 11) | digit) : ((__ldcg(&st->prefix) << 10) | digit);
         if (PASS == 0) st->n = n;
         st->kth = kth - acc;
         st->prefix = prefix;
@@ -152,23 +154,24 @@ __device__ __forceinline__ void sel_pick(SelState* st, uint32_t* hist, uint32_t*
             } else if (MODE == 1) {
                 const float s = __fmul_rn(1.4826f, v);
                 const float five_s = __fmul_rn(5.0f, s);
-                const float nlo = __fsub_rn(st->c, five_s), nhi = __fadd_rn(st->c, five_s);
+                const float cc = __ldcg(&st->c), olo = __ldcg(&st->lo), ohi = __ldcg(&st->hi);
+                const float nlo = __fsub_rn(cc, five_s), nhi = __fadd_rn(cc, five_s);
                 st->s = s;
                 if (!last) {   // the next round starts from the intersection
-                    st->lo = nlo > st->lo ? nlo : st->lo;
-                    st->hi = nhi < st->hi ? nhi : st->hi;
+                    st->lo = nlo > olo ? nlo : olo;
+                    st->hi = nhi < ohi ? nhi : ohi;
                 }
             } else {
                 // v = mt, the typical signal.  sigma^2 gain^2 - gain - rn^2/mt = 0, positive root, in the
                 // oracle's operation order
-                const float s = st->s;
+                const float s = __ldcg(&st->s);
                 const float s2 = __fmul_rn(s, s);
                 const float a = __fdiv_rn(__fmul_rn(__fmul_rn(4.0f, s2), rn2), v);
                 const float g = __fdiv_rn(__fadd_rn(1.0f, __fsqrt_rn(__fadd_rn(1.0f, a))), __fmul_rn(2.0f, s2));
                 const float INF = __int_as_float(0x7f800000);
                 *gain_out = (s > 0.0f && s < INF && g > 0.0f && g < INF) ? g : 1.0f;
                 if (stats) {
-                    stats[0] = st->c; stats[1] = s; stats[2] = st->lo; stats[3] = st->hi; stats[4] = (float)st->n;
+                    stats[0] = __ldcg(&st->c); stats[1] = s; stats[2] = __ldcg(&st->lo); stats[3] = __ldcg(&st->hi); stats[4] = (float)__ldcg(&st->n);
                     stats[5] = v;
                 }
             }
@@ -179,31 +182,25 @@ __device__ __forceinline__ void sel_pick(SelState* st, uint32_t* hist, uint32_t*
 
 // MODE 0: value = r; MODE 1: value = |r - c|; MODE 2: value = max(med5, 1e-4) (plane M5), all over the kept
 // set lo <= r <= hi.  PASS 0/1/2: key bits 31..21 / 20..10 / 9..0.
+// sh: SEL_BINS words of shared memory; fast (MODE 2 only): the three rounds were resolved on the zone lists
+// (selectz.cuh) and the typical signal is selected over ALL pixels of the med5 plane minus the listed pixels outside
+// the kept interval (every such pixel is in the OUT list), so that the residual plane is not read again.
 template <int MODE, int PASS>
-__global__ void __launch_bounds__(256)
-k_sel_hist(const float* __restrict__ R, const float* __restrict__ M5, size_t npx, SelState* st, uint32_t* hist,
-           int last, float rn2, float* gain_out, float* stats, const int* prev_count, const uint32_t* zdone,
-           const uint32_t* zno, const float2* __restrict__ olist) {
-    if (prev_count && *prev_count == 0) {          // fixed point (R17): same image, same estimate
-        if (MODE == 2 && PASS == 2 && blockIdx.x == 0 && threadIdx.x == 0) *gain_out = gain_out[-1];
-        return;
-    }
-    // selectz.cuh: the three rounds were resolved on the zone lists.  The passes over r and |r - c| then have
-    // nothing to do, and the typical signal is selected over ALL pixels of the med5 plane minus the listed pixels
-    // outside the kept interval (every such pixel is in the OUT list), so that the residual plane is not read again.
-    const bool fast = zdone && *zdone;
-    if (MODE != 2 && fast) return;
-    __shared__ uint32_t sh[SEL_BINS];
+__device__ __forceinline__ void sel_hist_pass(const float* __restrict__ R, const float* __restrict__ M5, size_t npx, SelState* st,
+                                              uint32_t* hist, int last, float rn2, float* gain_out, float* stats, bool fast,
+                                              const uint32_t* zno, const float2* __restrict__ olist, uint32_t* sh) {
     for (int i = threadIdx.x; i < SEL_BINS; i += 256) sh[i] = 0;
     __syncthreads();
-    const float lo = st->lo, hi = st->hi, c = st->c;
+    // (the state is read past the L1: inside k_sel_rounds it was written by another CTA of the same launch)
+    const float lo = __ldcg(&st->lo), hi = __ldcg(&st->hi), c = __ldcg(&st->c);
+    const uint32_t st_prefix = __ldcg(&st->prefix);
     // keys under the digits already fixed form one range; MODE 0 intersects it with the kept interval, which
     // is a key range too (the key is monotone), so a value costs one key and one unsigned range check
     constexpr int SHIFT = PASS == 0 ? 21 : PASS == 1 ? 10 : 0;
     constexpr uint32_t MASK = PASS == 2 ? 0x3ffu : 0x7ffu;
     uint32_t klo = 0u, khi = 0xffffffffu;
-    if (PASS == 1) { klo = st->prefix << 21; khi = klo | 0x1fffffu; }
-    if (PASS == 2) { klo = st->prefix << 10; khi = klo | 0x3ffu; }
+    if (PASS == 1) { klo = st_prefix << 21; khi = klo | 0x1fffffu; }
+    if (PASS == 2) { klo = st_prefix << 10; khi = klo | 0x3ffu; }
     if (MODE == 0) {
         klo = max(klo, sel_key(lo));
         khi = min(khi, sel_key(hi));
@@ -271,6 +268,43 @@ k_sel_hist(const float* __restrict__ R, const float* __restrict__ M5, size_t npx
     __threadfence();
     sel_pick<MODE, PASS>(st, hist, sh, last, rn2, gain_out, stats);
     if (threadIdx.x == 0) st->ticket = 0;
+}
+
+// one pass as a launch (the typical signal: MODE 2)
+template <int MODE, int PASS>
+__global__ void __launch_bounds__(256)
+k_sel_hist(const float* __restrict__ R, const float* __restrict__ M5, size_t npx, SelState* st, uint32_t* hist,
+           int last, float rn2, float* gain_out, float* stats, const int* prev_count, const uint32_t* zdone,
+           const uint32_t* zno, const float2* __restrict__ olist) {
+    if (prev_count && *prev_count == 0) {          // fixed point (R17): same image, same estimate
+        if (MODE == 2 && PASS == 2 && blockIdx.x == 0 && threadIdx.x == 0) *gain_out = gain_out[-1];
+        return;
+    }
+    const bool fast = zdone && *zdone;
+    if (MODE != 2 && fast) return;
+    __shared__ uint32_t sh[SEL_BINS];
+    sel_hist_pass<MODE, PASS>(R, M5, npx, st, hist, last, rn2, gain_out, stats, fast, zno, olist, sh);
+}
+
+// The three clipping rounds by radix passes over the plane, as ONE cooperative launch (grid barriers between the
+// eighteen passes): the path of the frames the fast path of selectz.cuh does not fit.  Returns at once when that
+// path has resolved the rounds, which is why it is one launch and not eighteen.
+__global__ void __launch_bounds__(256)
+k_sel_rounds(const float* __restrict__ R, size_t npx, SelState* st, uint32_t* hist, const int* prev_count,
+             const uint32_t* zdone) {
+    if (prev_count && *prev_count == 0) return;
+    if (zdone && *zdone) return;
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    __shared__ uint32_t sh[SEL_BINS];
+    for (int j = 0; j < SEL_ROUNDS; ++j) {
+        const int last = j == SEL_ROUNDS - 1;
+        sel_hist_pass<0, 0>(R, nullptr, npx, st, hist, 0, 0.0f, nullptr, nullptr, false, nullptr, nullptr, sh); grid.sync();
+        sel_hist_pass<0, 1>(R, nullptr, npx, st, hist, 0, 0.0f, nullptr, nullptr, false, nullptr, nullptr, sh); grid.sync();
+        sel_hist_pass<0, 2>(R, nullptr, npx, st, hist, 0, 0.0f, nullptr, nullptr, false, nullptr, nullptr, sh); grid.sync();
+        sel_hist_pass<1, 0>(R, nullptr, npx, st, hist, 0, 0.0f, nullptr, nullptr, false, nullptr, nullptr, sh); grid.sync();
+        sel_hist_pass<1, 1>(R, nullptr, npx, st, hist, 0, 0.0f, nullptr, nullptr, false, nullptr, nullptr, sh); grid.sync();
+        sel_hist_pass<1, 2>(R, nullptr, npx, st, hist, last, 0.0f, nullptr, nullptr, false, nullptr, nullptr, sh); grid.sync();
+    }
 }
 
 }  // namespace lac
