@@ -177,8 +177,8 @@ constexpr int UW = 32, UH = 8;
 
 // sm: work tile with margins (NS_MX, NS_MY), edge-replicated
 // W4: w % 4 == 0 and 16-byte aligned planes (the TMA path): quads are whole and every store is one vector
-// CFG >= 0: the nullable outputs are known at compile time (bit 0: copy_out, bit 1: A1 / A2, bit 2: mask_zero; no debug
-// plane, no residual plane, no device-side gain), which takes their tests out of the unit loop; CFG < 0: decided at run time.
+// CFG >= 0: the nullable outputs are known at compile time (bit 0: copy_out, bit 1: A1 / A2, bit 2: mask_zero, bit 3: the
+// residual plane of the gain estimate instead of S; no debug plane, no device-side gain), which takes their tests out of the unit loop; CFG < 0: decided at run time.
 // The threshold tests and their packing run on the FMA pipe: for finite a, b the sign of fsub(a, b) is set iff a < b
 // (a difference of two floats never rounds to zero unless they are equal: gradual underflow), so
 // (s > thr) = sign(thr - s), (c < satlevel) = sign(c - satlevel), and the nibble is a sum of sign bits times 2^j.
@@ -189,7 +189,11 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
     const bool has_copy = CFG < 0 ? a.copy_out != nullptr : (CFG & 1) != 0;
     const bool has_A = CFG < 0 ? a.A1 != nullptr : (CFG & 2) != 0;
     const bool has_mz = CFG < 0 ? a.mask_zero != nullptr : (CFG & 4) != 0;
-    const bool has_lp = CFG < 0 && a.dbgLp != nullptr, has_n = CFG < 0 && a.dbgN != nullptr, has_R = CFG < 0 && a.R != nullptr;
+    const bool has_lp = CFG < 0 && a.dbgLp != nullptr, has_n = CFG < 0 && a.dbgN != nullptr;
+    const bool has_R = CFG < 0 ? a.R != nullptr : (CFG & 8) != 0;
+    // CFG 8 / 9: the residual pass of the gain estimate (R21) -- med5 and the residual are all it writes, so L+, N, S and
+    // the threshold tests are not computed at all
+    constexpr bool ONLY_R = CFG >= 0 && (CFG & 8) != 0;
     const float gain = (CFG < 0 && a.gain_dev) ? __ldg(a.gain_dev) : a.gain;
     static_assert((TW / UW) * (NS_TH / UH) <= NWARP || NS_TH % UH == 0, "units must tile the tile");
 #pragma unroll 1
@@ -206,6 +210,7 @@ __device__ __forceinline__ void noise_S_tile(const float* sm, const NoiseArgs& a
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 ctr[j] = win[2 + j][2];
+                if (ONLY_R) continue;
                 lp[j] = lplus_px(win[2 + j][2], win[2 + j][1], win[2 + j][3], win[1 + j][2], win[3 + j][2]);
                 n[j] = noise_px(m5[j], gain, a.rn2);
                 s[j] = fdiv_nn(lp[j], __fmul_rn(2.0f, n[j]));

@@ -124,7 +124,9 @@ DeviceInfo device_info() {
     if (cudaFuncSetAttribute(lac::k_noise_S_tma<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(lac::k_noise_S_tma<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess ||
         cudaFuncSetAttribute(lac::k_noise_S_tma<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess ||
-        cudaFuncSetAttribute(lac::k_noise_S_tma<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess)
+        cudaFuncSetAttribute(lac::k_noise_S_tma<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(lac::k_noise_S_tma<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess ||
+        cudaFuncSetAttribute(lac::k_noise_S_tma<9>, cudaFuncAttributeMaxDynamicSharedMemorySize, lac::NS_SMEM_BYTES) != cudaSuccess)
         return d;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_fine, lac::k_fine_gates_tma, lac::NT,
                                                       lac::FG_SMEM_BYTES) != cudaSuccess) return d;
@@ -435,6 +437,8 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                 if (plain && na.copy_out && na.A1 && na.mask_zero) lac::k_noise_S_tma<7><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
                 else if (plain && na.copy_out && na.A1 && !na.mask_zero) lac::k_noise_S_tma<3><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
                 else if (plain && !na.copy_out && !na.A1 && !na.mask_zero) lac::k_noise_S_tma<0><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
+                else if (na.R && !na.dbgLp && !na.dbgN && !na.gain_dev && !na.A1 && !na.mask_zero && !na.var && na.copy_out) lac::k_noise_S_tma<9><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
+                else if (na.R && !na.dbgLp && !na.dbgN && !na.gain_dev && !na.A1 && !na.mask_zero && !na.var && !na.copy_out) lac::k_noise_S_tma<8><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
                 else lac::k_noise_S_tma<-1><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
             }
             else lac::k_noise_S<<<ntilesNS, tb, 0, st>>>(from, na, ntx, prev);
