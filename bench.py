@@ -320,16 +320,28 @@ def run_cuda(args):
                                 want_gains=True)
         torch.cuda.synchronize()
         nsel = max(kt_est["gain_select"][1], 1)
-        # one estimate = 18 histogram passes over the residual plane (4 B/px) + 3 over residual and med5 (8 B/px)
         sel_ms = kt_est["gain_select"][0] / nsel
+        zi = lc.lacosmic_gain_zone_info(ws, h, w)
+        fast = bool(zi[24])
+        # bytes one estimate has to read: fast path (csrc/selectz.cuh) = the residual plane twice (bucket counts, then the
+        # zones' values) + the med5 plane three times (radix passes of the typical signal); plane path (csrc/select.cuh) =
+        # 18 passes over the residual plane + 3 over residual and med5
+        sel_bytes = (2 * 4 + 3 * 4 if fast else 18 * 4 + 3 * 8) * npx
         gain_est = dict(frames_per_s=world * 1e3 / ms_est, ms_per_step=ms_est,
                         gains=[float(v) for v in ge["gains"].cpu().numpy()],
                         new_cr_per_iteration=counts.cpu().numpy().tolist(),
                         select_ms_per_estimate=sel_ms,
-                        select_hbm_gbs=96 * npx / (sel_ms * 1e-3) / 1e9,
-                        select_hbm_frac=96 * npx / (sel_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                        note="gain = 0: residual plane + (3 rounds x 2 + 1) selections x 3 radix passes per iteration, "
-                             "then every plane recomputed with the estimated gain (no incremental iterations)")
+                        select_path="zone lists (two reads of the residual plane)" if fast else "radix passes over the plane",
+                        select_lists=dict(z0=int(zi[18]), z_minus_plus=int(zi[19]), out=int(zi[20]), zeros_counted=int(zi[26]),
+                                          buckets=dict(z0=[int(zi[2]), int(zi[3])], z_minus=[int(zi[4]), int(zi[5])],
+                                                       z_plus=[int(zi[6]), int(zi[7])], out_minus_upto=int(zi[8]),
+                                                       out_plus_from=int(zi[9]))),
+                        select_bytes_per_px=sel_bytes / npx,
+                        select_hbm_gbs=sel_bytes / (sel_ms * 1e-3) / 1e9,
+                        select_hbm_frac=sel_bytes / (sel_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                        note="gain = 0 (DESIGN.md R21, section 5.3): per iteration one residual pass, the sigma clipping "
+                             "(last estimate of the frame shown), then every plane recomputed with the estimated gain "
+                             "(no incremental iterations)")
 
     # ---- configs[3] in small: a stream of independent frames with per-frame parameters, resident in HBM,
     # through lacosmic_run_batch, back to back (concurrency 1) and with several frames in flight
