@@ -130,6 +130,14 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
     // (predicated loads: the address is never formed into an access there)
     const int base = (ya - 4) * wpr + wx;
     auto rowok = [&](int j) -> bool { return colok && (unsigned)(ya - 4 + j) < (unsigned)h; };
+    // one pointer per plane at the strip's first register row, one offset per row shared by all planes (half of this
+    // kernel's instructions used to be 64-bit address arithmetic, one chain per access)
+    const uint32_t *const pM1 = a.M1 + base, *const pG1 = a.G1 + base, *const pCo = a.Cold + base;
+    const uint32_t *const pA1 = a.A1 ? a.A1 + base : nullptr, *const pA2 = a.A2 ? a.A2 + base : nullptr;
+    uint32_t *const pG2 = a.G2 + base, *const pG2F = a.G2F + base, *const pCn = a.Cnew + base, *const pNE = a.NEED + base;
+    int ro[WG_J];
+#pragma unroll
+    for (int j = 0; j < WG_J; ++j) ro[j] = j * wpr;
     auto qof = [&](int j) -> int { return base + j * wpr; };
     const int pc = prev_count ? *prev_count : 1;             // tested below, after the M1 loads have been issued
     const bool lazy = a.A2 != nullptr;
@@ -141,22 +149,22 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
     bool anym1 = false;
 #pragma unroll
     for (int j = 0; j < WG_J; ++j) {
-        m1[j] = rowok(j) ? a.M1[qof(j)] : 0u;
+        m1[j] = rowok(j) ? pM1[ro[j]] : 0u;
         anym1 |= m1[j] != 0;
     }
     if (pc == 0) {
         // fixed point (R17): nothing changes; carry C over to the plane the next reader expects
 #pragma unroll
         for (int j = 4; j < 4 + WG_R; ++j)
-            if (own && ya - 4 + j < h) a.Cnew[qof(j)] = a.Cold[qof(j)];
+            if (own && ya - 4 + j < h) pCn[ro[j]] = pCo[ro[j]];
         return;
     }
     if (a.incremental && !__any_sync(FULL, anym1)) {
 #pragma unroll
         for (int j = 4; j < 4 + WG_R; ++j)
             if (own && ya - 4 + j < h) {
-                a.Cnew[qof(j)] = a.Cold[qof(j)];
-                a.NEED[qof(j)] = 0u;
+                pCn[ro[j]] = pCo[ro[j]];
+                pNE[ro[j]] = 0u;
             }
         return;
     }
@@ -168,12 +176,12 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
 #pragma unroll
         for (int j = 1; j < WG_J - 1; ++j) {
             const bool ok = rowok(j);
-            const int q = qof(j);
-            g1[j] = ok ? a.G1[q] : 0u;
+            const int q = ro[j];
+            g1[j] = ok ? pG1[q] : 0u;
             if (j >= 2 && j < WG_J - 2) {
-                g2[j] = ok ? a.G2[q] : 0u;
-                cold[j] = ok ? a.Cold[q] : 0u;
-                nbm[j] = (lazy && ok) ? (a.A2[q] & ~a.A1[q] & ~a.G2F[q]) : 0u;
+                g2[j] = ok ? pG2[q] : 0u;
+                cold[j] = ok ? pCo[q] : 0u;
+                nbm[j] = (lazy && ok) ? (pA2[q] & ~pA1[q] & ~pG2F[q]) : 0u;
             }
         }
         // ---- M2 = dil3(M1) & G1, rows 1 .. WG_J-2
@@ -223,8 +231,8 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
 #pragma unroll
             for (int j = 4; j < 4 + WG_R; ++j)
                 if (nb[j] && own && ya - 4 + j < h) {
-                    a.G2[qof(j)] = g2[j];
-                    a.G2F[qof(j)] |= nb[j] & ~g2[j];
+                    pG2[ro[j]] = g2[j];
+                    pG2F[ro[j]] |= nb[j] & ~g2[j];
                 }
         }
     }
@@ -239,7 +247,7 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
         cn[j] = cold[j] | m3;
         anyfresh |= fresh[j] != 0;
         if (j >= 4 && j < 4 + WG_R && own && ya - 4 + j < h) {
-            a.Cnew[qof(j)] = cn[j];
+            pCn[ro[j]] = cn[j];
             if (a.M2out) a.M2out[qof(j)] = m2[j];
             if (a.M3out) a.M3out[qof(j)] = m3;
             nfresh += __popc(fresh[j]);
@@ -261,7 +269,7 @@ k_grow_replace(GrowArgs a, const int* prev_count) {
     }
 #pragma unroll
     for (int j = 4; j < 4 + WG_R; ++j)
-        if (own && ya - 4 + j < h) a.NEED[qof(j)] = need[j];
+        if (own && ya - 4 + j < h) pNE[ro[j]] = need[j];
     bool anyneed = false;
 #pragma unroll
     for (int j = 4; j < 4 + WG_R; ++j) anyneed |= need[j] != 0;
@@ -380,11 +388,17 @@ k_dirty_lists(const uint32_t* __restrict__ NEED, const uint32_t* __restrict__ A1
     const bool colok = wx >= 0 && wx < wpr;
     const bool own = lane >= 1 && lane <= WG_OWN && colok;
     const int base = (ya - 4) * wpr + wx;           // word (row ya - 4 + j, this lane's column) = base + j * wpr
+    // one pointer per plane at the strip's first register row, one offset per row shared by all planes
+    const uint32_t *const pNE = NEED + base, *const pA1 = A1 + base;
+    uint32_t *const pG1 = G1 + base, *const pG2 = G2 + base, *const pG2F = G2F + base, *const pM1 = M1 + base;
+    int ro[WG_J];
+#pragma unroll
+    for (int j = 0; j < WG_J; ++j) ro[j] = j * wpr;
     uint32_t h2[WG_J], h4[WG_J];
     bool any = false;
 #pragma unroll
     for (int j = 0; j < WG_J; ++j) {
-        h2[j] = (colok && (unsigned)(ya - 4 + j) < (unsigned)h) ? NEED[base + j * wpr] : 0u;
+        h2[j] = (colok && (unsigned)(ya - 4 + j) < (unsigned)h) ? pNE[ro[j]] : 0u;
         any |= h2[j] != 0;
     }
     if (pc == 0 || !__any_sync(FULL, any)) return;            // fixed point (R17), or nothing was rewritten near this strip
@@ -431,20 +445,20 @@ k_dirty_lists(const uint32_t* __restrict__ NEED, const uint32_t* __restrict__ A1
 #pragma unroll
     for (int k = 0; k < WG_R; ++k) {
         const bool rd = Rr[k] != 0;
-        const int q = base + (4 + k) * wpr;
-        a1[k] = rd ? A1[q] : 0u; g1[k] = rd ? G1[q] : 0u; g2[k] = rd ? G2[q] : 0u;
-        g2f[k] = rd ? G2F[q] : 0u; m1[k] = rd ? M1[q] : 0u;
+        const int q = ro[4 + k];
+        a1[k] = rd ? pA1[q] : 0u; g1[k] = rd ? pG1[q] : 0u; g2[k] = rd ? pG2[q] : 0u;
+        g2f[k] = rd ? pG2F[q] : 0u; m1[k] = rd ? pM1[q] : 0u;
     }
 #pragma unroll
     for (int k = 0; k < WG_R; ++k) {
         const uint32_t R = Rr[k];
         if (R) {
-            const int q = base + (4 + k) * wpr;
+            const int q = ro[4 + k];
             cand[k + 4] = a1[k] & R & ~dqr[k];
-            if (g1[k] & R) G1[q] = g1[k] & ~R;
-            if (g2[k] & R) G2[q] = g2[k] & ~R;
-            if (g2f[k] & R) G2F[q] = g2f[k] & ~R;
-            if (m1[k] & R) M1[q] = m1[k] & ~R;
+            if (g1[k] & R) pG1[q] = g1[k] & ~R;
+            if (g2[k] & R) pG2[q] = g2[k] & ~R;
+            if (g2f[k] & R) pG2F[q] = g2f[k] & ~R;
+            if (m1[k] & R) pM1[q] = m1[k] & ~R;
         }
     }
     const int p0 = ya * w + wx * 32;
