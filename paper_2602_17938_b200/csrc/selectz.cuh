@@ -10,13 +10,13 @@
 //                   the clipping bounds -- wide enough to hold every value a round can select or compare with.
 //   k_selz_compact  read 2: the residuals of Z0 go to one list (1-2 % of the plane), those of Z- and Z+ to a second
 //                   one (about 5 %), those of OUT- and OUT+ to a third one together with their med5 (about 2 %).
-//   k_selz_resolve  one cluster of 8 CTAs runs the three rounds EXACTLY on the lists: the pixels outside the
+//   k_selz_resolve  one cluster of 16 CTAs runs the three rounds EXACTLY on the lists: the pixels outside the
 //                   zones only enter through their counts, which the histogram holds exactly; every selection is
 //                   a radix selection over a list.  Every step checks that what it selected lies inside its zone
 //                   (the first and last floats of a bucket are found by bisection on the bucket function, so the
 //                   bounds are exact): if a check fails -- a frame of few distinct values, a plan that missed -- the
-//                   state says so and the radix passes of select.cuh, which are launched behind this kernel and
-//                   otherwise return at once, do the estimate over the plane.
+//                   state says so and k_sel_rounds (select.cuh: the eighteen radix passes as one cooperative launch,
+//                   which otherwise returns at once) does the rounds over the plane.
 // The typical signal (rank (n-1)/2 of max(med5, 1e-4) over the kept set) then takes the three radix passes of
 // select.cuh over the med5 plane alone: the pixels outside the kept interval are all in the OUT list, whose
 // entries are subtracted from the histograms.
