@@ -60,6 +60,8 @@ struct SelZone {
     uint32_t why;                             // diagnostic: where the fast path stopped (0 = it did not)
     uint32_t nzero;                           // residuals that are exactly +0 (a pixel that is the median of its own window:
                                               // 4 % of a frame).  Inside Z0 they are counted, not listed.
+    uint32_t nneg0;                           // negative residuals in the bucket of 0: when a centre's rank inside that bucket
+                                              // falls on the zeros, the centre is +0 without a selection (the usual case)
 };
 
 // capacities of the four lists inside `words` 32-bit words of storage
@@ -155,7 +157,7 @@ k_selz_init(const float* __restrict__ R, size_t npx, SelState* st, SelZone* zn, 
         z.ok = (!force_classic && nv > 0 && s0 > 0.0f && s0 < INF && scale > 0.0f && scale < INF && fabsf(base) < INF) ? 1u : 0u;
         z.done = 0;
         z.why = z.ok ? 0u : 1u;                             // 1: switched off, or no usable bucket grid
-        z.nzero = 0;
+        z.nzero = z.nneg0 = 0;
         *zn = z;
     }
 }
@@ -205,6 +207,7 @@ __device__ void selz_plan(const uint32_t* cum, SelZone* zn, SelzLists cap) {
     }
     SelZone z = *zn;
     z.nzero = __ldcg(&zn->nzero);             // (summed by the other CTAs; this CTA's L1 may hold the line from before)
+    z.nneg0 = __ldcg(&zn->nneg0);
     if (ok) {
         const int mo = 10 + (int)(0.03f * extmin);
         z.z0lo = bmin - 3; z.z0hi = bmax + 3;
@@ -244,15 +247,23 @@ k_selz_hist(const float* __restrict__ R, size_t npx, SelState* st, SelZone* zn, 
     for (int i = threadIdx.x; i < SELZ_NB; i += SELZ_HT) sh[i] = 0;
     __syncthreads();
     const float base = zn->base, scale = zn->scale;
-    uint32_t nzero = 0;
+    const int bzero = selz_bucket(0.0f, base, scale);
+    uint32_t nzero = 0, nneg0 = 0;
     sel_visit_plane<false, SELZ_HT>(R, nullptr, npx, [&](float r, float, bool ok, size_t) {
         if (ok) {
-            atomicAdd(&sh[selz_bucket(r, base, scale)], 1u);
-            if (__float_as_uint(r) == 0u) ++nzero;
+            const int b = selz_bucket(r, base, scale);
+            atomicAdd(&sh[b], 1u);
+            if (b == bzero) {
+                const uint32_t u = __float_as_uint(r);
+                nzero += u == 0u ? 1u : 0u;
+                nneg0 += u >> 31;
+            }
         }
     });
     nzero = __reduce_add_sync(0xffffffffu, nzero);
+    nneg0 = __reduce_add_sync(0xffffffffu, nneg0);
     if ((threadIdx.x & 31) == 0 && nzero) atomicAdd(&zn->nzero, nzero);
+    if ((threadIdx.x & 31) == 0 && nneg0) atomicAdd(&zn->nneg0, nneg0);
     __syncthreads();
     for (int i = threadIdx.x; i < SELZ_NB; i += SELZ_HT)
         if (sh[i]) atomicAdd(&histz[i], sh[i]);
@@ -660,13 +671,17 @@ k_selz_resolve(SelState* st, SelZone* zn, const uint32_t* __restrict__ histz, vo
             if (g < acc + hq) break;
             acc += hq;
         }
-        __syncthreads();
-        if (threadIdx.x < 2) sm->edge[6 + threadIdx.x] = selz_edge_key(bq + threadIdx.x, base, scale);
-        __syncthreads();
-        const uint32_t kclo = sm->edge[6], kchi = sm->edge[7] - 1u;
-        const uint32_t kc = selz_select(cl, sm, L.z0, n0, kclo, kchi, g - acc, L.scr, L.capscr, zn->nscr, 0x80000000u, vzero,
-                                        par, cpar, [&](float r) -> uint32_t { return sel_key(r); });
-        c = sel_unkey(kc);
+        if (vzero && bq == bzero && g - acc >= z.nneg0 && g - acc - z.nneg0 < vzero) {
+            c = 0.0f;                                    // the rank falls on the residuals +0 of that bucket
+        } else {
+            __syncthreads();
+            if (threadIdx.x < 2) sm->edge[6 + threadIdx.x] = selz_edge_key(bq + threadIdx.x, base, scale);
+            __syncthreads();
+            const uint32_t kclo = sm->edge[6], kchi = sm->edge[7] - 1u;
+            const uint32_t kc = selz_select(cl, sm, L.z0, n0, kclo, kchi, g - acc, L.scr, L.capscr, zn->nscr, 0x80000000u, vzero,
+                                            par, cpar, [&](float r) -> uint32_t { return sel_key(r); });
+            c = sel_unkey(kc);
+        }
         // MAD: rank k of |r - c| over the kept set.  With c between Z- and Z+, every value between them is at
         // most vin away from c and every kept value beyond them at least vout; if the element of rank k - inner of
         // V = { |r - c| : r in Z- or Z+ } lies in [vin, vout], it is the element of rank k of all.

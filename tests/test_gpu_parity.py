@@ -459,7 +459,7 @@ def test_estimate_gain_ties_and_degenerate(lc, orc):
         assert _n(g)[0] == go and np.array_equal(_n(st), sto)
 
 
-@pytest.mark.parametrize("kind", ["frame", "integer", "gain4", "gain0p2", "skewed", "coarse"])
+@pytest.mark.parametrize("kind", ["frame", "integer", "gain4", "gain0p2", "skewed", "skewed_low", "coarse"])
 def test_estimate_gain_fast_path_equals_oracle_and_plane_path(lc, orc, kind):
     """The fast path of the estimate (two reads of the residual plane, rounds resolved on zone lists, csrc/selectz.cuh)
     and the radix passes over the plane (csrc/select.cuh) give the oracle's bits; on frames like the paper's the fast
@@ -477,6 +477,9 @@ def test_estimate_gain_fast_path_equals_oracle_and_plane_path(lc, orc, kind):
     elif kind == "skewed":             # 8 % of the pixels far above the rest: the centre moves between the rounds
         x = (200.0 + 12.0 * rng.standard_normal((600, 700))).astype(np.float32)
         x.flat[rng.integers(0, x.size, x.size // 12)] += rng.uniform(100.0, 3000.0, x.size // 12).astype(np.float32)
+    elif kind == "skewed_low":         # the same below the rest: the centres are negative (and never the residual 0)
+        x = (2000.0 + 12.0 * rng.standard_normal((600, 700))).astype(np.float32)
+        x.flat[rng.integers(0, x.size, x.size // 9)] -= rng.uniform(100.0, 1500.0, x.size // 9).astype(np.float32)
     else:                              # 16 distinct values only
         x = (100.0 + 4.0 * rng.integers(0, 16, (500, 640))).astype(np.float32)
     go, sto = orc.estimate_gain(x, 6.0)
@@ -492,7 +495,7 @@ def test_estimate_gain_fast_path_equals_oracle_and_plane_path(lc, orc, kind):
     finally:
         lc.lacosmic_gain_fast_path_enable(True)
     assert paths[False] == 0.0
-    print("estimate_gain[%s]: fast path taken = %s" % (kind, paths[True]))
+    print("estimate_gain[%s]: fast path taken = %s, centre %r" % (kind, paths[True], float(sto[0])))
     if kind in ("frame", "gain4", "gain0p2"):
         assert paths[True] == 1.0, kind
 
