@@ -362,16 +362,16 @@ k_selz_compact(const float* __restrict__ R, const float* __restrict__ M5, size_t
             const float4 q = okv[u] ? __ldg(reinterpret_cast<const float4*>(R) + i) : make_float4(0.f, 0.f, 0.f, 0.f);
             v[4 * u] = q.x; v[4 * u + 1] = q.y; v[4 * u + 2] = q.z; v[4 * u + 3] = q.w;
         }
-        uint32_t codes = 0, c0 = 0, c1 = 0, co = 0;   // 2 bits per value: its list; entries of this thread per list
+        uint32_t codes = 0;                   // 2 bits per value: its list
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
             uint32_t cls = okv[e >> 2] ? s_cls[selz_bucket(v[e], base, scale)] : 0u;
             if (cls == 1 && __float_as_uint(v[e]) == 0u) cls = 0;
             codes |= cls << (2 * e);
-            c0 += cls == 1 ? 1u : 0u;
-            c1 += cls == 2 ? 1u : 0u;
-            co += cls == 3 ? 1u : 0u;
         }
+        // entries of this thread per list: fields equal to 1, 2, 3
+        const uint32_t lo1 = codes & 0x55555555u, hi1 = (codes >> 1) & 0x55555555u;
+        const uint32_t c0 = __popc(lo1 & ~hi1), c1 = __popc(hi1 & ~lo1), co = __popc(lo1 & hi1);
         if (__ballot_sync(0xffffffffu, codes != 0u) == 0) continue;
         // inclusive prefix sums over the warp (at most 16 x 32 = 512 entries per list: two lists share a word)
         const uint32_t own_a = c0 | (c1 << 16), own_b = co;
