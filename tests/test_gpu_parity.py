@@ -570,6 +570,25 @@ def test_whole_path_with_estimated_gain(lc, orc, cfg, mode):
     assert np.all(_n(g1["gains"]) == np.float32(PARAMS["gain"]))
 
 
+def test_estimated_gain_on_config2_whole_frame(lc, orc):
+    """The bench workload with no gain supplied (configs[2], 4000 x 6500): per-iteration gains, counts, mask and cleaned frame
+    equal the oracle's over every pixel, and the clipping rounds of the last estimate ran on the zone lists (about two
+    minutes of oracle time: four estimates of seven full sorts each)."""
+    import torch
+    f = synth.make_config(2)
+    p = dict(PARAMS, gain=0.0)
+    o = orc.run(f.img, **p)
+    h, w = f.img.shape
+    ws = torch.empty(lc.lacosmic_workspace_bytes(h, w), dtype=torch.uint8, device="cuda")
+    g = lc.lacosmic_run_ws(_t(f.img), lc.Params(**p), workspace=ws, want_gains=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(_n(g["gains"]), o["gains"]), (_n(g["gains"]), o["gains"])
+    assert np.array_equal(_n(g["counts"])[:4], o["counts"])
+    assert np.array_equal(_n(g["mask"]), o["mask"]) and np.array_equal(_n(g["clean"]), o["clean"])
+    zi = lc.lacosmic_gain_zone_info(ws, h, w)
+    assert zi[23] == 1 and zi[24] == 1 and zi[25] == 0, zi[18:28]
+
+
 def test_estimated_gain_on_config0(lc, orc):
     import torch
     f = synth.make_config(0)
