@@ -779,6 +779,33 @@ def test_repeated_call_replays_from_library_graph(lc, orc):
     lc.lacosmic_graph_replay_enable(True)
 
 
+def test_repeated_call_with_estimated_gain_replays_from_library_graph(lc, orc):
+    """The same with no gain supplied: the captured sequence then holds the estimate's cluster launch (k_selz_resolve) and
+    cooperative launch (k_sel_rounds); frame contents change between the replays."""
+    import torch
+    frames = [synth.make_frame(220, 300, seed=170 + k, n_star=15, n_cr=100 + 40 * k, n_hot=30, sp_frac=0.004) for k in range(3)]
+    p = dict(PARAMS, gain=0.0)
+    oracle = [orc.run(f.img, **p) for f in frames]
+    h, w = frames[0].img.shape
+    s = torch.cuda.Stream()
+    img = torch.empty((h, w), dtype=torch.float32, device="cuda")
+    mask = torch.empty((h, w), dtype=torch.uint8, device="cuda")
+    clean = torch.empty_like(img)
+    ws = torch.empty(lc.lacosmic_workspace_bytes(h, w), dtype=torch.uint8, device="cuda")
+    counts = torch.zeros(p["niter"], dtype=torch.int32, device="cuda")
+    P = lc.Params(**p)
+    with torch.cuda.stream(s):
+        for rep in range(6):                              # calls 0 direct, 1 captures, 2.. replay
+            k = rep % len(frames)
+            img.copy_(_t(frames[k].img))
+            mask.fill_(7); clean.fill_(-1.0); counts.fill_(-3)
+            lc.lacosmic_run_ws(img, P, mask_out=mask, clean_out=clean, workspace=ws, iter_counts=counts, stream=s)
+            s.synchronize()
+            o = oracle[k]
+            assert np.array_equal(_n(mask), o["mask"]) and np.array_equal(_n(clean), o["clean"]), rep
+            assert np.array_equal(_n(counts), o["counts"]), rep
+
+
 def test_config3_stream_full_size(lc, orc):
     """configs[3] at full frame size, shortened to 8 frames (seeds 1000..1007, sigclip cycling 4.0/4.5/5.0 by
     seed: per-frame parameters): lacosmic_run_batch with 4 frames in flight, in the configuration bench.py's
