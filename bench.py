@@ -323,16 +323,20 @@ def run_cuda(args):
         sel_ms = kt_est["gain_select"][0] / nsel
         zi = lc.lacosmic_gain_zone_info(ws, h, w)
         fast = bool(zi[24])
-        # bytes one estimate has to read: fast path (csrc/selectz.cuh) = the residual plane twice (bucket counts, then the
-        # zones' values) + the med5 plane three times (radix passes of the typical signal); plane path (csrc/select.cuh) =
-        # 18 passes over the residual plane + 3 over residual and med5
-        sel_bytes = (2 * 4 + 3 * 4 if fast else 18 * 4 + 3 * 8) * npx
+        mfast = bool(zi[36])
+        # bytes one estimate has to read: fast path (csrc/selectz.cuh) = the residual and the med5 plane twice each (bucket
+        # counts, then the zones' values); if only the rounds ran on the lists, the residual plane twice + the med5 plane
+        # three times (radix passes of the typical signal); plane path (csrc/select.cuh) = 18 passes over the residual
+        # plane + 3 over residual and med5
+        sel_bytes = ((2 * 8 if mfast else 2 * 4 + 3 * 4) if fast else 18 * 4 + 3 * 8) * npx
         gain_est = dict(frames_per_s=world * 1e3 / ms_est, ms_per_step=ms_est,
                         gains=[float(v) for v in ge["gains"].cpu().numpy()],
                         new_cr_per_iteration=counts.cpu().numpy().tolist(),
                         select_ms_per_estimate=sel_ms,
-                        select_path="zone lists (two reads of the residual plane)" if fast else "radix passes over the plane",
+                        select_path=("zone lists (two reads of the residual and the med5 plane)" if mfast else
+                                     "zone lists for the rounds, radix passes for the typical signal") if fast else "radix passes over the planes",
                         select_lists=dict(z0=int(zi[18]), z_minus_plus=int(zi[19]), out=int(zi[20]), zeros_counted=int(zi[26]),
+                                          typical_signal=int(zi[34]),
                                           buckets=dict(z0=[int(zi[2]), int(zi[3])], z_minus=[int(zi[4]), int(zi[5])],
                                                        z_plus=[int(zi[6]), int(zi[7])], out_minus_upto=int(zi[8]),
                                                        out_plus_from=int(zi[9]))),

@@ -252,8 +252,10 @@ int lacosmic_estimate_gain(const float *img, int h, int w, float readnoise, floa
  *   OUT-, first of OUT+; 10 values below Z0; 11-13 values in Z0, Z-, Z+; 14 values between Z- and Z+; 15-16 values in
  *   OUT-, OUT+; 17 pixels; 18-22 list cursors; 23 plan made; 24 rounds resolved on the lists; 25 where the fast path
  *   stopped (0 it did not; 1 off / no grid; 2-4 plan; 10 j + 1..4: round j, bounds / centre / MAD rank / MAD); 26 the
- *   residuals that are exactly +0; 27 the negative residuals in the bucket of 0. */
-#define LACOSMIC_GAIN_ZONE_WORDS 32
+ *   residuals that are exactly +0; 27 the negative residuals in the bucket of 0; the typical signal: 28-29 base, scale of
+ *   its bucket grid (float bits); 30-31 bucket range of its zone; 32 values below the zone; 33 values in it; 34 list
+ *   cursor; 35 zone made; 36 selected on the list (0: by radix passes over the med5 plane). */
+#define LACOSMIC_GAIN_ZONE_WORDS 40
 int lacosmic_gain_zone_info(const void *workspace, int h, int w, int32_t *info_host, void *stream);
 
 /* Switches the fast path of the gain estimate on (default; environment LACOSMIC_GAIN_FAST=0 starts with it off)

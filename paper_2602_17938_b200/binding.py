@@ -534,10 +534,10 @@ def lacosmic_run_host_batch(imgs_host, params, masks_host=None, cleans_host=None
 
 # ----------------------------------------------------------------------------- single steps
 def lacosmic_gain_zone_info(workspace, h, w, stream=None):
-    """Diagnostic: the plan of the last gain estimate run in `workspace` as 32 int32 words (include/lacosmic.h)."""
+    """Diagnostic: the plan of the last gain estimate run in `workspace` as 40 int32 words (include/lacosmic.h)."""
     import numpy as np
     torch = _torch()
-    buf = np.zeros(32, np.int32)
+    buf = np.zeros(40, np.int32)
     _check(load_library().lacosmic_gain_zone_info(_dev(workspace, torch.uint8, "workspace"), int(h), int(w),
                                                   buf.ctypes.data, _stream(stream)), "lacosmic_gain_zone_info")
     return buf

@@ -178,7 +178,7 @@ struct Workspace {
     lac::SelState* sel; // radix selection state and histogram of the gain estimation (select.cuh)
     uint32_t* hist;
     lac::SelZone* zone; // fast path of the gain estimation (selectz.cuh): plan, bucket counts, zone id of every bucket
-    uint32_t* histz;
+    uint32_t *histz, *histm;
     size_t bytes;      // total
     size_t zero_off, zero_bytes;   // region cleared at the start of a frame: the counters
 };
@@ -207,6 +207,7 @@ Workspace carve(void* base, int h, int w) {
     ws.hist = (uint32_t*)(p + off); off += align_up(lac::SEL_BINS * 4, 256);
     ws.zone = (lac::SelZone*)(p + off); off += align_up(sizeof(lac::SelZone), 256);
     ws.histz = (uint32_t*)(p + off); off += align_up(lac::SELZ_NB * 4, 256);
+    ws.histm = (uint32_t*)(p + off); off += align_up(lac::SELZ_NB * 4, 256);
     ws.zero_bytes = off - ws.zero_off;
     ws.bytes = off;
     return ws;
@@ -252,14 +253,6 @@ bool gain_fast_enabled() {
     }
     return g_gain_fast == 1;
 }
-template <int MODE, int PASS>
-int sel_step(const float* R, const float* M5, size_t npx, const Workspace& ws, const float2* olist, int grid, int last,
-             float rn2, float* gain_out, float* stats, const int* prev, cudaStream_t st) {
-    lac::k_sel_hist<MODE, PASS><<<grid, 256, 0, st>>>(R, M5, npx, ws.sel, ws.hist, last, rn2, gain_out, stats, prev,
-                                                      &ws.zone->done, &ws.zone->no, olist);
-    LAUNCHED();
-    return LACOSMIC_OK;
-}
 int sigma_clip_gain(const float* R, const float* M5, size_t npx, const Workspace& ws, void* lists, size_t list_words,
                     float rn2, float* gain_out, float* stats, const int* prev, cudaStream_t st) {
     int dev = 0, sms = 148;
@@ -271,7 +264,7 @@ int sigma_clip_gain(const float* R, const float* M5, size_t npx, const Workspace
     const int grid = (int)std::min<size_t>((size_t)sms * LAC_SEL_CTAS_PER_SM, (npx / 4 + 255) / 256 + 1);
     // the lists of the fast path (selectz.cuh) live in the quad list's storage
     const float2* olist = lac::selz_carve(lists, list_words).o;
-    const int grid_h = (int)std::min<size_t>((size_t)sms * 2, (npx / 4 + 4 * lac::SELZ_HT - 1) / (4 * lac::SELZ_HT) + 1);
+    const int grid_h = (int)std::min<size_t>((size_t)sms, (npx / 4 + 4 * lac::SELZ_HT - 1) / (4 * lac::SELZ_HT) + 1);
     if (lac::SELZ_CLUSTER > 8) {              // once per device: clusters of 16 CTAs are a non-portable size
         static bool allowed[MAX_DEVICES] = {};
         if (dev >= 0 && dev < MAX_DEVICES && !allowed[dev]) {
@@ -280,19 +273,19 @@ int sigma_clip_gain(const float* R, const float* M5, size_t npx, const Workspace
         }
     }
     Span sp(KC_SELECT, st);
-    lac::k_selz_init<<<1, lac::SELZ_SAMPLE, 0, st>>>(R, npx, ws.sel, ws.zone, ws.hist, ws.histz, gain_fast_enabled() ? 0 : 1, prev);
+    lac::k_selz_init<<<1, lac::SELZ_IT, 0, st>>>(R, M5, npx, ws.sel, ws.zone, ws.hist, ws.histz, ws.histm,
+                                                     gain_fast_enabled() ? 0 : 1, prev);
     LAUNCHED();
-    lac::k_selz_hist<<<grid_h, lac::SELZ_HT, 0, st>>>(R, npx, ws.sel, ws.zone, ws.histz, lists, list_words, prev);
+    lac::k_selz_hist<<<grid_h, lac::SELZ_HT, 0, st>>>(R, M5, npx, ws.sel, ws.zone, ws.histz, ws.histm, lists, list_words, prev);
     LAUNCHED();
     lac::k_selz_compact<<<grid, 256, 0, st>>>(R, M5, npx, ws.zone, lists, list_words, prev);
     LAUNCHED();
-    lac::k_selz_resolve<<<lac::SELZ_CLUSTER, lac::SELZ_RT, 0, st>>>(ws.sel, ws.zone, ws.histz, lists, list_words,
-                                                                    stats ? stats + 6 : nullptr, prev);
+    lac::k_selz_resolve<<<lac::SELZ_CLUSTER, lac::SELZ_RT, 0, st>>>(ws.sel, ws.zone, ws.histz, lists, list_words, rn2, gain_out,
+                                                                    stats, prev);
     LAUNCHED();
-    int rc;
     {
-        // the rounds by radix passes over the plane: one cooperative launch, which returns at once when the fast path
-        // has resolved them.  Its grid must be resident as a whole.
+        // the selections by radix passes over the planes: one cooperative launch, which returns at once when the fast
+        // path has done them.  Its grid must be resident as a whole.
         static int per_sm[MAX_DEVICES] = {};
         if (dev < 0 || dev >= MAX_DEVICES) return LACOSMIC_ERR_CUDA;
         if (!per_sm[dev]) {
@@ -301,15 +294,12 @@ int sigma_clip_gain(const float* R, const float* M5, size_t npx, const Workspace
             per_sm[dev] = std::max(1, std::min(n, LAC_SEL_CTAS_PER_SM));
         }
         const int grid_c = std::min(grid, sms * per_sm[dev]);
-        const uint32_t* zdone = &ws.zone->done;
-        void* args[] = {(void*)&R, (void*)&npx, (void*)&ws.sel, (void*)&ws.hist, (void*)&prev, (void*)&zdone};
+        const uint32_t *zdone = &ws.zone->done, *zmdone = &ws.zone->mdone, *zno = &ws.zone->no;
+        void* args[] = {(void*)&R, (void*)&M5, (void*)&npx, (void*)&ws.sel, (void*)&ws.hist, (void*)&rn2, (void*)&gain_out,
+                        (void*)&stats, (void*)&prev, (void*)&zdone, (void*)&zmdone, (void*)&zno, (void*)&olist};
         CK(cudaLaunchCooperativeKernel((const void*)lac::k_sel_rounds, dim3((unsigned)grid_c), dim3(256), args, 0, st));
         LAUNCHED();
     }
-    // typical signal over the set the last round kept, then the gain
-    if ((rc = sel_step<2, 0>(R, M5, npx, ws, olist, grid, 1, rn2, gain_out, stats, prev, st))) return rc;
-    if ((rc = sel_step<2, 1>(R, M5, npx, ws, olist, grid, 1, rn2, gain_out, stats, prev, st))) return rc;
-    if ((rc = sel_step<2, 2>(R, M5, npx, ws, olist, grid, 1, rn2, gain_out, stats, prev, st))) return rc;
     return LACOSMIC_OK;
 }
 

@@ -270,41 +270,38 @@ __device__ __forceinline__ void sel_hist_pass(const float* __restrict__ R, const
     if (threadIdx.x == 0) st->ticket = 0;
 }
 
-// one pass as a launch (the typical signal: MODE 2)
-template <int MODE, int PASS>
+// The selections by radix passes over the planes, as ONE cooperative launch (grid barriers between the passes): the
+// path of the frames the fast path of selectz.cuh does not fit -- the three clipping rounds (eighteen passes) when
+// *zdone is 0, the typical signal and the gain (three passes) when *zmdone is 0.  Returns at once when that path has
+// done both, which is why it is one launch and not twenty-one.
 __global__ void __launch_bounds__(256)
-k_sel_hist(const float* __restrict__ R, const float* __restrict__ M5, size_t npx, SelState* st, uint32_t* hist,
-           int last, float rn2, float* gain_out, float* stats, const int* prev_count, const uint32_t* zdone,
-           const uint32_t* zno, const float2* __restrict__ olist) {
+k_sel_rounds(const float* __restrict__ R, const float* __restrict__ M5, size_t npx, SelState* st, uint32_t* hist, float rn2,
+             float* gain_out, float* stats, const int* prev_count, const uint32_t* zdone, const uint32_t* zmdone,
+             const uint32_t* zno, const float2* __restrict__ olist) {
     if (prev_count && *prev_count == 0) {          // fixed point (R17): same image, same estimate
-        if (MODE == 2 && PASS == 2 && blockIdx.x == 0 && threadIdx.x == 0) *gain_out = gain_out[-1];
+        if (blockIdx.x == 0 && threadIdx.x == 0) *gain_out = gain_out[-1];
         return;
     }
     const bool fast = zdone && *zdone;
-    if (MODE != 2 && fast) return;
-    __shared__ uint32_t sh[SEL_BINS];
-    sel_hist_pass<MODE, PASS>(R, M5, npx, st, hist, last, rn2, gain_out, stats, fast, zno, olist, sh);
-}
-
-// The three clipping rounds by radix passes over the plane, as ONE cooperative launch (grid barriers between the
-// eighteen passes): the path of the frames the fast path of selectz.cuh does not fit.  Returns at once when that
-// path has resolved the rounds, which is why it is one launch and not eighteen.
-__global__ void __launch_bounds__(256)
-k_sel_rounds(const float* __restrict__ R, size_t npx, SelState* st, uint32_t* hist, const int* prev_count,
-             const uint32_t* zdone) {
-    if (prev_count && *prev_count == 0) return;
-    if (zdone && *zdone) return;
+    if (fast && zmdone && *zmdone) return;
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     __shared__ uint32_t sh[SEL_BINS];
-    for (int j = 0; j < SEL_ROUNDS; ++j) {
-        const int last = j == SEL_ROUNDS - 1;
-        sel_hist_pass<0, 0>(R, nullptr, npx, st, hist, 0, 0.0f, nullptr, nullptr, false, nullptr, nullptr, sh); grid.sync();
-        sel_hist_pass<0, 1>(R, nullptr, npx, st, hist, 0, 0.0f, nullptr, nullptr, false, nullptr, nullptr, sh); grid.sync();
-        sel_hist_pass<0, 2>(R, nullptr, npx, st, hist, 0, 0.0f, nullptr, nullptr, false, nullptr, nullptr, sh); grid.sync();
-        sel_hist_pass<1, 0>(R, nullptr, npx, st, hist, 0, 0.0f, nullptr, nullptr, false, nullptr, nullptr, sh); grid.sync();
-        sel_hist_pass<1, 1>(R, nullptr, npx, st, hist, 0, 0.0f, nullptr, nullptr, false, nullptr, nullptr, sh); grid.sync();
-        sel_hist_pass<1, 2>(R, nullptr, npx, st, hist, last, 0.0f, nullptr, nullptr, false, nullptr, nullptr, sh); grid.sync();
+    if (!fast) {
+        for (int j = 0; j < SEL_ROUNDS; ++j) {
+            const int last = j == SEL_ROUNDS - 1;
+            sel_hist_pass<0, 0>(R, M5, npx, st, hist, 0, rn2, gain_out, stats, false, zno, olist, sh); grid.sync();
+            sel_hist_pass<0, 1>(R, M5, npx, st, hist, 0, rn2, gain_out, stats, false, zno, olist, sh); grid.sync();
+            sel_hist_pass<0, 2>(R, M5, npx, st, hist, 0, rn2, gain_out, stats, false, zno, olist, sh); grid.sync();
+            sel_hist_pass<1, 0>(R, M5, npx, st, hist, 0, rn2, gain_out, stats, false, zno, olist, sh); grid.sync();
+            sel_hist_pass<1, 1>(R, M5, npx, st, hist, 0, rn2, gain_out, stats, false, zno, olist, sh); grid.sync();
+            sel_hist_pass<1, 2>(R, M5, npx, st, hist, last, rn2, gain_out, stats, false, zno, olist, sh); grid.sync();
+        }
     }
+    // typical signal over the set the last round kept, then the gain (fast: over the med5 plane alone, the listed
+    // pixels outside the kept interval subtracted)
+    sel_hist_pass<2, 0>(R, M5, npx, st, hist, 1, rn2, gain_out, stats, fast, zno, olist, sh); grid.sync();
+    sel_hist_pass<2, 1>(R, M5, npx, st, hist, 1, rn2, gain_out, stats, fast, zno, olist, sh); grid.sync();
+    sel_hist_pass<2, 2>(R, M5, npx, st, hist, 1, rn2, gain_out, stats, fast, zno, olist, sh);
 }
 
 }  // namespace lac

@@ -35,6 +35,7 @@ namespace cg = cooperative_groups;
 #endif
 constexpr int SELZ_NB = LAC_SELZ_NB;          // buckets
 constexpr int SELZ_SAMPLE = 128;
+constexpr int SELZ_IT = 1024;                 // threads of k_selz_init (the first SELZ_SAMPLE sample, all clear the histograms)
 constexpr int SELZ_HT = 1024;                 // threads per CTA of k_selz_hist
 #ifndef LAC_SELZ_CLUSTER
 #define LAC_SELZ_CLUSTER 16
@@ -62,23 +63,32 @@ struct SelZone {
                                               // 4 % of a frame).  Inside Z0 they are counted, not listed.
     uint32_t nneg0;                           // negative residuals in the bucket of 0: when a centre's rank inside that bucket
                                               // falls on the zeros, the centre is +0 without a selection (the usual case)
+    // the typical signal: a second grid over max(med5, 1e-4) and one zone ZM around its median
+    float mbase, mscale;
+    int m5lo, m5hi;                           // bucket range of ZM
+    uint32_t below_m5, cnt_m5;                // values in buckets < m5lo; in ZM
+    uint32_t nm;                              // list cursor
+    uint32_t mok;                             // 1: grid and zone made, the list fits
+    uint32_t mdone;                           // 1: k_selz_resolve selected the typical signal and wrote the gain
 };
 
-// capacities of the four lists inside `words` 32-bit words of storage
+// capacities of the five lists inside `words` 32-bit words of storage
 struct SelzLists {
     float* z0;
     float* z1;
     float2* o;
+    float* zm;
     uint32_t* scr;
-    uint32_t cap0, cap1, capo, capscr;
+    uint32_t cap0, cap1, capo, capm, capscr;
 };
 __host__ __device__ inline SelzLists selz_carve(void* base, size_t words) {
     SelzLists l;
-    const size_t e = (words / 16) & ~(size_t)1;      // a sixteenth, even
-    l.z0 = (float*)base;                 l.cap0 = (uint32_t)(3 * e);     // (the residual 0 alone is 4 % of a frame: every
-    l.z1 = l.z0 + 3 * e;                 l.cap1 = (uint32_t)(4 * e);     //  pixel that is the median of its own window)
+    const size_t e = (words / 20) & ~(size_t)1;      // a twentieth, even
+    l.z0 = (float*)base;                 l.cap0 = (uint32_t)(3 * e);
+    l.z1 = l.z0 + 3 * e;                 l.cap1 = (uint32_t)(4 * e);
     l.o = (float2*)(l.z1 + 4 * e);       l.capo = (uint32_t)(3 * e);
-    l.scr = (uint32_t*)(l.z1 + 10 * e);  l.capscr = (uint32_t)(3 * e);
+    l.zm = l.z1 + 10 * e;                l.capm = (uint32_t)(4 * e);
+    l.scr = (uint32_t*)(l.z1 + 14 * e);  l.capscr = (uint32_t)(3 * e);
     return l;
 }
 
@@ -88,17 +98,17 @@ __device__ __forceinline__ int selz_bucket(float r, float base, float scale) {
 
 // One CTA of SELZ_SAMPLE threads: state, histograms, and the bucket grid from a strided sample of the plane (the median and
 // the MAD of the sample by rank counting: thread i counts the sample values below its own).
-__global__ void __launch_bounds__(SELZ_SAMPLE)
-k_selz_init(const float* __restrict__ R, size_t npx, SelState* st, SelZone* zn, uint32_t* hist, uint32_t* histz,
-            int force_classic, const int* prev_count) {
+__global__ void __launch_bounds__(SELZ_IT)
+k_selz_init(const float* __restrict__ R, const float* __restrict__ M5, size_t npx, SelState* st, SelZone* zn, uint32_t* hist,
+            uint32_t* histz, uint32_t* histm, int force_classic, const int* prev_count) {
     if (prev_count && *prev_count == 0) return;
     __shared__ __align__(16) uint32_t k[SELZ_SAMPLE];
-    __shared__ uint32_t s_res[2];
+    __shared__ uint32_t s_res[4];
     const int tid = threadIdx.x;
-    for (int i = tid; i < SEL_BINS; i += SELZ_SAMPLE) hist[i] = 0;
-    for (int i = tid; i < SELZ_NB; i += SELZ_SAMPLE) histz[i] = 0;
+    for (int i = tid; i < SEL_BINS; i += SELZ_IT) hist[i] = 0;
+    for (int i = tid; i < SELZ_NB; i += SELZ_IT) { histz[i] = 0; histm[i] = 0; }
     const uint32_t ns = (uint32_t)(npx < SELZ_SAMPLE ? npx : SELZ_SAMPLE);
-    float v = 0.0f;
+    float v = 0.0f, vm = 1e-4f;
     bool valid = false;
     if ((uint32_t)tid < ns) {
         // groups of 32 values 61 apart (few pages to touch), the groups spread over the plane
@@ -106,32 +116,47 @@ k_selz_init(const float* __restrict__ R, size_t npx, SelState* st, SelZone* zn, 
         const size_t i = npx < SELZ_SAMPLE ? (size_t)tid : (size_t)(tid >> 5) * grp + (size_t)(tid & 31) * step;
         v = R[i];
         valid = v == v;                                   // NaN (caller error) is left out of the sample
+        vm = M5[i];
+        vm = vm > 1e-4f ? vm : 1e-4f;
     }
     const uint32_t nv = (uint32_t)__syncthreads_count(valid);
-    if (tid == 0) s_res[0] = s_res[1] = 0x80000000u;      // key of +0
-    // rank of a key among the valid keys (ties by index); invalid entries hold the largest key and sort last
-    auto rank_of = [&](uint32_t mine) -> uint32_t {
-        k[tid] = mine;
+    if (tid == 0) s_res[0] = s_res[1] = s_res[2] = s_res[3] = 0x80000000u;      // key of +0
+    // ranks of two keys among the valid keys of their arrays (ties by index); invalid entries hold the largest key and
+    // sort last.  One loop for both: the residual and max(med5, 1e-4) at the sampled pixels.
+    __shared__ __align__(16) uint32_t k2[SELZ_SAMPLE];
+    auto rank_of2 = [&](uint32_t mine, uint32_t mine2, uint32_t& rk, uint32_t& rk2) {
+        if (tid < SELZ_SAMPLE) { k[tid] = mine; k2[tid] = mine2; }
         __syncthreads();
-        uint32_t rk = 0;
+        rk = rk2 = 0;
 #pragma unroll 4
-        for (int j = 0; j < SELZ_SAMPLE; j += 4) {
-            const uint4 o = *reinterpret_cast<const uint4*>(k + j);
+        for (int j = 0; j < (tid < SELZ_SAMPLE ? SELZ_SAMPLE : 0); j += 4) {
+            const uint4 o = *reinterpret_cast<const uint4*>(k + j), p = *reinterpret_cast<const uint4*>(k2 + j);
             rk += (o.x < mine || (o.x == mine && j < tid)) ? 1u : 0u;
             rk += (o.y < mine || (o.y == mine && j + 1 < tid)) ? 1u : 0u;
             rk += (o.z < mine || (o.z == mine && j + 2 < tid)) ? 1u : 0u;
             rk += (o.w < mine || (o.w == mine && j + 3 < tid)) ? 1u : 0u;
+            rk2 += (p.x < mine2 || (p.x == mine2 && j < tid)) ? 1u : 0u;
+            rk2 += (p.y < mine2 || (p.y == mine2 && j + 1 < tid)) ? 1u : 0u;
+            rk2 += (p.z < mine2 || (p.z == mine2 && j + 2 < tid)) ? 1u : 0u;
+            rk2 += (p.w < mine2 || (p.w == mine2 && j + 3 < tid)) ? 1u : 0u;
         }
         __syncthreads();
-        return rk;
     };
     const uint32_t want = nv ? (nv - 1u) / 2u : 0u;
+    uint32_t ra, rb;
     const uint32_t key0 = valid ? sel_key(v) : 0xffffffffu;
-    if (rank_of(key0) == want && valid) s_res[0] = key0;
+    const uint32_t key2 = valid ? (__float_as_uint(vm) | 0x80000000u) : 0xffffffffu;
+    rank_of2(key0, key2, ra, rb);
+    if (ra == want && valid) s_res[0] = key0;
+    if (rb == want && valid) s_res[2] = key2;
     __syncthreads();
     const float c0 = sel_unkey(s_res[0]);
+    const float cm = __uint_as_float(s_res[2] & 0x7fffffffu);
     const uint32_t key1 = valid ? (__float_as_uint(fabsf(v - c0)) | 0x80000000u) : 0xffffffffu;
-    if (rank_of(key1) == want && valid) s_res[1] = key1;
+    const uint32_t key3 = valid ? (__float_as_uint(fabsf(vm - cm)) | 0x80000000u) : 0xffffffffu;
+    rank_of2(key1, key3, ra, rb);
+    if (ra == want && valid) s_res[1] = key1;
+    if (rb == want && valid) s_res[3] = key3;
     __syncthreads();
     if (tid == 0) {
         st->lo = -__int_as_float(0x7f800000);
@@ -158,6 +183,13 @@ k_selz_init(const float* __restrict__ R, size_t npx, SelState* st, SelZone* zn, 
         z.done = 0;
         z.why = z.ok ? 0u : 1u;                             // 1: switched off, or no usable bucket grid
         z.nzero = z.nneg0 = 0;
+        const float sm0 = 1.4826f * __uint_as_float(s_res[3] & 0x7fffffffu);
+        z.mbase = cm - 8.0f * sm0;
+        z.mscale = (float)SELZ_NB / (16.0f * sm0);
+        z.m5lo = z.m5hi = 0;
+        z.below_m5 = z.cnt_m5 = z.nm = 0;
+        z.mok = (z.ok && sm0 > 0.0f && sm0 < INF && z.mscale > 0.0f && z.mscale < INF && fabsf(z.mbase) < INF) ? 1u : 0u;
+        z.mdone = 0;
         *zn = z;
     }
 }
@@ -238,50 +270,15 @@ __device__ void selz_plan(const uint32_t* cum, SelZone* zn, SelzLists cap) {
     *zn = z;
 }
 
-__global__ void __launch_bounds__(SELZ_HT)
-k_selz_hist(const float* __restrict__ R, size_t npx, SelState* st, SelZone* zn, uint32_t* histz, void* lists,
-            size_t list_words, const int* prev_count) {
-    if (prev_count && *prev_count == 0) return;
-    if (!zn->ok) return;
-    __shared__ uint32_t sh[SELZ_NB + 1];
-    for (int i = threadIdx.x; i < SELZ_NB; i += SELZ_HT) sh[i] = 0;
-    __syncthreads();
-    const float base = zn->base, scale = zn->scale;
-    const int bzero = selz_bucket(0.0f, base, scale);
-    uint32_t nzero = 0, nneg0 = 0;
-    sel_visit_plane<false, SELZ_HT>(R, nullptr, npx, [&](float r, float, bool ok, size_t) {
-        if (ok) {
-            const int b = selz_bucket(r, base, scale);
-            atomicAdd(&sh[b], 1u);
-            if (b == bzero) {
-                const uint32_t u = __float_as_uint(r);
-                nzero += u == 0u ? 1u : 0u;
-                nneg0 += u >> 31;
-            }
-        }
-    });
-    nzero = __reduce_add_sync(0xffffffffu, nzero);
-    nneg0 = __reduce_add_sync(0xffffffffu, nneg0);
-    if ((threadIdx.x & 31) == 0 && nzero) atomicAdd(&zn->nzero, nzero);
-    if ((threadIdx.x & 31) == 0 && nneg0) atomicAdd(&zn->nneg0, nneg0);
-    __syncthreads();
-    for (int i = threadIdx.x; i < SELZ_NB; i += SELZ_HT)
-        if (sh[i]) atomicAdd(&histz[i], sh[i]);
-    __shared__ bool s_last;
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) s_last = atomicAdd(&st->ticket, 1u) == gridDim.x - 1;
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    // cumulative counts (the histogram stays in global memory: k_selz_resolve reads single buckets of it)
+// cumulative counts of a global histogram into cum[0 .. SELZ_NB] (shared memory), by the first 256 threads of the CTA;
+// scan: 256 words of shared memory.  Contains block barriers (all threads call).
+__device__ __forceinline__ void selz_cumulate(const uint32_t* hist_g, uint32_t* cum, uint32_t* scan) {
     constexpr int PER = SELZ_NB / 256;
-    __shared__ uint32_t scan[256];
-    uint32_t loc[PER], sum = 0, incl = 0;
+    uint32_t loc[PER], sum = 0;
     if (threadIdx.x < 256) {
 #pragma unroll
         for (int i = 0; i < PER; ++i) {
-            loc[i] = __ldcg(histz + threadIdx.x * PER + i);
+            loc[i] = __ldcg(hist_g + threadIdx.x * PER + i);
             sum += loc[i];
         }
         scan[threadIdx.x] = sum;
@@ -293,18 +290,91 @@ k_selz_hist(const float* __restrict__ R, size_t npx, SelState* st, SelZone* zn, 
     }
     __syncthreads();
     if (threadIdx.x < 256) {
-        incl = scan[threadIdx.x];
-        uint32_t acc = incl - sum;
+        uint32_t acc = scan[threadIdx.x] - sum;
 #pragma unroll
         for (int i = 0; i < PER; ++i) {
-            sh[threadIdx.x * PER + i] = acc;
+            cum[threadIdx.x * PER + i] = acc;
             acc += loc[i];
         }
-        if (threadIdx.x == 255) sh[SELZ_NB] = acc;
+        if (threadIdx.x == 255) cum[SELZ_NB] = acc;
     }
     __syncthreads();
+}
+
+// The zone of the typical signal, by one thread, after selz_plan.  The wanted element has rank (n3 - 1) / 2 among the
+// kept pixels, n3 = npx - (excluded pixels), and every excluded pixel is in an OUT zone: among ALL pixels its position
+// lies in [(npx - nout - 1) / 2, (npx - 1) / 2 + nout].
+__device__ void selz_plan_m(const uint32_t* cum, SelZone* zn, SelzLists cap) {
+    SelZone z = *zn;
+    bool ok = z.ok && z.mok;
+    if (ok) {
+        const uint32_t nout = z.cnt_om + z.cnt_op;
+        ok = nout < z.npx;
+        if (ok) {
+            const uint32_t glo = (z.npx - nout - 1u) / 2u;
+            const unsigned long long gh = (unsigned long long)(z.npx - 1u) / 2u + nout;
+            const uint32_t ghi = gh < z.npx ? (uint32_t)gh : z.npx - 1u;
+            z.m5lo = max(selz_bucket_of_rank(cum, glo) - 1, 0);
+            z.m5hi = min(selz_bucket_of_rank(cum, ghi) + 1, SELZ_NB - 1);
+            z.below_m5 = cum[z.m5lo];
+            z.cnt_m5 = cum[z.m5hi + 1] - cum[z.m5lo];
+            ok = z.cnt_m5 <= cap.capm;
+        }
+    }
+    z.mok = ok ? 1u : 0u;
+    z.nm = 0;
+    *zn = z;
+}
+
+__global__ void __launch_bounds__(SELZ_HT)
+k_selz_hist(const float* __restrict__ R, const float* __restrict__ M5, size_t npx, SelState* st, SelZone* zn, uint32_t* histz,
+            uint32_t* histm, void* lists, size_t list_words, const int* prev_count) {
+    if (prev_count && *prev_count == 0) return;
+    if (!zn->ok) return;
+    __shared__ uint32_t sh[SELZ_NB + 1], shm[SELZ_NB + 1];
+    for (int i = threadIdx.x; i < SELZ_NB; i += SELZ_HT) sh[i] = shm[i] = 0;
+    __syncthreads();
+    const float base = zn->base, scale = zn->scale, mbase = zn->mbase, mscale = zn->mscale;
+    const bool wm = zn->mok != 0;             // also the grid of the typical signal
+    const int bzero = selz_bucket(0.0f, base, scale);
+    uint32_t nzero = 0, nneg0 = 0;
+    auto visit = [&](float r, float m5, bool ok, size_t) {
+        if (ok) {
+            const int b = selz_bucket(r, base, scale);
+            atomicAdd(&sh[b], 1u);
+            if (b == bzero) {
+                const uint32_t u = __float_as_uint(r);
+                nzero += u == 0u ? 1u : 0u;
+                nneg0 += u >> 31;
+            }
+            if (wm) atomicAdd(&shm[selz_bucket(m5 > 1e-4f ? m5 : 1e-4f, mbase, mscale)], 1u);
+        }
+    };
+    if (wm) sel_visit_plane<true, SELZ_HT>(R, M5, npx, visit);
+    else sel_visit_plane<false, SELZ_HT>(R, nullptr, npx, visit);
+    nzero = __reduce_add_sync(0xffffffffu, nzero);
+    nneg0 = __reduce_add_sync(0xffffffffu, nneg0);
+    if ((threadIdx.x & 31) == 0 && nzero) atomicAdd(&zn->nzero, nzero);
+    if ((threadIdx.x & 31) == 0 && nneg0) atomicAdd(&zn->nneg0, nneg0);
+    __syncthreads();
+    for (int i = threadIdx.x; i < SELZ_NB; i += SELZ_HT) {
+        if (sh[i]) atomicAdd(&histz[i], sh[i]);
+        if (wm && shm[i]) atomicAdd(&histm[i], shm[i]);
+    }
+    __shared__ bool s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(&st->ticket, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    // cumulative counts (the histograms stay in global memory: k_selz_resolve reads single buckets of the first)
+    __shared__ uint32_t scan[256];
+    selz_cumulate(histz, sh, scan);
+    if (wm) selz_cumulate(histm, shm, scan);
     if (threadIdx.x == 0) {
         selz_plan(sh, zn, selz_carve(lists, list_words));
+        selz_plan_m(shm, zn, selz_carve(lists, list_words));
         st->ticket = 0;
     }
 }
@@ -332,17 +402,23 @@ k_selz_compact(const float* __restrict__ R, const float* __restrict__ M5, size_t
     __shared__ float s_0[SELZ_BUF], s_1[SELZ_BUF];
     __shared__ float2 s_o[SELZ_BUF];
     __shared__ uint8_t s_cls[SELZ_NB];        // list of a bucket: 0 none, 1 Z0, 2 Z- / Z+, 3 OUT
-    __shared__ uint32_t s_n[3], s_b[3];
+    __shared__ float s_m[SELZ_BUF];           // max(med5, 1e-4) of the pixels in ZM
+    __shared__ uint32_t s_n[4], s_b[4];
     const SelzLists L = selz_carve(lists, list_words);
     const SelZone z = *zn;
     for (int i = threadIdx.x; i < SELZ_NB; i += 256) {
         const uint32_t zid = selz_zone_of(z, i);
         s_cls[i] = (uint8_t)(zid == 2 ? 1 : (zid == 1 || zid == 3) ? 2 : zid >= 4 ? 3 : 0);
     }
-    if (threadIdx.x < 3) s_n[threadIdx.x] = 0;
+    if (threadIdx.x < 4) s_n[threadIdx.x] = 0;
     __syncthreads();
     const int lane = threadIdx.x & 31;
-    const float base = z.base, scale = z.scale;
+    const float base = z.base, scale = z.scale, mbase = z.mbase, mscale = z.mscale;
+    const bool wm = z.mok != 0;               // the list of the typical signal's zone too (reads the med5 plane as well)
+    const int m5lo = z.m5lo, m5w = z.m5hi - z.m5lo;
+    auto putm = [&](uint32_t p, float m5c) {
+        if (p < SELZ_BUF) s_m[p] = m5c; else L.zm[atomicAdd(&zn->nm, 1u)] = m5c;
+    };
     auto put = [&](uint32_t cls, uint32_t p, float r, size_t idx) {
         if (cls == 1) { if (p < SELZ_BUF) s_0[p] = r; else L.z0[atomicAdd(&zn->n0, 1u)] = r; }
         else if (cls == 2) { if (p < SELZ_BUF) s_1[p] = r; else L.z1[atomicAdd(&zn->n1, 1u)] = r; }
@@ -353,7 +429,7 @@ k_selz_compact(const float* __restrict__ R, const float* __restrict__ M5, size_t
     };
     const size_t nvec = npx / 4;
     for (size_t b0 = (size_t)blockIdx.x * 1024; b0 < nvec; b0 += (size_t)gridDim.x * 1024) {
-        float v[16];
+        float v[16], mv[16];
         bool okv[4];
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
@@ -361,6 +437,17 @@ k_selz_compact(const float* __restrict__ R, const float* __restrict__ M5, size_t
             okv[u] = i < nvec;
             const float4 q = okv[u] ? __ldg(reinterpret_cast<const float4*>(R) + i) : make_float4(0.f, 0.f, 0.f, 0.f);
             v[4 * u] = q.x; v[4 * u + 1] = q.y; v[4 * u + 2] = q.z; v[4 * u + 3] = q.w;
+            const float4 m = (wm && okv[u]) ? __ldg(reinterpret_cast<const float4*>(M5) + i) : make_float4(0.f, 0.f, 0.f, 0.f);
+            mv[4 * u] = m.x; mv[4 * u + 1] = m.y; mv[4 * u + 2] = m.z; mv[4 * u + 3] = m.w;
+        }
+        uint32_t mbits = 0;                   // values whose med5 lies in ZM
+        if (wm) {
+#pragma unroll
+            for (int e = 0; e < 16; ++e) {
+                mv[e] = mv[e] > 1e-4f ? mv[e] : 1e-4f;
+                const uint32_t in = (uint32_t)(selz_bucket(mv[e], mbase, mscale) - m5lo) <= (uint32_t)m5w ? 1u : 0u;
+                mbits |= (okv[e >> 2] ? in : 0u) << e;
+            }
         }
         uint32_t codes = 0;                   // 2 bits per value: its list
 #pragma unroll
@@ -372,26 +459,36 @@ k_selz_compact(const float* __restrict__ R, const float* __restrict__ M5, size_t
         // entries of this thread per list: fields equal to 1, 2, 3
         const uint32_t lo1 = codes & 0x55555555u, hi1 = (codes >> 1) & 0x55555555u;
         const uint32_t c0 = __popc(lo1 & ~hi1), c1 = __popc(hi1 & ~lo1), co = __popc(lo1 & hi1);
-        if (__ballot_sync(0xffffffffu, codes != 0u) == 0) continue;
+        if (__ballot_sync(0xffffffffu, (codes | mbits) != 0u) == 0) continue;
         // inclusive prefix sums over the warp (at most 16 x 32 = 512 entries per list: two lists share a word)
-        const uint32_t own_a = c0 | (c1 << 16), own_b = co;
+        const uint32_t own_a = c0 | (c1 << 16), own_b = co | ((uint32_t)__popc(mbits) << 16);
         uint32_t inc_a = own_a, inc_b = own_b;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
             const uint32_t oa = __shfl_up_sync(0xffffffffu, inc_a, d), ob = __shfl_up_sync(0xffffffffu, inc_b, d);
             if (lane >= d) { inc_a += oa; inc_b += ob; }
         }
-        uint32_t base0 = 0, base1 = 0, baseo = 0;
+        uint32_t base0 = 0, base1 = 0, baseo = 0, basem = 0;
         if (lane == 31) {
-            const uint32_t t0 = inc_a & 0xffffu, t1 = inc_a >> 16, to = inc_b;
+            const uint32_t t0 = inc_a & 0xffffu, t1 = inc_a >> 16, to = inc_b & 0xffffu, tm = inc_b >> 16;
             if (t0) base0 = atomicAdd(&s_n[0], t0);
             if (t1) base1 = atomicAdd(&s_n[1], t1);
             if (to) baseo = atomicAdd(&s_n[2], to);
+            if (tm) basem = atomicAdd(&s_n[3], tm);
         }
         const uint32_t ex_a = inc_a - own_a, ex_b = inc_b - own_b;
         uint32_t p0 = __shfl_sync(0xffffffffu, base0, 31) + (ex_a & 0xffffu);
         uint32_t p1 = __shfl_sync(0xffffffffu, base1, 31) + (ex_a >> 16);
-        uint32_t po = __shfl_sync(0xffffffffu, baseo, 31) + ex_b;
+        uint32_t po = __shfl_sync(0xffffffffu, baseo, 31) + (ex_b & 0xffffu);
+        uint32_t pm = __shfl_sync(0xffffffffu, basem, 31) + (ex_b >> 16);
+        while (mbits) {
+            const int e = __ffs(mbits) - 1;
+            mbits &= mbits - 1;
+            float m = mv[0];
+#pragma unroll
+            for (int q = 1; q < 16; ++q) m = (e == q) ? mv[q] : m;
+            putm(pm++, m);
+        }
         uint32_t rem = codes;                 // (a thread has one hit in 16 values on average: loop over the hits)
         while (rem) {
             const int e = (__ffs(rem) - 1) >> 1;
@@ -411,19 +508,24 @@ k_selz_compact(const float* __restrict__ R, const float* __restrict__ M5, size_t
             uint32_t cls = s_cls[selz_bucket(r, base, scale)];
             if (cls == 1 && __float_as_uint(r) == 0u) cls = 0;
             if (cls) put(cls, SELZ_BUF, r, t);
+            if (wm) {
+                const float m = M5[t] > 1e-4f ? M5[t] : 1e-4f;
+                if ((uint32_t)(selz_bucket(m, mbase, mscale) - m5lo) <= (uint32_t)m5w) putm(SELZ_BUF, m);
+            }
         }
     }
     __syncthreads();
-    if (threadIdx.x < 3) {
+    if (threadIdx.x < 4) {
         const uint32_t n = min(s_n[threadIdx.x], (uint32_t)SELZ_BUF);
         s_n[threadIdx.x] = n;
-        uint32_t* cur = threadIdx.x == 0 ? &zn->n0 : threadIdx.x == 1 ? &zn->n1 : &zn->no;
+        uint32_t* cur = threadIdx.x == 0 ? &zn->n0 : threadIdx.x == 1 ? &zn->n1 : threadIdx.x == 2 ? &zn->no : &zn->nm;
         s_b[threadIdx.x] = n ? atomicAdd(cur, n) : 0u;
     }
     __syncthreads();
     for (uint32_t i = threadIdx.x; i < s_n[0]; i += 256) L.z0[s_b[0] + i] = s_0[i];
     for (uint32_t i = threadIdx.x; i < s_n[1]; i += 256) L.z1[s_b[1] + i] = s_1[i];
     for (uint32_t i = threadIdx.x; i < s_n[2]; i += 256) L.o[s_b[2] + i] = s_o[i];
+    for (uint32_t i = threadIdx.x; i < s_n[3]; i += 256) L.zm[s_b[3] + i] = s_m[i];
 }
 
 // ---- the three rounds on the lists ----------------------------------------------------------------
@@ -595,9 +697,67 @@ __device__ __forceinline__ uint32_t selz_edge_key(int b, float base, float scale
     return hi;
 }
 
+// the same for the grid of max(med5, 1e-4) (positive values: key = bits | 0x80000000): smallest key with bucket >= b
+__device__ __forceinline__ uint32_t selz_edge_key_m(int b, float base, float scale) {
+    uint32_t lo = 0x80000000u, hi = 0xff800000u;        // +0 (below every value: they are >= 1e-4) .. +inf
+    if (selz_bucket(__uint_as_float(lo & 0x7fffffffu), base, scale) >= b) return lo;
+    if (b >= SELZ_NB || selz_bucket(__uint_as_float(hi & 0x7fffffffu), base, scale) < b) return hi + 1u;
+    while (hi - lo > 1u) {                               // invariant: bucket(lo) < b <= bucket(hi)
+        const uint32_t mid = lo + ((hi - lo) >> 1);
+        if (selz_bucket(__uint_as_float(mid & 0x7fffffffu), base, scale) >= b) hi = mid; else lo = mid;
+    }
+    return hi;
+}
+
+// Radix selection on the cluster over the multiset { keys of `add` } minus { keyfn_sub of the entries of `sub` it accepts }
+// inside [klo, khi]: the key of rank kth (the caller guarantees more than kth members).  No scratch list: two or
+// three passes over the lists.
+template <class KS>
+__device__ __forceinline__ uint32_t selz_select_sub(cg::cluster_group& cl, SelzShared* sm, const float* __restrict__ add, uint32_t nadd,
+                                                    const float2* __restrict__ sub, uint32_t nsub, uint32_t klo, uint32_t khi,
+                                                    uint32_t kth, int& par, KS keyfn_sub) {
+    const bool lead = cl.block_rank() == 0;
+    const SelzShared* lsm = cl.map_shared_rank(sm, 0);
+    while (khi > klo) {
+        const uint32_t span = khi - klo;
+        const int bits = 32 - __clz(span);
+        const int shift = bits > 11 ? bits - 11 : 0;
+        for (int i = threadIdx.x; i < SEL_BINS; i += SELZ_RT) sm->hist[i] = 0;
+        __syncthreads();
+        selz_for_each(cl, add, nadd, [&](float v, bool ok) {
+            const uint32_t dk = (__float_as_uint(v) | 0x80000000u) - klo;
+            if (ok && dk <= span) atomicAdd(&sm->hist[dk >> shift], 1u);
+        });
+        selz_for_each(cl, sub, nsub, [&](float2 e, bool ok) {
+            uint32_t k = 0;
+            if (ok && keyfn_sub(e, k) && k - klo <= span) atomicSub(&sm->hist[(k - klo) >> shift], 1u);   // (wraps; the sum is exact)
+        });
+        cl.sync();
+        if (lead) {
+            uint32_t t2[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                uint32_t t = 0;
+                for (int r = 0; r < SELZ_CLUSTER; ++r) t += cl.map_shared_rank(sm, r)->hist[2 * threadIdx.x + u];
+                t2[u] = t;
+            }
+            selz_pick(sm, t2[0], t2[1], kth, sm->bc[par & 1]);
+        }
+        cl.sync();
+        const uint32_t digit = lsm->bc[par & 1][0];
+        kth = lsm->bc[par & 1][1];
+        ++par;
+        klo += digit << shift;
+        const uint32_t nhi = shift ? klo + ((1u << shift) - 1u) : klo;
+        khi = nhi < khi ? nhi : khi;
+    }
+    return klo;
+}
+
 __global__ void __cluster_dims__(SELZ_CLUSTER, 1, 1) __launch_bounds__(SELZ_RT)
 k_selz_resolve(SelState* st, SelZone* zn, const uint32_t* __restrict__ histz, void* lists, size_t list_words,
-               float* path_out, const int* prev_count) {
+               float rn2, float* gain_out, float* stats, const int* prev_count) {
+    float* const path_out = stats ? stats + 6 : nullptr;
     if (prev_count && *prev_count == 0) return;
     if (!zn->ok) {
         if (path_out && blockIdx.x == 0 && threadIdx.x == 0) *path_out = 0.0f;
@@ -708,6 +868,55 @@ k_selz_resolve(SelState* st, SelZone* zn, const uint32_t* __restrict__ histz, vo
             hi = nhi < hi ? nhi : hi;
         }
     }
+    // The typical signal: rank (n - 1) / 2 of max(med5, 1e-4) over the kept pixels = all pixels minus the OUT entries
+    // outside the interval the last round started from.  Everything outside ZM enters through the exact bucket counts.
+    bool mok = ok && z.mok;
+    float mt = 0.0f;
+    if (mok) {
+        const float mbase = z.mbase, mscale = z.mscale;
+        uint32_t nb = 0, nin = 0;                 // excluded pixels below ZM / inside ZM
+        selz_for_each(cl, L.o, no, [&](float2 e, bool v) {
+            if (v && !(e.x >= lo0 && e.x <= hi0)) {
+                const int bm = selz_bucket(e.y > 1e-4f ? e.y : 1e-4f, mbase, mscale);
+                nb += bm < z.m5lo ? 1u : 0u;
+                nin += (bm >= z.m5lo && bm <= z.m5hi) ? 1u : 0u;
+            }
+        });
+        nb = __reduce_add_sync(0xffffffffu, nb);
+        nin = __reduce_add_sync(0xffffffffu, nin);
+        __syncthreads();
+        if ((threadIdx.x & 31) == 0) { sm->red[0][threadIdx.x >> 5] = nb; sm->red[1][threadIdx.x >> 5] = nin; }
+        __syncthreads();
+        if (threadIdx.x < 2) {
+            uint32_t t = 0;
+            for (int i = 0; i < SELZ_RT / 32; ++i) t += sm->red[threadIdx.x][i];
+            sm->sums[1][threadIdx.x] = t;         // (slot 1 was last used by round 1; round 2 used slot 0)
+        }
+        cl.sync();
+        uint32_t xb = 0, xin = 0;
+        for (int r = 0; r < SELZ_CLUSTER; ++r) {
+            const SelzShared* o = cl.map_shared_rank(sm, r);
+            xb += o->sums[1][0];
+            xin += o->sums[1][1];
+        }
+        const uint32_t k3 = (nkept - 1u) / 2u;
+        const uint32_t kept_below = z.below_m5 - xb;
+        mok = xb <= z.below_m5 && xin <= z.cnt_m5 && k3 >= kept_below && k3 - kept_below < z.cnt_m5 - xin;
+        if (mok) {
+            __syncthreads();
+            if (threadIdx.x < 2) sm->edge[8 + threadIdx.x] = selz_edge_key_m(threadIdx.x == 0 ? z.m5lo : z.m5hi + 1, mbase, mscale);
+            __syncthreads();
+            const uint32_t km = selz_select_sub(cl, sm, L.zm, z.cnt_m5, L.o, no, sm->edge[8], sm->edge[9] - 1u, k3 - kept_below, par,
+                                                [&](float2 e, uint32_t& key) {
+                if (e.x >= lo0 && e.x <= hi0) return false;
+                const float m = e.y > 1e-4f ? e.y : 1e-4f;
+                const int bm = selz_bucket(m, mbase, mscale);
+                key = __float_as_uint(m) | 0x80000000u;
+                return bm >= z.m5lo && bm <= z.m5hi;
+            });
+            mt = __uint_as_float(km & 0x7fffffffu);
+        }
+    }
     cl.sync();                                            // nobody leaves while its shared memory may still be read
     if (cl.block_rank() == 0 && threadIdx.x == 0) {
         if (ok) {
@@ -716,7 +925,19 @@ k_selz_resolve(SelState* st, SelZone* zn, const uint32_t* __restrict__ histz, vo
         }
         zn->done = ok ? 1u : 0u;
         zn->why = ok ? 0u : why;
+        zn->mdone = mok ? 1u : 0u;
         if (path_out) *path_out = ok ? 1.0f : 0.0f;
+        if (mok) {
+            // sigma^2 gain^2 - gain - rn^2 / mt = 0, positive root, in the oracle's operation order (as sel_pick<2, 2>)
+            const float s2 = __fmul_rn(s, s);
+            const float aa = __fdiv_rn(__fmul_rn(__fmul_rn(4.0f, s2), rn2), mt);
+            const float g = __fdiv_rn(__fadd_rn(1.0f, __fsqrt_rn(__fadd_rn(1.0f, aa))), __fmul_rn(2.0f, s2));
+            *gain_out = (s > 0.0f && s < INF && g > 0.0f && g < INF) ? g : 1.0f;
+            if (stats) {
+                stats[0] = c; stats[1] = s; stats[2] = lo0; stats[3] = hi0; stats[4] = (float)nkept;
+                stats[5] = mt;
+            }
+        }
     }
 }
 
