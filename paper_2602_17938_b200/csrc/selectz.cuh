@@ -17,9 +17,12 @@
 //                   bounds are exact): if a check fails -- a frame of few distinct values, a plan that missed -- the
 //                   state says so and k_sel_rounds (select.cuh: the eighteen radix passes as one cooperative launch,
 //                   which otherwise returns at once) does the rounds over the plane.
-// The typical signal (rank (n-1)/2 of max(med5, 1e-4) over the kept set) then takes the three radix passes of
-// select.cuh over the med5 plane alone: the pixels outside the kept interval are all in the OUT list, whose
-// entries are subtracted from the histograms.
+// The typical signal (rank (n-1)/2 of max(med5, 1e-4) over the kept set) rides along: a second grid over max(med5,
+// 1e-4), its counts in k_selz_hist, ONE zone ZM around the positions the wanted element can have among all pixels
+// (every pixel outside the kept interval is in an OUT zone, so the position is known to within their number),
+// compacted in k_selz_compact and selected in k_selz_resolve as the zone list MINUS the OUT entries outside the kept
+// interval; the gain formula follows there.  If that fails, k_sel_rounds selects it by three radix passes over the med5
+// plane (the listed pixels outside the kept interval subtracted from the histograms).
 #pragma once
 #include <cooperative_groups.h>
 
