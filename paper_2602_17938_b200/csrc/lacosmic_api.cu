@@ -101,7 +101,7 @@ bool make_map(CUtensorMap* m, const float* base, int h, int w, int boxW, int box
 #define LAC_FG_WAVES 6
 #endif
 struct DeviceInfo {
-    int sms = 0, occ_noise = 0, occ_fine = 0, occ_quads = 0, occ_eval = 0;
+    int sms = 0, occ_noise = 0, occ_fine = 0, occ_quads = 0, occ_eval = 0, occ_rounds = 0;
     bool ok = false;
 };
 
@@ -134,7 +134,12 @@ DeviceInfo device_info() {
                                                       lac::NS_SMEM_BYTES) != cudaSuccess) return d;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_quads, lac::k_noise_S_quads, 256, 0) != cudaSuccess) return d;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_eval, lac::k_eval_candidates<0>, 128, 0) != cudaSuccess) return d;
-    d.ok = d.sms > 0 && d.occ_fine > 0 && d.occ_noise > 0 && d.occ_quads > 0 && d.occ_eval > 0;
+    // gain estimate: the grid of the cooperative k_sel_rounds must be resident as a whole; clusters of 16 CTAs
+    // (k_selz_resolve) are a non-portable size
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d.occ_rounds, lac::k_sel_rounds, 256, 0) != cudaSuccess) return d;
+    if (lac::SELZ_CLUSTER > 8 &&
+        cudaFuncSetAttribute(lac::k_selz_resolve, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) return d;
+    d.ok = d.sms > 0 && d.occ_fine > 0 && d.occ_noise > 0 && d.occ_quads > 0 && d.occ_eval > 0 && d.occ_rounds > 0;
     return d;
 }
 
@@ -255,8 +260,9 @@ bool gain_fast_enabled() {
 }
 int sigma_clip_gain(const float* R, const float* M5, size_t npx, const Workspace& ws, void* lists, size_t list_words,
                     float rn2, float* gain_out, float* stats, const int* prev, cudaStream_t st) {
-    int dev = 0, sms = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const DeviceInfo di = device_info();
+    if (!di.ok) { g_last_cuda_error = (int)cudaGetLastError(); return LACOSMIC_ERR_CUDA; }
+    const int sms = di.sms;
 #ifndef LAC_SEL_CTAS_PER_SM
 #define LAC_SEL_CTAS_PER_SM 8
 #endif
@@ -265,13 +271,6 @@ int sigma_clip_gain(const float* R, const float* M5, size_t npx, const Workspace
     // the lists of the fast path (selectz.cuh) live in the quad list's storage
     const float2* olist = lac::selz_carve(lists, list_words).o;
     const int grid_h = (int)std::min<size_t>((size_t)sms, (npx / 4 + 4 * lac::SELZ_HT - 1) / (4 * lac::SELZ_HT) + 1);
-    if (lac::SELZ_CLUSTER > 8) {              // once per device: clusters of 16 CTAs are a non-portable size
-        static bool allowed[MAX_DEVICES] = {};
-        if (dev >= 0 && dev < MAX_DEVICES && !allowed[dev]) {
-            CK(cudaFuncSetAttribute(lac::k_selz_resolve, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-            allowed[dev] = true;
-        }
-    }
     Span sp(KC_SELECT, st);
     lac::k_selz_init<<<1, lac::SELZ_IT, 0, st>>>(R, M5, npx, ws.sel, ws.zone, ws.hist, ws.histz, ws.histm,
                                                      gain_fast_enabled() ? 0 : 1, prev);
@@ -286,14 +285,7 @@ int sigma_clip_gain(const float* R, const float* M5, size_t npx, const Workspace
     {
         // the selections by radix passes over the planes: one cooperative launch, which returns at once when the fast
         // path has done them.  Its grid must be resident as a whole.
-        static int per_sm[MAX_DEVICES] = {};
-        if (dev < 0 || dev >= MAX_DEVICES) return LACOSMIC_ERR_CUDA;
-        if (!per_sm[dev]) {
-            int n = 0;
-            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, lac::k_sel_rounds, 256, 0));
-            per_sm[dev] = std::max(1, std::min(n, LAC_SEL_CTAS_PER_SM));
-        }
-        const int grid_c = std::min(grid, sms * per_sm[dev]);
+        const int grid_c = std::min(grid, sms * std::max(1, std::min(di.occ_rounds, LAC_SEL_CTAS_PER_SM)));
         const uint32_t *zdone = &ws.zone->done, *zmdone = &ws.zone->mdone, *zno = &ws.zone->no;
         void* args[] = {(void*)&R, (void*)&M5, (void*)&npx, (void*)&ws.sel, (void*)&ws.hist, (void*)&rn2, (void*)&gain_out,
                         (void*)&stats, (void*)&prev, (void*)&zdone, (void*)&zmdone, (void*)&zno, (void*)&olist};
