@@ -468,7 +468,7 @@ __device__ __forceinline__ void replicate_fix(float* sm, int oy, int ox, int h, 
 template <int CFG>
 __global__ void __launch_bounds__(NT, LAC_NS_MINB)
 k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx, int ntiles,
-              const int* prev_count) {
+              const int* prev_count, int tile0) {
     if (prev_count && *prev_count == 0) return;
     zero_counters(a);
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -482,8 +482,8 @@ k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx,
         fence_mbar_init();
     }
     __syncthreads();
-    const int nt = ntiles;
-    auto tile_of = [&](int i) { return i; };
+    const int nt = ntiles;                                  // this launch: tiles tile0 .. tile0 + ntiles - 1
+    auto tile_of = [&](int i) { return tile0 + i; };
     auto issue = [&](int t, int st) {
         int ty = t / ntx, tx = t - ty * ntx;
         mbar_expect_tx(&full[st], TILE_BYTES);

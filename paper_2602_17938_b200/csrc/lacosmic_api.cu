@@ -333,10 +333,19 @@ inline int check_variant(const lacosmic_variant* v) {
     return LACOSMIC_OK;
 }
 
+// A frame that is still arriving (lacosmic_run_host*): rows [0, row_end[b]) of img are on the device once ready[b] has
+// fired.  The first noise/S pass is then launched band by band behind the copies instead of behind the whole frame.
+constexpr int MAX_BANDS = 8;
+struct BandSync {
+    int n = 0;
+    cudaEvent_t ready[MAX_BANDS];
+    int row_end[MAX_BANDS];
+};
+
 // The iteration loop (O0-O7) for one frame.  vr: nullable variants (R22-R25).
 int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t* mask_out,
               float* clean_out, const Workspace& ws, int32_t* iter_counts, const lacosmic_debug* dbg,
-              cudaStream_t st, const lacosmic_variant* vr = nullptr) {
+              cudaStream_t st, const lacosmic_variant* vr = nullptr, const BandSync* bands = nullptr) {
     const size_t P = (size_t)h * w;
     const int wpr = words_per_row(w);
     const size_t bp_bytes = (size_t)h * wpr * 4;
@@ -410,22 +419,49 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
         const bool d = dbg && dbg->iter == t;
         int rc = LACOSMIC_OK;
         const float* src = (fused_copy && t == 0) ? img : work;
-        auto noise_pass = [&](const lac::NoiseArgs& na, const float* from) -> int {
-            Span sp(KC_NOISE_S, st);
-            if (tma) {
-                // the two configurations of a plain frame are compiled without the tests of the nullable outputs
-                const CUtensorMap& map = from == img ? mapImgNS : mapWorkNS;
-                const bool plain = !na.dbgLp && !na.dbgN && !na.R && !na.gain_dev;
-                if (plain && na.copy_out && na.A1 && na.mask_zero) lac::k_noise_S_tma<7><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
-                else if (plain && na.copy_out && na.A1 && !na.mask_zero) lac::k_noise_S_tma<3><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
-                else if (plain && !na.copy_out && !na.A1 && !na.mask_zero) lac::k_noise_S_tma<0><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
-                else if (na.R && !na.dbgLp && !na.dbgN && !na.gain_dev && !na.A1 && !na.mask_zero && !na.var && na.copy_out) lac::k_noise_S_tma<9><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
-                else if (na.R && !na.dbgLp && !na.dbgN && !na.gain_dev && !na.A1 && !na.mask_zero && !na.var && !na.copy_out) lac::k_noise_S_tma<8><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
-                else lac::k_noise_S_tma<-1><<<gridNS, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, ntilesNS, prev);
-            }
-            else lac::k_noise_S<<<ntilesNS, tb, 0, st>>>(from, na, ntx, prev);
+        // tiles tile0 .. tile0 + nt - 1 of the noise/S pass (TMA path; the generic path always runs the whole frame)
+        auto noise_tiles = [&](const lac::NoiseArgs& na, const float* from, int tile0, int nt) -> int {
+            const CUtensorMap& map = from == img ? mapImgNS : mapWorkNS;
+            const int g = std::min(nt, gridNS);
+            // the configurations of a plain frame are compiled without the tests of the nullable outputs
+            const bool plain = !na.dbgLp && !na.dbgN && !na.R && !na.gain_dev;
+            const bool resid = na.R && !na.dbgLp && !na.dbgN && !na.gain_dev && !na.A1 && !na.mask_zero && !na.var;
+            if (plain && na.copy_out && na.A1 && na.mask_zero) lac::k_noise_S_tma<7><<<g, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, nt, prev, tile0);
+            else if (plain && na.copy_out && na.A1 && !na.mask_zero) lac::k_noise_S_tma<3><<<g, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, nt, prev, tile0);
+            else if (plain && !na.copy_out && !na.A1 && !na.mask_zero) lac::k_noise_S_tma<0><<<g, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, nt, prev, tile0);
+            else if (resid && na.copy_out) lac::k_noise_S_tma<9><<<g, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, nt, prev, tile0);
+            else if (resid && !na.copy_out) lac::k_noise_S_tma<8><<<g, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, nt, prev, tile0);
+            else lac::k_noise_S_tma<-1><<<g, tb, lac::NS_SMEM_BYTES, st>>>(map, na, ntx, nt, prev, tile0);
             LAUNCHED();
             return LACOSMIC_OK;
+        };
+        auto noise_pass = [&](const lac::NoiseArgs& na, const float* from) -> int {
+            Span sp(KC_NOISE_S, st);
+            if (!tma) {
+                lac::k_noise_S<<<ntilesNS, tb, 0, st>>>(from, na, ntx, prev);
+                LAUNCHED();
+                return LACOSMIC_OK;
+            }
+            if (bands && t == 0 && from == img && bands->n > 0) {
+                // the frame is still arriving: a row of tiles (NS_TH rows + 2 rows of margin below) runs as soon as the
+                // band that holds its last input row is on the device
+                const int ntyNS = ntilesNS / ntx;
+                int done = 0;                          // rows of tiles launched so far
+                for (int b = 0; b < bands->n; ++b) {
+                    CK(cudaStreamWaitEvent(st, bands->ready[b], 0));
+                    const int re = bands->row_end[b];
+                    int upto = re >= h ? ntyNS : (re - lac::NS_MY) / lac::NS_TH;     // rows of tiles wholly fed by rows < re
+                    upto = std::max(done, std::min(upto, ntyNS));
+                    if (upto > done) {
+                        int rc2 = noise_tiles(na, from, done * ntx, (upto - done) * ntx);
+                        if (rc2) return rc2;
+                        done = upto;
+                    }
+                }
+                if (done < ntyNS) return noise_tiles(na, from, done * ntx, (ntyNS - done) * ntx);
+                return LACOSMIC_OK;
+            }
+            return noise_tiles(na, from, 0, ntilesNS);
         };
         if (estimate) {
             // R21: the gain of this iteration from its input image.  One dense pass writes the residual plane
@@ -604,6 +640,8 @@ struct BatchStreams {
     int dev = -1;
     cudaStream_t st[LACOSMIC_MAX_BATCH_STREAMS];
     cudaEvent_t fork, join[LACOSMIC_MAX_BATCH_STREAMS];
+    cudaStream_t copy;                  // H2D copies of a single host frame, band by band (run_host_frame)
+    cudaEvent_t band[MAX_BANDS];
 };
 BatchStreams* batch_streams() {
     thread_local BatchStreams pool[16];
@@ -619,6 +657,9 @@ BatchStreams* batch_streams() {
         if (!cuda_ok(cudaStreamCreateWithFlags(&b.st[s], cudaStreamNonBlocking))) return nullptr;
         if (!cuda_ok(cudaEventCreateWithFlags(&b.join[s], cudaEventDisableTiming))) return nullptr;
     }
+    if (!cuda_ok(cudaStreamCreateWithFlags(&b.copy, cudaStreamNonBlocking))) return nullptr;
+    for (int k = 0; k < MAX_BANDS; ++k)
+        if (!cuda_ok(cudaEventCreateWithFlags(&b.band[k], cudaEventDisableTiming))) return nullptr;
     b.dev = dev;
     ++npool;
     return &b;
@@ -922,7 +963,10 @@ struct HostFrame {
 };
 
 // one frame through a staging slot: H2D, the path, D2H (slot layout: img | clean | mask | workspace)
-int run_host_frame(const HostFrame& io, int h, int w, const lacosmic_params& p, void* slot, cudaStream_t st) {
+// banded: the frame is the only one in flight on this thread's internal copy stream (single-frame entry points), so its
+// H2D copy may run there in bands, the first noise/S pass following band by band (hides that pass behind the copy)
+int run_host_frame(const HostFrame& io, int h, int w, const lacosmic_params& p, void* slot, cudaStream_t st,
+                   bool banded = false) {
     size_t P = (size_t)h * w, plane = align_up(P * 4, 256);
     char* base = (char*)slot;
     float* d_img = (float*)base;
@@ -935,10 +979,33 @@ int run_host_frame(const HostFrame& io, int h, int w, const lacosmic_params& p, 
         CK(cudaMemcpyAsync(d_raw, io.img, P * 2, cudaMemcpyHostToDevice, st));
         k_u16_to_f32<<<(unsigned)((P + 2047) / 2048), 256, 0, st>>>(d_raw, d_img, P);
         LAUNCHED();
-    } else {
+    }
+    BandSync bands;
+#ifndef LAC_HOST_BANDS
+#define LAC_HOST_BANDS 8
+#endif
+    const int nty = (h + lac::NS_TH - 1) / lac::NS_TH;
+    BatchStreams* bs = nullptr;
+    if (!io.u16 && banded && p.mode == LACOSMIC_MODE_LAZY && p.niter > 0 && p.gain != 0.0f && (w % 4) == 0 &&
+        nty >= 4 * LAC_HOST_BANDS && (bs = batch_streams())) {
+        const float* src = (const float*)io.img;
+        CK(cudaEventRecord(bs->fork, st));                 // the slot is free once the caller's earlier work is done
+        CK(cudaStreamWaitEvent(bs->copy, bs->fork, 0));
+        int r0 = 0;
+        for (int b = 0; b < LAC_HOST_BANDS; ++b) {
+            const int r1 = b == LAC_HOST_BANDS - 1 ? h : std::min(h, (int)((long long)nty * (b + 1) / LAC_HOST_BANDS) * lac::NS_TH);
+            CK(cudaMemcpyAsync(d_img + (size_t)r0 * w, src + (size_t)r0 * w, (size_t)(r1 - r0) * w * 4, cudaMemcpyHostToDevice, bs->copy));
+            CK(cudaEventRecord(bs->band[b], bs->copy));
+            bands.ready[b] = bs->band[b];
+            bands.row_end[b] = r1;
+            r0 = r1;
+        }
+        bands.n = LAC_HOST_BANDS;
+    } else if (!io.u16) {
         CK(cudaMemcpyAsync(d_img, io.img, P * 4, cudaMemcpyHostToDevice, st));
     }
-    int rc = run_frame(d_img, h, w, p, io.mask ? d_mask : nullptr, d_clean, ws, nullptr, nullptr, st);
+    int rc = run_frame(d_img, h, w, p, io.mask ? d_mask : nullptr, d_clean, ws, nullptr, nullptr, st, nullptr,
+                       bands.n ? &bands : nullptr);
     if (rc) return rc;
     if (io.mask) {
         CK(cudaMemcpyAsync(io.clean, d_clean, P * 4, cudaMemcpyDeviceToHost, st));
@@ -1011,7 +1078,7 @@ int lacosmic_run_host(const float* img_host, int h, int w, const lacosmic_params
     if ((uintptr_t)dev_workspace & 255) return LACOSMIC_ERR_ALIGN;
     if (dev_workspace_bytes < lacosmic_host_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
     return run_host_frame(HostFrame{img_host, false, mask_out_host, clean_out_host, nullptr, nullptr, nullptr, nullptr, 0},
-                          h, w, *p, dev_workspace, (cudaStream_t)stream);
+                          h, w, *p, dev_workspace, (cudaStream_t)stream, true);
 }
 
 int lacosmic_run_host_u16(const uint16_t* img_host, int h, int w, const lacosmic_params* p,
@@ -1041,7 +1108,7 @@ int lacosmic_run_host_sparse(const float* img_host, int h, int w, const lacosmic
     if ((uintptr_t)dev_workspace & 255) return LACOSMIC_ERR_ALIGN;
     if (dev_workspace_bytes < lacosmic_host_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
     return run_host_frame(HostFrame{img_host, false, nullptr, nullptr, maskbits_host, idx_host, val_host, count_host, capacity},
-                          h, w, *p, dev_workspace, (cudaStream_t)stream);
+                          h, w, *p, dev_workspace, (cudaStream_t)stream, true);
 }
 
 int lacosmic_run_host_stream_sparse(const void* imgs_host, int input_is_u16, int n, int h, int w,
