@@ -180,7 +180,10 @@ int lacosmic_run_batch(const float *imgs, int n, int h, int w, const lacosmic_pa
  * (pinned memory makes the copies asynchronous); the call enqueues H2D copy, the whole path and
  * the D2H copies on `stream`.  dev_workspace: device scratch of at least
  * lacosmic_host_workspace_bytes(h,w) bytes (frame staging + lacosmic_workspace_bytes), 256-byte
- * aligned.  Results are valid after the caller synchronises `stream`. */
+ * aligned.  Results are valid after the caller synchronises `stream`.  For frames of at least 1024 rows (lazy mode,
+ * gain supplied, w % 4 == 0) the H2D copy is issued in eight bands on a copy stream the library keeps per calling thread
+ * and device (ordered after the work already on `stream`), and the first pass of the path follows it band by band on
+ * `stream`; the img_host buffer must stay unchanged until `stream` has been synchronised, as for any asynchronous copy. */
 size_t lacosmic_host_workspace_bytes(int h, int w);
 int lacosmic_run_host(const float *img_host, int h, int w, const lacosmic_params *p,
                       uint8_t *mask_out_host, float *clean_out_host, void *dev_workspace,
