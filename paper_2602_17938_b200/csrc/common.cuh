@@ -8,6 +8,16 @@ namespace lac {
 
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return min(max(v, lo), hi); }
 
+// Programmatic dependent launch (the kernels of a lazy frame are launched with the programmatic-stream-serialization
+// attribute): let the NEXT kernel of the stream be scheduled while this one runs, then wait until the PREVIOUS one has
+// completed and its writes are visible.  Every thread calls this before its first global access, so the frame's kernels
+// still execute in order; what overlaps is the launch and the scheduling of the next grid with the tail of this one.
+// Without the attribute both instructions do nothing.
+__device__ __forceinline__ void pdl_entry() {
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 // 2-D CTA coordinates out of a 1-D grid of nbx * nby CTAs: gridDim.y stops at 65535, which a tall, narrow frame
 // (rows on y) would exceed; gridDim.x reaches 2^31 - 1, enough for every shape the boundary accepts.
 struct BlockXY { int x, y; };

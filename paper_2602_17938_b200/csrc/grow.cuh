@@ -113,6 +113,7 @@ struct GrowArgs {
 #endif
 __global__ void __launch_bounds__(32 * WG_WARPS, LAC_GROW_MINB)
 k_grow_replace(GrowArgs a, const int* prev_count) {
+    pdl_entry();
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const int h = a.h, w = a.w, wpr = a.wpr;
     const BlockXY bk = block_xy(a.nbx);
@@ -379,6 +380,7 @@ k_dirty_lists(const uint32_t* __restrict__ NEED, const uint32_t* __restrict__ A1
               uint32_t* __restrict__ G2, uint32_t* __restrict__ G2F, uint32_t* __restrict__ M1,
               int* __restrict__ qlist, int* __restrict__ nq, int* __restrict__ clist, int* __restrict__ nc,
               int h, int w, int wpr, int nbx, const int* prev_count) {
+    pdl_entry();
     const int pc = prev_count ? *prev_count : 1;             // tested below, after the NEED loads have been issued
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const BlockXY bk = block_xy(nbx);

@@ -469,6 +469,7 @@ template <int CFG>
 __global__ void __launch_bounds__(NT, LAC_NS_MINB)
 k_noise_S_tma(const __grid_constant__ CUtensorMap mapWork, NoiseArgs a, int ntx, int ntiles,
               const int* prev_count, int tile0) {
+    pdl_entry();
     if (prev_count && *prev_count == 0) return;
     zero_counters(a);
     extern __shared__ __align__(128) unsigned char smem_raw[];

@@ -35,6 +35,7 @@ __global__ void __launch_bounds__(256)
 k_list_candidates(const uint32_t* __restrict__ A1, const uint32_t* __restrict__ dirty, uint32_t* __restrict__ G1,
                   uint32_t* __restrict__ G2, uint32_t* __restrict__ G2F, uint32_t* __restrict__ M1, int* __restrict__ list,
                   int* __restrict__ nlist, uint32_t* __restrict__ Czero, int h, int w, int wpr, int nbx, const int* prev_count) {
+    pdl_entry();
     if (prev_count && *prev_count == 0) return;
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
     const BlockXY bk = block_xy(nbx);
@@ -189,6 +190,7 @@ template <int FS>
 __global__ void __launch_bounds__(128, LAC_EVAL_MINB)
 k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restrict__ nlist,
                   const int* prev_count) {
+    pdl_entry();
     // the two counters are read together (one round trip, not two dependent ones, in front of the list)
     const int pc = prev_count ? *prev_count : 1;
     const int n0 = *nlist;
@@ -270,6 +272,7 @@ k_eval_candidates(CandArgs a, const int* __restrict__ list, const int* __restric
 __global__ void __launch_bounds__(256, 4)
 k_noise_S_quads(const float* __restrict__ work, NoiseArgs a, const int* __restrict__ qlist,
                 const int* __restrict__ nq, int* __restrict__ clist, int* __restrict__ nc, const int* prev_count) {
+    pdl_entry();
     __shared__ int s_warp[8];
     __shared__ int s_base;
     const int pc = prev_count ? *prev_count : 1;      // read together with the list length: one round trip
