@@ -3,7 +3,8 @@
 // with TWO reads of the residual plane instead of eighteen.  The answer is the same element, bit for bit:
 //
 //   k_selz_init     a strided sample of 128 residuals gives a rough centre and scale (its median and MAD); they
-//                   only place a grid of 4096 value-linear buckets over the plane's values.
+//                   only place a grid of 4096 value-linear buckets over the plane's values (any grid gives the same
+//                   answer).
 //   k_selz_hist     read 1: exact counts of every bucket (shared-memory histograms).  The CTA that finishes last
 //                   PLANS: from the cumulative counts it follows the three rounds at bucket resolution and marks
 //                   five ZONES of buckets -- Z0 around the centres, Z- / Z+ around c -/+ d, OUT- / OUT+ beyond
@@ -99,8 +100,8 @@ __device__ __forceinline__ int selz_bucket(float r, float base, float scale) {
     return min(max(__float2int_rd(__fmul_rn(__fsub_rn(r, base), scale)), 0), SELZ_NB - 1);
 }
 
-// One CTA of SELZ_SAMPLE threads: state, histograms, and the bucket grid from a strided sample of the plane (the median and
-// the MAD of the sample by rank counting: thread i counts the sample values below its own).
+// One CTA of SELZ_IT threads: all clear the histograms; the first SELZ_SAMPLE take a strided sample of the two planes and
+// place the two bucket grids by its medians and MADs (rank counting: thread i counts the sample values below its own).
 __global__ void __launch_bounds__(SELZ_IT)
 k_selz_init(const float* __restrict__ R, const float* __restrict__ M5, size_t npx, SelState* st, SelZone* zn, uint32_t* hist,
             uint32_t* histz, uint32_t* histm, int force_classic, const int* prev_count) {
