@@ -47,7 +47,8 @@ REF_COMPARISONS_PER_PX_ITER = 19 + 99 + 99 + 480
 # dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture
 # (profiles/; None until captured)
 NCU_TRAFFIC_BYTES = {"fine_gates": 239900000,      # dense mode: profiles/r01_v9_ncu_full_dense.md
-                     "noise_S": 269300000}         # lazy mode (with the work = img_in copy): profiles/r01_v9_ncu_full.md
+                     "noise_S": 288200000}         # lazy mode (with the work = img_in copy and the cleared uint8 mask):
+                                                   # profiles/r02_ncu_full.md, launch 0 (104.5 MB read + 183.7 MB written)
 
 
 def _peaks():
@@ -543,8 +544,9 @@ def run_cuda(args):
                 break
             ncand, nq, nrep, nfine = st["candidates"][t], st["quads"][t], st["replaced"][t], st["fine_tests"][t]
             if t == 0:
-                # read img 4, write S 4 + work 4, A1/A2; med5 network 326 + 16 clip min/max per 4 pixels
-                add("noise_S", t, npx * 12 + 2 * bp, npx * KERNEL_MINMAX_PER_PX["noise_S"])
+                # read img 4, write S 4 + work 4 + the cleared uint8 mask 1, A1/A2; med5 network 554 + 32 clip min/max per
+                # 8 pixels
+                add("noise_S", t, npx * 13 + 2 * bp, npx * KERNEL_MINMAX_PER_PX["noise_S"])
                 add("list_candidates", t, bp + 5 * bp + 4 * ncand, 0)       # A1 read, G1/G2/G2F/M1/C cleared, list
             else:
                 add("dirty_lists", t, bp + 4 * nq + 4 * ncand, 0)           # NEED read, lists written
@@ -557,8 +559,8 @@ def run_cuda(args):
             # bit-planes M1 G1 G2 C A1 A2 G2F read, C' NEED written (t = 0; later iterations M1 + C carried over); per
             # replaced pixel 25 taps + 1 store and the 25-input sorting network (276 min/max)
             planes = 9 * bp if t == 0 else 4 * bp
-            add("grow_replace", t, planes + min(nrep * 100, plane) + nrep * 4, nrep * 276)
-        add("unpack_bits", niter, bp + npx, 0)
+            # (the flagged pixels are set in the uint8 mask directly: 1 more byte per replaced pixel, no unpack launch)
+            add("grow_replace", t, planes + min(nrep * 100, plane) + nrep * 5, nrep * 276)
         total_us = sum(max(x["t_hbm_us"], x["t_alu_us"]) for x in terms)
         return dict(step_frac=total_us / (ms_step * 1e3), bound_us=total_us, step_us=ms_step * 1e3,
                     bw_gbs=peaks["hbm_gbs"], alu_peak_T=probe["fmnmx"],
