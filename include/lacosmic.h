@@ -48,6 +48,7 @@ extern "C" {
 #define LACOSMIC_ERR_ALIAS (-5)     /* img, mask_out, clean_out (or workspace) overlap */
 #define LACOSMIC_ERR_WORKSPACE (-6) /* workspace_bytes smaller than lacosmic_workspace_bytes(h, w) */
 #define LACOSMIC_ERR_CUDA (-7)      /* a CUDA call failed; see lacosmic_last_cuda_error() */
+#define LACOSMIC_ERR_TOO_LARGE (-8) /* frame larger than the built-in scratch of lacosmic_masked_median_noalloc */
 
 #define LACOSMIC_MAX_NITER 64
 
@@ -291,6 +292,41 @@ int lacosmic_masked_median(const float *img, const uint8_t *mask_u8, float *out,
 /* Step (7) with bad pixels removed from the donors (R23); bpm_u8 nullable (then lacosmic_masked_median). */
 int lacosmic_masked_median_bpm(const float *img, const uint8_t *mask_u8, const uint8_t *bpm_u8, float *out, int h,
                                int w, void *workspace, size_t workspace_bytes, void *stream);
+
+/* ---- step (7) for callers that cannot allocate device memory ----------------------------------- */
+
+/* Some code that wants step (7) has no way to obtain scratch memory for it: a plug-in running inside a host
+ * application that owns the GPU's memory pool and hands out only the input and output buffers; a real-time loop
+ * that may not enter the allocator (cudaMalloc can block, and synchronises the device) once it has started; a
+ * process whose memory budget was fixed at start-up and is used up.  Every other entry point of this library
+ * that needs scratch takes a `workspace` the caller must have allocated, or (lacosmic_run) draws from the
+ * stream-ordered pool.  This one needs neither: its scratch -- five bit-planes and a counter -- is a fixed array
+ * inside the library's own device image.
+ *
+ * Same operation and same kernels as lacosmic_masked_median_bpm (bpm_u8 nullable), same results bit for bit:
+ * out = img where mask_u8 == 0, else the median of the unmasked (and not bad) 5x5 edge-replicated neighbours.
+ * img, mask_u8, bpm_u8, out are the caller's DEVICE buffers ([h][w]; img and out must not overlap).
+ *
+ * Limit: h * lacosmic_bitplane_pitch_words(w) <= LACOSMIC_NOALLOC_MAX_WORDS (131072 words: any frame up to 2048 x 2048
+ * pixels, or e.g. 1024 x 4096).  A larger frame returns LACOSMIC_ERR_TOO_LARGE and enqueues nothing.  The array
+ * occupies LACOSMIC_NOALLOC_SCRATCH_BYTES (2.5 MiB + 256 bytes) of every GPU on which the process loads this library, from the
+ * moment the library's device code is loaded there until the process exits, whether or not this call is ever made.
+ *
+ * The call itself makes no cudaMalloc / cudaFree / cudaMallocAsync and calls no routine that allocates: it enqueues
+ * two or three small kernels, one device-to-device copy and two memsets on `stream`.  The FIRST call on each device
+ * also looks up the array's address on that device (cudaGetSymbolAddress, with that device current; the result is
+ * kept per device under a lock).  That look-up may make the CUDA runtime load the library's device code, so make
+ * the first call on a device during set-up, before any stream capture and before the phase that must not allocate.
+ *
+ * There is ONE array per GPU and every call on that GPU uses it, from whichever thread or stream.  Calls that are
+ * ordered on the GPU (same stream, or streams ordered by events) are safe: each call re-initialises the parts it
+ * relies on and never reads what an earlier call left behind.  Two calls that can run on the GPU at the same time
+ * (different streams with no ordering between them) race on the array and give undefined results: serialise them
+ * yourself, or use lacosmic_masked_median_bpm with one workspace per stream. */
+#define LACOSMIC_NOALLOC_MAX_WORDS 131072
+#define LACOSMIC_NOALLOC_SCRATCH_BYTES (5 * LACOSMIC_NOALLOC_MAX_WORDS * 4 + 256)
+int lacosmic_masked_median_noalloc(const float *img, const uint8_t *mask_u8, const uint8_t *bpm_u8, float *out,
+                                   int h, int w, void *stream);
 
 /* R25 alone: out_u8[h][w] = 1 on dil3^grow(med5(img) >= satlevel), else 0.  workspace as for lacosmic_run_ws. */
 int lacosmic_satstar_mask(const float *img, int h, int w, float satlevel, int grow, uint8_t *out_u8, void *workspace,

@@ -27,8 +27,10 @@ EXPORTS = (
     "lacosmic_kernel_timing_enable", "lacosmic_kernel_timing_read", "lacosmic_kernel_class_name",
     "lacosmic_probe_minmax_rate", "lacosmic_stats_enable", "lacosmic_frame_stats", "lacosmic_graph_replay_enable", "lacosmic_gain_fast_path_enable", "lacosmic_gain_zone_info",
     "lacosmic_run_ex", "lacosmic_sepmed_workspace_bytes", "lacosmic_run_sepmed_compare", "lacosmic_sepmedfilt",
-    "lacosmic_masked_median_bpm", "lacosmic_satstar_mask",
+    "lacosmic_masked_median_bpm", "lacosmic_satstar_mask", "lacosmic_masked_median_noalloc",
 )
+NOALLOC_MAX_WORDS = 131072       # include/lacosmic.h LACOSMIC_NOALLOC_MAX_WORDS
+ERR_TOO_LARGE = -8
 NUM_KERNEL_CLASSES = 9
 MODE_LAZY, MODE_DENSE = 0, 1
 FS_ADU, FS_NORMALISED = 0, 1
@@ -136,6 +138,7 @@ def load_library():
         "lacosmic_sepmedfilt": (i, [vp, vp, vp, i, i, i, vp]),
         "lacosmic_masked_median_bpm": (i, [vp, vp, vp, vp, i, i, vp, sz, vp]),
         "lacosmic_satstar_mask": (i, [vp, i, i, f, i, vp, vp, sz, vp]),
+        "lacosmic_masked_median_noalloc": (i, [vp, vp, vp, vp, i, i, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)      # AttributeError if the header and the library disagree
@@ -639,6 +642,26 @@ def lacosmic_masked_median(img, mask_u8, out=None, workspace=None, stream=None, 
 
 
 lacosmic_masked_median_bpm = lacosmic_masked_median
+
+
+def lacosmic_masked_median_noalloc(img, mask_u8, out, bpm=None, stream=None):
+    """Step (7) for a caller that cannot allocate device memory (a plug-in inside an application that owns the GPU
+    memory pool, a real-time loop that must stay out of the allocator, a process at its memory budget): the scratch
+    is a fixed array inside the library instead of a workspace.  `out` is required -- this wrapper allocates nothing
+    either.  Same result as lacosmic_masked_median(img, mask_u8, bpm=bpm), bit for bit.
+
+    Limit: h * ceil(w / 32) <= NOALLOC_MAX_WORDS (any frame up to 2048 x 2048); larger frames raise LacosmicError with
+    code ERR_TOO_LARGE and leave `out` untouched.  All calls on one GPU share the one array: calls ordered on the GPU
+    (same stream) are fine, calls that may overlap on the GPU race.  The first call on a device looks the array's
+    address up; make it during set-up."""
+    torch = _torch()
+    h, w = img.shape
+    rc = load_library().lacosmic_masked_median_noalloc(
+        _dev(img, torch.float32, "img"), _dev(mask_u8, torch.uint8, "mask_u8", (h, w)),
+        None if bpm is None else _dev(bpm, torch.uint8, "bpm", (h, w)),
+        _dev(out, torch.float32, "out", (h, w)), h, w, _stream(stream))
+    _check(rc, "lacosmic_masked_median_noalloc")
+    return out
 
 
 def lacosmic_strerror(code):

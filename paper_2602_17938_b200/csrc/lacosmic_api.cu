@@ -1362,6 +1362,7 @@ const char* lacosmic_strerror(int code) {
         case LACOSMIC_ERR_ALIAS: return "buffers overlap";
         case LACOSMIC_ERR_WORKSPACE: return "workspace too small";
         case LACOSMIC_ERR_CUDA: return "CUDA call failed (see lacosmic_last_cuda_error)";
+        case LACOSMIC_ERR_TOO_LARGE: return "frame exceeds the built-in scratch (h * ceil(w/32) <= 131072 words); use the workspace variant";
         default: return "unknown error code";
     }
 }
@@ -1470,3 +1471,72 @@ int lacosmic_last_launch_count(void) { return g_launches; }
 const char* lacosmic_version(void) { return "lacosmic-b200 0.3 (sm_100a)"; }
 
 }  // extern "C"
+
+// ---- step (7) without any allocation (include/lacosmic.h, lacosmic_masked_median_noalloc) -----------------
+// For callers that cannot bring a workspace: the five bit-planes and the counter that lacosmic_masked_median_bpm
+// carves out of the caller's workspace live in a fixed array of this library's device image instead.  The array
+// exists once per GPU that loads the library and is shared by every call on that GPU.
+//
+// In host code the NAME of a __device__ array is only a handle for the runtime's symbol functions, not a device
+// address; handing `g_noalloc_scratch` itself to a kernel or to cudaMemsetAsync would make the GPU touch unrelated
+// memory.  noalloc_scratch() asks the runtime for the real address on the current device and keeps it.
+namespace {
+
+constexpr size_t NA_PLANE_WORDS = LACOSMIC_NOALLOC_MAX_WORDS;     // stride between planes: 512 KiB, keeps 256-byte alignment
+constexpr int NA_PLANES = 5;                                       // M1, DONX, C[0], C[1], NEED
+constexpr size_t NA_WORDS = NA_PLANES * NA_PLANE_WORDS + 64;       // + 256 bytes for the counter
+static_assert(NA_WORDS * 4 == LACOSMIC_NOALLOC_SCRATCH_BYTES, "header and library disagree");
+static __device__ __align__(256) uint32_t g_noalloc_scratch[NA_WORDS];
+
+// Device address of g_noalloc_scratch on the CURRENT device (nullptr if the look-up fails; the CUDA error is kept for
+// lacosmic_last_cuda_error).  One look-up per device, under a lock, with that device current.
+uint32_t* noalloc_scratch() {
+    static uint32_t* addr[MAX_DEVICES];
+    static std::mutex mu;
+    int dev = 0;
+    if (!cuda_ok(cudaGetDevice(&dev))) return nullptr;
+    if (dev < 0 || dev >= MAX_DEVICES) { g_last_cuda_error = (int)cudaErrorInvalidDevice; return nullptr; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        uint32_t* ptr = nullptr;
+        if (!cuda_ok(cudaGetSymbolAddress((void**)&ptr, g_noalloc_scratch)) || !ptr) return nullptr;
+        addr[dev] = ptr;
+    }
+    return addr[dev];
+}
+
+}  // namespace
+
+extern "C" int lacosmic_masked_median_noalloc(const float* img, const uint8_t* mask_u8, const uint8_t* bpm_u8, float* out,
+                                              int h, int w, void* stream) {
+    g_launches = 0;
+    if (!img || !mask_u8 || !out) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    const int wpr = words_per_row(w);
+    const size_t words = (size_t)h * wpr, P = (size_t)h * w;
+    if (words > NA_PLANE_WORDS) return LACOSMIC_ERR_TOO_LARGE;       // nothing enqueued, `out` untouched
+    if (overlap(img, P * 4, out, P * 4)) return LACOSMIC_ERR_ALIAS;
+    uint32_t* base = noalloc_scratch();                               // first call on this device: the address look-up
+    if (!base) return LACOSMIC_ERR_CUDA;
+    uint32_t* M1 = base;
+    uint32_t* DONX = base + NA_PLANE_WORDS;
+    uint32_t* C0 = base + 2 * NA_PLANE_WORDS;
+    uint32_t* C1 = base + 3 * NA_PLANE_WORDS;
+    uint32_t* NEED = base + 4 * NA_PLANE_WORDS;
+    int* count = (int*)(base + NA_PLANES * NA_PLANE_WORDS);
+    cudaStream_t st = (cudaStream_t)stream;
+    // The array still holds whatever the previous call (any shape, any stream) left in it.  M1 and DONX are written in
+    // full by the packing kernels, C1 and NEED by k_grow_replace before anything reads them; what the kernel expects to
+    // find at zero -- the old cumulative mask C0 and the counter it adds to -- is cleared here, on every call.
+    if ((rc = pack_bits(mask_u8, M1, h, w, nullptr, st))) return rc;
+    if (bpm_u8 && (rc = pack_bits(bpm_u8, DONX, h, w, nullptr, st))) return rc;
+    CK(cudaMemcpyAsync(out, img, P * 4, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemsetAsync(C0, 0, words * 4, st));
+    CK(cudaMemsetAsync(count, 0, 4, st));
+    // as in lacosmic_masked_median_bpm: with M1 = G1 = G2 = mask and C = 0 the fused kernel flags exactly the mask and
+    // replaces every pixel of it
+    lac::GrowArgs ga{M1, M1, M1, nullptr, nullptr, nullptr, C0, C1, NEED, nullptr, nullptr,
+                     nullptr, img, out, count, 0, h, w, wpr, 0.0f, grow_nbx(w), bpm_u8 ? DONX : nullptr, nullptr, nullptr};
+    return grow_replace(ga, nullptr, st);
+}
