@@ -35,8 +35,8 @@ import numpy as np  # noqa: E402
 from paper_2602_17938_b200 import replicas, synth  # noqa: E402
 
 METRIC = "frames/s, 4000x6500 fp32 L.A.Cosmic (niter=4)"
-# ALU-pipe roofline: FMNMX/FMNMX3 issue at 64 lanes/clk/SM (measured,
-# profiles/r01_alu_minmax_microbench.txt) -> 148 SM x 64 x clocks.max.sm.
+# ALU-pipe roofline: FMNMX/FMNMX3 issue at 64 lanes/clk/SM (measured in every run by
+# lacosmic_probe_minmax_rate, csrc/probe.cuh; profiles/r02_alu_probe.md) -> 148 SM x 64 x clocks.max.sm.
 ALU_LANES_PER_CLK_SM = 64
 N_SM = 148
 # min/max (ALU-pipe FMNMX) instructions the dominant kernel executes per output pixel, from its SASS
@@ -44,11 +44,18 @@ N_SM = 148
 FINE_GATES_MINMAX_PER_PX = None   # filled from the library's own accounting below
 # reference compare-exchanges per pixel per iteration with per-pixel networks:
 REF_COMPARISONS_PER_PX_ITER = 19 + 99 + 99 + 480
-# dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture
-# (profiles/; None until captured)
-NCU_TRAFFIC_BYTES = {"fine_gates": 239900000,      # dense mode: profiles/r01_v9_ncu_full_dense.md
-                     "noise_S": 288200000}         # lazy mode (with the work = img_in copy and the cleared uint8 mask):
-                                                   # profiles/r02_ncu_full.md, launch 0 (104.5 MB read + 183.7 MB written)
+# dram bytes per launch of the dominant kernel, read from profiles/ncu_traffic.json, which
+# `python -m paper_2602_17938_b200.ncu_summary full ... --traffic profiles/ncu_traffic.json` writes from a committed
+# `ncu --set full` capture (keys: noise_S = lazy mode, fine_gates = dense mode); absent -> traffic is null
+def _ncu_traffic():
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    try:
+        return json.load(open(path))
+    except (OSError, ValueError):
+        return {}
+
+
+NCU_TRAFFIC = _ncu_traffic()
 
 
 def _peaks():
@@ -355,10 +362,9 @@ def run_cuda(args):
         nf = args.stream_frames
         cfg = synth.stream_config(nf)
         imgs = torch.empty((nf, h, w), dtype=torch.float32, device=dev)
-        for j, (kwj, _) in enumerate(cfg):
-            kwj = dict(kwj)
-            kwj["seed"] = replicas.rank_seed(kwj["seed"], rank)
-            imgs[j].copy_(torch.from_numpy(synth.make_frame(**kwj).img))
+        kws = [dict(kwj, seed=replicas.rank_seed(kwj["seed"], rank)) for kwj, _ in cfg]
+        for j, fimg in enumerate(synth.make_images(kws)):
+            imgs[j].copy_(torch.from_numpy(fimg))
         plist = [lc.Params(mode=lc.MODE_LAZY, **pj) for _, pj in cfg]
         masks = torch.empty((nf, h, w), dtype=torch.uint8, device=dev)
         cleans = torch.empty_like(imgs)
@@ -394,6 +400,19 @@ def run_cuda(args):
         lc.lacosmic_run_host(img_h, P[main_mode], mask_out_host=mask_h, clean_out_host=clean_h, dev_workspace=hws)
 
     ms_e2e = timed(step_host, args.steps, max(1, args.warmup // 2))
+
+    def poison_host_slot():
+        # The timed steps push the SAME frame through the same staging slot, so rows a kernel read before their band of the
+        # H2D copy had landed would still hold the right pixels from the step before.  The checked call therefore starts
+        # from a slot (and result buffers) full of NaN bytes: an early read can no longer go unnoticed.
+        hws.fill_(0xFF)
+        mask_h.fill_(0xFF)
+        clean_h.fill_(float("nan"))
+        torch.cuda.synchronize()
+
+    poison_host_slot()
+    step_host()
+    torch.cuda.synchronize()
     same = bool((mask_h.numpy() == res["mask"].cpu().numpy()).all() and
                 (clean_h.numpy() == res["clean"].cpu().numpy()).all())
     # ---- raw uint16 ingest: the same frame rounded to detector counts, 2 bytes per pixel H2D
@@ -412,6 +431,11 @@ def run_cuda(args):
     def step_host_sparse():
         lc.lacosmic_run_host_sparse(img_h, P[main_mode], out=sp_out, dev_workspace=hws)
     ms_sp = timed(step_host_sparse, args.steps, max(1, args.warmup // 2))
+    poison_host_slot()
+    for k_ in ("maskbits", "idx", "val", "count"):
+        sp_out[k_].fill_(-1)
+    step_host_sparse()
+    torch.cuda.synchronize()
     nsp = int(sp_out["count"][0])
     sp_idx = sp_out["idx"].numpy()[:nsp]
     ref_mask = res["mask"].cpu().numpy()
@@ -515,7 +539,8 @@ def run_cuda(args):
         ops_px = KERNEL_MINMAX_PER_PX[dom]
         achieved = npx * ops_px / (dom_avg_ms * 1e-3) / 1e12
         return dict(bound="alu", kernel=dom, achieved=achieved, peak=alu_peak, unit="T min/max instr/s",
-                    frac=achieved / alu_peak, traffic=(NCU_TRAFFIC_BYTES or {}).get(dom),
+                    frac=achieved / alu_peak, traffic=(NCU_TRAFFIC.get(dom) or {}).get("bytes"),
+                    traffic_source=(NCU_TRAFFIC.get(dom) or {}).get("source"),
                     peak_source="derived: 148 SM x 64 ALU lanes/clk x %.0f MHz (DESIGN.md section 5)" % sm_max,
                     peak_measured=probe["fmnmx"], peak_measured_fmnmx3=probe["fmnmx3"],
                     peak_measured_source="lacosmic_probe_minmax_rate in this run (csrc/probe.cuh: register-only "
@@ -606,13 +631,15 @@ def run_cuda(args):
                            "graph (every kernel runs every step; direct_launches = the same without the replay)",
                     parallelism="replicas (one frame per GPU, no collective)"),
         mpix_per_s=frames_per_s * npx / 1e6,
-        # e2e leads with the sparse-result call: the cleaned frame equals the input outside the mask,
-        # so the host call that returns the mask bit-plane + the replaced pixels moves 114 MB instead of 234 MB over PCIe;
-        # the dense-result call (mask and cleaned planes copied back in full) is reported beside it
-        e2e=dict(e2e_sparse, note="results = mask bit-plane + ascending list of replaced pixels with their values"),
-        e2e_dense=dict(value=e2e_fps, unit="frames/s", h2d_bytes_per_step=npx * 4,
-                       d2h_bytes_per_step=npx * 5, ms_per_step=ms_e2e, matches_device_path=same,
-                       call="lacosmic_run_host (pinned host buffers; mask uint8 + cleaned fp32 planes copied back)"),
+        # e2e is the call that returns what the north-star signature returns: the uint8 mask and the cleaned fp32 plane on
+        # the host (234 MB over PCIe per frame).  The sparse-result call (mask bit-plane + the replaced pixels, 114 MB: the
+        # cleaned frame equals the input outside the mask) is a different deliverable and is reported beside it.  Both
+        # matches_device_path flags come from a call made after the timed steps with the staging slot poisoned with NaN.
+        e2e=dict(value=e2e_fps, unit="frames/s", h2d_bytes_per_step=npx * 4,
+                 d2h_bytes_per_step=npx * 5, ms_per_step=ms_e2e, matches_device_path=same,
+                 call="lacosmic_run_host (pinned host buffers; mask uint8 + cleaned fp32 planes copied back)"),
+        e2e_sparse=dict(e2e_sparse, note="results = mask bit-plane + ascending list of replaced pixels with their values; "
+                                         "the host-side scatter that rebuilds the cleaned plane is not part of the call"),
         gpu_launches=res["launches"] * args.steps,
         launches_per_step=res["launches"],
         roofline=dict(roofline(res), step=step_roofline(res["ms"])), hbm=hbm,
@@ -679,8 +706,8 @@ def run_stream(args):
         if n == 0:
             return 0, 0.0
         imgs = torch.empty((n, h, w), dtype=torch.float32, device=dev)
-        for j, i in enumerate(mine):
-            imgs[j].copy_(torch.from_numpy(synth.make_frame(**cfg[i][0]).img))
+        for j, fimg in enumerate(synth.make_images([cfg[i][0] for i in mine])):
+            imgs[j].copy_(torch.from_numpy(fimg))
         plist = [lc.Params(mode=lc.MODE_LAZY, **cfg[i][1]) for i in mine]
         masks = torch.empty((n, h, w), dtype=torch.uint8, device=dev)
         cleans = torch.empty_like(imgs)
@@ -774,8 +801,8 @@ def main():
                     help="which evaluation mode is the headline (the other is measured and reported too)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-gain-estimation", action="store_true", help="skip the gain = 0 leg (DESIGN.md R21)")
-    ap.add_argument("--stream-frames", type=int, default=12,
-                    help="frames of the configs[3] stream leg (0 = skip; 64 = the full configuration)")
+    ap.add_argument("--stream-frames", type=int, default=64,
+                    help="frames of the configs[3] stream leg (0 = skip; 64 = the full configuration, the default)")
     ap.add_argument("--stream-concurrency", type=int, default=4,
                     help="frames in flight in the stream leg (lacosmic_run_batch internal streams)")
     args = ap.parse_args()

@@ -101,3 +101,51 @@ def test_product_path_never_imports_oracle():
         if fn.endswith((".py", ".c")):
             code = open(os.path.join(ROOT, "oracle", fn)).read()
             assert not re.search(r"^\s*(import|from)\s+paper_2602_17938_b200", code, flags=re.M), fn
+
+
+def test_band_plan_never_releases_a_tile_row_early(L):
+    """The banded H2D copy of the single-frame host calls (include/lacosmic.h, lacosmic_host_band_plan): for EVERY height
+    the rows of tiles released after band b read only rows that bands 0..b have delivered.  A row of tiles j of the first
+    pass reads input rows [32 j - 2, 32 (j + 1) + 2) (LACOSMIC_HOST_TILE_ROWS / _MARGIN: the TMA box of k_noise_S_tma).
+    The GPU tests (tests/test_gpu_host_banded.py) poison the staging plane, but a read that is early by a few rows is
+    usually hidden by the copy engine outrunning the kernel; this check does not depend on timing."""
+    TH, MY, NB = 32, 2, 8
+    re, up = (C.c_int32 * NB)(), (C.c_int32 * NB)()
+    for w in (4, 8, 6500, 6504):
+        for h in list(range(1, 2200)) + [3999, 4000, 4001, 4097, 65535]:
+            if h * w >= 2 ** 31:
+                continue
+            n = L.lacosmic_host_band_plan(h, w, re, up)
+            nty = (h + TH - 1) // TH
+            if nty < 4 * NB:
+                assert n == 0, (h, w)
+                continue
+            assert n == NB, (h, w)
+            ends, rows = [re[b] for b in range(n)], [up[b] for b in range(n)]
+            assert ends == sorted(ends) and ends[-1] == h and ends[0] > 0, (h, w, ends)
+            assert rows == sorted(rows) and rows[-1] == nty, (h, w, rows)
+            for b in range(n):
+                if ends[b] < h:
+                    assert TH * rows[b] + MY <= ends[b], "tile row %d released before row %d arrived (h=%d)" % (
+                        rows[b] - 1, TH * rows[b] + MY - 1, h)
+                    # and not needlessly late: one more row of tiles would not have been fed (or an earlier band already
+                    # released it)
+                    assert TH * (rows[b] + 1) + MY > ends[b] or rows[b] == nty, (h, w, b)
+                else:
+                    assert rows[b] == nty
+    assert L.lacosmic_host_band_plan(4000, 6501, re, up) == 0          # no TMA path for this pitch: one piece
+    assert L.lacosmic_host_band_plan(0, 8, re, up) == -2 and L.lacosmic_host_band_plan(8, 8, None, up) == -1
+
+
+def test_variant_inputs_may_not_alias_the_workspace(L):
+    from paper_2602_17938_b200.binding import _CParams, _CVariant
+    ok = _CParams(1.0, 10.0, 4.5, 0.3, 5.0, 65535.0, 4, 0)
+    fake = lambda a: C.c_void_p(a)
+    img, mask, clean, ws = 0x10000000, 0x20000000, 0x30000000, 0x40000000
+    need = L.lacosmic_workspace_bytes(64, 64)
+    run = lambda v: L.lacosmic_run_ex(fake(img), 64, 64, C.byref(ok), C.byref(v), fake(mask), fake(clean), fake(ws),
+                                      need, None, None, None)
+    assert run(_CVariant(0, -1, ws + 512, None)) == -5                 # bpm inside the workspace
+    assert run(_CVariant(0, -1, None, ws + need - 16)) == -5           # var overlapping its end
+    assert run(_CVariant(0, -1, clean + 4, None)) == -5 and run(_CVariant(0, -1, None, mask)) == -5
+    assert run(_CVariant(2, -1, None, None)) == -3                     # (unknown fsmode: still a parameter error)
