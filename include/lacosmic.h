@@ -133,7 +133,8 @@ int lacosmic_run_ws(const float *img, int h, int w, const lacosmic_params *p, ui
  *            the replacement; its value still enters the filters.
  *   var    : nullable DEVICE fp32 [h][w] (16-byte aligned), variance in ADU^2 (R24): N = sqrt(max(var, 1e-8)) replaces
  *            the noise model of step (2); gain and readnoise are then unused (gain = 0 does not trigger the estimate).
- * bpm / var are read during the call's stream work and must not overlap the outputs. */
+ * bpm / var are read during the call's stream work and must overlap neither the outputs nor the workspace
+ * (LACOSMIC_ERR_ALIAS). */
 typedef struct lacosmic_variant {
     int32_t fsmode;
     int32_t satgrow;
@@ -186,6 +187,16 @@ int lacosmic_run_batch(const float *imgs, int n, int h, int w, const lacosmic_pa
  * and device (ordered after the work already on `stream`), and the first pass of the path follows it band by band on
  * `stream`; the img_host buffer must stay unchanged until `stream` has been synchronised, as for any asynchronous copy. */
 size_t lacosmic_host_workspace_bytes(int h, int w);
+/* Diagnostic: the plan of that banded copy for an h x w frame, a function of the shape alone (no GPU needed).  Returns
+ * the number of bands n <= LACOSMIC_HOST_BANDS (0: the frame is copied in one piece; negative: error code) and fills the
+ * HOST arrays row_end[b] = first row NOT in bands 0..b and tile_rows[b] = how many rows of tiles of the first pass
+ * (LACOSMIC_HOST_TILE_ROWS input rows each, reading LACOSMIC_HOST_TILE_MARGIN more rows above and below) are released once
+ * band b has arrived.  tests/test_abi_cpu.py checks for every height that no row of tiles is released before the last
+ * row it reads is on the device.  (Bands are also conditional on lazy mode, a supplied gain and fp32 input.) */
+#define LACOSMIC_HOST_BANDS 8
+#define LACOSMIC_HOST_TILE_ROWS 32
+#define LACOSMIC_HOST_TILE_MARGIN 2
+int lacosmic_host_band_plan(int h, int w, int32_t *row_end, int32_t *tile_rows);
 int lacosmic_run_host(const float *img_host, int h, int w, const lacosmic_params *p,
                       uint8_t *mask_out_host, float *clean_out_host, void *dev_workspace,
                       size_t dev_workspace_bytes, void *stream);
@@ -241,14 +252,18 @@ int lacosmic_run_host_batch(const float *imgs_host, int n, int h, int w, const l
 
 /* R21 alone: the gain estimate of one image (what the whole path computes at the start of an iteration when
  * p->gain == 0), for the given read noise [e-].  gain_out: DEVICE pointer to one float; stats_out: nullable
- * DEVICE pointer to 7 floats {c, s, lo, hi, kept, mt, fast}: centre, 1.4826 MAD, the interval the last clipping
+ * DEVICE pointer to 6 floats {c, s, lo, hi, kept, mt}: centre, 1.4826 MAD, the interval the last clipping
  * round started from, the number of pixels inside it, the typical signal (rank-(kept-1)/2 element of
- * max(med5, 1e-4) over those pixels), and 1 if the three clipping rounds were resolved on the zone lists
- * (two reads of the residual plane, csrc/selectz.cuh), 0 if by radix passes over the plane (csrc/select.cuh;
- * taken when the fast path is switched off, on frames of a few pixels or of few distinct values, or when a
- * check of the fast path fails) -- the values are the same bits either way.  workspace as for lacosmic_run_ws. */
+ * max(med5, 1e-4) over those pixels).  workspace as for lacosmic_run_ws.  (Version 0.3 of the library wrote a seventh
+ * float behind the six; from 0.4 on this symbol writes six again and the seventh has its own pointer below.) */
 int lacosmic_estimate_gain(const float *img, int h, int w, float readnoise, float *gain_out,
                            float *stats_out, void *workspace, size_t workspace_bytes, void *stream);
+/* The same with path_out: nullable DEVICE pointer to one float that receives 1 if the three clipping rounds were
+ * resolved on the zone lists (two reads of the residual plane, csrc/selectz.cuh), 0 if by radix passes over the plane
+ * (csrc/select.cuh; taken when the fast path is switched off, on frames of a few pixels or of few distinct values, or
+ * when a check of the fast path fails) -- gain and statistics are the same bits either way. */
+int lacosmic_estimate_gain_ex(const float *img, int h, int w, float readnoise, float *gain_out, float *stats_out,
+                              float *path_out, void *workspace, size_t workspace_bytes, void *stream);
 
 /* Diagnostic: the plan of the last gain estimate that ran in `workspace` (csrc/selectz.cuh, struct SelZone), copied to
  * the HOST array info_host[LACOSMIC_GAIN_ZONE_WORDS] as 32-bit words after synchronising `stream`:
@@ -341,13 +356,6 @@ int lacosmic_last_cuda_error(void);
 int lacosmic_last_launch_count(void);
 const char *lacosmic_version(void);
 
-/* Optional CUDA-event timing per kernel class, per calling thread.  After
- * lacosmic_kernel_timing_enable(1) every launch of the whole-path entry points is bracketed by an
- * event pair on the caller's stream (up to 8192 spans between reads).  Once the caller has
- * synchronised the stream, lacosmic_kernel_timing_read() writes, for each class c <
- * LACOSMIC_NUM_KERNEL_CLASSES, the summed device time ms_sum[c] and the number of spans[c] (HOST
- * arrays), and clears the record.  Class names: lacosmic_kernel_class_name(c); the last class is the
- * whole frame (copies included). */
 /* Work counters of the last frame that ran in `workspace` (the lazy path's data-dependent work; bench.py turns them into
  * the per-kernel terms of the whole-step roofline).  stats_host: HOST array
  * [LACOSMIC_NUM_FRAME_STATS][LACOSMIC_MAX_NITER] of int32, row r, iteration t:
@@ -368,7 +376,10 @@ int lacosmic_frame_stats(const void *workspace, int h, int w, int32_t *stats_hos
  * launch mechanism the Blackwell guide recommends for launch-bound loops).  The 16 most recently used argument sets are
  * kept.  Not used when `dbg` is given, while kernel timing or statistics are enabled, on the legacy default stream, or
  * on a stream the caller is capturing (the call then enqueues its kernels directly, as always).  enable = 0 also drops
- * the cached graphs.  Results and ordering on `stream` are identical either way. */
+ * the cached graphs.  Results and ordering on `stream` are identical either way.  Threads: the table of cached graphs is
+ * locked only for the look-up; capture, instantiation and launch hold a lock of the one entry, so calls with different
+ * arguments (other GPUs, streams, frames) do not serialise on each other.  The switch of the gain estimate's fast path is
+ * part of the key, so flipping it never replays a sequence captured under the other setting. */
 int lacosmic_graph_replay_enable(int enable);
 
 /* Measured peak of the "alu" roofline (the medians of PAPER.md:23,64 are fp32 min/max selection
@@ -378,6 +389,13 @@ int lacosmic_graph_replay_enable(int enable);
  * diagnostic allocates 256 bytes of device memory, SYNCHRONISES `stream` and takes about 10 ms. */
 int lacosmic_probe_minmax_rate(int kind, double *instr_per_s_host, void *stream);
 
+/* Optional CUDA-event timing per kernel class, per calling thread.  After
+ * lacosmic_kernel_timing_enable(1) every launch of the whole-path entry points is bracketed by an
+ * event pair on the caller's stream (up to 8192 spans between reads).  Once the caller has
+ * synchronised the stream, lacosmic_kernel_timing_read() writes, for each class c <
+ * LACOSMIC_NUM_KERNEL_CLASSES, the summed device time ms_sum[c] and the number of spans[c] (HOST
+ * arrays), and clears the record.  Class names: lacosmic_kernel_class_name(c); the last class is the
+ * whole frame (copies included). */
 #define LACOSMIC_NUM_KERNEL_CLASSES 9
 int lacosmic_kernel_timing_enable(int enable);
 int lacosmic_kernel_timing_read(float *ms_sum, int32_t *spans);

@@ -27,7 +27,7 @@ EXPORTS = (
     "lacosmic_kernel_timing_enable", "lacosmic_kernel_timing_read", "lacosmic_kernel_class_name",
     "lacosmic_probe_minmax_rate", "lacosmic_stats_enable", "lacosmic_frame_stats", "lacosmic_graph_replay_enable", "lacosmic_gain_fast_path_enable", "lacosmic_gain_zone_info",
     "lacosmic_run_ex", "lacosmic_sepmed_workspace_bytes", "lacosmic_run_sepmed_compare", "lacosmic_sepmedfilt",
-    "lacosmic_masked_median_bpm", "lacosmic_satstar_mask", "lacosmic_masked_median_noalloc",
+    "lacosmic_masked_median_bpm", "lacosmic_satstar_mask", "lacosmic_masked_median_noalloc", "lacosmic_estimate_gain_ex", "lacosmic_host_band_plan",
 )
 NOALLOC_MAX_WORDS = 131072       # include/lacosmic.h LACOSMIC_NOALLOC_MAX_WORDS
 ERR_TOO_LARGE = -8
@@ -106,11 +106,13 @@ def load_library():
                                 C.POINTER(_CDebug), vp]),
         "lacosmic_run_batch": (i, [vp, i, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp, vp]),
         "lacosmic_host_workspace_bytes": (sz, [i, i]),
+        "lacosmic_host_band_plan": (i, [i, i, vp, vp]),
         "lacosmic_run_host": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp]),
         "lacosmic_run_host_u16": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, sz, vp]),
         "lacosmic_run_host_sparse": (i, [vp, i, i, C.POINTER(_CParams), vp, vp, vp, vp, i, vp, sz, vp]),
         "lacosmic_run_host_stream_sparse": (i, [vp, i, i, i, i, C.POINTER(_CParams), vp, vp, vp, vp, i, vp, sz, vp]),
         "lacosmic_estimate_gain": (i, [vp, i, i, f, vp, vp, vp, sz, vp]),
+        "lacosmic_estimate_gain_ex": (i, [vp, i, i, f, vp, vp, vp, vp, sz, vp]),
         "lacosmic_lplus": (i, [vp, vp, i, i, vp]),
         "lacosmic_medfilt": (i, [vp, vp, i, i, i, vp]),
         "lacosmic_bitplane_pitch_words": (i, [i]),
@@ -185,11 +187,17 @@ def _scratch_on(t, stream):
 
 def _on_device(fn):
     """Host-buffer entry points take device=...: make it the current device for the call (the library works on the
-    current device, and stream=None means that device's current stream)."""
+    current device, and stream=None means that device's current stream).  `device` may be given by keyword or by
+    position; it is resolved against the wrapped function's own signature."""
+    import inspect
+    sig = inspect.signature(fn)
+
     @functools.wraps(fn)
-    def wrapped(*args, device="cuda:0", **kw):
-        with _torch().cuda.device(device):
-            return fn(*args, device=device, **kw)
+    def wrapped(*args, **kw):
+        bound = sig.bind(*args, **kw)
+        bound.apply_defaults()
+        with _torch().cuda.device(bound.arguments["device"]):
+            return fn(*bound.args, **bound.kwargs)
     return wrapped
 
 
@@ -223,6 +231,15 @@ def lacosmic_batch_workspace_bytes(h, w, concurrency):
 
 def lacosmic_host_workspace_bytes(h, w):
     return int(load_library().lacosmic_host_workspace_bytes(int(h), int(w)))
+
+
+def lacosmic_host_band_plan(h, w):
+    """[(row_end, tile_rows)] per band of the banded H2D copy of the single-frame host calls ([] = one piece)."""
+    re, up = (C.c_int32 * 8)(), (C.c_int32 * 8)()
+    n = load_library().lacosmic_host_band_plan(int(h), int(w), re, up)
+    if n < 0:
+        raise LacosmicError(n, "lacosmic_host_band_plan")
+    return [(int(re[b]), int(up[b])) for b in range(n)]
 
 
 def lacosmic_run(img, gain=1.0, readnoise=10.0, sigclip=4.5, sigfrac=0.3, objlim=5.0, niter=4,
@@ -394,7 +411,10 @@ def lacosmic_run_host(img_host, params=None, mask_out_host=None, clean_out_host=
             clean_out_host.data_ptr(), _dev(dev_workspace, torch.uint8, "dev_workspace"),
             dev_workspace.numel(), _stream(stream))
     _check(rc, "lacosmic_run_host")
-    return dict(mask=mask_out_host, clean=clean_out_host)
+    # the call has only ENQUEUED the H2D copy (on `stream`, or in bands on the library's copy stream): the result keeps
+    # the input tensor referenced so that a temporary (e.g. x.pin_memory()) is not handed back to torch's host allocator,
+    # and possibly reused, before the copy has read it.  The caller must still not WRITE img_host before synchronising.
+    return dict(mask=mask_out_host, clean=clean_out_host, _img_host=img_host)
 
 
 @_on_device
@@ -425,6 +445,7 @@ def lacosmic_run_host_sparse(img_host, params=None, capacity=None, out=None, dev
                                     int(out["capacity"]), _dev(dev_workspace, torch.uint8, "dev_workspace"),
                                     dev_workspace.numel(), _stream(stream))
     _check(rc, "lacosmic_run_host_sparse")
+    out["_img_host"] = img_host          # stays referenced until the caller drops the result (see lacosmic_run_host)
     return out
 
 
@@ -458,6 +479,7 @@ def lacosmic_run_host_stream_sparse(imgs_host, params, capacity=None, out=None, 
                                            _dev(dev_workspace, torch.uint8, "dev_workspace"), dev_workspace.numel(),
                                            _stream(stream))
     _check(rc, "lacosmic_run_host_stream_sparse")
+    out["_img_host"] = imgs_host
     return out
 
 
@@ -532,7 +554,7 @@ def lacosmic_run_host_batch(imgs_host, params, masks_host=None, cleans_host=None
                                    cleans_host.data_ptr(), _dev(dev_workspace, torch.uint8, "dev_workspace"),
                                    dev_workspace.numel(), _stream(stream))
     _check(rc, "lacosmic_run_host_batch")
-    return dict(mask=masks_host, clean=cleans_host)
+    return dict(mask=masks_host, clean=cleans_host, _img_host=imgs_host)
 
 
 # ----------------------------------------------------------------------------- single steps
@@ -558,13 +580,18 @@ def lacosmic_estimate_gain(img, readnoise=0.0, workspace=None, stream=None, want
     if workspace is None:
         workspace = _scratch_on(_workspace(h, w, img.device), stream)
     gain = torch.zeros(1, dtype=torch.float32, device=img.device)
-    stats = torch.zeros(7, dtype=torch.float32, device=img.device)
-    _check(load_library().lacosmic_estimate_gain(
-        _dev(img, torch.float32, "img"), h, w, float(readnoise), gain.data_ptr(), stats.data_ptr(),
-        _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)), "lacosmic_estimate_gain")
+    stats = torch.zeros(6, dtype=torch.float32, device=img.device)
+    args = (_dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream))
     if want_path:
-        return gain, stats[:6], stats[6:7]
-    return gain, stats[:6]
+        path = torch.zeros(1, dtype=torch.float32, device=img.device)
+        _check(load_library().lacosmic_estimate_gain_ex(
+            _dev(img, torch.float32, "img"), h, w, float(readnoise), gain.data_ptr(), stats.data_ptr(), path.data_ptr(),
+            *args), "lacosmic_estimate_gain_ex")
+        return gain, stats, path
+    _check(load_library().lacosmic_estimate_gain(
+        _dev(img, torch.float32, "img"), h, w, float(readnoise), gain.data_ptr(), stats.data_ptr(), *args),
+        "lacosmic_estimate_gain")
+    return gain, stats
 
 
 def lacosmic_lplus(img, out=None, stream=None):

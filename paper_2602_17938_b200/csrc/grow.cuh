@@ -1,6 +1,6 @@
 // Steps (6)-(7) fused, and the bit-plane pass that opens an incremental iteration.
 //
-// Both kernels are WARP-AUTONOMOUS: a warp owns a strip of 30 words x 8 rows (960 x 8 pixels) of the
+// Both kernels are WARP-AUTONOMOUS: a warp owns a strip of 30 words x WG_R = 4 rows (960 x 4 pixels) of the
 // bit-planes, lane l holds word column wx0 - 1 + l (lanes 0 and 31 are the horizontal halo) of every row it
 // needs in registers, horizontal neighbours come from warp shuffles, and everything in the halo is
 // recomputed from the same inputs by the neighbouring warp (bit arithmetic, plus a handful of redundant G2

@@ -3,6 +3,7 @@
 #include "../../include/lacosmic.h"
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -36,13 +37,15 @@ inline bool cuda_ok(cudaError_t e) {
 // Launch of a kernel of the lazy frame with programmatic dependent launch (common.cuh, pdl_entry): the grid may be
 // scheduled while its predecessor in the stream drains; the kernel itself waits for the predecessor before it reads
 // anything.  LACOSMIC_PDL=0 in the environment launches plainly.
-int g_pdl = -1;
+std::atomic<int> g_pdl{-1};   // -1: not decided yet; two threads deciding at once store the same value
 bool pdl_enabled() {
-    if (g_pdl < 0) {
+    int v = g_pdl.load(std::memory_order_relaxed);
+    if (v < 0) {
         const char* e = std::getenv("LACOSMIC_PDL");
-        g_pdl = (e && e[0] == '0') ? 0 : 1;
+        v = (e && e[0] == '0') ? 0 : 1;
+        g_pdl.store(v, std::memory_order_relaxed);
     }
-    return g_pdl == 1;
+    return v == 1;
 }
 template <class... KArgs, class... Args>
 void launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
@@ -261,7 +264,7 @@ int unpack(const uint32_t* bits, uint8_t* u8, int h, int w, cudaStream_t st, con
 // (1-D grids of nbx * nby CTAs, block_xy in common.cuh: rows on gridDim.y would stop at 65535 rows of CTAs)
 inline int bit_nbx(int w) { return (words_per_row(w) + 31) / 32; }
 inline unsigned bit_grid(int h, int w) { return (unsigned)bit_nbx(w) * (unsigned)((h + lac::BW_CTA_ROWS - 1) / lac::BW_CTA_ROWS); }
-// grid of k_grow_replace / k_dirty_lists: 30 words x 64 rows per CTA, one 30 x 8 strip per warp (grow.cuh)
+// grid of k_grow_replace / k_dirty_lists: 30 words x WG_R * WG_WARPS = 32 rows per CTA, one 30-word x 4-row strip per warp (grow.cuh)
 inline int grow_nbx(int w) { return (words_per_row(w) + lac::WG_OWN - 1) / lac::WG_OWN; }
 inline unsigned grow_grid(int h, int w) {
     const int rows = lac::WG_R * lac::WG_WARPS;
@@ -280,13 +283,16 @@ int grow_replace(const lac::GrowArgs& ga, const int* prev, cudaStream_t st) {
 // -> *gain_out (device), stats (nullable, device, 7 floats).  `lists`: storage of the fast path's lists (list_words
 // 32-bit words: the quad list and the planes G1, G2, G2F, M1, M2, M3 behind it, which hold nothing at this point of an
 // iteration that estimates the gain -- such an iteration is never incremental and rewrites them all).
-int g_gain_fast = -1;          // -1: not decided yet (environment LACOSMIC_GAIN_FAST=0 switches the fast path off)
+std::atomic<int> g_gain_fast{-1};   // -1: not decided yet (environment LACOSMIC_GAIN_FAST=0 switches the fast path off)
 bool gain_fast_enabled() {
-    if (g_gain_fast < 0) {
+    int v = g_gain_fast.load(std::memory_order_relaxed);
+    if (v < 0) {
         const char* e = std::getenv("LACOSMIC_GAIN_FAST");
-        g_gain_fast = (e && e[0] == '0') ? 0 : 1;
+        v = (e && e[0] == '0') ? 0 : 1;
+        int expect = -1;
+        if (!g_gain_fast.compare_exchange_strong(expect, v)) v = expect;   // lacosmic_gain_fast_path_enable got there first
     }
-    return g_gain_fast == 1;
+    return v == 1;
 }
 int sigma_clip_gain(const float* R, const float* M5, size_t npx, const Workspace& ws, void* lists, size_t list_words,
                     float rn2, float* gain_out, float* stats, const int* prev, cudaStream_t st) {
@@ -365,12 +371,35 @@ inline int check_variant(const lacosmic_variant* v) {
 
 // A frame that is still arriving (lacosmic_run_host*): rows [0, row_end[b]) of img are on the device once ready[b] has
 // fired.  The first noise/S pass is then launched band by band behind the copies instead of behind the whole frame.
-constexpr int MAX_BANDS = 8;
+constexpr int MAX_BANDS = LACOSMIC_HOST_BANDS;
+static_assert(lac::NS_TH == LACOSMIC_HOST_TILE_ROWS && lac::NS_MY == LACOSMIC_HOST_TILE_MARGIN, "header and library disagree");
 struct BandSync {
     int n = 0;
     cudaEvent_t ready[MAX_BANDS];
     int row_end[MAX_BANDS];
+    int upto[MAX_BANDS];      // rows of tiles of the first pass that may run once band b has arrived (cumulative)
 };
+
+// The plan of the banded copy, a function of the shape alone (exported as lacosmic_host_band_plan so that a test can
+// check the margin for every height without a GPU).  Band b ends at row row_end[b] (exclusive); once it has arrived,
+// the rows of tiles below upto[b] may run.  A row of tiles j of the noise/S pass reads input rows
+// [j * NS_TH - NS_MY, (j + 1) * NS_TH + NS_MY) (its TMA box, kernels.cuh), so it is released only when
+// (j + 1) * NS_TH + NS_MY <= row_end[b], or when the band is the last one (the whole frame is there).
+// Returns the number of bands; 0 = this shape is copied in one piece.
+int band_plan(int h, int w, int* row_end, int* upto) {
+    const int nty = (h + lac::NS_TH - 1) / lac::NS_TH;
+    if ((w % 4) != 0 || nty < 4 * MAX_BANDS) return 0;
+    int done = 0;
+    for (int b = 0; b < MAX_BANDS; ++b) {
+        const int re = b == MAX_BANDS - 1 ? h : std::min(h, (int)((long long)nty * (b + 1) / MAX_BANDS) * lac::NS_TH);
+        int u = re >= h ? nty : (re - lac::NS_MY) / lac::NS_TH;      // rows of tiles wholly fed by rows < re
+        u = std::max(done, std::min(u, nty));
+        row_end[b] = re;
+        upto[b] = u;
+        done = u;
+    }
+    return MAX_BANDS;
+}
 
 // The iteration loop (O0-O7) for one frame.  vr: nullable variants (R22-R25).
 int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t* mask_out,
@@ -479,9 +508,7 @@ int run_frame(const float* img, int h, int w, const lacosmic_params& p, uint8_t*
                 int done = 0;                          // rows of tiles launched so far
                 for (int b = 0; b < bands->n; ++b) {
                     CK(cudaStreamWaitEvent(st, bands->ready[b], 0));
-                    const int re = bands->row_end[b];
-                    int upto = re >= h ? ntyNS : (re - lac::NS_MY) / lac::NS_TH;     // rows of tiles wholly fed by rows < re
-                    upto = std::max(done, std::min(upto, ntyNS));
+                    const int upto = bands->upto[b];                                 // band_plan: rows of tiles wholly fed by now
                     if (upto > done) {
                         int rc2 = noise_tiles(na, from, done * ntx, (upto - done) * ntx);
                         if (rc2) return rc2;
@@ -733,27 +760,45 @@ namespace {
 // timing or statistics on, on the legacy default stream or on a stream that is being captured by the caller.
 struct GraphKey {
     int dev, h, w;
+    int gain_fast;            // which path of the gain estimate the captured sequence takes (a process-wide switch)
     const void *img, *mask, *clean, *ws, *counts;
     size_t ws_bytes;
     lacosmic_params p;
     bool operator==(const GraphKey& o) const {
-        return dev == o.dev && h == o.h && w == o.w && img == o.img && mask == o.mask && clean == o.clean &&
-               ws == o.ws && counts == o.counts && ws_bytes == o.ws_bytes && std::memcmp(&p, &o.p, sizeof p) == 0;
+        return dev == o.dev && h == o.h && w == o.w && gain_fast == o.gain_fast && img == o.img && mask == o.mask &&
+               clean == o.clean && ws == o.ws && counts == o.counts && ws_bytes == o.ws_bytes &&
+               std::memcmp(&p, &o.p, sizeof p) == 0;
     }
 };
+// Locking.  g_graph_mu guards the table itself (keys, seen / used / users / doomed) and is held only for the look-up
+// and the release, never across a CUDA call that takes long.  An entry's own `mu` is held while its graph is
+// captured, instantiated and launched (a cudaGraphExec_t must not be launched from two threads at once), so threads
+// that work with different argument sets -- different GPUs, streams, frames -- do not wait for each other.  An entry
+// with users > 0 is neither evicted nor destroyed; lacosmic_graph_replay_enable(0) marks it doomed and its last user
+// destroys it.
 struct GraphEntry {
     GraphKey key;
     cudaGraphExec_t exec = nullptr;
     int launches = 0;
     int seen = 0;             // calls with this key so far
     bool failed = false;      // capture or instantiation failed once: this key always takes the direct path
+    bool doomed = false;      // the replay was switched off while a thread was using the entry
+    int users = 0;            // threads between look-up and release
     unsigned long long used = 0;
+    std::mutex mu;
+    void reset() {            // g_graph_mu held, users == 0
+        if (exec) cudaGraphExecDestroy(exec);
+        exec = nullptr;
+        launches = seen = 0;
+        failed = doomed = false;
+        used = 0;
+    }
 };
 constexpr int GRAPH_CACHE = 16;
 GraphEntry g_graphs[GRAPH_CACHE];
 std::mutex g_graph_mu;
 unsigned long long g_graph_clock = 0;
-int g_graphs_on = -1;         // -1: not decided yet (environment LACOSMIC_GRAPHS=0 switches the replay off)
+int g_graphs_on = -1;         // -1: not decided yet (environment LACOSMIC_GRAPHS=0 switches the replay off); under g_graph_mu
 
 bool graphs_enabled() {
     if (g_graphs_on < 0) {
@@ -770,8 +815,8 @@ int lacosmic_graph_replay_enable(int enable) {
     g_graphs_on = enable ? 1 : 0;
     if (!enable)
         for (GraphEntry& e : g_graphs) {
-            if (e.exec) cudaGraphExecDestroy(e.exec);
-            e = GraphEntry();
+            if (e.users > 0) e.doomed = true;
+            else e.reset();
         }
     return LACOSMIC_OK;
 }
@@ -795,57 +840,66 @@ int lacosmic_run_ws(const float* img, int h, int w, const lacosmic_params* p, ui
         cudaGetLastError();     // cudaStreamIsCapturing on the legacy stream during someone else's capture reports an error
         return run_frame(img, h, w, *p, mask_out, clean_out, ws, iter_counts, dbg, st);
     }
-    std::unique_lock<std::mutex> lock(g_graph_mu);
-    if (!graphs_enabled()) {
-        lock.unlock();
-        return run_frame(img, h, w, *p, mask_out, clean_out, ws, iter_counts, dbg, st);
-    }
     GraphKey key;
     std::memset(&key, 0, sizeof key);
     cudaGetDevice(&key.dev);
     key.h = h; key.w = w; key.img = img; key.mask = mask_out; key.clean = clean_out; key.ws = workspace;
     key.counts = iter_counts; key.ws_bytes = workspace_bytes; key.p = *p;
+    key.gain_fast = gain_fast_enabled() ? 1 : 0;
     GraphEntry* e = nullptr;
-    GraphEntry* lru = &g_graphs[0];
-    for (GraphEntry& g : g_graphs) {
-        if (g.seen && g.key == key) { e = &g; break; }
-        if (g.used < lru->used) lru = &g;
+    {   // look-up: the only part under the table lock
+        std::lock_guard<std::mutex> lock(g_graph_mu);
+        if (graphs_enabled()) {
+            GraphEntry* lru = nullptr;
+            for (GraphEntry& g : g_graphs) {
+                if (g.seen && !g.doomed && g.key == key) { e = &g; break; }
+                if (g.users == 0 && (!lru || g.used < lru->used)) lru = &g;
+            }
+            if (e) {
+                e->used = ++g_graph_clock;
+                ++e->seen;
+                ++e->users;
+            } else if (lru) {       // first call with these arguments: remember them, run directly
+                lru->reset();
+                lru->key = key;
+                lru->seen = 1;
+                lru->used = ++g_graph_clock;
+            }                       // (every entry in use by another thread: run directly, remember nothing)
+        }
     }
-    if (!e) {                   // first call with these arguments: remember them, run directly
-        if (lru->exec) cudaGraphExecDestroy(lru->exec);
-        *lru = GraphEntry();
-        lru->key = key;
-        lru->seen = 1;
-        lru->used = ++g_graph_clock;
-        lock.unlock();
-        return run_frame(img, h, w, *p, mask_out, clean_out, ws, iter_counts, dbg, st);
-    }
-    e->used = ++g_graph_clock;
-    ++e->seen;
-    if (!e->exec && !e->failed) {   // second call: capture the sequence
-        cudaGraph_t graph = nullptr;
-        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-            rc = run_frame(img, h, w, *p, mask_out, clean_out, ws, iter_counts, dbg, st);
-            const cudaError_t ce = cudaStreamEndCapture(st, &graph);
-            if (rc == LACOSMIC_OK && ce == cudaSuccess && graph &&
-                cudaGraphInstantiate(&e->exec, graph, 0) == cudaSuccess) {
-                e->launches = g_launches;
+    if (!e) return run_frame(img, h, w, *p, mask_out, clean_out, ws, iter_counts, dbg, st);
+    bool launched = false, launch_failed = false;
+    {
+        std::lock_guard<std::mutex> mine(e->mu);
+        if (!e->exec && !e->failed) {   // second call: capture the sequence
+            cudaGraph_t graph = nullptr;
+            if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                rc = run_frame(img, h, w, *p, mask_out, clean_out, ws, iter_counts, dbg, st);
+                const cudaError_t ce = cudaStreamEndCapture(st, &graph);
+                if (rc == LACOSMIC_OK && ce == cudaSuccess && graph &&
+                    cudaGraphInstantiate(&e->exec, graph, 0) == cudaSuccess) {
+                    e->launches = g_launches;
+                } else {
+                    e->exec = nullptr;
+                    e->failed = true;
+                }
+                if (graph) cudaGraphDestroy(graph);
             } else {
-                e->exec = nullptr;
                 e->failed = true;
             }
-            if (graph) cudaGraphDestroy(graph);
-        } else {
-            e->failed = true;
+            cudaGetLastError();
         }
-        cudaGetLastError();
+        if (e->exec) {
+            g_launches = e->launches;
+            launched = true;
+            launch_failed = !cuda_ok(cudaGraphLaunch(e->exec, st));
+        }
     }
-    if (e->exec) {
-        g_launches = e->launches;
-        CK(cudaGraphLaunch(e->exec, st));
-        return LACOSMIC_OK;
+    {   // release
+        std::lock_guard<std::mutex> lock(g_graph_mu);
+        if (--e->users == 0 && e->doomed) e->reset();
     }
-    lock.unlock();
+    if (launched) return launch_failed ? LACOSMIC_ERR_CUDA : LACOSMIC_OK;
     g_launches = 0;
     return run_frame(img, h, w, *p, mask_out, clean_out, ws, iter_counts, dbg, st);
 }
@@ -861,9 +915,13 @@ int lacosmic_run_ex(const float* img, int h, int w, const lacosmic_params* p, co
     if (dbg)
         for (const float* pl : {dbg->Lp, dbg->N, dbg->S, dbg->Sp, dbg->m3, dbg->F})
             if ((uintptr_t)pl & 15) return LACOSMIC_ERR_ALIGN;
-    const size_t P = (size_t)h * w;
-    if (v && ((v->bpm && (overlap(v->bpm, P, clean_out, P * 4) || overlap(v->bpm, P, mask_out, P))) ||
-              (v->var && (overlap(v->var, P * 4, clean_out, P * 4) || overlap(v->var, P * 4, mask_out, P)))))
+    const size_t P = (size_t)h * w, need = lacosmic_workspace_bytes(h, w);
+    // bpm / var are inputs read throughout the frame: they may coincide with nothing the frame writes (the outputs and
+    // the workspace, whose first launches already write planes and counters).  They may alias img: all three are read-only.
+    if (v && ((v->bpm && (overlap(v->bpm, P, clean_out, P * 4) || overlap(v->bpm, P, mask_out, P) ||
+                          overlap(v->bpm, P, workspace, need))) ||
+              (v->var && (overlap(v->var, P * 4, clean_out, P * 4) || overlap(v->var, P * 4, mask_out, P) ||
+                          overlap(v->var, P * 4, workspace, need)))))
         return LACOSMIC_ERR_ALIAS;
     return run_frame(img, h, w, *p, mask_out, clean_out, carve(workspace, h, w), iter_counts, dbg,
                      (cudaStream_t)stream, v);
@@ -1011,26 +1069,22 @@ int run_host_frame(const HostFrame& io, int h, int w, const lacosmic_params& p, 
         LAUNCHED();
     }
     BandSync bands;
-#ifndef LAC_HOST_BANDS
-#define LAC_HOST_BANDS 8
-#endif
-    const int nty = (h + lac::NS_TH - 1) / lac::NS_TH;
     BatchStreams* bs = nullptr;
-    if (!io.u16 && banded && p.mode == LACOSMIC_MODE_LAZY && p.niter > 0 && p.gain != 0.0f && (w % 4) == 0 &&
-        nty >= 4 * LAC_HOST_BANDS && (bs = batch_streams())) {
+    int nb = 0;
+    if (!io.u16 && banded && p.mode == LACOSMIC_MODE_LAZY && p.niter > 0 && p.gain != 0.0f &&
+        (nb = band_plan(h, w, bands.row_end, bands.upto)) > 0 && (bs = batch_streams())) {
         const float* src = (const float*)io.img;
         CK(cudaEventRecord(bs->fork, st));                 // the slot is free once the caller's earlier work is done
         CK(cudaStreamWaitEvent(bs->copy, bs->fork, 0));
         int r0 = 0;
-        for (int b = 0; b < LAC_HOST_BANDS; ++b) {
-            const int r1 = b == LAC_HOST_BANDS - 1 ? h : std::min(h, (int)((long long)nty * (b + 1) / LAC_HOST_BANDS) * lac::NS_TH);
+        for (int b = 0; b < nb; ++b) {
+            const int r1 = bands.row_end[b];
             CK(cudaMemcpyAsync(d_img + (size_t)r0 * w, src + (size_t)r0 * w, (size_t)(r1 - r0) * w * 4, cudaMemcpyHostToDevice, bs->copy));
             CK(cudaEventRecord(bs->band[b], bs->copy));
             bands.ready[b] = bs->band[b];
-            bands.row_end[b] = r1;
             r0 = r1;
         }
-        bands.n = LAC_HOST_BANDS;
+        bands.n = nb;
     } else if (!io.u16) {
         CK(cudaMemcpyAsync(d_img, io.img, P * 4, cudaMemcpyHostToDevice, st));
     }
@@ -1096,6 +1150,16 @@ int run_host_stream(int n, int h, int w, const lacosmic_params* params, void* de
 }
 }  // namespace
 }  // extern "C++"
+
+int lacosmic_host_band_plan(int h, int w, int32_t* row_end, int32_t* tile_rows) {
+    if (!row_end || !tile_rows) return LACOSMIC_ERR_NULL;
+    int rc = check_shape(h, w);
+    if (rc) return rc;
+    int re[MAX_BANDS], up[MAX_BANDS];
+    const int n = band_plan(h, w, re, up);
+    for (int b = 0; b < n; ++b) row_end[b] = re[b], tile_rows[b] = up[b];
+    return n;
+}
 
 int lacosmic_run_host(const float* img_host, int h, int w, const lacosmic_params* p,
                       uint8_t* mask_out_host, float* clean_out_host, void* dev_workspace,
@@ -1191,8 +1255,8 @@ int lacosmic_run_host_batch(const float* imgs_host, int n, int h, int w, const l
 
 // ---- single steps -----------------------------------------------------------------------------
 
-int lacosmic_estimate_gain(const float* img, int h, int w, float readnoise, float* gain_out, float* stats_out,
-                           void* workspace, size_t workspace_bytes, void* stream) {
+int lacosmic_estimate_gain_ex(const float* img, int h, int w, float readnoise, float* gain_out, float* stats_out,
+                              float* path_out, void* workspace, size_t workspace_bytes, void* stream) {
     g_launches = 0;
     if (!img || !gain_out || !workspace) return LACOSMIC_ERR_NULL;
     int rc = check_shape(h, w);
@@ -1209,12 +1273,26 @@ int lacosmic_estimate_gain(const float* img, int h, int w, float readnoise, floa
     const int ntx = (w + lac::TW - 1) / lac::TW, nt = ntx * ((h + lac::NS_TH - 1) / lac::NS_TH);
     lac::k_noise_S<<<nt, lac::NT, 0, st>>>(img, ne, ntx, nullptr);
     LAUNCHED();
-    return sigma_clip_gain((const float*)ws.clist, ws.S, P, ws, ws.qlist, (size_t)((char*)ws.C[0] - (char*)ws.qlist) / 4, readnoise * readnoise, gain_out, stats_out,
-                           nullptr, st);
+    // the selection kernels write seven floats (six statistics + the path flag) in one block; they go to the tail of the
+    // workspace's per-iteration gain array, which a stand-alone estimate does not use, and from there to the caller's
+    // two buffers -- so stats_out is six floats, as it has always been documented for this symbol
+    float* const seven = (stats_out || path_out) ? ws.gains + 8 : nullptr;
+    static_assert(LACOSMIC_MAX_NITER >= 16, "the gain array holds the seven floats at 8..14");
+    rc = sigma_clip_gain((const float*)ws.clist, ws.S, P, ws, ws.qlist, (size_t)((char*)ws.C[0] - (char*)ws.qlist) / 4,
+                         readnoise * readnoise, gain_out, seven, nullptr, st);
+    if (rc) return rc;
+    if (stats_out) CK(cudaMemcpyAsync(stats_out, seven, 6 * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    if (path_out) CK(cudaMemcpyAsync(path_out, seven + 6, sizeof(float), cudaMemcpyDeviceToDevice, st));
+    return LACOSMIC_OK;
+}
+
+int lacosmic_estimate_gain(const float* img, int h, int w, float readnoise, float* gain_out, float* stats_out,
+                           void* workspace, size_t workspace_bytes, void* stream) {
+    return lacosmic_estimate_gain_ex(img, h, w, readnoise, gain_out, stats_out, nullptr, workspace, workspace_bytes, stream);
 }
 
 int lacosmic_gain_fast_path_enable(int enable) {
-    g_gain_fast = enable ? 1 : 0;
+    g_gain_fast.store(enable ? 1 : 0);   // cached graphs are keyed on the switch (GraphKey::gain_fast): none goes stale
     return LACOSMIC_OK;
 }
 
@@ -1318,6 +1396,9 @@ int lacosmic_run_sepmed_compare(const float* img, int h, int w, const lacosmic_p
     if (p->gain == 0.0f) return LACOSMIC_ERR_PARAM;      // the comparison path takes a supplied gain only
     if (workspace_bytes < lacosmic_sepmed_workspace_bytes(h, w)) return LACOSMIC_ERR_WORKSPACE;
     if (dbg && (dbg->iter < -1 || dbg->iter >= LACOSMIC_MAX_NITER)) return LACOSMIC_ERR_PARAM;
+    if (dbg)   // as in lacosmic_run_ws: fp32 debug planes are written with 16-byte vectors
+        for (const float* pl : {dbg->Lp, dbg->N, dbg->S, dbg->Sp, dbg->m3, dbg->F})
+            if ((uintptr_t)pl & 15) return LACOSMIC_ERR_ALIGN;
     const size_t P = (size_t)h * w, need = lacosmic_sepmed_workspace_bytes(h, w);
     if (overlap(workspace, need, img, P * 4) || overlap(workspace, need, clean_out, P * 4) || overlap(workspace, need, mask_out, P))
         return LACOSMIC_ERR_ALIAS;
@@ -1468,7 +1549,7 @@ int lacosmic_gain_zone_info(const void* workspace, int h, int w, int32_t* info_h
 
 int lacosmic_last_cuda_error(void) { return g_last_cuda_error; }
 int lacosmic_last_launch_count(void) { return g_launches; }
-const char* lacosmic_version(void) { return "lacosmic-b200 0.3 (sm_100a)"; }
+const char* lacosmic_version(void) { return "lacosmic-b200 0.4 (sm_100a)"; }
 
 }  // extern "C"
 

@@ -143,6 +143,29 @@ def make_config(i: int, **override) -> Frame:
     return make_frame(**kw)
 
 
+def _image(kw):
+    return make_frame(**kw).img
+
+
+def make_images(kws, workers=None):
+    """The fp32 images make_frame(**kw).img for kw in kws, in order, drawn in worker processes (bench.py's 64-frame
+    stream: a 4000 x 6500 frame takes about 3 s of one core).  The workers are SPAWNED, not forked, so this is safe in a
+    process that has already initialised CUDA; each draw is seeded by its own kw, so the result does not depend on the
+    number of workers."""
+    import multiprocessing as mp
+    import os
+    from concurrent.futures import ProcessPoolExecutor
+    kws = list(kws)
+    workers = min(len(kws), workers or min(16, os.cpu_count() or 1))
+    if workers <= 1:
+        for kw in kws:
+            yield _image(kw)
+        return
+    with ProcessPoolExecutor(max_workers=workers, mp_context=mp.get_context("spawn")) as ex:
+        for img in ex.map(_image, kws):
+            yield img
+
+
 def stream_config(n_frames=64, h=4000, w=6500, first_seed=1000):
     """configs[3]: per-frame (seed, params) of the 64-frame stream.
 

@@ -779,6 +779,112 @@ def test_repeated_call_replays_from_library_graph(lc, orc):
     lc.lacosmic_graph_replay_enable(True)
 
 
+def test_two_threads_replay_their_own_graphs(lc, orc):
+    """Two host threads, each with its own stream, buffers and frames, calling lacosmic_run_ws with the replay on: the
+    table of cached graphs is locked only for the look-up and each entry has its own lock (csrc/lacosmic_api.cu), so the
+    threads capture and replay side by side.  Every result of every call is held against the oracle; meanwhile a third
+    thread flips the replay switch, which dooms entries that are in use instead of destroying them under their user."""
+    import threading
+    import torch
+    nthreads, reps = 2, 10
+    frames = [[synth.make_frame(180 + 16 * t, 260, seed=400 + 10 * t + k, n_star=12, n_cr=120, sp_frac=0.004) for k in range(3)]
+              for t in range(nthreads)]
+    oracle = [[orc.run(f.img, **PARAMS) for f in fs] for fs in frames]
+    errors = []
+    stop = threading.Event()
+
+    def worker(t):
+        try:
+            torch.cuda.set_device(0)
+            s = torch.cuda.Stream()
+            h, w = frames[t][0].img.shape
+            dev_frames = [_t(f.img) for f in frames[t]]
+            img = torch.empty((h, w), dtype=torch.float32, device="cuda")
+            mask = torch.empty((h, w), dtype=torch.uint8, device="cuda")
+            clean = torch.empty_like(img)
+            ws = torch.empty(lc.lacosmic_workspace_bytes(h, w), dtype=torch.uint8, device="cuda")
+            counts = torch.zeros(PARAMS["niter"], dtype=torch.int32, device="cuda")
+            torch.cuda.synchronize()
+            with torch.cuda.stream(s):
+                for rep in range(reps):
+                    k = rep % 3
+                    img.copy_(dev_frames[k])
+                    mask.fill_(9); clean.fill_(-2.0); counts.fill_(-1)
+                    lc.lacosmic_run_ws(img, lc.Params(**PARAMS), mask_out=mask, clean_out=clean, workspace=ws,
+                                       iter_counts=counts, stream=s)
+                    s.synchronize()
+                    o = oracle[t][k]
+                    if not (np.array_equal(_n(mask), o["mask"]) and np.array_equal(_n(clean), o["clean"]) and
+                            np.array_equal(_n(counts), o["counts"])):
+                        errors.append((t, rep))
+        except Exception as e:      # noqa: BLE001 -- reported by the main thread
+            errors.append((t, repr(e)))
+
+    def flipper():
+        on = True
+        while not stop.is_set():
+            on = not on
+            lc.lacosmic_graph_replay_enable(on)
+            stop.wait(0.003)
+
+    lc.lacosmic_graph_replay_enable(True)
+    ths = [threading.Thread(target=worker, args=(t,)) for t in range(nthreads)]
+    fl = threading.Thread(target=flipper)
+    for th in ths:
+        th.start()
+    fl.start()
+    for th in ths:
+        th.join()
+    stop.set()
+    fl.join()
+    lc.lacosmic_graph_replay_enable(True)
+    torch.cuda.synchronize()
+    assert not errors, errors
+
+
+def test_gain_path_switch_is_part_of_the_graph_key(lc, orc):
+    """lacosmic_gain_fast_path_enable between replays of the same arguments: the cached graph of the other setting must
+    not be replayed.  Results do not depend on the switch, so what is checked is the result (against the oracle) and, from
+    the estimate's own diagnostics, which path the replayed kernels took."""
+    import torch
+    f = synth.make_frame(260, 420, seed=431, n_star=15, n_cr=150, sp_frac=0.004)
+    p = dict(PARAMS, gain=0.0)
+    o = orc.run(f.img, **p)
+    h, w = f.img.shape
+    s = torch.cuda.Stream()
+    img = _t(f.img)
+    mask = torch.empty((h, w), dtype=torch.uint8, device="cuda")
+    clean = torch.empty_like(img)
+    ws = torch.empty(lc.lacosmic_workspace_bytes(h, w), dtype=torch.uint8, device="cuda")
+    stopped = {True: set(), False: set()}
+    try:
+        for fast in (True, False, True, False):
+            lc.lacosmic_gain_fast_path_enable(fast)
+            for rep in range(3):                     # direct, capture, replay -- per setting on first sight, replay after
+                mask.fill_(5); clean.fill_(-1.0)
+                lc.lacosmic_run_ws(img, lc.Params(**p), mask_out=mask, clean_out=clean, workspace=ws, stream=s)
+                s.synchronize()
+                assert np.array_equal(_n(mask), o["mask"]) and np.array_equal(_n(clean), o["clean"]), (fast, rep)
+                # word 25 of the plan of the last estimate that ran in ws: where the fast path stopped (0: it did not,
+                # 1: switched off) -- the launch sequence is the same either way, the kernels' arguments are not
+                stopped[fast].add(int(lc.lacosmic_gain_zone_info(ws, h, w, stream=s)[25]))
+    finally:
+        lc.lacosmic_gain_fast_path_enable(True)
+    assert stopped[False] == {1}, "a graph captured with the fast path on was replayed with it off: %r" % (stopped,)
+    assert 1 not in stopped[True], "a graph captured with the fast path off was replayed with it on: %r" % (stopped,)
+
+
+def test_host_call_takes_device_by_position(lc, orc):
+    """binding._on_device: `device` given positionally reaches the wrapped call once (it used to raise TypeError)."""
+    import torch
+    f = synth.make_frame(64, 96, seed=432, n_star=3, n_cr=30)
+    o = orc.run(f.img, **PARAMS)
+    r = lc.lacosmic_run_host(torch.from_numpy(f.img).pin_memory(), lc.Params(**PARAMS), None, None, None, "cuda:0")
+    torch.cuda.synchronize()
+    assert np.array_equal(r["mask"].numpy(), o["mask"]) and np.array_equal(r["clean"].numpy(), o["clean"])
+    assert r["_img_host"] is not None          # the input stays referenced while the enqueued copy may still read it
+
+
 def test_repeated_call_with_estimated_gain_replays_from_library_graph(lc, orc):
     """The same with no gain supplied: the captured sequence then holds the estimate's cluster launch (k_selz_resolve) and
     cooperative launch (k_sel_rounds); frame contents change between the replays."""
