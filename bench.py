@@ -593,6 +593,26 @@ def run_cuda(args):
                                "copy rate, ALU_peak = the min/max issue rate measured in this run",
                     frame_stats={k: v[:niter] for k, v in st.items()}, terms=terms)
 
+    def kernel_hbm_gbs(step, r):
+        """Per kernel class: the algorithmic bytes of its launches in one frame (the terms above) over the class's
+        event-timed device time per frame -> achieved GB/s against the measured copy rate and against the ~8 TB/s nominal
+        figure BASELINE.json's north_star quotes.  (The dram bytes actually moved are in profiles/r03_ncu_full.md.)"""
+        if not step:
+            return None
+        cls = {"list_candidates": "lists", "dirty_lists": "lists"}
+        nbytes = {}
+        for t in step["terms"]:
+            k = cls.get(t["kernel"], t["kernel"])
+            nbytes[k] = nbytes.get(k, 0) + t["bytes"]
+        out = {}
+        for k, b in nbytes.items():
+            ms, spans = r["kt"].get(k, (0.0, 0))
+            if spans and ms > 0:
+                gbs = b / (ms / args.steps * 1e-3) / 1e9
+                out[k] = dict(algorithmic_bytes=int(b), ms_per_step=round(ms / args.steps, 4), gbs=round(gbs, 1),
+                              frac_of_measured=round(gbs / peaks["hbm_gbs"], 4), frac_of_nominal_8tbs=round(gbs / 8000.0, 4))
+        return out
+
     frames_per_s = world * 1e3 / res["ms"]
     e2e_fps = world * 1e3 / ms_e2e
     bytes_iter = HBM_BYTES_PER_PX_ITER[main_mode]
@@ -620,6 +640,7 @@ def run_cuda(args):
         cpu = oracle_baseline(frame.img, params)
 
     main_sum = summarise(res)
+    step_rf = step_roofline(res["ms"])
     line = dict(
         metric=METRIC, value=frames_per_s, unit="frames/s", n_gpus=world, steps=args.steps,
         warmup=args.warmup, ms_per_step=res["ms"], higher_is_better=True, scaling="weak",
@@ -642,7 +663,7 @@ def run_cuda(args):
                                          "the host-side scatter that rebuilds the cleaned plane is not part of the call"),
         gpu_launches=res["launches"] * args.steps,
         launches_per_step=res["launches"],
-        roofline=dict(roofline(res), step=step_roofline(res["ms"])), hbm=hbm,
+        roofline=dict(roofline(res), step=step_rf), hbm=hbm, kernel_hbm_gbs=kernel_hbm_gbs(step_rf, res),
         kernels_ms_per_step=main_sum["kernels_ms_per_step"],
         kernel_share_of_step=main_sum["kernel_share_of_step"],
         ms_per_step_with_kernel_event_spans=res["ms_spans"],
